@@ -1,0 +1,198 @@
+/*
+ * gs.h -- C ABI of the B200-native W-VEG sampler (world-space volume-encoding Gaussians).
+ *
+ * The library evaluates, at 3D query positions, the normalised Gaussian kernel regression of
+ * arxiv/paper_2607_01164 (PAPER.md = /root/reference/PAPER.md):
+ *
+ *     Phi(p) = sum_i w_i v_i G_i(p) / sum_i w_i G_i(p)                      (Eq. 2)
+ *     G_i(p) = exp(-1/2 (p-mu_i)^T R_i^T S_i^-2 R_i (p-mu_i))               (Eq. 3)
+ *
+ * over the Gaussians whose cutoff support {G_i >= tau} contains p (tau_1 = 0.01),
+ * and the analytic gradients of a loss L(Phi, I) w.r.t. every Gaussian parameter
+ * (PAPER.md:130, :140), for a structured grid (section 4.1) or an unstructured point
+ * list (section 5.1).  DESIGN.md lists the readings D1..D14 taken where the paper is
+ * silent; the ones a caller must know are repeated at the entry points below.
+ *
+ * Conventions
+ *   - Every pointer is DEVICE memory on the context's GPU unless its name ends in _host
+ *     (gs_step_host takes host memory only).  The caller owns every buffer it passes; the library never
+ *     frees or retains them beyond the call's enqueued work (gs_preprocess retains NOTHING: it copies
+ *     what it needs into context-owned records).  The context owns all scratch (grow-only) and
+ *     frees it in gs_destroy.
+ *   - All work is enqueued on the stream given to gs_create.  Calls return after enqueueing,
+ *     except that gs_build_accel for a grid synchronises once to read the pair count T, and
+ *     gs_step_host / gs_debug_point_sets synchronise before returning.  Outputs are valid once the
+ *     caller synchronises the stream.
+ *   - Every call returns a gs_status; no exception or abort crosses the ABI.  Arguments are
+ *     validated before any launch.  gs_last_error gives a human-readable message for the last
+ *     non-OK status of that context.
+ *   - Call order: gs_preprocess -> gs_build_accel -> gs_sample_fwd -> gs_sample_bwd.  A call made
+ *     out of order returns GS_ERR_STATE.  gs_build_accel may be repeated with a new query (a new
+ *     batch) without repeating gs_preprocess as long as the Gaussians are unchanged.
+ *   - Layouts are dense, row-major, fp32: mean[N,3], scale[N,3], quat[N,4] in (w,x,y,z) order,
+ *     opacity[N], scalar[N]; per-sample arrays are [P].
+ */
+#ifndef GS_H_
+#define GS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GS_OK = 0,
+    GS_ERR_INVALID_ARG = 1, /* null pointer, bad size, bad enum, non-positive spacing, ...            */
+    GS_ERR_STATE = 2,       /* call order violated, or query differs from the one the accel was built for */
+    GS_ERR_OOM = 3,         /* device allocation failed                                                 */
+    GS_ERR_OVERFLOW = 4,    /* pair count T does not fit 32 bits, or a traversal stack overflowed       */
+    GS_ERR_CUDA = 5         /* any other CUDA runtime error (message in gs_last_error)                  */
+} gs_status;
+
+typedef struct gs_ctx gs_ctx;
+
+/* The model: N Gaussians with mean mu_i, scale S_i, rotation R_i, value v_i ("scalar")
+ * and weight w_i ("opacity").  Values are ACTIVATED (DESIGN D2): scale is the linear standard deviation
+ * per principal axis (> 0), opacity the weight in (0,1), scalar the value; the quaternion need not be
+ * unit -- it is normalised inside gs_preprocess and gradients are w.r.t. the raw quaternion.
+ * R is the standard rotation matrix of the unit quaternion and u = S^-1 R (p - mu) (Eq. 3 read
+ * literally, DESIGN D1).  A Gaussian with a non-finite parameter, a non-positive scale or a
+ * zero quaternion has empty support (contributes nowhere, receives zero gradient). */
+typedef struct {
+    uint32_t n;
+    const float *mean;    /* [n,3] */
+    const float *scale;   /* [n,3] */
+    const float *quat;    /* [n,4] (w,x,y,z) */
+    const float *opacity; /* [n]   */
+    const float *scalar;  /* [n]   */
+} gs_gaussians;
+
+/* Axis-aligned box used to quantise Morton codes (unstructured path).  lo < hi on every axis. */
+typedef struct {
+    float lo[3], hi[3];
+} gs_domain;
+
+typedef enum { GS_QUERY_GRID = 0, GS_QUERY_POINTS = 1 } gs_query_kind;
+
+/* Where to sample.
+ * GS_QUERY_GRID (section 4.1): voxel centres of a regular grid, p_k = fmaf((float)i_k + 0.5f, spacing_k,
+ *   origin_k) for global voxel index i (DESIGN D6).  A query is one BATCH: the brick-aligned sub-box
+ *   of brick_cnt bricks starting at brick brick_lo, a brick being 8^3 voxels; voxels beyond dims are
+ *   clipped.  Per-sample arrays are indexed x-fastest over the batch's clipped voxel box
+ *   (bx = min(8*brick_cnt_x, dims_x - 8*brick_lo_x), ...), P = bx*by*bz.
+ * GS_QUERY_POINTS (section 5.1): num_points arbitrary positions xyz[P,3]; per-sample arrays follow the
+ *   caller's order.  presorted != 0 promises that xyz is already spatially coherent (skips the
+ *   Morton sort of the queries; results are identical either way). */
+typedef struct {
+    int32_t kind; /* gs_query_kind */
+    int32_t dims[3];
+    float origin[3];
+    float spacing[3];
+    int32_t brick_lo[3];
+    int32_t brick_cnt[3];
+    uint64_t num_points;
+    const float *xyz; /* [P,3] */
+    int32_t presorted;
+} gs_query;
+
+/* Gradient outputs, OVERWRITTEN (not accumulated): dL/dmean[N,3], dL/dscale[N,3], dL/dquat[N,4],
+ * dL/dopacity[N], dL/dscalar[N] and the per-Gaussian sampling-error statistic err[N] (nullable;
+ * DESIGN D10 -- E_i = sum over covered samples of |Phi_c - t_c| w_i G_ic / I_c; NOT from the paper,
+ * which densifies from per-sample errors). */
+typedef struct {
+    float *dmean, *dscale, *dquat, *dopacity, *dscalar, *err;
+} gs_grads;
+
+/* Create a context bound to CUDA device `device`; cuda_stream is a cudaStream_t (NULL = default
+ * stream).  *out receives the context.  Errors: INVALID_ARG, CUDA, OOM. */
+gs_status gs_create(int device, void *cuda_stream, gs_ctx **out);
+void gs_destroy(gs_ctx *ctx);
+const char *gs_last_error(const gs_ctx *ctx);
+
+/* S1 (section 4.1.1): per Gaussian, normalise the quaternion, build R, the whitening matrix
+ * M = S^-1 R (M^T M is the paper's "conic" R^T S^-2 R), the cutoff ellipsoid {|M d|^2 <= -2 ln tau}
+ * and its world AABB (inflated by 1 + 2^-8, a safe cull for the fp32 predicate).  Results are
+ * stored in the context.  dom may be NULL for grid-only use.  tau in (0,1).
+ * Errors: INVALID_ARG (null, n = 0 is allowed), OOM, CUDA. */
+gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom, float tau);
+
+/* S2 / S3: build the acceleration structure for one query.
+ * Grid (section 4.1.2): count the bricks of the batch each AABB overlaps, prefix-sum,
+ *   write (brick, gaussian) pairs in parallel over pairs, radix-sort by brick (stable, so each
+ *   brick's list is in ascending Gaussian id), per-brick ranges.
+ * Points (north_star (2); the paper uses a BVH over the samples instead):
+ *   30-bit Morton codes of the Gaussian means in `dom`, radix sort of (code, id), Karras radix
+ *   tree, bottom-up AABB refit; the query points are Morton-sorted for coherence unless presorted.
+ * Errors: STATE (no preprocess; no domain for a point query), INVALID_ARG, OVERFLOW, OOM, CUDA. */
+gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
+
+/* S4/S5/S6 (section 4.1.3; section 5.1.2): for every sample c
+ *     I_c = sum_hits w_i G_i(p_c),  Phi_c = (sum_hits v_i w_i G_i(p_c)) / I_c  if I_c > tau, else 0
+ * (strict compare, empty value 0, I_c always written: DESIGN D5).  If target != NULL the fused
+ * epilogue also produces (each output nullable):
+ *     *loss      += (1/P) sum_c (Phi_c - target_c)^2      (double, device; the CALLER zeroes it)
+ *     dL_dphi[c]  = covered ? 2 (Phi_c - target_c) / P : 0
+ *     sample_err[c] = |Phi_c - target_c|
+ * q must be the query the accel was built for.  Errors: STATE, INVALID_ARG, OVERFLOW, CUDA. */
+gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss,
+                        float *dL_dphi, float *sample_err);
+
+/* S7/S8 (section 4.1.4; section 5.1.2): gradients of L w.r.t. the Gaussian parameters
+ * from dL_dphi[P] and dL_dI[P] (nullable = 0), re-computing the kernel weights from phi/I of the
+ * forward pass (nothing else is kept from it).  dL_dphi of an uncovered sample (I_c <= tau) is
+ * ignored.  target (nullable) is only used for the error statistic out->err.
+ * Errors: STATE, INVALID_ARG, OVERFLOW, CUDA. */
+gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi,
+                        const float *dL_dI, const float *target, const gs_grads *out);
+
+/* One whole training-step pass of the hot path from HOST buffers (all pointers are host memory,
+ * q->xyz included): copies the model, the query points and the target to the device, runs
+ * preprocess -> build_accel -> forward (fused MSE) -> backward, copies phi, I, the loss and the
+ * gradients back, and synchronises.  Output pointers may be NULL to skip their copy (loss excepted).
+ * Errors: any of the above. */
+gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *g_host, const gs_domain *dom, float tau, const gs_query *q_host,
+                       const float *target_host, float *phi_host, float *I_host, double *loss_host,
+                       const gs_grads *grads_host);
+
+/* ---- parity / introspection: read-only views of context-owned device buffers ---------------- */
+typedef enum {
+    GS_DBG_RECORDS = 0,      /* float4 [4][N]: (mu.xyz,w) (M row0,v) (M row1,0) (M row2,0); count = N      */
+    GS_DBG_AABB = 1,         /* float [N][6] lo.xyz hi.xyz                                                 */
+    GS_DBG_BRICK_COUNT = 2,  /* uint32 [N] bricks of the current batch each Gaussian overlaps              */
+    GS_DBG_PAIR_BRICK = 3,   /* uint32 [T] sorted brick ids (batch-local)                                  */
+    GS_DBG_PAIR_GAUSS = 4,   /* uint32 [T] Gaussian ids, ascending inside a brick                          */
+    GS_DBG_BRICK_START = 5,  /* uint32 [nbricks+1]                                                         */
+    GS_DBG_LEAF_MORTON = 6,  /* uint32 [N] sorted Morton codes of the Gaussians                            */
+    GS_DBG_LEAF_ORDER = 7,   /* uint32 [N] Gaussian id of each leaf in sorted order                        */
+    GS_DBG_NODE_LEFT = 8,    /* int32 [N-1] child: >= 0 internal node, < 0 is ~leaf                        */
+    GS_DBG_NODE_RIGHT = 9,   /* int32 [N-1]                                                                */
+    GS_DBG_NODE_PARENT = 10, /* int32 [N-1], root = -1                                                     */
+    GS_DBG_LEAF_PARENT = 11, /* int32 [N]                                                                  */
+    GS_DBG_NODE_AABB = 12,   /* float [N-1][6]                                                             */
+    GS_DBG_POINT_ORDER = 13, /* uint32 [P] caller index of the k-th point in traversal order               */
+    GS_DBG_POINT_MORTON = 14 /* uint32 [P] sorted Morton codes of the query points                         */
+} gs_debug_item;
+
+/* *dev_ptr / *count describe the buffer as of the work enqueued so far (synchronise before reading).
+ * Errors: STATE if the item has not been built, INVALID_ARG. */
+gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *count);
+
+/* Convenience: synchronise and copy the first `bytes` bytes of a debug buffer to HOST memory.
+ * Errors: as gs_debug_get; INVALID_ARG if bytes exceeds the buffer. */
+gs_status gs_debug_read(gs_ctx *ctx, int32_t what, void *dst_host, size_t bytes);
+
+/* Per-sample intersection SETS for bit-exact comparison: number of Gaussians whose support contains
+ * the sample, and the sum and xor over them of mix64(id) (splitmix64 finaliser of id + golden
+ * gamma), through the same traversal as gs_sample_fwd.  Device outputs [P]; synchronises. */
+gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, uint64_t *hash_sum, uint64_t *hash_xor);
+
+/* Counters of the last forward pass (device-side work statistics, for the roofline report):
+ * pairs tested (predicate evaluated) and pairs hit.  Only collected by gs_debug_point_sets. */
+gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GS_H_ */

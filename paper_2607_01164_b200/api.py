@@ -1,0 +1,251 @@
+"""Thin Python binding of the C ABI in include/gs.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of ``csrc/``; torch is used for device memory and
+the stream handle.  There is no CPU fallback: if ``libgs.so`` is missing or cannot be loaded the
+import of the library fails loudly (``GsLibraryError``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgs.so")
+
+GS_OK, GS_ERR_INVALID_ARG, GS_ERR_STATE, GS_ERR_OOM, GS_ERR_OVERFLOW, GS_ERR_CUDA = range(6)
+GS_QUERY_GRID, GS_QUERY_POINTS = 0, 1
+_STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OOM", 4: "GS_ERR_OVERFLOW", 5: "GS_ERR_CUDA"}
+
+# gs_debug_item
+(DBG_RECORDS, DBG_AABB, DBG_BRICK_COUNT, DBG_PAIR_BRICK, DBG_PAIR_GAUSS, DBG_BRICK_START, DBG_LEAF_MORTON, DBG_LEAF_ORDER,
+ DBG_NODE_LEFT, DBG_NODE_RIGHT, DBG_NODE_PARENT, DBG_LEAF_PARENT, DBG_NODE_AABB, DBG_POINT_ORDER, DBG_POINT_MORTON) = range(15)
+
+EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
+           "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters"]
+
+
+class GsLibraryError(RuntimeError):
+    pass
+
+
+class GsError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class _Gaussians(C.Structure):
+    _fields_ = [("n", C.c_uint32), ("mean", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p),
+                ("opacity", C.c_void_p), ("scalar", C.c_void_p)]
+
+
+class _Domain(C.Structure):
+    _fields_ = [("lo", C.c_float * 3), ("hi", C.c_float * 3)]
+
+
+class _Query(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float * 3),
+                ("brick_lo", C.c_int32 * 3), ("brick_cnt", C.c_int32 * 3), ("num_points", C.c_uint64), ("xyz", C.c_void_p),
+                ("presorted", C.c_int32)]
+
+
+class _Grads(C.Structure):
+    _fields_ = [("dmean", C.c_void_p), ("dscale", C.c_void_p), ("dquat", C.c_void_p), ("dopacity", C.c_void_p),
+                ("dscalar", C.c_void_p), ("err", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libgs.so and declare the prototypes.  Raises GsLibraryError when it is missing (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GsLibraryError(f"{LIB_PATH} is missing: build it with `python -m paper_2607_01164_b200.build` "
+                             "(there is no CPU fallback)")
+    try:
+        lib = C.CDLL(LIB_PATH)
+    except OSError as e:  # pragma: no cover
+        raise GsLibraryError(f"cannot load {LIB_PATH}: {e}") from e
+    P = C.c_void_p
+    lib.gs_create.argtypes = [C.c_int, P, C.POINTER(P)]
+    lib.gs_destroy.argtypes = [P]
+    lib.gs_destroy.restype = None
+    lib.gs_last_error.argtypes = [P]
+    lib.gs_last_error.restype = C.c_char_p
+    lib.gs_preprocess.argtypes = [P, C.POINTER(_Gaussians), C.POINTER(_Domain), C.c_float]
+    lib.gs_build_accel.argtypes = [P, C.POINTER(_Query)]
+    lib.gs_sample_fwd.argtypes = [P, C.POINTER(_Query), P, P, P, P, P, P]
+    lib.gs_sample_bwd.argtypes = [P, C.POINTER(_Query), P, P, P, P, P, C.POINTER(_Grads)]
+    lib.gs_step_host.argtypes = [P, C.POINTER(_Gaussians), C.POINTER(_Domain), C.c_float, C.POINTER(_Query), P, P, P, P,
+                                 C.POINTER(_Grads)]
+    lib.gs_debug_get.argtypes = [P, C.c_int32, C.POINTER(P), C.POINTER(C.c_size_t)]
+    lib.gs_debug_read.argtypes = [P, C.c_int32, P, C.c_size_t]
+    lib.gs_debug_point_sets.argtypes = [P, C.POINTER(_Query), P, P, P]
+    lib.gs_debug_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    for name in EXPORTS:
+        if name not in ("gs_destroy", "gs_last_error"):
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    """Device (torch) or host (numpy) array -> address; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return C.c_void_p(t.ctypes.data)
+    assert t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def grid_query(grid) -> _Query:
+    """``grid``: object with dims, origin, spacing, brick_lo, brick_cnt (e.g. inputs.Grid)."""
+    q = _Query()
+    q.kind = GS_QUERY_GRID
+    for k in range(3):
+        q.dims[k] = int(grid.dims[k])
+        q.origin[k] = float(grid.origin[k])
+        q.spacing[k] = float(grid.spacing[k])
+        q.brick_lo[k] = int(grid.brick_lo[k])
+        q.brick_cnt[k] = int(grid.brick_cnt[k])
+    return q
+
+
+def points_query(xyz, presorted: bool = False) -> _Query:
+    """``xyz``: [P,3] float32, device tensor (or host array for step_host)."""
+    q = _Query()
+    q.kind = GS_QUERY_POINTS
+    q.num_points = int(xyz.shape[0])
+    q.xyz = _ptr(xyz).value if xyz.shape[0] else None
+    q.presorted = int(bool(presorted))
+    q._keep = xyz
+    return q
+
+
+def query_num_points(q: _Query) -> int:
+    if q.kind == GS_QUERY_POINTS:
+        return int(q.num_points)
+    n = 1
+    for k in range(3):
+        n *= min(8 * q.brick_cnt[k], q.dims[k] - 8 * q.brick_lo[k])
+    return n
+
+
+def _gaussians(mean, scale, quat, opacity, scalar) -> _Gaussians:
+    g = _Gaussians()
+    g.n = int(mean.shape[0])
+    g.mean, g.scale, g.quat, g.opacity, g.scalar = (_ptr(a).value if g.n else None for a in (mean, scale, quat, opacity, scalar))
+    return g
+
+
+def _domain(dom):
+    if dom is None:
+        return None
+    d = _Domain()
+    for k in range(3):
+        d.lo[k] = float(dom[0][k])
+        d.hi[k] = float(dom[1][k])
+    return C.byref(d)
+
+
+class Context:
+    """One gs_ctx bound to the current torch CUDA device and stream."""
+
+    def __init__(self, device: int | None = None, stream=None):
+        import torch
+        self._torch = torch
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise GsLibraryError("no CUDA device: the W-VEG sampler has no CPU fallback")
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        h = C.c_void_p()
+        st = self.lib.gs_create(self.device, C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if st != GS_OK:
+            raise GsError(st, "gs_create failed")
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.gs_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != GS_OK:
+            raise GsError(st, self.lib.gs_last_error(self.h).decode())
+
+    # ---- the four calls of the path ---------------------------------------------------------
+    def gs_preprocess(self, mean, scale, quat, opacity, scalar, domain=None, tau: float = 0.01):
+        g = _gaussians(mean, scale, quat, opacity, scalar)
+        self._check(self.lib.gs_preprocess(self.h, C.byref(g), _domain(domain), C.c_float(tau)))
+
+    def gs_build_accel(self, q: _Query):
+        self._check(self.lib.gs_build_accel(self.h, C.byref(q)))
+
+    def gs_sample_fwd(self, q: _Query, phi, I, target=None, loss=None, dL_dphi=None, sample_err=None):
+        self._check(self.lib.gs_sample_fwd(self.h, C.byref(q), _ptr(target), _ptr(phi), _ptr(I), _ptr(loss), _ptr(dL_dphi),
+                                           _ptr(sample_err)))
+
+    def gs_sample_bwd(self, q: _Query, phi, I, dL_dphi, grads: dict, dL_dI=None, target=None):
+        g = _Grads(*[(_ptr(grads.get(k)).value if grads.get(k) is not None else None)
+                     for k in ("dmean", "dscale", "dquat", "dopacity", "dscalar", "err")])
+        self._check(self.lib.gs_sample_bwd(self.h, C.byref(q), _ptr(phi), _ptr(I), _ptr(dL_dphi), _ptr(dL_dI), _ptr(target),
+                                           C.byref(g)))
+
+    def gs_step_host(self, g_host: dict, q_host: _Query, target_host, phi_host, I_host, grads_host: dict | None, domain=None,
+                     tau: float = 0.01) -> float:
+        """All arrays are numpy (host).  Returns the loss."""
+        g = _gaussians(g_host["mean"], g_host["scale"], g_host["quat"], g_host["opacity"], g_host["scalar"])
+        loss = C.c_double(0.0)
+        gr = None
+        if grads_host is not None:
+            gr = C.byref(_Grads(*[(_ptr(grads_host.get(k)).value if grads_host.get(k) is not None else None)
+                                  for k in ("dmean", "dscale", "dquat", "dopacity", "dscalar", "err")]))
+        self._check(self.lib.gs_step_host(self.h, C.byref(g), _domain(domain), C.c_float(tau), C.byref(q_host), _ptr(target_host),
+                                          _ptr(phi_host), _ptr(I_host), C.byref(loss), gr))
+        return float(loss.value)
+
+    # ---- helpers -----------------------------------------------------------------------------
+    def alloc_grads(self, n: int, with_err: bool = True) -> dict:
+        t = self._torch
+        dev = t.device("cuda", self.device)
+        out = dict(dmean=t.empty((n, 3), dtype=t.float32, device=dev), dscale=t.empty((n, 3), dtype=t.float32, device=dev),
+                   dquat=t.empty((n, 4), dtype=t.float32, device=dev), dopacity=t.empty(n, dtype=t.float32, device=dev),
+                   dscalar=t.empty(n, dtype=t.float32, device=dev))
+        if with_err:
+            out["err"] = t.empty(n, dtype=t.float32, device=dev)
+        return out
+
+    def debug_get(self, what: int, dtype, cols: int = 1):
+        """Copy a context-owned debug buffer to a numpy array (synchronises)."""
+        p, n = C.c_void_p(), C.c_size_t()
+        self._check(self.lib.gs_debug_get(self.h, what, C.byref(p), C.byref(n)))
+        out = np.empty(int(n.value) * cols, dtype)
+        self._check(self.lib.gs_debug_read(self.h, what, _ptr(out), out.nbytes))
+        return out.reshape(-1, cols) if cols > 1 else out
+
+    def debug_point_sets(self, q: _Query):
+        t = self._torch
+        dev = t.device("cuda", self.device)
+        P = query_num_points(q)
+        cnt = t.zeros(max(P, 1), dtype=t.int32, device=dev)
+        hs = t.zeros(max(P, 1), dtype=t.int64, device=dev)
+        hx = t.zeros(max(P, 1), dtype=t.int64, device=dev)
+        self._check(self.lib.gs_debug_point_sets(self.h, C.byref(q), _ptr(cnt), _ptr(hs), _ptr(hx)))
+        a, b = C.c_uint64(), C.c_uint64()
+        self._check(self.lib.gs_debug_counters(self.h, C.byref(a), C.byref(b)))
+        return (cnt.cpu().numpy().view(np.uint32)[:P], hs.cpu().numpy().view(np.uint64)[:P], hx.cpu().numpy().view(np.uint64)[:P],
+                int(a.value), int(b.value))

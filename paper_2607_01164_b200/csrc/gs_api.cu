@@ -1,0 +1,426 @@
+// gs_api.cu -- the C ABI of include/gs.h: argument validation, context-owned scratch, launch order.
+// Every step of the path runs in the kernels of this directory; this file only orchestrates.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+#include "gs_internal.cuh"
+
+using namespace gs;
+
+namespace {
+
+gs_status fail(gs_ctx *ctx, gs_status st, const char *what) {
+    if (ctx) ctx->err = what;
+    return st;
+}
+gs_status fail_cuda(gs_ctx *ctx, cudaError_t e, const char *where) {
+    if (ctx) {
+        ctx->err = std::string(where) + ": " + cudaGetErrorString(e);
+    }
+    cudaGetLastError();  // clear sticky-less error state
+    return e == cudaErrorMemoryAllocation ? GS_ERR_OOM : GS_ERR_CUDA;
+}
+
+#define CK(expr, where)                                        \
+    do {                                                       \
+        cudaError_t e__ = (expr);                              \
+        if (e__ != cudaSuccess) return fail_cuda(ctx, e__, where); \
+    } while (0)
+
+bool same_query(const gs_query &a, const gs_query &b) {
+    if (a.kind != b.kind) return false;
+    if (a.kind == GS_QUERY_GRID) {
+        for (int k = 0; k < 3; k++)
+            if (a.dims[k] != b.dims[k] || a.origin[k] != b.origin[k] || a.spacing[k] != b.spacing[k] ||
+                a.brick_lo[k] != b.brick_lo[k] || a.brick_cnt[k] != b.brick_cnt[k])
+                return false;
+        return true;
+    }
+    return a.num_points == b.num_points && a.xyz == b.xyz && a.presorted == b.presorted;
+}
+
+gs_status validate_query(gs_ctx *ctx, const gs_query *q, GridDesc *gd, uint64_t *P) {
+    if (!q) return fail(ctx, GS_ERR_INVALID_ARG, "query is NULL");
+    if (q->kind == GS_QUERY_GRID) {
+        uint64_t p = 1, nb = 1;
+        for (int k = 0; k < 3; k++) {
+            if (q->dims[k] <= 0 || !(q->spacing[k] > 0.f) || !isfinite(q->spacing[k]) || !isfinite(q->origin[k]))
+                return fail(ctx, GS_ERR_INVALID_ARG, "grid: dims and spacing must be positive and finite");
+            const int nbk = (q->dims[k] + BRICK - 1) / BRICK;
+            if (q->brick_lo[k] < 0 || q->brick_cnt[k] <= 0 || q->brick_lo[k] + q->brick_cnt[k] > nbk)
+                return fail(ctx, GS_ERR_INVALID_ARG, "grid: brick_lo/brick_cnt outside the grid");
+            gd->dims[k] = q->dims[k];
+            gd->origin[k] = q->origin[k];
+            gd->spacing[k] = q->spacing[k];
+            gd->brick_lo[k] = q->brick_lo[k];
+            gd->brick_cnt[k] = q->brick_cnt[k];
+            const int ext = BRICK * q->brick_cnt[k], rest = q->dims[k] - BRICK * q->brick_lo[k];
+            gd->bdim[k] = ext < rest ? ext : rest;
+            gd->inv_brick[k] = 1.0f / (8.0f * q->spacing[k]);
+            gd->nb_total[k] = nbk;
+            p *= (uint64_t)gd->bdim[k];
+            nb *= (uint64_t)q->brick_cnt[k];
+        }
+        if (nb >= (1ull << 31)) return fail(ctx, GS_ERR_INVALID_ARG, "grid: too many bricks in one batch");
+        *P = p;
+        return GS_OK;
+    }
+    if (q->kind == GS_QUERY_POINTS) {
+        if (q->num_points > 0 && !q->xyz) return fail(ctx, GS_ERR_INVALID_ARG, "points: xyz is NULL");
+        if (q->num_points >= (1ull << 32)) return fail(ctx, GS_ERR_INVALID_ARG, "points: more than 2^32-1 points in one query");
+        *P = q->num_points;
+        return GS_OK;
+    }
+    return fail(ctx, GS_ERR_INVALID_ARG, "query kind");
+}
+
+int bits_for(uint64_t n) {  // bits needed to represent values in [0, n)
+    int b = 0;
+    while (b < 32 && (1ull << b) < n) b++;
+    return b < 1 ? 1 : b;
+}
+
+}  // namespace
+
+extern "C" {
+
+gs_status gs_create(int device, void *cuda_stream, gs_ctx **out) {
+    if (!out) return GS_ERR_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) { cudaGetLastError(); return GS_ERR_CUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return GS_ERR_CUDA; }
+    gs_ctx *ctx = new (std::nothrow) gs_ctx();
+    if (!ctx) return GS_ERR_OOM;
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    if (ctx->counters.reserve(64) != cudaSuccess) { delete ctx; cudaGetLastError(); return GS_ERR_OOM; }
+    *out = ctx;
+    return GS_OK;
+}
+
+void gs_destroy(gs_ctx *ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->boffset, &ctx->pair_key[0], &ctx->pair_key[1],
+                     &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->leaf_key[0], &ctx->leaf_key[1],
+                     &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
+                     &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->pt_key[0], &ctx->pt_key[1],
+                     &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters};
+    for (DevBuf *b : all) b->release();
+    for (DevBuf &b : ctx->h2d) b.release();
+    delete ctx;
+}
+
+const char *gs_last_error(const gs_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom, float tau) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    if (!g) return fail(ctx, GS_ERR_INVALID_ARG, "gaussians is NULL");
+    if (g->n > 0 && (!g->mean || !g->scale || !g->quat || !g->opacity || !g->scalar))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gaussians: NULL parameter array");
+    if (g->n >= (1u << 31)) return fail(ctx, GS_ERR_INVALID_ARG, "gaussians: n must be < 2^31");
+    if (!(tau > 0.f && tau < 1.f)) return fail(ctx, GS_ERR_INVALID_ARG, "tau must lie in (0,1)");
+    if (dom)
+        for (int k = 0; k < 3; k++)
+            if (!(dom->hi[k] > dom->lo[k]) || !isfinite(dom->hi[k]) || !isfinite(dom->lo[k]))
+                return fail(ctx, GS_ERR_INVALID_ARG, "domain: need finite lo < hi");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ctx->have_pre = false;
+    ctx->accel_kind = -1;
+    const size_t n = g->n ? g->n : 1;
+    CK(ctx->rec.reserve(n * 64), "alloc records");
+    CK(ctx->aabb.reserve(n * 24), "alloc aabb");
+    CK(ctx->params.reserve(n * 32), "alloc params");
+    ctx->N = g->n;
+    ctx->tau = tau;
+    // support G >= tau  <=>  |u|^2 <= r2 = -2 ln tau (D3); both rounded to fp32 once, here
+    ctx->r2 = (float)(-2.0 * log((double)tau));
+    ctx->r = (float)sqrt((double)ctx->r2);
+    ctx->have_dom = dom != nullptr;
+    if (dom) ctx->dom = *dom;
+    CK(launch_preprocess(*g, ctx->r, ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->params.as<float>(), ctx->stream), "preprocess");
+    ctx->have_pre = true;
+    return GS_OK;
+}
+
+gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "gs_build_accel before gs_preprocess");
+    GridDesc gd{};
+    uint64_t P = 0;
+    gs_status st = validate_query(ctx, q, &gd, &P);
+    if (st != GS_OK) return st;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ctx->accel_kind = -1;
+    cudaStream_t s = ctx->stream;
+    const uint32_t N = ctx->N;
+    if (q->kind == GS_QUERY_GRID) {
+        const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
+        CK(ctx->bcount.reserve(((size_t)N + 1) * 4), "alloc brick counts");
+        CK(ctx->boffset.reserve(((size_t)N + 1) * 4), "alloc brick offsets");
+        CK(ctx->brick_start.reserve(((size_t)nbricks + 1) * 4), "alloc brick_start");
+        unsigned long long *total = ctx->counters.as<unsigned long long>() + 4;
+        CK(launch_brick_count(ctx->aabb.as<float>(), N, gd, ctx->bcount.as<uint32_t>(), total, s), "brick count");
+        CK(exclusive_scan_u32(ctx->bcount.as<uint32_t>(), ctx->boffset.as<uint32_t>(), N, ctx->scan_tmp, s), "scan");
+        unsigned long long T64 = 0;
+        CK(cudaMemcpyAsync(&T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
+        CK(cudaStreamSynchronize(s), "sync (T)");
+        if (T64 >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
+        const uint32_t T = (uint32_t)T64;
+        const size_t tb = ((size_t)T + 1) * 4;
+        for (int k = 0; k < 2; k++) {
+            CK(ctx->pair_key[k].reserve(tb), "alloc pair keys");
+            CK(ctx->pair_val[k].reserve(tb), "alloc pair vals");
+        }
+        CK(launch_pair_write(ctx->aabb.as<float>(), N, gd, ctx->boffset.as<uint32_t>(), T, ctx->pair_key[0].as<uint32_t>(),
+                             ctx->pair_val[0].as<uint32_t>(), s), "pair write");
+        uint32_t *keys[2] = {ctx->pair_key[0].as<uint32_t>(), ctx->pair_key[1].as<uint32_t>()};
+        uint32_t *vals[2] = {ctx->pair_val[0].as<uint32_t>(), ctx->pair_val[1].as<uint32_t>()};
+        CK(radix_sort_pairs(keys, vals, T, bits_for(nbricks), ctx->sort_hist, ctx->scan_tmp, s, &ctx->pair_sel), "pair sort");
+        CK(launch_brick_start(keys[ctx->pair_sel], T, nbricks, ctx->brick_start.as<uint32_t>(), s), "brick_start");
+        ctx->T = T;
+        ctx->nbricks = nbricks;
+        ctx->grid = gd;
+    } else {
+        if (!ctx->have_dom) return fail(ctx, GS_ERR_STATE, "point query needs the domain given to gs_preprocess");
+        const size_t n = N ? N : 1;
+        for (int k = 0; k < 2; k++) {
+            CK(ctx->leaf_key[k].reserve(n * 4), "alloc leaf keys");
+            CK(ctx->leaf_val[k].reserve(n * 4), "alloc leaf vals");
+        }
+        CK(ctx->node_left.reserve(n * 4), "alloc nodes");
+        CK(ctx->node_right.reserve(n * 4), "alloc nodes");
+        CK(ctx->node_parent.reserve(n * 4), "alloc nodes");
+        CK(ctx->leaf_parent.reserve(n * 4), "alloc nodes");
+        CK(ctx->node_aabb.reserve(n * 24), "alloc nodes");
+        CK(ctx->node_flag.reserve(n * 4), "alloc nodes");
+        CK(ctx->bvh_nodes.reserve(n * 64), "alloc nodes");
+        // Morton codes of the means (record plane 0: mu.xyz, w; NaN marks an invalid Gaussian)
+        CK(launch_morton(ctx->rec.as<float>(), 4, ctx->rec.as<float>(), N, ctx->dom, ctx->leaf_key[0].as<uint32_t>(),
+                         ctx->leaf_val[0].as<uint32_t>(), s), "morton (gaussians)");
+        uint32_t *keys[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
+        uint32_t *vals[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
+        CK(radix_sort_pairs(keys, vals, N, 31, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "morton sort (gaussians)");
+        CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), N, ctx->node_left.as<int32_t>(),
+                       ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(), ctx->leaf_parent.as<int32_t>(),
+                       ctx->node_aabb.as<float>(), ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), s), "lbvh");
+        // coherence sort of the queries
+        ctx->have_pt_order = false;
+        if (!q->presorted && P > 0) {
+            for (int k = 0; k < 2; k++) {
+                CK(ctx->pt_key[k].reserve(P * 4), "alloc point keys");
+                CK(ctx->pt_val[k].reserve(P * 4), "alloc point order");
+            }
+            CK(launch_morton(q->xyz, 3, nullptr, P, ctx->dom, ctx->pt_key[0].as<uint32_t>(), ctx->pt_val[0].as<uint32_t>(), s),
+               "morton (points)");
+            uint32_t *pk[2] = {ctx->pt_key[0].as<uint32_t>(), ctx->pt_key[1].as<uint32_t>()};
+            uint32_t *pv[2] = {ctx->pt_val[0].as<uint32_t>(), ctx->pt_val[1].as<uint32_t>()};
+            CK(radix_sort_pairs(pk, pv, P, 30, ctx->sort_hist, ctx->scan_tmp, s, &ctx->pt_sel), "morton sort (points)");
+            ctx->have_pt_order = true;
+        }
+    }
+    ctx->P = P;
+    ctx->accel_q = *q;
+    ctx->accel_kind = q->kind;
+    return GS_OK;
+}
+
+static gs_status check_ready(gs_ctx *ctx, const gs_query *q, const char *who) {
+    if (!ctx->have_pre || ctx->accel_kind < 0) return fail(ctx, GS_ERR_STATE, who);
+    if (!q) return fail(ctx, GS_ERR_INVALID_ARG, "query is NULL");
+    if (!same_query(*q, ctx->accel_q)) return fail(ctx, GS_ERR_STATE, "query differs from the one gs_build_accel was called with");
+    return GS_OK;
+}
+
+static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
+    cudaStream_t s = ctx->stream;
+    if (ctx->accel_kind == GS_QUERY_GRID) {
+        CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_val[ctx->pair_sel].as<uint32_t>(),
+                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, s), "grid forward");
+    } else {
+        uint32_t *ovf = ctx->counters.as<uint32_t>();
+        CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
+        CK(launch_points_fwd(ctx->rec.as<float4>(), ctx->N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, o,
+                             ovf, s), "points forward");
+    }
+    return GS_OK;
+}
+
+gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss, float *dL_dphi,
+                        float *sample_err) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    gs_status st = check_ready(ctx, q, "gs_sample_fwd before gs_preprocess/gs_build_accel");
+    if (st != GS_OK) return st;
+    if (ctx->P > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "phi and I must be given");
+    if (!target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr};
+    return run_fwd(ctx, o);
+}
+
+gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi, const float *dL_dI,
+                        const float *target, const gs_grads *out) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    gs_status st = check_ready(ctx, q, "gs_sample_bwd before gs_preprocess/gs_build_accel");
+    if (st != GS_OK) return st;
+    if (!out || (ctx->N > 0 && (!out->dmean || !out->dscale || !out->dquat || !out->dopacity || !out->dscalar)))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gradient outputs must be given");
+    if (ctx->P > 0 && (!phi || !I || !dL_dphi)) return fail(ctx, GS_ERR_INVALID_ARG, "phi, I and dL_dphi must be given");
+    if (ctx->N > 0 && ((uintptr_t)out->dquat & 15)) return fail(ctx, GS_ERR_INVALID_ARG, "dquat must be 16-byte aligned");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    const uint32_t N = ctx->N;
+    if (N == 0) return GS_OK;
+    CK(ctx->gacc.reserve((size_t)N * GACC * 4), "alloc gradient accumulator");
+    BwdIn in{phi, I, dL_dphi, dL_dI, target};
+    if (ctx->accel_kind == GS_QUERY_GRID) {
+        CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc sample pack");
+        CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
+        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.as<float4>(), ctx->r2,
+                           ctx->gacc.as<float>(), s), "grid backward");
+    } else {
+        uint32_t *ovf = ctx->counters.as<uint32_t>();
+        CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
+        CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
+        CK(launch_points_bwd(ctx->rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, in,
+                             ctx->gacc.as<float>(), ovf, s), "points backward");
+    }
+    CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, *out, s), "finalize");
+    return GS_OK;
+}
+
+gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *count) {
+    if (!ctx || !dev_ptr || !count) return GS_ERR_INVALID_ARG;
+    if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "nothing built yet");
+    const size_t N = ctx->N;
+    const bool grid = ctx->accel_kind == GS_QUERY_GRID, pts = ctx->accel_kind == GS_QUERY_POINTS;
+    const size_t ni = N >= 1 ? N - 1 : 0;
+    switch (what) {
+        case GS_DBG_RECORDS: *dev_ptr = ctx->rec.p; *count = N; return GS_OK;
+        case GS_DBG_AABB: *dev_ptr = ctx->aabb.p; *count = N; return GS_OK;
+        case GS_DBG_BRICK_COUNT: if (!grid) break; *dev_ptr = ctx->bcount.p; *count = N; return GS_OK;
+        case GS_DBG_PAIR_BRICK: if (!grid) break; *dev_ptr = ctx->pair_key[ctx->pair_sel].p; *count = ctx->T; return GS_OK;
+        case GS_DBG_PAIR_GAUSS: if (!grid) break; *dev_ptr = ctx->pair_val[ctx->pair_sel].p; *count = ctx->T; return GS_OK;
+        case GS_DBG_BRICK_START: if (!grid) break; *dev_ptr = ctx->brick_start.p; *count = (size_t)ctx->nbricks + 1; return GS_OK;
+        case GS_DBG_LEAF_MORTON: if (!pts) break; *dev_ptr = ctx->leaf_key[ctx->leaf_sel].p; *count = N; return GS_OK;
+        case GS_DBG_LEAF_ORDER: if (!pts) break; *dev_ptr = ctx->leaf_val[ctx->leaf_sel].p; *count = N; return GS_OK;
+        case GS_DBG_NODE_LEFT: if (!pts) break; *dev_ptr = ctx->node_left.p; *count = ni; return GS_OK;
+        case GS_DBG_NODE_RIGHT: if (!pts) break; *dev_ptr = ctx->node_right.p; *count = ni; return GS_OK;
+        case GS_DBG_NODE_PARENT: if (!pts) break; *dev_ptr = ctx->node_parent.p; *count = ni; return GS_OK;
+        case GS_DBG_LEAF_PARENT: if (!pts) break; *dev_ptr = ctx->leaf_parent.p; *count = N; return GS_OK;
+        case GS_DBG_NODE_AABB: if (!pts) break; *dev_ptr = ctx->node_aabb.p; *count = ni; return GS_OK;
+        case GS_DBG_POINT_ORDER: if (!pts || !ctx->have_pt_order) break; *dev_ptr = ctx->pt_val[ctx->pt_sel].p; *count = ctx->P; return GS_OK;
+        case GS_DBG_POINT_MORTON: if (!pts || !ctx->have_pt_order) break; *dev_ptr = ctx->pt_key[ctx->pt_sel].p; *count = ctx->P; return GS_OK;
+        default: return fail(ctx, GS_ERR_INVALID_ARG, "unknown debug item");
+    }
+    return fail(ctx, GS_ERR_STATE, "debug item not built for the current accel");
+}
+
+gs_status gs_debug_read(gs_ctx *ctx, int32_t what, void *dst_host, size_t bytes) {
+    if (!ctx || (!dst_host && bytes)) return GS_ERR_INVALID_ARG;
+    const void *p = nullptr;
+    size_t count = 0;
+    gs_status st = gs_debug_get(ctx, what, &p, &count);
+    if (st != GS_OK) return st;
+    static const size_t elem[] = {64, 24, 4, 4, 4, 4, 4, 4, 4, 4, 4, 4, 24, 4, 4};
+    if (bytes > count * elem[what]) return fail(ctx, GS_ERR_INVALID_ARG, "gs_debug_read: more bytes than the buffer holds");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    if (bytes) CK(cudaMemcpy(dst_host, p, bytes, cudaMemcpyDeviceToHost), "debug read");
+    return GS_OK;
+}
+
+gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, uint64_t *hash_sum, uint64_t *hash_xor) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    gs_status st = check_ready(ctx, q, "gs_debug_point_sets before gs_preprocess/gs_build_accel");
+    if (st != GS_OK) return st;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc scratch");
+    unsigned long long *ctr = ctx->counters.as<unsigned long long>() + 2;
+    CK(cudaMemsetAsync(ctr, 0, 16, ctx->stream), "memset");
+    float *phi = ctx->misc.as<float>();
+    float *I = phi + (ctx->P ? ctx->P : 1);
+    FwdOut o{nullptr, phi, I, nullptr, nullptr, nullptr, count, reinterpret_cast<unsigned long long *>(hash_sum),
+             reinterpret_cast<unsigned long long *>(hash_xor), ctr};
+    st = run_fwd(ctx, o);
+    if (st != GS_OK) return st;
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    if (ctx->accel_kind == GS_QUERY_POINTS) {
+        uint32_t ovf = 0;
+        CK(cudaMemcpy(&ovf, ctx->counters.p, 4, cudaMemcpyDeviceToHost), "read overflow flag");
+        if (ovf) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
+    }
+    return GS_OK;
+}
+
+gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_host) {
+    if (!ctx || !tested_host || !hits_host) return GS_ERR_INVALID_ARG;
+    unsigned long long v[2] = {0, 0};
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    CK(cudaMemcpy(v, ctx->counters.as<unsigned long long>() + 2, 16, cudaMemcpyDeviceToHost), "read counters");
+    *tested_host = v[0];
+    *hits_host = v[1];
+    return GS_OK;
+}
+
+gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom, float tau, const gs_query *qh,
+                       const float *target_host, float *phi_host, float *I_host, double *loss_host, const gs_grads *grads_host) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    if (!gh || !qh || !target_host || !loss_host) return fail(ctx, GS_ERR_INVALID_ARG, "gs_step_host: NULL argument");
+    GridDesc gd{};
+    uint64_t P = 0;
+    gs_status st = validate_query(ctx, qh, &gd, &P);
+    if (st != GS_OK) return st;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    const size_t N = gh->n, n1 = N ? N : 1, p1 = P ? P : 1;
+    // staging layout: 0 mean 1 scale 2 quat 3 opacity 4 scalar 5 xyz 6 target 7 phi 8 I 9 dL_dphi 10 loss 11.. grads
+    const size_t sizes[16] = {n1 * 12, n1 * 12, n1 * 16, n1 * 4, n1 * 4, p1 * 12, p1 * 4, p1 * 4, p1 * 4, p1 * 4, 8,
+                              n1 * 12, n1 * 12, n1 * 16, n1 * 4, n1 * 8};
+    for (int k = 0; k < 16; k++) CK(ctx->h2d[k].reserve(sizes[k]), "alloc staging");
+    const void *src[5] = {gh->mean, gh->scale, gh->quat, gh->opacity, gh->scalar};
+    for (int k = 0; k < 5; k++)
+        if (N) CK(cudaMemcpyAsync(ctx->h2d[k].p, src[k], N * (sizes[k] / n1), cudaMemcpyHostToDevice, s), "H2D model");
+    gs_query q = *qh;
+    if (q.kind == GS_QUERY_POINTS) {
+        if (P) CK(cudaMemcpyAsync(ctx->h2d[5].p, qh->xyz, P * 12, cudaMemcpyHostToDevice, s), "H2D points");
+        q.xyz = ctx->h2d[5].as<float>();
+    }
+    if (P) CK(cudaMemcpyAsync(ctx->h2d[6].p, target_host, P * 4, cudaMemcpyHostToDevice, s), "H2D target");
+    CK(cudaMemsetAsync(ctx->h2d[10].p, 0, 8, s), "zero loss");
+    gs_gaussians gdv{gh->n, ctx->h2d[0].as<float>(), ctx->h2d[1].as<float>(), ctx->h2d[2].as<float>(), ctx->h2d[3].as<float>(),
+                     ctx->h2d[4].as<float>()};
+    if ((st = gs_preprocess(ctx, &gdv, dom, tau)) != GS_OK) return st;
+    if ((st = gs_build_accel(ctx, &q)) != GS_OK) return st;
+    float *phi = ctx->h2d[7].as<float>(), *I = ctx->h2d[8].as<float>(), *dphi = ctx->h2d[9].as<float>();
+    if ((st = gs_sample_fwd(ctx, &q, ctx->h2d[6].as<float>(), phi, I, ctx->h2d[10].as<double>(), dphi, nullptr)) != GS_OK) return st;
+    gs_grads gdev{ctx->h2d[11].as<float>(), ctx->h2d[12].as<float>(), ctx->h2d[13].as<float>(), ctx->h2d[14].as<float>(),
+                  ctx->h2d[15].as<float>(), ctx->h2d[15].as<float>() + n1};
+    if ((st = gs_sample_bwd(ctx, &q, phi, I, dphi, nullptr, ctx->h2d[6].as<float>(), &gdev)) != GS_OK) return st;
+    if (phi_host && P) CK(cudaMemcpyAsync(phi_host, phi, P * 4, cudaMemcpyDeviceToHost, s), "D2H phi");
+    if (I_host && P) CK(cudaMemcpyAsync(I_host, I, P * 4, cudaMemcpyDeviceToHost, s), "D2H I");
+    CK(cudaMemcpyAsync(loss_host, ctx->h2d[10].p, 8, cudaMemcpyDeviceToHost, s), "D2H loss");
+    if (grads_host && N) {
+        float *dst[6] = {grads_host->dmean, grads_host->dscale, grads_host->dquat, grads_host->dopacity, grads_host->dscalar, grads_host->err};
+        const float *srcd[6] = {gdev.dmean, gdev.dscale, gdev.dquat, gdev.dopacity, gdev.dscalar, gdev.err};
+        const size_t bytes[6] = {N * 12, N * 12, N * 16, N * 4, N * 4, N * 4};
+        for (int k = 0; k < 6; k++)
+            if (dst[k]) CK(cudaMemcpyAsync(dst[k], srcd[k], bytes[k], cudaMemcpyDeviceToHost, s), "D2H grads");
+    }
+    CK(cudaStreamSynchronize(s), "sync");
+    if (ctx->accel_kind == GS_QUERY_POINTS) {
+        uint32_t ovf = 0;
+        CK(cudaMemcpy(&ovf, ctx->counters.p, 4, cudaMemcpyDeviceToHost), "read overflow flag");
+        if (ovf) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
+    }
+    return GS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,132 @@
+// gs_internal.cuh -- shared declarations of the sm_100a W-VEG sampler (not part of the C ABI).
+// Citations: PAPER.md:<line> of arxiv/paper_2607_01164; "D<n>" = the numbered readings in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+
+#include "../../include/gs.h"
+
+namespace gs {
+
+constexpr int BRICK = 8;            // bricks of 8^3 voxels (north_star (3))
+constexpr int BRICK_VOX = 512;
+constexpr int GACC = 16;            // floats per Gaussian in the gradient accumulator (13 used)
+// gacc layout: 0 dv | 1 dw | 2..4 U | 5..10 W00 W01 W02 W11 W12 W22 | 11 E | 12..15 unused
+
+// Grow-only device buffer owned by the context.
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; cap = 0; }
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { p = nullptr; cap = 0; return e; }
+        cap = want;
+        return cudaSuccess;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <class T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+struct GridDesc {          // one batch of a structured grid (gs_query, GS_QUERY_GRID)
+    int dims[3];
+    float origin[3], spacing[3];
+    int brick_lo[3], brick_cnt[3];
+    int bdim[3];           // clipped voxel extent of the batch
+    float inv_brick[3];    // 1.0f / (8.0f * spacing)  (D7)
+    int nb_total[3];       // bricks of the whole grid per axis
+};
+
+}  // namespace gs
+
+struct gs_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    // ---- S1 state
+    bool have_pre = false;
+    uint32_t N = 0;
+    float tau = 0.f, r2 = 0.f, r = 0.f;
+    bool have_dom = false;
+    gs_domain dom{};
+    const float *scale_in = nullptr;  // NOT retained beyond gs_preprocess; see params copy below
+    gs::DevBuf rec;      // float4 [4][N]
+    gs::DevBuf aabb;     // float [N][6]
+    gs::DevBuf params;   // float [N][8]: scale.xyz, quat (raw) wxyz, pad  (needed by S8)
+    // ---- accel (grid)
+    int accel_kind = -1;  // -1 none, else gs_query_kind
+    gs_query accel_q{};
+    gs::GridDesc grid{};
+    uint32_t T = 0, nbricks = 0;
+    gs::DevBuf bcount;    // uint32 [N+1]
+    gs::DevBuf boffset;   // uint32 [N+1]
+    gs::DevBuf pair_key[2], pair_val[2];
+    int pair_sel = 0;
+    gs::DevBuf brick_start;  // uint32 [nbricks+1]
+    // ---- accel (points)
+    uint64_t P = 0;
+    gs::DevBuf leaf_key[2], leaf_val[2];
+    int leaf_sel = 0;
+    gs::DevBuf node_left, node_right, node_parent, leaf_parent, node_aabb, node_flag;
+    gs::DevBuf bvh_nodes;  // packed traversal nodes
+    gs::DevBuf pt_key[2], pt_val[2];
+    int pt_sel = 0;
+    bool have_pt_order = false;
+    // ---- scratch
+    gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters;
+    gs::DevBuf h2d[16];  // staging for gs_step_host
+};
+
+namespace gs {
+
+// ---- launchers (each enqueues on `s`, returns the launch error) ---------------------------------
+cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, cudaStream_t s);
+
+// exclusive prefix sum of n uint32 (out may alias in); out[n] = total is written too (out has n+1 slots)
+cudaError_t exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, DevBuf &tmp, cudaStream_t s);
+// stable LSD radix sort of (key, val) pairs on key bits [0, bits); returns the index (0/1) of the
+// buffer pair holding the result.  keys[0]/vals[0] hold the input.
+cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int bits, DevBuf &hist, DevBuf &tmp,
+                             cudaStream_t s, int *result_sel);
+
+cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd, uint32_t *count, unsigned long long *total,
+                               cudaStream_t s);
+cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
+                              uint32_t *key, uint32_t *val, cudaStream_t s);
+cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks, uint32_t *start, cudaStream_t s);
+
+struct FwdOut {
+    const float *target; float *phi; float *I; double *loss; float *dL_dphi; float *sample_err;
+    uint32_t *set_count; unsigned long long *set_sum; unsigned long long *set_xor;   // debug sets (nullable)
+    unsigned long long *counters;                                                   // [2] tested, hits (nullable)
+};
+struct BwdIn {
+    const float *phi; const float *I; const float *dL_dphi; const float *dL_dI; const float *target;
+};
+
+cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
+                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
+cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
+cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
+                            float *gacc, cudaStream_t s);
+
+cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
+                            cudaStream_t s);
+
+// LBVH
+cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *aabb_valid /*nullable: aabb[N][6]*/, size_t n,
+                          const gs_domain &dom, uint32_t *codes, uint32_t *ids, cudaStream_t s);
+cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, uint32_t N, int32_t *left, int32_t *right,
+                        int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed, cudaStream_t s);
+cudaError_t launch_points_fwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
+                              const uint32_t *pt_order, uint64_t P, float tau, float r2, const FwdOut &o, uint32_t *overflow,
+                              cudaStream_t s);
+cudaError_t launch_points_bwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
+                              const uint32_t *pt_order, uint64_t P, float tau, float r2, const BwdIn &in, float *gacc,
+                              uint32_t *overflow, cudaStream_t s);
+
+}  // namespace gs

@@ -1,0 +1,155 @@
+// lbvh.cu -- S3: LBVH over the Gaussians' cutoff AABBs, rebuilt every step (north_star (2)).
+// The paper builds a BVH over the sample positions with cuBQL and queries it per Gaussian
+// (PAPER.md:184-190); north_star fixes the opposite direction (per-point traversal), see DESIGN.md.
+//   k_morton      : 30-bit Morton code of a position inside the domain box (D8), x in the low bit
+//   (radix sort)  : stable sort of (code, id) => order by the unique 64-bit key (code << 32 | id)
+//   k_karras      : binary radix tree, one thread per internal node (Karras 2012)
+//   k_refit       : bottom-up exact min/max boxes with per-node arrival counters
+//   k_pack_nodes  : 64-byte traversal nodes holding both children's boxes
+#include "gs_internal.cuh"
+
+namespace gs {
+
+__device__ __forceinline__ uint32_t expand10(uint32_t v) {  // 10 bits -> every third bit
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+struct MortonParams { float lo[3], scale[3]; };
+
+__global__ void __launch_bounds__(256) k_morton(const float *__restrict__ xyz, int stride, int nan_is_invalid, size_t n, MortonParams mp,
+                                                 uint32_t *__restrict__ codes, uint32_t *__restrict__ ids) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float x = xyz[i * stride], y = xyz[i * stride + 1], z = xyz[i * stride + 2];
+    uint32_t code;
+    if (nan_is_invalid && x != x) {
+        code = 1u << 30;  // invalid Gaussians sort to the end
+    } else {
+        // D8: q = (int) min(max((x - lo) * scale, 0), 1023), truncation
+        const float tx = __fmul_rn(__fsub_rn(x, mp.lo[0]), mp.scale[0]);
+        const float ty = __fmul_rn(__fsub_rn(y, mp.lo[1]), mp.scale[1]);
+        const float tz = __fmul_rn(__fsub_rn(z, mp.lo[2]), mp.scale[2]);
+        const uint32_t qx = (uint32_t)(int)fminf(fmaxf(tx, 0.0f), 1023.0f);
+        const uint32_t qy = (uint32_t)(int)fminf(fmaxf(ty, 0.0f), 1023.0f);
+        const uint32_t qz = (uint32_t)(int)fminf(fmaxf(tz, 0.0f), 1023.0f);
+        code = expand10(qx) | (expand10(qy) << 1) | (expand10(qz) << 2);
+    }
+    codes[i] = code;
+    ids[i] = (uint32_t)i;
+}
+
+cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *nan_invalid, size_t n, const gs_domain &dom,
+                          uint32_t *codes, uint32_t *ids, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    MortonParams mp;
+    for (int k = 0; k < 3; k++) {
+        mp.lo[k] = dom.lo[k];
+        mp.scale[k] = 1024.0f / (dom.hi[k] - dom.lo[k]);
+    }
+    k_morton<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(xyz, (int)stride_floats, nan_invalid != nullptr, n, mp, codes, ids);
+    return cudaGetLastError();
+}
+
+// common-prefix length of the 64-bit keys at sorted positions i and j; -1 outside [0, n)
+__device__ __forceinline__ int delta(const uint32_t *__restrict__ codes, const uint32_t *__restrict__ ids, int n, int i, int j) {
+    if (j < 0 || j >= n) return -1;
+    const unsigned long long a = ((unsigned long long)codes[i] << 32) | ids[i];
+    const unsigned long long b = ((unsigned long long)codes[j] << 32) | ids[j];
+    return __clzll((long long)(a ^ b));  // keys are unique, so a ^ b != 0
+}
+
+__global__ void __launch_bounds__(256) k_karras(const uint32_t *__restrict__ codes, const uint32_t *__restrict__ ids, int n,
+                                                 int32_t *__restrict__ left, int32_t *__restrict__ right, int32_t *__restrict__ parent,
+                                                 int32_t *__restrict__ leaf_parent) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n - 1) return;
+    const int d = (delta(codes, ids, n, i, i + 1) - delta(codes, ids, n, i, i - 1)) >= 0 ? 1 : -1;
+    const int dmin = delta(codes, ids, n, i, i - d);
+    int lmax = 2;
+    while (delta(codes, ids, n, i, i + lmax * d) > dmin) lmax <<= 1;
+    int l = 0;
+    for (int t = lmax >> 1; t >= 1; t >>= 1)
+        if (delta(codes, ids, n, i, i + (l + t) * d) > dmin) l += t;
+    const int j = i + l * d;
+    const int dnode = delta(codes, ids, n, i, j);
+    int s = 0;
+    for (int t = (l + 1) >> 1;; t = (t + 1) >> 1) {
+        if (delta(codes, ids, n, i, i + (s + t) * d) > dnode) s += t;
+        if (t == 1) break;
+    }
+    const int gamma = i + s * d + min(d, 0);
+    const int lo = min(i, j), hi = max(i, j);
+    if (lo == gamma) { left[i] = ~gamma; leaf_parent[gamma] = i; }
+    else { left[i] = gamma; parent[gamma] = i; }
+    if (hi == gamma + 1) { right[i] = ~(gamma + 1); leaf_parent[gamma + 1] = i; }
+    else { right[i] = gamma + 1; parent[gamma + 1] = i; }
+    if (i == 0) parent[0] = -1;
+}
+
+__device__ __forceinline__ void load_box(const float *p, float (&b)[6]) {
+#pragma unroll
+    for (int k = 0; k < 6; k++) b[k] = __ldcg(p + k);  // L2: written by other threads of this launch
+}
+
+__global__ void __launch_bounds__(256) k_refit(const uint32_t *__restrict__ ids, const float *__restrict__ aabb, int n,
+                                                const int32_t *__restrict__ left, const int32_t *__restrict__ right,
+                                                const int32_t *__restrict__ parent, const int32_t *__restrict__ leaf_parent,
+                                                float *__restrict__ node_aabb, uint32_t *__restrict__ flags) {
+    const int leaf = blockIdx.x * blockDim.x + threadIdx.x;
+    if (leaf >= n) return;
+    int node = leaf_parent[leaf];
+    while (node >= 0) {
+        if (atomicAdd(&flags[node], 1u) == 0u) return;  // first arrival: the sibling subtree is not done yet
+        __threadfence();
+        float a[6], b[6];
+        const int l = left[node], r = right[node];
+        load_box(l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l, a);
+        load_box(r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r, b);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            __stcg(node_aabb + 6 * (size_t)node + k, fminf(a[k], b[k]));
+            __stcg(node_aabb + 6 * (size_t)node + 3 + k, fmaxf(a[3 + k], b[3 + k]));
+        }
+        __threadfence();
+        node = parent[node];
+    }
+}
+
+// traversal node (64 B): [0] l.lo.xyz l.hi.x | [1] l.hi.yz r.lo.xy | [2] r.lo.z r.hi.xyz | [3] left, right (bits), -, -
+// a leaf child is stored as ~gaussian_id so the traversal needs no second indirection
+__global__ void __launch_bounds__(256) k_pack_nodes(const uint32_t *__restrict__ ids, const float *__restrict__ aabb, int n,
+                                                     const int32_t *__restrict__ left, const int32_t *__restrict__ right,
+                                                     const float *__restrict__ node_aabb, float4 *__restrict__ packed) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n - 1) return;
+    const int l = left[i], r = right[i];
+    const float *a = l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l;
+    const float *b = r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r;
+    const int lc = l < 0 ? ~(int)ids[~l] : l, rc = r < 0 ? ~(int)ids[~r] : r;
+    packed[4 * (size_t)i + 0] = make_float4(a[0], a[1], a[2], a[3]);
+    packed[4 * (size_t)i + 1] = make_float4(a[4], a[5], b[0], b[1]);
+    packed[4 * (size_t)i + 2] = make_float4(b[2], b[3], b[4], b[5]);
+    packed[4 * (size_t)i + 3] = make_float4(__int_as_float(lc), __int_as_float(rc), 0.f, 0.f);
+}
+
+cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, uint32_t N, int32_t *left, int32_t *right,
+                        int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed, cudaStream_t s) {
+    if (N < 2) {
+        if (N == 1) return cudaMemsetAsync(leaf_parent, 0xff, sizeof(int32_t), s);
+        return cudaSuccess;
+    }
+    const int n = (int)N;
+    cudaError_t e = cudaMemsetAsync(flags, 0, sizeof(uint32_t) * (N - 1), s);
+    if (e != cudaSuccess) return e;
+    k_karras<<<(n - 1 + 255) / 256, 256, 0, s>>>(codes, ids, n, left, right, parent, leaf_parent);
+    k_refit<<<(n + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, parent, leaf_parent, node_aabb, flags);
+    k_pack_nodes<<<(n - 1 + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, node_aabb, packed);
+    return cudaGetLastError();
+}
+
+}  // namespace gs

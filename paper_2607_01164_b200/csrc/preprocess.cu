@@ -1,0 +1,162 @@
+// preprocess.cu -- S1 (section 4.1.1) and S8 (backward of S1; implied by PAPER.md:140).
+//
+// S1: one thread per Gaussian.  Everything here feeds integer decisions downstream (brick
+// ranges, the hit predicate), so the arithmetic is a fixed sequence of single IEEE operations
+// (round-to-nearest intrinsics; the compiler may not contract or reorder them) -- D4/D7.
+#include "gs_internal.cuh"
+
+namespace gs {
+
+__device__ __forceinline__ bool finitef(float x) { return fabsf(x) <= 3.402823466e38f; }  // false for NaN/inf
+
+__global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ mean, const float *__restrict__ scale,
+                                                     const float *__restrict__ quat, const float *__restrict__ opacity,
+                                                     const float *__restrict__ scalar, uint32_t N, float r,
+                                                     float4 *__restrict__ rec, float *__restrict__ aabb,
+                                                     float *__restrict__ params) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float mx = mean[3 * i], my = mean[3 * i + 1], mz = mean[3 * i + 2];
+    const float s0 = scale[3 * i], s1 = scale[3 * i + 1], s2 = scale[3 * i + 2];
+    const float qw = quat[4 * i], qx = quat[4 * i + 1], qy = quat[4 * i + 2], qz = quat[4 * i + 3];
+    const float w = opacity[i], v = scalar[i];
+    // raw parameters kept for S8 (the caller's arrays are not retained)
+    float4 *pp = reinterpret_cast<float4 *>(params) + 2 * (size_t)i;
+    pp[0] = make_float4(s0, s1, s2, qw);
+    pp[1] = make_float4(qx, qy, qz, 0.f);
+
+    // validity (empty support otherwise): finite parameters, positive scale, non-zero quaternion
+    float n2chk = __fmul_rn(qw, qw);
+    n2chk = __fadd_rn(n2chk, __fmul_rn(qx, qx));
+    n2chk = __fadd_rn(n2chk, __fmul_rn(qy, qy));
+    n2chk = __fadd_rn(n2chk, __fmul_rn(qz, qz));
+    bool valid = finitef(mx) && finitef(my) && finitef(mz) && (s0 > 0.f) && (s1 > 0.f) && (s2 > 0.f) && finitef(s0) &&
+                 finitef(s1) && finitef(s2) && finitef(qw) && finitef(qx) && finitef(qy) && finitef(qz) && (n2chk > 0.f) &&
+                 finitef(n2chk) && finitef(w) && finitef(v);
+    float4 *r0 = rec + i, *r1 = rec + (size_t)N + i, *r2p = rec + 2 * (size_t)N + i, *r3 = rec + 3 * (size_t)N + i;
+    float *bb = aabb + 6 * (size_t)i;
+    if (!valid) {
+        const float nan = __int_as_float(0x7fc00000);
+        const float inf = __int_as_float(0x7f800000);
+        *r0 = make_float4(nan, nan, nan, 0.f);  // d = p - NaN makes the predicate false everywhere
+        *r1 = make_float4(0.f, 0.f, 0.f, 0.f);
+        *r2p = make_float4(0.f, 0.f, 0.f, 0.f);
+        *r3 = make_float4(0.f, 0.f, 0.f, 0.f);
+        bb[0] = inf; bb[1] = inf; bb[2] = inf; bb[3] = -inf; bb[4] = -inf; bb[5] = -inf;
+        return;
+    }
+    // normalisation activation of the rotation
+    const float n2 = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, __fmul_rn(qw, qw))));
+    const float nrm = __fsqrt_rn(n2);
+    const float a = __fdiv_rn(qw, nrm), x = __fdiv_rn(qx, nrm), y = __fdiv_rn(qy, nrm), z = __fdiv_rn(qz, nrm);
+    const float xx = __fmul_rn(x, x), yy = __fmul_rn(y, y), zz = __fmul_rn(z, z);
+    const float xy = __fmul_rn(x, y), xz = __fmul_rn(x, z), yz = __fmul_rn(y, z);
+    const float ax = __fmul_rn(a, x), ay = __fmul_rn(a, y), az = __fmul_rn(a, z);
+    float R[9];
+    R[0] = __fsub_rn(1.f, __fmul_rn(2.f, __fadd_rn(yy, zz)));
+    R[1] = __fmul_rn(2.f, __fsub_rn(xy, az));
+    R[2] = __fmul_rn(2.f, __fadd_rn(xz, ay));
+    R[3] = __fmul_rn(2.f, __fadd_rn(xy, az));
+    R[4] = __fsub_rn(1.f, __fmul_rn(2.f, __fadd_rn(xx, zz)));
+    R[5] = __fmul_rn(2.f, __fsub_rn(yz, ax));
+    R[6] = __fmul_rn(2.f, __fsub_rn(xz, ay));
+    R[7] = __fmul_rn(2.f, __fadd_rn(yz, ax));
+    R[8] = __fsub_rn(1.f, __fmul_rn(2.f, __fadd_rn(xx, yy)));
+    const float s[3] = {s0, s1, s2};
+    float M[9];
+#pragma unroll
+    for (int j = 0; j < 3; j++)
+#pragma unroll
+        for (int k = 0; k < 3; k++) M[3 * j + k] = __fdiv_rn(R[3 * j + k], s[j]);  // M = S^-1 R;  M^T M = R^T S^-2 R (Eq. 3)
+    *r0 = make_float4(mx, my, mz, w);
+    *r1 = make_float4(M[0], M[1], M[2], v);
+    *r2p = make_float4(M[3], M[4], M[5], 0.f);
+    *r3 = make_float4(M[6], M[7], M[8], 0.f);
+    // AABB of the cutoff ellipsoid: half extent along world axis k = r sqrt(sum_j (s_j R_jk)^2), inflated by 1 + 2^-8
+    const float mu[3] = {mx, my, mz};
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const float a0 = __fmul_rn(s0, R[k]), a1 = __fmul_rn(s1, R[3 + k]), a2 = __fmul_rn(s2, R[6 + k]);
+        const float e = __fmul_rn(r, __fsqrt_rn(__fmaf_rn(a2, a2, __fmaf_rn(a1, a1, __fmul_rn(a0, a0)))));
+        const float ei = __fmul_rn(e, 1.00390625f);
+        bb[k] = __fsub_rn(mu[k], ei);
+        bb[3 + k] = __fadd_rn(mu[k], ei);
+    }
+}
+
+cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, cudaStream_t s) {
+    if (g.n == 0) return cudaSuccess;
+    k_preprocess<<<(g.n + 255) / 256, 256, 0, s>>>(g.mean, g.scale, g.quat, g.opacity, g.scalar, g.n, r, rec, aabb, params);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// S8: from the accumulated (dv, dw, U, W, E) of S7 to gradients of the raw parameters.
+//   dmu = M^T U;  ds_j = W_jj / s_j;  dR_jk = -(1/s_j) sum_l W_jl s_l R_lk;
+//   dqhat = <dR, dR/dqhat>;  dq = (dqhat - qhat (qhat . dqhat)) / |q|        (chain rule of Eq. 3)
+// Values only (no integer decision depends on them), so plain fp32 with FMA contraction.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
+                                                   const float *__restrict__ gacc, uint32_t N, gs_grads out) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float4 *ga = reinterpret_cast<const float4 *>(gacc) + 4 * (size_t)i;
+    const float4 g0 = ga[0], g1 = ga[1], g2 = ga[2];
+    const float dv = g0.x, dw = g0.y;
+    const float U[3] = {g0.z, g0.w, g1.x};
+    const float W00 = g1.y, W01 = g1.z, W02 = g1.w, W11 = g2.x, W12 = g2.y, W22 = g2.z, E = g2.w;
+    const float4 p0 = reinterpret_cast<const float4 *>(params)[2 * (size_t)i];
+    const float4 p1 = reinterpret_cast<const float4 *>(params)[2 * (size_t)i + 1];
+    const float4 c0 = rec[i];
+    const bool valid = (c0.x == c0.x);  // invalid Gaussians carry a NaN mean
+    float dmu[3] = {0, 0, 0}, ds[3] = {0, 0, 0}, dq[4] = {0, 0, 0, 0};
+    if (valid) {
+        const float s[3] = {p0.x, p0.y, p0.z};
+        float q[4] = {p0.w, p1.x, p1.y, p1.z};
+        const float nrm = sqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+        const float inv = 1.f / nrm;
+        const float a = q[0] * inv, x = q[1] * inv, y = q[2] * inv, z = q[3] * inv;
+        float R[9];
+        R[0] = 1.f - 2.f * (y * y + z * z); R[1] = 2.f * (x * y - a * z);       R[2] = 2.f * (x * z + a * y);
+        R[3] = 2.f * (x * y + a * z);       R[4] = 1.f - 2.f * (x * x + z * z); R[5] = 2.f * (y * z - a * x);
+        R[6] = 2.f * (x * z - a * y);       R[7] = 2.f * (y * z + a * x);       R[8] = 1.f - 2.f * (x * x + y * y);
+        const float W[9] = {W00, W01, W02, W01, W11, W12, W02, W12, W22};
+#pragma unroll
+        for (int k = 0; k < 3; k++) dmu[k] = R[k] / s[0] * U[0] + R[3 + k] / s[1] * U[1] + R[6 + k] / s[2] * U[2];
+        ds[0] = W00 / s[0]; ds[1] = W11 / s[1]; ds[2] = W22 / s[2];
+        float D[9];
+#pragma unroll
+        for (int j = 0; j < 3; j++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                float acc = 0.f;
+#pragma unroll
+                for (int l = 0; l < 3; l++) acc += W[3 * j + l] * s[l] * R[3 * l + k];
+                D[3 * j + k] = -acc / s[j];
+            }
+        float dh[4];
+        dh[0] = 2.f * (-z * D[1] + y * D[2] + z * D[3] - x * D[5] - y * D[6] + x * D[7]);
+        dh[1] = 2.f * (y * D[1] + z * D[2] + y * D[3] - 2.f * x * D[4] - a * D[5] + z * D[6] + a * D[7] - 2.f * x * D[8]);
+        dh[2] = 2.f * (-2.f * y * D[0] + x * D[1] + a * D[2] + x * D[3] + z * D[5] - a * D[6] + z * D[7] - 2.f * y * D[8]);
+        dh[3] = 2.f * (-2.f * z * D[0] - a * D[1] + x * D[2] + a * D[3] - 2.f * z * D[4] + y * D[5] + x * D[6] + y * D[7]);
+        const float qh[4] = {a, x, y, z};
+        const float dot = qh[0] * dh[0] + qh[1] * dh[1] + qh[2] * dh[2] + qh[3] * dh[3];
+#pragma unroll
+        for (int k = 0; k < 4; k++) dq[k] = (dh[k] - qh[k] * dot) * inv;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; k++) { out.dmean[3 * (size_t)i + k] = dmu[k]; out.dscale[3 * (size_t)i + k] = ds[k]; }
+    reinterpret_cast<float4 *>(out.dquat)[i] = make_float4(dq[0], dq[1], dq[2], dq[3]);
+    out.dopacity[i] = valid ? dw : 0.f;
+    out.dscalar[i] = valid ? dv : 0.f;
+    if (out.err) out.err[i] = valid ? E : 0.f;
+}
+
+cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
+                            cudaStream_t s) {
+    if (N == 0) return cudaSuccess;
+    k_finalize<<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, out);
+    return cudaGetLastError();
+}
+
+}  // namespace gs

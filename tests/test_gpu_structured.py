@@ -1,0 +1,165 @@
+"""-m gpu parity: structured path (S1, S2, S4, S6, S7, S8) through the C ABI vs the oracle.
+
+Bar (BASELINE.json north_star): integer stages bit-exact (AABB / records feed them, so those are
+compared bit-exactly too), per-point intersection ID sets bit-exact, forward max abs error <= 1e-5
+of the scalar range, gradient relative L2 error <= 1e-4 per parameter tensor.
+"""
+import numpy as np
+import pytest
+
+from paper_2607_01164_b200 import inputs
+from tests.gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_all(oracle, g, grid, target, dL_dI=None):
+    xyz = oracle.grid_points(grid)
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, dL_dI, target, TAU, mode=1)
+    return xyz, fwd, loss, a, serr, gr
+
+
+def _check_integer_stages(oracle, run, g, grid):
+    api = run.api
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    rec = run.ctx.debug_get(api.DBG_RECORDS, np.float32, 4).reshape(4, g.n, 4)
+    gaabb = run.ctx.debug_get(api.DBG_AABB, np.float32, 6)
+    v = valid.astype(bool)
+    assert np.array_equal(gaabb.view(np.uint32), aabb.view(np.uint32)), "AABBs are not bit-exact"
+    gM = np.concatenate([rec[1][:, :3], rec[2][:, :3], rec[3][:, :3]], axis=1)
+    assert np.array_equal(gM[v].view(np.uint32), M[v].view(np.uint32)), "whitening matrices are not bit-exact"
+    assert np.array_equal(rec[0][v, :3], g.mean[v]) and np.array_equal(rec[0][v, 3], g.opacity[v]) and np.array_equal(rec[1][v, 3], g.scalar[v])
+    assert np.all(np.isnan(rec[0][~v, 0]))
+    blo, bhi, cnt = oracle.brick_ranges(aabb, valid, grid)
+    keys, start = oracle.brick_keys(blo, bhi, cnt, grid)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_BRICK_COUNT, np.uint32), cnt)
+    pb = run.ctx.debug_get(api.DBG_PAIR_BRICK, np.uint32)
+    pg = run.ctx.debug_get(api.DBG_PAIR_GAUSS, np.uint32)
+    gkeys = (pb.astype(np.uint64) << np.uint64(32)) | pg.astype(np.uint64)
+    assert np.array_equal(gkeys, keys), "sorted (brick, gaussian) keys differ"
+    assert np.array_equal(run.ctx.debug_get(api.DBG_BRICK_START, np.uint32).astype(np.int64), start)
+    return len(keys)
+
+
+def test_c1_tiny_structured_full(oracle):
+    # BASELINE.json configs[0]: 1,024 Gaussians, 32^3 voxel-centre grid, target from a second seeded set
+    g = inputs.c1_gaussians(seed=0, n=1024)
+    grid = inputs.c1_grid(32)
+    g2 = inputs.c1_gaussians(seed=1, n=1024)
+    xyz = oracle.grid_points(grid)
+    target = oracle.forward(g2, xyz, TAU, mode=1, want_sets=False)["phi"].astype(np.float32)
+    xyz, fwd, loss, a, serr, gr = _oracle_all(oracle, g, grid, target)
+    run = GpuRun(g, "grid", grid, target)
+    T = _check_integer_stages(oracle, run, g, grid)
+    assert T > 1024
+    tested, hits = check_sets(run, fwd)
+    assert hits > 40000 and (fwd["count"] == 0).sum() > 1000  # exercises the empty path
+    near, e_phi, e_I = check_forward(run, fwd)
+    assert near == 0
+    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+    np.testing.assert_allclose(run.np(run.dphi), a, rtol=2e-5, atol=1e-7 * np.abs(a).max())
+    np.testing.assert_allclose(run.np(run.serr), serr, atol=1e-5)
+    check_grads(run, gr)
+
+
+def test_ragged_batch_anisotropic(oracle):
+    # grid whose dims are not multiples of 8, sampled in a sub-box batch; 20:1 elongated Gaussians; dL/dI present
+    gridfull = inputs.Grid((44, 29, 21), (-0.1, 0.2, 0.0), (1 / 40, 1 / 32, 1 / 20))
+    g = inputs.c4_gaussians(seed=7, n_grid=40, n=3000)
+    g.quat[:] = (g.quat * np.random.default_rng(1).uniform(0.3, 3.0, (g.n, 1))).astype(np.float32)  # non-unit quaternions
+    rng = np.random.default_rng(3)
+    for grid in (gridfull, gridfull.batch((1, 1, 0), (3, 3, 3)), gridfull.batch((5, 3, 2), (1, 1, 1))):
+        P = grid.num_points
+        target = rng.uniform(0, 1, P).astype(np.float32)
+        dI = rng.standard_normal(P) * 1e-3
+        xyz, fwd, loss, a, serr, gr = _oracle_all(oracle, g, grid, target, dI)
+        run = GpuRun(g, "grid", grid, target, dL_dI=dI.astype(np.float32))
+        _check_integer_stages(oracle, run, g, grid)
+        check_sets(run, fwd)
+        check_forward(run, fwd)
+        assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+        check_grads(run, gr)
+
+
+def test_invalid_empty_and_degenerate(oracle):
+    import torch
+    from paper_2607_01164_b200 import api
+    grid = inputs.c1_grid(16)
+    g = inputs.c1_gaussians(seed=4, n=200)
+    g.scale[0, 1] = 0.0
+    g.quat[1] = 0.0
+    g.mean[2, 0] = np.nan
+    g.opacity[3] = np.inf
+    g.scale[4] = -1.0
+    target = np.full(grid.num_points, 0.5, np.float32)
+    xyz, fwd, loss, a, serr, gr = _oracle_all(oracle, g, grid, target)
+    run = GpuRun(g, "grid", grid, target)
+    _check_integer_stages(oracle, run, g, grid)
+    check_sets(run, fwd)
+    check_forward(run, fwd)
+    check_grads(run, gr)
+    got = run.grads_np()
+    for k in got:
+        assert np.all(got[k][:5] == 0.0), k  # invalid Gaussians receive zero gradient
+    # a model that covers nothing: every sample takes the empty value, loss = mean(t^2), no gradient
+    far = inputs.c1_gaussians(seed=5, n=8)
+    far.mean[:] += 10.0
+    run = GpuRun(far, "grid", grid, target)
+    assert np.all(run.np(run.phi) == 0.0) and np.all(run.np(run.I) == 0.0) and np.all(run.np(run.dphi) == 0.0)
+    assert float(run.loss.item()) == pytest.approx(0.25, rel=1e-6)
+    assert all(np.all(v == 0.0) for v in run.grads_np().values())
+    # N = 0
+    empty = far.subset(np.arange(0))
+    run = GpuRun(empty, "grid", grid, target)
+    assert np.all(run.np(run.phi) == 0.0) and float(run.loss.item()) == pytest.approx(0.25, rel=1e-6)
+    # single Gaussian at a voxel centre: contribution at its mean is exactly w (Eq. 3, G(mu) = 1)
+    one = inputs.Gaussians(np.array([[0.53125, 0.46875, 0.59375]], np.float32), np.array([[0.05, 0.02, 0.09]], np.float32),
+                           np.array([[0.2, -0.4, 0.1, 0.7]], np.float32), np.array([0.75], np.float32), np.array([0.3], np.float32))
+    run = GpuRun(one, "grid", grid, target)
+    c = (9 * 16 + 7) * 16 + 8
+    assert run.np(run.I)[c] == np.float32(0.75) and abs(run.np(run.phi)[c] - np.float32(0.3)) < 1e-7
+    # error handling: calls out of order / bad arguments
+    ctx = api.Context()
+    q = api.grid_query(grid)
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_build_accel(q)
+    assert ei.value.status == api.GS_ERR_STATE
+    dev = [torch.from_numpy(x).cuda() for x in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_preprocess(*dev, tau=1.5)
+    assert ei.value.status == api.GS_ERR_INVALID_ARG
+    ctx.gs_preprocess(*dev)
+    phi = torch.zeros(grid.num_points, device="cuda")
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_sample_fwd(q, phi, phi.clone())
+    assert ei.value.status == api.GS_ERR_STATE
+    bad = api.grid_query(inputs.Grid((16, 16, 16), (0, 0, 0), (1 / 16,) * 3, (1, 0, 0), (2, 2, 2)))
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_build_accel(bad)
+    assert ei.value.status == api.GS_ERR_INVALID_ARG
+    ctx.close()
+
+
+def test_step_host_matches_device_path(oracle):
+    # the HOST-buffer entry point (bench.py's e2e leg) gives the same results as the device-pointer calls
+    from paper_2607_01164_b200 import api
+    g = inputs.c1_gaussians(seed=0, n=512)
+    grid = inputs.c1_grid(24)
+    rng = np.random.default_rng(0)
+    target = rng.uniform(0, 1, grid.num_points).astype(np.float32)
+    xyz, fwd, loss, a, serr, gr = _oracle_all(oracle, g, grid, target)
+    ctx = api.Context()
+    P, n = grid.num_points, g.n
+    phi, I = np.zeros(P, np.float32), np.zeros(P, np.float32)
+    grads = dict(dmean=np.zeros((n, 3), np.float32), dscale=np.zeros((n, 3), np.float32), dquat=np.zeros((n, 4), np.float32),
+                 dopacity=np.zeros(n, np.float32), dscalar=np.zeros(n, np.float32), err=np.zeros(n, np.float32))
+    gh = dict(mean=g.mean, scale=g.scale, quat=g.quat, opacity=g.opacity, scalar=g.scalar)
+    got_loss = ctx.gs_step_host(gh, api.grid_query(grid), target, phi, I, grads)
+    assert got_loss == pytest.approx(loss, rel=1e-6)
+    assert np.abs(phi - fwd["phi"]).max() <= 1e-5
+    from tests.gpu_util import rel_l2
+    for k, v in gr.items():
+        assert rel_l2(grads[k], v) <= 1e-4, k
+    ctx.close()

@@ -1,0 +1,123 @@
+"""-m gpu parity: unstructured path (S1, S3, S5, S6, S7, S8) through the C ABI vs the oracle.
+
+Integer stages (Morton keys, leaf order, radix-tree topology, node boxes, query order, per-point ID
+sets) are bit-exact; fp32 values within the north_star tolerances.
+"""
+import numpy as np
+import pytest
+
+from paper_2607_01164_b200 import inputs
+from tests.gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_all(oracle, g, xyz, target, dL_dI=None):
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, dL_dI, target, TAU, mode=1)
+    return fwd, loss, a, serr, gr
+
+
+def _check_lbvh(oracle, run, g, xyz, dom, presorted=False):
+    api = run.api
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    codes = oracle.morton_codes(g.mean, dom[0], dom[1], valid)
+    order, keys = oracle.morton_order(codes)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_MORTON, np.uint32), codes[order]), "sorted Morton codes differ"
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_ORDER, np.uint32), order), "BVH leaf order differs"
+    if g.n >= 2:
+        tree = oracle.lbvh_build(keys, aabb[order])
+        assert np.array_equal(run.ctx.debug_get(api.DBG_NODE_LEFT, np.int32), tree["left"])
+        assert np.array_equal(run.ctx.debug_get(api.DBG_NODE_RIGHT, np.int32), tree["right"])
+        assert np.array_equal(run.ctx.debug_get(api.DBG_NODE_PARENT, np.int32), tree["parent"])
+        assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_PARENT, np.int32), tree["leaf_parent"])
+        nb = run.ctx.debug_get(api.DBG_NODE_AABB, np.float32, 6)
+        assert np.array_equal(nb.view(np.uint32), tree["node_aabb"].view(np.uint32)), "node boxes are not the exact min/max"
+    if not presorted and len(xyz):
+        pcodes = oracle.morton_codes(xyz, dom[0], dom[1])
+        porder, _ = oracle.morton_order(pcodes)
+        assert np.array_equal(run.ctx.debug_get(api.DBG_POINT_ORDER, np.uint32), porder), "query coherence order differs"
+        assert np.array_equal(run.ctx.debug_get(api.DBG_POINT_MORTON, np.uint32), pcodes[porder])
+
+
+@pytest.mark.parametrize("presorted", [False, True])
+def test_c3_reduced(oracle, presorted):
+    # reduced copy of BASELINE.json configs[2]: same distributions, sizes the oracle finishes in seconds;
+    # 40,003 points = many packets and a ragged tail
+    xyz_all, t_all = inputs.c3_points(seed=3, p=60000)
+    g = inputs.c3_gaussians(xyz_all, t_all, seed=3, n=20000, sigma_lo=0.004, sigma_hi=0.04)
+    idx = inputs.batch_indices(3, 0, len(xyz_all), 40003)
+    xyz, target = np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])
+    dom = inputs.points_domain(xyz_all)
+    fwd, loss, a, serr, gr = _oracle_all(oracle, g, xyz, target)
+    run = GpuRun(g, "points", xyz, target, domain=dom, presorted=presorted)
+    _check_lbvh(oracle, run, g, xyz, dom, presorted)
+    tested, hits = check_sets(run, fwd)
+    assert hits > 20 * len(xyz)
+    check_forward(run, fwd)
+    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+    np.testing.assert_allclose(run.np(run.serr), serr, atol=1e-5)
+    check_grads(run, gr)
+
+
+def test_c5_like_sparse_with_dI(oracle):
+    # shell-and-fragments distribution (configs[4] shape): most of the box is empty, many uncovered samples
+    xyz_all, t_all = inputs.c5_points(seed=5, p=50000, clusters=64, chunk=1 << 15)
+    g = inputs.c3_gaussians(xyz_all, t_all, seed=5, n=6000, sigma_lo=0.002, sigma_hi=0.01)
+    rng = np.random.default_rng(9)
+    extra = rng.uniform(0, 1, (3000, 3)).astype(np.float32)  # queries far from any Gaussian
+    xyz = np.concatenate([xyz_all[:30001], extra])
+    target = np.concatenate([t_all[:30001], np.zeros(3000, np.float32)])
+    dI = rng.standard_normal(len(xyz)) * 1e-3
+    dom = (np.zeros(3, np.float32), np.ones(3, np.float32))
+    fwd, loss, a, serr, gr = _oracle_all(oracle, g, xyz, target, dI)
+    assert (fwd["count"] == 0).sum() > 1000
+    run = GpuRun(g, "points", xyz, target, domain=dom, dL_dI=dI.astype(np.float32))
+    _check_lbvh(oracle, run, g, xyz, dom)
+    check_sets(run, fwd)
+    check_forward(run, fwd)
+    check_grads(run, gr)
+
+
+def test_degenerate_unstructured(oracle):
+    rng = np.random.default_rng(2)
+    dom = (np.zeros(3, np.float32), np.ones(3, np.float32))
+    xyz = rng.uniform(0, 1, (1000, 3)).astype(np.float32)
+    target = rng.uniform(0, 1, 1000).astype(np.float32)
+    base = inputs.c1_gaussians(seed=6, n=64)
+    base.scale[:] = (base.scale * 4).astype(np.float32)
+    for n in (0, 1, 2, 3):
+        g = base.subset(np.arange(n))
+        run = GpuRun(g, "points", xyz, target, domain=dom)
+        if n:
+            fwd, loss, a, serr, gr = _oracle_all(oracle, g, xyz, target)
+            _check_lbvh(oracle, run, g, xyz, dom)
+            check_sets(run, fwd)
+            check_forward(run, fwd)
+            check_grads(run, gr)
+        else:
+            assert np.all(run.np(run.phi) == 0.0) and np.all(run.np(run.I) == 0.0)
+    # identical means (equal Morton codes: the id in the low word keeps keys unique), invalid Gaussians, P = 0 / 1 / 33
+    g = base.subset(np.arange(40))
+    g.mean[5:25] = g.mean[5]
+    g.scale[30, 0] = np.nan
+    g.quat[31] = 0
+    for P in (0, 1, 33):
+        run = GpuRun(g, "points", xyz[:P], target[:P], domain=dom)
+        if P:
+            fwd, loss, a, serr, gr = _oracle_all(oracle, g, xyz[:P], target[:P])
+            _check_lbvh(oracle, run, g, xyz[:P], dom)
+            check_sets(run, fwd)
+            check_forward(run, fwd)
+            check_grads(run, gr)
+    # a point query without a domain is a state error
+    from paper_2607_01164_b200 import api
+    import torch
+    ctx = api.Context()
+    dev = [torch.from_numpy(x).cuda() for x in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    ctx.gs_preprocess(*dev)
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_build_accel(api.points_query(torch.from_numpy(xyz).cuda()))
+    assert ei.value.status == api.GS_ERR_STATE
+    ctx.close()
