@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from paper_2607_01164_b200 import inputs
-from tests.gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
+from gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
 
 pytestmark = pytest.mark.gpu
 
@@ -159,7 +159,7 @@ def test_step_host_matches_device_path(oracle):
     got_loss = ctx.gs_step_host(gh, api.grid_query(grid), target, phi, I, grads)
     assert got_loss == pytest.approx(loss, rel=1e-6)
     assert np.abs(phi - fwd["phi"]).max() <= 1e-5
-    from tests.gpu_util import rel_l2
+    from gpu_util import rel_l2
     for k, v in gr.items():
         assert rel_l2(grads[k], v) <= 1e-4, k
     ctx.close()

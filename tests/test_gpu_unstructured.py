@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2607_01164_b200 import inputs
-from tests.gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
+from gpu_util import TAU, GpuRun, check_forward, check_grads, check_sets
 
 pytestmark = pytest.mark.gpu
 
