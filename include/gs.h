@@ -192,6 +192,25 @@ gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, u
  * pairs tested (predicate evaluated) and pairs hit.  Only collected by gs_debug_point_sets. */
 gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_host);
 
+/* ---- measurement: CUDA-event timing of the stages, on the context's stream --------------------
+ * While enabled, every stage of the calls above is bracketed by a pair of CUDA events recorded on
+ * the context's stream.  gs_profile_read synchronises the stream, adds up the elapsed time of all
+ * pairs recorded since the last read and resets them.  ms_host[GS_PROF_STAGES] receives milliseconds,
+ * calls_host[GS_PROF_STAGES] the number of times the stage ran, *launches_host the number of kernels
+ * this library launched since the last read (memsets and copies not counted).  All outputs nullable.
+ * Errors: INVALID_ARG, CUDA. */
+typedef enum {
+    GS_PROF_PREPROCESS = 0, /* S1 kernel                                                   */
+    GS_PROF_BUILD = 1,      /* S2 or S3: every kernel of gs_build_accel                    */
+    GS_PROF_FWD = 2,        /* S4/S5 + S6: the forward sampling kernel                     */
+    GS_PROF_BWD_PACK = 3,   /* per-sample coefficients (structured backward only)          */
+    GS_PROF_BWD = 4,        /* S7: the backward sampling kernel                            */
+    GS_PROF_FINALIZE = 5,   /* S8                                                          */
+    GS_PROF_STAGES = 6
+} gs_prof_stage;
+gs_status gs_profile_enable(gs_ctx *ctx, int32_t on);
+gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uint64_t *launches_host);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,9 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
  DBG_NODE_LEFT, DBG_NODE_RIGHT, DBG_NODE_PARENT, DBG_LEAF_PARENT, DBG_NODE_AABB, DBG_POINT_ORDER, DBG_POINT_MORTON) = range(15)
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
-           "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters"]
+           "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
+           "gs_profile_enable", "gs_profile_read"]
+PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize"]
 
 
 class GsLibraryError(RuntimeError):
@@ -87,6 +89,8 @@ def load_library():
     lib.gs_debug_read.argtypes = [P, C.c_int32, P, C.c_size_t]
     lib.gs_debug_point_sets.argtypes = [P, C.POINTER(_Query), P, P, P]
     lib.gs_debug_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.gs_profile_enable.argtypes = [P, C.c_int32]
+    lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
     for name in EXPORTS:
         if name not in ("gs_destroy", "gs_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -217,6 +221,18 @@ class Context:
         self._check(self.lib.gs_step_host(self.h, C.byref(g), _domain(domain), C.c_float(tau), C.byref(q_host), _ptr(target_host),
                                           _ptr(phi_host), _ptr(I_host), C.byref(loss), gr))
         return float(loss.value)
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.gs_profile_enable(self.h, int(on)))
+
+    def profile_read(self):
+        """(ms per stage dict, calls per stage dict, kernel launches) since the last read; synchronises."""
+        ms = (C.c_float * len(PROF_STAGES))()
+        calls = (C.c_uint32 * len(PROF_STAGES))()
+        launches = C.c_uint64()
+        self._check(self.lib.gs_profile_read(self.h, ms, calls, C.byref(launches)))
+        return ({k: float(ms[i]) for i, k in enumerate(PROF_STAGES)}, {k: int(calls[i]) for i, k in enumerate(PROF_STAGES)},
+                int(launches.value))
 
     # ---- helpers -----------------------------------------------------------------------------
     def alloc_grads(self, n: int, with_err: bool = True) -> dict:

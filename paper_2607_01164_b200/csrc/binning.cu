@@ -101,14 +101,14 @@ cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd
                                cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(total, 0, sizeof(unsigned long long), s);
     if (e != cudaSuccess || N == 0) return e;
-    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, count, total);
+    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, count, total); count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
                               uint32_t *key, uint32_t *val, cudaStream_t s) {
     if (T == 0) return cudaSuccess;
-    k_pair_write<<<(T + 255) / 256, 256, 0, s>>>(aabb, N, gd, offset, T, key, val);
+    k_pair_write<<<(T + 255) / 256, 256, 0, s>>>(aabb, N, gd, offset, T, key, val); count_launch();
     return cudaGetLastError();
 }
 
@@ -116,7 +116,7 @@ cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks
     const uint32_t n = (T == 0) ? nbricks + 1 : T + 1;
     unsigned blocks = (n + 255) / 256;
     if (T == 0 && blocks > 1024) blocks = 1024;
-    k_brick_start<<<blocks, 256, 0, s>>>(key, T, nbricks, start);
+    k_brick_start<<<blocks, 256, 0, s>>>(key, T, nbricks, start); count_launch();
     return cudaGetLastError();
 }
 

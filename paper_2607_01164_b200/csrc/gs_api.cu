@@ -9,7 +9,30 @@
 
 using namespace gs;
 
+namespace gs {
+unsigned long long g_launches = 0;
+}
+
 namespace {
+
+// RAII bracket: two CUDA events around a stage on the context's stream while profiling is enabled
+struct Stage {
+    gs_ctx *ctx;
+    gs_ctx::ProfPair pp{};
+    bool on = false;
+    Stage(gs_ctx *c, int stage) : ctx(c) {
+        if (!c->prof) return;
+        if (!c->prof_free.empty()) { pp = c->prof_free.back(); c->prof_free.pop_back(); }
+        else if (cudaEventCreate(&pp.a) != cudaSuccess || cudaEventCreate(&pp.b) != cudaSuccess) { cudaGetLastError(); return; }
+        pp.stage = stage;
+        on = cudaEventRecord(pp.a, c->stream) == cudaSuccess;
+    }
+    ~Stage() {
+        if (!on) return;
+        cudaEventRecord(pp.b, ctx->stream);
+        ctx->prof_pending.push_back(pp);
+    }
+};
 
 gs_status fail(gs_ctx *ctx, gs_status st, const char *what) {
     if (ctx) ctx->err = what;
@@ -112,6 +135,8 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
+    for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
+        for (auto &pp : *v) { cudaEventDestroy(pp.a); cudaEventDestroy(pp.b); }
     delete ctx;
 }
 
@@ -142,7 +167,10 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     ctx->r = (float)sqrt((double)ctx->r2);
     ctx->have_dom = dom != nullptr;
     if (dom) ctx->dom = *dom;
-    CK(launch_preprocess(*g, ctx->r, ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->params.as<float>(), ctx->stream), "preprocess");
+    {
+        Stage stage(ctx, GS_PROF_PREPROCESS);
+        CK(launch_preprocess(*g, ctx->r, ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->params.as<float>(), ctx->stream), "preprocess");
+    }
     ctx->have_pre = true;
     return GS_OK;
 }
@@ -158,6 +186,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     ctx->accel_kind = -1;
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
+    Stage stage(ctx, GS_PROF_BUILD);
     if (q->kind == GS_QUERY_GRID) {
         const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
         CK(ctx->bcount.reserve(((size_t)N + 1) * 4), "alloc brick counts");
@@ -239,11 +268,13 @@ static gs_status check_ready(gs_ctx *ctx, const gs_query *q, const char *who) {
 static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
     cudaStream_t s = ctx->stream;
     if (ctx->accel_kind == GS_QUERY_GRID) {
+        Stage stage(ctx, GS_PROF_FWD);
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_val[ctx->pair_sel].as<uint32_t>(),
                            ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, s), "grid forward");
     } else {
         uint32_t *ovf = ctx->counters.as<uint32_t>();
         CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
+        Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->rec.as<float4>(), ctx->N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, o,
                              ovf, s), "points forward");
@@ -280,17 +311,23 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     BwdIn in{phi, I, dL_dphi, dL_dI, target};
     if (ctx->accel_kind == GS_QUERY_GRID) {
         CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc sample pack");
-        CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
+        {
+            Stage stage(ctx, GS_PROF_BWD_PACK);
+            CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
+        }
+        Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.as<float4>(), ctx->r2,
                            ctx->gacc.as<float>(), s), "grid backward");
     } else {
         uint32_t *ovf = ctx->counters.as<uint32_t>();
         CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
+        Stage stage(ctx, GS_PROF_BWD);
         CK(launch_points_bwd(ctx->rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, in,
                              ctx->gacc.as<float>(), ovf, s), "points backward");
     }
+    Stage stage(ctx, GS_PROF_FINALIZE);
     CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, *out, s), "finalize");
     return GS_OK;
 }
@@ -367,6 +404,35 @@ gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_h
     CK(cudaMemcpy(v, ctx->counters.as<unsigned long long>() + 2, 16, cudaMemcpyDeviceToHost), "read counters");
     *tested_host = v[0];
     *hits_host = v[1];
+    return GS_OK;
+}
+
+gs_status gs_profile_enable(gs_ctx *ctx, int32_t on) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    ctx->prof = on != 0;
+    return GS_OK;
+}
+
+gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uint64_t *launches_host) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    float ms[GS_PROF_STAGES] = {0};
+    uint32_t calls[GS_PROF_STAGES] = {0};
+    for (auto &pp : ctx->prof_pending) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, pp.a, pp.b), "event elapsed");
+        ms[pp.stage] += t;
+        calls[pp.stage]++;
+        ctx->prof_free.push_back(pp);
+    }
+    ctx->prof_pending.clear();
+    for (int k = 0; k < GS_PROF_STAGES; k++) {
+        if (ms_host) ms_host[k] = ms[k];
+        if (calls_host) calls_host[k] = calls[k];
+    }
+    if (launches_host) *launches_host = g_launches;
+    g_launches = 0;
     return GS_OK;
 }
 

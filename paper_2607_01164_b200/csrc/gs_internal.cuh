@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <stddef.h>
 #include <string>
+#include <vector>
 
 #include "../../include/gs.h"
 
@@ -79,7 +80,16 @@ struct gs_ctx {
     // ---- scratch
     gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters;
     gs::DevBuf h2d[16];  // staging for gs_step_host
+    // ---- measurement (gs_profile_*)
+    bool prof = false;
+    struct ProfPair { cudaEvent_t a, b; int stage; };
+    std::vector<ProfPair> prof_pending, prof_free;
 };
+
+namespace gs {
+extern unsigned long long g_launches;  // kernels launched by this library (host-side count)
+inline void count_launch(int n = 1) { g_launches += (unsigned long long)n; }
+}  // namespace gs
 
 namespace gs {
 

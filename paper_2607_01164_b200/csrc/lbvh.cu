@@ -51,7 +51,7 @@ cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *n
         mp.lo[k] = dom.lo[k];
         mp.scale[k] = 1024.0f / (dom.hi[k] - dom.lo[k]);
     }
-    k_morton<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(xyz, (int)stride_floats, nan_invalid != nullptr, n, mp, codes, ids);
+    k_morton<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(xyz, (int)stride_floats, nan_invalid != nullptr, n, mp, codes, ids); count_launch();
     return cudaGetLastError();
 }
 
@@ -146,9 +146,9 @@ cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float 
     const int n = (int)N;
     cudaError_t e = cudaMemsetAsync(flags, 0, sizeof(uint32_t) * (N - 1), s);
     if (e != cudaSuccess) return e;
-    k_karras<<<(n - 1 + 255) / 256, 256, 0, s>>>(codes, ids, n, left, right, parent, leaf_parent);
-    k_refit<<<(n + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, parent, leaf_parent, node_aabb, flags);
-    k_pack_nodes<<<(n - 1 + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, node_aabb, packed);
+    k_karras<<<(n - 1 + 255) / 256, 256, 0, s>>>(codes, ids, n, left, right, parent, leaf_parent); count_launch();
+    k_refit<<<(n + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, parent, leaf_parent, node_aabb, flags); count_launch();
+    k_pack_nodes<<<(n - 1 + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, node_aabb, packed); count_launch();
     return cudaGetLastError();
 }
 

@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ me
 
 cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, cudaStream_t s) {
     if (g.n == 0) return cudaSuccess;
-    k_preprocess<<<(g.n + 255) / 256, 256, 0, s>>>(g.mean, g.scale, g.quat, g.opacity, g.scalar, g.n, r, rec, aabb, params);
+    k_preprocess<<<(g.n + 255) / 256, 256, 0, s>>>(g.mean, g.scale, g.quat, g.opacity, g.scalar, g.n, r, rec, aabb, params); count_launch();
     return cudaGetLastError();
 }
 
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
                             cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    k_finalize<<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, out);
+    k_finalize<<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, out); count_launch();
     return cudaGetLastError();
 }
 

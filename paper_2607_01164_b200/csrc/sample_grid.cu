@@ -147,6 +147,7 @@ cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, c
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
     if (sets) k_grid_fwd<true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
     else k_grid_fwd<false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+    count_launch();
     return cudaGetLastError();
 }
 
@@ -230,14 +231,14 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
 
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
-    k_pack_samples<<<(unsigned)((P + 255) / 256), 256, 0, s>>>(in.phi, in.I, in.dL_dphi, in.dL_dI, in.target, P, tau, pack);
+    k_pack_samples<<<(unsigned)((P + 255) / 256), 256, 0, s>>>(in.phi, in.I, in.dL_dphi, in.dL_dI, in.target, P, tau, pack); count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
                              float *gacc, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    k_grid_bwd<<<(N + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc);
+    k_grid_bwd<<<(N + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc); count_launch();
     return cudaGetLastError();
 }
 

@@ -175,6 +175,7 @@ cudaError_t launch_points_fwd(const float4 *rec, uint32_t N, const float4 *nodes
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
     if (sets) k_points_fwd<true><<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, tau, r2, o, 1.0 / (double)P, overflow);
     else k_points_fwd<false><<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, tau, r2, o, 1.0 / (double)P, overflow);
+    count_launch();
     return cudaGetLastError();
 }
 
@@ -184,7 +185,7 @@ cudaError_t launch_points_bwd(const float4 *rec, uint32_t N, const float4 *nodes
     (void)leaf_order;
     if (P == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((P + PT_WARPS * 32 - 1) / (PT_WARPS * 32));
-    k_points_bwd<<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, tau, r2, in, gacc, overflow);
+    k_points_bwd<<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, tau, r2, in, gacc, overflow); count_launch();
     return cudaGetLastError();
 }
 

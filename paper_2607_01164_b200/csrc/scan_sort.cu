@@ -78,15 +78,15 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_tile(const uint32_t *__re
 static cudaError_t scan_rec(const uint32_t *in, uint32_t *out, size_t n, uint32_t *tmp, int write_total, cudaStream_t s) {
     const size_t tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (tiles <= 1) {
-        k_scan_tile<<<1, SCAN_THREADS, 0, s>>>(in, out, n, nullptr, write_total);
+        k_scan_tile<<<1, SCAN_THREADS, 0, s>>>(in, out, n, nullptr, write_total); count_launch();
         return cudaGetLastError();
     }
     uint32_t *sums = tmp;                  // [tiles]
     uint32_t *next = tmp + ((tiles + 63) & ~size_t(63));
-    k_scan_reduce<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(in, n, sums);
+    k_scan_reduce<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(in, n, sums); count_launch();
     cudaError_t e = scan_rec(sums, sums, tiles, next, 0, s);
     if (e != cudaSuccess) return e;
-    k_scan_tile<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(in, out, n, sums, write_total);
+    k_scan_tile<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(in, out, n, sums, write_total); count_launch();
     return cudaGetLastError();
 }
 
@@ -191,13 +191,13 @@ cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int
     for (int shift = 0; shift < bits; shift += 8) {
         const int nb = (bits - shift) < 8 ? (bits - shift) : 8;
         const uint32_t mask = (1u << nb) - 1u;
-        k_sort_hist<<<ntiles, SORT_WARPS * 32, 0, s>>>(keys[sel], n, shift, mask, hist.as<uint32_t>(), ntiles);
+        k_sort_hist<<<ntiles, SORT_WARPS * 32, 0, s>>>(keys[sel], n, shift, mask, hist.as<uint32_t>(), ntiles); count_launch();
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         e = exclusive_scan_u32(hist.as<uint32_t>(), hist.as<uint32_t>(), hn, tmp, s);
         if (e != cudaSuccess) return e;
         k_sort_scatter<<<ntiles, SORT_WARPS * 32, 0, s>>>(keys[sel], vals[sel], keys[sel ^ 1], vals[sel ^ 1], n, shift, mask,
-                                                         hist.as<uint32_t>(), ntiles);
+                                                         hist.as<uint32_t>(), ntiles); count_launch();
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         sel ^= 1;

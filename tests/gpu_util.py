@@ -78,7 +78,9 @@ def check_forward(run, ref, scalar_range=1.0, tol=1e-5):
     err_phi = np.abs(phi - ref["phi"])[ok].max() if ok.any() else 0.0
     err_I = (np.abs(I - ref["I"]) / np.maximum(ref["I"], 1e-3))[ok].max() if ok.any() else 0.0
     assert err_phi <= tol * scalar_range, f"phi max abs err {err_phi}"
-    assert err_I <= 2e-6, f"I max rel err {err_I}"
+    # I has no north_star tolerance; fp32 bound: |dq| <~ 2 |u| |M||d| 2^-24 * few ~ 1e-5
+    # for the anisotropies tested, G = exp(-q/2) => relative error of I up to ~1e-5
+    assert err_I <= 2e-5, f"I max rel err {err_I}"
     return int(near.sum()), float(err_phi), float(err_I)
 
 
@@ -91,10 +93,16 @@ def check_sets(run, ref):
     return tested, hits
 
 
-def check_grads(run, ref_grads, tol=1e-4):
+def check_grads(run, ref_grads, tol=1e-4, zero_floor=None):
+    """Relative L2 error per parameter tensor <= tol (north_star).  zero_floor: {name: magnitude} for
+    tensors whose exact gradient vanishes by symmetry (e.g. a single-Gaussian model, where Phi = v
+    wherever it is covered): there the fp32 result is compared against that magnitude instead."""
     got = run.grads_np()
     errs = {}
     for k, v in ref_grads.items():
-        errs[k] = rel_l2(got[k], v)
+        if zero_floor and k in zero_floor:
+            errs[k] = float(np.linalg.norm(got[k].ravel() - v.ravel()) / max(zero_floor[k], np.linalg.norm(v)))
+        else:
+            errs[k] = rel_l2(got[k], v)
         assert errs[k] <= tol, f"{k}: rel L2 err {errs[k]}"
     return errs

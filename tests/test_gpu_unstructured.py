@@ -95,7 +95,10 @@ def test_degenerate_unstructured(oracle):
             _check_lbvh(oracle, run, g, xyz, dom)
             check_sets(run, fwd)
             check_forward(run, fwd)
-            check_grads(run, gr)
+            # one Gaussian (or a few that do not overlap): Phi = v wherever covered, so every gradient except
+            # dL/dv vanishes exactly; compare those against the size of the terms that cancel (~ |dL/dv|)
+            floor = {k: float(np.linalg.norm(gr["dscalar"])) for k in ("dmean", "dscale", "dquat", "dopacity")}
+            check_grads(run, gr, zero_floor=floor)
         else:
             assert np.all(run.np(run.phi) == 0.0) and np.all(run.np(run.I) == 0.0)
     # identical means (equal Morton codes: the id in the low word keeps keys unique), invalid Gaussians, P = 0 / 1 / 33
@@ -110,7 +113,7 @@ def test_degenerate_unstructured(oracle):
             _check_lbvh(oracle, run, g, xyz[:P], dom)
             check_sets(run, fwd)
             check_forward(run, fwd)
-            check_grads(run, gr)
+            check_grads(run, gr, zero_floor={k: float(np.linalg.norm(gr["dscalar"])) for k in ("dmean", "dscale", "dquat", "dopacity")})
     # a point query without a domain is a state error
     from paper_2607_01164_b200 import api
     import torch
