@@ -288,7 +288,7 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     gs_status st = check_ready(ctx, q, "gs_sample_fwd before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
     if (ctx->P > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "phi and I must be given");
-    if (!target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
+    if (ctx->P > 0 && !target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr};
     return run_fwd(ctx, o);
