@@ -33,8 +33,21 @@ __device__ __forceinline__ uint32_t brick_range(const float *__restrict__ bb, co
     return cnt;
 }
 
+__device__ __forceinline__ uint32_t spread3(uint32_t v) {  // 10 bits -> every third bit
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+// Also emits the processing order key of the backward pass: Morton code of the Gaussian's central
+// brick (performance only: neighbouring Gaussians are processed together so their voxel data stays
+// in L1/L2); Gaussians that touch no brick of the batch get `untouched_key` and sort to the end.
 __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
-                                                      uint32_t *__restrict__ count, unsigned long long *__restrict__ total) {
+                                                      uint32_t *__restrict__ count, unsigned long long *__restrict__ total,
+                                                      uint32_t *__restrict__ okey, uint32_t *__restrict__ oval, uint32_t untouched_key) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t c = 0;
     if (i < N) {
@@ -47,12 +60,24 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         BrickRange br;
         c = brick_range(b6, gd, br);
         count[i] = c;
+        uint32_t key = untouched_key;
+        if (c) {
+            const uint32_t mx = (uint32_t)(((br.lo[0] + br.hi[0]) >> 1) - gd.brick_lo[0]);
+            const uint32_t my = (uint32_t)(((br.lo[1] + br.hi[1]) >> 1) - gd.brick_lo[1]);
+            const uint32_t mz = (uint32_t)(((br.lo[2] + br.hi[2]) >> 1) - gd.brick_lo[2]);
+            key = spread3(mx) | (spread3(my) << 1) | (spread3(mz) << 2);
+        }
+        okey[i] = key;
+        oval[i] = i;
     }
-    // 64-bit total for the overflow check
-    unsigned long long s = c;
+    // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
+    unsigned long long s = c, m = c ? 1ull : 0ull;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
-    if ((threadIdx.x & 31) == 0 && s) atomicAdd(total, s);
+    for (int d = 16; d > 0; d >>= 1) {
+        s += __shfl_xor_sync(0xffffffffu, s, d);
+        m += __shfl_xor_sync(0xffffffffu, m, d);
+    }
+    if ((threadIdx.x & 31) == 0 && s) { atomicAdd(total, s); atomicAdd(total + 1, m); }
 }
 
 __global__ void __launch_bounds__(256) k_pair_write(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
@@ -98,10 +123,10 @@ __global__ void __launch_bounds__(256) k_brick_start(const uint32_t *__restrict_
 }
 
 cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd, uint32_t *count, unsigned long long *total,
-                               cudaStream_t s) {
-    cudaError_t e = cudaMemsetAsync(total, 0, sizeof(unsigned long long), s);
+                               uint32_t *okey, uint32_t *oval, uint32_t untouched_key, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(total, 0, 2 * sizeof(unsigned long long), s);
     if (e != cudaSuccess || N == 0) return e;
-    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, count, total); count_launch();
+    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, count, total, okey, oval, untouched_key); count_launch();
     return cudaGetLastError();
 }
 

@@ -193,13 +193,30 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         CK(ctx->boffset.reserve(((size_t)N + 1) * 4), "alloc brick offsets");
         CK(ctx->brick_start.reserve(((size_t)nbricks + 1) * 4), "alloc brick_start");
         unsigned long long *total = ctx->counters.as<unsigned long long>() + 4;
-        CK(launch_brick_count(ctx->aabb.as<float>(), N, gd, ctx->bcount.as<uint32_t>(), total, s), "brick count");
+        // the backward's processing order (Gaussians by the Morton code of their central brick) shares this pass;
+        // in grid mode the leaf_key/leaf_val buffers hold that order
+        const size_t n1 = N ? N : 1;
+        for (int k = 0; k < 2; k++) {
+            CK(ctx->leaf_key[k].reserve(n1 * 4), "alloc order keys");
+            CK(ctx->leaf_val[k].reserve(n1 * 4), "alloc order vals");
+        }
+        int axis_bits = 1;
+        for (int k = 0; k < 3; k++) axis_bits = bits_for((uint64_t)gd.brick_cnt[k]) > axis_bits ? bits_for((uint64_t)gd.brick_cnt[k]) : axis_bits;
+        const uint32_t untouched_key = 1u << (3 * axis_bits);
+        CK(launch_brick_count(ctx->aabb.as<float>(), N, gd, ctx->bcount.as<uint32_t>(), total, ctx->leaf_key[0].as<uint32_t>(),
+                              ctx->leaf_val[0].as<uint32_t>(), untouched_key, s), "brick count");
         CK(exclusive_scan_u32(ctx->bcount.as<uint32_t>(), ctx->boffset.as<uint32_t>(), N, ctx->scan_tmp, s), "scan");
-        unsigned long long T64 = 0;
-        CK(cudaMemcpyAsync(&T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
+        unsigned long long T64[2] = {0, 0};
+        CK(cudaMemcpyAsync(T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
+        {
+            uint32_t *ok[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
+            uint32_t *ov[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
+            CK(radix_sort_pairs(ok, ov, N, 3 * axis_bits + 1, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "order sort");
+        }
         CK(cudaStreamSynchronize(s), "sync (T)");
-        if (T64 >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
-        const uint32_t T = (uint32_t)T64;
+        if (T64[0] >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
+        const uint32_t T = (uint32_t)T64[0];
+        ctx->M = (uint32_t)T64[1];
         const size_t tb = ((size_t)T + 1) * 4;
         for (int k = 0; k < 2; k++) {
             CK(ctx->pair_key[k].reserve(tb), "alloc pair keys");
@@ -317,7 +334,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         }
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.as<float4>(), ctx->r2,
-                           ctx->gacc.as<float>(), s), "grid backward");
+                           ctx->gacc.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
         uint32_t *ovf = ctx->counters.as<uint32_t>();
         CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");

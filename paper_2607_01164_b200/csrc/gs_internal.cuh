@@ -63,6 +63,7 @@ struct gs_ctx {
     gs_query accel_q{};
     gs::GridDesc grid{};
     uint32_t T = 0, nbricks = 0;
+    uint32_t M = 0;       // Gaussians that touch the current batch (grid): length of the backward's order list
     gs::DevBuf bcount;    // uint32 [N+1]
     gs::DevBuf boffset;   // uint32 [N+1]
     gs::DevBuf pair_key[2], pair_val[2];
@@ -104,7 +105,7 @@ cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int
                              cudaStream_t s, int *result_sel);
 
 cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd, uint32_t *count, unsigned long long *total,
-                               cudaStream_t s);
+                               uint32_t *okey, uint32_t *oval, uint32_t untouched_key, cudaStream_t s);
 cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
                               uint32_t *key, uint32_t *val, cudaStream_t s);
 cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks, uint32_t *start, cudaStream_t s);
@@ -122,7 +123,7 @@ cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, c
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
 cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
-                            float *gacc, cudaStream_t s);
+                            float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
                             cudaStream_t s);

@@ -13,7 +13,7 @@
 namespace gs {
 
 constexpr int FWD_THREADS = 512;
-constexpr int CH = 128;  // Gaussians per staged chunk
+constexpr int CH = 64;   // Gaussians per staged chunk = 2 sub-chunks of 32 (one lane per Gaussian in the cell test)
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -30,9 +30,9 @@ struct FwdSmem {
 
 __device__ __forceinline__ void stage_chunk(FwdSmem &sm, int buf, const float4 *__restrict__ rec, uint32_t N,
                                             const uint32_t *__restrict__ list, uint32_t n, uint32_t chunk) {
-    const int plane = threadIdx.x >> 7, j = threadIdx.x & (CH - 1);
+    const int plane = threadIdx.x >> 6, j = threadIdx.x & (CH - 1);
     const uint32_t idx = chunk * CH + j;
-    if (idx < n) {
+    if (plane < 4 && idx < n) {
         const uint32_t id = list[idx];
         cp_async16(&sm.rec[buf][plane][j], rec + (size_t)plane * N + id);
         if (plane == 0) sm.id[buf][j] = id;
@@ -49,7 +49,10 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
     const uint32_t b = blockIdx.x;
     const uint32_t bx = b % gd.brick_cnt[0], by = (b / gd.brick_cnt[0]) % gd.brick_cnt[1], bz = b / (gd.brick_cnt[0] * gd.brick_cnt[1]);
     const int t = threadIdx.x;
-    const int lx = bx * BRICK + (t & 7), ly = by * BRICK + ((t >> 3) & 7), lz = bz * BRICK + (t >> 6);  // batch-local voxel
+    // A warp owns a row of four 2x2x2-voxel CELLS (8 x 2 x 2 voxels); lanes 8g..8g+7 are cell g.
+    const int warp = t >> 5, lane = t & 31, cell = lane >> 3;
+    const int vx = 2 * cell + (lane & 1), vy = 2 * (warp & 3) + ((lane >> 1) & 1), vz = 2 * (warp >> 2) + ((lane >> 2) & 1);
+    const int lx = bx * BRICK + vx, ly = by * BRICK + vy, lz = bz * BRICK + vz;  // batch-local voxel
     const bool active = lx < gd.bdim[0] && ly < gd.bdim[1] && lz < gd.bdim[2];
     const float nanv = __int_as_float(0x7fc00000);
     // inactive threads (voxels clipped by the grid) carry a NaN position: the predicate is false for them
@@ -61,8 +64,14 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
     const uint32_t *list = pair_gauss + start;
     const uint32_t nchunks = (n + CH - 1) / CH;
     float I = 0.f, Nacc = 0.f;
-    uint32_t cnt = 0;
+    uint32_t cnt = 0, ntest = 0;
     unsigned long long hsum = 0, hxor = 0;
+    // cell geometry of this warp (cull only: not canonical): centre of cell 0, x step = 2 voxels
+    const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
+    const float ccx0 = fmaf((float)(BRICK * (bx + gd.brick_lo[0]) + 1), gd.spacing[0], gd.origin[0]);
+    const float ccy = fmaf((float)(BRICK * (by + gd.brick_lo[1]) + 2 * (warp & 3) + 1), gd.spacing[1], gd.origin[1]);
+    const float ccz = fmaf((float)(BRICK * (bz + gd.brick_lo[2]) + 2 * (warp >> 2) + 1), gd.spacing[2], gd.origin[2]);
+    const float rcut = sqrtf(r2);
 
     if (nchunks) stage_chunk(sm, 0, rec, N, list, n, 0);
     for (uint32_t c = 0; c < nchunks; c++) {
@@ -75,20 +84,54 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
         }
         __syncthreads();
         const int m = min((uint32_t)CH, n - c * CH);
-#pragma unroll 2
-        for (int j = 0; j < m; j++) {
-            Rec g;
-            g.a = sm.rec[buf][0][j]; g.b = sm.rec[buf][1][j]; g.c = sm.rec[buf][2][j]; g.d = sm.rec[buf][3][j];
-            float u0, u1, u2;
-            const float qd = mahalanobis(g, px, py, pz, u0, u1, u2);
-            const bool hit = qd <= r2;
-            if (hit) {
-                const float wG = g.a.w * gauss_weight(qd);
-                I += wG;
-                Nacc = fmaf(g.b.w, wG, Nacc);
-                if (SETS) {
-                    const unsigned long long h = mix64(sm.id[buf][j]);
-                    cnt++; hsum += h; hxor ^= h;
+        for (int sub = 0; sub < m; sub += 32) {
+            // ---- cull below the brick: lane = Gaussian, tested against the warp's four cells.
+            // For a cell with centre cc and half extent h (its voxel centres are cc +- h), every voxel p has
+            // |M(p - mu)| >= |M(cc - mu)| - rho,  rho = |(sum_k |M_jk| h_k)_j|  =>  no hit unless |M(cc - mu)|^2 <= (r + rho)^2.
+            // Conservative (1 + 2^-9 slack covers fp32 rounding); the canonical predicate still decides every pair.
+            uint32_t mymask;
+            {
+                const int j = sub + lane;
+                const bool have = j < m;
+                Rec g;
+                g.a = sm.rec[buf][0][j & (CH - 1)]; g.b = sm.rec[buf][1][j & (CH - 1)];
+                g.c = sm.rec[buf][2][j & (CH - 1)]; g.d = sm.rec[buf][3][j & (CH - 1)];
+                const float r0 = fabsf(g.b.x) * hx + fabsf(g.b.y) * hy + fabsf(g.b.z) * hz;
+                const float r1 = fabsf(g.c.x) * hx + fabsf(g.c.y) * hy + fabsf(g.c.z) * hz;
+                const float r2c = fabsf(g.d.x) * hx + fabsf(g.d.y) * hy + fabsf(g.d.z) * hz;
+                const float reach = rcut + sqrtf(r0 * r0 + r1 * r1 + r2c * r2c);
+                const float thr = reach * reach * 1.001953125f;
+                const float dy = ccy - g.a.y, dz = ccz - g.a.z;
+                const float e0 = g.b.y * dy + g.b.z * dz, e1 = g.c.y * dy + g.c.z * dz, e2 = g.d.y * dy + g.d.z * dz;
+                uint32_t masks[4];
+#pragma unroll
+                for (int k = 0; k < 4; k++) {
+                    const float dx = (ccx0 + (float)(2 * k) * gd.spacing[0]) - g.a.x;
+                    const float u0 = fmaf(g.b.x, dx, e0), u1 = fmaf(g.c.x, dx, e1), u2 = fmaf(g.d.x, dx, e2);
+                    const float qc = u0 * u0 + u1 * u1 + u2 * u2;
+                    masks[k] = __ballot_sync(0xffffffffu, have && qc <= thr);
+                }
+                mymask = cell == 0 ? masks[0] : cell == 1 ? masks[1] : cell == 2 ? masks[2] : masks[3];
+            }
+            // ---- each cell (8 lanes) walks its own list; the warp iterates until all four are done
+            while (__any_sync(0xffffffffu, mymask != 0u)) {
+                if (mymask) {
+                    const int j = sub + __ffs(mymask) - 1;
+                    mymask &= mymask - 1;
+                    Rec g;
+                    g.a = sm.rec[buf][0][j]; g.b = sm.rec[buf][1][j]; g.c = sm.rec[buf][2][j]; g.d = sm.rec[buf][3][j];
+                    float u0, u1, u2;
+                    const float qd = mahalanobis(g, px, py, pz, u0, u1, u2);
+                    if (SETS) ntest++;
+                    if (qd <= r2) {
+                        const float wG = g.a.w * gauss_weight(qd);
+                        I += wG;
+                        Nacc = fmaf(g.b.w, wG, Nacc);
+                        if (SETS) {
+                            const unsigned long long h = mix64(sm.id[buf][j]);
+                            cnt++; hsum += h; hxor ^= h;
+                        }
+                    }
                 }
             }
         }
@@ -129,7 +172,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
         }
     }
     if (SETS && o.counters) {
-        unsigned long long tested = active ? n : 0, hits = cnt;
+        unsigned long long tested = active ? ntest : 0, hits = cnt;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
             tested += __shfl_xor_sync(0xffffffffu, tested, d);
@@ -175,9 +218,12 @@ constexpr int BWD_WARPS = 8;
 
 __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__restrict__ rec, const float *__restrict__ aabb, uint32_t N,
                                                               GridDesc gd, const float4 *__restrict__ pack, float r2,
-                                                              float *__restrict__ gacc) {
-    const uint32_t i = blockIdx.x * BWD_WARPS + (threadIdx.x >> 5);
-    if (i >= N) return;
+                                                              float *__restrict__ gacc, const uint32_t *__restrict__ order,
+                                                              uint32_t M) {
+    // warp w processes the w-th Gaussian of the brick-ordered list of the M Gaussians that touch the batch
+    const uint32_t w = blockIdx.x * BWD_WARPS + (threadIdx.x >> 5);
+    if (w >= M) return;
+    const uint32_t i = order[w];
     const int lane = threadIdx.x & 31;
     Rec g;
     g.a = rec[i]; g.b = rec[(size_t)N + i]; g.c = rec[2 * (size_t)N + i]; g.d = rec[3 * (size_t)N + i];
@@ -236,9 +282,11 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
 }
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
-                             float *gacc, cudaStream_t s) {
-    if (N == 0) return cudaSuccess;
-    k_grid_bwd<<<(N + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc); count_launch();
+                            float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
+    // untouched Gaussians keep a zero accumulator row
+    cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC * sizeof(float), s);
+    if (e != cudaSuccess || M == 0) return e;
+    k_grid_bwd<<<(M + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc, order, M); count_launch();
     return cudaGetLastError();
 }
 
