@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 }
 
 constexpr int BWD_WARPS = 4;
+constexpr int GPW = 1;    // Gaussians per warp (consecutive in the order list); 8 measured slower on C2 (0.84 vs 0.73 ms)
 constexpr int QCAP = 64;  // per-warp queue of surviving cells (power of two, >= 2 * 32)
 
 __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__restrict__ rec, const float *__restrict__ aabb, uint32_t N,
@@ -41,7 +42,10 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
     // warp w processes the w-th Gaussian of the brick-ordered list of the M Gaussians that touch the batch
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t w = blockIdx.x * BWD_WARPS + warp;
+    // A CTA owns BWD_WARPS * GPW consecutive Gaussians of the order list (one neighbourhood of the grid, so
+    // that its per-sample coefficients are shared through this SM's L1); the warps interleave over them.
+    for (int rep = 0; rep < GPW; rep++) {
+    const uint32_t w = blockIdx.x * (BWD_WARPS * GPW) + rep * BWD_WARPS + warp;
     if (w >= M) return;  // whole warps leave; no block-wide barrier is used below
     const uint32_t i = order[w];
     const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
@@ -63,7 +67,7 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
         clo[k] = lo >> 1;
         nc[k] = (hi >> 1) - clo[k] + 1;
     }
-    if (empty) return;  // the accumulator row stays zero (memset by the launcher)
+    if (empty) continue;  // the accumulator row stays zero (memset by the launcher)
 
     // cull bound (not canonical): |M(p - mu)| >= |M(cc - mu)| - rho for every voxel p of a cell with centre cc
     const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
@@ -160,6 +164,8 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
     // lane 2c holds component c: 16 floats per Gaussian, written as one coalesced 64-byte row
     const float val = __shfl_sync(0xffffffffu, acc[0], (lane & 15) * 2);
     if (lane < 16) gacc[(size_t)i * GACC + lane] = val;
+    __syncwarp();
+    }  // rep
 }
 
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s) {
@@ -174,7 +180,7 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, co
     // untouched Gaussians keep a zero accumulator row
     cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC * sizeof(float), s);
     if (e != cudaSuccess || M == 0) return e;
-    k_grid_bwd<<<(M + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc, order, M);
+    k_grid_bwd<<<(M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW), BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc, order, M);
     count_launch();
     return cudaGetLastError();
 }
