@@ -4,8 +4,9 @@
 // cp.async ("each thread block cooperatively loads a batch of Gaussians ... into shared memory").
 // Below the brick the kernel culls per CELL of 2x2x2 voxels:
 //   * list building: lane = Gaussian; it tests its Gaussian against the warp's 32 cells with a
-//     conservative whitened-space bound (see cell_reach2) and a ballot hands every cell its bit mask;
-//   * evaluation: lane = cell; the lane walks its own mask and evaluates its 8 voxels against each
+//     conservative whitened-space bound and a ballot per cell produces the cell's bit mask
+//     (|u0 + ix ex|^2 is expanded per cell row, so a cell costs ~2 FFMA + compare + vote);
+//   * evaluation: lane = cell; the lane walks its own masks and evaluates its 8 voxels against each
 //     listed Gaussian.  The canonical fp32 predicate sequence (D4) shares sub-expressions between
 //     voxels with equal x / y coordinates, so 8 voxel tests cost 72 FP32 instructions instead of 136
 //     with bit-identical results.
@@ -16,7 +17,7 @@
 namespace gs {
 
 constexpr int FWD_THREADS = 64;
-constexpr int CAP = 128;  // Gaussians staged per round
+constexpr int CAP = 128;  // Gaussians staged per round (4 sub-chunks of 32)
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -31,6 +32,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
                                                            double invP) {
     __shared__ float4 srec[4][CAP];
     __shared__ uint32_t sid[CAP];
+    __shared__ uint4 smask[FWD_THREADS / 32][32];  // [warp][cell] -> masks of the 4 sub-chunks
     const uint32_t b = blockIdx.x;
     const int bx = b % gd.brick_cnt[0], by = (b / gd.brick_cnt[0]) % gd.brick_cnt[1], bz = b / (gd.brick_cnt[0] * gd.brick_cnt[1]);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -65,6 +67,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
 
     const uint32_t start = brick_start[b], n = brick_start[b + 1] - start;
     const uint32_t *list = pair_gauss + start;
+    uint32_t *mywords = reinterpret_cast<uint32_t *>(&smask[warp][0]);
     for (uint32_t round = 0; round < n; round += CAP) {
         const int m = min((uint32_t)CAP, n - round);
         if (round) __syncthreads();  // everyone is done with the previous round's records
@@ -76,89 +79,95 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
             cp_async16(&srec[3][j], rec + 3 * (size_t)N + id);
             if (SETS) sid[j] = id;
         }
+        smask[warp][lane] = make_uint4(0u, 0u, 0u, 0u);
         cp_async_wait_all();
         __syncthreads();
+        // ---- list building: lane = Gaussian sub + lane, against the warp's 32 cells.
+        // For a cell with centre cc and half extent h (its voxel centres are cc +- h) every voxel p obeys
+        // |M(p - mu)| >= |M(cc - mu)| - rho, rho = |(sum_k |M_jk| h_k)_j|, so the cell holds no hit unless
+        // |M(cc - mu)|^2 <= (r + rho)^2.  2^-9 slack covers fp32 rounding; the canonical predicate decides.
         for (int sub = 0; sub < m; sub += 32) {
-            // ---- list building: lane = Gaussian sub + lane, against the warp's 32 cells.
-            // For a cell with centre cc and half extent h (its voxel centres are cc +- h) every voxel p obeys
-            // |M(p - mu)| >= |M(cc - mu)| - rho, rho = |(sum_k |M_jk| h_k)_j|, so the cell holds no hit unless
-            // |M(cc - mu)|^2 <= (r + rho)^2.  2^-9 slack covers fp32 rounding; the canonical predicate decides.
-            uint32_t mymask = 0;
-            {
-                const int j = sub + lane;
-                const bool have = j < m;
-                const int js = have ? j : 0;
-                const float4 ga = srec[0][js], gb = srec[1][js], gc = srec[2][js], gd4 = srec[3][js];
-                const float q0 = fabsf(gb.x) * hx + fabsf(gb.y) * hy + fabsf(gb.z) * hz;
-                const float q1 = fabsf(gc.x) * hx + fabsf(gc.y) * hy + fabsf(gc.z) * hz;
-                const float q2 = fabsf(gd4.x) * hx + fabsf(gd4.y) * hy + fabsf(gd4.z) * hz;
-                const float reach = rcut + sqrtf(q0 * q0 + q1 * q1 + q2 * q2);
-                const float thr = have ? reach * reach * 1.001953125f : -1.f;
-                const float dx0 = c0x - ga.x, dy0 = c0y - ga.y, dz0 = c0z - ga.z;
-                const float ub0 = gb.x * dx0 + gb.y * dy0 + gb.z * dz0;
-                const float ub1 = gc.x * dx0 + gc.y * dy0 + gc.z * dz0;
-                const float ub2 = gd4.x * dx0 + gd4.y * dy0 + gd4.z * dz0;
-                const float sx2 = 2.f * gd.spacing[0], sy2 = 2.f * gd.spacing[1], sz2 = 2.f * gd.spacing[2];
-                const float ex0 = gb.x * sx2, ex1 = gc.x * sx2, ex2 = gd4.x * sx2;
-                const float ey0 = gb.y * sy2, ey1 = gc.y * sy2, ey2 = gd4.y * sy2;
-                const float ez0 = gb.z * sz2, ez1 = gc.z * sz2, ez2 = gd4.z * sz2;
+            const int j = sub + lane;
+            const bool have = j < m;
+            const int js = have ? j : 0;
+            const float4 ga = srec[0][js], gb = srec[1][js], gc = srec[2][js], gd4 = srec[3][js];
+            const float q0 = fabsf(gb.x) * hx + fabsf(gb.y) * hy + fabsf(gb.z) * hz;
+            const float q1 = fabsf(gc.x) * hx + fabsf(gc.y) * hy + fabsf(gc.z) * hz;
+            const float q2 = fabsf(gd4.x) * hx + fabsf(gd4.y) * hy + fabsf(gd4.z) * hz;
+            const float reach = rcut + sqrtf(q0 * q0 + q1 * q1 + q2 * q2);
+            const float thr = have ? reach * reach * 1.001953125f : -1.f;
+            const float dx0 = c0x - ga.x, dy0 = c0y - ga.y, dz0 = c0z - ga.z;
+            const float ub0 = gb.x * dx0 + gb.y * dy0 + gb.z * dz0;
+            const float ub1 = gc.x * dx0 + gc.y * dy0 + gc.z * dz0;
+            const float ub2 = gd4.x * dx0 + gd4.y * dy0 + gd4.z * dz0;
+            const float sx2 = 2.f * gd.spacing[0], sy2 = 2.f * gd.spacing[1], sz2 = 2.f * gd.spacing[2];
+            const float ex0 = gb.x * sx2, ex1 = gc.x * sx2, ex2 = gd4.x * sx2;
+            const float ey0 = gb.y * sy2, ey1 = gc.y * sy2, ey2 = gd4.y * sy2;
+            const float ez0 = gb.z * sz2, ez1 = gc.z * sz2, ez2 = gd4.z * sz2;
+            const float exx = ex0 * ex0 + ex1 * ex1 + ex2 * ex2;  // |ex|^2
+            const int word = sub >> 5;
 #pragma unroll
-                for (int iz = 0; iz < 2; iz++) {
-                    const float z0 = fmaf((float)iz, ez0, ub0), z1 = fmaf((float)iz, ez1, ub1), z2 = fmaf((float)iz, ez2, ub2);
+            for (int iz = 0; iz < 2; iz++) {
+                const float z0 = fmaf((float)iz, ez0, ub0), z1 = fmaf((float)iz, ez1, ub1), z2 = fmaf((float)iz, ez2, ub2);
 #pragma unroll
-                    for (int iy = 0; iy < 4; iy++) {
-                        const float y0 = fmaf((float)iy, ey0, z0), y1 = fmaf((float)iy, ey1, z1), y2 = fmaf((float)iy, ey2, z2);
+                for (int iy = 0; iy < 4; iy++) {
+                    const float y0 = fmaf((float)iy, ey0, z0), y1 = fmaf((float)iy, ey1, z1), y2 = fmaf((float)iy, ey2, z2);
+                    // |y + ix ex|^2 = |y|^2 + ix (2 y.ex) + ix^2 |ex|^2
+                    const float yy = y0 * y0 + y1 * y1 + y2 * y2;
+                    const float ye = 2.f * (y0 * ex0 + y1 * ex1 + y2 * ex2);
 #pragma unroll
-                        for (int ix = 0; ix < 4; ix++) {
-                            const float u0 = fmaf((float)ix, ex0, y0), u1 = fmaf((float)ix, ex1, y1), u2 = fmaf((float)ix, ex2, y2);
-                            const float qc = u0 * u0 + u1 * u1 + u2 * u2;
-                            const uint32_t bal = __ballot_sync(0xffffffffu, qc <= thr);
-                            if (lane == iz * 16 + iy * 4 + ix) mymask = bal;
-                        }
+                    for (int ix = 0; ix < 4; ix++) {
+                        const float qc = fmaf((float)(ix * ix), exx, fmaf((float)ix, ye, yy));
+                        const uint32_t bal = __ballot_sync(0xffffffffu, qc <= thr);
+                        if (lane == 0) mywords[4 * (iz * 16 + iy * 4 + ix) + word] = bal;
                     }
                 }
             }
-            // ---- evaluation: lane = cell, walking its own list; 8 voxels per listed Gaussian
-            while (mymask) {
-                const int j = sub + __ffs(mymask) - 1;
-                mymask &= mymask - 1;
-                const float4 ga = srec[0][j], gb = srec[1][j], gc = srec[2][j], gd4 = srec[3][j];
-                // canonical sequence (D4), shared between voxels: d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx));
-                // qd = fma(u2, u2, fma(u1, u1, u0 * u0))
-                float dx[2], dy[2], dz[2], qd[8];
+        }
+        __syncwarp();
+        // ---- evaluation: lane = cell, walking its own masks over the whole round; 8 voxels per listed Gaussian
+        const uint4 mk = smask[warp][lane];
+        unsigned long long mlo = ((unsigned long long)mk.y << 32) | mk.x, mhi = ((unsigned long long)mk.w << 32) | mk.z;
+        while (mlo | mhi) {
+            int j;
+            if (mlo) { j = __ffsll((long long)mlo) - 1; mlo &= mlo - 1; }
+            else { j = 63 + __ffsll((long long)mhi); mhi &= mhi - 1; }
+            const float4 ga = srec[0][j], gb = srec[1][j], gc = srec[2][j], gd4 = srec[3][j];
+            // canonical sequence (D4), shared between voxels: d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx));
+            // qd = fma(u2, u2, fma(u1, u1, u0 * u0))
+            float dx[2], dy[2], dz[2], qd[8];
 #pragma unroll
-                for (int d = 0; d < 2; d++) {
-                    dx[d] = __fsub_rn(px[d], ga.x);
-                    dy[d] = __fsub_rn(py[d], ga.y);
-                    dz[d] = __fsub_rn(pz[d], ga.z);
-                }
+            for (int d = 0; d < 2; d++) {
+                dx[d] = __fsub_rn(px[d], ga.x);
+                dy[d] = __fsub_rn(py[d], ga.y);
+                dz[d] = __fsub_rn(pz[d], ga.z);
+            }
 #pragma unroll
-                for (int row = 0; row < 3; row++) {
-                    const float4 mr = row == 0 ? gb : row == 1 ? gc : gd4;
-                    float a[2], ab[4];
+            for (int row = 0; row < 3; row++) {
+                const float4 mr = row == 0 ? gb : row == 1 ? gc : gd4;
+                float a[2], ab[4];
 #pragma unroll
-                    for (int ix = 0; ix < 2; ix++) a[ix] = __fmul_rn(mr.x, dx[ix]);
+                for (int ix = 0; ix < 2; ix++) a[ix] = __fmul_rn(mr.x, dx[ix]);
 #pragma unroll
-                    for (int iy = 0; iy < 2; iy++)
+                for (int iy = 0; iy < 2; iy++)
 #pragma unroll
-                        for (int ix = 0; ix < 2; ix++) ab[iy * 2 + ix] = __fmaf_rn(mr.y, dy[iy], a[ix]);
-#pragma unroll
-                    for (int v = 0; v < 8; v++) {
-                        const float u = __fmaf_rn(mr.z, dz[v >> 2], ab[v & 3]);
-                        qd[v] = row == 0 ? __fmul_rn(u, u) : __fmaf_rn(u, u, qd[v]);
-                    }
-                }
-                if (SETS) ntest += 8;
+                    for (int ix = 0; ix < 2; ix++) ab[iy * 2 + ix] = __fmaf_rn(mr.y, dy[iy], a[ix]);
 #pragma unroll
                 for (int v = 0; v < 8; v++) {
-                    if (qd[v] <= r2) {
-                        const float wG = ga.w * gauss_weight(qd[v]);
-                        I[v] += wG;
-                        Nacc[v] = fmaf(gb.w, wG, Nacc[v]);
-                        if (SETS) {
-                            const unsigned long long h = mix64(sid[j]);
-                            cnt[v]++; hsum[v] += h; hxor[v] ^= h;
-                        }
+                    const float u = __fmaf_rn(mr.z, dz[v >> 2], ab[v & 3]);
+                    qd[v] = row == 0 ? __fmul_rn(u, u) : __fmaf_rn(u, u, qd[v]);
+                }
+            }
+            if (SETS) ntest += 8;
+#pragma unroll
+            for (int v = 0; v < 8; v++) {
+                if (qd[v] <= r2) {
+                    const float wG = ga.w * gauss_weight(qd[v]);
+                    I[v] += wG;
+                    Nacc[v] = fmaf(gb.w, wG, Nacc[v]);
+                    if (SETS) {
+                        const unsigned long long h = mix64(sid[j]);
+                        cnt[v]++; hsum[v] += h; hxor[v] ^= h;
                     }
                 }
             }
@@ -168,28 +177,54 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
     // ---- S6 epilogue: coverage rule I > tau (strict), empty value 0, I always written (D5)
     float res2 = 0.f;
     unsigned long long tested = 0, hits = 0;
+    const float dscale = (float)(2.0 * invP);
+    const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
+    const bool vec2 = !SETS && !(bdx & 1u);  // x-pairs are 8-byte aligned when the batch's x extent is even
 #pragma unroll
-    for (int v = 0; v < 8; v++) {
-        const int x = lx + (v & 1), y = ly + ((v >> 1) & 1), z = lz + (v >> 2);
-        const bool active = x < gd.bdim[0] && y < gd.bdim[1] && z < gd.bdim[2];
-        if (!active) continue;
-        const bool covered = I[v] > tau;
-        const float phi = covered ? __fdividef(Nacc[v], I[v]) : 0.f;
-        const size_t c = ((size_t)z * gd.bdim[1] + y) * gd.bdim[0] + x;
-        o.phi[c] = phi;
-        o.I[c] = I[v];
-        if (o.target) {
-            const float res = phi - o.target[c];
-            res2 = fmaf(res, res, res2);
-            if (o.dL_dphi) o.dL_dphi[c] = covered ? (float)(2.0 * invP) * res : 0.f;
-            if (o.sample_err) o.sample_err[c] = fabsf(res);
+    for (int r = 0; r < 4; r++) {  // the cell's four x-rows: (y, z) = (ly + (r & 1), lz + (r >> 1))
+        const uint32_t y = (uint32_t)ly + (r & 1), z = (uint32_t)lz + (r >> 1);
+        if (y >= bdy || z >= (uint32_t)gd.bdim[2] || (uint32_t)lx >= bdx) continue;
+        const uint32_t c = (z * bdy + y) * bdx + (uint32_t)lx;  // P < 2^32
+        float ph[2], Iv[2];
+        bool cov[2];
+#pragma unroll
+        for (int d = 0; d < 2; d++) {
+            const int v = r * 2 + d;
+            cov[d] = I[v] > tau;
+            ph[d] = cov[d] ? __fdividef(Nacc[v], I[v]) : 0.f;
+            Iv[d] = I[v];
         }
-        if (SETS) {
-            if (o.set_count) o.set_count[c] = cnt[v];
-            if (o.set_sum) o.set_sum[c] = hsum[v];
-            if (o.set_xor) o.set_xor[c] = hxor[v];
-            tested += ntest / 8;
-            hits += cnt[v];
+        if (vec2) {
+            *reinterpret_cast<float2 *>(o.phi + c) = make_float2(ph[0], ph[1]);
+            *reinterpret_cast<float2 *>(o.I + c) = make_float2(Iv[0], Iv[1]);
+            if (o.target) {
+                const float2 t = *reinterpret_cast<const float2 *>(o.target + c);
+                const float r0 = ph[0] - t.x, r1 = ph[1] - t.y;
+                res2 = fmaf(r0, r0, fmaf(r1, r1, res2));
+                if (o.dL_dphi) *reinterpret_cast<float2 *>(o.dL_dphi + c) = make_float2(cov[0] ? dscale * r0 : 0.f, cov[1] ? dscale * r1 : 0.f);
+                if (o.sample_err) *reinterpret_cast<float2 *>(o.sample_err + c) = make_float2(fabsf(r0), fabsf(r1));
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < 2; d++) {
+                if ((uint32_t)lx + d >= bdx) continue;
+                const int v = r * 2 + d;
+                o.phi[c + d] = ph[d];
+                o.I[c + d] = Iv[d];
+                if (o.target) {
+                    const float res = ph[d] - o.target[c + d];
+                    res2 = fmaf(res, res, res2);
+                    if (o.dL_dphi) o.dL_dphi[c + d] = cov[d] ? dscale * res : 0.f;
+                    if (o.sample_err) o.sample_err[c + d] = fabsf(res);
+                }
+                if (SETS) {
+                    if (o.set_count) o.set_count[c + d] = cnt[v];
+                    if (o.set_sum) o.set_sum[c + d] = hsum[v];
+                    if (o.set_xor) o.set_xor[c + d] = hxor[v];
+                    tested += ntest / 8;
+                    hits += cnt[v];
+                }
+            }
         }
     }
     if (o.target && o.loss) {
