@@ -166,7 +166,6 @@ def run_ours(args):
     target = dev(wl["target"])
     phi = torch.empty(P, device="cuda")
     I = torch.empty(P, device="cuda")
-    dphi = torch.empty(P, device="cuda")
     loss = torch.zeros(1, dtype=torch.float64, device="cuda")
     grads = ctx.alloc_grads(g.n)
     flat = None
@@ -177,8 +176,8 @@ def run_ours(args):
         loss.zero_()
         ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
         ctx.gs_build_accel(q)
-        ctx.gs_sample_fwd(q, phi, I, target=target, loss=loss, dL_dphi=dphi)
-        ctx.gs_sample_bwd(q, phi, I, dphi, grads, target=target)
+        ctx.gs_sample_fwd(q, phi, I, target=target, loss=loss)  # fused MSE: keeps the backward coefficients
+        ctx.gs_sample_bwd(q, None, None, None, grads)           # dL_dphi = NULL: backward of that fused loss
         if world > 1:
             from paper_2607_01164_b200 import dist as gsdist
             gsdist.allreduce_grads(grads, flat)

@@ -132,7 +132,7 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->pt_key[0], &ctx->pt_key[1],
-                     &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters};
+                     &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
@@ -156,6 +156,7 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->have_pre = false;
     ctx->accel_kind = -1;
+    ctx->fused_pack = false;
     const size_t n = g->n ? g->n : 1;
     CK(ctx->rec.reserve(n * 64), "alloc records");
     CK(ctx->aabb.reserve(n * 24), "alloc aabb");
@@ -184,6 +185,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     if (st != GS_OK) return st;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->accel_kind = -1;
+    ctx->fused_pack = false;
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
     Stage stage(ctx, GS_PROF_BUILD);
@@ -307,8 +309,15 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     if (ctx->P > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "phi and I must be given");
     if (ctx->P > 0 && !target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
-    FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr};
-    return run_fwd(ctx, o);
+    FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr, nullptr};
+    ctx->fused_pack = false;
+    if (target && ctx->P > 0) {  // keep the backward coefficients of the fused MSE for gs_sample_bwd(dL_dphi = NULL)
+        CK(ctx->misc.reserve(ctx->P * 16), "alloc sample pack");
+        o.pack = ctx->misc.as<float4>();
+    }
+    st = run_fwd(ctx, o);
+    if (st == GS_OK && o.pack) ctx->fused_pack = true;
+    return st;
 }
 
 gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi, const float *dL_dI,
@@ -318,17 +327,21 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     if (st != GS_OK) return st;
     if (!out || (ctx->N > 0 && (!out->dmean || !out->dscale || !out->dquat || !out->dopacity || !out->dscalar)))
         return fail(ctx, GS_ERR_INVALID_ARG, "gradient outputs must be given");
-    if (ctx->P > 0 && (!phi || !I || !dL_dphi)) return fail(ctx, GS_ERR_INVALID_ARG, "phi, I and dL_dphi must be given");
+    const bool fused = dL_dphi == nullptr;
+    if (fused && ctx->P > 0 && (!ctx->fused_pack || dL_dI))
+        return fail(ctx, GS_ERR_STATE, "dL_dphi = NULL needs a preceding gs_sample_fwd with a target on the same accel (and dL_dI = NULL)");
+    if (!fused && ctx->P > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "phi and I must be given with dL_dphi");
     if (ctx->N > 0 && ((uintptr_t)out->dquat & 15)) return fail(ctx, GS_ERR_INVALID_ARG, "dquat must be 16-byte aligned");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
     if (N == 0) return GS_OK;
     CK(ctx->gacc.reserve((size_t)N * GACC * 4), "alloc gradient accumulator");
-    BwdIn in{phi, I, dL_dphi, dL_dI, target};
+    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused ? ctx->misc.as<float4>() : nullptr};
     if (ctx->accel_kind == GS_QUERY_GRID) {
-        CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc sample pack");
-        {
+        if (!fused) {
+            ctx->fused_pack = false;  // misc is overwritten with the caller's coefficients
+            CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc sample pack");
             Stage stage(ctx, GS_PROF_BWD_PACK);
             CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
         }
@@ -395,13 +408,13 @@ gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, u
     gs_status st = check_ready(ctx, q, "gs_debug_point_sets before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
-    CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc scratch");
+    CK(ctx->dbg.reserve((ctx->P ? ctx->P : 1) * 8), "alloc scratch");
     unsigned long long *ctr = ctx->counters.as<unsigned long long>() + 2;
     CK(cudaMemsetAsync(ctr, 0, 16, ctx->stream), "memset");
-    float *phi = ctx->misc.as<float>();
+    float *phi = ctx->dbg.as<float>();
     float *I = phi + (ctx->P ? ctx->P : 1);
     FwdOut o{nullptr, phi, I, nullptr, nullptr, nullptr, count, reinterpret_cast<unsigned long long *>(hash_sum),
-             reinterpret_cast<unsigned long long *>(hash_xor), ctr};
+             reinterpret_cast<unsigned long long *>(hash_xor), ctr, nullptr};
     st = run_fwd(ctx, o);
     if (st != GS_OK) return st;
     CK(cudaStreamSynchronize(ctx->stream), "sync");
@@ -465,7 +478,7 @@ gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom
     cudaStream_t s = ctx->stream;
     const size_t N = gh->n, n1 = N ? N : 1, p1 = P ? P : 1;
     // staging layout: 0 mean 1 scale 2 quat 3 opacity 4 scalar 5 xyz 6 target 7 phi 8 I 9 dL_dphi 10 loss 11.. grads
-    const size_t sizes[16] = {n1 * 12, n1 * 12, n1 * 16, n1 * 4, n1 * 4, p1 * 12, p1 * 4, p1 * 4, p1 * 4, p1 * 4, 8,
+    const size_t sizes[16] = {n1 * 12, n1 * 12, n1 * 16, n1 * 4, n1 * 4, qh->kind == GS_QUERY_POINTS ? p1 * 12 : 4, p1 * 4, p1 * 4, p1 * 4, 4, 8,
                               n1 * 12, n1 * 12, n1 * 16, n1 * 4, n1 * 8};
     for (int k = 0; k < 16; k++) CK(ctx->h2d[k].reserve(sizes[k]), "alloc staging");
     const void *src[5] = {gh->mean, gh->scale, gh->quat, gh->opacity, gh->scalar};
@@ -482,11 +495,11 @@ gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom
                      ctx->h2d[4].as<float>()};
     if ((st = gs_preprocess(ctx, &gdv, dom, tau)) != GS_OK) return st;
     if ((st = gs_build_accel(ctx, &q)) != GS_OK) return st;
-    float *phi = ctx->h2d[7].as<float>(), *I = ctx->h2d[8].as<float>(), *dphi = ctx->h2d[9].as<float>();
-    if ((st = gs_sample_fwd(ctx, &q, ctx->h2d[6].as<float>(), phi, I, ctx->h2d[10].as<double>(), dphi, nullptr)) != GS_OK) return st;
+    float *phi = ctx->h2d[7].as<float>(), *I = ctx->h2d[8].as<float>();
+    if ((st = gs_sample_fwd(ctx, &q, ctx->h2d[6].as<float>(), phi, I, ctx->h2d[10].as<double>(), nullptr, nullptr)) != GS_OK) return st;
     gs_grads gdev{ctx->h2d[11].as<float>(), ctx->h2d[12].as<float>(), ctx->h2d[13].as<float>(), ctx->h2d[14].as<float>(),
                   ctx->h2d[15].as<float>(), ctx->h2d[15].as<float>() + n1};
-    if ((st = gs_sample_bwd(ctx, &q, phi, I, dphi, nullptr, ctx->h2d[6].as<float>(), &gdev)) != GS_OK) return st;
+    if ((st = gs_sample_bwd(ctx, &q, nullptr, nullptr, nullptr, nullptr, nullptr, &gdev)) != GS_OK) return st;  // fused MSE backward
     if (phi_host && P) CK(cudaMemcpyAsync(phi_host, phi, P * 4, cudaMemcpyDeviceToHost, s), "D2H phi");
     if (I_host && P) CK(cudaMemcpyAsync(I_host, I, P * 4, cudaMemcpyDeviceToHost, s), "D2H I");
     CK(cudaMemcpyAsync(loss_host, ctx->h2d[10].p, 8, cudaMemcpyDeviceToHost, s), "D2H loss");

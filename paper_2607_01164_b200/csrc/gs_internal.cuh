@@ -79,7 +79,8 @@ struct gs_ctx {
     int pt_sel = 0;
     bool have_pt_order = false;
     // ---- scratch
-    gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters;
+    gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters, dbg;
+    bool fused_pack = false;  // misc holds the coefficients written by the last gs_sample_fwd with a target
     gs::DevBuf h2d[16];  // staging for gs_step_host
     // ---- measurement (gs_profile_*)
     bool prof = false;
@@ -114,9 +115,11 @@ struct FwdOut {
     const float *target; float *phi; float *I; double *loss; float *dL_dphi; float *sample_err;
     uint32_t *set_count; unsigned long long *set_sum; unsigned long long *set_xor;   // debug sets (nullable)
     unsigned long long *counters;                                                   // [2] tested, hits (nullable)
+    float4 *pack;  // nullable: per-sample backward coefficients (alpha, beta, eps, -) of the fused MSE loss
 };
 struct BwdIn {
     const float *phi; const float *I; const float *dL_dphi; const float *dL_dI; const float *target;
+    const float4 *pack;  // non-null: coefficients already packed by the forward (fused MSE); the other fields are unused
 };
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,

@@ -86,14 +86,15 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
         const int X = 2 * (clo[0] + (int)(code & 1023u)), Y = 2 * (clo[1] + (int)((code >> 10) & 1023u)), Z = 2 * (clo[2] + (int)(code >> 20));
         const float nanv = __int_as_float(0x7fc00000);
         float dx[2], dy[2], dz[2];
+        bool okx[2], oky[2], okz[2];
 #pragma unroll
         for (int d = 0; d < 2; d++) {  // canonical positions (D6); voxels outside the batch (or an idle lane) become NaN
-            const bool okx = on && X + d >= first[0] && X + d <= last[0];
-            const bool oky = Y + d >= first[1] && Y + d <= last[1];
-            const bool okz = Z + d >= first[2] && Z + d <= last[2];
-            dx[d] = __fsub_rn(okx ? voxel_centre(X + d, gd.spacing[0], gd.origin[0]) : nanv, ga.x);
-            dy[d] = __fsub_rn(oky ? voxel_centre(Y + d, gd.spacing[1], gd.origin[1]) : nanv, ga.y);
-            dz[d] = __fsub_rn(okz ? voxel_centre(Z + d, gd.spacing[2], gd.origin[2]) : nanv, ga.z);
+            okx[d] = on && X + d >= first[0] && X + d <= last[0];
+            oky[d] = Y + d >= first[1] && Y + d <= last[1];
+            okz[d] = Z + d >= first[2] && Z + d <= last[2];
+            dx[d] = __fsub_rn(okx[d] ? voxel_centre(X + d, gd.spacing[0], gd.origin[0]) : nanv, ga.x);
+            dy[d] = __fsub_rn(oky[d] ? voxel_centre(Y + d, gd.spacing[1], gd.origin[1]) : nanv, ga.y);
+            dz[d] = __fsub_rn(okz[d] ? voxel_centre(Z + d, gd.spacing[2], gd.origin[2]) : nanv, ga.z);
         }
         // canonical sequence (D4) with shared sub-expressions: u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx))
         float ab[3][4];
@@ -108,17 +109,21 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
         const uint32_t base = ((uint32_t)(Z - first[2]) * (uint32_t)gd.bdim[1] + (uint32_t)(Y - first[1])) * (uint32_t)gd.bdim[0] + (uint32_t)(X - first[0]);
 #pragma unroll
         for (int iz = 0; iz < 2; iz++) {
+            // the four coefficient loads of this z-slice are issued up front (no data dependence on the predicate),
+            // so their L1/L2 latency overlaps the arithmetic below instead of stalling each hit in turn
+            float4 s[4];
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+                const uint32_t c = base + ((uint32_t)iz * (uint32_t)gd.bdim[1] + (uint32_t)(v >> 1)) * (uint32_t)gd.bdim[0] + (uint32_t)(v & 1);
+                s[v] = (okx[v & 1] && oky[v >> 1] && okz[iz]) ? __ldg(pack + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
 #pragma unroll
             for (int v = 0; v < 4; v++) {
                 const float u0 = __fmaf_rn(gb.z, dz[iz], ab[0][v]);
                 const float u1 = __fmaf_rn(gc.z, dz[iz], ab[1][v]);
                 const float u2 = __fmaf_rn(gd4.z, dz[iz], ab[2][v]);
                 const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
-                if (qd <= r2) {
-                    const uint32_t c = base + ((uint32_t)iz * (uint32_t)gd.bdim[1] + (uint32_t)(v >> 1)) * (uint32_t)gd.bdim[0] + (uint32_t)(v & 1);
-                    const float4 s = __ldg(pack + c);
-                    bwd_accumulate(acc, s.x, s.y, s.z, ga.w, gb.w, gauss_weight(qd), u0, u1, u2);
-                }
+                if (qd <= r2) bwd_accumulate(acc, s[v].x, s[v].y, s[v].z, ga.w, gb.w, gauss_weight(qd), u0, u1, u2);
             }
         }
     };

@@ -14,7 +14,8 @@ def to_dev(torch, *arrays):
 class GpuRun:
     """One preprocess -> build -> fwd (fused MSE) -> bwd pass on the GPU; results as numpy arrays."""
 
-    def __init__(self, g, query_kind, query_obj, target, domain=None, dL_dI=None, presorted=False, tau=TAU):
+    def __init__(self, g, query_kind, query_obj, target, domain=None, dL_dI=None, presorted=False, tau=TAU, fused=False):
+        """fused=True: gs_sample_bwd(dL_dphi=NULL), i.e. the backward of the forward's fused MSE loss."""
         import torch
         from paper_2607_01164_b200 import api
         self.api = api
@@ -48,7 +49,11 @@ class GpuRun:
             for v in self.grads.values():
                 v.fill_(-7.0)
             self.dI = to_dev(torch, dL_dI)[0] if dL_dI is not None else None
-            ctx.gs_sample_bwd(self.q, self.phi, self.I, self.dphi, self.grads, dL_dI=self.dI, target=self.target)
+            if fused:
+                assert dL_dI is None
+                ctx.gs_sample_bwd(self.q, None, None, None, self.grads)
+            else:
+                ctx.gs_sample_bwd(self.q, self.phi, self.I, self.dphi, self.grads, dL_dI=self.dI, target=self.target)
         torch.cuda.synchronize()
 
     def np(self, t):

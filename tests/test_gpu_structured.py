@@ -163,3 +163,30 @@ def test_step_host_matches_device_path(oracle):
     for k, v in gr.items():
         assert rel_l2(grads[k], v) <= 1e-4, k
     ctx.close()
+
+
+def test_fused_mse_backward(oracle):
+    # gs_sample_bwd(dL_dphi = NULL): the backward of the forward's fused MSE loss (coefficients kept by the forward)
+    # gives the same gradients as the explicit dL_dphi form; misuse is a state error
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c4_gaussians(seed=11, n_grid=40, n=2500)
+    grid = inputs.Grid((40, 37, 26), (0.0, 0.0, 0.0), (1 / 40, 1 / 40, 1 / 40))
+    rng = np.random.default_rng(5)
+    target = rng.uniform(0, 1, grid.num_points).astype(np.float32)
+    xyz, fwd, loss, a, serr, gr = _oracle_all(oracle, g, grid, target)
+    run = GpuRun(g, "grid", grid, target, fused=True)
+    check_forward(run, fwd)
+    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+    check_grads(run, gr)
+    # a forward without target leaves no coefficients: the fused backward must refuse
+    ctx = run.ctx
+    ctx.gs_sample_fwd(run.q, run.phi, run.I)
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_sample_bwd(run.q, None, None, None, run.grads)
+    assert ei.value.status == api.GS_ERR_STATE
+    # dL_dI cannot be combined with the fused form
+    ctx.gs_sample_fwd(run.q, run.phi, run.I, target=run.target)
+    with pytest.raises(api.GsError) as ei:
+        ctx.gs_sample_bwd(run.q, None, None, None, run.grads, dL_dI=torch.zeros_like(run.phi))
+    assert ei.value.status == api.GS_ERR_STATE

@@ -59,6 +59,8 @@ def test_c3_reduced(oracle, presorted):
     assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
     np.testing.assert_allclose(run.np(run.serr), serr, atol=1e-5)
     check_grads(run, gr)
+    if not presorted:  # fused-MSE backward (dL_dphi = NULL) gives the same gradients
+        check_grads(GpuRun(g, "points", xyz, target, domain=dom, fused=True), gr)
 
 
 def test_c5_like_sparse_with_dI(oracle):
