@@ -87,6 +87,9 @@ gs_status validate_query(gs_ctx *ctx, const gs_query *q, GridDesc *gd, uint64_t 
             nb *= (uint64_t)q->brick_cnt[k];
         }
         if (nb >= (1ull << 31)) return fail(ctx, GS_ERR_INVALID_ARG, "grid: too many bricks in one batch");
+        for (int k = 0; k < 3; k++)  // the kernels index samples with 32 bits and cells with 10 bits per axis
+            if (gd->bdim[k] > 2048) return fail(ctx, GS_ERR_INVALID_ARG, "grid: a batch may span at most 2048 voxels per axis");
+        if (p >= (1ull << 32)) return fail(ctx, GS_ERR_INVALID_ARG, "grid: a batch may hold at most 2^32-1 samples");
         *P = p;
         return GS_OK;
     }
@@ -313,10 +316,10 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     ctx->fused_pack = false;
     if (target && ctx->P > 0) {  // keep the backward coefficients of the fused MSE for gs_sample_bwd(dL_dphi = NULL)
         CK(ctx->misc.reserve(ctx->P * 16), "alloc sample pack");
-        o.pack = ctx->misc.as<float4>();
+        o.pack2 = ctx->misc.as<float2>();
     }
     st = run_fwd(ctx, o);
-    if (st == GS_OK && o.pack) ctx->fused_pack = true;
+    if (st == GS_OK && o.pack2) ctx->fused_pack = true;
     return st;
 }
 
@@ -337,7 +340,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     const uint32_t N = ctx->N;
     if (N == 0) return GS_OK;
     CK(ctx->gacc.reserve((size_t)N * GACC * 4), "alloc gradient accumulator");
-    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused ? ctx->misc.as<float4>() : nullptr};
+    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused ? ctx->misc.as<float2>() : nullptr, 0.5f * (float)ctx->P};
     if (ctx->accel_kind == GS_QUERY_GRID) {
         if (!fused) {
             ctx->fused_pack = false;  // misc is overwritten with the caller's coefficients
@@ -346,7 +349,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
             CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
         }
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.as<float4>(), ctx->r2,
+        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
                            ctx->gacc.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
         uint32_t *ovf = ctx->counters.as<uint32_t>();

@@ -115,18 +115,19 @@ struct FwdOut {
     const float *target; float *phi; float *I; double *loss; float *dL_dphi; float *sample_err;
     uint32_t *set_count; unsigned long long *set_sum; unsigned long long *set_xor;   // debug sets (nullable)
     unsigned long long *counters;                                                   // [2] tested, hits (nullable)
-    float4 *pack;  // nullable: per-sample backward coefficients (alpha, beta, eps, -) of the fused MSE loss
+    float2 *pack2;  // nullable: per-sample backward coefficients (alpha, beta) of the fused MSE loss; eps = |alpha| P / 2
 };
 struct BwdIn {
     const float *phi; const float *I; const float *dL_dphi; const float *dL_dI; const float *target;
-    const float4 *pack;  // non-null: coefficients already packed by the forward (fused MSE); the other fields are unused
+    const float2 *pack2;  // non-null: (alpha, beta) already written by the forward (fused MSE); the other fields are unused
+    float eps_scale;      // with pack2: eps = |alpha| * eps_scale  (= P / 2 for the mean-squared error)
 };
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
-cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
-                            float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
+cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
+                            float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
                             cudaStream_t s);

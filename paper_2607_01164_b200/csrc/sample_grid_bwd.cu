@@ -1,14 +1,23 @@
 // sample_grid_bwd.cu -- structured backward (S7; section 4.1.4, in the warp-per-Gaussian form of
 // section 5.1.2 PAPER.md:196 applied to a grid, where the "traversal" is index arithmetic).
 //
-// One warp per Gaussian, no atomics: the warp enumerates the 2x2x2-voxel CELLS of the Gaussian's
-// AABB, culls them with the conservative whitened-space bound (same bound as the forward),
-// compacts the surviving cells through a small shared-memory queue so that all 32 lanes stay busy,
-// and evaluates 8 voxels per lane with shared canonical sub-expressions.  The weights are
-// recomputed (nothing is stored by the forward); each lane keeps the 12 partial sums in registers
-// and one transposing-butterfly warp reduction at the end writes the accumulator row.
+// One warp per Gaussian, no atomics.  The warp
+//   1. enumerates the ROWS (y, z) of 2x2x2-voxel cells of the Gaussian's AABB, one row per lane, and
+//      solves the conservative whitened-space cull bound for the row in closed form: the cells of a
+//      row that can hold a hit form an interval [lo, hi] around the row's closest approach;
+//   2. pushes the surviving cells through a shared-memory ring (warp scan of the interval lengths)
+//      so that every evaluation round has 32 busy lanes;
+//   3. evaluates one cell (8 voxels) per lane with the canonical predicate (shared sub-expressions),
+//      recomputing the weights (nothing is stored by the forward) and keeping the 12 partial sums
+//      in registers;
+//   4. finishes with one transposing butterfly and writes the 64-byte accumulator row.
 // Gaussians are processed in the Morton order of their central brick so that the per-sample
 // coefficients of neighbouring Gaussians stay in L1/L2.
+//
+// Per-sample coefficients: PACK2 = float2 (alpha, beta) written by the fused-MSE forward, where the error
+// share is eps = |alpha| * eps_scale; otherwise float4 (alpha, beta, eps, -) written by k_pack_samples.
+#include <type_traits>
+
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
 
@@ -32,27 +41,41 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 }
 
 constexpr int BWD_WARPS = 4;
-constexpr int GPW = 1;    // Gaussians per warp (consecutive in the order list); 8 measured slower on C2 (0.84 vs 0.73 ms)
-constexpr int QCAP = 64;  // per-warp queue of surviving cells (power of two, >= 2 * 32)
+constexpr int QCAP = 512;  // per-warp ring of surviving cells (power of two, >= 31 + 32 * SLICE)
+constexpr int SLICE = 8;   // cells of its interval a lane pushes per pass
 
+// The backward contribution of one hit with the weight w factored out of the sums (applied once after the
+// reduction):  gamma = alpha v + beta,  g = gamma G:
+//   acc0 += alpha G (dv / w) | acc1 += g (dw) | acc2..4 += g u (U / w) | acc5..10 += g u u^T (W / w) | acc11 += eps G (E / w)
+__device__ __forceinline__ void bwd_hit(float (&acc)[16], float alpha, float beta, float eps, float v, float G, float u0, float u1,
+                                        float u2) {
+    const float gamma = fmaf(alpha, v, beta);
+    const float g = gamma * G;
+    acc[0] = fmaf(alpha, G, acc[0]);
+    acc[1] += g;
+    const float t0 = g * u0, t1 = g * u1, t2 = g * u2;
+    acc[2] += t0; acc[3] += t1; acc[4] += t2;
+    acc[5] = fmaf(t0, u0, acc[5]); acc[6] = fmaf(t0, u1, acc[6]); acc[7] = fmaf(t0, u2, acc[7]);
+    acc[8] = fmaf(t1, u1, acc[8]); acc[9] = fmaf(t1, u2, acc[9]); acc[10] = fmaf(t2, u2, acc[10]);
+    acc[11] = fmaf(eps, G, acc[11]);
+}
+
+template <bool PACK2>
 __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__restrict__ rec, const float *__restrict__ aabb, uint32_t N,
-                                                              GridDesc gd, const float4 *__restrict__ pack, float r2,
+                                                              GridDesc gd, const void *__restrict__ pack_, float r2, float eps_scale,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
                                                               uint32_t M) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
-    // warp w processes the w-th Gaussian of the brick-ordered list of the M Gaussians that touch the batch
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // A CTA owns BWD_WARPS * GPW consecutive Gaussians of the order list (one neighbourhood of the grid, so
-    // that its per-sample coefficients are shared through this SM's L1); the warps interleave over them.
-    for (int rep = 0; rep < GPW; rep++) {
-    const uint32_t w = blockIdx.x * (BWD_WARPS * GPW) + rep * BWD_WARPS + warp;
+    // warp w processes the w-th Gaussian of the brick-ordered list of the M Gaussians that touch the batch
+    const uint32_t w = blockIdx.x * BWD_WARPS + warp;
     if (w >= M) return;  // whole warps leave; no block-wide barrier is used below
     const uint32_t i = order[w];
     const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
                  gd4 = __ldg(rec + 3 * (size_t)N + i);
     // voxel index box of the AABB inside the batch (conservative; the predicate decides), then its cells
     int clo[3], nc[3], first[3], last[3];
-    bool empty = false;
+    bool empty = false, edge = false;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         const float inv_sp = 1.0f / gd.spacing[k];
@@ -66,8 +89,11 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
         const int lo = (int)fl, hi = (int)fh;
         clo[k] = lo >> 1;
         nc[k] = (hi >> 1) - clo[k] + 1;
+        // first[k] is a multiple of 8, so a cell can only stick out of the batch at the upper end (odd extent)
+        edge |= 2 * (clo[k] + nc[k]) - 1 > last[k];
     }
-    if (empty) continue;  // the accumulator row stays zero (memset by the launcher)
+    if (empty) return;  // the accumulator row stays zero (memset by the launcher)
+    edge |= (gd.bdim[0] & 1) != 0;  // x-pairs of coefficients are 16-byte aligned only for an even x extent
 
     // cull bound (not canonical): |M(p - mu)| >= |M(cc - mu)| - rho for every voxel p of a cell with centre cc
     const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
@@ -80,21 +106,57 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
     float acc[16];
 #pragma unroll
     for (int k = 0; k < 16; k++) acc[k] = 0.f;
+    const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
 
-    // evaluate one cell per lane: (cxi, cyi, czi) = cell coordinates relative to clo
-    auto process = [&](uint32_t code, bool on) {
+    // evaluate one cell per lane: code = cell coordinates relative to clo (x | y << 10 | z << 20).
+    // EDGE = some cell of this Gaussian may stick out of the batch: voxels outside become NaN positions.
+    auto process = [&](uint32_t code, bool on, auto edge_tag) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
         const int X = 2 * (clo[0] + (int)(code & 1023u)), Y = 2 * (clo[1] + (int)((code >> 10) & 1023u)), Z = 2 * (clo[2] + (int)(code >> 20));
-        const float nanv = __int_as_float(0x7fc00000);
-        float dx[2], dy[2], dz[2];
+        // 32-bit sample index (P < 2^32) of the cell's first voxel
+        const uint32_t base = ((uint32_t)(Z - first[2]) * bdy + (uint32_t)(Y - first[1])) * bdx + (uint32_t)(X - first[0]);
+        // per-sample coefficients of the 8 voxels: issued up front (no data dependence on the predicate), so their
+        // L1/L2 latency overlaps the arithmetic below
+        float al[8], be[8], ep[8];
         bool okx[2], oky[2], okz[2];
 #pragma unroll
+        for (int d = 0; d < 2; d++) {
+            okx[d] = !EDGE || (on && X + d <= last[0]);
+            oky[d] = !EDGE || Y + d <= last[1];
+            okz[d] = !EDGE || Z + d <= last[2];
+        }
+        if (!EDGE && PACK2) {
+            const float2 *p2 = reinterpret_cast<const float2 *>(pack_);
+#pragma unroll
+            for (int r = 0; r < 4; r++) {  // (y, z) rows of the cell: one 16-byte load per x-pair
+                const uint32_t c = base + ((uint32_t)(r >> 1) * bdy + (uint32_t)(r & 1)) * bdx;
+                const float4 s = on ? __ldg(reinterpret_cast<const float4 *>(p2 + c)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                al[2 * r] = s.x; be[2 * r] = s.y; al[2 * r + 1] = s.z; be[2 * r + 1] = s.w;
+            }
+        } else {
+#pragma unroll
+            for (int v = 0; v < 8; v++) {
+                const uint32_t c = base + ((uint32_t)(v >> 2) * bdy + (uint32_t)((v >> 1) & 1)) * bdx + (uint32_t)(v & 1);
+                const bool ok = on && okx[v & 1] && oky[(v >> 1) & 1] && okz[v >> 2];
+                if (PACK2) {
+                    const float2 s = ok ? __ldg(reinterpret_cast<const float2 *>(pack_) + c) : make_float2(0.f, 0.f);
+                    al[v] = s.x; be[v] = s.y;
+                } else {
+                    const float4 s = ok ? __ldg(reinterpret_cast<const float4 *>(pack_) + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    al[v] = s.x; be[v] = s.y; ep[v] = s.z;
+                }
+            }
+        }
+        const float nanv = __int_as_float(0x7fc00000);
+        float dx[2], dy[2], dz[2];
+#pragma unroll
         for (int d = 0; d < 2; d++) {  // canonical positions (D6); voxels outside the batch (or an idle lane) become NaN
-            okx[d] = on && X + d >= first[0] && X + d <= last[0];
-            oky[d] = Y + d >= first[1] && Y + d <= last[1];
-            okz[d] = Z + d >= first[2] && Z + d <= last[2];
-            dx[d] = __fsub_rn(okx[d] ? voxel_centre(X + d, gd.spacing[0], gd.origin[0]) : nanv, ga.x);
-            dy[d] = __fsub_rn(oky[d] ? voxel_centre(Y + d, gd.spacing[1], gd.origin[1]) : nanv, ga.y);
-            dz[d] = __fsub_rn(okz[d] ? voxel_centre(Z + d, gd.spacing[2], gd.origin[2]) : nanv, ga.z);
+            const float px = voxel_centre(X + d, gd.spacing[0], gd.origin[0]);
+            const float py = voxel_centre(Y + d, gd.spacing[1], gd.origin[1]);
+            const float pz = voxel_centre(Z + d, gd.spacing[2], gd.origin[2]);
+            dx[d] = __fsub_rn((EDGE ? okx[d] : on) ? px : nanv, ga.x);
+            dy[d] = __fsub_rn(oky[d] ? py : nanv, ga.y);
+            dz[d] = __fsub_rn(okz[d] ? pz : nanv, ga.z);
         }
         // canonical sequence (D4) with shared sub-expressions: u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx))
         float ab[3][4];
@@ -105,72 +167,86 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
             ab[row][0] = __fmaf_rn(mr.y, dy[0], a0); ab[row][1] = __fmaf_rn(mr.y, dy[0], a1);
             ab[row][2] = __fmaf_rn(mr.y, dy[1], a0); ab[row][3] = __fmaf_rn(mr.y, dy[1], a1);
         }
-        // 32-bit sample index (P < 2^32); wraps for voxels outside the batch, which are never dereferenced
-        const uint32_t base = ((uint32_t)(Z - first[2]) * (uint32_t)gd.bdim[1] + (uint32_t)(Y - first[1])) * (uint32_t)gd.bdim[0] + (uint32_t)(X - first[0]);
 #pragma unroll
-        for (int iz = 0; iz < 2; iz++) {
-            // the four coefficient loads of this z-slice are issued up front (no data dependence on the predicate),
-            // so their L1/L2 latency overlaps the arithmetic below instead of stalling each hit in turn
-            float4 s[4];
-#pragma unroll
-            for (int v = 0; v < 4; v++) {
-                const uint32_t c = base + ((uint32_t)iz * (uint32_t)gd.bdim[1] + (uint32_t)(v >> 1)) * (uint32_t)gd.bdim[0] + (uint32_t)(v & 1);
-                s[v] = (okx[v & 1] && oky[v >> 1] && okz[iz]) ? __ldg(pack + c) : make_float4(0.f, 0.f, 0.f, 0.f);
-            }
-#pragma unroll
-            for (int v = 0; v < 4; v++) {
-                const float u0 = __fmaf_rn(gb.z, dz[iz], ab[0][v]);
-                const float u1 = __fmaf_rn(gc.z, dz[iz], ab[1][v]);
-                const float u2 = __fmaf_rn(gd4.z, dz[iz], ab[2][v]);
-                const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
-                if (qd <= r2) bwd_accumulate(acc, s[v].x, s[v].y, s[v].z, ga.w, gb.w, gauss_weight(qd), u0, u1, u2);
-            }
+        for (int v = 0; v < 8; v++) {  // v = x | y << 1 | z << 2
+            const float u0 = __fmaf_rn(gb.z, dz[v >> 2], ab[0][v & 3]);
+            const float u1 = __fmaf_rn(gc.z, dz[v >> 2], ab[1][v & 3]);
+            const float u2 = __fmaf_rn(gd4.z, dz[v >> 2], ab[2][v & 3]);
+            const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
+            if (qd <= r2) bwd_hit(acc, al[v], be[v], PACK2 ? fabsf(al[v]) : ep[v], gb.w, gauss_weight(qd), u0, u1, u2);
         }
     };
 
-    // enumerate the cells of the AABB, 32 per step; lane-private incremental (x, y, z) decode of the linear index
-    const int ncx = nc[0], ncy = nc[1], ncxy = ncx * ncy;
-    const int ncells = ncxy * nc[2];
-    int z = lane / ncxy, rem = lane - z * ncxy;
-    int y = rem / ncx, x = rem - y * ncx;
-    const int sz = 32 / ncxy, r32 = 32 - sz * ncxy, sy = r32 / ncx, sx = r32 - sy * ncx;
+    // ---- enumeration: lane = row (y, z) of cells.  Along the row the cell centre moves by 2 voxels in x:
+    // u(cx) = u_row + cx * e, e = M[:,0] * 2 sx.  |u(cx)|^2 <= thr  <=>  |cx - cx*| <= sqrt((thr - Dmin) / |e|^2),
+    // cx* = -(u_row . e) / |e|^2 the closest approach and Dmin = |u(cx*)|^2 (evaluated from the vector: no cancellation).
+    const int ncx = nc[0], ncy = nc[1];
+    const int nrows = ncy * nc[2];
+    const float sx2 = 2.f * gd.spacing[0];
+    const float e0 = gb.x * sx2, e1 = gc.x * sx2, e2 = gd4.x * sx2;
+    const float invA = 1.0f / (e0 * e0 + e1 * e1 + e2 * e2);
+    const float ccx0 = fmaf((float)(2 * clo[0] + 1), gd.spacing[0], gd.origin[0]) - ga.x;
     uint32_t *q = queue[warp];
     uint32_t head = 0, qn = 0;  // warp-uniform
-    for (int basek = 0; basek < ncells; basek += 32) {
-        const bool valid = basek + lane < ncells;
-        // centre of cell (x, y, z): voxels 2X, 2X+1 -> origin + (2X + 1) spacing
-        const float ccx = fmaf((float)(2 * (clo[0] + x) + 1), gd.spacing[0], gd.origin[0]) - ga.x;
+    auto drain = [&](uint32_t keep) {
+        while (qn > keep) {
+            const bool on = (uint32_t)lane < qn;
+            const uint32_t code = on ? q[(head + lane) & (QCAP - 1)] : 0u;
+            __syncwarp();
+            if (edge) process(code, on, std::true_type{});
+            else process(code, on, std::false_type{});
+            const uint32_t used = qn < 32u ? qn : 32u;
+            head = (head + used) & (QCAP - 1);
+            qn -= used;
+        }
+    };
+    for (int rbase = 0; rbase < nrows; rbase += 32) {
+        const int r = rbase + lane;
+        const int z = r / ncy, y = r - z * ncy;
         const float ccy = fmaf((float)(2 * (clo[1] + y) + 1), gd.spacing[1], gd.origin[1]) - ga.y;
         const float ccz = fmaf((float)(2 * (clo[2] + z) + 1), gd.spacing[2], gd.origin[2]) - ga.z;
-        const float u0 = gb.x * ccx + gb.y * ccy + gb.z * ccz;
-        const float u1 = gc.x * ccx + gc.y * ccy + gc.z * ccz;
-        const float u2 = gd4.x * ccx + gd4.y * ccy + gd4.z * ccz;
-        const bool pass = valid && (u0 * u0 + u1 * u1 + u2 * u2 <= thr);
-        const uint32_t bal = __ballot_sync(0xffffffffu, pass);
-        if (pass) q[(head + qn + __popc(bal & ((1u << lane) - 1u))) & (QCAP - 1)] = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
-        qn += __popc(bal);
-        __syncwarp();
-        if (qn >= 32) {
-            process(q[(head + lane) & (QCAP - 1)], true);
-            head = (head + 32) & (QCAP - 1);
-            qn -= 32;
-            __syncwarp();
+        const float u0 = gb.x * ccx0 + gb.y * ccy + gb.z * ccz;
+        const float u1 = gc.x * ccx0 + gc.y * ccy + gc.z * ccz;
+        const float u2 = gd4.x * ccx0 + gd4.y * ccy + gd4.z * ccz;
+        const float cs = -(u0 * e0 + u1 * e1 + u2 * e2) * invA;
+        const float v0 = fmaf(cs, e0, u0), v1 = fmaf(cs, e1, u1), v2 = fmaf(cs, e2, u2);
+        const float room = thr - (v0 * v0 + v1 * v1 + v2 * v2);
+        int x = 0, remaining = 0;
+        if (r < nrows && room >= 0.f) {
+            const float hw = sqrtf(room * invA) + 2e-3f + 1e-6f * fabsf(cs);
+            const float flo = fmaxf(ceilf(cs - hw), 0.f), fhi = fminf(floorf(cs + hw), (float)(ncx - 1));
+            if (flo <= fhi) { x = (int)flo; remaining = (int)fhi - x + 1; }
         }
-        x += sx; y += sy; z += sz;
-        if (x >= ncx) { x -= ncx; y++; }
-        if (y >= ncy) { y -= ncy; z++; }
+        while (__any_sync(0xffffffffu, remaining > 0)) {
+            const int take = remaining < SLICE ? remaining : SLICE;
+            int incl = take;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            const uint32_t total = (uint32_t)__shfl_sync(0xffffffffu, incl, 31);
+            const uint32_t pos = head + qn + (uint32_t)(incl - take);
+            const uint32_t code0 = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
+#pragma unroll
+            for (int j = 0; j < SLICE; j++)
+                if (j < take) q[(pos + j) & (QCAP - 1)] = code0 + j;
+            qn += total;
+            x += take;
+            remaining -= take;
+            __syncwarp();
+            drain(31u);
+        }
     }
-    if (qn) {
-        const bool on = (uint32_t)lane < qn;
-        process(on ? q[(head + lane) & (QCAP - 1)] : 0u, on);
-    }
+    drain(0u);
 
     warp_reduce16(acc, lane);
-    // lane 2c holds component c: 16 floats per Gaussian, written as one coalesced 64-byte row
-    const float val = __shfl_sync(0xffffffffu, acc[0], (lane & 15) * 2);
+    // lane 2c holds component c: 16 floats per Gaussian, written as one coalesced 64-byte row.  The weight w that
+    // bwd_hit leaves out multiplies every sum except dw; the error share also takes its scale.
+    float val = __shfl_sync(0xffffffffu, acc[0], (lane & 15) * 2);
+    if (lane != 1) val *= ga.w;
+    if (PACK2 && lane == 11) val *= eps_scale;
     if (lane < 16) gacc[(size_t)i * GACC + lane] = val;
-    __syncwarp();
-    }  // rep
 }
 
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s) {
@@ -180,12 +256,14 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
     return cudaGetLastError();
 }
 
-cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const float4 *pack, float r2,
-                            float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
+cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
+                            float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
     // untouched Gaussians keep a zero accumulator row
     cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC * sizeof(float), s);
     if (e != cudaSuccess || M == 0) return e;
-    k_grid_bwd<<<(M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW), BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, gacc, order, M);
+    const unsigned blocks = (M + BWD_WARPS - 1) / BWD_WARPS;
+    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, eps_scale, gacc, order, M);
+    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, eps_scale, gacc, order, M);
     count_launch();
     return cudaGetLastError();
 }

@@ -203,11 +203,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
                 res2 = fmaf(r0, r0, fmaf(r1, r1, res2));
                 if (o.dL_dphi) *reinterpret_cast<float2 *>(o.dL_dphi + c) = make_float2(cov[0] ? dscale * r0 : 0.f, cov[1] ? dscale * r1 : 0.f);
                 if (o.sample_err) *reinterpret_cast<float2 *>(o.sample_err + c) = make_float2(fabsf(r0), fabsf(r1));
-                if (o.pack) {  // backward coefficients of the fused MSE: alpha = a / I, beta = -alpha Phi, eps = |res| / I
-                    const float i0 = cov[0] ? 1.0f / Iv[0] : 0.f, i1 = cov[1] ? 1.0f / Iv[1] : 0.f;
-                    const float a0 = dscale * r0 * i0, a1 = dscale * r1 * i1;
-                    o.pack[c] = make_float4(a0, -a0 * ph[0], fabsf(r0) * i0, 0.f);
-                    o.pack[c + 1] = make_float4(a1, -a1 * ph[1], fabsf(r1) * i1, 0.f);
+                if (o.pack2) {  // backward coefficients of the fused MSE: alpha = a / I, beta = -alpha Phi (eps = |alpha| P / 2)
+                    const float a0 = cov[0] ? __fdividef(dscale * r0, Iv[0]) : 0.f, a1 = cov[1] ? __fdividef(dscale * r1, Iv[1]) : 0.f;
+                    *reinterpret_cast<float4 *>(o.pack2 + c) = make_float4(a0, -a0 * ph[0], a1, -a1 * ph[1]);
                 }
             }
         } else {
@@ -222,10 +220,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
                     res2 = fmaf(res, res, res2);
                     if (o.dL_dphi) o.dL_dphi[c + d] = cov[d] ? dscale * res : 0.f;
                     if (o.sample_err) o.sample_err[c + d] = fabsf(res);
-                    if (o.pack) {
-                        const float inv = cov[d] ? 1.0f / Iv[d] : 0.f;
-                        const float al = dscale * res * inv;
-                        o.pack[c + d] = make_float4(al, -al * ph[d], fabsf(res) * inv, 0.f);
+                    if (o.pack2) {
+                        const float al = cov[d] ? __fdividef(dscale * res, Iv[d]) : 0.f;
+                        o.pack2[c + d] = make_float2(al, -al * ph[d]);
                     }
                 }
                 if (SETS) {

@@ -102,10 +102,9 @@ __global__ void __launch_bounds__(PT_WARPS * 32) k_points_fwd(const float4 *__re
             res2 = res * res;
             if (o.dL_dphi) o.dL_dphi[c] = covered ? (float)(2.0 * invP) * res : 0.f;
             if (o.sample_err) o.sample_err[c] = fabsf(res);
-            if (o.pack) {
-                const float inv = covered ? 1.0f / I : 0.f;
-                const float al = (float)(2.0 * invP) * res * inv;
-                o.pack[c] = make_float4(al, -al * phi, fabsf(res) * inv, 0.f);
+            if (o.pack2) {
+                const float al = covered ? __fdividef((float)(2.0 * invP) * res, I) : 0.f;
+                o.pack2[c] = make_float2(al, -al * phi);
             }
         }
         if (SETS) {
@@ -147,9 +146,9 @@ __global__ void __launch_bounds__(PT_WARPS * 32) k_points_bwd(const float4 *__re
     const float px = active ? xyz[3 * c] : nanv, py = active ? xyz[3 * c + 1] : nanv, pz = active ? xyz[3 * c + 2] : nanv;
     // per-sample coefficients: alpha = covered ? a/I : 0, beta = b - alpha Phi, eps = covered ? |Phi - t|/I : 0
     float alpha = 0.f, beta = 0.f, eps = 0.f;
-    if (active && in.pack) {
-        const float4 s = __ldg(in.pack + c);
-        alpha = s.x; beta = s.y; eps = s.z;
+    if (active && in.pack2) {  // fused MSE: eps = |res| / I = |alpha| * P / 2
+        const float2 s = __ldg(in.pack2 + c);
+        alpha = s.x; beta = s.y; eps = fabsf(s.x) * in.eps_scale;
     } else if (active) {
         const float Ic = in.I[c], ph = in.phi[c];
         const bool covered = Ic > tau;
