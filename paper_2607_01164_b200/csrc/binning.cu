@@ -45,9 +45,17 @@ __device__ __forceinline__ uint32_t spread3(uint32_t v) {  // 10 bits -> every t
 // Also emits the processing order key of the backward pass: Morton code of the Gaussian's central
 // brick (performance only: neighbouring Gaussians are processed together so their voxel data stays
 // in L1/L2); Gaussians that touch no brick of the batch get `untouched_key` and sort to the end.
-__global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
-                                                      uint32_t *__restrict__ count, unsigned long long *__restrict__ total,
-                                                      uint32_t *__restrict__ okey, uint32_t *__restrict__ oval, uint32_t untouched_key) {
+//
+// And the per-Gaussian constants of the backward kernel (performance only, nothing canonical): the box of
+// 2x2x2-voxel cells that covers the AABB inside the batch, the whitened-space cull threshold of a cell and
+// 1 / |e|^2 for the closed-form row intervals (sample_grid_bwd.cu):
+//   setup[2 i]     = (clo.x, clo.y, clo.z, flags: 1 = touches no voxel of the batch, 2 = a cell sticks out of the batch)
+//   setup[2 i + 1] = (ncx | ncy << 11 | ncz << 22, thr, invA, -)
+__global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, const float4 *__restrict__ rec, uint32_t N,
+                                                      GridDesc gd, float rcut, uint32_t *__restrict__ count,
+                                                      unsigned long long *__restrict__ total, uint32_t *__restrict__ okey,
+                                                      uint32_t *__restrict__ oval, uint32_t untouched_key,
+                                                      float4 *__restrict__ setup) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t c = 0;
     if (i < N) {
@@ -69,6 +77,37 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         }
         okey[i] = key;
         oval[i] = i;
+        // ---- backward setup
+        int clo[3], nc[3];
+        bool empty = false, edge = false;
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const float inv_sp = 1.0f / gd.spacing[k];
+            const float tl = (b6[k] - gd.origin[k]) * inv_sp - 0.5f;
+            const float th = (b6[3 + k] - gd.origin[k]) * inv_sp - 0.5f;
+            const int first = BRICK * gd.brick_lo[k], last = BRICK * gd.brick_lo[k] + gd.bdim[k] - 1;
+            const float fl = fmaxf(ceilf(tl - (1e-3f + 4e-7f * fabsf(tl))), (float)first);
+            const float fh = fminf(floorf(th + (1e-3f + 4e-7f * fabsf(th))), (float)last);
+            empty |= !(fl <= fh);  // also true for the empty (+inf,-inf) box of an invalid Gaussian
+            const int lo = empty ? 0 : (int)fl, hi = empty ? 0 : (int)fh;
+            clo[k] = lo >> 1;
+            nc[k] = (hi >> 1) - clo[k] + 1;
+            // `first` is a multiple of 8, so a cell can only stick out of the batch at the upper end (odd extent)
+            edge |= 2 * (clo[k] + nc[k]) - 1 > last;
+        }
+        // cull bound: |M(p - mu)| >= |M(cc - mu)| - rho for every voxel p of a cell with centre cc
+        const float4 gb = rec[(size_t)N + i], gc = rec[2 * (size_t)N + i], gd4 = rec[3 * (size_t)N + i];
+        const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
+        const float q0 = fabsf(gb.x) * hx + fabsf(gb.y) * hy + fabsf(gb.z) * hz;
+        const float q1 = fabsf(gc.x) * hx + fabsf(gc.y) * hy + fabsf(gc.z) * hz;
+        const float q2 = fabsf(gd4.x) * hx + fabsf(gd4.y) * hy + fabsf(gd4.z) * hz;
+        const float reach = rcut + sqrtf(q0 * q0 + q1 * q1 + q2 * q2);
+        const float sx2 = 2.f * gd.spacing[0];
+        const float e0 = gb.x * sx2, e1 = gc.x * sx2, e2 = gd4.x * sx2;
+        setup[2 * (size_t)i] = make_float4(__int_as_float(clo[0]), __int_as_float(clo[1]), __int_as_float(clo[2]),
+                                           __uint_as_float((empty ? 1u : 0u) | (edge ? 2u : 0u)));
+        setup[2 * (size_t)i + 1] = make_float4(__uint_as_float((uint32_t)nc[0] | ((uint32_t)nc[1] << 11) | ((uint32_t)nc[2] << 22)),
+                                               reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
     }
     // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
     unsigned long long s = c, m = c ? 1ull : 0ull;
@@ -122,11 +161,12 @@ __global__ void __launch_bounds__(256) k_brick_start(const uint32_t *__restrict_
     for (uint32_t b = prev; b <= cur; b++) start[b] = t;
 }
 
-cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd, uint32_t *count, unsigned long long *total,
-                               uint32_t *okey, uint32_t *oval, uint32_t untouched_key, cudaStream_t s) {
+cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
+                               unsigned long long *total, uint32_t *okey, uint32_t *oval, uint32_t untouched_key, float4 *setup,
+                               cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(total, 0, 2 * sizeof(unsigned long long), s);
     if (e != cudaSuccess || N == 0) return e;
-    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, count, total, okey, oval, untouched_key); count_launch();
+    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, rec, N, gd, rcut, count, total, okey, oval, untouched_key, setup); count_launch();
     return cudaGetLastError();
 }
 

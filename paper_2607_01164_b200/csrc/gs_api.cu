@@ -132,7 +132,7 @@ void gs_destroy(gs_ctx *ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->boffset, &ctx->pair_key[0], &ctx->pair_key[1],
-                     &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->leaf_key[0], &ctx->leaf_key[1],
+                     &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg};
@@ -208,8 +208,10 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         int axis_bits = 1;
         for (int k = 0; k < 3; k++) axis_bits = bits_for((uint64_t)gd.brick_cnt[k]) > axis_bits ? bits_for((uint64_t)gd.brick_cnt[k]) : axis_bits;
         const uint32_t untouched_key = 1u << (3 * axis_bits);
-        CK(launch_brick_count(ctx->aabb.as<float>(), N, gd, ctx->bcount.as<uint32_t>(), total, ctx->leaf_key[0].as<uint32_t>(),
-                              ctx->leaf_val[0].as<uint32_t>(), untouched_key, s), "brick count");
+        CK(ctx->bwd_setup.reserve(n1 * 32), "alloc backward setup");
+        CK(launch_brick_count(ctx->aabb.as<float>(), ctx->rec.as<float4>(), N, gd, ctx->r, ctx->bcount.as<uint32_t>(), total,
+                              ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_val[0].as<uint32_t>(), untouched_key,
+                              ctx->bwd_setup.as<float4>(), s), "brick count");
         CK(exclusive_scan_u32(ctx->bcount.as<uint32_t>(), ctx->boffset.as<uint32_t>(), N, ctx->scan_tmp, s), "scan");
         unsigned long long T64[2] = {0, 0};
         CK(cudaMemcpyAsync(T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
@@ -349,7 +351,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
             CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
         }
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
+        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
                            ctx->gacc.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
         uint32_t *ovf = ctx->counters.as<uint32_t>();

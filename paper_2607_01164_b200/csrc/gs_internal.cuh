@@ -69,6 +69,7 @@ struct gs_ctx {
     gs::DevBuf pair_key[2], pair_val[2];
     int pair_sel = 0;
     gs::DevBuf brick_start;  // uint32 [nbricks+1]
+    gs::DevBuf bwd_setup;    // float4 [N][2]: per-Gaussian constants of the structured backward (k_brick_count)
     // ---- accel (points)
     uint64_t P = 0;
     gs::DevBuf leaf_key[2], leaf_val[2];
@@ -105,8 +106,9 @@ cudaError_t exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, DevB
 cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int bits, DevBuf &hist, DevBuf &tmp,
                              cudaStream_t s, int *result_sel);
 
-cudaError_t launch_brick_count(const float *aabb, uint32_t N, const GridDesc &gd, uint32_t *count, unsigned long long *total,
-                               uint32_t *okey, uint32_t *oval, uint32_t untouched_key, cudaStream_t s);
+cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
+                               unsigned long long *total, uint32_t *okey, uint32_t *oval, uint32_t untouched_key, float4 *setup,
+                               cudaStream_t s);
 cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
                               uint32_t *key, uint32_t *val, cudaStream_t s);
 cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks, uint32_t *start, cudaStream_t s);
@@ -126,7 +128,7 @@ struct BwdIn {
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
-cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
+cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
                             float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,

@@ -41,6 +41,8 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 }
 
 constexpr int BWD_WARPS = 4;
+constexpr int BWD_MINB = 6;  // resident CTAs per SM the register allocation must allow
+constexpr int GPW = 4;       // Gaussians per warp (consecutive in the order list)
 constexpr int QCAP = 512;  // per-warp ring of surviving cells (power of two, >= 31 + 32 * SLICE)
 constexpr int SLICE = 8;   // cells of its interval a lane pushes per pass
 
@@ -61,52 +63,47 @@ __device__ __forceinline__ void bwd_hit(float (&acc)[16], float alpha, float bet
 }
 
 template <bool PACK2>
-__global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__restrict__ rec, const float *__restrict__ aabb, uint32_t N,
+__global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
                                                               GridDesc gd, const void *__restrict__ pack_, float r2, float eps_scale,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
                                                               uint32_t M) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // warp w processes the w-th Gaussian of the brick-ordered list of the M Gaussians that touch the batch
-    const uint32_t w = blockIdx.x * BWD_WARPS + warp;
-    if (w >= M) return;  // whole warps leave; no block-wide barrier is used below
-    const uint32_t i = order[w];
-    const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
-                 gd4 = __ldg(rec + 3 * (size_t)N + i);
-    // voxel index box of the AABB inside the batch (conservative; the predicate decides), then its cells
-    int clo[3], nc[3], first[3], last[3];
-    bool empty = false, edge = false;
+    // a warp processes GPW consecutive Gaussians of the brick-ordered list of the M Gaussians that touch the batch
+    const uint32_t w0 = (blockIdx.x * BWD_WARPS + warp) * GPW;
+    if (w0 >= M) return;  // whole warps leave; no block-wide barrier is used below
+    const uint32_t my_id = (w0 + lane < M && lane < GPW) ? order[w0 + lane] : 0u;
+    const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
+    int first[3], last[3];
 #pragma unroll
     for (int k = 0; k < 3; k++) {
-        const float inv_sp = 1.0f / gd.spacing[k];
-        const float tl = (aabb[6 * (size_t)i + k] - gd.origin[k]) * inv_sp - 0.5f;
-        const float th = (aabb[6 * (size_t)i + 3 + k] - gd.origin[k]) * inv_sp - 0.5f;
         first[k] = BRICK * gd.brick_lo[k];
         last[k] = BRICK * gd.brick_lo[k] + gd.bdim[k] - 1;
-        const float fl = fmaxf(ceilf(tl - (1e-3f + 4e-7f * fabsf(tl))), (float)first[k]);
-        const float fh = fminf(floorf(th + (1e-3f + 4e-7f * fabsf(th))), (float)last[k]);
-        empty |= !(fl <= fh);  // also true for the empty (+inf,-inf) box of an invalid Gaussian
-        const int lo = (int)fl, hi = (int)fh;
-        clo[k] = lo >> 1;
-        nc[k] = (hi >> 1) - clo[k] + 1;
-        // first[k] is a multiple of 8, so a cell can only stick out of the batch at the upper end (odd extent)
-        edge |= 2 * (clo[k] + nc[k]) - 1 > last[k];
     }
-    if (empty) return;  // the accumulator row stays zero (memset by the launcher)
-    edge |= (gd.bdim[0] & 1) != 0;  // x-pairs of coefficients are 16-byte aligned only for an even x extent
+    const bool odd_x = (gd.bdim[0] & 1) != 0;  // x-pairs of coefficients are 16-byte aligned only for an even x extent
+    uint32_t *q = queue[warp];
 
-    // cull bound (not canonical): |M(p - mu)| >= |M(cc - mu)| - rho for every voxel p of a cell with centre cc
-    const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
-    const float q0 = fabsf(gb.x) * hx + fabsf(gb.y) * hy + fabsf(gb.z) * hz;
-    const float q1 = fabsf(gc.x) * hx + fabsf(gc.y) * hy + fabsf(gc.z) * hz;
-    const float q2 = fabsf(gd4.x) * hx + fabsf(gd4.y) * hy + fabsf(gd4.z) * hz;
-    const float reach = sqrtf(r2) + sqrtf(q0 * q0 + q1 * q1 + q2 * q2);
-    const float thr = reach * reach * 1.001953125f;
+    for (int rep = 0; rep < GPW && w0 + rep < M; rep++) {
+    const uint32_t i = __shfl_sync(0xffffffffu, my_id, rep);
+    const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
+                 gd4 = __ldg(rec + 3 * (size_t)N + i);
+    // cell box of the AABB inside the batch, cull threshold and 1 / |e|^2: precomputed per Gaussian (k_brick_count)
+    const float4 s0 = __ldg(setup + 2 * (size_t)i), s1 = __ldg(setup + 2 * (size_t)i + 1);
+    const int clo[3] = {__float_as_int(s0.x), __float_as_int(s0.y), __float_as_int(s0.z)};
+    const uint32_t flags = __float_as_uint(s0.w), ncp = __float_as_uint(s1.x);
+    if (flags & 1u) continue;  // empty: the accumulator row stays zero (memset by the launcher)
+    const bool edge = (flags & 2u) || odd_x;
+    const int ncx = (int)(ncp & 2047u), ncy = (int)((ncp >> 11) & 2047u), ncz = (int)(ncp >> 22);
+    const float thr = s1.y, invA = s1.z;
+    if (rep + 1 < GPW && w0 + rep + 1 < M) {  // pull the next Gaussian's records towards L1 while this one is processed
+        const uint32_t nx = __shfl_sync(0xffffffffu, my_id, rep + 1);
+        const void *pf = lane < 4 ? (const void *)(rec + (size_t)lane * N + nx) : (const void *)(setup + 2 * (size_t)nx);
+        if (lane < 5) asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
+    }
 
     float acc[16];
 #pragma unroll
     for (int k = 0; k < 16; k++) acc[k] = 0.f;
-    const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
 
     // evaluate one cell per lane: code = cell coordinates relative to clo (x | y << 10 | z << 20).
     // EDGE = some cell of this Gaussian may stick out of the batch: voxels outside become NaN positions.
@@ -180,18 +177,25 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
     // ---- enumeration: lane = row (y, z) of cells.  Along the row the cell centre moves by 2 voxels in x:
     // u(cx) = u_row + cx * e, e = M[:,0] * 2 sx.  |u(cx)|^2 <= thr  <=>  |cx - cx*| <= sqrt((thr - Dmin) / |e|^2),
     // cx* = -(u_row . e) / |e|^2 the closest approach and Dmin = |u(cx*)|^2 (evaluated from the vector: no cancellation).
-    const int ncx = nc[0], ncy = nc[1];
-    const int nrows = ncy * nc[2];
+    const int nrows = ncy * ncz;
     const float sx2 = 2.f * gd.spacing[0];
     const float e0 = gb.x * sx2, e1 = gc.x * sx2, e2 = gd4.x * sx2;
-    const float invA = 1.0f / (e0 * e0 + e1 * e1 + e2 * e2);
     const float ccx0 = fmaf((float)(2 * clo[0] + 1), gd.spacing[0], gd.origin[0]) - ga.x;
-    uint32_t *q = queue[warp];
     uint32_t head = 0, qn = 0;  // warp-uniform
     auto drain = [&](uint32_t keep) {
         while (qn > keep) {
             const bool on = (uint32_t)lane < qn;
             const uint32_t code = on ? q[(head + lane) & (QCAP - 1)] : 0u;
+            if (!edge && PACK2 && qn > 32u && (uint32_t)lane + 32u < qn) {
+                // pull the next round's coefficient rows towards L1 (no registers held)
+                const uint32_t c2 = q[(head + 32 + lane) & (QCAP - 1)];
+                const int X = 2 * (clo[0] + (int)(c2 & 1023u)), Y = 2 * (clo[1] + (int)((c2 >> 10) & 1023u)), Z = 2 * (clo[2] + (int)(c2 >> 20));
+                const uint32_t base = ((uint32_t)(Z - first[2]) * bdy + (uint32_t)(Y - first[1])) * bdx + (uint32_t)(X - first[0]);
+                const float2 *p2 = reinterpret_cast<const float2 *>(pack_);
+#pragma unroll
+                for (int r = 0; r < 4; r++)
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(p2 + base + ((uint32_t)(r >> 1) * bdy + (uint32_t)(r & 1)) * bdx));
+            }
             __syncwarp();
             if (edge) process(code, on, std::true_type{});
             else process(code, on, std::false_type{});
@@ -247,6 +251,8 @@ __global__ void __launch_bounds__(BWD_WARPS * 32) k_grid_bwd(const float4 *__res
     if (lane != 1) val *= ga.w;
     if (PACK2 && lane == 11) val *= eps_scale;
     if (lane < 16) gacc[(size_t)i * GACC + lane] = val;
+    __syncwarp();
+    }  // rep
 }
 
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s) {
@@ -256,14 +262,14 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
     return cudaGetLastError();
 }
 
-cudaError_t launch_grid_bwd(const float4 *rec, const float *aabb, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
+cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
                             float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
     // untouched Gaussians keep a zero accumulator row
     cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC * sizeof(float), s);
     if (e != cudaSuccess || M == 0) return e;
-    const unsigned blocks = (M + BWD_WARPS - 1) / BWD_WARPS;
-    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, eps_scale, gacc, order, M);
-    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, aabb, N, gd, pack, r2, eps_scale, gacc, order, M);
+    const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
+    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, eps_scale, gacc, order, M);
+    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, eps_scale, gacc, order, M);
     count_launch();
     return cudaGetLastError();
 }
