@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 }
 
 constexpr int BWD_WARPS = 4;
-constexpr int BWD_MINB = 6;  // resident CTAs per SM the register allocation must allow
+constexpr int BWD_MINB = 5;  // resident CTAs per SM the register allocation must allow
 constexpr int GPW = 4;       // Gaussians per warp (consecutive in the order list)
 constexpr int QCAP = 512;  // per-warp ring of surviving cells (power of two, >= 31 + 32 * SLICE)
 constexpr int SLICE = 8;   // cells of its interval a lane pushes per pass
@@ -186,16 +186,6 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
         while (qn > keep) {
             const bool on = (uint32_t)lane < qn;
             const uint32_t code = on ? q[(head + lane) & (QCAP - 1)] : 0u;
-            if (!edge && PACK2 && qn > 32u && (uint32_t)lane + 32u < qn) {
-                // pull the next round's coefficient rows towards L1 (no registers held)
-                const uint32_t c2 = q[(head + 32 + lane) & (QCAP - 1)];
-                const int X = 2 * (clo[0] + (int)(c2 & 1023u)), Y = 2 * (clo[1] + (int)((c2 >> 10) & 1023u)), Z = 2 * (clo[2] + (int)(c2 >> 20));
-                const uint32_t base = ((uint32_t)(Z - first[2]) * bdy + (uint32_t)(Y - first[1])) * bdx + (uint32_t)(X - first[0]);
-                const float2 *p2 = reinterpret_cast<const float2 *>(pack_);
-#pragma unroll
-                for (int r = 0; r < 4; r++)
-                    asm volatile("prefetch.global.L1 [%0];" ::"l"(p2 + base + ((uint32_t)(r >> 1) * bdy + (uint32_t)(r & 1)) * bdx));
-            }
             __syncwarp();
             if (edge) process(code, on, std::true_type{});
             else process(code, on, std::false_type{});
