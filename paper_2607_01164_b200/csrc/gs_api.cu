@@ -300,7 +300,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
         CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->rec.as<float4>(), ctx->N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, o,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->dom, ctx->tau, ctx->r2, ctx->r, o,
                              ovf, s), "points forward");
     }
     return GS_OK;
@@ -359,7 +359,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_points_bwd(ctx->rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, in,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->dom, ctx->tau, ctx->r2, ctx->r, in,
                              ctx->gacc.as<float>(), ovf, s), "points backward");
     }
     Stage stage(ctx, GS_PROF_FINALIZE);

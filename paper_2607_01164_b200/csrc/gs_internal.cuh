@@ -42,6 +42,37 @@ struct GridDesc {          // one batch of a structured grid (gs_query, GS_QUERY
     int nb_total[3];       // bricks of the whole grid per axis
 };
 
+// 30-bit Morton code of a position inside the domain box (D8): 10 bits per axis, x in the low bit,
+// q = (int) min(max((x - lo) * (1024 / (hi - lo)), 0), 1023) with the scale computed once on the host in fp32.
+struct MortonParams { float lo[3], scale[3]; };
+inline MortonParams morton_params(const gs_domain &dom) {
+    MortonParams mp;
+    for (int k = 0; k < 3; k++) {
+        mp.lo[k] = dom.lo[k];
+        mp.scale[k] = 1024.0f / (dom.hi[k] - dom.lo[k]);
+    }
+    return mp;
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t expand10(uint32_t v) {  // 10 bits -> every third bit
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+__device__ __forceinline__ uint32_t morton30(float x, float y, float z, const MortonParams &mp) {
+    const float tx = __fmul_rn(__fsub_rn(x, mp.lo[0]), mp.scale[0]);
+    const float ty = __fmul_rn(__fsub_rn(y, mp.lo[1]), mp.scale[1]);
+    const float tz = __fmul_rn(__fsub_rn(z, mp.lo[2]), mp.scale[2]);
+    const uint32_t qx = (uint32_t)(int)fminf(fmaxf(tx, 0.0f), 1023.0f);
+    const uint32_t qy = (uint32_t)(int)fminf(fmaxf(ty, 0.0f), 1023.0f);
+    const uint32_t qz = (uint32_t)(int)fminf(fmaxf(tz, 0.0f), 1023.0f);
+    return expand10(qx) | (expand10(qy) << 1) | (expand10(qz) << 2);
+}
+#endif
+
 }  // namespace gs
 
 struct gs_ctx {
@@ -140,10 +171,10 @@ cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *a
 cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, uint32_t N, int32_t *left, int32_t *right,
                         int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed, cudaStream_t s);
 cudaError_t launch_points_fwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, float tau, float r2, const FwdOut &o, uint32_t *overflow,
+                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const FwdOut &o, uint32_t *overflow,
                               cudaStream_t s);
 cudaError_t launch_points_bwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, float tau, float r2, const BwdIn &in, float *gacc,
+                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const BwdIn &in, float *gacc,
                               uint32_t *overflow, cudaStream_t s);
 
 }  // namespace gs

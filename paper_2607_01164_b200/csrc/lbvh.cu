@@ -10,17 +10,6 @@
 
 namespace gs {
 
-__device__ __forceinline__ uint32_t expand10(uint32_t v) {  // 10 bits -> every third bit
-    v &= 0x3ffu;
-    v = (v | (v << 16)) & 0x030000FFu;
-    v = (v | (v << 8)) & 0x0300F00Fu;
-    v = (v | (v << 4)) & 0x030C30C3u;
-    v = (v | (v << 2)) & 0x09249249u;
-    return v;
-}
-
-struct MortonParams { float lo[3], scale[3]; };
-
 __global__ void __launch_bounds__(256) k_morton(const float *__restrict__ xyz, int stride, int nan_is_invalid, size_t n, MortonParams mp,
                                                  uint32_t *__restrict__ codes, uint32_t *__restrict__ ids) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -31,13 +20,7 @@ __global__ void __launch_bounds__(256) k_morton(const float *__restrict__ xyz, i
         code = 1u << 30;  // invalid Gaussians sort to the end
     } else {
         // D8: q = (int) min(max((x - lo) * scale, 0), 1023), truncation
-        const float tx = __fmul_rn(__fsub_rn(x, mp.lo[0]), mp.scale[0]);
-        const float ty = __fmul_rn(__fsub_rn(y, mp.lo[1]), mp.scale[1]);
-        const float tz = __fmul_rn(__fsub_rn(z, mp.lo[2]), mp.scale[2]);
-        const uint32_t qx = (uint32_t)(int)fminf(fmaxf(tx, 0.0f), 1023.0f);
-        const uint32_t qy = (uint32_t)(int)fminf(fmaxf(ty, 0.0f), 1023.0f);
-        const uint32_t qz = (uint32_t)(int)fminf(fmaxf(tz, 0.0f), 1023.0f);
-        code = expand10(qx) | (expand10(qy) << 1) | (expand10(qz) << 2);
+        code = morton30(x, y, z, mp);
     }
     codes[i] = code;
     ids[i] = (uint32_t)i;
@@ -46,11 +29,7 @@ __global__ void __launch_bounds__(256) k_morton(const float *__restrict__ xyz, i
 cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *nan_invalid, size_t n, const gs_domain &dom,
                           uint32_t *codes, uint32_t *ids, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    MortonParams mp;
-    for (int k = 0; k < 3; k++) {
-        mp.lo[k] = dom.lo[k];
-        mp.scale[k] = 1024.0f / (dom.hi[k] - dom.lo[k]);
-    }
+    const MortonParams mp = morton_params(dom);
     k_morton<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(xyz, (int)stride_floats, nan_invalid != nullptr, n, mp, codes, ids); count_launch();
     return cudaGetLastError();
 }
