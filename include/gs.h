@@ -210,7 +210,9 @@ typedef enum {
     GS_PROF_BWD_PACK = 3,   /* per-sample coefficients (structured backward only)          */
     GS_PROF_BWD = 4,        /* S7: the backward sampling kernel                            */
     GS_PROF_FINALIZE = 5,   /* S8                                                          */
-    GS_PROF_STAGES = 6
+    GS_PROF_CULL = 6,       /* unstructured: per-packet LBVH traversal + cull lists (inside gs_build_accel;
+                               its time is ALSO part of GS_PROF_BUILD)                      */
+    GS_PROF_STAGES = 7
 } gs_prof_stage;
 gs_status gs_profile_enable(gs_ctx *ctx, int32_t on);
 gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uint64_t *launches_host);

@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read"]
-PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize"]
+PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
 class GsLibraryError(RuntimeError):

@@ -102,6 +102,11 @@ gs_status validate_query(gs_ctx *ctx, const gs_query *q, GridDesc *gd, uint64_t 
     return fail(ctx, GS_ERR_INVALID_ARG, "query kind");
 }
 
+CullLists cull_lists(gs_ctx *ctx) {
+    return CullLists{ctx->cull_ids.as<uint32_t>(), ctx->cull_link.as<uint32_t>(), ctx->cull_head.as<uint2>(),
+                     ctx->counters.as<uint32_t>() + 2, ctx->cull_cap};
+}
+
 int bits_for(uint64_t n) {  // bits needed to represent values in [0, n)
     int b = 0;
     while (b < 32 && (1ull << b) < n) b++;
@@ -134,7 +139,7 @@ void gs_destroy(gs_ctx *ctx) {
     DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->boffset, &ctx->pair_key[0], &ctx->pair_key[1],
                      &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
-                     &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->pt_key[0], &ctx->pt_key[1],
+                     &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
@@ -252,15 +257,17 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         CK(ctx->node_aabb.reserve(n * 24), "alloc nodes");
         CK(ctx->node_flag.reserve(n * 4), "alloc nodes");
         CK(ctx->bvh_nodes.reserve(n * 64), "alloc nodes");
+        CK(ctx->sorted_rec.reserve(n * 64), "alloc sorted records");
         // Morton codes of the means (record plane 0: mu.xyz, w; NaN marks an invalid Gaussian)
         CK(launch_morton(ctx->rec.as<float>(), 4, ctx->rec.as<float>(), N, ctx->dom, ctx->leaf_key[0].as<uint32_t>(),
                          ctx->leaf_val[0].as<uint32_t>(), s), "morton (gaussians)");
         uint32_t *keys[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
         uint32_t *vals[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
         CK(radix_sort_pairs(keys, vals, N, 31, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "morton sort (gaussians)");
-        CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), N, ctx->node_left.as<int32_t>(),
-                       ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(), ctx->leaf_parent.as<int32_t>(),
-                       ctx->node_aabb.as<float>(), ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), s), "lbvh");
+        CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), ctx->rec.as<float4>(), N,
+                       ctx->node_left.as<int32_t>(), ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(),
+                       ctx->leaf_parent.as<int32_t>(), ctx->node_aabb.as<float>(),
+                       ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), ctx->sorted_rec.as<float4>(), s), "lbvh");
         // coherence sort of the queries
         ctx->have_pt_order = false;
         if (!q->presorted && P > 0) {
@@ -274,6 +281,39 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
             uint32_t *pv[2] = {ctx->pt_val[0].as<uint32_t>(), ctx->pt_val[1].as<uint32_t>()};
             CK(radix_sort_pairs(pk, pv, P, 30, ctx->sort_hist, ctx->scan_tmp, s, &ctx->pt_sel), "morton sort (points)");
             ctx->have_pt_order = true;
+        }
+        // per-packet cull lists (the LBVH traversal; shared by the forward and the backward of this step).  The pool of
+        // list chunks grows on demand: the kernel counts the chunks it needs, the host reads that count back (the one
+        // device->host crossing of the unstructured path, like T of the structured path) and repeats the pass if it
+        // did not fit.
+        if (P > 0) {
+            Stage cull_stage(ctx, GS_PROF_CULL);
+            const uint64_t packets = (P + 31) / 32;
+            CK(ctx->cull_head.reserve(packets * 8), "alloc cull heads");
+            if (ctx->cull_cap == 0) {
+                const uint64_t guess = packets * 8 + 1024;   // 256 Gaussians per point-packet; grown below when exceeded
+                CK(ctx->cull_ids.reserve(guess * 128), "alloc cull pool");
+                CK(ctx->cull_link.reserve(guess * 4), "alloc cull pool");
+                ctx->cull_cap = (uint32_t)guess;
+            }
+            uint32_t *ovf = ctx->counters.as<uint32_t>();
+            for (int attempt = 0;; attempt++) {
+                CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
+                CK(launch_points_cull(ctx->sorted_rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), q->xyz,
+                                      ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->dom, ctx->r,
+                                      cull_lists(ctx), ovf, s), "points cull");
+                uint32_t host[3] = {0, 0, 0};   // [0] stack overflow flag, [2] chunks requested
+                CK(cudaMemcpyAsync(host, ctx->counters.p, 12, cudaMemcpyDeviceToHost, s), "read cull counters");
+                CK(cudaStreamSynchronize(s), "sync");
+                if (host[0]) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
+                if (host[2] <= ctx->cull_cap) break;
+                if (attempt >= 2) return fail(ctx, GS_ERR_OVERFLOW, "cull list pool did not converge");
+                const uint64_t want = (uint64_t)host[2] + host[2] / 8 + 1024;
+                if (want >= 0xffffffffull) return fail(ctx, GS_ERR_OVERFLOW, "cull lists exceed 2^32 chunks");
+                CK(ctx->cull_ids.reserve(want * 128), "alloc cull pool");
+                CK(ctx->cull_link.reserve(want * 4), "alloc cull pool");
+                ctx->cull_cap = (uint32_t)want;
+            }
         }
     }
     ctx->P = P;
@@ -296,12 +336,10 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_val[ctx->pair_sel].as<uint32_t>(),
                            ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, s), "grid forward");
     } else {
-        uint32_t *ovf = ctx->counters.as<uint32_t>();
-        CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
         Stage stage(ctx, GS_PROF_FWD);
-        CK(launch_points_fwd(ctx->rec.as<float4>(), ctx->N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->dom, ctx->tau, ctx->r2, ctx->r, o,
-                             ovf, s), "points forward");
+        CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
+                             ctx->r2, o, s), "points forward");
     }
     return GS_OK;
 }
@@ -354,13 +392,11 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
                            ctx->gacc.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
-        uint32_t *ovf = ctx->counters.as<uint32_t>();
-        CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_points_bwd(ctx->rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), nullptr, ctx->accel_q.xyz,
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->dom, ctx->tau, ctx->r2, ctx->r, in,
-                             ctx->gacc.as<float>(), ovf, s), "points backward");
+        CK(launch_points_bwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
+                             ctx->r2, in, ctx->gacc.as<float>(), s), "points backward");
     }
     Stage stage(ctx, GS_PROF_FINALIZE);
     CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, *out, s), "finalize");
@@ -423,11 +459,6 @@ gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, u
     st = run_fwd(ctx, o);
     if (st != GS_OK) return st;
     CK(cudaStreamSynchronize(ctx->stream), "sync");
-    if (ctx->accel_kind == GS_QUERY_POINTS) {
-        uint32_t ovf = 0;
-        CK(cudaMemcpy(&ovf, ctx->counters.p, 4, cudaMemcpyDeviceToHost), "read overflow flag");
-        if (ovf) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
-    }
     return GS_OK;
 }
 
@@ -516,11 +547,6 @@ gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom
             if (dst[k]) CK(cudaMemcpyAsync(dst[k], srcd[k], bytes[k], cudaMemcpyDeviceToHost, s), "D2H grads");
     }
     CK(cudaStreamSynchronize(s), "sync");
-    if (ctx->accel_kind == GS_QUERY_POINTS) {
-        uint32_t ovf = 0;
-        CK(cudaMemcpy(&ovf, ctx->counters.p, 4, cudaMemcpyDeviceToHost), "read overflow flag");
-        if (ovf) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
-    }
     return GS_OK;
 }
 

@@ -107,6 +107,9 @@ struct gs_ctx {
     int leaf_sel = 0;
     gs::DevBuf node_left, node_right, node_parent, leaf_parent, node_aabb, node_flag;
     gs::DevBuf bvh_nodes;  // packed traversal nodes
+    gs::DevBuf sorted_rec; // float4 [N][4]: records in leaf order (id in plane c's .w)
+    gs::DevBuf cull_ids, cull_link, cull_head;  // per-packet survivor lists (see CullLists)
+    uint32_t cull_cap = 0;   // chunks the pool holds
     gs::DevBuf pt_key[2], pt_val[2];
     int pt_sel = 0;
     bool have_pt_order = false;
@@ -168,13 +171,22 @@ cudaError_t launch_finalize(const float4 *rec, const float *params, const float 
 // LBVH
 cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *aabb_valid /*nullable: aabb[N][6]*/, size_t n,
                           const gs_domain &dom, uint32_t *codes, uint32_t *ids, cudaStream_t s);
-cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, uint32_t N, int32_t *left, int32_t *right,
-                        int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed, cudaStream_t s);
-cudaError_t launch_points_fwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const FwdOut &o, uint32_t *overflow,
-                              cudaStream_t s);
-cudaError_t launch_points_bwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const BwdIn &in, float *gacc,
-                              uint32_t *overflow, cudaStream_t s);
+cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, const float4 *rec, uint32_t N, int32_t *left,
+                        int32_t *right, int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed,
+                        float4 *sorted_rec, cudaStream_t s);
+// per-packet (32 sorted points) lists of the Gaussians that can reach the packet: chains of 32-entry chunks
+struct CullLists {
+    uint32_t *ids;    // [cap][32] sorted positions of Gaussians
+    uint32_t *link;   // [cap] next chunk of the chain (0xffffffff = end); every linked chunk is full
+    uint2 *head;      // [packets] (first chunk, entries in it)
+    uint32_t *top;    // chunks requested so far (may exceed cap: the host then grows the pool and repeats)
+    uint32_t cap;
+};
+cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
+                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, cudaStream_t s);
+cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+                              float tau, float r2, const FwdOut &o, cudaStream_t s);
+cudaError_t launch_points_bwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+                              float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s);
 
 }  // namespace gs

@@ -5,7 +5,9 @@
 //   (radix sort)  : stable sort of (code, id) => order by the unique 64-bit key (code << 32 | id)
 //   k_karras      : binary radix tree, one thread per internal node (Karras 2012)
 //   k_refit       : bottom-up exact min/max boxes with per-node arrival counters
-//   k_pack_nodes  : 64-byte traversal nodes holding both children's boxes
+//   k_pack_nodes  : 64-byte traversal nodes holding both children's boxes and links
+//   k_sort_records: the Gaussian records in leaf order, 64 contiguous bytes each (neighbouring leaves are
+//                   neighbouring in memory; a record is two full 32-byte sectors)
 #include "gs_internal.cuh"
 
 namespace gs {
@@ -100,7 +102,7 @@ __global__ void __launch_bounds__(256) k_refit(const uint32_t *__restrict__ ids,
 }
 
 // traversal node (64 B): [0] l.lo.xyz l.hi.x | [1] l.hi.yz r.lo.xy | [2] r.lo.z r.hi.xyz | [3] left, right (bits), -, -
-// a leaf child is stored as ~gaussian_id so the traversal needs no second indirection
+// child link >= 0: internal node; < 0: ~(sorted position of the leaf), which indexes the sorted records directly
 __global__ void __launch_bounds__(256) k_pack_nodes(const uint32_t *__restrict__ ids, const float *__restrict__ aabb, int n,
                                                      const int32_t *__restrict__ left, const int32_t *__restrict__ right,
                                                      const float *__restrict__ node_aabb, float4 *__restrict__ packed) {
@@ -109,15 +111,28 @@ __global__ void __launch_bounds__(256) k_pack_nodes(const uint32_t *__restrict__
     const int l = left[i], r = right[i];
     const float *a = l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l;
     const float *b = r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r;
-    const int lc = l < 0 ? ~(int)ids[~l] : l, rc = r < 0 ? ~(int)ids[~r] : r;
     packed[4 * (size_t)i + 0] = make_float4(a[0], a[1], a[2], a[3]);
     packed[4 * (size_t)i + 1] = make_float4(a[4], a[5], b[0], b[1]);
     packed[4 * (size_t)i + 2] = make_float4(b[2], b[3], b[4], b[5]);
-    packed[4 * (size_t)i + 3] = make_float4(__int_as_float(lc), __int_as_float(rc), 0.f, 0.f);
+    packed[4 * (size_t)i + 3] = make_float4(__int_as_float(l), __int_as_float(r), 0.f, 0.f);
 }
 
-cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, uint32_t N, int32_t *left, int32_t *right,
-                        int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed, cudaStream_t s) {
+// records in leaf order: sorted[4 k .. 4 k + 3] = planes a, b, c, d of Gaussian ids[k], with the id in c.w
+__global__ void __launch_bounds__(256) k_sort_records(const uint32_t *__restrict__ ids, const float4 *__restrict__ rec, uint32_t N,
+                                                       float4 *__restrict__ sorted) {
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;   // one thread per (leaf, plane): coalesced 16-byte stores
+    const uint32_t k = t >> 2, plane = t & 3u;
+    if (k >= N) return;
+    const uint32_t id = ids[k];
+    float4 v = __ldg(rec + (size_t)plane * N + id);
+    if (plane == 2u) v.w = __uint_as_float(id);
+    sorted[t] = v;
+}
+
+cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float *aabb, const float4 *rec, uint32_t N, int32_t *left,
+                        int32_t *right, int32_t *parent, int32_t *leaf_parent, float *node_aabb, uint32_t *flags, float4 *packed,
+                        float4 *sorted_rec, cudaStream_t s) {
+    if (N >= 1) { k_sort_records<<<(unsigned)(((size_t)N * 4 + 255) / 256), 256, 0, s>>>(ids, rec, N, sorted_rec); count_launch(); }
     if (N < 2) {
         if (N == 1) return cudaMemsetAsync(leaf_parent, 0xff, sizeof(int32_t), s);
         return cudaSuccess;

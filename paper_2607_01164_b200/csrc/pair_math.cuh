@@ -86,7 +86,8 @@ __device__ __forceinline__ void warp_reduce16(float (&v)[16], int lane) {
 // The backward contribution of one hit (S7):  with alpha = a/I, beta = b - alpha Phi (per sample),
 //   gamma = alpha v + beta,  t = gamma w G:  dv += alpha w G, dw += gamma G, U += t u, W += t u u^T, E += eps w G
 // acc layout: 0 dv | 1 dw | 2..4 U | 5..10 W00 W01 W02 W11 W12 W22 | 11 E
-__device__ __forceinline__ void bwd_accumulate(float (&acc)[16], float alpha, float beta, float eps, float w, float v, float G,
+template <int K>
+__device__ __forceinline__ void bwd_accumulate(float (&acc)[K], float alpha, float beta, float eps, float w, float v, float G,
                                                float u0, float u1, float u2) {
     const float wG = w * G;
     const float gamma = fmaf(alpha, v, beta);

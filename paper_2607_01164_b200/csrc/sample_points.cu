@@ -1,34 +1,38 @@
 // sample_points.cu -- unstructured sampling kernels (S5 forward, S7 backward; section 5.1.2).
-// A warp is a packet of 32 consecutive points of the coherence-sorted order and walks the LBVH
-// over the Gaussians with one short stack in shared memory.  Three stages, each with its own
-// lane mapping, connected by small shared-memory queues (so that no stage waits on a memory
-// round trip per pair):
-//   1. traverse  lane = tree node.  Up to 32 nodes are popped per step; both children's boxes
-//                (one 64-byte node) are tested against the packet's bounding box; internal
-//                children go back on the stack, leaf children (Gaussian ids) to the candidate queue.
-//   2. refine    lane = candidate Gaussian.  Its record is fetched and the cutoff ellipsoid is
-//                tested against the packet box in whitened space (|M (c - mu)| <= r + rho, the
-//                bound the structured kernels use per cell); survivors are compacted.
-//   3. evaluate  forward: lane = point, the staged survivor records are read from shared memory
-//                (broadcast) and every pair runs the canonical predicate (D4) + Eq. 3.
-//                backward: lane = Gaussian, loop over the packet's 32 points (broadcast from
-//                shared memory): the 12 per-Gaussian sums stay in registers -- the reduction over
-//                the packet costs no shuffles -- and leave with three 16-byte vector reductions
-//                (RED.ADD.F32x4) per (packet, Gaussian); the paper's backward is the same
-//                "per Gaussian, loop over the leaf's positions" shape.
-// Stages 1 and 2 are conservative culls only; membership is decided by the canonical predicate.
+// A warp is a packet of 32 consecutive points of the coherence-sorted order.
+//
+//   k_points_cull  (part of gs_build_accel)  The packet walks the LBVH over the Gaussians with one short stack in
+//       shared memory and writes the list of Gaussians that can reach it.  Two stages with their own lane mapping:
+//         traverse  lane = tree node.  Up to 32 nodes are popped per step; both children's boxes (one 64-byte
+//                   node) are tested against the packet's boxes; internal children go back on the stack, leaf
+//                   children (sorted positions of Gaussians) to the candidate queue.
+//         refine    lane = candidate Gaussian.  Its record is fetched and the cutoff ellipsoid is tested against
+//                   the packet's boxes in whitened space (|M (c - mu)| <= r + rho, the bound the structured
+//                   kernels use per cell); survivors are appended to the packet's list.
+//       Both are conservative culls only; membership is decided by the canonical predicate in the kernels below.
+//       The node loads of the next step and the record loads of the next refine round are issued before the
+//       previous ones are consumed.  The list is a chain of 32-entry chunks taken from a pool with one atomic
+//       per chunk; forward and backward both read it (the traversal runs once per step, not twice).
+//   k_points_fwd   lane = point: the chunk's 32 records are staged in shared memory (broadcast reads) and every
+//       pair runs the canonical predicate (D4) + Eq. 3; fused epilogue S6.
+//   k_points_bwd   lane = Gaussian, loop over the packet's 32 points (broadcast from shared memory): the 12
+//       per-Gaussian sums stay in registers -- the reduction over the packet costs no shuffles -- and leave with
+//       three 16-byte vector reductions (RED.ADD.F32x4) per (packet, Gaussian).  The paper's backward has the same
+//       "per Gaussian, loop over the leaf's positions" shape.
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
 
 namespace gs {
 
-constexpr int PT_WARPS = 8;
+constexpr int CULL_WARPS = 4;            // packets per CTA of k_points_cull
+constexpr int EVAL_WARPS = 4;            // packets per CTA of k_points_fwd / k_points_bwd
 constexpr int STK_CAP = 256;             // stack entries per packet
 constexpr int STK_WIDE = STK_CAP - 66;   // above this fill level one node is popped per step (pure DFS: growth <= tree height <= 64)
-constexpr int CQ_CAP = 96;               // candidate queue: < 32 before a step, a step adds <= 64
-constexpr int SV_CAP = 64;               // survivor buffer: < 32 before a refine round, a round adds <= 32
+constexpr int CQ_CAP = 128;              // candidate queue: a step runs only with <= 64 queued and adds <= 64
+constexpr uint32_t NO_CHUNK = 0xffffffffu;
 
 struct PacketBox { float lx, ly, lz, hx, hy, hz; };
+struct CullBox { float cx, cy, cz, hx, hy, hz; };
 
 __device__ __forceinline__ float warp_min(float v) {
 #pragma unroll
@@ -41,86 +45,30 @@ __device__ __forceinline__ float warp_max(float v) {
     return v;
 }
 
-// Stage 1: one traversal step.  sp, cn are warp-uniform.
 __device__ __forceinline__ bool boxes_overlap(const PacketBox &b, float lx, float ly, float lz, float hx, float hy, float hz) {
-    return lx <= b.hx && hx >= b.lx && ly <= b.hy && hy >= b.ly && lz <= b.hz && hz >= b.lz;
+    return (lx <= b.hx) & (hx >= b.lx) & (ly <= b.hy) & (hy >= b.ly) & (lz <= b.hz) & (hz >= b.lz);
 }
 
-__device__ __forceinline__ void traverse_step(const float4 *__restrict__ nodes, const PacketBox &b, const PacketBox &b2, int32_t *stack, int &sp,
-                                              uint32_t *cand, int &cn, int lane, uint32_t *overflow) {
-    int k = min(min(32, sp), max(1, STK_WIDE - sp));
-    const bool act = lane < k;
-    bool il = false, ir = false, ll = false, lr = false;
-    int32_t lc = 0, rc = 0;
-    if (act) {
-        const int32_t node = stack[sp - 1 - lane];
-        const float4 *np = nodes + 4 * (size_t)node;
-        const float4 n0 = __ldg(np), n1 = __ldg(np + 1), n2 = __ldg(np + 2), n3 = __ldg(np + 3);
-        const bool ol = boxes_overlap(b, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y) || boxes_overlap(b2, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
-        const bool orr = boxes_overlap(b, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w) || boxes_overlap(b2, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
-        lc = __float_as_int(n3.x); rc = __float_as_int(n3.y);
-        il = ol && lc >= 0; ll = ol && lc < 0;
-        ir = orr && rc >= 0; lr = orr && rc < 0;
-    }
-    __syncwarp();
-    sp -= k;
-    const uint32_t lt = (1u << lane) - 1u;
-    const uint32_t bil = __ballot_sync(0xffffffffu, il), bir = __ballot_sync(0xffffffffu, ir);
-    const uint32_t bll = __ballot_sync(0xffffffffu, ll), blr = __ballot_sync(0xffffffffu, lr);
-    const int nil = __popc(bil), nir = __popc(bir), nll = __popc(bll), nlr = __popc(blr);
-    if (sp + nil + nir > STK_CAP) {  // cannot happen for trees of height <= 64 (see STK_WIDE); never write out of bounds
-        if (lane == 0) *overflow = 1u;
-        sp = 0;
-        return;
-    }
-    if (il) stack[sp + __popc(bil & lt)] = lc;
-    if (ir) stack[sp + nil + __popc(bir & lt)] = rc;
-    sp += nil + nir;
-    if (ll) cand[cn + __popc(bll & lt)] = (uint32_t)~lc;
-    if (lr) cand[cn + nll + __popc(blr & lt)] = (uint32_t)~rc;
-    cn += nll + nlr;
-    __syncwarp();
-}
-
-// Stage 2 test: can the cutoff ellipsoid of `g` reach the box (centre c, half extent h)?  For every p in the box
+// Refine test: can the cutoff ellipsoid of `g` reach the box (centre c, half extent h)?  For every p in the box
 // |M (p - mu)| >= |M (c - mu)| - rho with rho = |(sum_k |M_jk| h_k)_j|, so the Gaussian is dropped when
 // |M (c - mu)|^2 > (r + rho)^2 (1 + 2^-9) (the slack covers fp32 rounding of this bound and of the canonical sequence).
-__device__ __forceinline__ bool ellipsoid_reaches(const Rec &g, float cx, float cy, float cz, float hx, float hy, float hz, float rcut) {
-    const float dx = cx - g.a.x, dy = cy - g.a.y, dz = cz - g.a.z;
+__device__ __forceinline__ bool ellipsoid_reaches(const Rec &g, const CullBox &c, float rcut) {
+    const float dx = c.cx - g.a.x, dy = c.cy - g.a.y, dz = c.cz - g.a.z;
     const float u0 = fmaf(g.b.z, dz, fmaf(g.b.y, dy, g.b.x * dx));
     const float u1 = fmaf(g.c.z, dz, fmaf(g.c.y, dy, g.c.x * dx));
     const float u2 = fmaf(g.d.z, dz, fmaf(g.d.y, dy, g.d.x * dx));
-    const float e0 = fmaf(fabsf(g.b.z), hz, fmaf(fabsf(g.b.y), hy, fabsf(g.b.x) * hx));
-    const float e1 = fmaf(fabsf(g.c.z), hz, fmaf(fabsf(g.c.y), hy, fabsf(g.c.x) * hx));
-    const float e2 = fmaf(fabsf(g.d.z), hz, fmaf(fabsf(g.d.y), hy, fabsf(g.d.x) * hx));
+    const float e0 = fmaf(fabsf(g.b.z), c.hz, fmaf(fabsf(g.b.y), c.hy, fabsf(g.b.x) * c.hx));
+    const float e1 = fmaf(fabsf(g.c.z), c.hz, fmaf(fabsf(g.c.y), c.hy, fabsf(g.c.x) * c.hx));
+    const float e2 = fmaf(fabsf(g.d.z), c.hz, fmaf(fabsf(g.d.y), c.hy, fabsf(g.d.x) * c.hx));
     const float qc = fmaf(u2, u2, fmaf(u1, u1, u0 * u0));
     const float reach = rcut + sqrtf(fmaf(e2, e2, fmaf(e1, e1, e0 * e0)));
     // false for NaN records (invalid Gaussians, D13) and for a NaN box (empty part); true for an infinite box (see segment_box)
     return qc <= reach * reach * 1.001953125f;
 }
 
-__device__ __forceinline__ Rec load_rec(const float4 *__restrict__ rec, uint32_t N, uint32_t id) {
-    Rec g;
-    g.a = __ldg(rec + id); g.b = __ldg(rec + (size_t)N + id); g.c = __ldg(rec + 2 * (size_t)N + id); g.d = __ldg(rec + 3 * (size_t)N + id);
-    return g;
-}
-
-struct PacketState {      // per-warp shared memory of stage 1
-    int32_t stack[STK_CAP];
-    uint32_t cand[CQ_CAP];
-};
-
-// Packet set-up shared by both kernels: the point of this lane, the packet's boxes and the root of the traversal.
 // A packet of 32 consecutive Morton-sorted points can straddle a jump of the Z curve (its box then spans a large
 // part of the domain).  The packet is therefore cut once, at its highest-level jump (largest code[i] ^ code[i+1]):
 // each part lies inside one Morton cell and gets its own box; a Gaussian is kept when it reaches either.
-struct CullBox { float cx, cy, cz, hx, hy, hz; };
-struct Packet {
-    uint64_t c; bool active; float px, py, pz;
-    PacketBox box[2]; CullBox cb[2];
-    int sp, cn;
-};
-
 __device__ __forceinline__ void segment_box(float px, float py, float pz, bool in_seg, PacketBox &b, CullBox &cb) {
     const float nanv = __int_as_float(0x7fc00000);
     const float x = in_seg ? px : nanv, y = in_seg ? py : nanv, z = in_seg ? pz : nanv;
@@ -138,94 +86,199 @@ __device__ __forceinline__ void segment_box(float px, float py, float pz, bool i
     }
 }
 
-__device__ __forceinline__ void packet_init(Packet &pk, PacketState &st, const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
-                                            uint64_t P, uint32_t N, const MortonParams &mp, int warp, int lane) {
-    const uint64_t k = ((uint64_t)blockIdx.x * PT_WARPS + warp) * 32 + lane;
-    pk.active = k < P;
-    pk.c = pk.active ? (pt_order ? (uint64_t)pt_order[k] : k) : 0;
+// The point of lane `lane` of packet `packet` (NaN for lanes past the end: never inside anything).
+struct PacketPoint { uint64_t c; bool active; float px, py, pz; };
+__device__ __forceinline__ PacketPoint load_point(const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order, uint64_t P,
+                                                  uint64_t packet, int lane) {
+    PacketPoint pp;
+    const uint64_t k = packet * 32 + lane;
+    pp.active = k < P;
+    pp.c = pp.active ? (pt_order ? (uint64_t)pt_order[k] : k) : 0;
     const float nanv = __int_as_float(0x7fc00000);
-    pk.px = pk.active ? xyz[3 * pk.c] : nanv; pk.py = pk.active ? xyz[3 * pk.c + 1] : nanv; pk.pz = pk.active ? xyz[3 * pk.c + 2] : nanv;
-    const uint32_t code = morton30(pk.px, pk.py, pk.pz, mp);
-    const uint32_t next = __shfl_down_sync(0xffffffffu, code, 1);
-    const uint32_t jump = lane < 31 ? (code ^ next) : 0u;
-    const uint32_t top = __reduce_max_sync(0xffffffffu, jump);
-    const int cut = top ? __ffs(__ballot_sync(0xffffffffu, jump == top)) - 1 : 31;   // part 0 = lanes [0, cut], part 1 = the rest
-    segment_box(pk.px, pk.py, pk.pz, lane <= cut, pk.box[0], pk.cb[0]);
-    segment_box(pk.px, pk.py, pk.pz, lane > cut, pk.box[1], pk.cb[1]);
-    pk.sp = 0; pk.cn = 0;
-    if (N >= 2) { if (lane == 0) st.stack[0] = 0; pk.sp = 1; }
-    else if (N == 1) { if (lane == 0) st.cand[0] = 0u; pk.cn = 1; }
-    __syncwarp();
+    pp.px = pp.active ? xyz[3 * pp.c] : nanv; pp.py = pp.active ? xyz[3 * pp.c + 1] : nanv; pp.pz = pp.active ? xyz[3 * pp.c + 2] : nanv;
+    return pp;
 }
 
-__device__ __forceinline__ bool reaches_packet(const Rec &g, const Packet &pk, float rcut) {
-    return ellipsoid_reaches(g, pk.cb[0].cx, pk.cb[0].cy, pk.cb[0].cz, pk.cb[0].hx, pk.cb[0].hy, pk.cb[0].hz, rcut) ||
-           ellipsoid_reaches(g, pk.cb[1].cx, pk.cb[1].cy, pk.cb[1].cz, pk.cb[1].hx, pk.cb[1].hy, pk.cb[1].hz, rcut);
-}
-
-template <bool SETS>
-__global__ void __launch_bounds__(PT_WARPS * 32) k_points_fwd(const float4 *__restrict__ rec, uint32_t N, const float4 *__restrict__ nodes,
-                                                               const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
-                                                               uint64_t P, MortonParams mp, float tau, float r2, float rcut, FwdOut o, double invP,
-                                                               uint32_t *__restrict__ overflow) {
-    __shared__ PacketState pstate[PT_WARPS];
-    __shared__ float4 srec_all[PT_WARPS][4][SV_CAP];   // staged survivor records (plane c's .w carries the Gaussian id)
-    __shared__ double red[PT_WARPS];
+// ---------------------------------------------------------------------------------------------------------
+// k_points_cull: per-packet list of the Gaussians (sorted positions) whose cutoff ellipsoid can reach the packet.
+// List = chain of chunks: head[packet] = (first chunk, entries in it); every further chunk (link[chunk]) is full.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *__restrict__ srt, uint32_t N, const float4 *__restrict__ nodes,
+                                                                  const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
+                                                                  uint64_t P, MortonParams mp, float rcut, CullLists o,
+                                                                  uint32_t *__restrict__ overflow) {
+    __shared__ int32_t stack_all[CULL_WARPS][STK_CAP];
+    __shared__ uint32_t cand_all[CULL_WARPS][CQ_CAP];
+    __shared__ uint32_t surv_all[CULL_WARPS][64];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    PacketState &st = pstate[warp];
-    float4 (*srec)[SV_CAP] = srec_all[warp];
-    Packet pk;
-    packet_init(pk, st, xyz, pt_order, P, N, mp, warp, lane);
-    const float px = pk.px, py = pk.py, pz = pk.pz;
+    const uint64_t packet = (uint64_t)blockIdx.x * CULL_WARPS + warp;
+    if (packet * 32 >= P) return;
+    int32_t *stack = stack_all[warp];
+    uint32_t *cand = cand_all[warp], *surv = surv_all[warp];
+    const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
+    PacketBox box0, box1;
+    CullBox cb0, cb1;
+    {
+        const uint32_t code = morton30(pp.px, pp.py, pp.pz, mp);
+        const uint32_t next = __shfl_down_sync(0xffffffffu, code, 1);
+        const uint32_t jump = (lane < 31 && (packet * 32 + lane + 1) < P) ? (code ^ next) : 0u;
+        const uint32_t top = __reduce_max_sync(0xffffffffu, jump);
+        const int cut = top ? __ffs(__ballot_sync(0xffffffffu, jump == top)) - 1 : 31;   // part 0 = lanes [0, cut], part 1 = the rest
+        segment_box(pp.px, pp.py, pp.pz, lane <= cut, box0, cb0);
+        segment_box(pp.px, pp.py, pp.pz, lane > cut, box1, cb1);
+    }
+    int sp = 0, cn = 0, sn = 0;   // stack entries, queued candidates, survivors not yet written (all warp-uniform)
+    uint32_t prev = NO_CHUNK;
+    if (N >= 2) { if (lane == 0) stack[0] = 0; sp = 1; }
+    else if (N == 1) { if (lane == 0) cand[0] = 0u; cn = 1; }
+    __syncwarp();
+    const uint32_t lt = (1u << lane) - 1u;
+    while (true) {
+        // ---- issue: nodes of the next traversal step (one node per step when the stack is nearly full: pure DFS grows
+        //      the stack by at most the tree height <= 64, so STK_CAP cannot be exceeded)
+        const int kA = (sp > 0 && cn <= CQ_CAP - 64) ? min(min(32, sp), max(1, STK_WIDE - sp)) : 0;
+        float4 n0, n1, n2, n3;
+        if (lane < kA) {
+            const float4 *np = nodes + 4 * (size_t)stack[sp - 1 - lane];
+            n0 = __ldg(np); n1 = __ldg(np + 1); n2 = __ldg(np + 2); n3 = __ldg(np + 3);
+        }
+        sp -= kA;
+        // ---- issue: records of the next refine round (full rounds while the traversal is running)
+        const int kB = (cn >= 32 || (sp == 0 && kA == 0)) ? min(cn, 32) : 0;
+        Rec g;
+        uint32_t pos = 0;
+        if (lane < kB) {
+            pos = cand[cn - 1 - lane];
+            const float4 *rp = srt + 4 * (size_t)pos;
+            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
+        }
+        cn -= kB;
+        const bool drain = kA == 0 && kB == 0;   // => stack and queue are empty
+        // ---- write a full chunk of survivors while the loads are in flight
+        if (sn >= 32) {
+            uint32_t c = 0;
+            if (lane == 0) c = atomicAdd(o.top, 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c < o.cap) {
+                o.ids[(size_t)c * 32 + lane] = surv[sn - 32 + lane];
+                if (lane == 0) o.link[c] = prev;
+            }
+            prev = c;
+            sn -= 32;
+        }
+        __syncwarp();
+        // ---- traverse: consume the nodes
+        if (kA > 0) {
+            bool il = false, ir = false, ll = false, lr = false;
+            int32_t lc = 0, rc = 0;
+            if (lane < kA) {
+                const bool ol = boxes_overlap(box0, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y) | boxes_overlap(box1, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
+                const bool orr = boxes_overlap(box0, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w) | boxes_overlap(box1, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
+                lc = __float_as_int(n3.x); rc = __float_as_int(n3.y);
+                il = ol & (lc >= 0); ll = ol & (lc < 0);
+                ir = orr & (rc >= 0); lr = orr & (rc < 0);
+            }
+            const uint32_t bil = __ballot_sync(0xffffffffu, il), bir = __ballot_sync(0xffffffffu, ir);
+            const uint32_t bll = __ballot_sync(0xffffffffu, ll), blr = __ballot_sync(0xffffffffu, lr);
+            const int nil = __popc(bil), nll = __popc(bll);
+            const int sp2 = sp + nil + __popc(bir);
+            if (sp2 > STK_CAP) {   // unreachable for trees of height <= 64; never write out of bounds
+                if (lane == 0) *overflow = 1u;
+            } else {
+                if (il) stack[sp + __popc(bil & lt)] = lc;
+                if (ir) stack[sp + nil + __popc(bir & lt)] = rc;
+                sp = sp2;
+            }
+            if (ll) cand[cn + __popc(bll & lt)] = (uint32_t)~lc;
+            if (lr) cand[cn + nll + __popc(blr & lt)] = (uint32_t)~rc;
+            cn += nll + __popc(blr);
+        }
+        // ---- refine: consume the records
+        if (kB > 0) {
+            const bool keep = lane < kB && (ellipsoid_reaches(g, cb0, rcut) | ellipsoid_reaches(g, cb1, rcut));
+            const uint32_t bk = __ballot_sync(0xffffffffu, keep);
+            if (keep) surv[sn + __popc(bk & lt)] = pos;
+            sn += __popc(bk);
+        }
+        __syncwarp();
+        if (drain) break;
+    }
+    // the remaining (< 32 ... or exactly 32 from the last round) survivors: at most two more chunks; the last one written is the head
+    uint32_t head_cnt = prev == NO_CHUNK ? 0u : 32u;
+    while (sn > 0) {
+        const int k = min(sn, 32);
+        uint32_t c = 0;
+        if (lane == 0) c = atomicAdd(o.top, 1u);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c < o.cap) {
+            // a partial chunk must be the head (every linked chunk is full): write the full one first
+            if (lane < k) o.ids[(size_t)c * 32 + lane] = surv[(sn > 32 ? 0 : sn - k) + lane];
+            if (lane == 0) o.link[c] = prev;
+        }
+        prev = c;
+        head_cnt = (uint32_t)k;
+        if (sn > 32) {   // 32 < sn < 64: entries [0, 32) went out as a full chunk, move the tail down
+            const uint32_t t = lane < sn - 32 ? surv[32 + lane] : 0u;
+            __syncwarp();
+            if (lane < sn - 32) surv[lane] = t;
+            __syncwarp();
+        }
+        sn -= k;
+    }
+    if (lane == 0) o.head[packet] = make_uint2(prev, head_cnt);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// k_points_fwd: lane = point; the packet's list is consumed chunk by chunk (32 records staged in shared memory).
+// ---------------------------------------------------------------------------------------------------------
+template <bool SETS>
+__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
+                                                                 const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
+                                                                 float r2, FwdOut o, double invP) {
+    __shared__ float4 srec_all[EVAL_WARPS][4][32];   // staged records (plane c's .w carries the Gaussian id)
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
+    if (packet * 32 >= P) return;
+    float4 (*srec)[32] = srec_all[warp];
+    const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
+    const float px = pp.px, py = pp.py, pz = pp.pz;
     float I = 0.f, Nacc = 0.f;
     uint32_t cnt = 0, tested = 0;
     unsigned long long hsum = 0, hxor = 0;
-    int sp = pk.sp, cn = pk.cn, sn = 0;
-    const uint32_t lt = (1u << lane) - 1u;
-    while (true) {
-        while (cn < 32 && sp > 0) traverse_step(nodes, pk.box[0], pk.box[1], st.stack, sp, st.cand, cn, lane, overflow);
-        if (cn > 0) {   // stage 2: refine up to 32 candidates
-            const int k = min(cn, 32);
-            bool keep = false;
-            Rec g;
-            uint32_t id = 0;
-            if (lane < k) {
-                id = st.cand[cn - 1 - lane];
-                g = load_rec(rec, N, id);
-                keep = reaches_packet(g, pk, rcut);
-            }
-            cn -= k;
-            const uint32_t bk = __ballot_sync(0xffffffffu, keep);
-            if (keep) {
-                const int slot = sn + __popc(bk & lt);
-                g.c.w = __uint_as_float(id);
-                srec[0][slot] = g.a; srec[1][slot] = g.b; srec[2][slot] = g.c; srec[3][slot] = g.d;
-            }
-            sn += __popc(bk);
-            __syncwarp();
+    const uint2 head = __ldg(L.head + packet);
+    uint32_t chunk = head.x;
+    int n = (int)head.y;
+    // the ids of the current chunk are fetched one chunk ahead, so a chunk costs one dependent round trip (its records)
+    uint32_t pos = (chunk != NO_CHUNK && lane < n) ? __ldg(L.ids + (size_t)chunk * 32 + lane) : 0u;
+    uint32_t link = chunk != NO_CHUNK ? __ldg(L.link + chunk) : NO_CHUNK;
+    while (chunk != NO_CHUNK) {
+        Rec g;
+        if (lane < n) {
+            const float4 *rp = srt + 4 * (size_t)pos;
+            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
         }
-        const bool done = cn == 0 && sp == 0;
-        if (sn >= 32 || (done && sn > 0)) {   // stage 3: every lane evaluates its point against the staged records
-#pragma unroll 2
-            for (int j = 0; j < sn; j++) {
-                Rec g;
-                g.a = srec[0][j]; g.b = srec[1][j]; g.c = srec[2][j]; g.d = srec[3][j];
-                float u0, u1, u2;
-                const float qd = mahalanobis(g, px, py, pz, u0, u1, u2);
-                const bool hit = qd <= r2;
-                const float wG = hit ? g.a.w * gauss_weight(qd) : 0.f;
-                I += wG;
-                Nacc = fmaf(g.b.w, wG, Nacc);
-                if (SETS && hit) { const unsigned long long h = mix64(__float_as_uint(g.c.w)); cnt++; hsum += h; hxor ^= h; }
-            }
-            if (SETS) tested += (uint32_t)sn;
-            sn = 0;
-            __syncwarp();
+        const uint32_t npos = link != NO_CHUNK ? __ldg(L.ids + (size_t)link * 32 + lane) : 0u;   // linked chunks are full
+        const uint32_t nlink = link != NO_CHUNK ? __ldg(L.link + link) : NO_CHUNK;
+        if (lane < n) { srec[0][lane] = g.a; srec[1][lane] = g.b; srec[2][lane] = g.c; srec[3][lane] = g.d; }
+        __syncwarp();
+#pragma unroll 4
+        for (int j = 0; j < n; j++) {
+            Rec q;
+            q.a = srec[0][j]; q.b = srec[1][j]; q.c = srec[2][j]; q.d = srec[3][j];
+            float u0, u1, u2;
+            const float qd = mahalanobis(q, px, py, pz, u0, u1, u2);
+            const bool hit = qd <= r2;
+            const float wG = hit ? q.a.w * gauss_weight(qd) : 0.f;
+            I += wG;
+            Nacc = fmaf(q.b.w, wG, Nacc);
+            if (SETS && hit) { const unsigned long long h = mix64(__float_as_uint(q.c.w)); cnt++; hsum += h; hxor ^= h; }
         }
-        if (done) break;
+        if (SETS) tested += (uint32_t)n;
+        __syncwarp();
+        chunk = link; pos = npos; link = nlink; n = 32;
     }
-    const bool active = pk.active;
-    const uint64_t c = pk.c;
+    const bool active = pp.active;
+    const uint64_t c = pp.c;
     const bool covered = I > tau;
     const float phi = covered ? __fdividef(Nacc, I) : 0.f;
     float res2 = 0.f;
@@ -248,17 +301,11 @@ __global__ void __launch_bounds__(PT_WARPS * 32) k_points_fwd(const float4 *__re
             if (o.set_xor) o.set_xor[c] = hxor;
         }
     }
-    if (o.target && o.loss) {
+    if (o.target && o.loss) {   // one reduction per packet (no CTA barrier: a warp's slot frees as soon as its packet is done)
         double s = (double)res2;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
-        if (lane == 0) red[warp] = s;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double v = 0.0;
-            for (int w = 0; w < PT_WARPS; w++) v += red[w];
-            if (v != 0.0) atomicAdd(o.loss, v * invP);
-        }
+        if (lane == 0 && s != 0.0) atomicAdd(o.loss, s * invP);
     }
     if (SETS && o.counters) {
         unsigned long long t = active ? tested : 0, h = cnt;
@@ -268,27 +315,26 @@ __global__ void __launch_bounds__(PT_WARPS * 32) k_points_fwd(const float4 *__re
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// k_points_bwd: lane = Gaussian of the chunk, loop over the packet's 32 points.
+// ---------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void red_add_v4(float *addr, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
-__global__ void __launch_bounds__(PT_WARPS * 32) k_points_bwd(const float4 *__restrict__ rec, uint32_t N, const float4 *__restrict__ nodes,
-                                                               const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
-                                                               uint64_t P, MortonParams mp, float tau, float r2, float rcut, BwdIn in,
-                                                               float *__restrict__ gacc, uint32_t *__restrict__ overflow) {
-    __shared__ PacketState pstate[PT_WARPS];
-    __shared__ uint32_t surv_all[PT_WARPS][SV_CAP];
-    __shared__ float4 pts_all[PT_WARPS][2][32];   // [0] x y z alpha   [1] beta eps - -
+__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
+                                                                 const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
+                                                                 float r2, BwdIn in, float *__restrict__ gacc) {
+    __shared__ float4 pts_all[EVAL_WARPS][2][32];   // [0] x y z alpha   [1] beta eps - -
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    PacketState &st = pstate[warp];
-    uint32_t *surv = surv_all[warp];
+    const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
+    if (packet * 32 >= P) return;
     float4 (*pts)[32] = pts_all[warp];
-    Packet pk;
-    packet_init(pk, st, xyz, pt_order, P, N, mp, warp, lane);
     {
+        const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
         // per-sample coefficients: alpha = covered ? a/I : 0, beta = b - alpha Phi, eps = covered ? |Phi - t|/I : 0
-        const bool active = pk.active;
-        const uint64_t c = pk.c;
+        const bool active = pp.active;
+        const uint64_t c = pp.c;
         float alpha = 0.f, beta = 0.f, eps = 0.f;
         if (active && in.pack2) {  // fused MSE: eps = |res| / I = |alpha| * P / 2
             const float2 s = __ldg(in.pack2 + c);
@@ -301,83 +347,85 @@ __global__ void __launch_bounds__(PT_WARPS * 32) k_points_bwd(const float4 *__re
             beta = (in.dL_dI ? in.dL_dI[c] : 0.f) - alpha * ph;
             eps = (covered && in.target) ? fabsf(ph - in.target[c]) * inv : 0.f;
         }
-        pts[0][lane] = make_float4(pk.px, pk.py, pk.pz, alpha);   // inactive lanes hold NaN positions: never a hit
+        pts[0][lane] = make_float4(pp.px, pp.py, pp.pz, alpha);   // inactive lanes hold NaN positions: never a hit
         pts[1][lane] = make_float4(beta, eps, 0.f, 0.f);
         __syncwarp();
     }
-    int sp = pk.sp, cn = pk.cn, sn = 0;
-    const uint32_t lt = (1u << lane) - 1u;
-    while (true) {
-        while (cn < 32 && sp > 0) traverse_step(nodes, pk.box[0], pk.box[1], st.stack, sp, st.cand, cn, lane, overflow);
-        if (cn > 0) {   // stage 2
-            const int k = min(cn, 32);
-            bool keep = false;
-            uint32_t id = 0;
-            if (lane < k) {
-                id = st.cand[cn - 1 - lane];
-                const Rec g = load_rec(rec, N, id);
-                keep = reaches_packet(g, pk, rcut);
-            }
-            cn -= k;
-            const uint32_t bk = __ballot_sync(0xffffffffu, keep);
-            if (keep) surv[sn + __popc(bk & lt)] = id;
-            sn += __popc(bk);
-            __syncwarp();
-        }
-        const bool done = cn == 0 && sp == 0;
-        if (sn >= 32 || (done && sn > 0)) {   // stage 3: lane = Gaussian, loop over the packet's points
-            const int k = min(sn, 32);
-            if (lane < k) {
-                const uint32_t id = surv[sn - 1 - lane];
-                const Rec g = load_rec(rec, N, id);
-                float acc[16];
+    const uint2 head = __ldg(L.head + packet);
+    uint32_t chunk = head.x;
+    int n = (int)head.y;
+    uint32_t pos = (chunk != NO_CHUNK && lane < n) ? __ldg(L.ids + (size_t)chunk * 32 + lane) : 0u;
+    uint32_t link = chunk != NO_CHUNK ? __ldg(L.link + chunk) : NO_CHUNK;
+    Rec g;
+    if (chunk != NO_CHUNK && lane < n) {
+        const float4 *rp = srt + 4 * (size_t)pos;
+        g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
+    }
+    while (chunk != NO_CHUNK) {
+        // the next chunk's ids and link are requested now; its records right after this chunk's loop is set up
+        const uint32_t npos = link != NO_CHUNK ? __ldg(L.ids + (size_t)link * 32 + lane) : 0u;
+        const uint32_t nlink = link != NO_CHUNK ? __ldg(L.link + link) : NO_CHUNK;
+        if (lane < n) {
+            float acc[12];
 #pragma unroll
-                for (int q = 0; q < 16; q++) acc[q] = 0.f;
-                bool any = false;
+            for (int q = 0; q < 12; q++) acc[q] = 0.f;
+            bool any = false;
 #pragma unroll 4
-                for (int p = 0; p < 32; p++) {
-                    const float4 pa = pts[0][p], pb = pts[1][p];
-                    float u0, u1, u2;
-                    const float qd = mahalanobis(g, pa.x, pa.y, pa.z, u0, u1, u2);
-                    if (qd <= r2) {
-                        any = true;
-                        bwd_accumulate(acc, pa.w, pb.x, pb.y, g.a.w, g.b.w, gauss_weight(qd), u0, u1, u2);
-                    }
-                }
-                if (any) {
-                    float *row = gacc + (size_t)id * GACC;
-                    red_add_v4(row, acc[0], acc[1], acc[2], acc[3]);
-                    red_add_v4(row + 4, acc[4], acc[5], acc[6], acc[7]);
-                    red_add_v4(row + 8, acc[8], acc[9], acc[10], acc[11]);
+            for (int p = 0; p < 32; p++) {
+                const float4 pa = pts[0][p], pb = pts[1][p];
+                float u0, u1, u2;
+                const float qd = mahalanobis(g, pa.x, pa.y, pa.z, u0, u1, u2);
+                if (qd <= r2) {
+                    any = true;
+                    bwd_accumulate(acc, pa.w, pb.x, pb.y, g.a.w, g.b.w, gauss_weight(qd), u0, u1, u2);
                 }
             }
-            sn -= k;
-            __syncwarp();
+            if (any) {
+                float *row = gacc + (size_t)__float_as_uint(g.c.w) * GACC;
+                red_add_v4(row, acc[0], acc[1], acc[2], acc[3]);
+                red_add_v4(row + 4, acc[4], acc[5], acc[6], acc[7]);
+                red_add_v4(row + 8, acc[8], acc[9], acc[10], acc[11]);
+            }
         }
-        if (done && sn == 0) break;
+        chunk = link; pos = npos; link = nlink; n = 32;
+        if (chunk != NO_CHUNK) {
+            const float4 *rp = srt + 4 * (size_t)pos;
+            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
+        }
     }
 }
 
-cudaError_t launch_points_fwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const FwdOut &o,
-                              uint32_t *overflow, cudaStream_t s) {
-    (void)leaf_order;
+cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
+                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)((P + PT_WARPS * 32 - 1) / (PT_WARPS * 32));
-    const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
-    if (sets) k_points_fwd<true><<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, morton_params(dom), tau, r2, rcut, o, 1.0 / (double)P, overflow);
-    else k_points_fwd<false><<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, morton_params(dom), tau, r2, rcut, o, 1.0 / (double)P, overflow);
+    cudaError_t e = cudaMemsetAsync(lists.top, 0, sizeof(uint32_t), s);
+    if (e != cudaSuccess) return e;
+    const uint64_t packets = (P + 31) / 32;
+    const unsigned blocks = (unsigned)((packets + CULL_WARPS - 1) / CULL_WARPS);
+    k_points_cull<<<blocks, CULL_WARPS * 32, 0, s>>>(sorted_rec, N, nodes, xyz, pt_order, P, morton_params(dom), rcut, lists, overflow);
     count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_points_bwd(const float4 *rec, uint32_t N, const float4 *nodes, const uint32_t *leaf_order, const float *xyz,
-                              const uint32_t *pt_order, uint64_t P, const gs_domain &dom, float tau, float r2, float rcut, const BwdIn &in, float *gacc,
-                              uint32_t *overflow, cudaStream_t s) {
-    (void)leaf_order;
+cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+                              float tau, float r2, const FwdOut &o, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)((P + PT_WARPS * 32 - 1) / (PT_WARPS * 32));
-    k_points_bwd<<<blocks, PT_WARPS * 32, 0, s>>>(rec, N, nodes, xyz, pt_order, P, morton_params(dom), tau, r2, rcut, in, gacc, overflow); count_launch();
+    const uint64_t packets = (P + 31) / 32;
+    const unsigned blocks = (unsigned)((packets + EVAL_WARPS - 1) / EVAL_WARPS);
+    const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
+    if (sets) k_points_fwd<true><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, 1.0 / (double)P);
+    else k_points_fwd<false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, 1.0 / (double)P);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_points_bwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+                              float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s) {
+    if (P == 0) return cudaSuccess;
+    const uint64_t packets = (P + 31) / 32;
+    const unsigned blocks = (unsigned)((packets + EVAL_WARPS - 1) / EVAL_WARPS);
+    k_points_bwd<<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, in, gacc);
+    count_launch();
     return cudaGetLastError();
 }
 
