@@ -99,6 +99,25 @@ __device__ __forceinline__ PacketPoint load_point(const float *__restrict__ xyz,
     return pp;
 }
 
+// Warp-cooperative gather of `count` (<= 32) 64-byte objects base[4 * index .. 4 * index + 3] into shared memory: lane l
+// copies the 16-byte piece l & 3 of four objects, so one copy instruction touches 8 cache lines instead of 32 (a
+// lane-per-object LDG.128 x 4 spends four times the L1 tag cycles).  Object j lands at dst[4 j + (piece ^ ((j >> 1) & 3))]:
+// the swizzle makes the later lane-per-object 16-byte reads bank-conflict free (SWIZZLE = false: plain layout, for
+// readers that broadcast one object to all lanes).  Completed by cp.async.wait_all.
+template <bool SWIZZLE = true>
+__device__ __forceinline__ void gather64(const float4 *__restrict__ base, uint32_t index_of_lane, int count, float4 *dst, int lane) {
+    const int piece = lane & 3;
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const int j = i * 8 + (lane >> 2);
+        const uint32_t idx = __shfl_sync(0xffffffffu, index_of_lane, j);
+        if (i * 8 < count && j < count) {
+            const unsigned sdst = (unsigned)__cvta_generic_to_shared(dst + 4 * j + (SWIZZLE ? (piece ^ ((j >> 1) & 3)) : piece));
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sdst), "l"(base + 4 * (size_t)idx + piece) : "memory");
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // k_points_cull: per-packet list of the Gaussians (sorted positions) whose cutoff ellipsoid can reach the packet.
 // List = chain of chunks: head[packet] = (first chunk, entries in it); every further chunk (link[chunk]) is full.
@@ -110,11 +129,13 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
     __shared__ int32_t stack_all[CULL_WARPS][STK_CAP];
     __shared__ uint32_t cand_all[CULL_WARPS][CQ_CAP];
     __shared__ uint32_t surv_all[CULL_WARPS][64];
+    __shared__ float4 nbuf_all[CULL_WARPS][128], rbuf_all[CULL_WARPS][128];   // 32 nodes / 32 records of 64 B, swizzled
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint64_t packet = (uint64_t)blockIdx.x * CULL_WARPS + warp;
     if (packet * 32 >= P) return;
     int32_t *stack = stack_all[warp];
     uint32_t *cand = cand_all[warp], *surv = surv_all[warp];
+    float4 *nbuf = nbuf_all[warp], *rbuf = rbuf_all[warp];
     const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
     PacketBox box0, box1;
     CullBox cb0, cb1;
@@ -137,21 +158,12 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
         // ---- issue: nodes of the next traversal step (one node per step when the stack is nearly full: pure DFS grows
         //      the stack by at most the tree height <= 64, so STK_CAP cannot be exceeded)
         const int kA = (sp > 0 && cn <= CQ_CAP - 64) ? min(min(32, sp), max(1, STK_WIDE - sp)) : 0;
-        float4 n0, n1, n2, n3;
-        if (lane < kA) {
-            const float4 *np = nodes + 4 * (size_t)stack[sp - 1 - lane];
-            n0 = __ldg(np); n1 = __ldg(np + 1); n2 = __ldg(np + 2); n3 = __ldg(np + 3);
-        }
+        if (kA > 0) gather64(nodes, lane < kA ? (uint32_t)stack[sp - 1 - lane] : 0u, kA, nbuf, lane);
         sp -= kA;
         // ---- issue: records of the next refine round (full rounds while the traversal is running)
         const int kB = (cn >= 32 || (sp == 0 && kA == 0)) ? min(cn, 32) : 0;
-        Rec g;
-        uint32_t pos = 0;
-        if (lane < kB) {
-            pos = cand[cn - 1 - lane];
-            const float4 *rp = srt + 4 * (size_t)pos;
-            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
-        }
+        const uint32_t pos = lane < kB ? cand[cn - 1 - lane] : 0u;
+        if (kB > 0) gather64(srt, pos, kB, rbuf, lane);
         cn -= kB;
         const bool drain = kA == 0 && kB == 0;   // => stack and queue are empty
         // ---- write a full chunk of survivors while the loads are in flight
@@ -166,12 +178,15 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
             prev = c;
             sn -= 32;
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");
         __syncwarp();
         // ---- traverse: consume the nodes
         if (kA > 0) {
             bool il = false, ir = false, ll = false, lr = false;
             int32_t lc = 0, rc = 0;
             if (lane < kA) {
+                const int f = (lane >> 1) & 3;
+                const float4 n0 = nbuf[4 * lane + f], n1 = nbuf[4 * lane + (1 ^ f)], n2 = nbuf[4 * lane + (2 ^ f)], n3 = nbuf[4 * lane + (3 ^ f)];
                 const bool ol = boxes_overlap(box0, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y) | boxes_overlap(box1, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
                 const bool orr = boxes_overlap(box0, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w) | boxes_overlap(box1, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
                 lc = __float_as_int(n3.x); rc = __float_as_int(n3.y);
@@ -195,7 +210,13 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
         }
         // ---- refine: consume the records
         if (kB > 0) {
-            const bool keep = lane < kB && (ellipsoid_reaches(g, cb0, rcut) | ellipsoid_reaches(g, cb1, rcut));
+            bool keep = false;
+            if (lane < kB) {
+                const int f = (lane >> 1) & 3;
+                Rec g;
+                g.a = rbuf[4 * lane + f]; g.b = rbuf[4 * lane + (1 ^ f)]; g.c = rbuf[4 * lane + (2 ^ f)]; g.d = rbuf[4 * lane + (3 ^ f)];
+                keep = ellipsoid_reaches(g, cb0, rcut) | ellipsoid_reaches(g, cb1, rcut);
+            }
             const uint32_t bk = __ballot_sync(0xffffffffu, keep);
             if (keep) surv[sn + __popc(bk & lt)] = pos;
             sn += __popc(bk);
@@ -235,36 +256,38 @@ template <bool SETS>
 __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, FwdOut o, double invP) {
-    __shared__ float4 srec_all[EVAL_WARPS][4][32];   // staged records (plane c's .w carries the Gaussian id)
+    __shared__ float4 buf_all[EVAL_WARPS][2][128];   // two chunks of 32 records of 64 B (plane c's .w carries the Gaussian id)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
     if (packet * 32 >= P) return;
-    float4 (*srec)[32] = srec_all[warp];
+    float4 (*buf)[128] = buf_all[warp];
     const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
     const float px = pp.px, py = pp.py, pz = pp.pz;
     float I = 0.f, Nacc = 0.f;
     uint32_t cnt = 0, tested = 0;
     unsigned long long hsum = 0, hxor = 0;
+    // Software pipeline over the chain of chunks: while chunk k is evaluated, the records of chunk k+1 are being
+    // copied into the other buffer and the ids of chunk k+2 are being loaded.
     const uint2 head = __ldg(L.head + packet);
-    uint32_t chunk = head.x;
-    int n = (int)head.y;
-    // the ids of the current chunk are fetched one chunk ahead, so a chunk costs one dependent round trip (its records)
-    uint32_t pos = (chunk != NO_CHUNK && lane < n) ? __ldg(L.ids + (size_t)chunk * 32 + lane) : 0u;
-    uint32_t link = chunk != NO_CHUNK ? __ldg(L.link + chunk) : NO_CHUNK;
-    while (chunk != NO_CHUNK) {
-        Rec g;
-        if (lane < n) {
-            const float4 *rp = srt + 4 * (size_t)pos;
-            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
-        }
-        const uint32_t npos = link != NO_CHUNK ? __ldg(L.ids + (size_t)link * 32 + lane) : 0u;   // linked chunks are full
-        const uint32_t nlink = link != NO_CHUNK ? __ldg(L.link + link) : NO_CHUNK;
-        if (lane < n) { srec[0][lane] = g.a; srec[1][lane] = g.b; srec[2][lane] = g.c; srec[3][lane] = g.d; }
+    uint32_t c0 = head.x, c1 = NO_CHUNK, c2 = NO_CHUNK, pos1 = 0u;
+    int n0 = (int)head.y, b = 0;
+    if (c0 != NO_CHUNK) {
+        const uint32_t pos0 = lane < n0 ? __ldg(L.ids + (size_t)c0 * 32 + lane) : 0u;
+        c1 = __ldg(L.link + c0);
+        gather64<false>(srt, pos0, n0, buf[0], lane);
+        if (c1 != NO_CHUNK) { pos1 = __ldg(L.ids + (size_t)c1 * 32 + lane); c2 = __ldg(L.link + c1); }   // linked chunks are full
+    }
+    while (c0 != NO_CHUNK) {
+        asm volatile("cp.async.wait_all;" ::: "memory");
         __syncwarp();
+        uint32_t pos2 = 0u, c3 = NO_CHUNK;
+        if (c1 != NO_CHUNK) gather64<false>(srt, pos1, 32, buf[b ^ 1], lane);
+        if (c2 != NO_CHUNK) { pos2 = __ldg(L.ids + (size_t)c2 * 32 + lane); c3 = __ldg(L.link + c2); }
+        const float4 *rb = buf[b];
 #pragma unroll 4
-        for (int j = 0; j < n; j++) {
+        for (int j = 0; j < n0; j++) {
             Rec q;
-            q.a = srec[0][j]; q.b = srec[1][j]; q.c = srec[2][j]; q.d = srec[3][j];
+            q.a = rb[4 * j]; q.b = rb[4 * j + 1]; q.c = rb[4 * j + 2]; q.d = rb[4 * j + 3];
             float u0, u1, u2;
             const float qd = mahalanobis(q, px, py, pz, u0, u1, u2);
             const bool hit = qd <= r2;
@@ -273,9 +296,9 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             Nacc = fmaf(q.b.w, wG, Nacc);
             if (SETS && hit) { const unsigned long long h = mix64(__float_as_uint(q.c.w)); cnt++; hsum += h; hxor ^= h; }
         }
-        if (SETS) tested += (uint32_t)n;
+        if (SETS) tested += (uint32_t)n0;
         __syncwarp();
-        chunk = link; pos = npos; link = nlink; n = 32;
+        c0 = c1; n0 = 32; c1 = c2; pos1 = pos2; c2 = c3; b ^= 1;
     }
     const bool active = pp.active;
     const uint64_t c = pp.c;
@@ -326,10 +349,12 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, BwdIn in, float *__restrict__ gacc) {
     __shared__ float4 pts_all[EVAL_WARPS][2][32];   // [0] x y z alpha   [1] beta eps - -
+    __shared__ float4 buf_all[EVAL_WARPS][2][128];  // two chunks of 32 records of 64 B, swizzled (see gather64)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
     if (packet * 32 >= P) return;
     float4 (*pts)[32] = pts_all[warp];
+    float4 (*buf)[128] = buf_all[warp];
     {
         const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
         // per-sample coefficients: alpha = covered ? a/I : 0, beta = b - alpha Phi, eps = covered ? |Phi - t|/I : 0
@@ -351,21 +376,27 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
         pts[1][lane] = make_float4(beta, eps, 0.f, 0.f);
         __syncwarp();
     }
+    // same software pipeline as the forward: records of chunk k+1 and ids of chunk k+2 are in flight during chunk k
     const uint2 head = __ldg(L.head + packet);
-    uint32_t chunk = head.x;
-    int n = (int)head.y;
-    uint32_t pos = (chunk != NO_CHUNK && lane < n) ? __ldg(L.ids + (size_t)chunk * 32 + lane) : 0u;
-    uint32_t link = chunk != NO_CHUNK ? __ldg(L.link + chunk) : NO_CHUNK;
-    Rec g;
-    if (chunk != NO_CHUNK && lane < n) {
-        const float4 *rp = srt + 4 * (size_t)pos;
-        g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
+    uint32_t c0 = head.x, c1 = NO_CHUNK, c2 = NO_CHUNK, pos1 = 0u;
+    int n0 = (int)head.y, b = 0;
+    if (c0 != NO_CHUNK) {
+        const uint32_t pos0 = lane < n0 ? __ldg(L.ids + (size_t)c0 * 32 + lane) : 0u;
+        c1 = __ldg(L.link + c0);
+        gather64<true>(srt, pos0, n0, buf[0], lane);
+        if (c1 != NO_CHUNK) { pos1 = __ldg(L.ids + (size_t)c1 * 32 + lane); c2 = __ldg(L.link + c1); }   // linked chunks are full
     }
-    while (chunk != NO_CHUNK) {
-        // the next chunk's ids and link are requested now; its records right after this chunk's loop is set up
-        const uint32_t npos = link != NO_CHUNK ? __ldg(L.ids + (size_t)link * 32 + lane) : 0u;
-        const uint32_t nlink = link != NO_CHUNK ? __ldg(L.link + link) : NO_CHUNK;
-        if (lane < n) {
+    while (c0 != NO_CHUNK) {
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncwarp();
+        uint32_t pos2 = 0u, c3 = NO_CHUNK;
+        if (c1 != NO_CHUNK) gather64<true>(srt, pos1, 32, buf[b ^ 1], lane);
+        if (c2 != NO_CHUNK) { pos2 = __ldg(L.ids + (size_t)c2 * 32 + lane); c3 = __ldg(L.link + c2); }
+        if (lane < n0) {
+            const float4 *rb = buf[b] + 4 * lane;
+            const int f = (lane >> 1) & 3;
+            Rec g;
+            g.a = rb[f]; g.b = rb[1 ^ f]; g.c = rb[2 ^ f]; g.d = rb[3 ^ f];
             float acc[12];
 #pragma unroll
             for (int q = 0; q < 12; q++) acc[q] = 0.f;
@@ -387,11 +418,8 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
                 red_add_v4(row + 8, acc[8], acc[9], acc[10], acc[11]);
             }
         }
-        chunk = link; pos = npos; link = nlink; n = 32;
-        if (chunk != NO_CHUNK) {
-            const float4 *rp = srt + 4 * (size_t)pos;
-            g.a = __ldg(rp); g.b = __ldg(rp + 1); g.c = __ldg(rp + 2); g.d = __ldg(rp + 3);
-        }
+        __syncwarp();
+        c0 = c1; n0 = 32; c1 = c2; pos1 = pos2; c2 = c3; b ^= 1;
     }
 }
 
