@@ -2,7 +2,8 @@
 configs[1] (C2): 256^3 Marschner-Lobb grid, 262,144 Gaussians, one whole-grid forward+backward.
 The oracle finishes this size in seconds (cell-grid cull, OpenMP), so every output is compared element
 by element: all 16.8 M intersection sets and the 2.56 M sorted pair keys bit-exact, Phi within 1e-5,
-every gradient tensor within 1e-4 relative L2."""
+every gradient tensor within 1e-4 relative L2.
+configs[2] (C3) is checked the same way on one 2^20-point batch (the oracle needs about a minute for it)."""
 import numpy as np
 import pytest
 
@@ -45,6 +46,40 @@ def test_c2_full_size(oracle):
     assert got["dscalar"].sum() == pytest.approx(a[covered].sum(), rel=1e-4, abs=1e-7)
     assert got["err"].sum() == pytest.approx(serr[covered].sum(), rel=1e-4)
     print("C2 full size: T", len(keys), "hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs)
+
+
+def test_c3_full_size(oracle):
+    # BASELINE.json configs[2] at full size: 2,000,000 points, 1,048,576 Gaussians, one 2^20-point batch without
+    # replacement, LBVH + query sort + cull lists rebuilt by gs_build_accel (what `bench.py --workload c3` times)
+    xyz_all, t_all = inputs.c3_points()
+    g = inputs.c3_gaussians(xyz_all, t_all)
+    idx = inputs.batch_indices(3, 0, len(xyz_all), 1 << 20)
+    xyz, target = np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])
+    dom = inputs.points_domain(xyz_all)
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+    run = GpuRun(g, "points", xyz, target, domain=dom, fused=True)
+    api = run.api
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    codes = oracle.morton_codes(g.mean, dom[0], dom[1], valid)
+    order, keys = oracle.morton_order(codes)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_MORTON, np.uint32), codes[order])
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_ORDER, np.uint32), order)
+    pcodes = oracle.morton_codes(xyz, dom[0], dom[1])
+    porder, _ = oracle.morton_order(pcodes)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_POINT_ORDER, np.uint32), porder)
+    tested, hits = check_sets(run, fwd)   # all 2^20 intersection sets, bit-exact
+    assert hits > 400_000_000
+    near, e_phi, e_I = check_forward(run, fwd)
+    assert near <= 16
+    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+    errs = check_grads(run, gr)
+    got = run.grads_np()
+    covered = fwd["I"].astype(np.float32) > np.float32(TAU)
+    assert got["dscalar"].sum() == pytest.approx(a[covered].sum(), rel=1e-4, abs=1e-7)
+    assert got["err"].sum() == pytest.approx(serr[covered].sum(), rel=1e-4)
+    print("C3 full size: hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs)
 
 
 def test_c4_like_batches(oracle):

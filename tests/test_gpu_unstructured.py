@@ -82,6 +82,58 @@ def test_c5_like_sparse_with_dI(oracle):
     check_grads(run, gr)
 
 
+def test_cull_pool_growth_and_context_reuse(oracle):
+    # every Gaussian reaches every packet: the per-packet lists (gs_build_accel) outgrow the initial pool, so the
+    # count-and-repeat path runs; then the same context serves a light query (lists shrink, pool is re-used)
+    rng = np.random.default_rng(11)
+    n = 1500
+    g = inputs.c1_gaussians(seed=12, n=n)
+    g.scale[:] = rng.uniform(0.3, 0.6, (n, 3)).astype(np.float32)
+    xyz = rng.uniform(0, 1, (20011, 3)).astype(np.float32)
+    target = rng.uniform(0, 1, len(xyz)).astype(np.float32)
+    dom = (np.zeros(3, np.float32), np.ones(3, np.float32))
+    fwd, loss, a, serr, gr = _oracle_all(oracle, g, xyz, target)
+    assert fwd["count"].astype(np.int64).sum() > 256 * len(xyz)   # more than the initial 256 list entries per point
+    run = GpuRun(g, "points", xyz, target, domain=dom)
+    check_sets(run, fwd)
+    check_forward(run, fwd)
+    check_grads(run, gr)
+    # light query on the same context
+    import torch
+    xyz2 = np.ascontiguousarray(xyz[:777])
+    q2 = run.api.points_query(torch.from_numpy(xyz2).cuda())
+    run.ctx.gs_build_accel(q2)
+    phi, I = torch.empty(777, device="cuda"), torch.empty(777, device="cuda")
+    run.ctx.gs_sample_fwd(q2, phi, I)
+    ref = oracle.forward(g, xyz2, TAU, mode=1)
+    assert np.abs(phi.cpu().numpy() - ref["phi"]).max() <= 1e-5
+    assert np.abs(I.cpu().numpy() - ref["I"]).max() <= 2e-5 * max(1.0, float(ref["I"].max()))
+
+
+def test_nonfinite_query_points(oracle):
+    # NaN / infinite coordinates: such a sample hits nothing (Phi = 0, I = 0) and must not disturb the finite
+    # samples that share its packet (their packet box then culls nothing)
+    rng = np.random.default_rng(4)
+    xyz_all, t_all = inputs.c3_points(seed=3, p=8000)
+    g = inputs.c3_gaussians(xyz_all, t_all, seed=3, n=3000, sigma_lo=0.01, sigma_hi=0.05)
+    xyz = np.ascontiguousarray(xyz_all[:2000]).copy()
+    bad = rng.choice(len(xyz), 40, replace=False)
+    xyz[bad[:15], 0] = np.nan
+    xyz[bad[15:30], 1] = np.inf
+    xyz[bad[30:], 2] = -np.inf
+    good = np.setdiff1d(np.arange(len(xyz)), bad)
+    dom = inputs.points_domain(xyz_all)
+    ref = oracle.forward(g, np.ascontiguousarray(xyz[good]), TAU, mode=0)
+    run = GpuRun(g, "points", xyz, None, domain=dom)
+    phi, I = run.np(run.phi), run.np(run.I)
+    assert np.all(phi[bad] == 0.0) and np.all(I[bad] == 0.0)
+    cnt, hs, hx, tested, hits = run.sets()
+    assert np.all(cnt[bad] == 0)
+    assert np.array_equal(cnt[good], ref["count"]) and np.array_equal(hs[good], ref["hsum"]) and np.array_equal(hx[good], ref["hxor"])
+    near = np.abs(ref["I"] - TAU) <= 2e-6 * TAU
+    assert np.abs(phi[good] - ref["phi"])[~near].max() <= 1e-5
+
+
 def test_degenerate_unstructured(oracle):
     rng = np.random.default_rng(2)
     dom = (np.zeros(3, np.float32), np.ones(3, np.float32))
