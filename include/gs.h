@@ -20,8 +20,8 @@
  *     what it needs into context-owned records).  The context owns all scratch (grow-only) and
  *     frees it in gs_destroy.
  *   - All work is enqueued on the stream given to gs_create.  Calls return after enqueueing,
- *     except that gs_build_accel for a grid synchronises once to read the pair count T, and
- *     gs_step_host / gs_debug_point_sets synchronise before returning.  Outputs are valid once the
+ *     except that gs_build_accel synchronises once (grid: to read the pair count T; points: to read
+ *     the size of the per-packet cull lists and grow their pool if needed), and gs_step_host / gs_debug_point_sets synchronise before returning.  Outputs are valid once the
  *     caller synchronises the stream.
  *   - Every call returns a gs_status; no exception or abort crosses the ABI.  Arguments are
  *     validated before any launch.  gs_last_error gives a human-readable message for the last
@@ -125,6 +125,10 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
  * Points (north_star (2); the paper uses a BVH over the samples instead):
  *   30-bit Morton codes of the Gaussian means in `dom`, radix sort of (code, id), Karras radix
  *   tree, bottom-up AABB refit; the query points are Morton-sorted for coherence unless presorted.
+ *   Then every packet of 32 consecutive sorted points walks the tree once (short stack in shared
+ *   memory) and its list of reachable Gaussians is stored for gs_sample_fwd AND gs_sample_bwd of this
+ *   query; the pool of list chunks is context-owned, grow-only, and sized by count-and-repeat.
+ *   The lists are conservative culls: membership is decided per pair by the canonical predicate (D4).
  * Errors: STATE (no preprocess; no domain for a point query), INVALID_ARG, OVERFLOW, OOM, CUDA. */
 gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
 
