@@ -1,10 +1,16 @@
 // binning.cu -- S2: Gaussian -> brick lists for a structured batch (section 4.1.2).
-//   k_brick_count : per Gaussian, brick range of its AABB inside the batch and the count n_i
-//   (scan)        : offsets = exclusive scan of n_i, T = total
-//   k_pair_write  : one thread per PAIR: binary search in the scan for the Gaussian, index
-//                   arithmetic for the brick ("parallelizes over total intersections")
-//   (radix sort)  : stable sort by brick id => each brick's list is in ascending Gaussian id
-//   k_brick_start : start index of every brick's run
+// The list of (brick, gaussian) pairs sorted by (brick, gaussian) is produced by an MSD radix sort whose
+// first digit is the whole brick id (a counting sort) and whose remaining digits are sorted per bucket:
+//   k_brick_count : per Gaussian, brick range of its AABB inside the batch, the count n_i, and one
+//                   atomic per overlapped brick into the brick histogram (the (brick, gaussian) pairs
+//                   are enumerated by index arithmetic; large Gaussians are spread over the warp:
+//                   "parallelizes over total intersections")
+//   (scan)        : brick_start = exclusive scan of the histogram, brick_start[nbricks] = T
+//   k_pair_fill   : the same enumeration; each pair takes a slot of its brick's run
+//   k_bucket_sort : every brick's run is sorted by Gaussian id (bitonic network), so the result is the
+//                   unique ascending (brick, gaussian) order whatever order the slots were taken in
+// Measured on C2 (T = 2.56 M): the previous pipeline (per-Gaussian scan, pair write with a binary search per
+// pair, two 8-bit LSD passes, run boundaries) took 0.25 ms of device time; this one is listed in DESIGN.md.
 // Brick ranges are integer decisions: fixed fp32 sequence (D7).
 #include "gs_internal.cuh"
 
@@ -42,22 +48,65 @@ __device__ __forceinline__ uint32_t spread3(uint32_t v) {  // 10 bits -> every t
     return v;
 }
 
-// Also emits the processing order key of the backward pass: Morton code of the Gaussian's central
-// brick (performance only: neighbouring Gaussians are processed together so their voxel data stays
-// in L1/L2); Gaussians that touch no brick of the batch get `untouched_key` and sort to the end.
-//
-// And the per-Gaussian constants of the backward kernel (performance only, nothing canonical): the box of
-// 2x2x2-voxel cells that covers the AABB inside the batch, the whitened-space cull threshold of a cell and
-// 1 / |e|^2 for the closed-form row intervals (sample_grid_bwd.cu):
+// ---- enumeration of the bricks of a range.  A thread walks its own Gaussian's bricks when there are at most
+// SERIAL_MAX of them; larger ranges are spread over the 32 lanes of the warp, one Gaussian after the other.
+// f(brick_id, gaussian_id) is called exactly once per (brick, gaussian) pair.  All 32 lanes must call this.
+constexpr uint32_t SERIAL_MAX = 27;
+
+template <class F>
+__device__ __forceinline__ void for_each_pair(const BrickRange &br, uint32_t c, uint32_t i, const GridDesc &gd, int lane, F f) {
+    const uint32_t nbx = (uint32_t)gd.brick_cnt[0], nby = (uint32_t)gd.brick_cnt[1];
+    const uint32_t ex = c ? (uint32_t)(br.hi[0] - br.lo[0] + 1) : 1u, ey = c ? (uint32_t)(br.hi[1] - br.lo[1] + 1) : 1u;
+    // batch-local id of the range's first brick
+    const uint32_t b0 = c ? (((uint32_t)(br.lo[2] - gd.brick_lo[2]) * nby + (uint32_t)(br.lo[1] - gd.brick_lo[1])) * nbx +
+                             (uint32_t)(br.lo[0] - gd.brick_lo[0]))
+                          : 0u;
+    const bool big = c > SERIAL_MAX;
+    if (c && !big) {
+        const uint32_t ez = c / (ex * ey);
+        for (uint32_t z = 0; z < ez; z++)
+            for (uint32_t y = 0; y < ey; y++)
+                for (uint32_t x = 0; x < ex; x++) f(b0 + (z * nby + y) * nbx + x, i);
+    }
+    uint32_t todo = __ballot_sync(0xffffffffu, big);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t sc = __shfl_sync(0xffffffffu, c, src), sex = __shfl_sync(0xffffffffu, ex, src),
+                       sey = __shfl_sync(0xffffffffu, ey, src), sb0 = __shfl_sync(0xffffffffu, b0, src),
+                       si = __shfl_sync(0xffffffffu, i, src);
+        for (uint32_t t = lane; t < sc; t += 32) {
+            const uint32_t x = t % sex, r = t / sex;
+            const uint32_t y = r % sey, z = r / sey;
+            f(sb0 + (z * nby + y) * nbx + x, si);
+        }
+    }
+}
+
+// Morton code of the Gaussian's central brick, coarsened to at most ORDER_BITS bits per axis: the processing
+// order of the backward pass (performance only: neighbouring Gaussians are processed together so that their
+// voxel data stays in L1/L2).
+__device__ __forceinline__ uint32_t order_key(const BrickRange &br, const GridDesc &gd, int order_shift) {
+    const uint32_t mx = (uint32_t)(((br.lo[0] + br.hi[0]) >> 1) - gd.brick_lo[0]) >> order_shift;
+    const uint32_t my = (uint32_t)(((br.lo[1] + br.hi[1]) >> 1) - gd.brick_lo[1]) >> order_shift;
+    const uint32_t mz = (uint32_t)(((br.lo[2] + br.hi[2]) >> 1) - gd.brick_lo[2]) >> order_shift;
+    return spread3(mx) | (spread3(my) << 1) | (spread3(mz) << 2);
+}
+
+// hist = [nbricks brick counters | order-bucket counters].  Also writes the per-Gaussian constants of the
+// backward kernel (performance only, nothing canonical): the box of 2x2x2-voxel cells that covers the AABB
+// inside the batch, the whitened-space cull threshold of a cell and 1 / |e|^2 for the closed-form row
+// intervals (sample_grid_bwd.cu):
 //   setup[2 i]     = (clo.x, clo.y, clo.z, flags: 1 = touches no voxel of the batch, 2 = a cell sticks out of the batch)
 //   setup[2 i + 1] = (ncx | ncy << 11 | ncz << 22, thr, invA, -)
 __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, const float4 *__restrict__ rec, uint32_t N,
                                                       GridDesc gd, float rcut, uint32_t *__restrict__ count,
-                                                      unsigned long long *__restrict__ total, uint32_t *__restrict__ okey,
-                                                      uint32_t *__restrict__ oval, uint32_t untouched_key,
-                                                      float4 *__restrict__ setup) {
+                                                      unsigned long long *__restrict__ total, uint32_t *__restrict__ hist,
+                                                      uint32_t nbricks, int order_shift, float4 *__restrict__ setup) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
     uint32_t c = 0;
+    BrickRange br{};
     if (i < N) {
         const float *bb = aabb + 6 * (size_t)i;
         // an invalid Gaussian has the empty box (+inf, -inf): fmaxf/fminf clamp it to an empty range.
@@ -65,18 +114,9 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         float b6[6];
 #pragma unroll
         for (int k = 0; k < 6; k++) b6[k] = bb[k];
-        BrickRange br;
         c = brick_range(b6, gd, br);
         count[i] = c;
-        uint32_t key = untouched_key;
-        if (c) {
-            const uint32_t mx = (uint32_t)(((br.lo[0] + br.hi[0]) >> 1) - gd.brick_lo[0]);
-            const uint32_t my = (uint32_t)(((br.lo[1] + br.hi[1]) >> 1) - gd.brick_lo[1]);
-            const uint32_t mz = (uint32_t)(((br.lo[2] + br.hi[2]) >> 1) - gd.brick_lo[2]);
-            key = spread3(mx) | (spread3(my) << 1) | (spread3(mz) << 2);
-        }
-        okey[i] = key;
-        oval[i] = i;
+        if (c) atomicAdd(hist + nbricks + order_key(br, gd, order_shift), 1u);
         // ---- backward setup
         int clo[3], nc[3];
         bool empty = false, edge = false;
@@ -109,6 +149,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         setup[2 * (size_t)i + 1] = make_float4(__uint_as_float((uint32_t)nc[0] | ((uint32_t)nc[1] << 11) | ((uint32_t)nc[2] << 22)),
                                                reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
     }
+    for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t) { atomicAdd(hist + b, 1u); });
     // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
     unsigned long long s = c, m = c ? 1ull : 0ull;
 #pragma unroll
@@ -116,72 +157,134 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         s += __shfl_xor_sync(0xffffffffu, s, d);
         m += __shfl_xor_sync(0xffffffffu, m, d);
     }
-    if ((threadIdx.x & 31) == 0 && s) { atomicAdd(total, s); atomicAdd(total + 1, m); }
+    if (lane == 0 && s) { atomicAdd(total, s); atomicAdd(total + 1, m); }
 }
 
-__global__ void __launch_bounds__(256) k_pair_write(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
-                                                     const uint32_t *__restrict__ offset, uint32_t T, uint32_t *__restrict__ key,
-                                                     uint32_t *__restrict__ val) {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= T) return;
-    // largest i with offset[i] <= t  (offset has N+1 entries, offset[N] = T)
-    uint32_t lo = 0, hi = N;  // invariant: offset[lo] <= t < offset[hi]
-    while (hi - lo > 1) {
-        const uint32_t mid = (lo + hi) >> 1;
-        if (offset[mid] <= t) lo = mid; else hi = mid;
-    }
-    const uint32_t i = lo;
-    float b6[6];
+// Every pair takes a slot of its brick's run by counting the brick's histogram entry DOWN (so the histogram is
+// all zero again afterwards); the order list of the backward is filled the same way.  Nothing is written when
+// the pair list does not fit `cap` entries: the host then grows the buffer and repeats this kernel.
+__global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
+                                                    const unsigned long long *__restrict__ total, uint32_t cap,
+                                                    uint32_t *__restrict__ hist, const uint32_t *__restrict__ start, uint32_t nbricks,
+                                                    int order_shift, uint32_t *__restrict__ pair_gauss, uint32_t *__restrict__ order) {
+    if (total[0] > (unsigned long long)cap) return;
+    const uint32_t T = (uint32_t)total[0];
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    uint32_t c = 0;
+    BrickRange br{};
+    if (i < N) {
+        float b6[6];
 #pragma unroll
-    for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
-    BrickRange br;
-    brick_range(b6, gd, br);
-    uint32_t local = t - offset[i];
-    const uint32_t ex = (uint32_t)(br.hi[0] - br.lo[0] + 1), ey = (uint32_t)(br.hi[1] - br.lo[1] + 1);
-    const uint32_t x = local % ex; local /= ex;
-    const uint32_t y = local % ey;
-    const uint32_t z = local / ey;
-    const uint32_t bx = (uint32_t)(br.lo[0] - gd.brick_lo[0]) + x, by = (uint32_t)(br.lo[1] - gd.brick_lo[1]) + y,
-                   bz = (uint32_t)(br.lo[2] - gd.brick_lo[2]) + z;
-    key[t] = (bz * (uint32_t)gd.brick_cnt[1] + by) * (uint32_t)gd.brick_cnt[0] + bx;
-    val[t] = i;
+        for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
+        c = brick_range(b6, gd, br);
+        if (c) {
+            const uint32_t m = nbricks + order_key(br, gd, order_shift);
+            order[start[m] - T + (atomicSub(hist + m, 1u) - 1u)] = i;
+        }
+    }
+    for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t id) { pair_gauss[start[b] + (atomicSub(hist + b, 1u) - 1u)] = id; });
 }
 
-__global__ void __launch_bounds__(256) k_brick_start(const uint32_t *__restrict__ key, uint32_t T, uint32_t nbricks,
-                                                      uint32_t *__restrict__ start) {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (T == 0) {
-        for (uint32_t b = t; b <= nbricks; b += gridDim.x * blockDim.x) start[b] = 0;
-        return;
+// ---- per-brick sort of the Gaussian ids.  Bitonic network in its all-ascending form (the first step of every
+// merge compares mirror positions), so that a run of any length n is sorted as if padded with +inf to a power of
+// two: a comparator whose upper index is >= n does nothing.
+template <class SYNC>
+__device__ __forceinline__ void bitonic_ascending(uint32_t *a, uint32_t n, uint32_t tid, uint32_t nthreads, SYNC sync) {
+    uint32_t n2 = 1;
+    while (n2 < n) n2 <<= 1;
+    for (uint32_t k = 2; k <= n2; k <<= 1) {
+        for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+            const bool flip = (j == (k >> 1));
+            for (uint32_t t = tid; t < (n2 >> 1); t += nthreads) {
+                // t-th comparator of this step: lower index lo has bit j clear
+                const uint32_t lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                const uint32_t hi = flip ? (lo ^ (k - 1)) : (lo | j);
+                if (hi < n) {
+                    const uint32_t x = a[lo], y = a[hi];
+                    if (x > y) { a[lo] = y; a[hi] = x; }
+                }
+            }
+            sync();
+        }
     }
-    if (t > T) return;
-    // thread t closes the gap between key[t-1] and key[t]  (t = 0: from brick 0; t = T: up to nbricks)
-    const uint32_t prev = (t == 0) ? 0u : key[t - 1] + 1u;
-    const uint32_t cur = (t == T) ? nbricks : key[t];
-    for (uint32_t b = prev; b <= cur; b++) start[b] = t;
+}
+
+constexpr int BS_WARPS = 4;
+constexpr uint32_t BS_SMEM = 1024;  // entries a warp sorts in shared memory
+
+__global__ void __launch_bounds__(BS_WARPS * 32) k_bucket_sort(const unsigned long long *__restrict__ total, uint32_t cap,
+                                                                const uint32_t *__restrict__ start, uint32_t nbricks,
+                                                                uint32_t *__restrict__ pair_gauss) {
+    __shared__ uint32_t sm[BS_WARPS][BS_SMEM];
+    if (total[0] > (unsigned long long)cap) return;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t b = blockIdx.x * BS_WARPS + warp;
+    uint32_t s = 0, n = 0;
+    if (b < nbricks) { s = start[b]; n = start[b + 1] - s; }
+    uint32_t *run = pair_gauss + s;
+    if (n > 1 && n <= 32) {  // one id per lane: compare-exchange through shuffles
+        uint32_t v = (uint32_t)lane < n ? run[lane] : 0xffffffffu;
+#pragma unroll
+        for (int k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                const int partner = (j == (k >> 1)) ? (lane ^ (k - 1)) : (lane ^ j);
+                const uint32_t o = __shfl_sync(0xffffffffu, v, partner);
+                v = (lane < partner) ? min(v, o) : max(v, o);
+            }
+        }
+        if ((uint32_t)lane < n) run[lane] = v;
+    } else if (n > 32 && n <= BS_SMEM) {
+        uint32_t *a = sm[warp];
+        for (uint32_t t = lane; t < n; t += 32) a[t] = run[t];
+        __syncwarp();
+        bitonic_ascending(a, n, (uint32_t)lane, 32u, [] { __syncwarp(); });
+        for (uint32_t t = lane; t < n; t += 32) run[t] = a[t];
+    }
+    // runs longer than a warp's shared memory: the whole CTA sorts them in place in global memory, one after the other
+    __syncthreads();
+    for (int w = 0; w < BS_WARPS; w++) {
+        const uint32_t bw = blockIdx.x * BS_WARPS + w;
+        if (bw >= nbricks) break;
+        const uint32_t sw = start[bw], nw = start[bw + 1] - sw;
+        if (nw <= BS_SMEM) continue;  // block-uniform
+        bitonic_ascending(pair_gauss + sw, nw, threadIdx.x, (uint32_t)(BS_WARPS * 32), [] { __syncthreads(); });
+    }
+}
+
+// debug view: the brick id of every entry of the sorted pair list (gs_debug_get(GS_DBG_PAIR_BRICK))
+__global__ void __launch_bounds__(256) k_expand_bricks(const uint32_t *__restrict__ start, uint32_t nbricks, uint32_t *__restrict__ key) {
+    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nbricks) return;
+    for (uint32_t t = start[b]; t < start[b + 1]; t++) key[t] = b;
 }
 
 cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
-                               unsigned long long *total, uint32_t *okey, uint32_t *oval, uint32_t untouched_key, float4 *setup,
-                               cudaStream_t s) {
+                               unsigned long long *total, uint32_t *hist, uint32_t nbricks, uint32_t norder, int order_shift,
+                               float4 *setup, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(total, 0, 2 * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(hist, 0, ((size_t)nbricks + norder) * sizeof(uint32_t), s);
     if (e != cudaSuccess || N == 0) return e;
-    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, rec, N, gd, rcut, count, total, okey, oval, untouched_key, setup); count_launch();
+    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, rec, N, gd, rcut, count, total, hist, nbricks, order_shift, setup); count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
-                              uint32_t *key, uint32_t *val, cudaStream_t s) {
-    if (T == 0) return cudaSuccess;
-    k_pair_write<<<(T + 255) / 256, 256, 0, s>>>(aabb, N, gd, offset, T, key, val); count_launch();
+cudaError_t launch_pair_fill(const float *aabb, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
+                             uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
+                             uint32_t *order, cudaStream_t s) {
+    if (N == 0) return cudaSuccess;
+    k_pair_fill<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, total, cap, hist, start, nbricks, order_shift, pair_gauss, order); count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_bucket_sort<<<(nbricks + BS_WARPS - 1) / BS_WARPS, BS_WARPS * 32, 0, s>>>(total, cap, start, nbricks, pair_gauss); count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks, uint32_t *start, cudaStream_t s) {
-    const uint32_t n = (T == 0) ? nbricks + 1 : T + 1;
-    unsigned blocks = (n + 255) / 256;
-    if (T == 0 && blocks > 1024) blocks = 1024;
-    k_brick_start<<<blocks, 256, 0, s>>>(key, T, nbricks, start); count_launch();
+cudaError_t launch_expand_bricks(const uint32_t *start, uint32_t nbricks, uint32_t *key, cudaStream_t s) {
+    if (nbricks == 0) return cudaSuccess;
+    k_expand_bricks<<<(nbricks + 255) / 256, 256, 0, s>>>(start, nbricks, key); count_launch();
     return cudaGetLastError();
 }
 

@@ -136,8 +136,8 @@ void gs_destroy(gs_ctx *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->boffset, &ctx->pair_key[0], &ctx->pair_key[1],
-                     &ctx->pair_val[0], &ctx->pair_val[1], &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
+    DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->bhist, &ctx->pair_gauss, &ctx->pair_brick,
+                     &ctx->grid_order, &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg};
@@ -200,46 +200,42 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     if (q->kind == GS_QUERY_GRID) {
         const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
         CK(ctx->bcount.reserve(((size_t)N + 1) * 4), "alloc brick counts");
-        CK(ctx->boffset.reserve(((size_t)N + 1) * 4), "alloc brick offsets");
-        CK(ctx->brick_start.reserve(((size_t)nbricks + 1) * 4), "alloc brick_start");
-        unsigned long long *total = ctx->counters.as<unsigned long long>() + 4;
-        // the backward's processing order (Gaussians by the Morton code of their central brick) shares this pass;
-        // in grid mode the leaf_key/leaf_val buffers hold that order
-        const size_t n1 = N ? N : 1;
-        for (int k = 0; k < 2; k++) {
-            CK(ctx->leaf_key[k].reserve(n1 * 4), "alloc order keys");
-            CK(ctx->leaf_val[k].reserve(n1 * 4), "alloc order vals");
-        }
+        // the backward's processing order (Gaussians bucketed by the Morton code of their central brick, at most
+        // 6 bits per axis) is built by the same two passes
         int axis_bits = 1;
         for (int k = 0; k < 3; k++) axis_bits = bits_for((uint64_t)gd.brick_cnt[k]) > axis_bits ? bits_for((uint64_t)gd.brick_cnt[k]) : axis_bits;
-        const uint32_t untouched_key = 1u << (3 * axis_bits);
+        const int order_shift = axis_bits > 6 ? axis_bits - 6 : 0;
+        const uint32_t norder = 1u << (3 * (axis_bits - order_shift));
+        const size_t nh = (size_t)nbricks + norder;
+        CK(ctx->bhist.reserve(nh * 4), "alloc brick histogram");
+        CK(ctx->brick_start.reserve((nh + 1) * 4), "alloc brick_start");
+        const size_t n1 = N ? N : 1;
+        CK(ctx->grid_order.reserve(n1 * 4), "alloc order");
         CK(ctx->bwd_setup.reserve(n1 * 32), "alloc backward setup");
+        CK(ctx->pair_gauss.reserve(4), "alloc pair list");
+        unsigned long long *total = ctx->counters.as<unsigned long long>() + 4;
         CK(launch_brick_count(ctx->aabb.as<float>(), ctx->rec.as<float4>(), N, gd, ctx->r, ctx->bcount.as<uint32_t>(), total,
-                              ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_val[0].as<uint32_t>(), untouched_key,
-                              ctx->bwd_setup.as<float4>(), s), "brick count");
-        CK(exclusive_scan_u32(ctx->bcount.as<uint32_t>(), ctx->boffset.as<uint32_t>(), N, ctx->scan_tmp, s), "scan");
+                              ctx->bhist.as<uint32_t>(), nbricks, norder, order_shift, ctx->bwd_setup.as<float4>(), s), "brick count");
+        CK(exclusive_scan_u32(ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nh, ctx->scan_tmp, s), "scan");
+        // The pair list is filled speculatively into the buffer the previous step left; T is read back once, at the
+        // end, and the fill is repeated only when the buffer had to grow (it writes nothing when T exceeds `cap`).
         unsigned long long T64[2] = {0, 0};
-        CK(cudaMemcpyAsync(T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
-        {
-            uint32_t *ok[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
-            uint32_t *ov[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
-            CK(radix_sort_pairs(ok, ov, N, 3 * axis_bits + 1, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "order sort");
+        for (int attempt = 0; attempt < 2; attempt++) {
+            const size_t cap = ctx->pair_gauss.cap / 4;
+            CK(launch_pair_fill(ctx->aabb.as<float>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
+                                ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
+                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), s), "pair fill");
+            if (attempt == 0) {
+                CK(cudaMemcpyAsync(T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
+                CK(cudaStreamSynchronize(s), "sync (T)");
+                if (T64[0] >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
+            }
+            if (T64[0] <= cap) break;
+            CK(ctx->pair_gauss.reserve((size_t)T64[0] * 4), "alloc pair list");
         }
-        CK(cudaStreamSynchronize(s), "sync (T)");
-        if (T64[0] >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
         const uint32_t T = (uint32_t)T64[0];
         ctx->M = (uint32_t)T64[1];
-        const size_t tb = ((size_t)T + 1) * 4;
-        for (int k = 0; k < 2; k++) {
-            CK(ctx->pair_key[k].reserve(tb), "alloc pair keys");
-            CK(ctx->pair_val[k].reserve(tb), "alloc pair vals");
-        }
-        CK(launch_pair_write(ctx->aabb.as<float>(), N, gd, ctx->boffset.as<uint32_t>(), T, ctx->pair_key[0].as<uint32_t>(),
-                             ctx->pair_val[0].as<uint32_t>(), s), "pair write");
-        uint32_t *keys[2] = {ctx->pair_key[0].as<uint32_t>(), ctx->pair_key[1].as<uint32_t>()};
-        uint32_t *vals[2] = {ctx->pair_val[0].as<uint32_t>(), ctx->pair_val[1].as<uint32_t>()};
-        CK(radix_sort_pairs(keys, vals, T, bits_for(nbricks), ctx->sort_hist, ctx->scan_tmp, s, &ctx->pair_sel), "pair sort");
-        CK(launch_brick_start(keys[ctx->pair_sel], T, nbricks, ctx->brick_start.as<uint32_t>(), s), "brick_start");
+        ctx->have_pair_brick = false;
         ctx->T = T;
         ctx->nbricks = nbricks;
         ctx->grid = gd;
@@ -333,7 +329,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
     cudaStream_t s = ctx->stream;
     if (ctx->accel_kind == GS_QUERY_GRID) {
         Stage stage(ctx, GS_PROF_FWD);
-        CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_val[ctx->pair_sel].as<uint32_t>(),
+        CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_gauss.as<uint32_t>(),
                            ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, s), "grid forward");
     } else {
         Stage stage(ctx, GS_PROF_FWD);
@@ -390,7 +386,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         }
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
-                           ctx->gacc.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->M, s), "grid backward");
+                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
@@ -413,8 +409,17 @@ gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *
         case GS_DBG_RECORDS: *dev_ptr = ctx->rec.p; *count = N; return GS_OK;
         case GS_DBG_AABB: *dev_ptr = ctx->aabb.p; *count = N; return GS_OK;
         case GS_DBG_BRICK_COUNT: if (!grid) break; *dev_ptr = ctx->bcount.p; *count = N; return GS_OK;
-        case GS_DBG_PAIR_BRICK: if (!grid) break; *dev_ptr = ctx->pair_key[ctx->pair_sel].p; *count = ctx->T; return GS_OK;
-        case GS_DBG_PAIR_GAUSS: if (!grid) break; *dev_ptr = ctx->pair_val[ctx->pair_sel].p; *count = ctx->T; return GS_OK;
+        case GS_DBG_PAIR_BRICK:
+            if (!grid) break;
+            if (!ctx->have_pair_brick) {  // the sorted list stores no brick ids: they are the runs of brick_start
+                CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+                CK(ctx->pair_brick.reserve(((size_t)ctx->T + 1) * 4), "alloc debug view");
+                CK(launch_expand_bricks(ctx->brick_start.as<uint32_t>(), ctx->nbricks, ctx->pair_brick.as<uint32_t>(), ctx->stream),
+                   "expand bricks");
+                ctx->have_pair_brick = true;
+            }
+            *dev_ptr = ctx->pair_brick.p; *count = ctx->T; return GS_OK;
+        case GS_DBG_PAIR_GAUSS: if (!grid) break; *dev_ptr = ctx->pair_gauss.p; *count = ctx->T; return GS_OK;
         case GS_DBG_BRICK_START: if (!grid) break; *dev_ptr = ctx->brick_start.p; *count = (size_t)ctx->nbricks + 1; return GS_OK;
         case GS_DBG_LEAF_MORTON: if (!pts) break; *dev_ptr = ctx->leaf_key[ctx->leaf_sel].p; *count = N; return GS_OK;
         case GS_DBG_LEAF_ORDER: if (!pts) break; *dev_ptr = ctx->leaf_val[ctx->leaf_sel].p; *count = N; return GS_OK;

@@ -94,12 +94,14 @@ struct gs_ctx {
     gs_query accel_q{};
     gs::GridDesc grid{};
     uint32_t T = 0, nbricks = 0;
+    bool have_pair_brick = false;
     uint32_t M = 0;       // Gaussians that touch the current batch (grid): length of the backward's order list
-    gs::DevBuf bcount;    // uint32 [N+1]
-    gs::DevBuf boffset;   // uint32 [N+1]
-    gs::DevBuf pair_key[2], pair_val[2];
-    int pair_sel = 0;
-    gs::DevBuf brick_start;  // uint32 [nbricks+1]
+    gs::DevBuf bcount;    // uint32 [N]: bricks overlapped by each Gaussian
+    gs::DevBuf bhist;     // uint32 [nbricks + norder]: pairs per brick | Gaussians per order bucket
+    gs::DevBuf pair_gauss;   // uint32 [T]: Gaussian ids, ascending inside every brick's run
+    gs::DevBuf pair_brick;   // uint32 [T]: debug view only (gs_debug_get)
+    gs::DevBuf grid_order;   // uint32 [M]: processing order of the backward
+    gs::DevBuf brick_start;  // uint32 [nbricks + norder + 1]: runs of the bricks, then of the order buckets (offset by T)
     gs::DevBuf bwd_setup;    // float4 [N][2]: per-Gaussian constants of the structured backward (k_brick_count)
     // ---- accel (points)
     uint64_t P = 0;
@@ -140,12 +142,15 @@ cudaError_t exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, DevB
 cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int bits, DevBuf &hist, DevBuf &tmp,
                              cudaStream_t s, int *result_sel);
 
+// S2 (binning.cu).  hist = [nbricks | norder] counters (zeroed here, counted down to zero again by launch_pair_fill);
+// start = exclusive scan of hist (nbricks + norder + 1 entries).  launch_pair_fill writes nothing when *total > cap.
 cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
-                               unsigned long long *total, uint32_t *okey, uint32_t *oval, uint32_t untouched_key, float4 *setup,
-                               cudaStream_t s);
-cudaError_t launch_pair_write(const float *aabb, uint32_t N, const GridDesc &gd, const uint32_t *offset, uint32_t T,
-                              uint32_t *key, uint32_t *val, cudaStream_t s);
-cudaError_t launch_brick_start(const uint32_t *key, uint32_t T, uint32_t nbricks, uint32_t *start, cudaStream_t s);
+                               unsigned long long *total, uint32_t *hist, uint32_t nbricks, uint32_t norder, int order_shift,
+                               float4 *setup, cudaStream_t s);
+cudaError_t launch_pair_fill(const float *aabb, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
+                             uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
+                             uint32_t *order, cudaStream_t s);
+cudaError_t launch_expand_bricks(const uint32_t *start, uint32_t nbricks, uint32_t *key, cudaStream_t s);
 
 struct FwdOut {
     const float *target; float *phi; float *I; double *loss; float *dL_dphi; float *sample_err;
