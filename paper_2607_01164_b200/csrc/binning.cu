@@ -216,7 +216,7 @@ constexpr uint32_t BS_SMEM = 1024;  // entries a warp sorts in shared memory
 __global__ void __launch_bounds__(BS_WARPS * 32) k_bucket_sort(const unsigned long long *__restrict__ total, uint32_t cap,
                                                                 const uint32_t *__restrict__ start, uint32_t nbricks,
                                                                 uint32_t *__restrict__ pair_gauss) {
-    __shared__ uint32_t sm[BS_WARPS][BS_SMEM];
+    __shared__ __align__(16) uint32_t sm[BS_WARPS][BS_SMEM];
     if (total[0] > (unsigned long long)cap) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t b = blockIdx.x * BS_WARPS + warp;
@@ -235,7 +235,31 @@ __global__ void __launch_bounds__(BS_WARPS * 32) k_bucket_sort(const unsigned lo
             }
         }
         if ((uint32_t)lane < n) run[lane] = v;
-    } else if (n > 32 && n <= BS_SMEM) {
+    } else if (n > 32 && n <= 128) {
+        // rank sort: the ids of a run are distinct, so an id's place is the number of smaller ids.  A lane owns up to
+        // four ids and counts against the whole run, read four at a time as a broadcast from shared memory.
+        uint32_t *a = sm[warp];
+        uint32_t v[4];
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            const uint32_t t = (uint32_t)lane + 32u * r;
+            v[r] = t < n ? run[t] : 0xffffffffu;
+            a[t] = v[r];  // the padding (+inf) is never smaller than an id
+        }
+        __syncwarp();
+        uint32_t rank[4] = {0u, 0u, 0u, 0u};
+        const uint4 *a4 = reinterpret_cast<const uint4 *>(a);
+        const uint32_t groups = (n + 3) >> 2;
+        for (uint32_t t = 0; t < groups; t++) {
+            const uint4 q = a4[t];
+#pragma unroll
+            for (int r = 0; r < 4; r++)
+                if (32u * r < n) rank[r] += (q.x < v[r]) + (q.y < v[r]) + (q.z < v[r]) + (q.w < v[r]);  // warp-uniform test
+        }
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+            if ((uint32_t)lane + 32u * r < n) run[rank[r]] = v[r];
+    } else if (n > 128 && n <= BS_SMEM) {
         uint32_t *a = sm[warp];
         for (uint32_t t = lane; t < n; t += 32) a[t] = run[t];
         __syncwarp();

@@ -375,7 +375,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
     if (N == 0) return GS_OK;
-    CK(ctx->gacc.reserve((size_t)N * GACC * 4), "alloc gradient accumulator");
+    CK(ctx->gacc.reserve((size_t)N * GACC_GRID * 4), "alloc gradient accumulator");
     BwdIn in{phi, I, dL_dphi, dL_dI, target, fused ? ctx->misc.as<float2>() : nullptr, 0.5f * (float)ctx->P};
     if (ctx->accel_kind == GS_QUERY_GRID) {
         if (!fused) {
@@ -385,7 +385,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
             CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
         }
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, in.eps_scale, ctx->r2,
+        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, ctx->r2,
                            ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, s), "grid backward");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
@@ -395,7 +395,9 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
                              ctx->r2, in, ctx->gacc.as<float>(), s), "points backward");
     }
     Stage stage(ctx, GS_PROF_FINALIZE);
-    CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, *out, s), "finalize");
+    const bool grid = ctx->accel_kind == GS_QUERY_GRID;
+    CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused) ? in.eps_scale : 1.f,
+                       *out, s), "finalize");
     return GS_OK;
 }
 

@@ -15,6 +15,7 @@ constexpr int BRICK = 8;            // bricks of 8^3 voxels (north_star (3))
 constexpr int BRICK_VOX = 512;
 constexpr int GACC = 16;            // floats per Gaussian in the gradient accumulator (13 used)
 // gacc layout: 0 dv | 1 dw | 2..4 U | 5..10 W00 W01 W02 W11 W12 W22 | 11 E | 12..15 unused
+constexpr int GACC_GRID = 32;       // the structured backward writes a row of moment sums instead (sample_grid_bwd.cu)
 
 // Grow-only device buffer owned by the context.
 struct DevBuf {
@@ -168,10 +169,12 @@ cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, c
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);
 
-cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
-                            cudaStream_t s);
+// grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the
+// cell steps are folded in); eps_scale multiplies the error share (fused MSE: eps = |alpha| * eps_scale, else 1)
+cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
+                            float eps_scale, const gs_grads &out, cudaStream_t s);
 
 // LBVH
 cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *aabb_valid /*nullable: aabb[N][6]*/, size_t n,

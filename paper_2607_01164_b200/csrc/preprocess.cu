@@ -96,15 +96,52 @@ cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float
 //   dqhat = <dR, dR/dqhat>;  dq = (dqhat - qhat (qhat . dqhat)) / |q|        (chain rule of Eq. 3)
 // Values only (no integer decision depends on them), so plain fp32 with FMA contraction.
 // ------------------------------------------------------------------------------------------------
+// MOMENTS: gacc holds the structured backward's rows of moment sums (layout in sample_grid_bwd.cu) with the
+// weight w factored out.  With E_a = column a of M:
+//   U = A + sum_a s1_a E_a;   W = Q + sum_a (E_a B_a^T + B_a E_a^T) + sum_{a<=b} s2_ab (E_a E_b^T + E_b E_a^T) / (1 + [a = b])
+template <bool MOMENTS>
 __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
-                                                   const float *__restrict__ gacc, uint32_t N, gs_grads out) {
+                                                   const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const float4 *ga = reinterpret_cast<const float4 *>(gacc) + 4 * (size_t)i;
-    const float4 g0 = ga[0], g1 = ga[1], g2 = ga[2];
-    const float dv = g0.x, dw = g0.y;
-    const float U[3] = {g0.z, g0.w, g1.x};
-    const float W00 = g1.y, W01 = g1.z, W02 = g1.w, W11 = g2.x, W12 = g2.y, W22 = g2.z, E = g2.w;
+    float dv, dw, E, U[3], W00, W01, W02, W11, W12, W22;
+    if (MOMENTS) {
+        const float4 *ga = reinterpret_cast<const float4 *>(gacc) + (GACC_GRID / 4) * (size_t)i;
+        float m[32];
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            const float4 t = ga[k];
+            m[4 * k] = t.x; m[4 * k + 1] = t.y; m[4 * k + 2] = t.z; m[4 * k + 3] = t.w;
+        }
+        const float4 r0 = rec[i], r1 = rec[(size_t)N + i], r2 = rec[2 * (size_t)N + i], r3 = rec[3 * (size_t)N + i];
+        const float w = r0.w;
+        const float Ec[3][3] = {{r1.x, r2.x, r3.x}, {r1.y, r2.y, r3.y}, {r1.z, r2.z, r3.z}};  // Ec[a] = column a of M
+        float Wm[3][3];
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            U[j] = m[3 + j] + m[6] * Ec[0][j] + m[7] * Ec[1][j] + m[8] * Ec[2][j];
+#pragma unroll
+            for (int k = j; k < 3; k++) {
+                const int q = j == 0 ? k : (j == 1 ? 2 + k : 5);  // 00 01 02 11 12 22
+                float t = m[9 + q];
+#pragma unroll
+                for (int a = 0; a < 3; a++) t += Ec[a][j] * m[15 + 3 * a + k] + m[15 + 3 * a + j] * Ec[a][k];
+                t += m[24] * Ec[0][j] * Ec[0][k] + m[25] * Ec[1][j] * Ec[1][k] + m[26] * Ec[2][j] * Ec[2][k];
+                t += m[27] * (Ec[0][j] * Ec[1][k] + Ec[1][j] * Ec[0][k]) + m[28] * (Ec[0][j] * Ec[2][k] + Ec[2][j] * Ec[0][k]) +
+                     m[29] * (Ec[1][j] * Ec[2][k] + Ec[2][j] * Ec[1][k]);
+                Wm[j][k] = t * w;
+            }
+            U[j] *= w;
+        }
+        dv = m[0] * w; dw = m[1]; E = m[2] * w * eps_scale;
+        W00 = Wm[0][0]; W01 = Wm[0][1]; W02 = Wm[0][2]; W11 = Wm[1][1]; W12 = Wm[1][2]; W22 = Wm[2][2];
+    } else {
+        const float4 *ga = reinterpret_cast<const float4 *>(gacc) + 4 * (size_t)i;
+        const float4 g0 = ga[0], g1 = ga[1], g2 = ga[2];
+        dv = g0.x; dw = g0.y;
+        U[0] = g0.z; U[1] = g0.w; U[2] = g1.x;
+        W00 = g1.y; W01 = g1.z; W02 = g1.w; W11 = g2.x; W12 = g2.y; W22 = g2.z; E = g2.w;
+    }
     const float4 p0 = reinterpret_cast<const float4 *>(params)[2 * (size_t)i];
     const float4 p1 = reinterpret_cast<const float4 *>(params)[2 * (size_t)i + 1];
     const float4 c0 = rec[i];
@@ -152,10 +189,12 @@ __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec
     if (out.err) out.err[i] = valid ? E : 0.f;
 }
 
-cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, const gs_grads &out,
-                            cudaStream_t s) {
+cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
+                            float eps_scale, const gs_grads &out, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    k_finalize<<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, out); count_launch();
+    if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out);
+    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out);
+    count_launch();
     return cudaGetLastError();
 }
 

@@ -8,9 +8,13 @@
 //   2. pushes the surviving cells through a shared-memory ring (warp scan of the interval lengths)
 //      so that every evaluation round has 32 busy lanes;
 //   3. evaluates one cell (8 voxels) per lane with the canonical predicate (shared sub-expressions),
-//      recomputing the weights (nothing is stored by the forward) and keeping the 12 partial sums
-//      in registers;
-//   4. finishes with one transposing butterfly and writes the 64-byte accumulator row.
+//      recomputing the weights (nothing is stored by the forward).  Inside a cell the whitened
+//      coordinate is affine in the voxel index, u(v) = u(0) + ix dx E_x + iy dy E_y + iz dz E_z (E_a = column a
+//      of M, dx/dy/dz the cell's exact position steps), so the sums U = sum g u and W = sum g u u^T are
+//      accumulated through the cell's index moments of g (sum g, sum g ix, sum g ix iy, ...) instead of
+//      per voxel: 59 instructions per cell instead of 96, no branches (a miss has G = 0);
+//   4. finishes with one transposing butterfly and writes the 128-byte row of moment sums, which
+//      k_finalize turns into (dv, dw, U, W, E).
 // Gaussians are processed in the Morton order of their central brick so that the per-sample
 // coefficients of neighbouring Gaussians stay in L1/L2.
 //
@@ -40,39 +44,51 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
     pack[c] = make_float4(alpha, beta, eps, 0.f);
 }
 
-constexpr int BWD_WARPS = 4;
-constexpr int BWD_MINB = 5;  // resident CTAs per SM the register allocation must allow
-constexpr int GPW = 4;       // Gaussians per warp (consecutive in the order list)
+#ifndef GS_BWD_WARPS
+#define GS_BWD_WARPS 4
+#define GS_BWD_MINB 4
+#define GS_BWD_GPW 4
+#define GS_BWD_INTERLEAVE 1
+#endif
+constexpr int BWD_WARPS = GS_BWD_WARPS;
+constexpr int BWD_MINB = GS_BWD_MINB;  // resident CTAs per SM the register allocation must allow
+constexpr int GPW = GS_BWD_GPW;        // Gaussians per warp
+constexpr bool INTERLEAVE = GS_BWD_INTERLEAVE;  // the warps of a CTA take neighbouring Gaussians of the order list at the same time
 constexpr int QCAP = 512;  // per-warp ring of surviving cells (power of two, >= 31 + 32 * SLICE)
 constexpr int SLICE = 8;   // cells of its interval a lane pushes per pass
 
-// The backward contribution of one hit with the weight w factored out of the sums (applied once after the
-// reduction):  gamma = alpha v + beta,  g = gamma G:
-//   acc0 += alpha G (dv / w) | acc1 += g (dw) | acc2..4 += g u (U / w) | acc5..10 += g u u^T (W / w) | acc11 += eps G (E / w)
-__device__ __forceinline__ void bwd_hit(float (&acc)[16], float alpha, float beta, float eps, float v, float G, float u0, float u1,
-                                        float u2) {
-    const float gamma = fmaf(alpha, v, beta);
-    const float g = gamma * G;
-    acc[0] = fmaf(alpha, G, acc[0]);
-    acc[1] += g;
-    const float t0 = g * u0, t1 = g * u1, t2 = g * u2;
-    acc[2] += t0; acc[3] += t1; acc[4] += t2;
-    acc[5] = fmaf(t0, u0, acc[5]); acc[6] = fmaf(t0, u1, acc[6]); acc[7] = fmaf(t0, u2, acc[7]);
-    acc[8] = fmaf(t1, u1, acc[8]); acc[9] = fmaf(t1, u2, acc[9]); acc[10] = fmaf(t2, u2, acc[10]);
-    acc[11] = fmaf(eps, G, acc[11]);
+// Row of moment sums of one Gaussian (GACC_GRID floats; the weight w is factored out of all of them and applied by
+// k_finalize).  With g = gamma G, gamma = alpha v + beta, per cell m000 = sum g, a100 = dx sum_{ix=1} g, a200 = dx a100,
+// a110 = dx dy sum_{ix=iy=1} g, ... and u0 = u(voxel 0 of the cell):
+//   0 sum alpha G | 1 sum g | 2 sum eps G | 3..5 sum m000 u0 | 6..8 sum (a100, a010, a001) | 9..14 sum m000 u0 u0^T (00 01 02 11 12 22)
+//   15..17 sum a100 u0 | 18..20 sum a010 u0 | 21..23 sum a001 u0 | 24..29 sum (a200, a020, a002, a110, a101, a011) | 30, 31 unused
+// Transposing butterfly over 32 values: afterwards lane L holds in v[0] the warp-wide sum of component L (31 SHFL).
+__device__ __forceinline__ void warp_reduce32(float (&v)[32], int lane) {
+#pragma unroll
+    for (int h = 16; h >= 1; h >>= 1) {
+        const bool up = lane & h;
+#pragma unroll
+        for (int k = 0; k < h; k++) {
+            const float send = up ? v[k] : v[k + h];
+            const float keep = up ? v[k + h] : v[k];
+            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, h);
+        }
+    }
 }
 
 template <bool PACK2>
 __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
-                                                              GridDesc gd, const void *__restrict__ pack_, float r2, float eps_scale,
+                                                              GridDesc gd, const void *__restrict__ pack_, float r2,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
                                                               uint32_t M) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // a warp processes GPW consecutive Gaussians of the brick-ordered list of the M Gaussians that touch the batch
-    const uint32_t w0 = (blockIdx.x * BWD_WARPS + warp) * GPW;
+    // slot `rep` of this warp is entry w0 + rep * wstride of the order list
+    const uint32_t wstride = INTERLEAVE ? BWD_WARPS : 1;
+    const uint32_t w0 = INTERLEAVE ? blockIdx.x * (BWD_WARPS * GPW) + warp : (blockIdx.x * BWD_WARPS + warp) * GPW;
     if (w0 >= M) return;  // whole warps leave; no block-wide barrier is used below
-    const uint32_t my_id = (w0 + lane < M && lane < GPW) ? order[w0 + lane] : 0u;
+    const uint32_t my_id = (lane < GPW && w0 + lane * wstride < M) ? order[w0 + lane * wstride] : 0u;
     const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
     int first[3], last[3];
 #pragma unroll
@@ -83,7 +99,7 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     const bool odd_x = (gd.bdim[0] & 1) != 0;  // x-pairs of coefficients are 16-byte aligned only for an even x extent
     uint32_t *q = queue[warp];
 
-    for (int rep = 0; rep < GPW && w0 + rep < M; rep++) {
+    for (int rep = 0; rep < GPW && w0 + rep * wstride < M; rep++) {
     const uint32_t i = __shfl_sync(0xffffffffu, my_id, rep);
     const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
                  gd4 = __ldg(rec + 3 * (size_t)N + i);
@@ -95,18 +111,19 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     const bool edge = (flags & 2u) || odd_x;
     const int ncx = (int)(ncp & 2047u), ncy = (int)((ncp >> 11) & 2047u), ncz = (int)(ncp >> 22);
     const float thr = s1.y, invA = s1.z;
-    if (rep + 1 < GPW && w0 + rep + 1 < M) {  // pull the next Gaussian's records towards L1 while this one is processed
+    if (rep + 1 < GPW && w0 + (rep + 1) * wstride < M) {  // pull the next Gaussian's records towards L1 while this one is processed
         const uint32_t nx = __shfl_sync(0xffffffffu, my_id, rep + 1);
         const void *pf = lane < 4 ? (const void *)(rec + (size_t)lane * N + nx) : (const void *)(setup + 2 * (size_t)nx);
         if (lane < 5) asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
     }
 
-    float acc[16];
+    float acc[32];
 #pragma unroll
-    for (int k = 0; k < 16; k++) acc[k] = 0.f;
+    for (int k = 0; k < 32; k++) acc[k] = 0.f;
 
     // evaluate one cell per lane: code = cell coordinates relative to clo (x | y << 10 | z << 20).
-    // EDGE = some cell of this Gaussian may stick out of the batch: voxels outside become NaN positions.
+    // EDGE = some cell of this Gaussian may stick out of the batch.  Voxels outside the batch and idle lanes (which
+    // re-evaluate cell 0) get zero coefficients, so whatever their G is, they add nothing.
     auto process = [&](uint32_t code, bool on, auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
         const int X = 2 * (clo[0] + (int)(code & 1023u)), Y = 2 * (clo[1] + (int)((code >> 10) & 1023u)), Z = 2 * (clo[2] + (int)(code >> 20));
@@ -115,13 +132,6 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
         // per-sample coefficients of the 8 voxels: issued up front (no data dependence on the predicate), so their
         // L1/L2 latency overlaps the arithmetic below
         float al[8], be[8], ep[8];
-        bool okx[2], oky[2], okz[2];
-#pragma unroll
-        for (int d = 0; d < 2; d++) {
-            okx[d] = !EDGE || (on && X + d <= last[0]);
-            oky[d] = !EDGE || Y + d <= last[1];
-            okz[d] = !EDGE || Z + d <= last[2];
-        }
         if (!EDGE && PACK2) {
             const float2 *p2 = reinterpret_cast<const float2 *>(pack_);
 #pragma unroll
@@ -131,6 +141,13 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                 al[2 * r] = s.x; be[2 * r] = s.y; al[2 * r + 1] = s.z; be[2 * r + 1] = s.w;
             }
         } else {
+            bool okx[2], oky[2], okz[2];
+#pragma unroll
+            for (int d = 0; d < 2; d++) {
+                okx[d] = !EDGE || X + d <= last[0];
+                oky[d] = !EDGE || Y + d <= last[1];
+                okz[d] = !EDGE || Z + d <= last[2];
+            }
 #pragma unroll
             for (int v = 0; v < 8; v++) {
                 const uint32_t c = base + ((uint32_t)(v >> 2) * bdy + (uint32_t)((v >> 1) & 1)) * bdx + (uint32_t)(v & 1);
@@ -144,16 +161,12 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                 }
             }
         }
-        const float nanv = __int_as_float(0x7fc00000);
         float dx[2], dy[2], dz[2];
 #pragma unroll
-        for (int d = 0; d < 2; d++) {  // canonical positions (D6); voxels outside the batch (or an idle lane) become NaN
-            const float px = voxel_centre(X + d, gd.spacing[0], gd.origin[0]);
-            const float py = voxel_centre(Y + d, gd.spacing[1], gd.origin[1]);
-            const float pz = voxel_centre(Z + d, gd.spacing[2], gd.origin[2]);
-            dx[d] = __fsub_rn((EDGE ? okx[d] : on) ? px : nanv, ga.x);
-            dy[d] = __fsub_rn(oky[d] ? py : nanv, ga.y);
-            dz[d] = __fsub_rn(okz[d] ? pz : nanv, ga.z);
+        for (int d = 0; d < 2; d++) {  // canonical positions (D6)
+            dx[d] = __fsub_rn(voxel_centre(X + d, gd.spacing[0], gd.origin[0]), ga.x);
+            dy[d] = __fsub_rn(voxel_centre(Y + d, gd.spacing[1], gd.origin[1]), ga.y);
+            dz[d] = __fsub_rn(voxel_centre(Z + d, gd.spacing[2], gd.origin[2]), ga.z);
         }
         // canonical sequence (D4) with shared sub-expressions: u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx))
         float ab[3][4];
@@ -164,14 +177,43 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
             ab[row][0] = __fmaf_rn(mr.y, dy[0], a0); ab[row][1] = __fmaf_rn(mr.y, dy[0], a1);
             ab[row][2] = __fmaf_rn(mr.y, dy[1], a0); ab[row][3] = __fmaf_rn(mr.y, dy[1], a1);
         }
+        float g[8], c0 = 0.f, c1 = 0.f, c2 = 0.f;  // c = u(voxel 0)
 #pragma unroll
         for (int v = 0; v < 8; v++) {  // v = x | y << 1 | z << 2
             const float u0 = __fmaf_rn(gb.z, dz[v >> 2], ab[0][v & 3]);
             const float u1 = __fmaf_rn(gc.z, dz[v >> 2], ab[1][v & 3]);
             const float u2 = __fmaf_rn(gd4.z, dz[v >> 2], ab[2][v & 3]);
+            if (v == 0) { c0 = u0; c1 = u1; c2 = u2; }
             const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
-            if (qd <= r2) bwd_hit(acc, al[v], be[v], PACK2 ? fabsf(al[v]) : ep[v], gb.w, gauss_weight(qd), u0, u1, u2);
+            g[v] = qd <= r2 ? gauss_weight(qd) : 0.f;  // G; the canonical predicate decides membership
         }
+        // the coefficients are first needed here, a whole cell's worth of arithmetic after their loads were issued
+#pragma unroll
+        for (int v = 0; v < 8; v++) {
+            const float G = g[v];
+            g[v] = fmaf(al[v], gb.w, be[v]) * G;
+            acc[0] = fmaf(al[v], G, acc[0]);
+            acc[2] = fmaf(PACK2 ? fabsf(al[v]) : ep[v], G, acc[2]);
+        }
+        // index moments of g over the cell
+        const float s01 = g[0] + g[1], s23 = g[2] + g[3], s45 = g[4] + g[5], s67 = g[6] + g[7];
+        const float x13 = g[1] + g[3], m101 = g[5] + g[7], m110 = g[3] + g[7];
+        const float m100 = x13 + m101, m010 = s23 + s67, m001 = s45 + s67, m011 = s67;
+        const float m000 = (s01 + s23) + m001;
+        // exact position steps of this cell (the canonical positions are rounded, so they differ from the spacing by an ulp)
+        const float ex = dx[1] - dx[0], ey = dy[1] - dy[0], ez = dz[1] - dz[0];
+        const float a100 = m100 * ex, a010 = m010 * ey, a001 = m001 * ez;
+        acc[1] += m000;
+        const float t0 = m000 * c0, t1 = m000 * c1, t2 = m000 * c2;
+        acc[3] += t0; acc[4] += t1; acc[5] += t2;
+        acc[6] += a100; acc[7] += a010; acc[8] += a001;
+        acc[9] = fmaf(t0, c0, acc[9]); acc[10] = fmaf(t0, c1, acc[10]); acc[11] = fmaf(t0, c2, acc[11]);
+        acc[12] = fmaf(t1, c1, acc[12]); acc[13] = fmaf(t1, c2, acc[13]); acc[14] = fmaf(t2, c2, acc[14]);
+        acc[15] = fmaf(a100, c0, acc[15]); acc[16] = fmaf(a100, c1, acc[16]); acc[17] = fmaf(a100, c2, acc[17]);
+        acc[18] = fmaf(a010, c0, acc[18]); acc[19] = fmaf(a010, c1, acc[19]); acc[20] = fmaf(a010, c2, acc[20]);
+        acc[21] = fmaf(a001, c0, acc[21]); acc[22] = fmaf(a001, c1, acc[22]); acc[23] = fmaf(a001, c2, acc[23]);
+        acc[24] = fmaf(a100, ex, acc[24]); acc[25] = fmaf(a010, ey, acc[25]); acc[26] = fmaf(a001, ez, acc[26]);
+        acc[27] = fmaf(m110 * ex, ey, acc[27]); acc[28] = fmaf(m101 * ex, ez, acc[28]); acc[29] = fmaf(m011 * ey, ez, acc[29]);
     };
 
     // ---- enumeration: lane = row (y, z) of cells.  Along the row the cell centre moves by 2 voxels in x:
@@ -234,13 +276,9 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     }
     drain(0u);
 
-    warp_reduce16(acc, lane);
-    // lane 2c holds component c: 16 floats per Gaussian, written as one coalesced 64-byte row.  The weight w that
-    // bwd_hit leaves out multiplies every sum except dw; the error share also takes its scale.
-    float val = __shfl_sync(0xffffffffu, acc[0], (lane & 15) * 2);
-    if (lane != 1) val *= ga.w;
-    if (PACK2 && lane == 11) val *= eps_scale;
-    if (lane < 16) gacc[(size_t)i * GACC + lane] = val;
+    warp_reduce32(acc, lane);
+    // lane c holds component c: one coalesced 128-byte row per Gaussian
+    gacc[(size_t)i * GACC_GRID + lane] = acc[0];
     __syncwarp();
     }  // rep
 }
@@ -253,13 +291,13 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
 }
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float eps_scale, float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
     // untouched Gaussians keep a zero accumulator row
-    cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC * sizeof(float), s);
+    cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC_GRID * sizeof(float), s);
     if (e != cudaSuccess || M == 0) return e;
     const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
-    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, eps_scale, gacc, order, M);
-    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, eps_scale, gacc, order, M);
+    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
     count_launch();
     return cudaGetLastError();
 }

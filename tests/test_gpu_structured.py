@@ -190,3 +190,32 @@ def test_fused_mse_backward(oracle):
     with pytest.raises(api.GsError) as ei:
         ctx.gs_sample_bwd(run.q, None, None, None, run.grads, dL_dI=torch.zeros_like(run.phi))
     assert ei.value.status == api.GS_ERR_STATE
+
+
+def test_long_brick_runs_sorted(oracle):
+    # brick runs of every length class of the per-brick sort (<= 32 shuffles, <= 128 rank sort, <= 1024 bitonic in
+    # shared memory, longer in global memory): 5,000 Gaussians several bricks wide over a 3 x 2 x 2 brick grid,
+    # plus many that are smaller than a brick; the sorted (brick, gaussian) list must be bit-exact either way
+    rng = np.random.default_rng(11)
+    grid = inputs.Grid((24, 16, 12), (0.0, 0.0, 0.0), (1 / 24, 1 / 24, 1 / 24))
+    n_big, n_small = 5000, 600
+    g = inputs.c1_gaussians(seed=12, n=n_big + n_small)
+    g.mean[:] = rng.uniform((0, 0, 0), (1.0, 16 / 24, 0.5), (g.n, 3)).astype(np.float32)
+    g.scale[:n_big] = rng.uniform(0.08, 0.2, (n_big, 3)).astype(np.float32)
+    g.scale[n_big:] = rng.uniform(0.004, 0.01, (n_small, 3)).astype(np.float32)
+    perm = rng.permutation(g.n)
+    for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar):
+        a[:] = a[perm]
+    for sub in (grid, grid.batch((2, 1, 1), (1, 1, 1))):
+        run = GpuRun(g, "grid", sub, None)
+        T = _check_integer_stages(oracle, run, g, sub)
+        start = run.ctx.debug_get(run.api.DBG_BRICK_START, np.uint32).astype(np.int64)
+        lens = np.diff(start)
+        assert T == start[-1] and lens.max() > 1024
+    # a second grid whose runs fall in the middle classes
+    g2 = inputs.c1_gaussians(seed=13, n=1500)
+    g2.scale[:] = rng.uniform(0.02, 0.06, (g2.n, 3)).astype(np.float32)
+    run = GpuRun(g2, "grid", inputs.c1_grid(32), None)
+    _check_integer_stages(oracle, run, g2, inputs.c1_grid(32))
+    lens = np.diff(run.ctx.debug_get(run.api.DBG_BRICK_START, np.uint32).astype(np.int64))
+    assert ((lens > 32) & (lens <= 128)).any() and ((lens > 128) & (lens <= 1024)).any()
