@@ -12,7 +12,7 @@ struct Rec {          // one Gaussian's record: 4 float4 planes
     float4 a;         // mu.xyz, w
     float4 b;         // M row 0, v
     float4 c;         // M row 1, -
-    float4 d;         // M row 2, -
+    float4 d;         // M row 2, v w
 };
 
 // canonical fp32 sequence (D4): 3 FSUB; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx)); qd = fma(u2,u2, fma(u1,u1, u0*u0))

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ me
     *r0 = make_float4(mx, my, mz, w);
     *r1 = make_float4(M[0], M[1], M[2], v);
     *r2p = make_float4(M[3], M[4], M[5], 0.f);
-    *r3 = make_float4(M[6], M[7], M[8], 0.f);
+    *r3 = make_float4(M[6], M[7], M[8], v * w);  // v w: the forward accumulates Nacc += (v w) G with one FMA
     // AABB of the cutoff ellipsoid: half extent along world axis k = r sqrt(sum_j (s_j R_jk)^2), inflated by 1 + 2^-8
     const float mu[3] = {mx, my, mz};
 #pragma unroll

@@ -125,13 +125,15 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
             }
         }
         __syncwarp();
-        // ---- evaluation: lane = cell, walking its own masks over the whole round; 8 voxels per listed Gaussian
+        // ---- evaluation: lane = cell, walking its own masks over the whole round; 8 voxels per listed Gaussian.
+        // The 128-bit mask is walked with 32-bit operations: `cur` is the word being consumed, w1..w3 the ones behind it.
         const uint4 mk = smask[warp][lane];
-        unsigned long long mlo = ((unsigned long long)mk.y << 32) | mk.x, mhi = ((unsigned long long)mk.w << 32) | mk.z;
-        while (mlo | mhi) {
-            int j;
-            if (mlo) { j = __ffsll((long long)mlo) - 1; mlo &= mlo - 1; }
-            else { j = 63 + __ffsll((long long)mhi); mhi &= mhi - 1; }
+        uint32_t cur = mk.x, w1 = mk.y, w2 = mk.z, w3 = mk.w;
+        int jbase = 0;
+        for (int left = __popc(cur) + __popc(w1) + __popc(w2) + __popc(w3); left > 0; left--) {
+            while (cur == 0u) { cur = w1; w1 = w2; w2 = w3; w3 = 0u; jbase += 32; }
+            const int j = jbase + __ffs((int)cur) - 1;
+            cur &= cur - 1u;
             const float4 ga = srec[0][j], gb = srec[1][j], gc = srec[2][j], gd4 = srec[3][j];
             // canonical sequence (D4), shared between voxels: d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx));
             // qd = fma(u2, u2, fma(u1, u1, u0 * u0))
@@ -162,9 +164,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
 #pragma unroll
             for (int v = 0; v < 8; v++) {
                 if (qd[v] <= r2) {
-                    const float wG = ga.w * gauss_weight(qd[v]);
-                    I[v] += wG;
-                    Nacc[v] = fmaf(gb.w, wG, Nacc[v]);
+                    const float G = gauss_weight(qd[v]);
+                    I[v] = fmaf(ga.w, G, I[v]);
+                    Nacc[v] = fmaf(gd4.w, G, Nacc[v]);  // gd4.w = v w
                     if (SETS) {
                         const unsigned long long h = mix64(sid[j]);
                         cnt[v]++; hsum[v] += h; hxor[v] ^= h;

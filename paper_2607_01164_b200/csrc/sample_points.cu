@@ -291,9 +291,9 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             float u0, u1, u2;
             const float qd = mahalanobis(q, px, py, pz, u0, u1, u2);
             const bool hit = qd <= r2;
-            const float wG = hit ? q.a.w * gauss_weight(qd) : 0.f;
-            I += wG;
-            Nacc = fmaf(q.b.w, wG, Nacc);
+            const float G = hit ? gauss_weight(qd) : 0.f;
+            I = fmaf(q.a.w, G, I);
+            Nacc = fmaf(q.d.w, G, Nacc);  // d.w = v w
             if (SETS && hit) { const unsigned long long h = mix64(__float_as_uint(q.c.w)); cnt++; hsum += h; hxor ^= h; }
         }
         if (SETS) tested += (uint32_t)n0;
