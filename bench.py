@@ -76,14 +76,23 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
 
-    def stop(self):
+    def wait_first(self, timeout: float = 5.0):
+        """nvidia-smi takes a moment to attach to the driver: let that happen outside the timed region."""
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.02)
+
+    def stop(self, window=None):
+        """window = (t0, t1) host times of the timed region: only samples taken inside it count (all, if none fell inside)."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
         self.proc.terminate()
-        rows = [r for r in self.rows if len(r) >= 7]
+        allrows = [(t, r) for t, r in self.rows if len(r) >= 7]
+        rows = [r for t, r in allrows if window is None or window[0] <= t <= window[1] + 0.1]
+        if not rows:
+            rows = [r for _, r in allrows]
         if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         sm = sorted(float(r[0]) for r in rows)
@@ -197,15 +206,20 @@ def run_ours(args):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+        sampler.wait_first()
+    for _ in range(3):
+        step()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
     e0.record()
     for _ in range(args.steps):
         step()
     e1.record()
     barrier()
+    w1 = time.time()
     ms_total = e0.elapsed_time(e1)
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop((w0, w1)) if rank == 0 else None
     stage_ms, stage_calls, launches = ctx.profile_read()
     ctx.profile_enable(False)
     t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
@@ -290,7 +304,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
