@@ -31,6 +31,13 @@ INSTR_FWD = 19.0
 INSTR_BWD = 40.0
 # plain-ALU peak: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts / max SM clock)
 ALU_PEAK_TINSTR = 148 * 128 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (bytes); a kernel
+# that has no capture of the current build reports null
+NCU_TRAFFIC = {
+    ("c2", "k_grid_bwd"): (190.37e6 + 28.29e6, "profiles/r1_step4_c2_ncu_full.md"),
+    ("c2", "k_grid_fwd"): (113.57e6 + 224.11e6, "profiles/r1_step4_c2_ncu_full.md"),
+    ("c3", "k_points_bwd"): (576.11e6 + 67.30e6, "profiles/r1_step3_c3_ncu_full.md"),
+}
 
 
 def make_workload(name: str, rank: int = 0):
@@ -132,12 +139,15 @@ def run_reference(args):
     oracle.build()
     wl = make_workload(args.workload)
     note = []
+    # the per-step sample shrinks with the number of steps so that the whole run ends within a few minutes
+    total = args.steps + args.warmup
+    cap_bricks, cap_points = (12, 1 << 15) if total <= 250 else (6, 1 << 12) if total <= 1000 else (4, 1 << 10)
     for _ in range(args.warmup):
-        oracle_step(wl, note)
+        oracle_step(wl, note, cap_bricks, cap_points)
     t0 = time.perf_counter()
     pts = 0
     for _ in range(args.steps):
-        p, _h = oracle_step(wl, note)
+        p, _h = oracle_step(wl, note, cap_bricks, cap_points)
         pts += p
     dt = time.perf_counter() - t0
     val = pts / dt
@@ -264,6 +274,8 @@ def run_ours(args):
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         except OSError:
             pass
+        kernel = ("k_grid_" if wl["kind"] == "grid" else "k_points_") + dom_name
+        traffic, traffic_src = NCU_TRAFFIC.get((args.workload, kernel), (None, None))
         line = {
             "metric": "query_points_per_s_fwd_bwd", "value": value, "unit": "points/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -281,9 +293,11 @@ def run_ours(args):
                       "fwd_bwd_kernels_roofline_frac": roof_fb / ALU_PEAK_TINSTR,
                       "cull_efficiency": hits / tested if tested else None,
                       "hbm_peak_gbs_measured": peaks.get("hbm_gbs")},
-            "roofline": {"bound": "alu", "kernel": "k_grid_" + dom_name if wl["kind"] == "grid" else "k_points_" + dom_name,
+            "roofline": {"bound": "alu", "kernel": kernel,
                          "achieved": achieved, "peak": ALU_PEAK_TINSTR, "unit": "T FP32 lane-instr/s (algorithmic: hit pairs x "
-                         f"{instr:.0f} instr)", "frac": achieved / ALU_PEAK_TINSTR, "traffic": None,
+                         f"{instr:.0f} instr)", "frac": achieved / ALU_PEAK_TINSTR, "traffic": traffic,
+                         "traffic_unit": "bytes per launch (dram read + write, ncu --set full)", "traffic_source": traffic_src,
+                         "launch_ms": dom_ms,
                          "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md); measured FFMA 36.3 T/s"},
         }
         if not args.no_cpu and world == 1:
