@@ -119,9 +119,11 @@ const char *gs_last_error(const gs_ctx *ctx);
 gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom, float tau);
 
 /* S2 / S3: build the acceleration structure for one query.
- * Grid (section 4.1.2): count the bricks of the batch each AABB overlaps, prefix-sum,
- *   write (brick, gaussian) pairs in parallel over pairs, radix-sort by brick (stable, so each
- *   brick's list is in ascending Gaussian id), per-brick ranges.
+ * Grid (section 4.1.2): the (brick, gaussian) pairs of the batch, sorted by
+ *   (brick, gaussian), with per-brick ranges.  The sort is a radix sort taken most-significant
+ *   digit first: a histogram over the bricks each AABB overlaps, its prefix sum (= the per-brick
+ *   ranges), a fill that gives every pair a slot in its brick's run, and a sort of every run by
+ *   Gaussian id, so each brick's list is in ascending Gaussian id whatever the fill order was.
  * Points (north_star (2); the paper uses a BVH over the samples instead):
  *   30-bit Morton codes of the Gaussian means in `dom`, radix sort of (code, id), Karras radix
  *   tree, bottom-up AABB refit; the query points are Morton-sorted for coherence unless presorted.
