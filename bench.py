@@ -211,6 +211,7 @@ def run_ours(args):
     barrier()
     # hit / tested pair counts of this workload (outside the timed region)
     _, _, _, tested, hits = ctx.debug_point_sets(q)
+    ffma_peak, ex2_peak = ctx.measure_alu_peaks()  # measured ALU denominators at the clocks of this run
     ctx.profile_read()
     ctx.profile_enable(True)
     sampler = ClockSampler(local)
@@ -298,7 +299,10 @@ def run_ours(args):
                          f"{instr:.0f} instr)", "frac": achieved / ALU_PEAK_TINSTR, "traffic": traffic,
                          "traffic_unit": "bytes per launch (dram read + write, ncu --set full)", "traffic_source": traffic_src,
                          "launch_ms": dom_ms,
-                         "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md); measured FFMA 36.3 T/s"},
+                         "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max SM clock)",
+                         "peak_measured": {"ffma_tinstr_s": ffma_peak / 1e12, "mufu_ex2_tinstr_s": ex2_peak / 1e12,
+                                           "how": "gs_measure_alu_peaks: register-only FMA / EX2 loops, CUDA events, this run"},
+                         "frac_of_measured": achieved / (ffma_peak / 1e12) if ffma_peak else None},
         }
         if not args.no_cpu and world == 1:
             from oracle import wveg_oracle as oracle

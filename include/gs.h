@@ -223,6 +223,13 @@ typedef enum {
 gs_status gs_profile_enable(gs_ctx *ctx, int32_t on);
 gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uint64_t *launches_host);
 
+/* Measured denominators of the plain-ALU roofline the sampling kernels are held against (the path is
+ * bound by FP32 issue, not by a dense contraction; north_star: "FP32/SFU issue utilisation against the
+ * chip's peak"): FP32 FMA lane-instructions per second and MUFU.EX2 per second of this device at its
+ * current clocks, from two register-only loops timed with CUDA events on the context's stream.
+ * HOST outputs; synchronises.  Errors: INVALID_ARG, OOM, CUDA. */
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
-           "gs_profile_enable", "gs_profile_read"]
+           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -89,6 +89,7 @@ def load_library():
     lib.gs_debug_read.argtypes = [P, C.c_int32, P, C.c_size_t]
     lib.gs_debug_point_sets.argtypes = [P, C.POINTER(_Query), P, P, P]
     lib.gs_debug_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
     for name in EXPORTS:
@@ -221,6 +222,12 @@ class Context:
         self._check(self.lib.gs_step_host(self.h, C.byref(g), _domain(domain), C.c_float(tau), C.byref(q_host), _ptr(target_host),
                                           _ptr(phi_host), _ptr(I_host), C.byref(loss), gr))
         return float(loss.value)
+
+    def measure_alu_peaks(self):
+        """(FP32 FMA lane-instructions per second, MUFU.EX2 per second) of this device now; synchronises."""
+        a, b = C.c_double(), C.c_double()
+        self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b)))
+        return float(a.value), float(b.value)
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.gs_profile_enable(self.h, int(on)))

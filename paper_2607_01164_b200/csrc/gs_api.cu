@@ -480,6 +480,14 @@ gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_h
     return GS_OK;
 }
 
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host) {
+    if (!ctx || !ffma_per_s_host || !ex2_per_s_host) return GS_ERR_INVALID_ARG;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(ctx->dbg.reserve(64), "alloc scratch");
+    CK(measure_alu_peaks(ctx->dbg.as<float>(), ctx->stream, ffma_per_s_host, ex2_per_s_host), "alu peaks");
+    return GS_OK;
+}
+
 gs_status gs_profile_enable(gs_ctx *ctx, int32_t on) {
     if (!ctx) return GS_ERR_INVALID_ARG;
     ctx->prof = on != 0;

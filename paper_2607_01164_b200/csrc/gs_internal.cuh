@@ -176,6 +176,9 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
                             float eps_scale, const gs_grads &out, cudaStream_t s);
 
+// peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)
+cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s);
+
 // LBVH
 cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *aabb_valid /*nullable: aabb[N][6]*/, size_t n,
                           const gs_domain &dom, uint32_t *codes, uint32_t *ids, cudaStream_t s);
