@@ -451,6 +451,74 @@ void wo_mse(const double *phi, const double *I, const float *target, int64_t P, 
 }
 
 /* ------------------------------------------------------------------------------------- */
+/* S6, the paper's training losses.  `defined` (nullable = all) marks the */
+/* samples that lie in the volume's domain (set D); the others form the set U of samples     */
+/* "undefined in the volume".  With nD = |D|:                                 */
+/*   reconstruction over D: L_rec = (1/nD) sum_D rho(Phi_d - t_d), rho = |.| ("L1            */
+/*     reconstruction loss"; kind 1) or (.)^2 (north_star's MSE; kind 0);      */
+/*     an uncovered sample of D enters as rho(0 - t) and passes no gradient through Phi      */
+/*     (DESIGN D5); d|x|/dx = sign(x), 0 at x = 0.                                           */
+/*   false negatives, Eq. 4: D- = { d in D | I_d < (1 + eps) tau },       */
+/*     L_FN = lambda_FN sum_{D-} ((1 + eps) tau - I_d) / |D-|   (0 when D- is empty)         */
+/*     => dL/dI_d = -lambda_FN / |D-| on D-.                                                 */
+/*   false positives, Eq. 5: U+ = { u in U | I_u >= tau },                    */
+/*     L_FP = lambda_FP sum_{U+} I_u / |U+|   => dL/dI_u = +lambda_FP / |U+| on U+.          */
+/* Membership of D- and U+ is decided on the fp32 value of I against fp32 thresholds         */
+/* ((1.0f + eps) * tau and tau), like the coverage rule.  The paper gives no eps / lambda.   */
+/* loss3 = (L_rec, L_FN, L_FP); counts3 = (nD, |D-|, |U+|); sample_err = |Phi - t| on D, 0 on U. */
+/* ------------------------------------------------------------------------------------- */
+void wo_loss(const double *phi, const double *I, const float *target, const uint8_t *defined, int64_t P, float tau, int kind,
+             float lambda_fn, float eps_fn, float lambda_fp, double *loss3, double *dL_dphi, double *dL_dI, double *sample_err,
+             int64_t *counts3) {
+    const float thr_fn = (1.0f + eps_fn) * tau;
+    int64_t nD = 0, nFN = 0, nFP = 0;
+    for (int64_t c = 0; c < P; c++) {
+        const int def = defined ? defined[c] != 0 : 1;
+        const float If = (float)I[c];
+        if (def) {
+            nD++;
+            if (If < thr_fn) nFN++;
+        } else if (If >= tau) {
+            nFP++;
+        }
+    }
+    double rec = 0.0, fn = 0.0, fp = 0.0;
+    for (int64_t c = 0; c < P; c++) {
+        const int def = defined ? defined[c] != 0 : 1;
+        const float If = (float)I[c];
+        const int covered = If > tau;
+        double a = 0.0, b = 0.0, e = 0.0;
+        if (def) {
+            const double res = phi[c] - (double)target[c];
+            e = fabs(res);
+            if (kind == 1) {
+                rec += fabs(res);
+                if (covered) a = (res > 0.0 ? 1.0 : res < 0.0 ? -1.0 : 0.0) / (double)nD;
+            } else {
+                rec += res * res;
+                if (covered) a = 2.0 * res / (double)nD;
+            }
+            if (If < thr_fn) {
+                fn += (double)thr_fn - I[c];
+                b = -(double)lambda_fn / (double)nFN;
+            }
+        } else if (If >= tau) {
+            fp += I[c];
+            b = (double)lambda_fp / (double)nFP;
+        }
+        if (dL_dphi) dL_dphi[c] = a;
+        if (dL_dI) dL_dI[c] = b;
+        if (sample_err) sample_err[c] = e;
+    }
+    if (loss3) {
+        loss3[0] = nD ? rec / (double)nD : 0.0;
+        loss3[1] = nFN ? (double)lambda_fn * fn / (double)nFN : 0.0;
+        loss3[2] = nFP ? (double)lambda_fp * fp / (double)nFP : 0.0;
+    }
+    if (counts3) { counts3[0] = nD; counts3[1] = nFN; counts3[2] = nFP; }
+}
+
+/* ------------------------------------------------------------------------------------- */
 /* BACKWARD (S7 + S8): analytic gradients of any loss L(Phi, I) w.r.t. the inputs of the    */
 /* forward, given a_c = dL/dPhi_c and b_c = dL/dI_c ("(I_c, V_c, dL/dI_c,      */
 /* dL/dV_c)"; "backpropagating gradients to (mu_i, S_i, R_i, v_i, w_i)").      */

@@ -150,6 +150,25 @@ def mse(phi, I, target, tau: float = 0.01):
     return float(loss.value), d, e
 
 
+def loss(phi, I, target, defined=None, tau: float = 0.01, kind: str = "l1", lambda_fn: float = 0.0, eps_fn: float = 0.0,
+         lambda_fp: float = 0.0):
+    """The paper's training losses (L1 or MSE reconstruction over the defined samples, Eq. 4 false-negative and Eq. 5
+    false-positive terms).  Returns dict(loss (rec, fn, fp), dL_dphi, dL_dI, sample_err f64 [P], counts (nD, nFN, nFP))."""
+    phi = np.ascontiguousarray(phi, np.float64)
+    I = np.ascontiguousarray(I, np.float64)
+    target = _f32(target)
+    P = phi.shape[0]
+    dmask = None if defined is None else np.ascontiguousarray(defined, np.uint8)
+    l3 = np.zeros(3, np.float64)
+    c3 = np.zeros(3, np.int64)
+    a = np.zeros(P, np.float64)
+    b = np.zeros(P, np.float64)
+    e = np.zeros(P, np.float64)
+    lib().wo_loss(_p(phi), _p(I), _p(target), _p(dmask), C.c_int64(P), C.c_float(tau), C.c_int({"mse": 0, "l1": 1}[kind]),
+                  C.c_float(lambda_fn), C.c_float(eps_fn), C.c_float(lambda_fp), _p(l3), _p(a), _p(b), _p(e), _p(c3))
+    return dict(loss=tuple(float(x) for x in l3), dL_dphi=a, dL_dI=b, sample_err=e, counts=tuple(int(x) for x in c3))
+
+
 def backward(g, xyz, phi, I, a, b=None, target=None, tau: float = 0.01, mode: int = 1, hit_mask_in=None,
              covered_in=None):
     """Returns dict(dmean [N,3], dscale [N,3], dquat [N,4], dopacity [N], dscalar [N], err [N]) in f64."""
