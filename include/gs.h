@@ -145,6 +145,39 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
 gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss,
                         float *dL_dphi, float *sample_err);
 
+/* The same forward with the paper's training losses fused into the epilogue.
+ * `defined` (device, uint8 [P], nullable = every sample) marks the samples that lie in the volume's
+ * domain (set D); the others are the samples "undefined in the volume" (set U).
+ *   reconstruction over D:  L_rec = (1/|D|) sum_D rho(Phi_d - target_d), rho = |.| for GS_LOSS_L1
+ *     ("L1 reconstruction loss") or (.)^2 for GS_LOSS_MSE; an uncovered sample of D
+ *     enters as rho(0 - target) and passes no gradient through Phi (DESIGN D5);
+ *   false negatives, Eq. 4: D- = { d in D | I_d < (1 + eps_fn) tau },
+ *     L_FN = lambda_fn sum_{D-} ((1 + eps_fn) tau - I_d) / |D-|;
+ *   false positives, Eq. 5: U+ = { u in U | I_u >= tau },
+ *     L_FP = lambda_fp sum_{U+} I_u / |U+|.
+ * Membership of D- and U+ is decided on the fp32 I against (1.0f + eps_fn) * tau and tau.  The paper
+ * gives no values for eps and the lambdas: they are the caller's.  num_defined = |D| (the caller
+ * knows its mask; P when defined == NULL).
+ * Outputs (device; nullable except phi, I):
+ *   loss_terms[3] = (L_rec, L_FN, L_FP)   (double; OVERWRITTEN, not accumulated)
+ *   dL_dphi[c] = covered and defined ? rho'(Phi_c - target_c) / |D| : 0        (|x|' = sign x, 0 at 0)
+ *   dL_dI[c]   = -lambda_fn / |D-| on D-,  +lambda_fp / |U+| on U+,  0 elsewhere
+ *   sample_err[c] = defined ? |Phi_c - target_c| : 0
+ * |D-| and |U+| are only known once every sample has been seen: the epilogue writes dL_dI
+ * un-normalised and a second, elementwise kernel divides by the counts and writes loss_terms.
+ * Pass the outputs to gs_sample_bwd(phi, I, dL_dphi, dL_dI, target).
+ * Errors: STATE, INVALID_ARG (negative lambda / eps, unknown kind, num_defined = 0 with P > 0), CUDA. */
+typedef enum { GS_LOSS_MSE = 0, GS_LOSS_L1 = 1 } gs_loss_kind;
+typedef struct gs_loss {
+    int32_t kind;            /* gs_loss_kind */
+    float lambda_fn, eps_fn; /* Eq. 4; lambda_fn = 0 switches the term off */
+    float lambda_fp;         /* Eq. 5; lambda_fp = 0 switches the term off */
+    const uint8_t *defined;  /* device [P] or NULL */
+    uint64_t num_defined;    /* |D| */
+} gs_loss;
+gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss, const float *target, float *phi, float *I,
+                             double *loss_terms, float *dL_dphi, float *dL_dI, float *sample_err);
+
 /* S7/S8 (section 4.1.4; section 5.1.2): gradients of L w.r.t. the Gaussian parameters
  * from dL_dphi[P] and dL_dI[P] (nullable = 0), re-computing the kernel weights from phi/I of the
  * forward pass (nothing else is kept from it).  dL_dphi of an uncovered sample (I_c <= tau) is

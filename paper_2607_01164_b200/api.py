@@ -24,7 +24,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
-           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks"]
+           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -58,6 +58,13 @@ class _Grads(C.Structure):
                 ("dscalar", C.c_void_p), ("err", C.c_void_p)]
 
 
+class _Loss(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("lambda_fn", C.c_float), ("eps_fn", C.c_float), ("lambda_fp", C.c_float),
+                ("defined", C.c_void_p), ("num_defined", C.c_uint64)]
+
+
+LOSS_MSE, LOSS_L1 = 0, 1
+
 _lib = None
 
 
@@ -83,6 +90,7 @@ def load_library():
     lib.gs_build_accel.argtypes = [P, C.POINTER(_Query)]
     lib.gs_sample_fwd.argtypes = [P, C.POINTER(_Query), P, P, P, P, P, P]
     lib.gs_sample_bwd.argtypes = [P, C.POINTER(_Query), P, P, P, P, P, C.POINTER(_Grads)]
+    lib.gs_sample_fwd_loss.argtypes = [P, C.POINTER(_Query), C.POINTER(_Loss), P, P, P, P, P, P, P]
     lib.gs_step_host.argtypes = [P, C.POINTER(_Gaussians), C.POINTER(_Domain), C.c_float, C.POINTER(_Query), P, P, P, P,
                                  C.POINTER(_Grads)]
     lib.gs_debug_get.argtypes = [P, C.c_int32, C.POINTER(P), C.POINTER(C.c_size_t)]
@@ -203,6 +211,15 @@ class Context:
     def gs_sample_fwd(self, q: _Query, phi, I, target=None, loss=None, dL_dphi=None, sample_err=None):
         self._check(self.lib.gs_sample_fwd(self.h, C.byref(q), _ptr(target), _ptr(phi), _ptr(I), _ptr(loss), _ptr(dL_dphi),
                                            _ptr(sample_err)))
+
+    def gs_sample_fwd_loss(self, q: _Query, phi, I, target, kind=LOSS_L1, lambda_fn=0.0, eps_fn=0.0, lambda_fp=0.0, defined=None,
+                           num_defined=None, loss_terms=None, dL_dphi=None, dL_dI=None, sample_err=None):
+        """Forward with the paper's losses fused (gs.h).  num_defined defaults to P (defined is None)."""
+        nd = query_num_points(q) if num_defined is None else int(num_defined)
+        d = _ptr(defined)
+        spec = _Loss(int(kind), float(lambda_fn), float(eps_fn), float(lambda_fp), d.value if d is not None else None, nd)
+        self._check(self.lib.gs_sample_fwd_loss(self.h, C.byref(q), C.byref(spec), _ptr(target), _ptr(phi), _ptr(I), _ptr(loss_terms),
+                                                _ptr(dL_dphi), _ptr(dL_dI), _ptr(sample_err)))
 
     def gs_sample_bwd(self, q: _Query, phi, I, dL_dphi, grads: dict, dL_dI=None, target=None):
         g = _Grads(*[(_ptr(grads.get(k)).value if grads.get(k) is not None else None)

@@ -127,7 +127,7 @@ gs_status gs_create(int device, void *cuda_stream, gs_ctx **out) {
     if (!ctx) return GS_ERR_OOM;
     ctx->device = device;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
-    if (ctx->counters.reserve(64) != cudaSuccess) { delete ctx; cudaGetLastError(); return GS_ERR_OOM; }
+    if (ctx->counters.reserve(128) != cudaSuccess) { delete ctx; cudaGetLastError(); return GS_ERR_OOM; }
     *out = ctx;
     return GS_OK;
 }
@@ -357,6 +357,46 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     st = run_fwd(ctx, o);
     if (st == GS_OK && o.pack2) ctx->fused_pack = true;
     return st;
+}
+
+gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss, const float *target, float *phi, float *I,
+                             double *loss_terms, float *dL_dphi, float *dL_dI, float *sample_err) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    gs_status st = check_ready(ctx, q, "gs_sample_fwd_loss before gs_preprocess/gs_build_accel");
+    if (st != GS_OK) return st;
+    if (!loss) return fail(ctx, GS_ERR_INVALID_ARG, "loss is NULL");
+    if (loss->kind != GS_LOSS_MSE && loss->kind != GS_LOSS_L1) return fail(ctx, GS_ERR_INVALID_ARG, "unknown loss kind");
+    if (!(loss->lambda_fn >= 0.f) || !(loss->lambda_fp >= 0.f) || !(loss->eps_fn >= 0.f) || !isfinite(loss->lambda_fn) ||
+        !isfinite(loss->lambda_fp) || !isfinite(loss->eps_fn))
+        return fail(ctx, GS_ERR_INVALID_ARG, "lambda_fn, lambda_fp and eps_fn must be finite and >= 0");
+    if (ctx->P > 0 && (!phi || !I || !target)) return fail(ctx, GS_ERR_INVALID_ARG, "phi, I and target must be given");
+    if (ctx->P > 0 && (loss->num_defined == 0 || loss->num_defined > ctx->P || (!loss->defined && loss->num_defined != ctx->P)))
+        return fail(ctx, GS_ERR_INVALID_ARG, "num_defined must be |D| (P when defined is NULL)");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    // accumulators of the epilogue: 3 sums (double) and 2 counts, in the context's counter block
+    double *sums = reinterpret_cast<double *>(ctx->counters.as<char>() + 64);
+    unsigned long long *counts = reinterpret_cast<unsigned long long *>(ctx->counters.as<char>() + 88);
+    CK(cudaMemsetAsync(sums, 0, 40, s), "memset loss sums");
+    FwdOut o{target, phi, I, nullptr, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr, nullptr, {}};
+    o.gen.on = 1;
+    o.gen.kind = loss->kind;
+    o.gen.defined = loss->defined;
+    o.gen.dL_dI = dL_dI;
+    o.gen.lam_fn = loss->lambda_fn;
+    o.gen.thr_fn = (1.0f + loss->eps_fn) * ctx->tau;
+    o.gen.lam_fp = loss->lambda_fp;
+    o.gen.inv_nd = ctx->P ? (float)(1.0 / (double)loss->num_defined) : 0.f;
+    o.gen.sums = sums;
+    o.gen.counts = counts;
+    ctx->fused_pack = false;  // the backward of this loss takes dL_dphi and dL_dI explicitly
+    if (ctx->P > 0) {
+        st = run_fwd(ctx, o);
+        if (st != GS_OK) return st;
+    }
+    Stage stage(ctx, GS_PROF_FWD);
+    CK(launch_loss_finish(o.gen, ctx->P, (double)loss->num_defined, loss_terms, s), "loss finish");
+    return GS_OK;
 }
 
 gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi, const float *dL_dI,

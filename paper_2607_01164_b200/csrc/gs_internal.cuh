@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "../../include/gs.h"
+#include "loss.cuh"
 
 namespace gs {
 
@@ -158,6 +159,7 @@ struct FwdOut {
     uint32_t *set_count; unsigned long long *set_sum; unsigned long long *set_xor;   // debug sets (nullable)
     unsigned long long *counters;                                                   // [2] tested, hits (nullable)
     float2 *pack2;  // nullable: per-sample backward coefficients (alpha, beta) of the fused MSE loss; eps = |alpha| P / 2
+    GenLoss gen;    // gen.on: the epilogue of gs_sample_fwd_loss (loss.cuh) instead of the fused MSE
 };
 struct BwdIn {
     const float *phi; const float *I; const float *dL_dphi; const float *dL_dI; const float *target;
@@ -167,6 +169,8 @@ struct BwdIn {
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, cudaStream_t s);
+// second pass of gs_sample_fwd_loss: dL_dI[c] /= |D-| or |U+| (by sign), loss_terms = (L_rec, L_FN, L_FP)
+cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *loss_terms, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
                             float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s);

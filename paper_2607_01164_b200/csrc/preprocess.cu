@@ -189,6 +189,31 @@ __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec
     if (out.err) out.err[i] = valid ? E : 0.f;
 }
 
+// ------------------------------------------------------------------------------------------------
+// second pass of gs_sample_fwd_loss (loss.cuh): the forward wrote dL/dI = -lambda_fn on D- and +lambda_fp on U+;
+// Eq. 4 / Eq. 5 divide by |D-| and |U+|, which are complete only now.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_loss_finish(GenLoss L, size_t P, double nd, double *__restrict__ loss_terms) {
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long nfn = L.counts[0], nfp = L.counts[1];
+    if (c == 0 && loss_terms) {
+        loss_terms[0] = nd > 0.0 ? L.sums[0] / nd : 0.0;
+        loss_terms[1] = nfn ? (double)L.lam_fn * L.sums[1] / (double)nfn : 0.0;
+        loss_terms[2] = nfp ? (double)L.lam_fp * L.sums[2] / (double)nfp : 0.0;
+    }
+    if (c >= P || !L.dL_dI) return;
+    const float b = L.dL_dI[c];
+    if (b < 0.f) L.dL_dI[c] = b / (float)nfn;
+    else if (b > 0.f) L.dL_dI[c] = b / (float)nfp;
+}
+
+cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *loss_terms, cudaStream_t s) {
+    const bool per_sample = L.dL_dI && (L.lam_fn > 0.f || L.lam_fp > 0.f);
+    const size_t n = per_sample && P ? P : 1;
+    k_loss_finish<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(L, per_sample ? P : 0, nd, loss_terms); count_launch();
+    return cudaGetLastError();
+}
+
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
                             float eps_scale, const gs_grads &out, cudaStream_t s) {
     if (N == 0) return cudaSuccess;

@@ -181,7 +181,8 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
     unsigned long long tested = 0, hits = 0;
     const float dscale = (float)(2.0 * invP);
     const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
-    const bool vec2 = !SETS && !(bdx & 1u);  // x-pairs are 8-byte aligned when the batch's x extent is even
+    const bool vec2 = !SETS && !(bdx & 1u) && !o.gen.on;  // x-pairs are 8-byte aligned when the batch's x extent is even
+    LossPartial lp;
 #pragma unroll
     for (int r = 0; r < 4; r++) {  // the cell's four x-rows: (y, z) = (ly + (r & 1), lz + (r >> 1))
         const uint32_t y = (uint32_t)ly + (r & 1), z = (uint32_t)lz + (r >> 1);
@@ -217,7 +218,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
                 const int v = r * 2 + d;
                 o.phi[c + d] = ph[d];
                 o.I[c + d] = Iv[d];
-                if (o.target) {
+                if (o.gen.on) {
+                    loss_sample(o.gen, c + d, ph[d], Iv[d], cov[d], tau, o.target, o.dL_dphi, o.sample_err, lp);
+                } else if (o.target) {
                     const float res = ph[d] - o.target[c + d];
                     res2 = fmaf(res, res, res2);
                     if (o.dL_dphi) o.dL_dphi[c + d] = cov[d] ? dscale * res : 0.f;
@@ -237,7 +240,8 @@ __global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restri
             }
         }
     }
-    if (o.target && o.loss) {
+    if (o.gen.on) loss_flush(o.gen, lp, lane);
+    if (!o.gen.on && o.target && o.loss) {
         double s = (double)res2;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);

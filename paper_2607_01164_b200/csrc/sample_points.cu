@@ -305,10 +305,13 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
     const bool covered = I > tau;
     const float phi = covered ? __fdividef(Nacc, I) : 0.f;
     float res2 = 0.f;
+    LossPartial lp;
     if (active) {
         o.phi[c] = phi;
         o.I[c] = I;
-        if (o.target) {
+        if (o.gen.on) {
+            loss_sample(o.gen, c, phi, I, covered, tau, o.target, o.dL_dphi, o.sample_err, lp);
+        } else if (o.target) {
             const float res = phi - o.target[c];
             res2 = res * res;
             if (o.dL_dphi) o.dL_dphi[c] = covered ? (float)(2.0 * invP) * res : 0.f;
@@ -324,7 +327,8 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             if (o.set_xor) o.set_xor[c] = hxor;
         }
     }
-    if (o.target && o.loss) {   // one reduction per packet (no CTA barrier: a warp's slot frees as soon as its packet is done)
+    if (o.gen.on) loss_flush(o.gen, lp, lane);
+    if (!o.gen.on && o.target && o.loss) {   // one reduction per packet (no CTA barrier: a warp's slot frees as soon as its packet is done)
         double s = (double)res2;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);

@@ -37,6 +37,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(api._Domain) == 24
     assert api._Query.num_points.offset == 64 and api._Query.xyz.offset == 72 and ctypes.sizeof(api._Query) == 88
     assert ctypes.sizeof(api._Grads) == 48
+    assert api._Loss.defined.offset == 16 and api._Loss.num_defined.offset == 24 and ctypes.sizeof(api._Loss) == 32
 
 
 def test_fails_loudly_without_gpu(lib):
