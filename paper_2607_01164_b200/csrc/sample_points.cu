@@ -62,8 +62,16 @@ __device__ __forceinline__ bool ellipsoid_reaches(const Rec &g, const CullBox &c
     const float e2 = fmaf(fabsf(g.d.z), c.hz, fmaf(fabsf(g.d.y), c.hy, fabsf(g.d.x) * c.hx));
     const float qc = fmaf(u2, u2, fmaf(u1, u1, u0 * u0));
     const float reach = rcut + sqrtf(fmaf(e2, e2, fmaf(e1, e1, e0 * e0)));
-    // false for NaN records (invalid Gaussians, D13) and for a NaN box (empty part); true for an infinite box (see segment_box)
-    return qc <= reach * reach * 1.001953125f;
+    // Tighter: component j of M (p - mu) stays within [u_j - e_j, u_j + e_j] over the box, so its magnitude is at least
+    // max(0, |u_j| - e_j) and |M (p - mu)|^2 >= sum_j max(0, |u_j| - e_j)^2 (the distance to the box that bounds the
+    // whitened image of the packet box).  It implies the spherical bound; for a Gaussian that is thin along one axis and
+    // lies beside the packet along another it is much smaller than r + rho.
+    const float v0 = fmaxf(fabsf(u0) - e0, 0.f), v1 = fmaxf(fabsf(u1) - e1, 0.f), v2 = fmaxf(fabsf(u2) - e2, 0.f);
+    const float dmin2 = fmaf(v2, v2, fmaf(v1, v1, v0 * v0));
+    const float r2s = rcut * rcut * 1.001953125f;
+    // the spherical test stays: it is false for NaN records (invalid Gaussians, D13) and for a NaN box (empty part),
+    // where fmaxf would drop the NaN; both are true for an infinite box (see segment_box)
+    return (qc <= reach * reach * 1.001953125f) & (dmin2 <= r2s);
 }
 
 // A packet of 32 consecutive Morton-sorted points can straddle a jump of the Z curve (its box then spans a large
