@@ -244,12 +244,14 @@ def run_ours(args):
     gh = dict(mean=pin(g.mean), scale=pin(g.scale), quat=pin(g.quat), opacity=pin(g.opacity), scalar=pin(g.scalar))
     th = pin(wl["target"])
     qh = api.grid_query(wl["grid"]) if wl["kind"] == "grid" else api.points_query(pin(wl["xyz"]))
-    phi_h, I_h = pin(np.empty(P, np.float32)), pin(np.empty(P, np.float32))
+    # the host-visible result of a training step is the loss and the gradients; the per-sample Phi / I stay on the device
+    # (gs_step_host copies them back only when asked to)
+    phi_h, I_h = None, None
     gr_h = dict(dmean=pin(np.empty((g.n, 3), np.float32)), dscale=pin(np.empty((g.n, 3), np.float32)),
                 dquat=pin(np.empty((g.n, 4), np.float32)), dopacity=pin(np.empty(g.n, np.float32)),
                 dscalar=pin(np.empty(g.n, np.float32)), err=pin(np.empty(g.n, np.float32)))
     h2d = g.n * 48 + P * 4 + (P * 12 if wl["kind"] == "points" else 0)
-    d2h = 2 * P * 4 + 8 + g.n * 52
+    d2h = 8 + g.n * 52
     e2e_steps = max(2, min(args.steps, 10))
     for _ in range(2):
         ctx.gs_step_host(gh, qh, th, phi_h, I_h, gr_h, domain=wl["domain"], tau=TAU)
@@ -286,7 +288,8 @@ def run_ours(args):
                        "step": "preprocess+build_accel+fwd(MSE)+bwd"},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": "points/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": float(te.item()), "api": "gs_step_host (pinned host buffers)"},
+                    "ms_per_step": float(te.item()),
+                    "api": "gs_step_host (pinned host buffers): H2D model + target (+ points), D2H loss + 6 gradient tensors"},
             "stage_ms": per,
             "extra": {"fwd_points_per_s": P / (per["fwd"] * 1e-3) if per["fwd"] else None,
                       "fwd_gaussian_evals_per_s": hits / (per["fwd"] * 1e-3) if per["fwd"] else None,

@@ -145,6 +145,7 @@ void gs_destroy(gs_ctx *ctx) {
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
         for (auto &pp : *v) { cudaEventDestroy(pp.a); cudaEventDestroy(pp.b); }
+    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_event); }
     delete ctx;
 }
 
@@ -580,13 +581,24 @@ gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom
         if (P) CK(cudaMemcpyAsync(ctx->h2d[5].p, qh->xyz, P * 12, cudaMemcpyHostToDevice, s), "H2D points");
         q.xyz = ctx->h2d[5].as<float>();
     }
-    if (P) CK(cudaMemcpyAsync(ctx->h2d[6].p, target_host, P * 4, cudaMemcpyHostToDevice, s), "H2D target");
+    // the target is first needed by the forward's epilogue: its copy runs on a second stream beside preprocess + build
+    if (!ctx->aux_stream) {
+        CK(cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking), "aux stream");
+        CK(cudaEventCreateWithFlags(&ctx->aux_event, cudaEventDisableTiming), "aux event");
+    }
+    if (P) {
+        CK(cudaEventRecord(ctx->aux_event, s), "event");                       // after everything enqueued so far
+        CK(cudaStreamWaitEvent(ctx->aux_stream, ctx->aux_event, 0), "wait");
+        CK(cudaMemcpyAsync(ctx->h2d[6].p, target_host, P * 4, cudaMemcpyHostToDevice, ctx->aux_stream), "H2D target");
+        CK(cudaEventRecord(ctx->aux_event, ctx->aux_stream), "event");
+    }
     CK(cudaMemsetAsync(ctx->h2d[10].p, 0, 8, s), "zero loss");
     gs_gaussians gdv{gh->n, ctx->h2d[0].as<float>(), ctx->h2d[1].as<float>(), ctx->h2d[2].as<float>(), ctx->h2d[3].as<float>(),
                      ctx->h2d[4].as<float>()};
     if ((st = gs_preprocess(ctx, &gdv, dom, tau)) != GS_OK) return st;
     if ((st = gs_build_accel(ctx, &q)) != GS_OK) return st;
     float *phi = ctx->h2d[7].as<float>(), *I = ctx->h2d[8].as<float>();
+    if (P) CK(cudaStreamWaitEvent(s, ctx->aux_event, 0), "wait for the target");
     if ((st = gs_sample_fwd(ctx, &q, ctx->h2d[6].as<float>(), phi, I, ctx->h2d[10].as<double>(), nullptr, nullptr)) != GS_OK) return st;
     gs_grads gdev{ctx->h2d[11].as<float>(), ctx->h2d[12].as<float>(), ctx->h2d[13].as<float>(), ctx->h2d[14].as<float>(),
                   ctx->h2d[15].as<float>(), ctx->h2d[15].as<float>() + n1};

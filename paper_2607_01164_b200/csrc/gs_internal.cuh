@@ -121,6 +121,8 @@ struct gs_ctx {
     gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters, dbg;
     bool fused_pack = false;  // misc holds the coefficients written by the last gs_sample_fwd with a target
     gs::DevBuf h2d[16];  // staging for gs_step_host
+    cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
+    cudaEvent_t aux_event = nullptr;
     // ---- measurement (gs_profile_*)
     bool prof = false;
     struct ProfPair { cudaEvent_t a, b; int stage; };
