@@ -519,6 +519,62 @@ void wo_loss(const double *phi, const double *I, const float *target, const uint
 }
 
 /* ------------------------------------------------------------------------------------- */
+/* Training-step completion.  Raw parameters and their activations        */
+/* (PAPER.md:140): "sigmoid activation functions for v_i and w_i", "an exponential            */
+/* activation for S_i" (the normalisation of R_i is part of the preprocess, DESIGN D2):       */
+/*   scale = exp(raw_scale), opacity = sigmoid(raw_opacity), scalar = sigmoid(raw_scalar).    */
+/* ------------------------------------------------------------------------------------- */
+static double wo_sigmoid(double x) { return 1.0 / (1.0 + exp(-x)); }
+
+void wo_activate(int64_t n, const float *raw_scale, const float *raw_opacity, const float *raw_scalar, double *scale,
+                 double *opacity, double *scalar) {
+    for (int64_t i = 0; i < n; i++) {
+        for (int k = 0; k < 3; k++) scale[3 * i + k] = exp((double)raw_scale[3 * i + k]);
+        opacity[i] = wo_sigmoid((double)raw_opacity[i]);
+        scalar[i] = wo_sigmoid((double)raw_scalar[i]);
+    }
+}
+
+/* Adam (Kingma & Ba, the paper's [20]), one step t >= 1 on one tensor of `count` elements: */
+/*   m = b1 m + (1 - b1) g;  v = b2 v + (1 - b2) g^2;  p -= lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps) */
+static void adam_tensor(int64_t count, double *p, const double *g, double *m, double *v, double lr, double b1, double b2,
+                        double eps, int t) {
+    const double c1 = 1.0 - pow(b1, (double)t), c2 = 1.0 - pow(b2, (double)t);
+    for (int64_t k = 0; k < count; k++) {
+        m[k] = b1 * m[k] + (1.0 - b1) * g[k];
+        v[k] = b2 * v[k] + (1.0 - b2) * g[k] * g[k];
+        p[k] -= lr * (m[k] / c1) / (sqrt(v[k] / c2) + eps);
+    }
+}
+
+/* One optimiser step on the RAW parameters given the gradients w.r.t. the ACTIVATED values (what the */
+/* backward returns).  Chain rule of the activations: d/d raw_scale = dscale * scale (exp' = exp),    */
+/* d/d raw_opacity = dopacity * w (1 - w), d/d raw_scalar = dscalar * v (1 - v) (sigmoid' = s (1 - s)); */
+/* mean and quaternion are their own raw parameters.  lr = (mean, scale, quat, opacity, scalar); the    */
+/* paper's values are 0.00016, 0.001, 0.0001, 0.025 (weights), 0.0025 (values).         */
+/* p* are updated in place; m*, v* are the Adam moments (same shapes).                                */
+void wo_adam_step(int64_t n, double *mean, double *raw_scale, double *quat, double *raw_opacity, double *raw_scalar,
+                  const double *dmean, const double *dscale, const double *dquat, const double *dopacity, const double *dscalar,
+                  double *m, double *v, const double *lr, double b1, double b2, double eps, int t) {
+    /* moments are laid out as one block of 12 n doubles: mean 3n | scale 3n | quat 4n | opacity n | scalar n */
+    double *graw_s = (double *)malloc(sizeof(double) * 3 * (size_t)(n ? n : 1));
+    double *graw_w = (double *)malloc(sizeof(double) * (size_t)(n ? n : 1));
+    double *graw_v = (double *)malloc(sizeof(double) * (size_t)(n ? n : 1));
+    for (int64_t i = 0; i < n; i++) {
+        for (int k = 0; k < 3; k++) graw_s[3 * i + k] = dscale[3 * i + k] * exp(raw_scale[3 * i + k]);
+        const double w = wo_sigmoid(raw_opacity[i]), s = wo_sigmoid(raw_scalar[i]);
+        graw_w[i] = dopacity[i] * w * (1.0 - w);
+        graw_v[i] = dscalar[i] * s * (1.0 - s);
+    }
+    adam_tensor(3 * n, mean, dmean, m, v, lr[0], b1, b2, eps, t);
+    adam_tensor(3 * n, raw_scale, graw_s, m + 3 * n, v + 3 * n, lr[1], b1, b2, eps, t);
+    adam_tensor(4 * n, quat, dquat, m + 6 * n, v + 6 * n, lr[2], b1, b2, eps, t);
+    adam_tensor(n, raw_opacity, graw_w, m + 10 * n, v + 10 * n, lr[3], b1, b2, eps, t);
+    adam_tensor(n, raw_scalar, graw_v, m + 11 * n, v + 11 * n, lr[4], b1, b2, eps, t);
+    free(graw_s); free(graw_w); free(graw_v);
+}
+
+/* ------------------------------------------------------------------------------------- */
 /* BACKWARD (S7 + S8): analytic gradients of any loss L(Phi, I) w.r.t. the inputs of the    */
 /* forward, given a_c = dL/dPhi_c and b_c = dL/dI_c ("(I_c, V_c, dL/dI_c,      */
 /* dL/dV_c)"; "backpropagating gradients to (mu_i, S_i, R_i, v_i, w_i)").      */

@@ -169,6 +169,32 @@ def loss(phi, I, target, defined=None, tau: float = 0.01, kind: str = "l1", lamb
     return dict(loss=tuple(float(x) for x in l3), dL_dphi=a, dL_dI=b, sample_err=e, counts=tuple(int(x) for x in c3))
 
 
+PAPER_LR = (0.00016, 0.001, 0.0001, 0.025, 0.0025)  # mean, scale, quat, opacity (weights), scalar (values): PAPER.md:231
+
+
+def activate(raw_scale, raw_opacity, raw_scalar):
+    """exp / sigmoid / sigmoid activations.  Returns (scale [n,3], opacity [n], scalar [n]) in f64."""
+    rs, rw, rv = _f32(raw_scale), _f32(raw_opacity), _f32(raw_scalar)
+    n = rw.shape[0]
+    s, w, v = np.zeros((n, 3)), np.zeros(n), np.zeros(n)
+    lib().wo_activate(C.c_int64(n), _p(rs), _p(rw), _p(rv), _p(s), _p(w), _p(v))
+    return s, w, v
+
+
+def adam_step(params: dict, grads: dict, m, v, t: int, lr=PAPER_LR, beta1=0.9, beta2=0.999, eps=1e-8):
+    """One Adam step on the raw parameters (dict mean, raw_scale, quat, raw_opacity, raw_scalar: f64 arrays, updated in
+    place) from the gradients w.r.t. the ACTIVATED values (dict dmean, dscale, dquat, dopacity, dscalar).  m, v: f64
+    [12 n] moment blocks (mean | scale | quat | opacity | scalar), updated in place."""
+    n = params["raw_opacity"].shape[0]
+    for k in ("mean", "raw_scale", "quat", "raw_opacity", "raw_scalar"):
+        assert params[k].dtype == np.float64 and params[k].flags["C_CONTIGUOUS"]
+    g = {k: np.ascontiguousarray(grads[k], np.float64) for k in ("dmean", "dscale", "dquat", "dopacity", "dscalar")}
+    lr = np.ascontiguousarray(lr, np.float64)
+    lib().wo_adam_step(C.c_int64(n), _p(params["mean"]), _p(params["raw_scale"]), _p(params["quat"]), _p(params["raw_opacity"]),
+                       _p(params["raw_scalar"]), _p(g["dmean"]), _p(g["dscale"]), _p(g["dquat"]), _p(g["dopacity"]),
+                       _p(g["dscalar"]), _p(m), _p(v), _p(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(t))
+
+
 def backward(g, xyz, phi, I, a, b=None, target=None, tau: float = 0.01, mode: int = 1, hit_mask_in=None,
              covered_in=None):
     """Returns dict(dmean [N,3], dscale [N,3], dquat [N,4], dopacity [N], dscalar [N], err [N]) in f64."""
