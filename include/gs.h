@@ -235,6 +235,42 @@ gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, u
  * pairs tested (predicate evaluated) and pairs hit.  Only collected by gs_debug_point_sets. */
 gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_host);
 
+/* ---- training-step completion ---------------------------------------------
+ * Raw parameters: scale = exp(raw_scale), opacity = sigmoid(raw_opacity),
+ * scalar = sigmoid(raw_scalar); mean and quat are their own raw parameters (the quaternion is
+ * normalised inside gs_preprocess).  All pointers are DEVICE memory owned by the caller. */
+typedef struct gs_raw_params {
+    uint32_t n;
+    float *mean;        /* [n,3] */
+    float *raw_scale;   /* [n,3] log of the scale */
+    float *quat;        /* [n,4] (w,x,y,z), any non-zero norm */
+    float *raw_opacity; /* [n]   logit of w */
+    float *raw_scalar;  /* [n]   logit of v */
+} gs_raw_params;
+/* scale[n,3], opacity[n], scalar[n] = the activated values gs_preprocess takes.  Errors: INVALID_ARG, CUDA. */
+gs_status gs_params_activate(gs_ctx *ctx, const gs_raw_params *p, float *scale, float *opacity, float *scalar);
+
+/* One Adam step (Kingma & Ba, the paper's optimiser) on the raw parameters, in place:
+ *     m = beta1 m + (1 - beta1) g;  v = beta2 v + (1 - beta2) g^2;
+ *     p -= lr (m / (1 - beta1^step)) / (sqrt(v / (1 - beta2^step)) + eps)
+ * `g` holds the gradients w.r.t. the ACTIVATED values exactly as gs_sample_bwd wrote them (err unused);
+ * the chain rule of the activations is applied here: d/d raw_scale = dscale * scale,
+ * d/d raw_opacity = dopacity * w (1 - w), d/d raw_scalar = dscalar * v (1 - v).
+ * lr = (mean, scale, quat, opacity, scalar); the paper's values are
+ * (0.00016, 0.001, 0.0001, 0.025, 0.0025) with Adam's defaults beta1 0.9, beta2 0.999, eps 1e-8.
+ * m, v: device [12 n] moment blocks laid out mean 3n | scale 3n | quat 4n | opacity n | scalar n,
+ * zeroed by the caller before step 1.  step >= 1.  scale_out / opacity_out / scalar_out (nullable)
+ * receive the activations of the UPDATED parameters, i.e. the next gs_preprocess's inputs.
+ * The paper's soft cap on the scales has no printed formula and is not applied.
+ * Errors: INVALID_ARG (null pointers, step < 1, betas outside [0,1), negative lr / eps), CUDA. */
+typedef struct gs_adam_cfg {
+    float lr[5];
+    float beta1, beta2, eps;
+    int32_t step;
+} gs_adam_cfg;
+gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, float *m, float *v, const gs_adam_cfg *cfg,
+                       float *scale_out, float *opacity_out, float *scalar_out);
+
 /* ---- measurement: CUDA-event timing of the stages, on the context's stream --------------------
  * While enabled, every stage of the calls above is bracketed by a pair of CUDA events recorded on
  * the context's stream.  gs_profile_read synchronises the stream, adds up the elapsed time of all

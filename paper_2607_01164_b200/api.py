@@ -24,7 +24,8 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
-           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss"]
+           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
+           "gs_params_activate", "gs_adam_step"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -63,7 +64,17 @@ class _Loss(C.Structure):
                 ("defined", C.c_void_p), ("num_defined", C.c_uint64)]
 
 
+class _RawParams(C.Structure):
+    _fields_ = [("n", C.c_uint32), ("mean", C.c_void_p), ("raw_scale", C.c_void_p), ("quat", C.c_void_p),
+                ("raw_opacity", C.c_void_p), ("raw_scalar", C.c_void_p)]
+
+
+class _AdamCfg(C.Structure):
+    _fields_ = [("lr", C.c_float * 5), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
+
+
 LOSS_MSE, LOSS_L1 = 0, 1
+PAPER_LR = (0.00016, 0.001, 0.0001, 0.025, 0.0025)  # mean, scale, quat, opacity (weights), scalar (values): PAPER.md:231
 
 _lib = None
 
@@ -97,6 +108,8 @@ def load_library():
     lib.gs_debug_read.argtypes = [P, C.c_int32, P, C.c_size_t]
     lib.gs_debug_point_sets.argtypes = [P, C.POINTER(_Query), P, P, P]
     lib.gs_debug_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.gs_params_activate.argtypes = [P, C.POINTER(_RawParams), P, P, P]
+    lib.gs_adam_step.argtypes = [P, C.POINTER(_RawParams), C.POINTER(_Grads), P, P, C.POINTER(_AdamCfg), P, P, P]
     lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
@@ -239,6 +252,25 @@ class Context:
         self._check(self.lib.gs_step_host(self.h, C.byref(g), _domain(domain), C.c_float(tau), C.byref(q_host), _ptr(target_host),
                                           _ptr(phi_host), _ptr(I_host), C.byref(loss), gr))
         return float(loss.value)
+
+    @staticmethod
+    def _raw(raw: dict) -> _RawParams:
+        n = int(raw["raw_opacity"].shape[0])
+        return _RawParams(n, *[_ptr(raw[k]).value for k in ("mean", "raw_scale", "quat", "raw_opacity", "raw_scalar")])
+
+    def gs_params_activate(self, raw: dict, scale, opacity, scalar):
+        """raw: dict of device tensors mean, raw_scale, quat, raw_opacity, raw_scalar."""
+        r = self._raw(raw)
+        self._check(self.lib.gs_params_activate(self.h, C.byref(r), _ptr(scale), _ptr(opacity), _ptr(scalar)))
+
+    def gs_adam_step(self, raw: dict, grads: dict, m, v, step: int, lr=PAPER_LR, beta1=0.9, beta2=0.999, eps=1e-8,
+                     scale_out=None, opacity_out=None, scalar_out=None):
+        r = self._raw(raw)
+        g = _Grads(*[(_ptr(grads.get(k)).value if grads.get(k) is not None else None)
+                     for k in ("dmean", "dscale", "dquat", "dopacity", "dscalar", "err")])
+        cfg = _AdamCfg((C.c_float * 5)(*lr), beta1, beta2, eps, int(step))
+        self._check(self.lib.gs_adam_step(self.h, C.byref(r), C.byref(g), _ptr(m), _ptr(v), C.byref(cfg), _ptr(scale_out),
+                                          _ptr(opacity_out), _ptr(scalar_out)))
 
     def measure_alu_peaks(self):
         """(FP32 FMA lane-instructions per second, MUFU.EX2 per second) of this device now; synchronises."""

@@ -521,6 +521,30 @@ gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_h
     return GS_OK;
 }
 
+gs_status gs_params_activate(gs_ctx *ctx, const gs_raw_params *p, float *scale, float *opacity, float *scalar) {
+    if (!ctx || !p) return GS_ERR_INVALID_ARG;
+    if (p->n > 0 && (!p->raw_scale || !p->raw_opacity || !p->raw_scalar || !scale || !opacity || !scalar))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gs_params_activate: null pointer");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(launch_activate(*p, scale, opacity, scalar, ctx->stream), "activate");
+    return GS_OK;
+}
+
+gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, float *m, float *v, const gs_adam_cfg *cfg,
+                       float *scale_out, float *opacity_out, float *scalar_out) {
+    if (!ctx || !p || !g || !cfg) return GS_ERR_INVALID_ARG;
+    if (p->n > 0 && (!p->mean || !p->raw_scale || !p->quat || !p->raw_opacity || !p->raw_scalar || !g->dmean || !g->dscale ||
+                     !g->dquat || !g->dopacity || !g->dscalar || !m || !v))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gs_adam_step: null pointer");
+    if (cfg->step < 1 || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->eps >= 0.f))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gs_adam_step: step >= 1, betas in [0,1), eps >= 0");
+    for (int k = 0; k < 5; k++)
+        if (!(cfg->lr[k] >= 0.f) || !isfinite(cfg->lr[k])) return fail(ctx, GS_ERR_INVALID_ARG, "gs_adam_step: lr must be finite and >= 0");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(launch_adam_step(*p, *g, m, v, *cfg, scale_out, opacity_out, scalar_out, ctx->stream), "adam step");
+    return GS_OK;
+}
+
 gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host) {
     if (!ctx || !ffma_per_s_host || !ex2_per_s_host) return GS_ERR_INVALID_ARG;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");

@@ -182,6 +182,11 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
                             float eps_scale, const gs_grads &out, cudaStream_t s);
 
+// optim.cu: activations of the raw parameters and one Adam step on them
+cudaError_t launch_activate(const gs_raw_params &p, float *scale, float *opacity, float *scalar, cudaStream_t s);
+cudaError_t launch_adam_step(const gs_raw_params &p, const gs_grads &g, float *m, float *v, const gs_adam_cfg &cfg, float *scale_out,
+                             float *opacity_out, float *scalar_out, cudaStream_t s);
+
 // peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)
 cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s);
 

@@ -37,6 +37,8 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(api._Domain) == 24
     assert api._Query.num_points.offset == 64 and api._Query.xyz.offset == 72 and ctypes.sizeof(api._Query) == 88
     assert ctypes.sizeof(api._Grads) == 48
+    assert ctypes.sizeof(api._RawParams) == 48 and api._RawParams.mean.offset == 8
+    assert ctypes.sizeof(api._AdamCfg) == 36 and api._AdamCfg.step.offset == 32
     assert api._Loss.defined.offset == 16 and api._Loss.num_defined.offset == 24 and ctypes.sizeof(api._Loss) == 32
 
 

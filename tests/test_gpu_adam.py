@@ -1,0 +1,145 @@
+"""-m gpu parity: gs_params_activate / gs_adam_step (PAPER.md:140 activations, PAPER.md:231 Adam with the paper's learning
+rates) vs the oracle, and a short training loop on configs[0] driven through the C ABI only."""
+import numpy as np
+import pytest
+
+from paper_2607_01164_b200 import inputs
+from gpu_util import TAU, to_dev
+
+pytestmark = pytest.mark.gpu
+
+KEYS = ("mean", "raw_scale", "quat", "raw_opacity", "raw_scalar")
+# the C ABI takes the hyperparameters as float32: the oracle gets exactly those values (0.999f != 0.999)
+F = lambda x: float(np.float32(x))
+HYPER = dict(lr=tuple(F(x) for x in (0.00016, 0.001, 0.0001, 0.025, 0.0025)), beta1=F(0.9), beta2=F(0.999), eps=F(1e-8))
+LR = dict(mean=0.00016, raw_scale=0.001, quat=0.0001, raw_opacity=0.025, raw_scalar=0.0025)
+
+
+def _raw_from(g):
+    """Raw parameters whose activations are the Gaussians g (float32 arrays)."""
+    logit = lambda x: np.log(x / (1 - x))
+    return dict(mean=g.mean.astype(np.float32).copy(), raw_scale=np.log(g.scale).astype(np.float32), quat=g.quat.astype(np.float32).copy(),
+                raw_opacity=logit(np.clip(g.opacity.astype(np.float64), 1e-4, 1 - 1e-4)).astype(np.float32),
+                raw_scalar=logit(np.clip(g.scalar.astype(np.float64), 1e-4, 1 - 1e-4)).astype(np.float32))
+
+
+def test_activate_and_adam_elementwise(oracle):
+    import torch
+    from paper_2607_01164_b200 import api
+    rng = np.random.default_rng(3)
+    n = 5000
+    raw = dict(mean=rng.uniform(0, 1, (n, 3)), raw_scale=rng.uniform(-6, -2, (n, 3)), quat=rng.standard_normal((n, 4)),
+               raw_opacity=2 * rng.standard_normal(n), raw_scalar=2 * rng.standard_normal(n))
+    raw = {k: v.astype(np.float32) for k, v in raw.items()}
+    ctx = api.Context()
+    rd = {k: to_dev(torch, raw[k])[0] for k in KEYS}
+    s_d, w_d, v_d = torch.empty(n, 3, device="cuda"), torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    ctx.gs_params_activate(rd, s_d, w_d, v_d)
+    s, w, v = oracle.activate(raw["raw_scale"], raw["raw_opacity"], raw["raw_scalar"])
+    np.testing.assert_allclose(s_d.cpu().numpy(), s, rtol=1e-6)
+    np.testing.assert_allclose(w_d.cpu().numpy(), w, rtol=1e-6)
+    np.testing.assert_allclose(v_d.cpu().numpy(), v, rtol=1e-6)
+    # three Adam steps with gradients of very different magnitudes (some exactly zero)
+    po = {k: raw[k].astype(np.float64) for k in KEYS}
+    mo, vo = np.zeros(12 * n), np.zeros(12 * n)
+    m_d, vv_d = torch.zeros(12 * n, device="cuda"), torch.zeros(12 * n, device="cuda")
+    for t in range(1, 4):
+        mag = 10.0 ** rng.uniform(-6, 1, n)
+        g = dict(dmean=mag[:, None] * rng.standard_normal((n, 3)), dscale=mag[:, None] * rng.standard_normal((n, 3)),
+                 dquat=mag[:, None] * rng.standard_normal((n, 4)), dopacity=mag * rng.standard_normal(n), dscalar=mag * rng.standard_normal(n))
+        for a in g.values():
+            a[:50] = 0.0
+        g = {k: a.astype(np.float32) for k, a in g.items()}
+        gd = {k: to_dev(torch, a)[0] for k, a in g.items()}
+        ctx.gs_adam_step(rd, gd, m_d, vv_d, t, scale_out=s_d, opacity_out=w_d, scalar_out=v_d)
+        oracle.adam_step(po, {k: a.astype(np.float64) for k, a in g.items()}, mo, vo, t, **HYPER)
+        torch.cuda.synchronize()
+        for k in KEYS:
+            got = rd[k].cpu().numpy().astype(np.float64)
+            # fp32: the parameter itself rounds at 6e-8 |p| per step; the update carries ~1e-6 relative error
+            tol = t * (1.2e-7 * np.abs(po[k]) + 3e-6 * LR[k])
+            assert np.all(np.abs(got - po[k]) <= tol), (k, t, np.abs(got - po[k]).max())
+        # b1 m + (1 - b1) g cancels when consecutive gradients differ in sign and size: relative to the result the fp32
+        # rounding of the terms can reach 1e-4; the second moment is a sum of squares (no cancellation)
+        np.testing.assert_allclose(m_d.cpu().numpy(), mo, rtol=5e-4, atol=1e-30)
+        np.testing.assert_allclose(vv_d.cpu().numpy(), vo, rtol=4e-6, atol=1e-36)
+    # the activations written by the step are those of the updated parameters
+    s, w, v = oracle.activate(rd["raw_scale"].cpu().numpy(), rd["raw_opacity"].cpu().numpy(), rd["raw_scalar"].cpu().numpy())
+    np.testing.assert_allclose(s_d.cpu().numpy(), s, rtol=1e-6)
+    np.testing.assert_allclose(w_d.cpu().numpy(), w, rtol=1e-6)
+    np.testing.assert_allclose(v_d.cpu().numpy(), v, rtol=1e-6)
+    # argument errors
+    with pytest.raises(api.GsError):
+        ctx.gs_adam_step(rd, gd, m_d, vv_d, 0)
+    with pytest.raises(api.GsError):
+        ctx.gs_adam_step(rd, gd, m_d, vv_d, 1, beta1=1.0)
+    ctx.close()
+
+
+def test_training_loop_c1(oracle):
+    """configs[0]: 1,024 Gaussians fitted to the field of a second set on the 32^3 grid with the paper's recipe (L1 + Eq. 4,
+    Adam).  The first steps are replayed with the oracle (forward, loss, backward, Adam in
+    double); afterwards the loss must keep falling."""
+    import torch
+    from paper_2607_01164_b200 import api
+    g0 = inputs.c1_gaussians(seed=0, n=1024)
+    g2 = inputs.c1_gaussians(seed=1, n=1024)
+    grid = inputs.c1_grid(32)
+    xyz = oracle.grid_points(grid)
+    target = oracle.forward(g2, xyz, TAU, mode=1, want_sets=False)["phi"].astype(np.float32)
+    P, n = grid.num_points, g0.n
+    raw = _raw_from(g0)
+    lam_fn, eps_fn = 0.5, 0.5
+
+    # ---- GPU loop
+    ctx = api.Context()
+    rd = {k: to_dev(torch, raw[k])[0] for k in KEYS}
+    s_d, w_d, v_d = torch.empty(n, 3, device="cuda"), torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    ctx.gs_params_activate(rd, s_d, w_d, v_d)
+    m_d, vv_d = torch.zeros(12 * n, device="cuda"), torch.zeros(12 * n, device="cuda")
+    q = api.grid_query(grid)
+    f32 = dict(dtype=torch.float32, device="cuda")
+    phi, I, dphi, dI = (torch.empty(P, **f32) for _ in range(4))
+    terms = torch.zeros(3, dtype=torch.float64, device="cuda")
+    t_d = to_dev(torch, target)[0]
+    grads = ctx.alloc_grads(n)
+    steps, replay = 150, 3
+    losses, snaps = [], []
+    for t in range(1, steps + 1):
+        ctx.gs_preprocess(rd["mean"], s_d, rd["quat"], w_d, v_d, tau=TAU)
+        ctx.gs_build_accel(q)
+        ctx.gs_sample_fwd_loss(q, phi, I, t_d, kind=api.LOSS_L1, lambda_fn=lam_fn, eps_fn=eps_fn, loss_terms=terms, dL_dphi=dphi, dL_dI=dI)
+        ctx.gs_sample_bwd(q, phi, I, dphi, grads, dL_dI=dI, target=t_d)
+        ctx.gs_adam_step(rd, grads, m_d, vv_d, t, scale_out=s_d, opacity_out=w_d, scalar_out=v_d)
+        losses.append(terms.cpu().numpy().copy())
+        if t <= replay:
+            snaps.append({k: rd[k].cpu().numpy().astype(np.float64) for k in KEYS})
+    ctx.close()
+    total = np.array([l[0] + l[1] for l in losses])
+    assert total[-1] < 0.9 * total[0] and total[-10:].mean() < total[:10].mean(), total[[0, -1]]
+    assert np.all(np.isfinite(total))
+
+    # ---- the same first steps with the oracle (parameters in double, cast to float32 where the sampler takes them)
+    class G:
+        pass
+    po = {k: raw[k].astype(np.float64) for k in KEYS}
+    mo, vo = np.zeros(12 * n), np.zeros(12 * n)
+    for t in range(1, replay + 1):
+        s, w, v = oracle.activate(po["raw_scale"].astype(np.float32), po["raw_opacity"].astype(np.float32), po["raw_scalar"].astype(np.float32))
+        g = G()
+        g.n, g.mean, g.scale, g.quat = n, po["mean"].astype(np.float32), s.astype(np.float32), po["quat"].astype(np.float32)
+        g.opacity, g.scalar = w.astype(np.float32), v.astype(np.float32)
+        fwd = oracle.forward(g, xyz, TAU, mode=1)
+        ref = oracle.loss(fwd["phi"], fwd["I"], target, None, TAU, "l1", lam_fn, eps_fn, 0.0)
+        gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], ref["dL_dphi"], ref["dL_dI"], target, TAU, mode=1)
+        # the two sides activate in different precisions (float32 expf vs double exp rounded), so their float32 parameters
+        # differ by an ulp here and there and a few boundary pairs / L1 signs may flip: compare with tolerances
+        assert losses[t - 1][0] == pytest.approx(ref["loss"][0], rel=2e-4)
+        assert losses[t - 1][1] == pytest.approx(ref["loss"][1], rel=2e-3, abs=1e-7)
+        oracle.adam_step(po, gr, mo, vo, t, **HYPER)
+        for k in KEYS:
+            d = np.abs(snaps[t - 1][k] - po[k])
+            # Adam's step is lr * g / (|g| + eps): elements whose gradient is ~0 may step either way; the rest must agree
+            frac_off = float((d > 0.02 * t * LR[k] + 2e-7 * np.abs(po[k])).mean())
+            assert frac_off < 0.03, (k, t, frac_off)
+            assert d.max() <= 2.001 * t * LR[k] + 2e-7 * np.abs(po[k]).max(), (k, t, d.max())
