@@ -36,7 +36,7 @@ ALU_PEAK_TINSTR = 148 * 128 * 1.965e9 / 1e12
 NCU_TRAFFIC = {
     ("c2", "k_grid_bwd"): (190.37e6 + 28.29e6, "profiles/r1_step4_c2_ncu_full.md"),
     ("c2", "k_grid_fwd"): (113.57e6 + 224.11e6, "profiles/r1_step4_c2_ncu_full.md"),
-    ("c3", "k_points_bwd"): (576.11e6 + 67.30e6, "profiles/r1_step3_c3_ncu_full.md"),
+    ("c3", "k_points_bwd"): (536.48e6 + 65.86e6, "profiles/r1_step4_c3.md"),
 }
 
 
