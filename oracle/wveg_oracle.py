@@ -195,6 +195,65 @@ def adam_step(params: dict, grads: dict, m, v, t: int, lr=PAPER_LR, beta1=0.9, b
                        _p(g["dscalar"]), _p(m), _p(v), _p(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(t))
 
 
+PARAM_KEYS = ("mean", "raw_scale", "quat", "raw_opacity", "raw_scalar")
+_WIDTH = dict(mean=3, raw_scale=3, quat=4, raw_opacity=1, raw_scalar=1)
+
+
+def _moment_blocks(m, n):
+    """Views of a [12 n] moment block: mean 3n | scale 3n | quat 4n | opacity n | scalar n."""
+    out, o = {}, 0
+    for k in PARAM_KEYS:
+        out[k] = m[o:o + _WIDTH[k] * n]
+        o += _WIDTH[k] * n
+    return out
+
+
+def prune(params: dict, m, v, opacity, tau2: float = 0.005):
+    """Pruning: "periodically removes Gaussians below a chosen ... threshold", here the weight threshold
+    0.005.  Keeps, in their order, the Gaussians with opacity >= tau2 (decided on the float32 activated opacity);
+    their parameters and Adam moments move with them.  Returns (params, m, v, kept indices)."""
+    keep = np.flatnonzero(np.asarray(opacity, np.float32) >= np.float32(tau2))
+    n, n2 = len(opacity), len(keep)
+    mb, vb = _moment_blocks(np.asarray(m), n), _moment_blocks(np.asarray(v), n)
+    p2 = {k: np.ascontiguousarray(np.asarray(params[k]).reshape(n, -1)[keep]).reshape((n2,) + np.asarray(params[k]).shape[1:]) for k in PARAM_KEYS}
+    m2 = np.concatenate([mb[k].reshape(n, -1)[keep].ravel() for k in PARAM_KEYS])
+    v2 = np.concatenate([vb[k].reshape(n, -1)[keep].ravel() for k in PARAM_KEYS])
+    return p2, m2, v2, keep
+
+
+def densify_select(sample_err, I, defined, k: int, tau: float = 0.01):
+    """Sample-error densification ("new Gaussians with means at the positions of the k highest error
+    samples"; "we include false negative positions as the top priority").  Candidates are the samples
+    defined in the volume; a false negative is a defined sample the model does not cover (I <= tau, Fig. 6A).  Order:
+    false negatives first, then by error, highest first; equal errors by sample index, lowest first.  Returns the
+    indices of the first min(k, number of defined samples) samples of that order."""
+    err = np.asarray(sample_err, np.float32)
+    If = np.asarray(I, np.float32)
+    P = len(err)
+    d = np.ones(P, bool) if defined is None else (np.asarray(defined) != 0)
+    fn = d & ~(If > np.float32(tau))
+    cand = np.flatnonzero(d)
+    order = sorted(cand.tolist(), key=lambda c: (not fn[c], -float(err[c]), c))
+    return np.asarray(order[:min(k, len(order))], np.int64)
+
+
+def densify(params: dict, m, v, positions, target, sel, raw_scale_init: float, raw_opacity_init: float, clamp: float = 1e-4):
+    """Appends one Gaussian per selected sample, "given parameters in the same way as initialization, with values
+    corresponding to the ground truth samples" (isotropic, initial weight 0.01, scale by the
+    caller): mean = sample position, raw_scale = raw_scale_init on the three axes, identity rotation,
+    raw_opacity = raw_opacity_init, raw_scalar = logit(clip(target, clamp, 1 - clamp)); zero Adam moments."""
+    n, a = len(params["raw_opacity"]), len(sel)
+    t = np.clip(np.asarray(target, np.float32)[sel].astype(np.float64), clamp, 1 - clamp)
+    new = dict(mean=np.asarray(positions, np.float32)[sel].astype(np.float64), raw_scale=np.full((a, 3), np.float32(raw_scale_init), np.float64),
+               quat=np.tile(np.array([1.0, 0, 0, 0]), (a, 1)), raw_opacity=np.full(a, np.float32(raw_opacity_init), np.float64),
+               raw_scalar=np.log(t / (1 - t)))
+    p2 = {k: np.concatenate([np.asarray(params[k], np.float64), new[k]]) for k in PARAM_KEYS}
+    mb, vb = _moment_blocks(np.asarray(m), n), _moment_blocks(np.asarray(v), n)
+    m2 = np.concatenate([np.concatenate([mb[k], np.zeros(_WIDTH[k] * a)]) for k in PARAM_KEYS])
+    v2 = np.concatenate([np.concatenate([vb[k], np.zeros(_WIDTH[k] * a)]) for k in PARAM_KEYS])
+    return p2, m2, v2
+
+
 def backward(g, xyz, phi, I, a, b=None, target=None, tau: float = 0.01, mode: int = 1, hit_mask_in=None,
              covered_in=None):
     """Returns dict(dmean [N,3], dscale [N,3], dquat [N,4], dopacity [N], dscalar [N], err [N]) in f64."""
