@@ -271,6 +271,27 @@ typedef struct gs_adam_cfg {
 gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, float *m, float *v, const gs_adam_cfg *cfg,
                        float *scale_out, float *opacity_out, float *scalar_out);
 
+/* Pruning (Gaussians below the weight threshold, 0.005 in the paper, are removed).  Keeps, in their
+ * order, the Gaussians with opacity[i] >= tau2 (`opacity` = the ACTIVATED weights, device [n], e.g. the
+ * opacity_out of gs_adam_step); parameters and both Adam moment blocks are compacted in place (the blocks are
+ * re-laid-out for the new count).  *n_new_host = the new count; the caller updates p->n.  Synchronises.
+ * Errors: INVALID_ARG, OOM, CUDA. */
+gs_status gs_prune(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, const float *opacity, float tau2, uint32_t *n_new_host);
+
+/* Sample-error densification: one new Gaussian at each of the k highest-error samples of the
+ * query the accel was built for, false negatives (defined samples with I <= tau) first, equal errors by lower sample
+ * index; only samples marked in `defined` (device uint8 [P], NULL = all; num_defined = their count) are candidates.
+ * sample_err, I, target: device [P] (the outputs / input of the last forward).  At most capacity - p->n Gaussians
+ * are added (`capacity` = Gaussians the caller's parameter arrays and [12 capacity] moment arrays can hold).
+ * A new Gaussian is initialised as in PAPER.md:140 / :154: mean = the sample position, raw_scale = raw_scale_init on
+ * all axes (the paper's density-dependent initial scale has no printed formula: the caller's), identity rotation,
+ * raw_opacity = raw_opacity_init (logit of 0.01 in the paper), raw_scalar = logit(clip(target, 1e-4, 1 - 1e-4)),
+ * zero Adam moments.  *n_new_host = the new count; the caller updates p->n.  Synchronises.
+ * Errors: STATE (no accel), INVALID_ARG, OOM, CUDA. */
+gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, uint32_t capacity, const gs_query *q,
+                     const float *sample_err, const float *I, const uint8_t *defined, uint64_t num_defined, const float *target,
+                     uint32_t k, float raw_scale_init, float raw_opacity_init, uint32_t *n_new_host);
+
 /* ---- measurement: CUDA-event timing of the stages, on the context's stream --------------------
  * While enabled, every stage of the calls above is bracketed by a pair of CUDA events recorded on
  * the context's stream.  gs_profile_read synchronises the stream, adds up the elapsed time of all

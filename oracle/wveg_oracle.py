@@ -241,9 +241,11 @@ def densify(params: dict, m, v, positions, target, sel, raw_scale_init: float, r
     """Appends one Gaussian per selected sample, "given parameters in the same way as initialization, with values
     corresponding to the ground truth samples" (isotropic, initial weight 0.01, scale by the
     caller): mean = sample position, raw_scale = raw_scale_init on the three axes, identity rotation,
-    raw_opacity = raw_opacity_init, raw_scalar = logit(clip(target, clamp, 1 - clamp)); zero Adam moments."""
+    raw_opacity = raw_opacity_init, raw_scalar = logit(clip(target, clamp, 1 - clamp)) with the float32 bounds clamp and
+    1.0f - clamp (the target is float32); zero Adam moments."""
     n, a = len(params["raw_opacity"]), len(sel)
-    t = np.clip(np.asarray(target, np.float32)[sel].astype(np.float64), clamp, 1 - clamp)
+    lo, hi = float(np.float32(clamp)), float(np.float32(1.0) - np.float32(clamp))
+    t = np.clip(np.asarray(target, np.float32)[sel].astype(np.float64), lo, hi)
     new = dict(mean=np.asarray(positions, np.float32)[sel].astype(np.float64), raw_scale=np.full((a, 3), np.float32(raw_scale_init), np.float64),
                quat=np.tile(np.array([1.0, 0, 0, 0]), (a, 1)), raw_opacity=np.full(a, np.float32(raw_opacity_init), np.float64),
                raw_scalar=np.log(t / (1 - t)))

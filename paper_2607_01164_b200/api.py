@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -110,6 +110,9 @@ def load_library():
     lib.gs_debug_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.gs_params_activate.argtypes = [P, C.POINTER(_RawParams), P, P, P]
     lib.gs_adam_step.argtypes = [P, C.POINTER(_RawParams), C.POINTER(_Grads), P, P, C.POINTER(_AdamCfg), P, P, P]
+    lib.gs_prune.argtypes = [P, C.POINTER(_RawParams), P, P, P, C.c_float, C.POINTER(C.c_uint32)]
+    lib.gs_densify.argtypes = [P, C.POINTER(_RawParams), P, P, C.c_uint32, C.POINTER(_Query), P, P, P, C.c_uint64, P, C.c_uint32,
+                               C.c_float, C.c_float, C.POINTER(C.c_uint32)]
     lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
@@ -271,6 +274,25 @@ class Context:
         cfg = _AdamCfg((C.c_float * 5)(*lr), beta1, beta2, eps, int(step))
         self._check(self.lib.gs_adam_step(self.h, C.byref(r), C.byref(g), _ptr(m), _ptr(v), C.byref(cfg), _ptr(scale_out),
                                           _ptr(opacity_out), _ptr(scalar_out)))
+
+    def gs_prune(self, raw: dict, n: int, m, v, opacity, tau2: float = 0.005) -> int:
+        """raw: dict of device tensors with room for >= n Gaussians; returns the new count."""
+        r = self._raw(raw)
+        r.n = int(n)
+        out = C.c_uint32()
+        self._check(self.lib.gs_prune(self.h, C.byref(r), _ptr(m), _ptr(v), _ptr(opacity), C.c_float(tau2), C.byref(out)))
+        return int(out.value)
+
+    def gs_densify(self, raw: dict, n: int, m, v, capacity: int, q: _Query, sample_err, I, target, k: int, raw_scale_init: float,
+                   raw_opacity_init: float, defined=None, num_defined=None) -> int:
+        r = self._raw(raw)
+        r.n = int(n)
+        nd = query_num_points(q) if num_defined is None else int(num_defined)
+        out = C.c_uint32()
+        self._check(self.lib.gs_densify(self.h, C.byref(r), _ptr(m), _ptr(v), int(capacity), C.byref(q), _ptr(sample_err), _ptr(I),
+                                        _ptr(defined), nd, _ptr(target), int(k), C.c_float(raw_scale_init),
+                                        C.c_float(raw_opacity_init), C.byref(out)))
+        return int(out.value)
 
     def measure_alu_peaks(self):
         """(FP32 FMA lane-instructions per second, MUFU.EX2 per second) of this device now; synchronises."""

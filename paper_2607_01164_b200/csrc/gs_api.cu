@@ -140,7 +140,8 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->grid_order, &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
-                     &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg};
+                     &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
+                     &ctx->sel_val[0], &ctx->sel_val[1]};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
@@ -542,6 +543,69 @@ gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, f
         if (!(cfg->lr[k] >= 0.f) || !isfinite(cfg->lr[k])) return fail(ctx, GS_ERR_INVALID_ARG, "gs_adam_step: lr must be finite and >= 0");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     CK(launch_adam_step(*p, *g, m, v, *cfg, scale_out, opacity_out, scalar_out, ctx->stream), "adam step");
+    return GS_OK;
+}
+
+gs_status gs_prune(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, const float *opacity, float tau2, uint32_t *n_new_host) {
+    if (!ctx || !p || !n_new_host) return GS_ERR_INVALID_ARG;
+    const uint32_t n = p->n;
+    if (n > 0 && (!p->mean || !p->raw_scale || !p->quat || !p->raw_opacity || !p->raw_scalar || !m || !v || !opacity))
+        return fail(ctx, GS_ERR_INVALID_ARG, "gs_prune: null pointer");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    CK(ctx->dens_work.reserve((3 * (size_t)n + 2) * 4), "alloc prune index");
+    uint32_t *work = ctx->dens_work.as<uint32_t>();
+    CK(launch_prune_index(opacity, n, tau2, work, ctx->scan_tmp, s), "prune index");
+    uint32_t kept = 0;
+    CK(cudaMemcpyAsync(&kept, work + 2 * (size_t)n, 4, cudaMemcpyDeviceToHost, s), "read kept count");
+    CK(cudaStreamSynchronize(s), "sync");
+    if (kept < n) {
+        CK(ctx->dens_scratch.reserve(37 * (size_t)(kept ? kept : 1) * 4), "alloc prune scratch");
+        CK(launch_regather(*p, m, v, kept, work + 2 * (size_t)n + 1, kept, ctx->dens_scratch.as<float>(), true, s), "prune gather");
+        CK(cudaStreamSynchronize(s), "sync");
+    }
+    *n_new_host = kept;
+    return GS_OK;
+}
+
+gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, uint32_t capacity, const gs_query *q,
+                     const float *sample_err, const float *I, const uint8_t *defined, uint64_t num_defined, const float *target,
+                     uint32_t k, float raw_scale_init, float raw_opacity_init, uint32_t *n_new_host) {
+    if (!ctx || !p || !n_new_host) return GS_ERR_INVALID_ARG;
+    gs_status st = check_ready(ctx, q, "gs_densify before gs_preprocess/gs_build_accel");
+    if (st != GS_OK) return st;
+    const uint32_t n = p->n;
+    const uint64_t P = ctx->P;
+    if (capacity < n) return fail(ctx, GS_ERR_INVALID_ARG, "gs_densify: capacity < n");
+    if (!p->mean || !p->raw_scale || !p->quat || !p->raw_opacity || !p->raw_scalar || !m || !v)
+        return fail(ctx, GS_ERR_INVALID_ARG, "gs_densify: null pointer");
+    if (P > 0 && (!sample_err || !I || !target)) return fail(ctx, GS_ERR_INVALID_ARG, "gs_densify: sample_err, I and target must be given");
+    if (num_defined > P || (!defined && num_defined != P)) return fail(ctx, GS_ERR_INVALID_ARG, "gs_densify: num_defined must be |D| (P when defined is NULL)");
+    if (!isfinite(raw_scale_init) || !isfinite(raw_opacity_init)) return fail(ctx, GS_ERR_INVALID_ARG, "gs_densify: init values must be finite");
+    uint64_t add64 = k;
+    if (add64 > capacity - n) add64 = capacity - n;
+    if (add64 > num_defined) add64 = num_defined;
+    const uint32_t add = (uint32_t)add64, n_new = n + add;
+    *n_new_host = n_new;
+    if (add == 0) return GS_OK;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    for (int b = 0; b < 2; b++) {
+        CK(ctx->sel_key[b].reserve(P * 4), "alloc selection keys");
+        CK(ctx->sel_val[b].reserve(P * 4), "alloc selection values");
+    }
+    uint32_t *keys[2] = {ctx->sel_key[0].as<uint32_t>(), ctx->sel_key[1].as<uint32_t>()};
+    uint32_t *vals[2] = {ctx->sel_val[0].as<uint32_t>(), ctx->sel_val[1].as<uint32_t>()};
+    CK(launch_select_keys(sample_err, I, defined, P, ctx->tau, keys[0], vals[0], s), "selection keys");
+    int sel = 0;
+    CK(radix_sort_pairs(keys, vals, P, 32, ctx->sort_hist, ctx->scan_tmp, s, &sel), "selection sort");
+    CK(ctx->dens_scratch.reserve(37 * (size_t)n_new * 4), "alloc densify scratch");
+    float *scratch = ctx->dens_scratch.as<float>();
+    CK(launch_regather(*p, m, v, n_new, nullptr, n, scratch, false, s), "densify gather");
+    const float *xyz = ctx->accel_kind == GS_QUERY_POINTS ? ctx->accel_q.xyz : nullptr;
+    CK(launch_new_gaussians(*p, m, v, n_new, vals[sel], ctx->grid, xyz, target, raw_scale_init, raw_opacity_init, 1e-4f, scratch, s),
+       "new gaussians");
+    CK(cudaStreamSynchronize(s), "sync");
     return GS_OK;
 }
 

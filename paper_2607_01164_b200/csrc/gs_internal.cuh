@@ -119,6 +119,7 @@ struct gs_ctx {
     bool have_pt_order = false;
     // ---- scratch
     gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters, dbg;
+    gs::DevBuf dens_work, dens_scratch, sel_key[2], sel_val[2];  // gs_prune / gs_densify
     bool fused_pack = false;  // misc holds the coefficients written by the last gs_sample_fwd with a target
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
@@ -186,6 +187,18 @@ cudaError_t launch_finalize(const float4 *rec, const float *params, const float 
 cudaError_t launch_activate(const gs_raw_params &p, float *scale, float *opacity, float *scalar, cudaStream_t s);
 cudaError_t launch_adam_step(const gs_raw_params &p, const gs_grads &g, float *m, float *v, const gs_adam_cfg &cfg, float *scale_out,
                              float *opacity_out, float *scalar_out, cudaStream_t s);
+
+// densify.cu: pruning and sample-error densification (all on `s`; `work` = 3 n + 1 uint32: flags | positions (n + 1) | kept indices)
+cudaError_t launch_prune_index(const float *opacity, uint32_t n, float tau2, uint32_t *work, DevBuf &scan_tmp, cudaStream_t s);
+// gathers the parameters and moments of the first n_copy Gaussians of the new set (src = NULL: identity) into `scratch`
+// (37 n_new floats, laid out for n_new) and, with back = true, copies all of it back over the caller's arrays
+cudaError_t launch_regather(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *src, uint32_t n_copy, float *scratch,
+                            bool back, cudaStream_t s);
+cudaError_t launch_select_keys(const float *err, const float *I, const uint8_t *defined, size_t P, float tau, uint32_t *key, uint32_t *val,
+                               cudaStream_t s);
+cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *sel, const GridDesc &gd,
+                                 const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
+                                 float *scratch, cudaStream_t s);
 
 // peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)
 cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s);
