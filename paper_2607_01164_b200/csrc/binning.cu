@@ -117,6 +117,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         c = brick_range(b6, gd, br);
         count[i] = c;
         if (c) atomicAdd(hist + nbricks + order_key(br, gd, order_shift), 1u);
+      if (c) {  // a Gaussian that touches no brick of the batch is never looked at again (no record read, no setup row)
         // ---- backward setup
         int clo[3], nc[3];
         bool empty = false, edge = false;
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
                                            __uint_as_float((empty ? 1u : 0u) | (edge ? 2u : 0u)));
         setup[2 * (size_t)i + 1] = make_float4(__uint_as_float((uint32_t)nc[0] | ((uint32_t)nc[1] << 11) | ((uint32_t)nc[2] << 22)),
                                                reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
+      }
     }
     for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t) { atomicAdd(hist + b, 1u); });
     // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
 // Every pair takes a slot of its brick's run by counting the brick's histogram entry DOWN (so the histogram is
 // all zero again afterwards); the order list of the backward is filled the same way.  Nothing is written when
 // the pair list does not fit `cap` entries: the host then grows the buffer and repeats this kernel.
-__global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aabb, uint32_t N, GridDesc gd,
+__global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aabb, const uint32_t *__restrict__ count, uint32_t N, GridDesc gd,
                                                     const unsigned long long *__restrict__ total, uint32_t cap,
                                                     uint32_t *__restrict__ hist, const uint32_t *__restrict__ start, uint32_t nbricks,
                                                     int order_shift, uint32_t *__restrict__ pair_gauss, uint32_t *__restrict__ order) {
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aab
     const int lane = threadIdx.x & 31;
     uint32_t c = 0;
     BrickRange br{};
-    if (i < N) {
+    if (i < N && count[i]) {  // the count pass left n_i: untouched Gaussians cost 4 bytes here
         float b6[6];
 #pragma unroll
         for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
@@ -295,11 +297,11 @@ cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N,
     return cudaGetLastError();
 }
 
-cudaError_t launch_pair_fill(const float *aabb, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
+cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
                              uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
                              uint32_t *order, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    k_pair_fill<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, gd, total, cap, hist, start, nbricks, order_shift, pair_gauss, order); count_launch();
+    k_pair_fill<<<(N + 255) / 256, 256, 0, s>>>(aabb, count, N, gd, total, cap, hist, start, nbricks, order_shift, pair_gauss, order); count_launch();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_bucket_sort<<<(nbricks + BS_WARPS - 1) / BS_WARPS, BS_WARPS * 32, 0, s>>>(total, cap, start, nbricks, pair_gauss); count_launch();

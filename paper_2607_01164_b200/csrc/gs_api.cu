@@ -224,7 +224,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         unsigned long long T64[2] = {0, 0};
         for (int attempt = 0; attempt < 2; attempt++) {
             const size_t cap = ctx->pair_gauss.cap / 4;
-            CK(launch_pair_fill(ctx->aabb.as<float>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
+            CK(launch_pair_fill(ctx->aabb.as<float>(), ctx->bcount.as<uint32_t>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
                                 ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
                                 ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), s), "pair fill");
             if (attempt == 0) {
@@ -439,7 +439,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     Stage stage(ctx, GS_PROF_FINALIZE);
     const bool grid = ctx->accel_kind == GS_QUERY_GRID;
     CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused) ? in.eps_scale : 1.f,
-                       *out, s), "finalize");
+                       *out, grid ? ctx->grid_order.as<uint32_t>() : nullptr, grid ? ctx->M : 0, s), "finalize");
     return GS_OK;
 }
 

@@ -152,7 +152,7 @@ cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int
 cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
                                unsigned long long *total, uint32_t *hist, uint32_t nbricks, uint32_t norder, int order_shift,
                                float4 *setup, cudaStream_t s);
-cudaError_t launch_pair_fill(const float *aabb, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
+cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
                              uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
                              uint32_t *order, cudaStream_t s);
 cudaError_t launch_expand_bricks(const uint32_t *start, uint32_t nbricks, uint32_t *key, cudaStream_t s);
@@ -180,8 +180,9 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
 
 // grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the
 // cell steps are folded in); eps_scale multiplies the error share (fused MSE: eps = |alpha| * eps_scale, else 1)
+// grid_moments: only the M Gaussians of `order` have a row; the gradients of the others are set to zero
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
-                            float eps_scale, const gs_grads &out, cudaStream_t s);
+                            float eps_scale, const gs_grads &out, const uint32_t *order, uint32_t M, cudaStream_t s);
 
 // optim.cu: activations of the raw parameters and one Adam step on them
 cudaError_t launch_activate(const gs_raw_params &p, float *scale, float *opacity, float *scalar, cudaStream_t s);

@@ -107,7 +107,10 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     const float4 s0 = __ldg(setup + 2 * (size_t)i), s1 = __ldg(setup + 2 * (size_t)i + 1);
     const int clo[3] = {__float_as_int(s0.x), __float_as_int(s0.y), __float_as_int(s0.z)};
     const uint32_t flags = __float_as_uint(s0.w), ncp = __float_as_uint(s1.x);
-    if (flags & 1u) continue;  // empty: the accumulator row stays zero (memset by the launcher)
+    if (flags & 1u) {  // touches a brick of the batch but none of its voxels: a zero row (rows are not pre-zeroed)
+        gacc[(size_t)i * GACC_GRID + lane] = 0.f;
+        continue;
+    }
     const bool edge = (flags & 2u) || odd_x;
     const int ncx = (int)(ncp & 2047u), ncy = (int)((ncp >> 11) & 2047u), ncz = (int)(ncp >> 22);
     const float thr = s1.y, invA = s1.z;
@@ -292,9 +295,8 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
                             float r2, float *gacc, const uint32_t *order, uint32_t M, cudaStream_t s) {
-    // untouched Gaussians keep a zero accumulator row
-    cudaError_t e = cudaMemsetAsync(gacc, 0, (size_t)N * GACC_GRID * sizeof(float), s);
-    if (e != cudaSuccess || M == 0) return e;
+    // only the M Gaussians of the order list get (and need) an accumulator row: k_finalize reads those alone
+    if (M == 0) return cudaSuccess;
     const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
     if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
     else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
