@@ -219,3 +219,20 @@ def test_long_brick_runs_sorted(oracle):
     _check_integer_stages(oracle, run, g2, inputs.c1_grid(32))
     lens = np.diff(run.ctx.debug_get(run.api.DBG_BRICK_START, np.uint32).astype(np.int64))
     assert ((lens > 32) & (lens <= 128)).any() and ((lens > 128) & (lens <= 1024)).any()
+
+
+def test_structured_path_is_deterministic(oracle):
+    # the brick lists are filled through atomics but every run is sorted, and the backward uses no atomics: two passes
+    # over the same inputs give bit-identical samples and gradients (the loss scalar is summed with atomics: not compared)
+    grid = inputs.Grid((44, 29, 21), (-0.1, 0.2, 0.0), (1 / 40, 1 / 32, 1 / 20))
+    g = inputs.c4_gaussians(seed=9, n_grid=40, n=4000)
+    target = np.random.default_rng(4).uniform(0, 1, grid.num_points).astype(np.float32)
+    runs = [GpuRun(g, "grid", grid, target, fused=True) for _ in range(2)]
+    a, b = runs
+    assert np.array_equal(a.np(a.phi).view(np.uint32), b.np(b.phi).view(np.uint32))
+    assert np.array_equal(a.np(a.I).view(np.uint32), b.np(b.I).view(np.uint32))
+    ga, gb = a.grads_np(), b.grads_np()
+    for k in ga:
+        assert np.array_equal(ga[k], gb[k]), k
+    pa = a.ctx.debug_get(a.api.DBG_PAIR_GAUSS, np.uint32)
+    assert np.array_equal(pa, b.ctx.debug_get(b.api.DBG_PAIR_GAUSS, np.uint32))
