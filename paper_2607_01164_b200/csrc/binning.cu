@@ -48,10 +48,12 @@ __device__ __forceinline__ uint32_t spread3(uint32_t v) {  // 10 bits -> every t
     return v;
 }
 
-// ---- enumeration of the bricks of a range.  A thread walks its own Gaussian's bricks when there are at most
-// SERIAL_MAX of them; larger ranges are spread over the 32 lanes of the warp, one Gaussian after the other.
+// ---- enumeration of the bricks of a range ("parallelizes over total intersections").  The ranges of the
+// 32 Gaussians of a warp are laid end to end (warp scan of their sizes) and the pairs are dealt to the lanes 32 at a
+// time: a lane finds the Gaussian of its pair by a binary search in the scan (5 shuffles) and the brick by index
+// arithmetic.  Ranges of more than COOP_MAX bricks are spread over the warp one Gaussian after the other.
 // f(brick_id, gaussian_id) is called exactly once per (brick, gaussian) pair.  All 32 lanes must call this.
-constexpr uint32_t SERIAL_MAX = 27;
+constexpr uint32_t COOP_MAX = 1024;
 
 template <class F>
 __device__ __forceinline__ void for_each_pair(const BrickRange &br, uint32_t c, uint32_t i, const GridDesc &gd, int lane, F f) {
@@ -61,12 +63,37 @@ __device__ __forceinline__ void for_each_pair(const BrickRange &br, uint32_t c, 
     const uint32_t b0 = c ? (((uint32_t)(br.lo[2] - gd.brick_lo[2]) * nby + (uint32_t)(br.lo[1] - gd.brick_lo[1])) * nbx +
                              (uint32_t)(br.lo[0] - gd.brick_lo[0]))
                           : 0u;
-    const bool big = c > SERIAL_MAX;
-    if (c && !big) {
-        const uint32_t ez = c / (ex * ey);
-        for (uint32_t z = 0; z < ez; z++)
-            for (uint32_t y = 0; y < ey; y++)
-                for (uint32_t x = 0; x < ex; x++) f(b0 + (z * nby + y) * nbx + x, i);
+    const bool big = c > COOP_MAX;
+    const uint32_t cs = big ? 0u : c;
+    uint32_t incl = cs;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += up;
+    }
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, 31), excl = incl - cs;
+    const float rex = 1.0f / (float)ex, rey = 1.0f / (float)ey;
+    for (uint32_t t0 = 0; t0 < total; t0 += 32) {
+        const uint32_t t = t0 + (uint32_t)lane;
+        int src = 0;  // smallest lane whose inclusive count exceeds t
+#pragma unroll
+        for (int step = 16; step > 0; step >>= 1) {
+            const uint32_t v = __shfl_sync(0xffffffffu, incl, src + step - 1);
+            if (v <= t) src += step;
+        }
+        const uint32_t sexcl = __shfl_sync(0xffffffffu, excl, src), sex = __shfl_sync(0xffffffffu, ex, src),
+                       sey = __shfl_sync(0xffffffffu, ey, src), sb0 = __shfl_sync(0xffffffffu, b0, src),
+                       si = __shfl_sync(0xffffffffu, i, src);
+        const float srex = __shfl_sync(0xffffffffu, rex, src), srey = __shfl_sync(0xffffffffu, rey, src);
+        if (t < total) {
+            // local < 1024: (local + 0.5) / e is at least 0.5 / 1024 away from an integer, far more than fp32 rounding
+            const uint32_t local = t - sexcl;
+            const uint32_t r = (uint32_t)(((float)local + 0.5f) * srex);
+            const uint32_t x = local - r * sex;
+            const uint32_t z = (uint32_t)(((float)r + 0.5f) * srey);
+            const uint32_t y = r - z * sey;
+            f(sb0 + (z * nby + y) * nbx + x, si);
+        }
     }
     uint32_t todo = __ballot_sync(0xffffffffu, big);
     while (todo) {
