@@ -168,6 +168,13 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2607_01164_b200 import build as gs_build
+    if not os.path.exists(gs_build.LIB):  # a fresh checkout: local rank 0 builds the library, the others wait for it
+        if local == 0:
+            gs_build.build()
+        t_wait = time.time()
+        while not os.path.exists(gs_build.LIB) and time.time() - t_wait < 600:
+            time.sleep(0.5)
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
