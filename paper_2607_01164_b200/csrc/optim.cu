@@ -1,7 +1,7 @@
 // optim.cu -- training-step completion: the activations of the raw parameters (PAPER.md:140:
 // sigmoid for v_i and w_i, exponential for S_i; R_i is normalised inside k_preprocess) and one Adam step
 // (Kingma & Ba, the paper's [20]; learning rates of PAPER.md:231) on the raw parameters, fed with the gradients
-// w.r.t. the ACTIVATED values that gs_sample_bwd returns.  One thread per Gaussian; HBM-bound
+// w.r.t. the ACTIVATED values that gs_sample_bwd returns.  One thread per parameter element; HBM-bound
 // (13 parameters + 13 gradients + 2 x 12 moments read, 12 + 24 + 5 written: 340 B per Gaussian).
 #include <math.h>
 
@@ -39,36 +39,38 @@ __device__ __forceinline__ float adam1(float p, float g, float *__restrict__ m, 
     return p - lr * (mk * a.c1inv) / (sqrtf(vk * a.c2inv) + a.eps);
 }
 
-// moments: one block of 12 n floats each, mean 3n | scale 3n | quat 4n | opacity n | scalar n
+// moments: one block of 12 n floats each, mean 3n | scale 3n | quat 4n | opacity n | scalar n -- the same order and
+// widths as the parameter tensors, so element e of the concatenated parameters has its moments at m[e], v[e].
+// One thread per ELEMENT (not per Gaussian): every load and store of a warp is one contiguous 128-byte run.
 __global__ void __launch_bounds__(256) k_adam_step(gs_raw_params p, gs_grads g, float *__restrict__ m, float *__restrict__ v, AdamK a,
                                                     float *__restrict__ scale_out, float *__restrict__ opacity_out,
                                                     float *__restrict__ scalar_out) {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t n = p.n;
-    if (i >= n) return;
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const size_t e = 3 * (size_t)i + k;
+    if (e >= 12 * n) return;
+    if (e < 3 * n) {
         p.mean[e] = adam1(p.mean[e], g.dmean[e], m, v, e, a.lr[0], a);
-        const float rs = p.raw_scale[e];
-        const float rs_new = adam1(rs, g.dscale[e] * expf(rs), m, v, 3 * n + e, a.lr[1], a);  // d exp(x) / dx = exp(x)
-        p.raw_scale[e] = rs_new;
-        if (scale_out) scale_out[e] = expf(rs_new);
-    }
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        const size_t e = 4 * (size_t)i + k;
-        p.quat[e] = adam1(p.quat[e], g.dquat[e], m, v, 6 * n + e, a.lr[2], a);
-    }
-    {
-        const float rw = p.raw_opacity[i];
-        const float rw_new = adam1(rw, g.dopacity[i] * sigmoid_deriv(rw), m, v, 10 * n + i, a.lr[3], a);  // sigmoid' = s (1 - s)
-        p.raw_opacity[i] = rw_new;
-        if (opacity_out) opacity_out[i] = 1.0f / (1.0f + expf(-rw_new));
-        const float rv = p.raw_scalar[i];
-        const float rv_new = adam1(rv, g.dscalar[i] * sigmoid_deriv(rv), m, v, 11 * n + i, a.lr[4], a);
-        p.raw_scalar[i] = rv_new;
-        if (scalar_out) scalar_out[i] = 1.0f / (1.0f + expf(-rv_new));
+    } else if (e < 6 * n) {
+        const size_t k = e - 3 * n;
+        const float rs = p.raw_scale[k];
+        const float rs_new = adam1(rs, g.dscale[k] * expf(rs), m, v, e, a.lr[1], a);  // d exp(x) / dx = exp(x)
+        p.raw_scale[k] = rs_new;
+        if (scale_out) scale_out[k] = expf(rs_new);
+    } else if (e < 10 * n) {
+        const size_t k = e - 6 * n;
+        p.quat[k] = adam1(p.quat[k], g.dquat[k], m, v, e, a.lr[2], a);
+    } else if (e < 11 * n) {
+        const size_t k = e - 10 * n;
+        const float rw = p.raw_opacity[k];
+        const float rw_new = adam1(rw, g.dopacity[k] * sigmoid_deriv(rw), m, v, e, a.lr[3], a);  // sigmoid' = s (1 - s)
+        p.raw_opacity[k] = rw_new;
+        if (opacity_out) opacity_out[k] = 1.0f / (1.0f + expf(-rw_new));
+    } else {
+        const size_t k = e - 11 * n;
+        const float rv = p.raw_scalar[k];
+        const float rv_new = adam1(rv, g.dscalar[k] * sigmoid_deriv(rv), m, v, e, a.lr[4], a);
+        p.raw_scalar[k] = rv_new;
+        if (scalar_out) scalar_out[k] = 1.0f / (1.0f + expf(-rv_new));
     }
 }
 
@@ -86,7 +88,8 @@ cudaError_t launch_adam_step(const gs_raw_params &p, const gs_grads &g, float *m
     a.b1 = cfg.beta1; a.b2 = cfg.beta2; a.eps = cfg.eps;
     a.c1inv = (float)(1.0 / (1.0 - pow((double)cfg.beta1, (double)cfg.step)));
     a.c2inv = (float)(1.0 / (1.0 - pow((double)cfg.beta2, (double)cfg.step)));
-    k_adam_step<<<(p.n + 255) / 256, 256, 0, s>>>(p, g, m, v, a, scale_out, opacity_out, scalar_out); count_launch();
+    const size_t elems = 12 * (size_t)p.n;
+    k_adam_step<<<(unsigned)((elems + 255) / 256), 256, 0, s>>>(p, g, m, v, a, scale_out, opacity_out, scalar_out); count_launch();
     return cudaGetLastError();
 }
 
