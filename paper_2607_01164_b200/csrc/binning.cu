@@ -265,29 +265,53 @@ __global__ void __launch_bounds__(BS_WARPS * 32) k_bucket_sort(const unsigned lo
         }
         if ((uint32_t)lane < n) run[lane] = v;
     } else if (n > 32 && n <= 128) {
-        // rank sort: the ids of a run are distinct, so an id's place is the number of smaller ids.  A lane owns up to
-        // four ids and counts against the whole run, read four at a time as a broadcast from shared memory.
-        uint32_t *a = sm[warp];
+        // four ids per lane (element e = 32 r + lane), the same all-ascending bitonic network: partners in other lanes
+        // come through shuffles, partners in the same lane (e ^ 32) are a register compare-exchange
         uint32_t v[4];
 #pragma unroll
-        for (int r = 0; r < 4; r++) {
-            const uint32_t t = (uint32_t)lane + 32u * r;
-            v[r] = t < n ? run[t] : 0xffffffffu;
-            a[t] = v[r];  // the padding (+inf) is never smaller than an id
-        }
-        __syncwarp();
-        uint32_t rank[4] = {0u, 0u, 0u, 0u};
-        const uint4 *a4 = reinterpret_cast<const uint4 *>(a);
-        const uint32_t groups = (n + 3) >> 2;
-        for (uint32_t t = 0; t < groups; t++) {
-            const uint4 q = a4[t];
+        for (int r = 0; r < 4; r++) v[r] = (uint32_t)lane + 32u * r < n ? run[lane + 32 * r] : 0xffffffffu;
+        auto cmpex = [&](uint32_t mine, uint32_t other, bool lower) { return lower ? min(mine, other) : max(mine, other); };
 #pragma unroll
-            for (int r = 0; r < 4; r++)
-                if (32u * r < n) rank[r] += (q.x < v[r]) + (q.y < v[r]) + (q.z < v[r]) + (q.w < v[r]);  // warp-uniform test
+        for (int k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                const int x = (j == (k >> 1)) ? (k - 1) : j;      // lane ^ x is the partner; the lower index has bit j clear
+                const bool lower = (lane & j) == 0;
+#pragma unroll
+                for (int r = 0; r < 4; r++) v[r] = cmpex(v[r], __shfl_xor_sync(0xffffffffu, v[r], x), lower);
+            }
+        }
+        {   // k = 64: flip e ^ 63 = (lane ^ 31, r ^ 1); the lower index has r even
+            uint32_t o[4];
+#pragma unroll
+            for (int r = 0; r < 4; r++) o[r] = __shfl_xor_sync(0xffffffffu, v[r ^ 1], 31);
+#pragma unroll
+            for (int r = 0; r < 4; r++) v[r] = cmpex(v[r], o[r], (r & 1) == 0);
+#pragma unroll
+            for (int j = 16; j > 0; j >>= 1) {
+                const bool lower = (lane & j) == 0;
+#pragma unroll
+                for (int r = 0; r < 4; r++) v[r] = cmpex(v[r], __shfl_xor_sync(0xffffffffu, v[r], j), lower);
+            }
+        }
+        if (n > 64) {  // k = 128: flip e ^ 127 = (lane ^ 31, r ^ 3), lower index has r < 2; then e ^ 32 = (lane, r ^ 1)
+            uint32_t o[4];
+#pragma unroll
+            for (int r = 0; r < 4; r++) o[r] = __shfl_xor_sync(0xffffffffu, v[r ^ 3], 31);
+#pragma unroll
+            for (int r = 0; r < 4; r++) v[r] = cmpex(v[r], o[r], (r & 2) == 0);
+            const uint32_t a0 = min(v[0], v[1]), a1 = max(v[0], v[1]), a2 = min(v[2], v[3]), a3 = max(v[2], v[3]);
+            v[0] = a0; v[1] = a1; v[2] = a2; v[3] = a3;
+#pragma unroll
+            for (int j = 16; j > 0; j >>= 1) {
+                const bool lower = (lane & j) == 0;
+#pragma unroll
+                for (int r = 0; r < 4; r++) v[r] = cmpex(v[r], __shfl_xor_sync(0xffffffffu, v[r], j), lower);
+            }
         }
 #pragma unroll
         for (int r = 0; r < 4; r++)
-            if ((uint32_t)lane + 32u * r < n) run[rank[r]] = v[r];
+            if ((uint32_t)lane + 32u * r < n) run[lane + 32 * r] = v[r];
     } else if (n > 128 && n <= BS_SMEM) {
         uint32_t *a = sm[warp];
         for (uint32_t t = lane; t < n; t += 32) a[t] = run[t];
