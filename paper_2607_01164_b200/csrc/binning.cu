@@ -178,6 +178,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
                                                reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
       }
     }
+    if (!__any_sync(0xffffffffu, c != 0u)) return;  // a warp whose 32 Gaussians all miss the batch (most warps of a small batch)
     for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t) { atomicAdd(hist + b, 1u); });
     // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
     unsigned long long s = c, m = c ? 1ull : 0ull;
@@ -212,6 +213,7 @@ __global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aab
             order[start[m] - T + (atomicSub(hist + m, 1u) - 1u)] = i;
         }
     }
+    if (!__any_sync(0xffffffffu, c != 0u)) return;
     for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t id) { pair_gauss[start[b] + (atomicSub(hist + b, 1u) - 1u)] = id; });
 }
 
