@@ -16,6 +16,9 @@
 
 namespace gs {
 
+#ifndef GS_FWD_MINB
+#define GS_FWD_MINB 14  // resident CTAs per SM the register allocation must allow (swept 1, 12, 14, 16, 20, 24)
+#endif
 constexpr int FWD_THREADS = 64;
 constexpr int CAP = 128;  // Gaussians staged per round (4 sub-chunks of 32)
 
@@ -26,7 +29,7 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
 
 template <bool SETS>
-__global__ void __launch_bounds__(FWD_THREADS) k_grid_fwd(const float4 *__restrict__ rec, uint32_t N, GridDesc gd,
+__global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const float4 *__restrict__ rec, uint32_t N, GridDesc gd,
                                                            const uint32_t *__restrict__ pair_gauss,
                                                            const uint32_t *__restrict__ brick_start, float tau, float r2, FwdOut o,
                                                            double invP) {
