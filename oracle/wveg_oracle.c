@@ -187,6 +187,37 @@ void wo_grid_points(const wo_grid *gr, float *xyz /*[P,3]*/) {
             }
 }
 
+/* In-cell jitter of the grid samples ("we select a random position in each cell every iteration of     */
+/* training").  The random numbers come from a counter-based generator so that both sides can draw the same ones      */
+/* (DESIGN D26): for the voxel with global index L = (gz * dims_y + gy) * dims_x + gx and axis a,                      */
+/*   h = splitmix64-finaliser(seed + 3 L + a + golden gamma),  j = (h >> 40) * 2^-24 - 0.5  in [-0.5, 0.5)             */
+/* and the sample position is p_a = fmaf(((float)i_a + 0.5f) + j, spacing_a, origin_a) (every step exact or one        */
+/* fp32 rounding; that fp32 value IS the position, as for voxel centres, D6).                                           */
+static inline uint64_t mix64_u64(uint64_t z) {
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+float wo_jitter(uint64_t seed, uint64_t voxel_linear, int axis) {
+    const uint64_t h = mix64_u64(seed + 3ull * voxel_linear + (uint64_t)axis);
+    return (float)(h >> 40) * 5.9604644775390625e-8f - 0.5f;
+}
+void wo_grid_points_jitter(const wo_grid *gr, uint64_t seed, float *xyz /*[P,3]*/) {
+    int32_t bd[3]; grid_batch_dims(gr, bd);
+    int64_t c = 0;
+    for (int32_t z = 0; z < bd[2]; z++)
+        for (int32_t y = 0; y < bd[1]; y++)
+            for (int32_t x = 0; x < bd[0]; x++, c++) {
+                const int32_t g[3] = {x + 8 * gr->brick_lo[0], y + 8 * gr->brick_lo[1], z + 8 * gr->brick_lo[2]};
+                const uint64_t L = ((uint64_t)g[2] * (uint64_t)gr->dims[1] + (uint64_t)g[1]) * (uint64_t)gr->dims[0] + (uint64_t)g[0];
+                for (int a = 0; a < 3; a++) {
+                    const float t = ((float)g[a] + 0.5f) + wo_jitter(seed, L, a);
+                    xyz[3 * c + a] = fmaf(t, gr->spacing[a], gr->origin[a]);
+                }
+            }
+}
+
 /* id hash used to compare per-point intersection SETS (order-free): count, sum and xor of mix(id). */
 static inline uint64_t mix_id(uint32_t id) {
     uint64_t z = (uint64_t)id + 0x9E3779B97F4A7C15ull;

@@ -45,6 +45,7 @@ def lib():
         _lib.wo_r_f32.restype = C.c_float
         _lib.wo_r_f32.argtypes = [C.c_float]
         _lib.wo_num_threads.restype = C.c_int
+        _lib.wo_jitter.restype = C.c_float
         _lib.wo_grid_num_points.restype = C.c_int64
         _lib.wo_brick_keys.restype = C.c_int64
         _lib.wo_forward.restype = C.c_int
@@ -104,13 +105,21 @@ def hit_f32(M9, mu, p, tau: float = 0.01) -> bool:
     return bool(lib().wo_hit_f32(_p(M9), _p(mu), _p(p), C.c_float(tau)))
 
 
-def grid_points(grid) -> np.ndarray:
-    """[P,3] f32 sample positions of a grid batch (voxel centres, x fastest)."""
+def grid_points(grid, jitter_seed=None) -> np.ndarray:
+    """[P,3] f32 sample positions of a grid batch (x fastest): voxel centres, or with jitter_seed one random position
+    inside every voxel's cell (counter-based generator, DESIGN D26)."""
     s = _grid(grid)
     P = int(lib().wo_grid_num_points(C.byref(s)))
     xyz = np.zeros((P, 3), np.float32)
-    lib().wo_grid_points(C.byref(s), _p(xyz))
+    if jitter_seed is None:
+        lib().wo_grid_points(C.byref(s), _p(xyz))
+    else:
+        lib().wo_grid_points_jitter(C.byref(s), C.c_uint64(int(jitter_seed)), _p(xyz))
     return xyz
+
+
+def jitter(seed: int, voxel_linear: int, axis: int) -> float:
+    return float(lib().wo_jitter(C.c_uint64(int(seed)), C.c_uint64(int(voxel_linear)), C.c_int(axis)))
 
 
 def forward(g, xyz, tau: float = 0.01, mode: int = 1, hit_mask_in=None, covered_in=None, want_mask: bool = False,

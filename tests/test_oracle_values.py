@@ -233,3 +233,35 @@ def test_mse_epilogue(oracle):
                     for c in range(0, 1000, 97)])
     np.testing.assert_allclose(d[::97], np.where(cov[::97], num, 0.0), rtol=1e-6, atol=1e-12)
     np.testing.assert_allclose(e, np.abs(phi - t), rtol=1e-15)
+
+
+def test_jittered_grid_positions(oracle):
+    """In-cell jitter: every sample stays inside its voxel's cell, the generator is the splitmix64
+    finaliser written out here with Python integers, positions are uniform in the cell and independent per axis."""
+    from paper_2607_01164_b200 import inputs
+    M = (1 << 64) - 1
+
+    def mix(z):
+        z = (z + 0x9E3779B97F4A7C15) & M
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & M
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & M
+        return z ^ (z >> 31)
+
+    for seed, L, a in ((0, 0, 0), (7, 123456789, 2), (2 ** 63 + 5, 2 ** 40 + 3, 1)):
+        want = (mix((seed + 3 * L + a) & M) >> 40) / 2.0 ** 24 - 0.5
+        assert oracle.jitter(seed, L, a) == want and -0.5 <= want < 0.5
+    grid = inputs.Grid((20, 13, 9), (-0.3, 0.1, 0.0), (0.05, 0.04, 0.1))
+    sub = grid.batch((1, 0, 0), (1, 2, 1))
+    centres = oracle.grid_points(sub).astype(np.float64)
+    a = oracle.grid_points(sub, jitter_seed=11).astype(np.float64)
+    b = oracle.grid_points(sub, jitter_seed=12).astype(np.float64)
+    assert np.array_equal(a, oracle.grid_points(sub, jitter_seed=11).astype(np.float64)) and not np.array_equal(a, b)
+    frac = (a - centres) / np.asarray(grid.spacing)
+    assert np.all(np.abs(frac) <= 0.5 + 1e-5)
+    # the batch's samples are those of the whole grid (the counter is the GLOBAL voxel index)
+    full = oracle.grid_points(grid, jitter_seed=11).reshape(9, 13, 20, 3)
+    assert np.array_equal(a.reshape(8, 13, 8, 3), full[0:8, 0:13, 8:16].astype(np.float64))
+    big = inputs.Grid((64, 64, 32), (0, 0, 0), (1, 1, 1))
+    f = oracle.grid_points(big, jitter_seed=3).astype(np.float64) - oracle.grid_points(big).astype(np.float64)
+    assert abs(f.mean()) < 2e-3 and abs(f.var() - 1 / 12) < 2e-3             # uniform on [-0.5, 0.5)
+    assert np.all(np.abs(np.corrcoef(f.T) - np.eye(3)) < 0.01)               # axes independent
