@@ -82,6 +82,10 @@ typedef enum { GS_QUERY_GRID = 0, GS_QUERY_POINTS = 1 } gs_query_kind;
  *   of brick_cnt bricks starting at brick brick_lo, a brick being 8^3 voxels; voxels beyond dims are
  *   clipped.  Per-sample arrays are indexed x-fastest over the batch's clipped voxel box
  *   (bx = min(8*brick_cnt_x, dims_x - 8*brick_lo_x), ...), P = bx*by*bz.
+ *   jitter != 0 ("a random position in each cell every iteration"): the sample of voxel i
+ *   sits at p_k = fmaf(((float)i_k + 0.5f) + j_k, spacing_k, origin_k), j_k in [-0.5, 0.5) drawn by a
+ *   counter-based generator from (jitter_seed, global voxel index, axis) (DESIGN D26): the same seed
+ *   gives the same samples in every batch and on every call; pass a new seed per training iteration.
  * GS_QUERY_POINTS (section 5.1): num_points arbitrary positions xyz[P,3]; per-sample arrays follow the
  *   caller's order.  presorted != 0 promises that xyz is already spatially coherent (skips the
  *   Morton sort of the queries; results are identical either way). */
@@ -95,6 +99,8 @@ typedef struct {
     uint64_t num_points;
     const float *xyz; /* [P,3] */
     int32_t presorted;
+    int32_t jitter;       /* GS_QUERY_GRID: 0 = voxel centres */
+    uint64_t jitter_seed; /* GS_QUERY_GRID with jitter */
 } gs_query;
 
 /* Gradient outputs, OVERWRITTEN (not accumulated): dL/dmean[N,3], dL/dscale[N,3], dL/dquat[N,4],

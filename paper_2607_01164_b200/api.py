@@ -51,7 +51,7 @@ class _Domain(C.Structure):
 class _Query(C.Structure):
     _fields_ = [("kind", C.c_int32), ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float * 3),
                 ("brick_lo", C.c_int32 * 3), ("brick_cnt", C.c_int32 * 3), ("num_points", C.c_uint64), ("xyz", C.c_void_p),
-                ("presorted", C.c_int32)]
+                ("presorted", C.c_int32), ("jitter", C.c_int32), ("jitter_seed", C.c_uint64)]
 
 
 class _Grads(C.Structure):
@@ -134,10 +134,14 @@ def _ptr(t):
     return C.c_void_p(t.data_ptr())
 
 
-def grid_query(grid) -> _Query:
-    """``grid``: object with dims, origin, spacing, brick_lo, brick_cnt (e.g. inputs.Grid)."""
+def grid_query(grid, jitter_seed=None) -> _Query:
+    """``grid``: object with dims, origin, spacing, brick_lo, brick_cnt (e.g. inputs.Grid).  jitter_seed: one random
+    sample position inside every voxel's cell instead of its centre (gs.h)."""
     q = _Query()
     q.kind = GS_QUERY_GRID
+    if jitter_seed is not None:
+        q.jitter = 1
+        q.jitter_seed = int(jitter_seed)
     for k in range(3):
         q.dims[k] = int(grid.dims[k])
         q.origin[k] = float(grid.origin[k])

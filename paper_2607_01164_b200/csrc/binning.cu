@@ -151,8 +151,9 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
 #pragma unroll
         for (int k = 0; k < 3; k++) {
             const float inv_sp = 1.0f / gd.spacing[k];
-            const float tl = (b6[k] - gd.origin[k]) * inv_sp - 0.5f;
-            const float th = (b6[3 + k] - gd.origin[k]) * inv_sp - 0.5f;
+            // voxel i is sampled at its centre i + 0.5, or with jitter anywhere in [i, i + 1) (in units of the spacing)
+            const float tl = (b6[k] - gd.origin[k]) * inv_sp - (gd.jitter ? 1.0f : 0.5f);
+            const float th = (b6[3 + k] - gd.origin[k]) * inv_sp - (gd.jitter ? 0.0f : 0.5f);
             const int first = BRICK * gd.brick_lo[k], last = BRICK * gd.brick_lo[k] + gd.bdim[k] - 1;
             const float fl = fmaxf(ceilf(tl - (1e-3f + 4e-7f * fabsf(tl))), (float)first);
             const float fh = fminf(floorf(th + (1e-3f + 4e-7f * fabsf(th))), (float)last);
@@ -165,7 +166,8 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         }
         // cull bound: |M(p - mu)| >= |M(cc - mu)| - rho for every voxel p of a cell with centre cc
         const float4 gb = rec[(size_t)N + i], gc = rec[2 * (size_t)N + i], gd4 = rec[3 * (size_t)N + i];
-        const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
+        const float hh = gd.jitter ? 1.0f : 0.5f;  // half extent of a cell's samples around the cell centre, in voxels
+        const float hx = hh * gd.spacing[0], hy = hh * gd.spacing[1], hz = hh * gd.spacing[2];
         const float q0 = fabsf(gb.x) * hx + fabsf(gb.y) * hy + fabsf(gb.z) * hz;
         const float q1 = fabsf(gc.x) * hx + fabsf(gc.y) * hy + fabsf(gc.z) * hz;
         const float q2 = fabsf(gd4.x) * hx + fabsf(gd4.y) * hy + fabsf(gd4.z) * hz;

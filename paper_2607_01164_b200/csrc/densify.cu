@@ -86,9 +86,17 @@ __global__ void __launch_bounds__(256) k_new_gaussians(ParamSet d, uint32_t n_ol
     } else {  // batch-local sample index, x fastest (D6)
         const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
         const uint32_t x = c % bdx, y = (c / bdx) % bdy, z = c / (bdx * bdy);
-        px = voxel_centre((int)x + BRICK * gd.brick_lo[0], gd.spacing[0], gd.origin[0]);
-        py = voxel_centre((int)y + BRICK * gd.brick_lo[1], gd.spacing[1], gd.origin[1]);
-        pz = voxel_centre((int)z + BRICK * gd.brick_lo[2], gd.spacing[2], gd.origin[2]);
+        const int gx = (int)x + BRICK * gd.brick_lo[0], gy = (int)y + BRICK * gd.brick_lo[1], gz = (int)z + BRICK * gd.brick_lo[2];
+        if (gd.jitter) {  // the sample the error was measured at (D26)
+            const unsigned long long L = voxel_linear(gx, gy, gz, gd.dims[0], gd.dims[1]);
+            px = voxel_sample(gx, voxel_jitter(gd.jitter_seed, L, 0), gd.spacing[0], gd.origin[0]);
+            py = voxel_sample(gy, voxel_jitter(gd.jitter_seed, L, 1), gd.spacing[1], gd.origin[1]);
+            pz = voxel_sample(gz, voxel_jitter(gd.jitter_seed, L, 2), gd.spacing[2], gd.origin[2]);
+        } else {
+            px = voxel_centre(gx, gd.spacing[0], gd.origin[0]);
+            py = voxel_centre(gy, gd.spacing[1], gd.origin[1]);
+            pz = voxel_centre(gz, gd.spacing[2], gd.origin[2]);
+        }
     }
     const size_t g = (size_t)n_old + j, nn = n_new;
     d.mean[3 * g] = px; d.mean[3 * g + 1] = py; d.mean[3 * g + 2] = pz;

@@ -59,7 +59,7 @@ bool same_query(const gs_query &a, const gs_query &b) {
             if (a.dims[k] != b.dims[k] || a.origin[k] != b.origin[k] || a.spacing[k] != b.spacing[k] ||
                 a.brick_lo[k] != b.brick_lo[k] || a.brick_cnt[k] != b.brick_cnt[k])
                 return false;
-        return true;
+        return (a.jitter != 0) == (b.jitter != 0) && (!a.jitter || a.jitter_seed == b.jitter_seed);
     }
     return a.num_points == b.num_points && a.xyz == b.xyz && a.presorted == b.presorted;
 }
@@ -90,6 +90,8 @@ gs_status validate_query(gs_ctx *ctx, const gs_query *q, GridDesc *gd, uint64_t 
         for (int k = 0; k < 3; k++)  // the kernels index samples with 32 bits and cells with 10 bits per axis
             if (gd->bdim[k] > 2048) return fail(ctx, GS_ERR_INVALID_ARG, "grid: a batch may span at most 2048 voxels per axis");
         if (p >= (1ull << 32)) return fail(ctx, GS_ERR_INVALID_ARG, "grid: a batch may hold at most 2^32-1 samples");
+        gd->jitter = q->jitter != 0;
+        gd->jitter_seed = q->jitter ? q->jitter_seed : 0ull;
         *P = p;
         return GS_OK;
     }

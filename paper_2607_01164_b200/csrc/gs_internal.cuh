@@ -42,6 +42,8 @@ struct GridDesc {          // one batch of a structured grid (gs_query, GS_QUERY
     int bdim[3];           // clipped voxel extent of the batch
     float inv_brick[3];    // 1.0f / (8.0f * spacing)  (D7)
     int nb_total[3];       // bricks of the whole grid per axis
+    int jitter;            // samples at a random position of their cell (D26) instead of its centre
+    unsigned long long jitter_seed;
 };
 
 // 30-bit Morton code of a position inside the domain box (D8): 10 bits per axis, x in the low bit,

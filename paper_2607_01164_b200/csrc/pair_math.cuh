@@ -36,6 +36,27 @@ __device__ __forceinline__ float voxel_centre(int i, float spacing, float origin
     return __fmaf_rn(__fadd_rn((float)i, 0.5f), spacing, origin);
 }
 
+// In-cell jitter of grid samples (DESIGN D26): counter-based, so every kernel (and the oracle) draws the same
+// numbers.  For the voxel with GLOBAL linear index L and axis a: h = splitmix64 finaliser of (seed + 3 L + a),
+// j = (h >> 40) * 2^-24 - 0.5 in [-0.5, 0.5); the sample sits at fmaf(((float)i + 0.5f) + j, spacing, origin).
+__device__ __forceinline__ unsigned long long mix64_u64(unsigned long long z) {
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ float voxel_jitter(unsigned long long seed, unsigned long long L, int axis) {
+    const unsigned long long h = mix64_u64(seed + 3ull * L + (unsigned long long)axis);
+    return __fsub_rn(__fmul_rn((float)(uint32_t)(h >> 40), 5.9604644775390625e-8f), 0.5f);
+}
+__device__ __forceinline__ float voxel_sample(int i, float j, float spacing, float origin) {
+    return __fmaf_rn(__fadd_rn(__fadd_rn((float)i, 0.5f), j), spacing, origin);
+}
+// global linear voxel index of the jitter counter
+__device__ __forceinline__ unsigned long long voxel_linear(int gx, int gy, int gz, int dimx, int dimy) {
+    return ((unsigned long long)gz * (unsigned long long)dimy + (unsigned long long)gy) * (unsigned long long)dimx + (unsigned long long)gx;
+}
+
 // id hash for order-free set comparison (splitmix64 finaliser of id + golden gamma)
 __device__ __forceinline__ unsigned long long mix64(uint32_t id) {
     unsigned long long z = (unsigned long long)id + 0x9E3779B97F4A7C15ull;

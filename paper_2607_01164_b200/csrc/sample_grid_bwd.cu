@@ -76,7 +76,7 @@ __device__ __forceinline__ void warp_reduce32(float (&v)[32], int lane) {
     }
 }
 
-template <bool PACK2>
+template <bool PACK2, bool JIT>
 __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
                                                               GridDesc gd, const void *__restrict__ pack_, float r2,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
@@ -163,6 +163,32 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                     al[v] = s.x; be[v] = s.y; ep[v] = s.z;
                 }
             }
+        }
+        if (JIT) {
+            // jittered samples (D26): no two voxels of the cell share a coordinate and u is not affine in the
+            // voxel index, so every voxel is its own "cell" of the moment sums: m000 = g, u0 = u(voxel), no index moments
+#pragma unroll
+            for (int v = 0; v < 8; v++) {
+                const int gx = X + (v & 1), gy = Y + ((v >> 1) & 1), gz = Z + (v >> 2);
+                const unsigned long long L = voxel_linear(gx, gy, gz, gd.dims[0], gd.dims[1]);
+                const float dxv = __fsub_rn(voxel_sample(gx, voxel_jitter(gd.jitter_seed, L, 0), gd.spacing[0], gd.origin[0]), ga.x);
+                const float dyv = __fsub_rn(voxel_sample(gy, voxel_jitter(gd.jitter_seed, L, 1), gd.spacing[1], gd.origin[1]), ga.y);
+                const float dzv = __fsub_rn(voxel_sample(gz, voxel_jitter(gd.jitter_seed, L, 2), gd.spacing[2], gd.origin[2]), ga.z);
+                const float u0 = __fmaf_rn(gb.z, dzv, __fmaf_rn(gb.y, dyv, __fmul_rn(gb.x, dxv)));
+                const float u1 = __fmaf_rn(gc.z, dzv, __fmaf_rn(gc.y, dyv, __fmul_rn(gc.x, dxv)));
+                const float u2 = __fmaf_rn(gd4.z, dzv, __fmaf_rn(gd4.y, dyv, __fmul_rn(gd4.x, dxv)));
+                const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
+                const float G = qd <= r2 ? gauss_weight(qd) : 0.f;
+                const float gg = fmaf(al[v], gb.w, be[v]) * G;
+                acc[0] = fmaf(al[v], G, acc[0]);
+                acc[2] = fmaf(PACK2 ? fabsf(al[v]) : ep[v], G, acc[2]);
+                acc[1] += gg;
+                const float t0 = gg * u0, t1 = gg * u1, t2 = gg * u2;
+                acc[3] += t0; acc[4] += t1; acc[5] += t2;
+                acc[9] = fmaf(t0, u0, acc[9]); acc[10] = fmaf(t0, u1, acc[10]); acc[11] = fmaf(t0, u2, acc[11]);
+                acc[12] = fmaf(t1, u1, acc[12]); acc[13] = fmaf(t1, u2, acc[13]); acc[14] = fmaf(t2, u2, acc[14]);
+            }
+            return;
         }
         float dx[2], dy[2], dz[2];
 #pragma unroll
@@ -298,8 +324,13 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
     // only the M Gaussians of the order list get (and need) an accumulator row: k_finalize reads those alone
     if (M == 0) return cudaSuccess;
     const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
-    if (pack2) k_grid_bwd<true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
-    else k_grid_bwd<false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+    if (gd.jitter) {
+        if (pack2) k_grid_bwd<true, true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+        else k_grid_bwd<false, true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+    } else {
+        if (pack2) k_grid_bwd<true, false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+        else k_grid_bwd<false, false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M);
+    }
     count_launch();
     return cudaGetLastError();
 }

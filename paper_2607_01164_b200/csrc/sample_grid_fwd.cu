@@ -28,7 +28,7 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
 
-template <bool SETS>
+template <bool SETS, bool JIT>
 __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const float4 *__restrict__ rec, uint32_t N, GridDesc gd,
                                                            const uint32_t *__restrict__ pair_gauss,
                                                            const uint32_t *__restrict__ brick_start, float tau, float r2, FwdOut o,
@@ -51,11 +51,27 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
         py[d] = (ly + d < gd.bdim[1]) ? voxel_centre(ly + d + BRICK * gd.brick_lo[1], gd.spacing[1], gd.origin[1]) : nanv;
         pz[d] = (lz + d < gd.bdim[2]) ? voxel_centre(lz + d + BRICK * gd.brick_lo[2], gd.spacing[2], gd.origin[2]) : nanv;
     }
+    // JIT: every voxel has its own position inside its cell (D26); v = x | y << 1 | z << 2
+    float jp[JIT ? 8 : 1][3];
+    if (JIT) {
+#pragma unroll
+        for (int v = 0; v < 8; v++) {
+            const int x = lx + (v & 1), y = ly + ((v >> 1) & 1), z = lz + (v >> 2);
+            const bool in = x < gd.bdim[0] && y < gd.bdim[1] && z < gd.bdim[2];
+            const int gx = x + BRICK * gd.brick_lo[0], gy = y + BRICK * gd.brick_lo[1], gz = z + BRICK * gd.brick_lo[2];
+            const unsigned long long L = voxel_linear(gx, gy, gz, gd.dims[0], gd.dims[1]);
+            jp[v][0] = in ? voxel_sample(gx, voxel_jitter(gd.jitter_seed, L, 0), gd.spacing[0], gd.origin[0]) : nanv;
+            jp[v][1] = in ? voxel_sample(gy, voxel_jitter(gd.jitter_seed, L, 1), gd.spacing[1], gd.origin[1]) : nanv;
+            jp[v][2] = in ? voxel_sample(gz, voxel_jitter(gd.jitter_seed, L, 2), gd.spacing[2], gd.origin[2]) : nanv;
+        }
+    }
     // cull geometry (not canonical): centre of the warp's cell (0,0,0), cell pitch = 2 voxels, half extent = half a voxel
     const float c0x = fmaf((float)(BRICK * (bx + gd.brick_lo[0]) + 1), gd.spacing[0], gd.origin[0]);
     const float c0y = fmaf((float)(BRICK * (by + gd.brick_lo[1]) + 1), gd.spacing[1], gd.origin[1]);
     const float c0z = fmaf((float)(BRICK * (bz + gd.brick_lo[2]) + 4 * warp + 1), gd.spacing[2], gd.origin[2]);
-    const float hx = 0.5f * gd.spacing[0], hy = 0.5f * gd.spacing[1], hz = 0.5f * gd.spacing[2];
+    // half extent of a cell's samples around the cell centre: half a voxel, a whole one when they are jittered
+    const float hh = JIT ? 1.0f : 0.5f;
+    const float hx = hh * gd.spacing[0], hy = hh * gd.spacing[1], hz = hh * gd.spacing[2];
     const float rcut = sqrtf(r2);
 
     float I[8], Nacc[8];
@@ -140,7 +156,18 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
             const float4 ga = srec[0][j], gb = srec[1][j], gc = srec[2][j], gd4 = srec[3][j];
             // canonical sequence (D4), shared between voxels: d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx));
             // qd = fma(u2, u2, fma(u1, u1, u0 * u0))
-            float dx[2], dy[2], dz[2], qd[8];
+            float qd[8];
+            if (JIT) {  // no two voxels share a coordinate: the plain canonical sequence per voxel
+#pragma unroll
+                for (int v = 0; v < 8; v++) {
+                    const float dx = __fsub_rn(jp[v][0], ga.x), dy = __fsub_rn(jp[v][1], ga.y), dz = __fsub_rn(jp[v][2], ga.z);
+                    const float u0 = __fmaf_rn(gb.z, dz, __fmaf_rn(gb.y, dy, __fmul_rn(gb.x, dx)));
+                    const float u1 = __fmaf_rn(gc.z, dz, __fmaf_rn(gc.y, dy, __fmul_rn(gc.x, dx)));
+                    const float u2 = __fmaf_rn(gd4.z, dz, __fmaf_rn(gd4.y, dy, __fmul_rn(gd4.x, dx)));
+                    qd[v] = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
+                }
+            } else {
+            float dx[2], dy[2], dz[2];
 #pragma unroll
             for (int d = 0; d < 2; d++) {
                 dx[d] = __fsub_rn(px[d], ga.x);
@@ -162,6 +189,7 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
                     const float u = __fmaf_rn(mr.z, dz[v >> 2], ab[v & 3]);
                     qd[v] = row == 0 ? __fmul_rn(u, u) : __fmaf_rn(u, u, qd[v]);
                 }
+            }
             }
             if (SETS) ntest += 8;
 #pragma unroll
@@ -266,8 +294,13 @@ cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, c
     if (nbricks == 0) return cudaSuccess;
     const double P = (double)gd.bdim[0] * gd.bdim[1] * gd.bdim[2];
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
-    if (sets) k_grid_fwd<true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
-    else k_grid_fwd<false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+    if (gd.jitter) {
+        if (sets) k_grid_fwd<true, true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+        else k_grid_fwd<false, true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+    } else {
+        if (sets) k_grid_fwd<true, false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+        else k_grid_fwd<false, false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P);
+    }
     count_launch();
     return cudaGetLastError();
 }

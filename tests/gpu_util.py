@@ -14,7 +14,8 @@ def to_dev(torch, *arrays):
 class GpuRun:
     """One preprocess -> build -> fwd (fused MSE) -> bwd pass on the GPU; results as numpy arrays."""
 
-    def __init__(self, g, query_kind, query_obj, target, domain=None, dL_dI=None, presorted=False, tau=TAU, fused=False):
+    def __init__(self, g, query_kind, query_obj, target, domain=None, dL_dI=None, presorted=False, tau=TAU, fused=False,
+                 jitter_seed=None):
         """fused=True: gs_sample_bwd(dL_dphi=NULL), i.e. the backward of the forward's fused MSE loss."""
         import torch
         from paper_2607_01164_b200 import api
@@ -25,7 +26,7 @@ class GpuRun:
         self.dev = to_dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
         ctx.gs_preprocess(*self.dev, domain=domain, tau=tau)
         if query_kind == "grid":
-            self.q = api.grid_query(query_obj)
+            self.q = api.grid_query(query_obj, jitter_seed=jitter_seed)
         else:
             self.xyz = to_dev(torch, query_obj)[0]
             self.q = api.points_query(self.xyz, presorted=presorted)

@@ -35,7 +35,7 @@ def test_struct_layouts_match_header():
     from paper_2607_01164_b200 import api
     assert ctypes.sizeof(api._Gaussians) == 48
     assert ctypes.sizeof(api._Domain) == 24
-    assert api._Query.num_points.offset == 64 and api._Query.xyz.offset == 72 and ctypes.sizeof(api._Query) == 88
+    assert api._Query.num_points.offset == 64 and api._Query.xyz.offset == 72 and api._Query.jitter.offset == 84 and ctypes.sizeof(api._Query) == 96
     assert ctypes.sizeof(api._Grads) == 48
     assert ctypes.sizeof(api._RawParams) == 48 and api._RawParams.mean.offset == 8
     assert ctypes.sizeof(api._AdamCfg) == 36 and api._AdamCfg.step.offset == 32

@@ -236,3 +236,32 @@ def test_structured_path_is_deterministic(oracle):
         assert np.array_equal(ga[k], gb[k]), k
     pa = a.ctx.debug_get(a.api.DBG_PAIR_GAUSS, np.uint32)
     assert np.array_equal(pa, b.ctx.debug_get(b.api.DBG_PAIR_GAUSS, np.uint32))
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_jittered_grid(oracle, fused):
+    """In-cell jitter (D26): one random sample position per voxel instead of its centre, drawn by the same
+    counter-based generator on both sides.  ID sets bit-exact, forward / gradients to the usual tolerances, on C1 and on
+    a ragged sub-box batch with elongated Gaussians."""
+    rng = np.random.default_rng(21)
+    cases = [(inputs.c1_gaussians(seed=0, n=1024), inputs.c1_grid(32), 5)]
+    gridfull = inputs.Grid((44, 29, 21), (-0.1, 0.2, 0.0), (1 / 40, 1 / 32, 1 / 20))
+    cases.append((inputs.c4_gaussians(seed=7, n_grid=40, n=3000), gridfull.batch((1, 1, 0), (3, 3, 3)), 2 ** 40 + 17))
+    for g, grid, seed in cases:
+        xyz = oracle.grid_points(grid, jitter_seed=seed)
+        assert not np.array_equal(xyz, oracle.grid_points(grid))
+        P = grid.num_points
+        target = rng.uniform(0, 1, P).astype(np.float32)
+        dI = None if fused else (rng.standard_normal(P) * 1e-3)
+        fwd = oracle.forward(g, xyz, TAU, mode=1)
+        loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+        gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, dI, target, TAU, mode=1)
+        run = GpuRun(g, "grid", grid, target, dL_dI=None if dI is None else dI.astype(np.float32), fused=fused, jitter_seed=seed)
+        _check_integer_stages(oracle, run, g, grid)   # the brick lists do not depend on the jitter
+        check_sets(run, fwd)
+        check_forward(run, fwd)
+        assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+        check_grads(run, gr)
+        # another seed gives other samples
+        run2 = GpuRun(g, "grid", grid, target, fused=True, jitter_seed=seed + 1)
+        assert not np.array_equal(run2.np(run2.phi), run.np(run.phi))
