@@ -84,7 +84,7 @@ typedef enum { GS_QUERY_GRID = 0, GS_QUERY_POINTS = 1 } gs_query_kind;
  *   (bx = min(8*brick_cnt_x, dims_x - 8*brick_lo_x), ...), P = bx*by*bz.
  *   jitter != 0 ("a random position in each cell every iteration"): the sample of voxel i
  *   sits at p_k = fmaf(((float)i_k + 0.5f) + j_k, spacing_k, origin_k), j_k in [-0.5, 0.5) drawn by a
- *   counter-based generator from (jitter_seed, global voxel index, axis) (DESIGN D26): the same seed
+ *   counter-based generator from (jitter_seed, global voxel index), 21 bits per axis (DESIGN D26): the same seed
  *   gives the same samples in every batch and on every call; pass a new seed per training iteration.
  * GS_QUERY_POINTS (section 5.1): num_points arbitrary positions xyz[P,3]; per-sample arrays follow the
  *   caller's order.  presorted != 0 promises that xyz is already spatially coherent (skips the

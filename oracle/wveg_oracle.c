@@ -189,10 +189,11 @@ void wo_grid_points(const wo_grid *gr, float *xyz /*[P,3]*/) {
 
 /* In-cell jitter of the grid samples ("we select a random position in each cell every iteration of     */
 /* training").  The random numbers come from a counter-based generator so that both sides can draw the same ones      */
-/* (DESIGN D26): for the voxel with global index L = (gz * dims_y + gy) * dims_x + gx and axis a,                      */
-/*   h = splitmix64-finaliser(seed + 3 L + a + golden gamma),  j = (h >> 40) * 2^-24 - 0.5  in [-0.5, 0.5)             */
-/* and the sample position is p_a = fmaf(((float)i_a + 0.5f) + j, spacing_a, origin_a) (every step exact or one        */
-/* fp32 rounding; that fp32 value IS the position, as for voxel centres, D6).                                           */
+/* (DESIGN D26): the voxel with global index L = (gz * dims_y + gy) * dims_x + gx draws ONE 64-bit number              */
+/*   h = splitmix64-finaliser(seed + L + golden gamma)                                                                 */
+/* and axis a takes 21 of its bits:  j_a = ((h >> 21 a) & (2^21 - 1)) * 2^-21 - 0.5  in [-0.5, 0.5).                   */
+/* The sample position is p_a = fmaf(((float)i_a + 0.5f) + j_a, spacing_a, origin_a) (every step exact or one fp32     */
+/* rounding; that fp32 value IS the position, as for voxel centres, D6).                                               */
 static inline uint64_t mix64_u64(uint64_t z) {
     z += 0x9E3779B97F4A7C15ull;
     z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
@@ -200,8 +201,8 @@ static inline uint64_t mix64_u64(uint64_t z) {
     return z ^ (z >> 31);
 }
 float wo_jitter(uint64_t seed, uint64_t voxel_linear, int axis) {
-    const uint64_t h = mix64_u64(seed + 3ull * voxel_linear + (uint64_t)axis);
-    return (float)(h >> 40) * 5.9604644775390625e-8f - 0.5f;
+    const uint64_t h = mix64_u64(seed + voxel_linear);
+    return (float)((h >> (21 * axis)) & 0x1FFFFFull) * 4.76837158203125e-7f - 0.5f;
 }
 void wo_grid_points_jitter(const wo_grid *gr, uint64_t seed, float *xyz /*[P,3]*/) {
     int32_t bd[3]; grid_batch_dims(gr, bd);

@@ -13,6 +13,7 @@
 // pair, two 8-bit LSD passes, run boundaries) took 0.25 ms of device time; this one is listed in DESIGN.md.
 // Brick ranges are integer decisions: fixed fp32 sequence (D7).
 #include "gs_internal.cuh"
+#include "pair_math.cuh"
 
 namespace gs {
 
@@ -360,6 +361,22 @@ cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t 
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_bucket_sort<<<(nbricks + BS_WARPS - 1) / BS_WARPS, BS_WARPS * 32, 0, s>>>(total, cap, start, nbricks, pair_gauss); count_launch();
+    return cudaGetLastError();
+}
+
+// random bits of every voxel of a jittered batch (D26): one hash per voxel, read by the forward, the
+// backward and the densification of this step
+__global__ void __launch_bounds__(256) k_jitter_table(GridDesc gd, uint2 *__restrict__ jit) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
+    if (x >= (uint32_t)gd.bdim[0]) return;
+    const unsigned long long L = voxel_linear((int)x + BRICK * gd.brick_lo[0], (int)y + BRICK * gd.brick_lo[1],
+                                              (int)z + BRICK * gd.brick_lo[2], gd.dims[0], gd.dims[1]);
+    jit[((size_t)z * gd.bdim[1] + y) * gd.bdim[0] + x] = voxel_hash(gd.jitter_seed, L);
+}
+
+cudaError_t launch_jitter_table(const GridDesc &gd, uint2 *jit, cudaStream_t s) {
+    const dim3 grid((unsigned)((gd.bdim[0] + 255) / 256), (unsigned)gd.bdim[1], (unsigned)gd.bdim[2]);
+    k_jitter_table<<<grid, 256, 0, s>>>(gd, jit); count_launch();
     return cudaGetLastError();
 }
 

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) k_select_keys(const float *__restrict__ e
 
 // Gaussian n_old + j from the j-th selected sample
 __global__ void __launch_bounds__(256) k_new_gaussians(ParamSet d, uint32_t n_old, uint32_t n_new, const uint32_t *__restrict__ sel,
-                                                        GridDesc gd, const float *__restrict__ xyz /*NULL: grid*/,
+                                                        GridDesc gd, const uint2 *__restrict__ jit, const float *__restrict__ xyz /*NULL: grid*/,
                                                         const float *__restrict__ target, float raw_scale_init, float raw_opacity_init,
                                                         float clamp) {
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -88,10 +88,11 @@ __global__ void __launch_bounds__(256) k_new_gaussians(ParamSet d, uint32_t n_ol
         const uint32_t x = c % bdx, y = (c / bdx) % bdy, z = c / (bdx * bdy);
         const int gx = (int)x + BRICK * gd.brick_lo[0], gy = (int)y + BRICK * gd.brick_lo[1], gz = (int)z + BRICK * gd.brick_lo[2];
         if (gd.jitter) {  // the sample the error was measured at (D26)
-            const unsigned long long L = voxel_linear(gx, gy, gz, gd.dims[0], gd.dims[1]);
-            px = voxel_sample(gx, voxel_jitter(gd.jitter_seed, L, 0), gd.spacing[0], gd.origin[0]);
-            py = voxel_sample(gy, voxel_jitter(gd.jitter_seed, L, 1), gd.spacing[1], gd.origin[1]);
-            pz = voxel_sample(gz, voxel_jitter(gd.jitter_seed, L, 2), gd.spacing[2], gd.origin[2]);
+            float jx, jy, jz;
+            voxel_jitter3(jit[c], jx, jy, jz);
+            px = voxel_sample(gx, jx, gd.spacing[0], gd.origin[0]);
+            py = voxel_sample(gy, jy, gd.spacing[1], gd.origin[1]);
+            pz = voxel_sample(gz, jz, gd.spacing[2], gd.origin[2]);
         } else {
             px = voxel_centre(gx, gd.spacing[0], gd.origin[0]);
             py = voxel_centre(gy, gd.spacing[1], gd.origin[1]);
@@ -164,13 +165,13 @@ cudaError_t launch_select_keys(const float *err, const float *I, const uint8_t *
 }
 
 cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *sel, const GridDesc &gd,
-                                 const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
+                                 const uint2 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
                                  float *scratch, cudaStream_t s) {
     const ParamSet o{p.mean, p.raw_scale, p.quat, p.raw_opacity, p.raw_scalar, m, v};
     const ParamSet d = carve(scratch, n_new);
     const uint32_t add = n_new - p.n;
     if (add) {
-        k_new_gaussians<<<(add + 255) / 256, 256, 0, s>>>(d, p.n, n_new, sel, gd, xyz, target, raw_scale_init, raw_opacity_init, clamp);
+        k_new_gaussians<<<(add + 255) / 256, 256, 0, s>>>(d, p.n, n_new, sel, gd, jit, xyz, target, raw_scale_init, raw_opacity_init, clamp);
         count_launch();
     }
     cudaError_t e = cudaGetLastError();

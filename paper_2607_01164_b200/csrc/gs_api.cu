@@ -139,7 +139,7 @@ void gs_destroy(gs_ctx *ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->bhist, &ctx->pair_gauss, &ctx->pair_brick,
-                     &ctx->grid_order, &ctx->brick_start, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
+                     &ctx->grid_order, &ctx->brick_start, &ctx->jit, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
@@ -240,6 +240,10 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         const uint32_t T = (uint32_t)T64[0];
         ctx->M = (uint32_t)T64[1];
         ctx->have_pair_brick = false;
+        if (gd.jitter && P > 0) {
+            CK(ctx->jit.reserve(P * sizeof(uint2)), "alloc jitter table");
+            CK(launch_jitter_table(gd, ctx->jit.as<uint2>(), s), "jitter table");
+        }
         ctx->T = T;
         ctx->nbricks = nbricks;
         ctx->grid = gd;
@@ -334,7 +338,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
     if (ctx->accel_kind == GS_QUERY_GRID) {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_gauss.as<uint32_t>(),
-                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, s), "grid forward");
+                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<uint2>(), s), "grid forward");
     } else {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
@@ -430,7 +434,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         }
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, ctx->r2,
-                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, s), "grid backward");
+                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<uint2>(), s), "grid backward");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
@@ -605,7 +609,7 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
     float *scratch = ctx->dens_scratch.as<float>();
     CK(launch_regather(*p, m, v, n_new, nullptr, n, scratch, false, s), "densify gather");
     const float *xyz = ctx->accel_kind == GS_QUERY_POINTS ? ctx->accel_q.xyz : nullptr;
-    CK(launch_new_gaussians(*p, m, v, n_new, vals[sel], ctx->grid, xyz, target, raw_scale_init, raw_opacity_init, 1e-4f, scratch, s),
+    CK(launch_new_gaussians(*p, m, v, n_new, vals[sel], ctx->grid, ctx->jit.as<uint2>(), xyz, target, raw_scale_init, raw_opacity_init, 1e-4f, scratch, s),
        "new gaussians");
     CK(cudaStreamSynchronize(s), "sync");
     return GS_OK;

@@ -37,17 +37,24 @@ __device__ __forceinline__ float voxel_centre(int i, float spacing, float origin
 }
 
 // In-cell jitter of grid samples (DESIGN D26): counter-based, so every kernel (and the oracle) draws the same
-// numbers.  For the voxel with GLOBAL linear index L and axis a: h = splitmix64 finaliser of (seed + 3 L + a),
-// j = (h >> 40) * 2^-24 - 0.5 in [-0.5, 0.5); the sample sits at fmaf(((float)i + 0.5f) + j, spacing, origin).
+// numbers.  The voxel with GLOBAL linear index L draws one 64-bit number h = splitmix64 finaliser of (seed + L); axis a
+// takes 21 of its bits, j_a = ((h >> 21 a) & (2^21 - 1)) * 2^-21 - 0.5 in [-0.5, 0.5); the sample sits at
+// fmaf(((float)i + 0.5f) + j, spacing, origin).  k_jitter_table writes h once per step (uint2 per voxel of the batch).
 __device__ __forceinline__ unsigned long long mix64_u64(unsigned long long z) {
     z += 0x9E3779B97F4A7C15ull;
     z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
     z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
     return z ^ (z >> 31);
 }
-__device__ __forceinline__ float voxel_jitter(unsigned long long seed, unsigned long long L, int axis) {
-    const unsigned long long h = mix64_u64(seed + 3ull * L + (unsigned long long)axis);
-    return __fsub_rn(__fmul_rn((float)(uint32_t)(h >> 40), 5.9604644775390625e-8f), 0.5f);
+__device__ __forceinline__ uint2 voxel_hash(unsigned long long seed, unsigned long long L) {
+    const unsigned long long h = mix64_u64(seed + L);
+    return make_uint2((uint32_t)h, (uint32_t)(h >> 32));
+}
+__device__ __forceinline__ float jitter_from_bits(uint32_t b21) { return __fmaf_rn((float)b21, 4.76837158203125e-7f, -0.5f); }  // exact
+__device__ __forceinline__ void voxel_jitter3(uint2 h, float &jx, float &jy, float &jz) {
+    jx = jitter_from_bits(h.x & 0x1FFFFFu);
+    jy = jitter_from_bits(((h.x >> 21) | (h.y << 11)) & 0x1FFFFFu);
+    jz = jitter_from_bits((h.y >> 10) & 0x1FFFFFu);
 }
 __device__ __forceinline__ float voxel_sample(int i, float j, float spacing, float origin) {
     return __fmaf_rn(__fadd_rn(__fadd_rn((float)i, 0.5f), j), spacing, origin);

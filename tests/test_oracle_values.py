@@ -248,7 +248,7 @@ def test_jittered_grid_positions(oracle):
         return z ^ (z >> 31)
 
     for seed, L, a in ((0, 0, 0), (7, 123456789, 2), (2 ** 63 + 5, 2 ** 40 + 3, 1)):
-        want = (mix((seed + 3 * L + a) & M) >> 40) / 2.0 ** 24 - 0.5
+        want = ((mix((seed + L) & M) >> (21 * a)) & (2 ** 21 - 1)) / 2.0 ** 21 - 0.5
         assert oracle.jitter(seed, L, a) == want and -0.5 <= want < 0.5
     grid = inputs.Grid((20, 13, 9), (-0.3, 0.1, 0.0), (0.05, 0.04, 0.1))
     sub = grid.batch((1, 0, 0), (1, 2, 1))
