@@ -60,7 +60,7 @@ def test_prune(oracle):
     ctx.close()
 
 
-@pytest.mark.parametrize("kind", ["grid", "points"])
+@pytest.mark.parametrize("kind", ["grid", "grid_jitter", "points"])
 def test_densify(oracle, kind):
     import torch
     from paper_2607_01164_b200 import api
@@ -72,10 +72,11 @@ def test_densify(oracle, kind):
     raw["raw_scale"][:n] = np.log(g.scale)
     raw["quat"][:n] = g.quat
     ctx = api.Context()
-    if kind == "grid":
+    if kind.startswith("grid"):
         grid = inputs.Grid((29, 18, 21), (0.0, 0.1, 0.0), (1 / 29, 1 / 24, 1 / 21)).batch((1, 0, 0), (2, 2, 3))
-        xyz = oracle.grid_points(grid)
-        q, dom = api.grid_query(grid), None
+        seed = 77 if kind == "grid_jitter" else None   # new Gaussians sit at the jittered samples (D26)
+        xyz = oracle.grid_points(grid, jitter_seed=seed)
+        q, dom = api.grid_query(grid, jitter_seed=seed), None
     else:
         xyz = rng.uniform(0, 1, (5000, 3)).astype(np.float32)
         xyz_d = to_dev(torch, xyz)[0]
