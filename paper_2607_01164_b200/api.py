@@ -265,14 +265,18 @@ class Context:
         n = int(raw["raw_opacity"].shape[0])
         return _RawParams(n, *[_ptr(raw[k]).value for k in ("mean", "raw_scale", "quat", "raw_opacity", "raw_scalar")])
 
-    def gs_params_activate(self, raw: dict, scale, opacity, scalar):
-        """raw: dict of device tensors mean, raw_scale, quat, raw_opacity, raw_scalar."""
+    def gs_params_activate(self, raw: dict, scale, opacity, scalar, n=None):
+        """raw: dict of device tensors mean, raw_scale, quat, raw_opacity, raw_scalar (n: Gaussians in use, default all)."""
         r = self._raw(raw)
+        if n is not None:
+            r.n = int(n)
         self._check(self.lib.gs_params_activate(self.h, C.byref(r), _ptr(scale), _ptr(opacity), _ptr(scalar)))
 
     def gs_adam_step(self, raw: dict, grads: dict, m, v, step: int, lr=PAPER_LR, beta1=0.9, beta2=0.999, eps=1e-8,
-                     scale_out=None, opacity_out=None, scalar_out=None):
+                     scale_out=None, opacity_out=None, scalar_out=None, n=None):
         r = self._raw(raw)
+        if n is not None:
+            r.n = int(n)
         g = _Grads(*[(_ptr(grads.get(k)).value if grads.get(k) is not None else None)
                      for k in ("dmean", "dscale", "dquat", "dopacity", "dscalar", "err")])
         cfg = _AdamCfg((C.c_float * 5)(*lr), beta1, beta2, eps, int(step))
