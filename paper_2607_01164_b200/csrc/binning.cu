@@ -364,17 +364,21 @@ cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t 
     return cudaGetLastError();
 }
 
-// random bits of every voxel of a jittered batch (D26): one hash per voxel, read by the forward, the
-// backward and the densification of this step
-__global__ void __launch_bounds__(256) k_jitter_table(GridDesc gd, uint2 *__restrict__ jit) {
+// sample positions of a jittered batch (D26): one hash per voxel, three 21-bit offsets, the canonical
+// position fmaf(((float)i + 0.5f) + j, spacing, origin) per axis; written once per step and read by the forward, the
+// backward and the densification (16 B per voxel)
+__global__ void __launch_bounds__(256) k_jitter_table(GridDesc gd, float4 *__restrict__ jit) {
     const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
     if (x >= (uint32_t)gd.bdim[0]) return;
-    const unsigned long long L = voxel_linear((int)x + BRICK * gd.brick_lo[0], (int)y + BRICK * gd.brick_lo[1],
-                                              (int)z + BRICK * gd.brick_lo[2], gd.dims[0], gd.dims[1]);
-    jit[((size_t)z * gd.bdim[1] + y) * gd.bdim[0] + x] = voxel_hash(gd.jitter_seed, L);
+    const int gx = (int)x + BRICK * gd.brick_lo[0], gy = (int)y + BRICK * gd.brick_lo[1], gz = (int)z + BRICK * gd.brick_lo[2];
+    float jx, jy, jz;
+    voxel_jitter3(voxel_hash(gd.jitter_seed, voxel_linear(gx, gy, gz, gd.dims[0], gd.dims[1])), jx, jy, jz);
+    jit[((size_t)z * gd.bdim[1] + y) * gd.bdim[0] + x] =
+        make_float4(voxel_sample(gx, jx, gd.spacing[0], gd.origin[0]), voxel_sample(gy, jy, gd.spacing[1], gd.origin[1]),
+                    voxel_sample(gz, jz, gd.spacing[2], gd.origin[2]), 0.f);
 }
 
-cudaError_t launch_jitter_table(const GridDesc &gd, uint2 *jit, cudaStream_t s) {
+cudaError_t launch_jitter_table(const GridDesc &gd, float4 *jit, cudaStream_t s) {
     const dim3 grid((unsigned)((gd.bdim[0] + 255) / 256), (unsigned)gd.bdim[1], (unsigned)gd.bdim[2]);
     k_jitter_table<<<grid, 256, 0, s>>>(gd, jit); count_launch();
     return cudaGetLastError();

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) k_select_keys(const float *__restrict__ e
 
 // Gaussian n_old + j from the j-th selected sample
 __global__ void __launch_bounds__(256) k_new_gaussians(ParamSet d, uint32_t n_old, uint32_t n_new, const uint32_t *__restrict__ sel,
-                                                        GridDesc gd, const uint2 *__restrict__ jit, const float *__restrict__ xyz /*NULL: grid*/,
+                                                        GridDesc gd, const float4 *__restrict__ jit, const float *__restrict__ xyz /*NULL: grid*/,
                                                         const float *__restrict__ target, float raw_scale_init, float raw_opacity_init,
                                                         float clamp) {
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -88,11 +88,8 @@ __global__ void __launch_bounds__(256) k_new_gaussians(ParamSet d, uint32_t n_ol
         const uint32_t x = c % bdx, y = (c / bdx) % bdy, z = c / (bdx * bdy);
         const int gx = (int)x + BRICK * gd.brick_lo[0], gy = (int)y + BRICK * gd.brick_lo[1], gz = (int)z + BRICK * gd.brick_lo[2];
         if (gd.jitter) {  // the sample the error was measured at (D26)
-            float jx, jy, jz;
-            voxel_jitter3(jit[c], jx, jy, jz);
-            px = voxel_sample(gx, jx, gd.spacing[0], gd.origin[0]);
-            py = voxel_sample(gy, jy, gd.spacing[1], gd.origin[1]);
-            pz = voxel_sample(gz, jz, gd.spacing[2], gd.origin[2]);
+            const float4 sp = jit[c];
+            px = sp.x; py = sp.y; pz = sp.z;
         } else {
             px = voxel_centre(gx, gd.spacing[0], gd.origin[0]);
             py = voxel_centre(gy, gd.spacing[1], gd.origin[1]);
@@ -165,7 +162,7 @@ cudaError_t launch_select_keys(const float *err, const float *I, const uint8_t *
 }
 
 cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *sel, const GridDesc &gd,
-                                 const uint2 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
+                                 const float4 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
                                  float *scratch, cudaStream_t s) {
     const ParamSet o{p.mean, p.raw_scale, p.quat, p.raw_opacity, p.raw_scalar, m, v};
     const ParamSet d = carve(scratch, n_new);

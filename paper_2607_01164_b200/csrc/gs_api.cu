@@ -241,8 +241,8 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         ctx->M = (uint32_t)T64[1];
         ctx->have_pair_brick = false;
         if (gd.jitter && P > 0) {
-            CK(ctx->jit.reserve(P * sizeof(uint2)), "alloc jitter table");
-            CK(launch_jitter_table(gd, ctx->jit.as<uint2>(), s), "jitter table");
+            CK(ctx->jit.reserve(P * sizeof(float4)), "alloc jitter table");
+            CK(launch_jitter_table(gd, ctx->jit.as<float4>(), s), "jitter table");
         }
         ctx->T = T;
         ctx->nbricks = nbricks;
@@ -338,7 +338,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
     if (ctx->accel_kind == GS_QUERY_GRID) {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_gauss.as<uint32_t>(),
-                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<uint2>(), s), "grid forward");
+                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<float4>(), s), "grid forward");
     } else {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
@@ -434,7 +434,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         }
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, ctx->r2,
-                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<uint2>(), s), "grid backward");
+                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<float4>(), s), "grid backward");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
@@ -609,7 +609,7 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
     float *scratch = ctx->dens_scratch.as<float>();
     CK(launch_regather(*p, m, v, n_new, nullptr, n, scratch, false, s), "densify gather");
     const float *xyz = ctx->accel_kind == GS_QUERY_POINTS ? ctx->accel_q.xyz : nullptr;
-    CK(launch_new_gaussians(*p, m, v, n_new, vals[sel], ctx->grid, ctx->jit.as<uint2>(), xyz, target, raw_scale_init, raw_opacity_init, 1e-4f, scratch, s),
+    CK(launch_new_gaussians(*p, m, v, n_new, vals[sel], ctx->grid, ctx->jit.as<float4>(), xyz, target, raw_scale_init, raw_opacity_init, 1e-4f, scratch, s),
        "new gaussians");
     CK(cudaStreamSynchronize(s), "sync");
     return GS_OK;

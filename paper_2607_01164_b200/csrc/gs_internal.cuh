@@ -106,7 +106,7 @@ struct gs_ctx {
     gs::DevBuf pair_brick;   // uint32 [T]: debug view only (gs_debug_get)
     gs::DevBuf grid_order;   // uint32 [M]: processing order of the backward
     gs::DevBuf brick_start;  // uint32 [nbricks + norder + 1]: runs of the bricks, then of the order buckets (offset by T)
-    gs::DevBuf jit;          // uint2 [P]: per-voxel random bits of a jittered grid batch (D26)
+    gs::DevBuf jit;          // float4 [P]: sample positions of a jittered grid batch (D26)
     gs::DevBuf bwd_setup;    // float4 [N][2]: per-Gaussian constants of the structured backward (k_brick_count)
     // ---- accel (points)
     uint64_t P = 0;
@@ -174,14 +174,14 @@ struct BwdIn {
 };
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
-                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const uint2 *jit, cudaStream_t s);
-// per-voxel random bits of a jittered batch (gd.jitter; D26), batch-local sample order, written once per gs_build_accel
-cudaError_t launch_jitter_table(const GridDesc &gd, uint2 *jit, cudaStream_t s);
+                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, cudaStream_t s);
+// per-voxel sample positions of a jittered batch (gd.jitter; D26), batch-local sample order, written once per gs_build_accel
+cudaError_t launch_jitter_table(const GridDesc &gd, float4 *jit, cudaStream_t s);
 // second pass of gs_sample_fwd_loss: dL_dI[c] /= |D-| or |U+| (by sign), loss_terms = (L_rec, L_FN, L_FP)
 cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *loss_terms, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float r2, float *gacc, const uint32_t *order, uint32_t M, const uint2 *jit, cudaStream_t s);
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, cudaStream_t s);
 
 // grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the
 // cell steps are folded in); eps_scale multiplies the error share (fused MSE: eps = |alpha| * eps_scale, else 1)
@@ -203,7 +203,7 @@ cudaError_t launch_regather(const gs_raw_params &p, float *m, float *v, uint32_t
 cudaError_t launch_select_keys(const float *err, const float *I, const uint8_t *defined, size_t P, float tau, uint32_t *key, uint32_t *val,
                                cudaStream_t s);
 cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *sel, const GridDesc &gd,
-                                 const uint2 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
+                                 const float4 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
                                  float *scratch, cudaStream_t s);
 
 // peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)

@@ -80,7 +80,7 @@ template <bool PACK2, bool JIT>
 __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
                                                               GridDesc gd, const void *__restrict__ pack_, float r2,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
-                                                              uint32_t M, const uint2 *__restrict__ jit /*JIT: per-voxel random bits*/) {
+                                                              uint32_t M, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // a warp processes GPW consecutive Gaussians of the brick-ordered list of the M Gaussians that touch the batch
@@ -170,14 +170,12 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
 #pragma unroll
             for (int v = 0; v < 8; v++) {
                 const int gx = X + (v & 1), gy = Y + ((v >> 1) & 1), gz = Z + (v >> 2);
-                // random bits of the voxel from the per-step table (zero for a voxel outside the batch: its coefficients are zero)
+                // the voxel's sample position from the per-step table (a voxel outside the batch has zero coefficients: any
+                // finite position will do)
                 const bool inb = gx <= last[0] && gy <= last[1] && gz <= last[2];
                 const uint32_t cv = base + ((uint32_t)(v >> 2) * bdy + (uint32_t)((v >> 1) & 1)) * bdx + (uint32_t)(v & 1);
-                float jx = 0.f, jy = 0.f, jz = 0.f;
-                if (on && inb) voxel_jitter3(__ldg(jit + cv), jx, jy, jz);
-                const float dxv = __fsub_rn(voxel_sample(gx, jx, gd.spacing[0], gd.origin[0]), ga.x);
-                const float dyv = __fsub_rn(voxel_sample(gy, jy, gd.spacing[1], gd.origin[1]), ga.y);
-                const float dzv = __fsub_rn(voxel_sample(gz, jz, gd.spacing[2], gd.origin[2]), ga.z);
+                const float4 sp = (on && inb) ? __ldg(jit + cv) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const float dxv = __fsub_rn(sp.x, ga.x), dyv = __fsub_rn(sp.y, ga.y), dzv = __fsub_rn(sp.z, ga.z);
                 const float u0 = __fmaf_rn(gb.z, dzv, __fmaf_rn(gb.y, dyv, __fmul_rn(gb.x, dxv)));
                 const float u1 = __fmaf_rn(gc.z, dzv, __fmaf_rn(gc.y, dyv, __fmul_rn(gc.x, dxv)));
                 const float u2 = __fmaf_rn(gd4.z, dzv, __fmaf_rn(gd4.y, dyv, __fmul_rn(gd4.x, dxv)));
@@ -324,7 +322,7 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
 }
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float r2, float *gacc, const uint32_t *order, uint32_t M, const uint2 *jit, cudaStream_t s) {
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, cudaStream_t s) {
     // only the M Gaussians of the order list get (and need) an accumulator row: k_finalize reads those alone
     if (M == 0) return cudaSuccess;
     const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);

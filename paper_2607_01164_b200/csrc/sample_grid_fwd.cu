@@ -32,7 +32,7 @@ template <bool SETS, bool JIT>
 __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const float4 *__restrict__ rec, uint32_t N, GridDesc gd,
                                                            const uint32_t *__restrict__ pair_gauss,
                                                            const uint32_t *__restrict__ brick_start, float tau, float r2, FwdOut o,
-                                                           double invP, const uint2 *__restrict__ jit /*JIT: per-voxel random bits*/) {
+                                                           double invP, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/) {
     __shared__ float4 srec[4][CAP];
     __shared__ uint32_t sid[CAP];
     __shared__ uint4 smask[FWD_THREADS / 32][32];  // [warp][cell] -> masks of the 4 sub-chunks
@@ -59,11 +59,9 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
             const int x = lx + (v & 1), y = ly + ((v >> 1) & 1), z = lz + (v >> 2);
             const bool in = x < gd.bdim[0] && y < gd.bdim[1] && z < gd.bdim[2];
             const int gx = x + BRICK * gd.brick_lo[0], gy = y + BRICK * gd.brick_lo[1], gz = z + BRICK * gd.brick_lo[2];
-            float jx = 0.f, jy = 0.f, jz = 0.f;
-            if (in) voxel_jitter3(jit[((uint32_t)z * (uint32_t)gd.bdim[1] + (uint32_t)y) * (uint32_t)gd.bdim[0] + (uint32_t)x], jx, jy, jz);
-            jp[v][0] = in ? voxel_sample(gx, jx, gd.spacing[0], gd.origin[0]) : nanv;
-            jp[v][1] = in ? voxel_sample(gy, jy, gd.spacing[1], gd.origin[1]) : nanv;
-            jp[v][2] = in ? voxel_sample(gz, jz, gd.spacing[2], gd.origin[2]) : nanv;
+            float4 sp = make_float4(nanv, nanv, nanv, 0.f);
+            if (in) sp = jit[((uint32_t)z * (uint32_t)gd.bdim[1] + (uint32_t)y) * (uint32_t)gd.bdim[0] + (uint32_t)x];
+            jp[v][0] = sp.x; jp[v][1] = sp.y; jp[v][2] = sp.z;
         }
     }
     // cull geometry (not canonical): centre of the warp's cell (0,0,0), cell pitch = 2 voxels, half extent = half a voxel
@@ -290,7 +288,7 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
 }
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
-                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const uint2 *jit, cudaStream_t s) {
+                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, cudaStream_t s) {
     const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
     if (nbricks == 0) return cudaSuccess;
     const double P = (double)gd.bdim[0] * gd.bdim[1] * gd.bdim[2];
