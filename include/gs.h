@@ -171,7 +171,9 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
  *   sample_err[c] = defined ? |Phi_c - target_c| : 0
  * |D-| and |U+| are only known once every sample has been seen: the epilogue writes dL_dI
  * un-normalised and a second, elementwise kernel divides by the counts and writes loss_terms.
- * Pass the outputs to gs_sample_bwd(phi, I, dL_dphi, dL_dI, target).
+ * Pass the outputs to gs_sample_bwd(phi, I, dL_dphi, dL_dI, target); on a GRID query the epilogue also keeps the
+ * per-sample backward coefficients (alpha, beta, eps), so gs_sample_bwd(dL_dphi = NULL) differentiates this loss
+ * without re-reading the five per-sample arrays.
  * Errors: STATE, INVALID_ARG (negative lambda / eps, unknown kind, num_defined = 0 with P > 0), CUDA. */
 typedef enum { GS_LOSS_MSE = 0, GS_LOSS_L1 = 1 } gs_loss_kind;
 typedef struct gs_loss {

@@ -168,7 +168,7 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->have_pre = false;
     ctx->accel_kind = -1;
-    ctx->fused_pack = false;
+    ctx->fused_pack = 0;
     const size_t n = g->n ? g->n : 1;
     CK(ctx->rec.reserve(n * 64), "alloc records");
     CK(ctx->aabb.reserve(n * 24), "alloc aabb");
@@ -197,7 +197,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     if (st != GS_OK) return st;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->accel_kind = -1;
-    ctx->fused_pack = false;
+    ctx->fused_pack = 0;
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
     Stage stage(ctx, GS_PROF_BUILD);
@@ -357,13 +357,13 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     if (ctx->P > 0 && !target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr, nullptr};
-    ctx->fused_pack = false;
+    ctx->fused_pack = 0;
     if (target && ctx->P > 0) {  // keep the backward coefficients of the fused MSE for gs_sample_bwd(dL_dphi = NULL)
         CK(ctx->misc.reserve(ctx->P * 16), "alloc sample pack");
         o.pack2 = ctx->misc.as<float2>();
     }
     st = run_fwd(ctx, o);
-    if (st == GS_OK && o.pack2) ctx->fused_pack = true;
+    if (st == GS_OK && o.pack2) ctx->fused_pack = 1;
     return st;
 }
 
@@ -397,13 +397,18 @@ gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss
     o.gen.inv_nd = ctx->P ? (float)(1.0 / (double)loss->num_defined) : 0.f;
     o.gen.sums = sums;
     o.gen.counts = counts;
-    ctx->fused_pack = false;  // the backward of this loss takes dL_dphi and dL_dI explicitly
+    ctx->fused_pack = 0;
+    if (ctx->accel_kind == GS_QUERY_GRID && ctx->P > 0) {  // keep the backward coefficients for gs_sample_bwd(dL_dphi = NULL)
+        CK(ctx->misc.reserve(ctx->P * 16), "alloc sample pack");
+        o.gen.pack4 = ctx->misc.as<float4>();
+    }
     if (ctx->P > 0) {
         st = run_fwd(ctx, o);
         if (st != GS_OK) return st;
     }
     Stage stage(ctx, GS_PROF_FWD);
     CK(launch_loss_finish(o.gen, ctx->P, (double)loss->num_defined, loss_terms, s), "loss finish");
+    if (o.gen.pack4) ctx->fused_pack = 2;
     return GS_OK;
 }
 
@@ -416,7 +421,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         return fail(ctx, GS_ERR_INVALID_ARG, "gradient outputs must be given");
     const bool fused = dL_dphi == nullptr;
     if (fused && ctx->P > 0 && (!ctx->fused_pack || dL_dI))
-        return fail(ctx, GS_ERR_STATE, "dL_dphi = NULL needs a preceding gs_sample_fwd with a target on the same accel (and dL_dI = NULL)");
+        return fail(ctx, GS_ERR_STATE, "dL_dphi = NULL needs a preceding gs_sample_fwd with a target (or, on a grid, gs_sample_fwd_loss) on the same accel, and dL_dI = NULL");
     if (!fused && ctx->P > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "phi and I must be given with dL_dphi");
     if (ctx->N > 0 && ((uintptr_t)out->dquat & 15)) return fail(ctx, GS_ERR_INVALID_ARG, "dquat must be 16-byte aligned");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
@@ -424,16 +429,17 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     const uint32_t N = ctx->N;
     if (N == 0) return GS_OK;
     CK(ctx->gacc.reserve((size_t)N * GACC_GRID * 4), "alloc gradient accumulator");
-    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused ? ctx->misc.as<float2>() : nullptr, 0.5f * (float)ctx->P};
+    const bool fused2 = fused && ctx->fused_pack == 1;  // float2 coefficients of the fused MSE; otherwise float4 coefficients
+    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused2 ? ctx->misc.as<float2>() : nullptr, 0.5f * (float)ctx->P};
     if (ctx->accel_kind == GS_QUERY_GRID) {
         if (!fused) {
-            ctx->fused_pack = false;  // misc is overwritten with the caller's coefficients
+            ctx->fused_pack = 0;  // misc is overwritten with the caller's coefficients
             CK(ctx->misc.reserve((ctx->P ? ctx->P : 1) * 16), "alloc sample pack");
             Stage stage(ctx, GS_PROF_BWD_PACK);
             CK(launch_pack_samples(in, ctx->P, ctx->tau, ctx->misc.as<float4>(), s), "pack samples");
         }
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused, ctx->r2,
+        CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused2, ctx->r2,
                            ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<float4>(), s), "grid backward");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
@@ -444,7 +450,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     }
     Stage stage(ctx, GS_PROF_FINALIZE);
     const bool grid = ctx->accel_kind == GS_QUERY_GRID;
-    CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused) ? in.eps_scale : 1.f,
+    CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused2) ? in.eps_scale : 1.f,
                        *out, grid ? ctx->grid_order.as<uint32_t>() : nullptr, grid ? ctx->M : 0, s), "finalize");
     return GS_OK;
 }

@@ -123,7 +123,8 @@ struct gs_ctx {
     // ---- scratch
     gs::DevBuf scan_tmp, sort_hist, gacc, misc, counters, dbg;
     gs::DevBuf dens_work, dens_scratch, sel_key[2], sel_val[2];  // gs_prune / gs_densify
-    bool fused_pack = false;  // misc holds the coefficients written by the last gs_sample_fwd with a target
+    int fused_pack = 0;  // misc holds backward coefficients written by the last forward: 1 = float2 (alpha, beta) of gs_sample_fwd's
+                         // fused MSE, 2 = float4 (alpha, beta, eps, -) of gs_sample_fwd_loss on a grid; 0 = none
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr;

@@ -14,6 +14,7 @@ struct GenLoss {
     int kind;                    // gs_loss_kind
     const uint8_t *defined;      // nullable
     float *dL_dI;                // nullable
+    float4 *pack4;               // nullable (grid): backward coefficients (alpha, beta, eps, -) for gs_sample_bwd(dL_dphi = NULL)
     float lam_fn, thr_fn, lam_fp;
     float inv_nd;                // 1 / |D|
     double *sums;                // [3] sum_D rho(res) | sum_{D-} (thr - I) | sum_{U+} I
@@ -53,6 +54,11 @@ __device__ __forceinline__ void loss_sample(const GenLoss &L, size_t c, float ph
     if (dL_dphi) dL_dphi[c] = a;
     if (L.dL_dI) L.dL_dI[c] = b;
     if (sample_err) sample_err[c] = e;
+    if (L.pack4) {  // alpha = a / I, beta = b - alpha Phi (b still un-normalised: kept in .w for k_loss_finish), eps = |res| / I
+        const float inv = covered ? __fdividef(1.0f, I) : 0.f;
+        const float alpha = a * inv;
+        L.pack4[c] = make_float4(alpha, -alpha * phi, e * inv, b);
+    }
 }
 
 // warp reduction of the partial sums, one atomic per non-zero term and warp

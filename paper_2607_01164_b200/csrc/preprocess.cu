@@ -204,14 +204,20 @@ __global__ void __launch_bounds__(256) k_loss_finish(GenLoss L, size_t P, double
         loss_terms[1] = nfn ? (double)L.lam_fn * L.sums[1] / (double)nfn : 0.0;
         loss_terms[2] = nfp ? (double)L.lam_fp * L.sums[2] / (double)nfp : 0.0;
     }
-    if (c >= P || !L.dL_dI) return;
-    const float b = L.dL_dI[c];
-    if (b < 0.f) L.dL_dI[c] = b / (float)nfn;
-    else if (b > 0.f) L.dL_dI[c] = b / (float)nfp;
+    if (c >= P) return;
+    if (L.dL_dI) {
+        const float b = L.dL_dI[c];
+        if (b < 0.f) L.dL_dI[c] = b / (float)nfn;
+        else if (b > 0.f) L.dL_dI[c] = b / (float)nfp;
+    }
+    if (L.pack4) {  // beta = b - alpha Phi with the normalised b
+        const float b = L.pack4[c].w;
+        if (b != 0.f) L.pack4[c].y += b / (float)(b < 0.f ? nfn : nfp);
+    }
 }
 
 cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *loss_terms, cudaStream_t s) {
-    const bool per_sample = L.dL_dI && (L.lam_fn > 0.f || L.lam_fp > 0.f);
+    const bool per_sample = (L.dL_dI || L.pack4) && (L.lam_fn > 0.f || L.lam_fp > 0.f);
     const size_t n = per_sample && P ? P : 1;
     k_loss_finish<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(L, per_sample ? P : 0, nd, loss_terms); count_launch();
     return cudaGetLastError();

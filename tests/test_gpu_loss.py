@@ -72,6 +72,19 @@ def _run(oracle, g, kind_name, query_kind, query_obj, xyz, target, defined, doma
     # which gs_sample_bwd does not take; compare the parameter gradients only
     gr = {k: v for k, v in gr.items() if k != "err"}
     errs = check_grads(r, gr)
+    if query_kind == "grid":
+        # on a grid the forward kept the backward coefficients: gs_sample_bwd(dL_dphi = NULL) must give the same gradients
+        grads2 = ctx.alloc_grads(g.n)
+        ctx.gs_sample_fwd_loss(q, phi, I, t_d, kind=kind, lambda_fn=LAM_FN, eps_fn=EPS_FN, lambda_fp=LAM_FP, defined=def_d,
+                               num_defined=nd, loss_terms=terms)
+        ctx.gs_sample_bwd(q, None, None, None, grads2)
+        torch.cuda.synchronize()
+        r2 = R()
+        r2.grads_np = lambda: {k: v.detach().cpu().numpy().astype(np.float64) for k, v in grads2.items()}
+        check_grads(r2, gr)
+    else:
+        with pytest.raises(api.GsError):   # a point query keeps no coefficients
+            ctx.gs_sample_bwd(q, None, None, None, grads)
     ctx.close()
     return errs, ref
 
