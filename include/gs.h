@@ -190,9 +190,10 @@ gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss
  * from dL_dphi[P] and dL_dI[P] (nullable = 0), re-computing the kernel weights from phi/I of the
  * forward pass (nothing else is kept from it).  dL_dphi of an uncovered sample (I_c <= tau) is
  * ignored.  target (nullable) is only used for the error statistic out->err.
- * Fused-loss form: dL_dphi == NULL means "the MSE loss of the preceding gs_sample_fwd(target != NULL) on this
- * accel": that forward keeps its per-sample backward coefficients (alpha, beta, eps) in context scratch, so the
- * backward reads them instead of phi / I / dL_dphi / target (all ignored, may be NULL); dL_dI must be NULL.
+ * Fused-loss form: dL_dphi == NULL means "the loss of the preceding forward on this accel" -- the MSE of
+ * gs_sample_fwd(target != NULL), or (grid queries) the losses of gs_sample_fwd_loss: that forward keeps its
+ * per-sample backward coefficients (alpha, beta, eps) in context scratch, so the backward reads them instead
+ * of phi / I / dL_dphi / target (all ignored, may be NULL); dL_dI must be NULL.
  * STATE if no such forward preceded (or the scratch was overwritten by a non-fused gs_sample_bwd).
  * Errors: STATE, INVALID_ARG, OVERFLOW, CUDA. */
 gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi,
