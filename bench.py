@@ -198,7 +198,29 @@ def run_ours(args):
     if world > 1:  # data-parallel exchange: one all-reduce of the gradients
         flat = torch.empty(g.n * 16, device="cuda")
 
+    recipe = args.step == "recipe"
+    cur_q = [q]  # the query the acceleration structure was last built for
+    if recipe:  # the paper's training step: raw parameters, jitter, L1 + Eq. 4, Adam
+        assert wl["kind"] == "grid", "--step recipe needs a grid workload"
+        logit = lambda x: np.log(x / (1 - x))
+        raw = dict(mean=gd[0], raw_scale=dev(np.log(g.scale)), quat=gd[2],
+                   raw_opacity=dev(logit(np.clip(g.opacity.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)),
+                   raw_scalar=dev(logit(np.clip(g.scalar.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)))
+        m_d, v_d = torch.zeros(12 * g.n, device="cuda"), torch.zeros(12 * g.n, device="cuda")
+        terms = torch.zeros(3, dtype=torch.float64, device="cuda")
+        it = [0]
+
     def step():
+        if recipe:
+            it[0] += 1
+            qj = api.grid_query(wl["grid"], jitter_seed=it[0])   # a new random position in every cell
+            ctx.gs_preprocess(raw["mean"], gd[1], raw["quat"], gd[3], gd[4], tau=TAU)
+            ctx.gs_build_accel(qj)
+            cur_q[0] = qj
+            ctx.gs_sample_fwd_loss(qj, phi, I, target, kind=api.LOSS_L1, lambda_fn=0.5, eps_fn=0.5, loss_terms=terms)
+            ctx.gs_sample_bwd(qj, None, None, None, grads)
+            ctx.gs_adam_step(raw, grads, m_d, v_d, it[0], scale_out=gd[1], opacity_out=gd[3], scalar_out=gd[4])
+            return
         loss.zero_()
         ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
         ctx.gs_build_accel(q)
@@ -217,7 +239,7 @@ def run_ours(args):
         step()
     barrier()
     # hit / tested pair counts of this workload (outside the timed region)
-    _, _, _, tested, hits = ctx.debug_point_sets(q)
+    _, _, _, tested, hits = ctx.debug_point_sets(cur_q[0])
     ffma_peak, ex2_peak = ctx.measure_alu_peaks()  # measured ALU denominators at the clocks of this run
     ctx.profile_read()
     ctx.profile_enable(True)
@@ -292,7 +314,7 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl["desc"], "points_per_step": P, "gaussians": g.n, "hit_pairs": hits, "tested_pairs": tested,
                        "l2": "working set per step (>600 MB of per-sample arrays) exceeds the 126 MB L2; no flush",
-                       "step": "preprocess+build_accel+fwd(MSE)+bwd"},
+                       "step": "preprocess+build_accel+fwd(L1+FN, jittered samples)+bwd+adam" if recipe else "preprocess+build_accel+fwd(MSE)+bwd"},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": "points/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": float(te.item()),
@@ -337,6 +359,8 @@ def main():
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--step", default="mse", choices=["mse", "recipe"],
+                    help="mse: the north_star step (default); recipe: the paper's training step (jitter, L1 + Eq. 4, Adam)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
