@@ -72,45 +72,6 @@ __device__ __forceinline__ unsigned long long mix64(uint32_t id) {
     return z ^ (z >> 31);
 }
 
-// Transposing butterfly: every lane contributes v[0..15]; afterwards lane L holds in v[0] the
-// warp-wide sum of component L >> 1 (16 SHFL instead of 16 x 5).
-__device__ __forceinline__ void warp_reduce16(float (&v)[16], int lane) {
-    {
-        const bool up = lane & 16;
-#pragma unroll
-        for (int k = 0; k < 8; k++) {
-            const float send = up ? v[k] : v[k + 8];
-            const float keep = up ? v[k + 8] : v[k];
-            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-        }
-    }
-    {
-        const bool up = lane & 8;
-#pragma unroll
-        for (int k = 0; k < 4; k++) {
-            const float send = up ? v[k] : v[k + 4];
-            const float keep = up ? v[k + 4] : v[k];
-            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        }
-    }
-    {
-        const bool up = lane & 4;
-#pragma unroll
-        for (int k = 0; k < 2; k++) {
-            const float send = up ? v[k] : v[k + 2];
-            const float keep = up ? v[k + 2] : v[k];
-            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-        }
-    }
-    {
-        const bool up = lane & 2;
-        const float send = up ? v[0] : v[1];
-        const float keep = up ? v[1] : v[0];
-        v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-    }
-    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-}
-
 // The backward contribution of one hit (S7):  with alpha = a/I, beta = b - alpha Phi (per sample),
 //   gamma = alpha v + beta,  t = gamma w G:  dv += alpha w G, dw += gamma G, U += t u, W += t u u^T, E += eps w G
 // acc layout: 0 dv | 1 dw | 2..4 U | 5..10 W00 W01 W02 W11 W12 W22 | 11 E
