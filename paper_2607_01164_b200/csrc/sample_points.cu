@@ -24,8 +24,14 @@
 
 namespace gs {
 
-constexpr int CULL_WARPS = 4;            // packets per CTA of k_points_cull
-constexpr int EVAL_WARPS = 4;            // packets per CTA of k_points_fwd / k_points_bwd
+#ifndef GS_CULL_WARPS
+#define GS_CULL_WARPS 4
+#endif
+#ifndef GS_EVAL_WARPS
+#define GS_EVAL_WARPS 4
+#endif
+constexpr int CULL_WARPS = GS_CULL_WARPS;  // packets per CTA of k_points_cull
+constexpr int EVAL_WARPS = GS_EVAL_WARPS;  // packets per CTA of k_points_fwd / k_points_bwd
 constexpr int STK_CAP = 256;             // stack entries per packet
 constexpr int STK_WIDE = STK_CAP - 66;   // above this fill level one node is popped per step (pure DFS: growth <= tree height <= 64)
 constexpr int CQ_CAP = 128;              // candidate queue: a step runs only with <= 64 queued and adds <= 64
