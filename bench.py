@@ -34,8 +34,8 @@ ALU_PEAK_TINSTR = 148 * 128 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (bytes); a kernel
 # that has no capture of the current build reports null
 NCU_TRAFFIC = {
-    ("c2", "k_grid_bwd"): (190.37e6 + 28.29e6, "profiles/r1_step4_c2_ncu_full.md"),
-    ("c2", "k_grid_fwd"): (113.57e6 + 224.11e6, "profiles/r1_step4_c2_ncu_full.md"),
+    ("c2", "k_grid_bwd"): (190.35e6 + 28.64e6, "profiles/r1_step6_c2_ncu_full.md"),
+    ("c2", "k_grid_fwd"): (113.68e6 + 224.00e6, "profiles/r1_step6_c2_ncu_full.md"),
     ("c3", "k_points_bwd"): (536.48e6 + 65.86e6, "profiles/r1_step4_c3.md"),
 }
 
