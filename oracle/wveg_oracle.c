@@ -22,8 +22,11 @@
  * Mahalanobis radius sqrt(-2 ln tau), textbook normal pdf (scipy), rotation about z by hand,
  * constant-scalar collections, convexity, weight splitting, central finite
  * differences of every gradient, sum rules, brute force vs culled, Morton/Karras brute force.
- * The per-Gaussian error statistic E_i (DESIGN D10) is NOT defined by the paper:
- * "parity unpinned" beyond its sum rule.
+ * The per-Gaussian error statistic E_i (DESIGN D10) is NOT defined by the paper (it is north_star's): its
+ * DEFINITION is "parity unpinned"; its arithmetic is pinned by the sum rule and by two closed forms
+ * (disjoint supports, coincident Gaussians: tests/test_oracle_atsize.py).
+ * The cell-grid cull (mode 1) is pinned against all pairs (mode 0) on tiny inputs AND against the full
+ * configs[1] / configs[2] models on point subsets (tests/test_oracle_atsize.py).
  */
 #include <math.h>
 #include <stdint.h>
@@ -234,7 +237,7 @@ static inline uint64_t mix_id(uint32_t id) {
 /* the plain all-pairs definition would reject too (tested: culled == all-pairs).          */
 /* ------------------------------------------------------------------------------------- */
 typedef struct {
-    double lo[3], inv_h[3];
+    double lo[3], hi[3], inv_h[3];   /* lo/hi: bounding box of the points */
     int32_t n[3];
     int64_t *cell_start;   /* [ncell+1] CSR over points */
     int64_t *cell_points;  /* [P] */
@@ -291,6 +294,7 @@ static int cellgrid_build(cellgrid *cg, const float *xyz, int64_t P, const float
     for (int k = 0; k < 3; k++) {
         double ext = hi[k] - lo[k];
         cg->lo[k] = lo[k];
+        cg->hi[k] = hi[k];
         cg->n[k] = (P > 0 && ext > 0.0) ? res : 1;
         cg->inv_h[k] = (cg->n[k] > 1) ? (double)cg->n[k] / ext : 0.0;
     }
@@ -656,6 +660,9 @@ int wo_backward(const wo_gaussians *g, const float *xyz, int64_t P, float tau, i
             int skip = 0;
             if (mode == 1) {
                 for (int k = 0; k < 3; k++) {
+                    /* an AABB that misses the points' bounding box holds no point: same skip as the forward's
+                       candidate lists (cellgrid_build), so that a small batch of a large model costs O(touched) */
+                    if ((double)t.aabb[6 * i + 3 + k] < cg.lo[k] || (double)t.aabb[6 * i + k] > cg.hi[k]) skip = 1;
                     ca[k] = cell_coord(&cg, k, (double)t.aabb[6 * i + k]);
                     cb[k] = cell_coord(&cg, k, (double)t.aabb[6 * i + 3 + k]);
                 }
