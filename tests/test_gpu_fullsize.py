@@ -3,7 +3,10 @@ configs[1] (C2): 256^3 Marschner-Lobb grid, 262,144 Gaussians, one whole-grid fo
 The oracle finishes this size in seconds (cell-grid cull, OpenMP), so every output is compared element
 by element: all 16.8 M intersection sets and the 2.56 M sorted pair keys bit-exact, Phi within 1e-5,
 every gradient tensor within 1e-4 relative L2.
-configs[2] (C3) is checked the same way on one 2^20-point batch (the oracle needs about a minute for it)."""
+configs[2] (C3) is checked the same way on one 2^20-point batch (the oracle needs about a minute for it).
+configs[3] (C4): the full 4,194,304-Gaussian model, two 128^3 brick-aligned batches of the 1024^3 grid with one
+gs_preprocess; configs[4] (C5): the full 8,388,608-Gaussian model, one 2^24-point batch -- forward AND backward, every
+output element against oracle mode 1 (whose cost is proportional to the hit pairs: ~5e6 and ~3e8)."""
 import numpy as np
 import pytest
 
@@ -109,3 +112,116 @@ def test_c4_like_batches(oracle):
         near = np.abs(ref["I"] - TAU) <= 2e-6 * TAU
         assert np.abs(phi.cpu().numpy() - ref["phi"])[~near].max() <= 1e-5
     ctx.close()
+
+
+class _Shim:
+    """What gpu_util.check_* need of a run, for flows that are not one GpuRun (several batches per preprocess)."""
+
+    def __init__(self, ctx, q, P, phi, I, grads):
+        self.ctx, self.q, self.P, self.phi, self.I, self.grads = ctx, q, P, phi, I, grads
+
+    def np(self, t):
+        return t.detach().cpu().numpy()[: self.P]
+
+    def grads_np(self):
+        return {k: v.detach().cpu().numpy().astype(np.float64) for k, v in self.grads.items()}
+
+    def sets(self):
+        return self.ctx.debug_point_sets(self.q)
+
+
+def test_c4_full_batch(oracle):
+    # BASELINE.json configs[3] at its stated size: 4,194,304 Gaussians (5 % needles of axis ratio 20:1) on a 1024^3 grid,
+    # decoded in 128^3 brick-aligned batches (16^3 bricks) with ONE gs_preprocess: an interior batch and the upper corner
+    import torch
+    from paper_2607_01164_b200 import api
+    field = inputs.c4_field(seed=4)
+    g = inputs.c4_gaussians(seed=4, n_grid=1024, n=4_194_304, field=field)
+    full = inputs.c4_grid(1024)
+    ctx = api.Context()
+    dev = [torch.from_numpy(x).cuda() for x in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    ctx.gs_preprocess(*dev)
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    assert np.array_equal(ctx.debug_get(api.DBG_AABB, np.float32, 6).view(np.uint32), aabb.view(np.uint32))
+    grads = ctx.alloc_grads(g.n)
+    for lo in ((48, 48, 48), (112, 112, 112)):
+        batch = full.batch(lo, (16, 16, 16))
+        P = batch.num_points
+        assert P == 128 ** 3
+        target = inputs.c4_target(batch, field)
+        xyz = oracle.grid_points(batch)
+        fwd = oracle.forward(g, xyz, TAU, mode=1)
+        loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+        gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+        q = api.grid_query(batch)
+        ctx.gs_build_accel(q)
+        # integer stage: the sorted (brick, gaussian) keys of this batch
+        blo, bhi, cnt = oracle.brick_ranges(aabb, valid, batch)
+        keys, start = oracle.brick_keys(blo, bhi, cnt, batch)
+        pb = ctx.debug_get(api.DBG_PAIR_BRICK, np.uint32)
+        pg = ctx.debug_get(api.DBG_PAIR_GAUSS, np.uint32)
+        assert len(keys) > 50_000
+        assert np.array_equal((pb.astype(np.uint64) << np.uint64(32)) | pg.astype(np.uint64), keys)
+        assert np.array_equal(ctx.debug_get(api.DBG_BRICK_START, np.uint32).astype(np.int64), start)
+        phi = torch.full((P,), -7.0, device="cuda")
+        I = torch.full((P,), -7.0, device="cuda")
+        dphi = torch.full((P,), -7.0, device="cuda")
+        lossd = torch.zeros(1, dtype=torch.float64, device="cuda")
+        t = torch.from_numpy(target).cuda()
+        ctx.gs_sample_fwd(q, phi, I, target=t, loss=lossd, dL_dphi=dphi)
+        for v in grads.values():
+            v.fill_(-7.0)
+        ctx.gs_sample_bwd(q, None, None, None, grads)   # backward of the fused MSE (what bench.py times)
+        torch.cuda.synchronize()
+        run = _Shim(ctx, q, P, phi, I, grads)
+        tested, hits = check_sets(run, fwd)
+        assert hits > 3_000_000
+        near, e_phi, e_I = check_forward(run, fwd)
+        assert near <= 16
+        assert float(lossd.item()) == pytest.approx(loss, rel=1e-6)
+        errs = check_grads(run, gr)
+        # the general backward (explicit dL/dPhi array) on the same batch
+        for v in grads.values():
+            v.fill_(-7.0)
+        ctx.gs_sample_bwd(q, phi, I, dphi, grads, target=t)
+        torch.cuda.synchronize()
+        errs2 = check_grads(run, gr)
+        print("C4 batch", lo, "T", len(keys), "hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs, errs2)
+    ctx.close()
+
+
+def test_c5_full_batch(oracle):
+    # BASELINE.json configs[4] at its stated size: 8,388,608 Gaussians (sigma 0.0005-0.002) centred on points of the
+    # shell-and-fragments distribution; one batch of 2^24 random points of a 40 M-point draw (the full 200 M-point set is
+    # only ever seen in such batches); LBVH, query sort and cull lists rebuilt by gs_build_accel
+    xyz_all, t_all = inputs.c5_points(seed=5, p=40_000_000)
+    g = inputs.c5_gaussians(xyz_all, t_all)
+    assert g.n == 8_388_608
+    idx = inputs.batch_indices(5, 0, len(xyz_all), 1 << 24)
+    xyz, target = np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])
+    dom = inputs.points_domain(xyz_all)
+    del xyz_all, t_all
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+    run = GpuRun(g, "points", xyz, target, domain=dom, fused=True)
+    api = run.api
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    codes = oracle.morton_codes(g.mean, dom[0], dom[1], valid)
+    order, keys = oracle.morton_order(codes)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_MORTON, np.uint32), codes[order])
+    assert np.array_equal(run.ctx.debug_get(api.DBG_LEAF_ORDER, np.uint32), order)
+    pcodes = oracle.morton_codes(xyz, dom[0], dom[1])
+    porder, _ = oracle.morton_order(pcodes)
+    assert np.array_equal(run.ctx.debug_get(api.DBG_POINT_ORDER, np.uint32), porder)
+    tested, hits = check_sets(run, fwd)   # all 2^24 intersection sets, bit-exact
+    assert hits > 200_000_000
+    near, e_phi, e_I = check_forward(run, fwd)
+    assert near <= 64
+    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
+    errs = check_grads(run, gr)
+    got = run.grads_np()
+    covered = fwd["I"].astype(np.float32) > np.float32(TAU)
+    assert got["dscalar"].sum() == pytest.approx(a[covered].sum(), rel=1e-4, abs=1e-7)
+    assert got["err"].sum() == pytest.approx(serr[covered].sum(), rel=1e-4)
+    print("C5 full batch: hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs)
