@@ -1,18 +1,23 @@
 #!/usr/bin/env python
-"""bench.py -- one JSON line for the W-VEG sampling hot path on B200 (contract: see DESIGN.md "Measurement").
+"""bench.py -- one JSON line for the W-VEG sampling hot path on B200 (contract: DESIGN.md section 9).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c1|c3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload all|c1|c2|c3|c4|c5] [--impl ours|reference]
 
 A step = one pass of the whole hot path over one batch of synthetic input:
 gs_preprocess -> gs_build_accel -> gs_sample_fwd (fused MSE) -> gs_sample_bwd.
-Default workload = BASELINE.json configs[1] (C2): 256^3 Marschner-Lobb grid, 262,144 Gaussians, full-grid
-forward+backward per step.  `value` = query points per second (whole job), inputs resident in HBM;
-`e2e` = the same through gs_step_host with pinned HOST buffers (H2D/D2H inside the timed region).
+The headline (`value`, `ms_per_step`, `roofline`, `e2e`, `cpu_baseline`) is the LARGEST single-GPU configuration of
+BASELINE.json, configs[4] (C5: 8,388,608 Gaussians, 2^24-point batches of the shell-and-fragments point set, LBVH
+rebuilt every step).  With the default `--workload all` the same figures for configs[1] (C2), configs[2] (C3) and
+configs[3] (C4, plus its forward-only decode rate) are printed beside it under `workloads`; `--workload cN` times that
+configuration alone.  `value` = query points per second (whole job), inputs resident in HBM; `e2e` = the same through
+gs_step_host with pinned HOST buffers (H2D/D2H inside the timed region).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
+import math
 import os
 import subprocess
 import sys
@@ -26,45 +31,145 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 TAU = 0.01
-# algorithmic FP32-pipe lane-instructions per HIT pair (DESIGN.md "Roofline"): canonical predicate + weight + accumulate
+HEADLINE = "c5"
+# algorithmic FP32-pipe lane-instructions per HIT pair (DESIGN.md section 7): canonical predicate + weight + accumulate
 INSTR_FWD = 19.0
 INSTR_BWD = 40.0
 # plain-ALU peak: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts / max SM clock)
 ALU_PEAK_TINSTR = 148 * 128 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (bytes); a kernel
-# that has no capture of the current build reports null
-NCU_TRAFFIC = {
-    ("c2", "k_grid_bwd"): (190.35e6 + 28.64e6, "profiles/r1_step6_c2_ncu_full.md"),
-    ("c2", "k_grid_fwd"): (113.68e6 + 224.00e6, "profiles/r1_step6_c2_ncu_full.md"),
-    ("c3", "k_points_bwd"): (536.48e6 + 65.86e6, "profiles/r1_step4_c3.md"),
-}
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+MIN_TIMED_S = 0.3   # secondary workloads repeat their step until the timed region is at least this long
 
 
-def make_workload(name: str, rank: int = 0):
+def csrc_sha16() -> str:
+    """Identity of the kernels this run executes: sha256 over csrc/* and include/gs.h (the GPU box has no .git)."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2607_01164_b200", "csrc")
+    for f in sorted(os.listdir(d)) + ["../../include/gs.h"]:
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def load_traffic():
+    """dram read + write bytes per launch from an `ncu --set full` capture, valid only for the build they were taken from
+    (profiles/traffic.json is written by `bench.py --record-traffic`, keyed by the csrc hash)."""
+    try:
+        t = json.load(open(TRAFFIC_JSON))
+    except (OSError, ValueError):
+        return {}, "no profiles/traffic.json"
+    if t.get("csrc_sha16") != csrc_sha16():
+        return {}, f"profiles/traffic.json is of another build ({t.get('csrc_sha16')} != {csrc_sha16()})"
+    return t.get("kernels", {}), t.get("source", "profiles/traffic.json")
+
+
+def record_traffic(csv_path: str, workload: str, source: str):
+    """Parse `ncu -i X.ncu-rep --page raw --csv` (one row per captured launch) and store dram bytes per launch."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr = rows[0]
+    ci = {h: i for i, h in enumerate(hdr)}
+    units = rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    acc = {}
+    for r in rows[2:]:
+        name = r[ci["Kernel Name"]]
+        short = name.split("(")[0].split("::")[-1].split("<")[0].replace("void ", "").strip()
+        tot = 0.0
+        for m in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            tot += float(r[ci[m]].replace(",", "")) * scale[units[ci[m]]]
+        acc.setdefault(short, []).append(tot)
+    try:
+        t = json.load(open(TRAFFIC_JSON))
+    except (OSError, ValueError):
+        t = {}
+    if t.get("csrc_sha16") != csrc_sha16():
+        t = {"csrc_sha16": csrc_sha16(), "kernels": {}, "source": source}
+    for k, v in acc.items():
+        t["kernels"][f"{workload}/{k}"] = {"bytes": sum(v) / len(v), "launches": len(v), "source": source}
+    json.dump(t, open(TRAFFIC_JSON, "w"), indent=1, sort_keys=True)
+    print(json.dumps(t, indent=1))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# workloads (BASELINE.json configs; the recipes are in DESIGN.md section 4)
+# ------------------------------------------------------------------------------------------------------------------
+def make_workload(name: str):
     from paper_2607_01164_b200 import inputs
-    if name == "c2":
-        grid = inputs.c2_grid(256)
-        g = inputs.c2_gaussians(seed=2 + 1000 * rank, n_grid=256, n=262144)
-        return dict(kind="grid", g=g, grid=grid, target=inputs.c2_target(grid), domain=None,
-                    desc="C2 structured 256^3 Marschner-Lobb, 262144 Gaussians (BASELINE.json configs[1])")
     if name == "c1":
         grid = inputs.c1_grid(32)
         g = inputs.c1_gaussians(seed=0, n=1024)
         rng = np.random.default_rng(1)
-        return dict(kind="grid", g=g, grid=grid, target=rng.uniform(0, 1, grid.num_points).astype(np.float32), domain=None,
+        return dict(name=name, kind="grid", g=g, grid=grid, target=rng.uniform(0, 1, grid.num_points).astype(np.float32), domain=None,
                     desc="C1 tiny structured 32^3, 1024 Gaussians (BASELINE.json configs[0])")
+    if name == "c2":
+        grid = inputs.c2_grid(256)
+        g = inputs.c2_gaussians(seed=2, n_grid=256, n=262144)
+        return dict(name=name, kind="grid", g=g, grid=grid, target=inputs.c2_target(grid), domain=None,
+                    desc="C2 structured 256^3 Marschner-Lobb, 262144 Gaussians, whole grid per step (BASELINE.json configs[1])")
     if name == "c3":
         xyz_all, t_all = inputs.c3_points(seed=3, p=2_000_000)
         g = inputs.c3_gaussians(xyz_all, t_all, seed=3, n=1_048_576)
-        idx = inputs.batch_indices(3, rank, len(xyz_all), 1 << 20)
-        return dict(kind="points", g=g, xyz=np.ascontiguousarray(xyz_all[idx]), target=np.ascontiguousarray(t_all[idx]),
-                    domain=inputs.points_domain(xyz_all),
-                    desc="C3 unstructured, 2^20-point batch of 2M, 1048576 Gaussians (BASELINE.json configs[2])")
+        batches = []
+        for b in range(4):   # a fresh batch (without replacement) per step, cycling through 4 resident ones
+            idx = inputs.batch_indices(3, b, len(xyz_all), 1 << 20)
+            batches.append((np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])))
+        return dict(name=name, kind="points", g=g, batches=batches, domain=inputs.points_domain(xyz_all),
+                    desc="C3 unstructured, 2^20-point batches (4 distinct, one per step) of 2M mixture points, 1048576 Gaussians, "
+                         "LBVH rebuilt per step (BASELINE.json configs[2])")
+    if name == "c4":
+        field = inputs.c4_field(seed=4)
+        g = inputs.c4_gaussians(seed=4, n_grid=1024, n=4_194_304, field=field)
+        full = inputs.c4_grid(1024)
+        grid = full.batch((48, 48, 48), (16, 16, 16))
+        return dict(name=name, kind="grid", g=g, grid=grid, full=full, target=inputs.c4_target(grid, field), domain=None,
+                    decode_blocks=[(16 * x, 16 * y, 16 * z) for z in range(4) for y in range(4) for x in range(4)],
+                    desc="C4 structured 1024^3 turbulence field, 4194304 Gaussians (5% 20:1 needles), one 128^3 brick-aligned batch "
+                         "per step (BASELINE.json configs[3])")
+    if name == "c5":
+        xyz_all, t_all = inputs.c5_points(seed=5, p=40_000_000)
+        g = inputs.c5_gaussians(xyz_all, t_all)
+        batches = []
+        for b in range(2):
+            idx = inputs.batch_indices(5, b, len(xyz_all), 1 << 24)
+            batches.append((np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])))
+        return dict(name=name, kind="points", g=g, batches=batches, domain=inputs.points_domain(xyz_all), decode_xyz=xyz_all,
+                    desc="C5 unstructured shell-and-fragments, 2^24-point batches (2 distinct, alternating) of a 40M-point draw of the "
+                         "200M-point set, 8388608 Gaussians, LBVH rebuilt per step (BASELINE.json configs[4])")
     raise SystemExit(f"unknown workload {name}")
 
 
+def shard_workload(wl, rank: int, world: int):
+    """This rank's share of every batch of the workload (host arrays; no GPU needed): a z-slab of the grid's bricks
+    (dist.shard_bricks) or a contiguous slice of each point batch (dist.shard_points).  Returns ([{grid | xyz, target}],
+    P_total); the list is empty for a rank whose slab is empty.  Every rank holds the SAME model."""
+    from paper_2607_01164_b200 import dist as gsdist
+    if wl["kind"] == "grid":
+        grid = wl["grid"]
+        P_total = grid.num_points
+        lo, cnt = gsdist.shard_bricks(grid.brick_cnt, rank, world)
+        if cnt[2] <= 0:
+            return [], P_total
+        sub = grid.batch(tuple(a + b for a, b in zip(grid.brick_lo, lo)), cnt)
+        bd = grid.batch_dims
+        z0 = 8 * lo[2]
+        t = np.asarray(wl["target"]).reshape(bd[2], bd[1], bd[0])[z0:z0 + sub.batch_dims[2]]
+        return [dict(grid=sub, target=np.ascontiguousarray(t).ravel())], P_total
+    P_total = len(wl["batches"][0][0])
+    a, b = gsdist.shard_points(P_total, rank, world)
+    return [dict(xyz=np.ascontiguousarray(x[a:b]), target=np.ascontiguousarray(t[a:b])) for x, t in wl["batches"]], P_total
+
+
+def config_of(wl) -> dict:
+    """The `config` object: identical in the `ours` and the `reference` arm (no measured quantity in it)."""
+    P = wl["grid"].num_points if wl["kind"] == "grid" else len(wl["batches"][0][0])
+    return {"workload": wl["desc"], "points_per_step": int(P), "gaussians": int(wl["g"].n),
+            "step": "preprocess+build_accel+fwd(MSE)+bwd",
+            "l2": "per-step working set (records, lists, per-sample arrays) exceeds the 126 MB L2 for C2-C5; no flush"}
+
+
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe), one sample per 20 ms."""
 
     def __init__(self, index: int):
         self.rows = []
@@ -75,7 +180,7 @@ class ClockSampler:
         q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100", "-i",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20", "-i",
                                           str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except OSError:
@@ -91,79 +196,298 @@ class ClockSampler:
         while self.proc and not self.rows and time.time() - t0 < timeout:
             time.sleep(0.02)
 
-    def stop(self, window=None):
-        """window = (t0, t1) host times of the timed region: only samples taken inside it count (all, if none fell inside)."""
+    def window(self, w0, w1):
+        """Clock record of the host-time window (w0, w1) of a timed region."""
         if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        allrows = [(t, r) for t, r in self.rows if len(r) >= 7]
-        rows = [r for t, r in allrows if window is None or window[0] <= t <= window[1] + 0.1]
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
+        rows = [r for t, r in self.rows if len(r) >= 7 and w0 <= t <= w1 + 0.05]
         if not rows:
-            rows = [r for _, r in allrows]
-        if not rows:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in the window"], "samples": 0}
         sm = sorted(float(r[0]) for r in rows)
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows)}
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows)}
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
 
 
-def oracle_step(wl, sample_note: list, cap_bricks: int = 12, cap_points: int = 1 << 15):
-    """One bounded-sample pass of the oracle (fwd + MSE + bwd).  Returns (points processed, hits)."""
+# ------------------------------------------------------------------------------------------------------------------
+# the oracle on a bounded sample of a workload (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_sample(wl):
+    """(xyz, target, note): the bounded sample of the workload the oracle is timed on (whole grid for C1/C2,
+    one 128^3 batch for C4, the first 2^17 / 2^20 points of a batch for C3 / C5; always against the whole model)."""
     from oracle import wveg_oracle as oracle
     g = wl["g"]
     if wl["kind"] == "grid":
         grid = wl["grid"]
-        nb = [min(c, cap_bricks) for c in grid.brick_cnt]  # a brick-aligned corner batch of the grid (12 -> 96^3)
-        sub = grid.batch((0, 0, 0), tuple(nb))
-        xyz = oracle.grid_points(sub)
-        bd = sub.batch_dims
-        full = np.asarray(wl["target"]).reshape(grid.batch_dims[2], grid.batch_dims[1], grid.batch_dims[0])
-        target = np.ascontiguousarray(full[:bd[2], :bd[1], :bd[0]]).ravel()
-        sample_note[:] = [f"{bd[0]}x{bd[1]}x{bd[2]} brick-aligned sub-grid, all {g.n} Gaussians, fwd+MSE+bwd"]
-    else:
-        n = min(len(wl["xyz"]), cap_points)
-        xyz, target = wl["xyz"][:n], wl["target"][:n]
-        sample_note[:] = [f"first {n} points of the batch, all {g.n} Gaussians, fwd+MSE+bwd"]
+        bd = grid.batch_dims
+        return oracle.grid_points(grid), wl["target"], f"the step's whole {bd[0]}x{bd[1]}x{bd[2]} batch, all {g.n} Gaussians, fwd+MSE+bwd"
+    n = {"c3": 1 << 17, "c5": 1 << 20}.get(wl["name"], 1 << 15)
+    xyz, t = wl["batches"][0]
+    n = min(n, len(xyz))
+    return xyz[:n], t[:n], f"first {n} points of a batch, all {g.n} Gaussians, fwd+MSE+bwd"
+
+
+def oracle_step(wl, xyz, target):
+    from oracle import wveg_oracle as oracle
+    g = wl["g"]
     fwd = oracle.forward(g, xyz, TAU, mode=1)
-    loss, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    _, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
     oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
-    return len(xyz), int(fwd["count"].astype(np.int64).sum())
+    return len(xyz)
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """The oracle, as it stands, on the box's host cores: every step is the cpu_baseline sample of the headline workload."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     from oracle import wveg_oracle as oracle
     oracle.build()
-    wl = make_workload(args.workload)
-    note = []
-    # the per-step sample shrinks with the number of steps so that the whole run ends within a few minutes
-    total = args.steps + args.warmup
-    cap_bricks, cap_points = (12, 1 << 15) if total <= 250 else (6, 1 << 12) if total <= 1000 else (4, 1 << 10)
-    for _ in range(args.warmup):
-        oracle_step(wl, note, cap_bricks, cap_points)
+    name = HEADLINE if args.workload == "all" else args.workload
+    wl = make_workload(name)
+    xyz, target, note = oracle_sample(wl)
+    for _ in range(min(args.warmup, 1)):   # the oracle has no caches to warm beyond the page cache: one pass at most
+        oracle_step(wl, xyz, target)
     t0 = time.perf_counter()
     pts = 0
     for _ in range(args.steps):
-        p, _h = oracle_step(wl, note, cap_bricks, cap_points)
-        pts += p
+        pts += oracle_step(wl, xyz, target)
     dt = time.perf_counter() - t0
     val = pts / dt
     line = {"impl": "reference", "metric": "query_points_per_s_fwd_bwd", "value": val, "unit": "points/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl["desc"], "sample": note[0]},
-            "cpu_baseline": {"value": val, "unit": "points/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": note[0]},
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_of(wl),
+            "cpu_baseline": {"value": val, "unit": "points/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": note},
             "e2e": {"value": val, "unit": "points/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------------------
+def measure(wl, args, sampler, world, rank, headline: bool):
+    """Times one workload: K steps (device-resident), the e2e leg through gs_step_host, decode legs where the config has
+    one.  Returns the workload's result dict."""
+    import torch
+    import torch.distributed as dist
+    from paper_2607_01164_b200 import api, dist as gsdist
+
+    g = wl["g"]
+    ctx = api.Context()
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    gd = [dev(a) for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    # ---- this rank's share of the samples (DESIGN.md section 10): same model everywhere, bricks / points are sharded
+    shards, P_total = shard_workload(wl, rank, world)
+    keep = [dev(s_["xyz"]) if wl["kind"] == "points" else None for s_ in shards]
+    queries = [api.grid_query(s_["grid"]) if wl["kind"] == "grid" else api.points_query(x) for s_, x in zip(shards, keep)]
+    tgt = [dev(s_["target"]) for s_ in shards]
+    P = api.query_num_points(queries[0]) if queries else 0
+    phi = torch.empty(max(P, 1), device="cuda")
+    I = torch.empty(max(P, 1), device="cuda")
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    grads = ctx.alloc_grads(g.n, flat=True)
+    if world > 1:
+        ctx.gs_set_sample_count(P_total)   # the loss mean runs over the samples of ALL ranks
+
+    it = [0]
+
+    def step():
+        k = it[0] % max(len(queries), 1)
+        it[0] += 1
+        loss.zero_()
+        ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
+        if queries:
+            q = queries[k]
+            ctx.gs_build_accel(q)
+            ctx.gs_sample_fwd(q, phi, I, target=tgt[k], loss=loss)  # fused MSE: keeps the backward coefficients
+            ctx.gs_sample_bwd(q, None, None, None, grads)           # dL_dphi = NULL: backward of that fused loss
+        else:
+            for v in grads.values():
+                v.zero_()
+        if world > 1:
+            gsdist.allreduce_grads(grads, loss)   # ONE collective on the flat gradient buffer (+ the loss scalar)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        step()
+    barrier()
+    # hit / tested pair counts of this workload (outside the timed region; first batch)
+    tested = hits = 0
+    if queries:
+        ctx.gs_build_accel(queries[0])
+        _, _, _, tested, hits = ctx.debug_point_sets(queries[0])
+    ctx.profile_read()
+    ctx.profile_enable(True)
+    for _ in range(2):
+        step()
+    barrier()
+    ctx.profile_read()
+    # K steps exactly for the headline; a secondary workload repeats until its timed region is long enough for clock samples
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); step(); e1.record(); barrier()
+    est_ms = max(e0.elapsed_time(e1), 1e-3)
+    steps = args.steps if headline else max(args.steps, int(math.ceil(1e3 * MIN_TIMED_S / est_ms)))
+    ctx.profile_read()
+    w0 = time.time()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    barrier()
+    w1 = time.time()
+    ms_total = e0.elapsed_time(e1)
+    stage_ms, stage_calls, launches = ctx.profile_read()
+    ctx.profile_enable(False)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / steps
+    out = {"config": config_of(wl), "steps": steps, "ms_per_step": ms_step, "value": P_total / (ms_step * 1e-3), "unit": "points/s",
+           "gpu_launches": launches, "clocks": sampler.window(w0, w1) if rank == 0 else None,
+           "hit_pairs": hits, "tested_pairs": tested, "cull_efficiency": hits / tested if tested else None}
+    per = {k: (stage_ms[k] / stage_calls[k] if stage_calls[k] else 0.0) for k in stage_ms}
+    out["stage_ms"] = per
+    # ---- roofline of the sampling kernels (this rank's share of the hits; ALU-bound, DESIGN.md section 7)
+    traffic, tsrc = load_traffic()
+    kpre = "k_grid_" if wl["kind"] == "grid" else "k_points_"
+    kernels = {}
+    for nm, instr in (("fwd", INSTR_FWD), ("bwd", INSTR_BWD)):
+        ms = per[nm]
+        ach = hits * instr / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        tr = traffic.get(f"{wl['name']}/{kpre}{nm}")
+        kernels[nm] = {"kernel": kpre + nm, "launch_ms": ms, "achieved": ach, "frac": ach / ALU_PEAK_TINSTR,
+                       "algorithmic_lane_instr": hits * instr, "traffic": tr["bytes"] if tr else None,
+                       "traffic_source": tr["source"] if tr else tsrc}
+    dom = "fwd" if per["fwd"] >= per["bwd"] else "bwd"
+    fb_ms = per["fwd"] + per["bwd_pack"] + per["bwd"]
+    out["roofline"] = {
+        "bound": "alu", "kernel": kernels[dom]["kernel"], "achieved": kernels[dom]["achieved"], "peak": ALU_PEAK_TINSTR,
+        "unit": "T FP32 lane-instr/s (algorithmic: hit pairs x 19 fwd / x 40 bwd)", "frac": kernels[dom]["frac"],
+        "traffic": kernels[dom]["traffic"], "traffic_unit": "bytes per launch (dram read + write, ncu --set full)",
+        "traffic_source": kernels[dom]["traffic_source"], "launch_ms": kernels[dom]["launch_ms"], "kernels": kernels,
+        "fwd_bwd_frac": (hits * (INSTR_FWD + INSTR_BWD) / (fb_ms * 1e-3) / 1e12 / ALU_PEAK_TINSTR) if fb_ms > 0 else None,
+        "step_frac": hits * (INSTR_FWD + INSTR_BWD) / (ms_step * 1e-3) / 1e12 / ALU_PEAK_TINSTR,
+        "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max SM clock)"}
+    out["rates"] = {"fwd_points_per_s": P / (per["fwd"] * 1e-3) if per["fwd"] else None,
+                    "fwd_gaussian_evals_per_s": hits / (per["fwd"] * 1e-3) if per["fwd"] else None,
+                    "fwd_bwd_gaussian_evals_per_s": hits / (ms_step * 1e-3)}
+
+    # ---- forward-only decode legs (configs[3]: 64 consecutive 128^3 batches; configs[4]: the 40M draw in 2^24 chunks)
+    if world == 1 and wl.get("decode_blocks"):
+        blocks = wl["decode_blocks"]
+        qs = [api.grid_query(wl["full"].batch(lo, (16, 16, 16))) for lo in blocks]
+        Pb = api.query_num_points(qs[0])
+        phis = torch.empty(len(qs) * Pb, device="cuda")   # every batch writes its own output: real HBM writes, not L2 hits
+        Is = torch.empty(len(qs) * Pb, device="cuda")
+        ctx.gs_preprocess(*gd, tau=TAU)
+
+        def decode():
+            for k, q in enumerate(qs):
+                ctx.gs_build_accel(q)
+                ctx.gs_sample_fwd(q, phis[k * Pb:(k + 1) * Pb], Is[k * Pb:(k + 1) * Pb])
+        decode(); barrier()
+        reps = max(1, int(math.ceil(1e3 * MIN_TIMED_S / (0.2 * len(qs)))))
+        ctx.profile_read(); ctx.profile_enable(True)
+        e0.record()
+        for _ in range(reps):
+            decode()
+        e1.record(); barrier()
+        sm, sc, _ = ctx.profile_read(); ctx.profile_enable(False)
+        ms_b = e0.elapsed_time(e1) / (reps * len(qs))
+        fwd_ms = sm["fwd"] / max(sc["fwd"], 1)
+        peaks = _peaks()
+        hbm = peaks.get("hbm_gbs")
+        out["decode"] = {"what": f"forward-only decode of {len(qs)} consecutive 128^3 batches (a 512^3 block), one gs_preprocess, "
+                                 "gs_build_accel + gs_sample_fwd per batch, each batch writing its own Phi/I",
+                         "batches": len(qs), "ms_per_batch": ms_b, "points_per_s": Pb / (ms_b * 1e-3),
+                         "build_ms": sm["build"] / max(sc["build"], 1), "fwd_ms": fwd_ms,
+                         "roofline": {"bound": "hbm", "kernel": "k_grid_fwd", "unit": "GB/s",
+                                      "achieved": Pb * 8 / (fwd_ms * 1e-3) / 1e9 if fwd_ms else None, "peak": hbm,
+                                      "frac": (Pb * 8 / (fwd_ms * 1e-3) / 1e9 / hbm) if (fwd_ms and hbm) else None,
+                                      "algorithmic_bytes": "8 B written per sample (Phi, I); records and lists are L2-resident",
+                                      "peak_source": "MEASURED_PEAKS.json hbm_gbs (burst copy)"}}
+        del phis, Is
+    if world == 1 and wl.get("decode_xyz") is not None:
+        allx = wl["decode_xyz"]
+        chunk = 1 << 24
+        xs = [dev(allx[a:a + chunk]) for a in range(0, len(allx), chunk)]
+        qs = [api.points_query(x) for x in xs]
+        pp = [torch.empty(len(x), device="cuda") for x in xs]
+        ii = [torch.empty(len(x), device="cuda") for x in xs]
+        ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
+
+        def decode():
+            for q, p_, i_ in zip(qs, pp, ii):
+                ctx.gs_build_accel(q)
+                ctx.gs_sample_fwd(q, p_, i_)
+        decode(); barrier()
+        ctx.profile_read(); ctx.profile_enable(True)
+        e0.record(); decode(); decode(); e1.record(); barrier()
+        sm, sc, _ = ctx.profile_read(); ctx.profile_enable(False)
+        ms_all = e0.elapsed_time(e1) / 2
+        out["decode"] = {"what": f"forward-only decode of the {len(allx)}-point draw in {len(qs)} chunks of <= 2^24 points, one "
+                                 "gs_preprocess, gs_build_accel (LBVH + query sort + cull lists) + gs_sample_fwd per chunk",
+                         "chunks": len(qs), "ms_total": ms_all, "points_per_s": len(allx) / (ms_all * 1e-3),
+                         "build_ms_per_chunk": sm["build"] / max(sc["build"], 1), "fwd_ms_per_chunk": sm["fwd"] / max(sc["fwd"], 1)}
+        del xs, qs, pp, ii
+
+    # ---- e2e through the HOST-buffer entry point (pinned memory, copies inside the timed region)
+    if world == 1:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        gh = dict(mean=pin(g.mean), scale=pin(g.scale), quat=pin(g.quat), opacity=pin(g.opacity), scalar=pin(g.scalar))
+        if wl["kind"] == "grid":
+            th, qh = pin(wl["target"]), api.grid_query(wl["grid"])
+        else:
+            th, qh = pin(wl["batches"][0][1]), api.points_query(pin(wl["batches"][0][0]))
+        # the host-visible result of a training step is the loss and the gradients; the per-sample Phi / I stay on the
+        # device (gs_step_host copies them back only when asked to)
+        gr_h = dict(dmean=pin(np.empty((g.n, 3), np.float32)), dscale=pin(np.empty((g.n, 3), np.float32)),
+                    dquat=pin(np.empty((g.n, 4), np.float32)), dopacity=pin(np.empty(g.n, np.float32)),
+                    dscalar=pin(np.empty(g.n, np.float32)), err=pin(np.empty(g.n, np.float32)))
+        h2d = g.n * 48 + P_total * 4 + (P_total * 12 if wl["kind"] == "points" else 0)
+        d2h = 8 + g.n * 52
+        for _ in range(2):
+            ctx.gs_step_host(gh, qh, th, None, None, gr_h, domain=wl["domain"], tau=TAU)
+        barrier()
+        e2e_steps = max(2, min(args.steps, 10))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            ctx.gs_step_host(gh, qh, th, None, None, gr_h, domain=wl["domain"], tau=TAU)
+        barrier()
+        e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+        out["e2e"] = {"value": P_total / (e2e_ms * 1e-3), "unit": "points/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                      "ms_per_step": e2e_ms, "steps": e2e_steps,
+                      "api": "gs_step_host (pinned host buffers): H2D model + target (+ points), D2H loss + 6 gradient tensors"}
+    if headline and rank == 0:
+        ffma_peak, ex2_peak, ffma2_peak = ctx.measure_alu_peaks()  # measured ALU denominators at the clocks of this run
+        out["roofline"]["peak_measured"] = {"ffma_tinstr_s": ffma_peak / 1e12, "ffma2_tlaneop_s": ffma2_peak / 1e12,
+                                            "mufu_ex2_tinstr_s": ex2_peak / 1e12,
+                                            "how": "gs_measure_alu_peaks: register-only FMA / packed FMA / EX2 loops, CUDA events, this run"}
+        out["roofline"]["frac_of_measured"] = out["roofline"]["achieved"] / (ffma_peak / 1e12) if ffma_peak else None
+    ctx.close()
+    del gd, phi, I, grads
+    torch.cuda.empty_cache()
+    return out
+
+
+def _peaks() -> dict:
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        return {}
 
 
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2607_01164_b200 import api
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -177,176 +501,44 @@ def run_ours(args):
             time.sleep(0.5)
     torch.cuda.set_device(local)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # a scaling run prints its communicator / transport lines
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    wl = make_workload(args.workload, rank)
-    g = wl["g"]
-    ctx = api.Context()
-    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    gd = [dev(a) for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
-    if wl["kind"] == "grid":
-        q = api.grid_query(wl["grid"])
-    else:
-        xyz_d = dev(wl["xyz"])
-        q = api.points_query(xyz_d)
-    P = api.query_num_points(q)
-    target = dev(wl["target"])
-    phi = torch.empty(P, device="cuda")
-    I = torch.empty(P, device="cuda")
-    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
-    grads = ctx.alloc_grads(g.n)
-    flat = None
-    if world > 1:  # data-parallel exchange: one all-reduce of the gradients
-        flat = torch.empty(g.n * 16, device="cuda")
-
-    recipe = args.step == "recipe"
-    cur_q = [q]  # the query the acceleration structure was last built for
-    if recipe:  # the paper's training step: raw parameters, jitter, L1 + Eq. 4, Adam
-        assert wl["kind"] == "grid", "--step recipe needs a grid workload"
-        logit = lambda x: np.log(x / (1 - x))
-        raw = dict(mean=gd[0], raw_scale=dev(np.log(g.scale)), quat=gd[2],
-                   raw_opacity=dev(logit(np.clip(g.opacity.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)),
-                   raw_scalar=dev(logit(np.clip(g.scalar.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)))
-        m_d, v_d = torch.zeros(12 * g.n, device="cuda"), torch.zeros(12 * g.n, device="cuda")
-        terms = torch.zeros(3, dtype=torch.float64, device="cuda")
-        it = [0]
-
-    def step():
-        if recipe:
-            it[0] += 1
-            qj = api.grid_query(wl["grid"], jitter_seed=it[0])   # a new random position in every cell
-            ctx.gs_preprocess(raw["mean"], gd[1], raw["quat"], gd[3], gd[4], tau=TAU)
-            ctx.gs_build_accel(qj)
-            cur_q[0] = qj
-            ctx.gs_sample_fwd_loss(qj, phi, I, target, kind=api.LOSS_L1, lambda_fn=0.5, eps_fn=0.5, loss_terms=terms)
-            ctx.gs_sample_bwd(qj, None, None, None, grads)
-            ctx.gs_adam_step(raw, grads, m_d, v_d, it[0], scale_out=gd[1], opacity_out=gd[3], scalar_out=gd[4])
-            return
-        loss.zero_()
-        ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
-        ctx.gs_build_accel(q)
-        ctx.gs_sample_fwd(q, phi, I, target=target, loss=loss)  # fused MSE: keeps the backward coefficients
-        ctx.gs_sample_bwd(q, None, None, None, grads)           # dL_dphi = NULL: backward of that fused loss
-        if world > 1:
-            from paper_2607_01164_b200 import dist as gsdist
-            gsdist.allreduce_grads(grads, flat)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    # hit / tested pair counts of this workload (outside the timed region)
-    _, _, _, tested, hits = ctx.debug_point_sets(cur_q[0])
-    ffma_peak, ex2_peak = ctx.measure_alu_peaks()  # measured ALU denominators at the clocks of this run
-    ctx.profile_read()
-    ctx.profile_enable(True)
+    names = ["c2", "c3", "c4", HEADLINE] if args.workload == "all" else [args.workload]
+    head = names[-1]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         sampler.wait_first()
-    for _ in range(3):
-        step()
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    w0 = time.time()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    w1 = time.time()
-    ms_total = e0.elapsed_time(e1)
-    clocks = sampler.stop((w0, w1)) if rank == 0 else None
-    stage_ms, stage_calls, launches = ctx.profile_read()
-    ctx.profile_enable(False)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * P / (ms_step * 1e-3)
-
-    # ---- e2e through the HOST-buffer entry point (pinned memory, copies inside the timed region)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
-    gh = dict(mean=pin(g.mean), scale=pin(g.scale), quat=pin(g.quat), opacity=pin(g.opacity), scalar=pin(g.scalar))
-    th = pin(wl["target"])
-    qh = api.grid_query(wl["grid"]) if wl["kind"] == "grid" else api.points_query(pin(wl["xyz"]))
-    # the host-visible result of a training step is the loss and the gradients; the per-sample Phi / I stay on the device
-    # (gs_step_host copies them back only when asked to)
-    phi_h, I_h = None, None
-    gr_h = dict(dmean=pin(np.empty((g.n, 3), np.float32)), dscale=pin(np.empty((g.n, 3), np.float32)),
-                dquat=pin(np.empty((g.n, 4), np.float32)), dopacity=pin(np.empty(g.n, np.float32)),
-                dscalar=pin(np.empty(g.n, np.float32)), err=pin(np.empty(g.n, np.float32)))
-    h2d = g.n * 48 + P * 4 + (P * 12 if wl["kind"] == "points" else 0)
-    d2h = 8 + g.n * 52
-    e2e_steps = max(2, min(args.steps, 10))
-    for _ in range(2):
-        ctx.gs_step_host(gh, qh, th, phi_h, I_h, gr_h, domain=wl["domain"], tau=TAU)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        ctx.gs_step_host(gh, qh, th, phi_h, I_h, gr_h, domain=wl["domain"], tau=TAU)
-    barrier()
-    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    te = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * P / (float(te.item()) * 1e-3)
-
-    if rank == 0:
-        per = {k: (stage_ms[k] / stage_calls[k] if stage_calls[k] else 0.0) for k in stage_ms}
-        dom_name, dom_ms, instr = ("fwd", per["fwd"], INSTR_FWD) if per["fwd"] >= per["bwd"] else ("bwd", per["bwd"], INSTR_BWD)
-        achieved = hits * instr / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
-        fb_ms = per["fwd"] + per["bwd_pack"] + per["bwd"] + per["finalize"]
-        roof_fb = hits * (INSTR_FWD + INSTR_BWD) / (fb_ms * 1e-3) / 1e12 if fb_ms > 0 else 0.0
-        peaks = {}
-        try:
-            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        except OSError:
-            pass
-        kernel = ("k_grid_" if wl["kind"] == "grid" else "k_points_") + dom_name
-        traffic, traffic_src = NCU_TRAFFIC.get((args.workload, kernel), (None, None))
-        line = {
-            "metric": "query_points_per_s_fwd_bwd", "value": value, "unit": "points/s", "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": wl["desc"], "points_per_step": P, "gaussians": g.n, "hit_pairs": hits, "tested_pairs": tested,
-                       "l2": "working set per step (>600 MB of per-sample arrays) exceeds the 126 MB L2; no flush",
-                       "step": "preprocess+build_accel+fwd(L1+FN, jittered samples)+bwd+adam" if recipe else "preprocess+build_accel+fwd(MSE)+bwd"},
-            "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": e2e_value, "unit": "points/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": float(te.item()),
-                    "api": "gs_step_host (pinned host buffers): H2D model + target (+ points), D2H loss + 6 gradient tensors"},
-            "stage_ms": per,
-            "extra": {"fwd_points_per_s": P / (per["fwd"] * 1e-3) if per["fwd"] else None,
-                      "fwd_gaussian_evals_per_s": hits / (per["fwd"] * 1e-3) if per["fwd"] else None,
-                      "fwd_bwd_gaussian_evals_per_s": hits / (fb_ms * 1e-3) if fb_ms else None,
-                      "fwd_bwd_kernels_roofline_frac": roof_fb / ALU_PEAK_TINSTR,
-                      "cull_efficiency": hits / tested if tested else None,
-                      "hbm_peak_gbs_measured": peaks.get("hbm_gbs")},
-            "roofline": {"bound": "alu", "kernel": kernel,
-                         "achieved": achieved, "peak": ALU_PEAK_TINSTR, "unit": "T FP32 lane-instr/s (algorithmic: hit pairs x "
-                         f"{instr:.0f} instr)", "frac": achieved / ALU_PEAK_TINSTR, "traffic": traffic,
-                         "traffic_unit": "bytes per launch (dram read + write, ncu --set full)", "traffic_source": traffic_src,
-                         "launch_ms": dom_ms,
-                         "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max SM clock)",
-                         "peak_measured": {"ffma_tinstr_s": ffma_peak / 1e12, "mufu_ex2_tinstr_s": ex2_peak / 1e12,
-                                           "how": "gs_measure_alu_peaks: register-only FMA / EX2 loops, CUDA events, this run"},
-                         "frac_of_measured": achieved / (ffma_peak / 1e12) if ffma_peak else None},
-        }
-        if not args.no_cpu and world == 1:
+    results = {}
+    for nm in names:
+        wl = make_workload(nm)
+        results[nm] = measure(wl, args, sampler, world, rank, headline=(nm == head))
+        if nm == head and rank == 0 and not args.no_cpu and world == 1:
             from oracle import wveg_oracle as oracle
             oracle.build()
-            note = []
+            xyz, target, note = oracle_sample(wl)
             t0 = time.perf_counter()
-            pts, _h = oracle_step(wl, note, cap_bricks=32, cap_points=1 << 17)  # C2: the whole 256^3 grid (~10-20 s)
+            pts = oracle_step(wl, xyz, target)
             dt = time.perf_counter() - t0
-            line["cpu_baseline"] = {"value": pts / dt, "unit": "points/s", "cores": oracle.num_threads(), "kind": "oracle",
-                                    "sample": note[0], "seconds": dt}
+            results[nm]["cpu_baseline"] = {"value": pts / dt, "unit": "points/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                           "sample": note, "seconds": dt}
+        del wl
+    sampler.stop()
+    if rank == 0:
+        r = results[head]
+        line = {"metric": "query_points_per_s_fwd_bwd", "value": r["value"], "unit": "points/s", "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                "scaling": "strong" if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": r["config"], "clocks": r["clocks"], "gpu_launches": r["gpu_launches"], "e2e": r.get("e2e"),
+                "stage_ms": r["stage_ms"], "roofline": r["roofline"], "csrc_sha16": csrc_sha16(),
+                "extra": {"hit_pairs": r["hit_pairs"], "tested_pairs": r["tested_pairs"], "cull_efficiency": r["cull_efficiency"],
+                          "rates": r["rates"], "decode": r.get("decode"), "hbm_peak_gbs_measured": _peaks().get("hbm_gbs")}}
+        if "cpu_baseline" in r:
+            line["cpu_baseline"] = r["cpu_baseline"]
+        if len(names) > 1:
+            line["workloads"] = {k: v for k, v in results.items() if k != head}
         print(json.dumps(line))
-    ctx.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -354,15 +546,17 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--step", default="mse", choices=["mse", "recipe"],
-                    help="mse: the north_star step (default); recipe: the paper's training step (jitter, L1 + Eq. 4, Adam)")
+    ap.add_argument("--record-traffic", nargs=3, metavar=("NCU_RAW_CSV", "WORKLOAD", "SOURCE"),
+                    help="store dram bytes per launch of an `ncu --page raw --csv` export in profiles/traffic.json")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.record_traffic:
+        record_traffic(*args.record_traffic)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -31,6 +31,11 @@
  *     batch) without repeating gs_preprocess as long as the Gaussians are unchanged.
  *   - Layouts are dense, row-major, fp32: mean[N,3], scale[N,3], quat[N,4] in (w,x,y,z) order,
  *     opacity[N], scalar[N]; per-sample arrays are [P].
+ *   - Alignment: every array must be aligned to its element type (4 bytes; 8 for double / uint64 arrays);
+ *     gs_grads.dquat must be 16-byte aligned (INVALID_ARG otherwise).  The per-sample arrays of gs_sample_fwd
+ *     (target, phi, I, dL_dphi, sample_err) MAY be only 4-byte aligned (a view such as tensor[1:]): the kernels
+ *     move grid samples in 8-byte x-pairs only when all of them are 8-byte aligned and fall back to scalar
+ *     accesses otherwise -- same results, never a misaligned-address fault.
  */
 #ifndef GS_H_
 #define GS_H_
@@ -105,8 +110,9 @@ typedef struct {
 
 /* Gradient outputs, OVERWRITTEN (not accumulated): dL/dmean[N,3], dL/dscale[N,3], dL/dquat[N,4],
  * dL/dopacity[N], dL/dscalar[N] and the per-Gaussian sampling-error statistic err[N] (nullable;
- * DESIGN D10 -- E_i = sum over covered samples of |Phi_c - t_c| w_i G_ic / I_c; NOT from the paper,
- * which densifies from per-sample errors). */
+ * DESIGN D10 -- E_i = sum over covered samples of |Phi_c - t_c| w_i G_ic / I_c).  E_i is a north_star
+ * quantity: the PAPER DEFINES NO per-Gaussian error (it densifies from per-sample errors, which
+ * gs_sample_fwd returns as sample_err), so its definition is this library's reading, not a result of the paper. */
 typedef struct {
     float *dmean, *dscale, *dquat, *dopacity, *dscalar, *err;
 } gs_grads;
@@ -150,6 +156,12 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
  * q must be the query the accel was built for.  Errors: STATE, INVALID_ARG, OVERFLOW, CUDA. */
 gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss,
                         float *dL_dphi, float *sample_err);
+
+/* Sample-sharded (multi-GPU) use: the number of samples the fused MSE mean of gs_sample_fwd runs over (loss,
+ * dL_dphi = 2 res / total, and the error statistic of the fused backward).  0 (the default) = the query's own P.
+ * A rank that holds 1/R of the samples sets the global count, so that the per-rank losses and gradients ADD UP
+ * to the one-batch ones.  Errors: INVALID_ARG (null context). */
+gs_status gs_set_sample_count(gs_ctx *ctx, uint64_t total_samples);
 
 /* The same forward with the paper's training losses fused into the epilogue.
  * `defined` (device, uint8 [P], nullable = every sample) marks the samples that lie in the volume's
@@ -301,6 +313,19 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
                      const float *sample_err, const float *I, const uint8_t *defined, uint64_t num_defined, const float *target,
                      uint32_t k, float raw_scale_init, float raw_opacity_init, uint32_t *n_new_host);
 
+/* Status of the context's current model / accel.  Gaussians with a non-finite parameter, a non-positive scale
+ * or a zero quaternion are not an error: they have empty support (see gs_gaussians) and are COUNTED by
+ * gs_preprocess; this call surfaces the count.  HOST output; synchronises the stream.
+ * Errors: INVALID_ARG, CUDA. */
+typedef struct gs_status_info {
+    uint64_t num_gaussians;       /* N of the last gs_preprocess (0 before it)                           */
+    uint64_t invalid_gaussians;   /* of those, how many have empty support because a parameter is invalid */
+    uint64_t grid_pairs;          /* grid accel: T = (brick, gaussian) pairs of the current batch          */
+    uint64_t grid_touched;        /* grid accel: Gaussians that overlap a brick of the current batch       */
+    uint64_t cull_chunk_capacity; /* point accel: 32-entry list chunks the pool holds                      */
+} gs_status_info;
+gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host);
+
 /* ---- measurement: CUDA-event timing of the stages, on the context's stream --------------------
  * While enabled, every stage of the calls above is bracketed by a pair of CUDA events recorded on
  * the context's stream.  gs_profile_read synchronises the stream, adds up the elapsed time of all
@@ -325,9 +350,10 @@ gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uin
 /* Measured denominators of the plain-ALU roofline the sampling kernels are held against (the path is
  * bound by FP32 issue, not by a dense contraction; north_star: "FP32/SFU issue utilisation against the
  * chip's peak"): FP32 FMA lane-instructions per second and MUFU.EX2 per second of this device at its
- * current clocks, from two register-only loops timed with CUDA events on the context's stream.
+ * current clocks, from register-only loops timed with CUDA events on the context's stream; ffma2 (nullable) =
+ * FMA lane-OPERATIONS per second through the packed fma.rn.f32x2 form (two per lane-instruction).
  * HOST outputs; synchronises.  Errors: INVALID_ARG, OOM, CUDA. */
-gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host);
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host);
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -67,6 +67,11 @@ class _Loss(C.Structure):
 class _RawParams(C.Structure):
     _fields_ = [("n", C.c_uint32), ("mean", C.c_void_p), ("raw_scale", C.c_void_p), ("quat", C.c_void_p),
                 ("raw_opacity", C.c_void_p), ("raw_scalar", C.c_void_p)]
+
+
+class _StatusInfo(C.Structure):
+    _fields_ = [("num_gaussians", C.c_uint64), ("invalid_gaussians", C.c_uint64), ("grid_pairs", C.c_uint64),
+                ("grid_touched", C.c_uint64), ("cull_chunk_capacity", C.c_uint64)]
 
 
 class _AdamCfg(C.Structure):
@@ -113,7 +118,9 @@ def load_library():
     lib.gs_prune.argtypes = [P, C.POINTER(_RawParams), P, P, P, C.c_float, C.POINTER(C.c_uint32)]
     lib.gs_densify.argtypes = [P, C.POINTER(_RawParams), P, P, C.c_uint32, C.POINTER(_Query), P, P, P, C.c_uint64, P, C.c_uint32,
                                C.c_float, C.c_float, C.POINTER(C.c_uint32)]
-    lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.gs_set_sample_count.argtypes = [P, C.c_uint64]
+    lib.gs_status_query.argtypes = [P, C.POINTER(_StatusInfo)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
     for name in EXPORTS:
@@ -303,10 +310,19 @@ class Context:
         return int(out.value)
 
     def measure_alu_peaks(self):
-        """(FP32 FMA lane-instructions per second, MUFU.EX2 per second) of this device now; synchronises."""
-        a, b = C.c_double(), C.c_double()
-        self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b)))
-        return float(a.value), float(b.value)
+        """(FP32 FMA lane-instructions per second, MUFU.EX2 per second, FMA lane-operations per second through the packed
+        f32x2 form) of this device now; synchronises."""
+        a, b, c = C.c_double(), C.c_double(), C.c_double()
+        self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b), C.byref(c)))
+        return float(a.value), float(b.value), float(c.value)
+
+    def gs_set_sample_count(self, total_samples: int):
+        self._check(self.lib.gs_set_sample_count(self.h, C.c_uint64(int(total_samples))))
+
+    def gs_status_query(self) -> dict:
+        info = _StatusInfo()
+        self._check(self.lib.gs_status_query(self.h, C.byref(info)))
+        return {k: int(getattr(info, k)) for k, _ in _StatusInfo._fields_}
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.gs_profile_enable(self.h, int(on)))
@@ -321,9 +337,18 @@ class Context:
                 int(launches.value))
 
     # ---- helpers -----------------------------------------------------------------------------
-    def alloc_grads(self, n: int, with_err: bool = True) -> dict:
+    def alloc_grads(self, n: int, with_err: bool = True, flat: bool = False) -> dict:
+        """Gradient tensors of n Gaussians.  flat=True: views into ONE contiguous float32 buffer (key "flat"; every section
+        starts on a 16-byte boundary), which dist.allreduce_grads sums over the ranks in place with a single collective."""
         t = self._torch
         dev = t.device("cuda", self.device)
+        if flat:
+            from .dist import flat_layout
+            off, total = flat_layout(n)
+            buf = t.zeros(total, dtype=t.float32, device=dev)
+            out = {k: buf[o:o + n * c].view((n, c) if c > 1 else (n,)) for k, (o, c) in off.items()}
+            out["flat"] = buf
+            return out
         out = dict(dmean=t.empty((n, 3), dtype=t.float32, device=dev), dscale=t.empty((n, 3), dtype=t.float32, device=dev),
                    dquat=t.empty((n, 4), dtype=t.float32, device=dev), dopacity=t.empty(n, dtype=t.float32, device=dev),
                    dscalar=t.empty(n, dtype=t.float32, device=dev))

@@ -126,7 +126,7 @@ __device__ __forceinline__ uint32_t order_key(const BrickRange &br, const GridDe
 // inside the batch, the whitened-space cull threshold of a cell and 1 / |e|^2 for the closed-form row
 // intervals (sample_grid_bwd.cu):
 //   setup[2 i]     = (clo.x, clo.y, clo.z, flags: 1 = touches no voxel of the batch, 2 = a cell sticks out of the batch)
-//   setup[2 i + 1] = (ncx | ncy << 11 | ncz << 22, thr, invA, -)
+//   setup[2 i + 1] = ((ncx - 1) | (ncy - 1) << 10 | (ncz - 1) << 20, thr, invA, -)   (a batch spans <= 2048 voxels = 1024 cells per axis)
 __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, const float4 *__restrict__ rec, uint32_t N,
                                                       GridDesc gd, float rcut, uint32_t *__restrict__ count,
                                                       unsigned long long *__restrict__ total, uint32_t *__restrict__ hist,
@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
         const float e0 = gb.x * sx2, e1 = gc.x * sx2, e2 = gd4.x * sx2;
         setup[2 * (size_t)i] = make_float4(__int_as_float(clo[0]), __int_as_float(clo[1]), __int_as_float(clo[2]),
                                            __uint_as_float((empty ? 1u : 0u) | (edge ? 2u : 0u)));
-        setup[2 * (size_t)i + 1] = make_float4(__uint_as_float((uint32_t)nc[0] | ((uint32_t)nc[1] << 11) | ((uint32_t)nc[2] << 22)),
+        setup[2 * (size_t)i + 1] = make_float4(__uint_as_float((uint32_t)(nc[0] - 1) | ((uint32_t)(nc[1] - 1) << 10) | ((uint32_t)(nc[2] - 1) << 20)),
                                                reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
       }
     }

@@ -10,10 +10,17 @@
 using namespace gs;
 
 namespace gs {
-unsigned long long g_launches = 0;
+thread_local unsigned long long *tl_launches = nullptr;
 }
 
 namespace {
+
+// binds the calling thread's launch counter to the context for the duration of one C-ABI call (nests)
+struct LaunchScope {
+    unsigned long long *prev;
+    explicit LaunchScope(gs_ctx *c) : prev(gs::tl_launches) { if (c) gs::tl_launches = &c->launches; }
+    ~LaunchScope() { gs::tl_launches = prev; }
+};
 
 // RAII bracket: two CUDA events around a stage on the context's stream while profiling is enabled
 struct Stage {
@@ -129,7 +136,7 @@ gs_status gs_create(int device, void *cuda_stream, gs_ctx **out) {
     if (!ctx) return GS_ERR_OOM;
     ctx->device = device;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
-    if (ctx->counters.reserve(128) != cudaSuccess) { delete ctx; cudaGetLastError(); return GS_ERR_OOM; }
+    if (ctx->counters.reserve(128) != cudaSuccess || cudaMemset(ctx->counters.p, 0, 128) != cudaSuccess) { delete ctx; cudaGetLastError(); return GS_ERR_OOM; }
     *out = ctx;
     return GS_OK;
 }
@@ -155,6 +162,7 @@ void gs_destroy(gs_ctx *ctx) {
 const char *gs_last_error(const gs_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom, float tau) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     if (!g) return fail(ctx, GS_ERR_INVALID_ARG, "gaussians is NULL");
     if (g->n > 0 && (!g->mean || !g->scale || !g->quat || !g->opacity || !g->scalar))
@@ -182,13 +190,15 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     if (dom) ctx->dom = *dom;
     {
         Stage stage(ctx, GS_PROF_PREPROCESS);
-        CK(launch_preprocess(*g, ctx->r, ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->params.as<float>(), ctx->stream), "preprocess");
+        CK(launch_preprocess(*g, ctx->r, ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->params.as<float>(),
+                             ctx->counters.as<unsigned long long>() + 6, ctx->stream), "preprocess");
     }
     ctx->have_pre = true;
     return GS_OK;
 }
 
 gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "gs_build_accel before gs_preprocess");
     GridDesc gd{};
@@ -350,6 +360,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
 
 gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss, float *dL_dphi,
                         float *sample_err) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_sample_fwd before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -357,6 +368,10 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
     if (ctx->P > 0 && !target && (loss || dL_dphi || sample_err)) return fail(ctx, GS_ERR_INVALID_ARG, "loss outputs need a target");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     FwdOut o{target, phi, I, loss, dL_dphi, sample_err, nullptr, nullptr, nullptr, nullptr, nullptr};
+    o.inv_count = ctx->sample_count ? 1.0 / (double)ctx->sample_count : 0.0;
+    // x-pairs of a grid batch are moved as float2 only when every per-sample array the caller passed is 8-byte aligned
+    // (a 4-byte-aligned view such as tensor[1:] takes the scalar epilogue: same values)
+    o.vec_ok = !(((uintptr_t)target | (uintptr_t)phi | (uintptr_t)I | (uintptr_t)dL_dphi | (uintptr_t)sample_err) & 7);
     ctx->fused_pack = 0;
     if (target && ctx->P > 0) {  // keep the backward coefficients of the fused MSE for gs_sample_bwd(dL_dphi = NULL)
         CK(ctx->misc.reserve(ctx->P * 16), "alloc sample pack");
@@ -369,6 +384,7 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
 
 gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss, const float *target, float *phi, float *I,
                              double *loss_terms, float *dL_dphi, float *dL_dI, float *sample_err) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_sample_fwd_loss before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -414,6 +430,7 @@ gs_status gs_sample_fwd_loss(gs_ctx *ctx, const gs_query *q, const gs_loss *loss
 
 gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const float *I, const float *dL_dphi, const float *dL_dI,
                         const float *target, const gs_grads *out) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_sample_bwd before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -430,7 +447,8 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     if (N == 0) return GS_OK;
     CK(ctx->gacc.reserve((size_t)N * GACC_GRID * 4), "alloc gradient accumulator");
     const bool fused2 = fused && ctx->fused_pack == 1;  // float2 coefficients of the fused MSE; otherwise float4 coefficients
-    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused2 ? ctx->misc.as<float2>() : nullptr, 0.5f * (float)ctx->P};
+    BwdIn in{phi, I, dL_dphi, dL_dI, target, fused2 ? ctx->misc.as<float2>() : nullptr,
+             0.5f * (float)(ctx->sample_count ? ctx->sample_count : ctx->P)};
     if (ctx->accel_kind == GS_QUERY_GRID) {
         if (!fused) {
             ctx->fused_pack = 0;  // misc is overwritten with the caller's coefficients
@@ -456,6 +474,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
 }
 
 gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *count) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !dev_ptr || !count) return GS_ERR_INVALID_ARG;
     if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "nothing built yet");
     const size_t N = ctx->N;
@@ -506,6 +525,7 @@ gs_status gs_debug_read(gs_ctx *ctx, int32_t what, void *dst_host, size_t bytes)
 }
 
 gs_status gs_debug_point_sets(gs_ctx *ctx, const gs_query *q, uint32_t *count, uint64_t *hash_sum, uint64_t *hash_xor) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_debug_point_sets before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -535,6 +555,7 @@ gs_status gs_debug_counters(gs_ctx *ctx, uint64_t *tested_host, uint64_t *hits_h
 }
 
 gs_status gs_params_activate(gs_ctx *ctx, const gs_raw_params *p, float *scale, float *opacity, float *scalar) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !p) return GS_ERR_INVALID_ARG;
     if (p->n > 0 && (!p->raw_scale || !p->raw_opacity || !p->raw_scalar || !scale || !opacity || !scalar))
         return fail(ctx, GS_ERR_INVALID_ARG, "gs_params_activate: null pointer");
@@ -545,6 +566,7 @@ gs_status gs_params_activate(gs_ctx *ctx, const gs_raw_params *p, float *scale, 
 
 gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, float *m, float *v, const gs_adam_cfg *cfg,
                        float *scale_out, float *opacity_out, float *scalar_out) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !p || !g || !cfg) return GS_ERR_INVALID_ARG;
     if (p->n > 0 && (!p->mean || !p->raw_scale || !p->quat || !p->raw_opacity || !p->raw_scalar || !g->dmean || !g->dscale ||
                      !g->dquat || !g->dopacity || !g->dscalar || !m || !v))
@@ -559,6 +581,7 @@ gs_status gs_adam_step(gs_ctx *ctx, const gs_raw_params *p, const gs_grads *g, f
 }
 
 gs_status gs_prune(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, const float *opacity, float tau2, uint32_t *n_new_host) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !p || !n_new_host) return GS_ERR_INVALID_ARG;
     const uint32_t n = p->n;
     if (n > 0 && (!p->mean || !p->raw_scale || !p->quat || !p->raw_opacity || !p->raw_scalar || !m || !v || !opacity))
@@ -583,6 +606,7 @@ gs_status gs_prune(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, cons
 gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, uint32_t capacity, const gs_query *q,
                      const float *sample_err, const float *I, const uint8_t *defined, uint64_t num_defined, const float *target,
                      uint32_t k, float raw_scale_init, float raw_opacity_init, uint32_t *n_new_host) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !p || !n_new_host) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_densify before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -621,11 +645,33 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
     return GS_OK;
 }
 
-gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host) {
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host) {
+    LaunchScope launch_scope(ctx);
     if (!ctx || !ffma_per_s_host || !ex2_per_s_host) return GS_ERR_INVALID_ARG;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     CK(ctx->dbg.reserve(64), "alloc scratch");
-    CK(measure_alu_peaks(ctx->dbg.as<float>(), ctx->stream, ffma_per_s_host, ex2_per_s_host), "alu peaks");
+    CK(measure_alu_peaks(ctx->dbg.as<float>(), ctx->stream, ffma_per_s_host, ex2_per_s_host, ffma2_per_s_host), "alu peaks");
+    return GS_OK;
+}
+
+gs_status gs_set_sample_count(gs_ctx *ctx, uint64_t total_samples) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    ctx->sample_count = total_samples;
+    ctx->fused_pack = 0;
+    return GS_OK;
+}
+
+gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host) {
+    if (!ctx || !out_host) return GS_ERR_INVALID_ARG;
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    unsigned long long inv = 0;
+    CK(cudaMemcpy(&inv, ctx->counters.as<unsigned long long>() + 6, 8, cudaMemcpyDeviceToHost), "read counters");
+    memset(out_host, 0, sizeof *out_host);
+    out_host->num_gaussians = ctx->have_pre ? ctx->N : 0;
+    out_host->invalid_gaussians = ctx->have_pre ? inv : 0;
+    if (ctx->accel_kind == GS_QUERY_GRID) { out_host->grid_pairs = ctx->T; out_host->grid_touched = ctx->M; }
+    if (ctx->accel_kind == GS_QUERY_POINTS) out_host->cull_chunk_capacity = ctx->cull_cap;
     return GS_OK;
 }
 
@@ -653,13 +699,14 @@ gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uin
         if (ms_host) ms_host[k] = ms[k];
         if (calls_host) calls_host[k] = calls[k];
     }
-    if (launches_host) *launches_host = g_launches;
-    g_launches = 0;
+    if (launches_host) *launches_host = ctx->launches;
+    ctx->launches = 0;
     return GS_OK;
 }
 
 gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom, float tau, const gs_query *qh,
                        const float *target_host, float *phi_host, float *I_host, double *loss_host, const gs_grads *grads_host) {
+    LaunchScope launch_scope(ctx);
     if (!ctx) return GS_ERR_INVALID_ARG;
     if (!gh || !qh || !target_host || !loss_host) return fail(ctx, GS_ERR_INVALID_ARG, "gs_step_host: NULL argument");
     GridDesc gd{};

@@ -128,21 +128,25 @@ struct gs_ctx {
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr;
+    uint64_t sample_count = 0;  // gs_set_sample_count: samples the fused loss mean runs over (0 = the query's own P)
     // ---- measurement (gs_profile_*)
+    unsigned long long launches = 0;  // kernels launched for this context since the last gs_profile_read
     bool prof = false;
     struct ProfPair { cudaEvent_t a, b; int stage; };
     std::vector<ProfPair> prof_pending, prof_free;
 };
 
 namespace gs {
-extern unsigned long long g_launches;  // kernels launched by this library (host-side count)
-inline void count_launch(int n = 1) { g_launches += (unsigned long long)n; }
+// kernels launched by this library, counted per context: every C-ABI entry point binds the calling thread to its
+// context's counter (LaunchScope in gs_api.cu); the launchers below bump it through this thread-local pointer
+extern thread_local unsigned long long *tl_launches;
+inline void count_launch(int n = 1) { if (tl_launches) *tl_launches += (unsigned long long)n; }
 }  // namespace gs
 
 namespace gs {
 
 // ---- launchers (each enqueues on `s`, returns the launch error) ---------------------------------
-cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, cudaStream_t s);
+cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, unsigned long long *invalid, cudaStream_t s);
 
 // exclusive prefix sum of n uint32 (out may alias in); out[n] = total is written too (out has n+1 slots)
 cudaError_t exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, DevBuf &tmp, cudaStream_t s);
@@ -167,6 +171,8 @@ struct FwdOut {
     unsigned long long *counters;                                                   // [2] tested, hits (nullable)
     float2 *pack2;  // nullable: per-sample backward coefficients (alpha, beta) of the fused MSE loss; eps = |alpha| P / 2
     GenLoss gen;    // gen.on: the epilogue of gs_sample_fwd_loss (loss.cuh) instead of the fused MSE
+    double inv_count;  // 1 / (samples of the MSE mean); 0 = 1 / (this query's P)  (gs_set_sample_count: sample-sharded ranks)
+    int vec_ok;        // the caller's per-sample arrays are all 8-byte aligned: x-pairs may be moved as float2
 };
 struct BwdIn {
     const float *phi; const float *I; const float *dL_dphi; const float *dL_dI; const float *target;
@@ -208,7 +214,7 @@ cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uin
                                  float *scratch, cudaStream_t s);
 
 // peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)
-cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s);
+cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s, double *ffma2_per_s);
 
 // LBVH
 cudaError_t launch_morton(const float *xyz, size_t stride_floats, const float *aabb_valid /*nullable: aabb[N][6]*/, size_t n,

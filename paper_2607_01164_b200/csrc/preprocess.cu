@@ -13,7 +13,7 @@ __global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ me
                                                      const float *__restrict__ quat, const float *__restrict__ opacity,
                                                      const float *__restrict__ scalar, uint32_t N, float r,
                                                      float4 *__restrict__ rec, float *__restrict__ aabb,
-                                                     float *__restrict__ params) {
+                                                     float *__restrict__ params, unsigned long long *__restrict__ invalid) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const float mx = mean[3 * i], my = mean[3 * i + 1], mz = mean[3 * i + 2];
@@ -43,6 +43,7 @@ __global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ me
         *r2p = make_float4(0.f, 0.f, 0.f, 0.f);
         *r3 = make_float4(0.f, 0.f, 0.f, 0.f);
         bb[0] = inf; bb[1] = inf; bb[2] = inf; bb[3] = -inf; bb[4] = -inf; bb[5] = -inf;
+        atomicAdd(invalid, 1ull);  // surfaced by gs_status_query (D13)
         return;
     }
     // normalisation activation of the rotation
@@ -84,9 +85,11 @@ __global__ void __launch_bounds__(256) k_preprocess(const float *__restrict__ me
     }
 }
 
-cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, cudaStream_t s) {
-    if (g.n == 0) return cudaSuccess;
-    k_preprocess<<<(g.n + 255) / 256, 256, 0, s>>>(g.mean, g.scale, g.quat, g.opacity, g.scalar, g.n, r, rec, aabb, params); count_launch();
+cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float *aabb, float *params, unsigned long long *invalid,
+                              cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(invalid, 0, sizeof(unsigned long long), s);
+    if (e != cudaSuccess || g.n == 0) return e;
+    k_preprocess<<<(g.n + 255) / 256, 256, 0, s>>>(g.mean, g.scale, g.quat, g.opacity, g.scalar, g.n, r, rec, aabb, params, invalid); count_launch();
     return cudaGetLastError();
 }
 

@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
         continue;
     }
     const bool edge = (flags & 2u) || odd_x;
-    const int ncx = (int)(ncp & 2047u), ncy = (int)((ncp >> 11) & 2047u), ncz = (int)(ncp >> 22);
+    const int ncx = (int)(ncp & 1023u) + 1, ncy = (int)((ncp >> 10) & 1023u) + 1, ncz = (int)((ncp >> 20) & 1023u) + 1;
     const float thr = s1.y, invA = s1.z;
     if (rep + 1 < GPW && w0 + (rep + 1) * wstride < M) {  // pull the next Gaussian's records towards L1 while this one is processed
         const uint32_t nx = __shfl_sync(0xffffffffu, my_id, rep + 1);

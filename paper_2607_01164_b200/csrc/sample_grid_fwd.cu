@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
     unsigned long long tested = 0, hits = 0;
     const float dscale = (float)(2.0 * invP);
     const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
-    const bool vec2 = !SETS && !(bdx & 1u) && !o.gen.on;  // x-pairs are 8-byte aligned when the batch's x extent is even
+    const bool vec2 = !SETS && !(bdx & 1u) && !o.gen.on && o.vec_ok;  // x-pairs are 8-byte aligned when the batch's x extent is even
     LossPartial lp;
 #pragma unroll
     for (int r = 0; r < 4; r++) {  // the cell's four x-rows: (y, z) = (ly + (r & 1), lz + (r >> 1))
@@ -291,7 +291,7 @@ cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, c
                             const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, cudaStream_t s) {
     const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
     if (nbricks == 0) return cudaSuccess;
-    const double P = (double)gd.bdim[0] * gd.bdim[1] * gd.bdim[2];
+    const double P = o.inv_count > 0.0 ? 1.0 / o.inv_count : (double)gd.bdim[0] * gd.bdim[1] * gd.bdim[2];
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
     if (gd.jitter) {
         if (sets) k_grid_fwd<true, true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit);

@@ -459,8 +459,8 @@ cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const 
     const uint64_t packets = (P + 31) / 32;
     const unsigned blocks = (unsigned)((packets + EVAL_WARPS - 1) / EVAL_WARPS);
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
-    if (sets) k_points_fwd<true><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, 1.0 / (double)P);
-    else k_points_fwd<false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, 1.0 / (double)P);
+    if (sets) k_points_fwd<true><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, o.inv_count > 0.0 ? o.inv_count : 1.0 / (double)P);
+    else k_points_fwd<false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, o.inv_count > 0.0 ? o.inv_count : 1.0 / (double)P);
     count_launch();
     return cudaGetLastError();
 }

@@ -27,25 +27,37 @@ def shard_points(num_points: int, rank: int, world: int):
     return lo, lo + base + (1 if rank < rem else 0)
 
 
-def allreduce_grads(grads: dict, flat=None):
-    """Sum the gradient tensors over all ranks, in place, with ONE collective on a flat staging buffer.
-    `flat` (optional) is a preallocated 1-D float32 tensor of at least sum(numel) elements."""
+GRAD_COLS = dict(dmean=3, dscale=3, dquat=4, dopacity=1, dscalar=1, err=1)
+
+
+def flat_layout(n: int):
+    """Offsets (in floats) of the six gradient tensors of n Gaussians inside one flat buffer; every section starts on a
+    multiple of 4 floats (16 bytes: gs_grads.dquat needs it).  Returns ({name: (offset, columns)}, total floats)."""
+    off, o = {}, 0
+    for k in GRAD_KEYS:
+        off[k] = (o, GRAD_COLS[k])
+        o += (n * GRAD_COLS[k] + 3) // 4 * 4
+    return off, o
+
+
+def allreduce_grads(grads: dict, loss=None):
+    """Sum the gradient tensors (and, if given, the loss scalar) over all ranks, in place.  With grads["flat"] (see
+    api.Context.alloc_grads(flat=True)) the six tensors are views of one buffer and the exchange is ONE collective with no
+    packing; otherwise they are packed into a staging buffer first."""
     import torch
     import torch.distributed as dist
 
-    keys = [k for k in GRAD_KEYS if grads.get(k) is not None]
-    total = sum(grads[k].numel() for k in keys)
-    if flat is None or flat.numel() < total:
-        flat = torch.empty(total, dtype=torch.float32, device=grads[keys[0]].device)
-    off = 0
-    for k in keys:
-        n = grads[k].numel()
-        flat[off:off + n].copy_(grads[k].reshape(-1))
-        off += n
-    dist.all_reduce(flat[:total], op=dist.ReduceOp.SUM)
-    off = 0
-    for k in keys:
-        n = grads[k].numel()
-        grads[k].reshape(-1).copy_(flat[off:off + n])
-        off += n
+    if grads.get("flat") is not None:
+        dist.all_reduce(grads["flat"], op=dist.ReduceOp.SUM)
+    else:
+        keys = [k for k in GRAD_KEYS if grads.get(k) is not None]
+        flat = torch.cat([grads[k].reshape(-1) for k in keys])
+        dist.all_reduce(flat, op=dist.ReduceOp.SUM)
+        o = 0
+        for k in keys:
+            n = grads[k].numel()
+            grads[k].reshape(-1).copy_(flat[o:o + n])
+            o += n
+    if loss is not None:
+        dist.all_reduce(loss, op=dist.ReduceOp.SUM)
     return grads

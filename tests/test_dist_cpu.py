@@ -85,3 +85,77 @@ def test_gradients_add_over_sample_shards(oracle):
         parts.append(oracle.backward(g, xyz[lo:hi], fwd["phi"][lo:hi], fwd["I"][lo:hi], a[lo:hi], None, target[lo:hi], 0.01, mode=1))
     for k in full:
         np.testing.assert_allclose(parts[0][k] + parts[1][k], full[k], rtol=1e-9, atol=1e-15)
+
+
+def _bench_worker(rank, world, port, out):
+    """bench.py's N > 1 arm on CPU: its own sharding function, the oracle in place of the CUDA library, the flat gradient
+    buffer and allreduce_grads over gloo.  Every rank holds the same model; the loss mean runs over the GLOBAL sample count."""
+    import bench
+    from oracle import wveg_oracle as oracle
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    res = {}
+    for kind in ("grid", "points"):
+        g = inputs.c1_gaussians(seed=0, n=300)
+        if kind == "grid":
+            grid = inputs.Grid((24, 20, 28), (0.0, 0.0, 0.0), (1 / 24, 1 / 24, 1 / 28))
+            target = np.random.default_rng(1).uniform(0, 1, grid.num_points).astype(np.float32)
+            wl = dict(name="t", kind="grid", g=g, grid=grid, target=target)
+        else:
+            xyz = np.random.default_rng(2).uniform(0, 1, (3001, 3)).astype(np.float32)
+            target = np.random.default_rng(3).uniform(0, 1, 3001).astype(np.float32)
+            wl = dict(name="t", kind="points", g=g, batches=[(xyz, target)])
+        shards, P_total = bench.shard_workload(wl, rank, world)
+        off, total = gsdist.flat_layout(g.n)
+        flat = torch.zeros(total, dtype=torch.float32)
+        grads = {k: flat[o:o + g.n * c].view((g.n, c) if c > 1 else (g.n,)) for k, (o, c) in off.items()}
+        grads["flat"] = flat
+        loss = torch.zeros(1, dtype=torch.float64)
+        npts = 0
+        for s in shards:
+            pts = oracle.grid_points(s["grid"]) if kind == "grid" else s["xyz"]
+            npts += len(pts)
+            fwd = oracle.forward(g, pts, 0.01, mode=1)
+            res_ = fwd["phi"] - s["target"]
+            covered = fwd["I"].astype(np.float32) > np.float32(0.01)
+            a = np.where(covered, 2.0 * res_ / P_total, 0.0)     # what gs_set_sample_count(P_total) makes the fused MSE do
+            loss += float((res_ ** 2).sum() / P_total)
+            gr = oracle.backward(g, pts, fwd["phi"], fwd["I"], a, None, s["target"], 0.01, mode=1)
+            for k, v in gr.items():
+                grads[k] += torch.from_numpy(v.astype(np.float32)).view(grads[k].shape)
+        gsdist.allreduce_grads(grads, loss)
+        cnt = torch.tensor([npts], dtype=torch.int64)
+        dist.all_reduce(cnt)
+        assert int(cnt.item()) == P_total
+        res[kind] = ({k: grads[k].numpy().copy() for k in gsdist.GRAD_KEYS}, float(loss.item()))
+    out.put((rank, res))
+    dist.destroy_process_group()
+
+
+def test_bench_sharding_dry_run_world2(oracle):
+    ctxm = mp.get_context("spawn")
+    q = ctxm.Queue()
+    port = _free_port()
+    procs = [ctxm.Process(target=_bench_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict(q.get(timeout=240) for _ in range(2))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    # one-batch reference
+    g = inputs.c1_gaussians(seed=0, n=300)
+    grid = inputs.Grid((24, 20, 28), (0.0, 0.0, 0.0), (1 / 24, 1 / 24, 1 / 28))
+    cases = {"grid": (oracle.grid_points(grid), np.random.default_rng(1).uniform(0, 1, grid.num_points).astype(np.float32)),
+             "points": (np.random.default_rng(2).uniform(0, 1, (3001, 3)).astype(np.float32),
+                        np.random.default_rng(3).uniform(0, 1, 3001).astype(np.float32))}
+    for kind, (pts, target) in cases.items():
+        fwd = oracle.forward(g, pts, 0.01, mode=1)
+        loss, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, 0.01)
+        full = oracle.backward(g, pts, fwd["phi"], fwd["I"], a, None, target, 0.01, mode=1)
+        for r in range(2):   # both ranks hold the all-reduced result
+            grads, l = got[r][kind]
+            assert l == pytest.approx(loss, rel=1e-9)
+            for k, v in full.items():
+                np.testing.assert_allclose(grads[k].reshape(v.shape), v, rtol=2e-4, atol=1e-6 * np.abs(v).max())

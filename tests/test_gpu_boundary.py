@@ -1,0 +1,164 @@
+"""-m gpu tests of the C-ABI boundary's contract (include/gs.h "Conventions"): unaligned per-sample views, the
+invalid-Gaussian count of gs_status_query, per-context launch counters, a Gaussian spanning a 2048-voxel batch axis,
+and the multi-GPU decomposition run on ONE GPU: two sample shards through the library add up to the one-batch result."""
+import numpy as np
+import pytest
+
+from paper_2607_01164_b200 import inputs
+from gpu_util import TAU, GpuRun, check_grads, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+def _dev(torch, *arrays):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
+
+
+def test_unaligned_sample_views(oracle):
+    # gs.h: per-sample arrays may be 4-byte-aligned views (tensor[1:]); even x extent => the kernel would otherwise take
+    # its float2 path.  Results must equal the aligned call bit for bit (same arithmetic, scalar moves).
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c1_gaussians(seed=0, n=1024)
+    grid = inputs.c1_grid(32)
+    P = grid.num_points
+    target = np.random.default_rng(2).uniform(0, 1, P).astype(np.float32)
+    ref = GpuRun(g, "grid", grid, target)
+    ctx = api.Context()
+    ctx.gs_preprocess(*_dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar))
+    q = api.grid_query(grid)
+    ctx.gs_build_accel(q)
+    big = [torch.full((P + 1,), -7.0, device="cuda") for _ in range(5)]
+    phi, I, dphi, serr, t = (b[1:] for b in big)
+    assert phi.data_ptr() % 8 == 4
+    t.copy_(torch.from_numpy(target))
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx.gs_sample_fwd(q, phi, I, target=t, loss=loss, dL_dphi=dphi, sample_err=serr)
+    grads = ctx.alloc_grads(g.n)
+    ctx.gs_sample_bwd(q, phi, I, dphi, grads, target=t)
+    torch.cuda.synchronize()
+    for got, want in ((phi, ref.phi), (I, ref.I), (dphi, ref.dphi), (serr, ref.serr)):
+        assert torch.equal(got, want[:P])
+    assert float(loss.item()) == pytest.approx(float(ref.loss.item()), rel=1e-7)   # float partial sums in another order
+    for b in big:
+        assert float(b[0].item()) == -7.0   # nothing written in front of the view
+    for k, v in grads.items():
+        assert torch.equal(v, ref.grads[k]), k
+    # only one of the arrays unaligned
+    phi2 = torch.full((P,), -7.0, device="cuda")
+    ctx.gs_sample_fwd(q, phi2, I, target=t)
+    torch.cuda.synchronize()
+    assert torch.equal(phi2, ref.phi[:P])
+    ctx.close()
+
+
+def test_status_query_counts_invalid_gaussians():
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c1_gaussians(seed=3, n=500)
+    g.scale[7, 1] = 0.0
+    g.scale[8, 0] = -1.0
+    g.quat[100] = 0.0
+    g.mean[200, 2] = np.nan
+    g.opacity[300] = np.inf
+    ctx = api.Context()
+    assert ctx.gs_status_query()["num_gaussians"] == 0
+    ctx.gs_preprocess(*_dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar))
+    st = ctx.gs_status_query()
+    assert st["num_gaussians"] == 500 and st["invalid_gaussians"] == 5
+    q = api.grid_query(inputs.c1_grid(16))
+    ctx.gs_build_accel(q)
+    st = ctx.gs_status_query()
+    assert st["grid_pairs"] > 0 and 0 < st["grid_touched"] <= 495
+    g2 = inputs.c1_gaussians(seed=4, n=300)
+    ctx.gs_preprocess(*_dev(torch, g2.mean, g2.scale, g2.quat, g2.opacity, g2.scalar))
+    st = ctx.gs_status_query()
+    assert st["num_gaussians"] == 300 and st["invalid_gaussians"] == 0   # reset by every gs_preprocess
+    ctx.close()
+
+
+def test_launch_counters_are_per_context():
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c1_gaussians(seed=0, n=256)
+    dev = _dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+    a, b = api.Context(), api.Context()
+    a.profile_read(); b.profile_read()
+    a.gs_preprocess(*dev)
+    a.gs_preprocess(*dev)
+    b.gs_preprocess(*dev)
+    assert a.profile_read()[2] == 2
+    assert b.profile_read()[2] == 1
+    assert a.profile_read()[2] == 0
+    a.close(); b.close()
+
+
+def test_gaussian_spanning_a_2048_voxel_axis(oracle):
+    # the backward's cell-count packing must hold 1024 cells along z (a batch may span 2048 voxels per axis)
+    grid = inputs.Grid((8, 8, 2048), (0.0, 0.0, 0.0), (1 / 8, 1 / 8, 1 / 2048))
+    mean = np.array([[0.5, 0.5, 0.5], [0.3, 0.6, 0.2]], np.float32)
+    scale = np.array([[0.08, 0.08, 0.4], [0.05, 0.05, 0.01]], np.float32)   # the first one reaches beyond both z ends
+    quat = np.array([[1, 0, 0, 0], [1, 0, 0, 0]], np.float32)
+    g = inputs.Gaussians(mean, scale, quat, np.array([0.5, 0.7], np.float32), np.array([0.2, 0.9], np.float32))
+    P = grid.num_points
+    target = np.random.default_rng(0).uniform(0, 1, P).astype(np.float32)
+    xyz = oracle.grid_points(grid)
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    _, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+    assert np.abs(gr["dscale"][0]).max() > 0
+    for fused in (False, True):
+        run = GpuRun(g, "grid", grid, target, fused=fused)
+        check_grads(run, gr)
+
+
+def test_two_sample_shards_add_up_on_one_gpu(oracle):
+    # DESIGN.md section 10 on one GPU: the grid's bricks are split into two z-slabs (dist.shard_bricks), each slab runs
+    # through the C ABI as its own batch with the GLOBAL sample count as the loss normaliser (gs_set_sample_count); the
+    # per-shard losses and gradients must ADD UP to the one-batch ones and Phi / I must concatenate bit-exactly.
+    import torch
+    from paper_2607_01164_b200 import api, dist as gsdist
+    g = inputs.c4_gaussians(seed=9, n_grid=48, n=6000)
+    grid = inputs.Grid((48, 40, 44), (0.0, 0.0, 0.0), (1 / 48, 1 / 48, 1 / 48))
+    P = grid.num_points
+    target = np.random.default_rng(5).uniform(0, 1, P).astype(np.float32)
+    one = GpuRun(g, "grid", grid, target, fused=True)
+    dev = _dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+    total = {k: torch.zeros_like(v) for k, v in one.grads.items()}
+    loss_sum = 0.0
+    phis, Is = [], []
+    bd = grid.batch_dims
+    t3 = target.reshape(bd[2], bd[1], bd[0])
+    for r in range(2):
+        lo, cnt = gsdist.shard_bricks(grid.brick_cnt, r, 2)
+        sub = grid.batch(lo, cnt)
+        ctx = api.Context()
+        ctx.gs_set_sample_count(P)
+        ctx.gs_preprocess(*dev)
+        q = api.grid_query(sub)
+        ctx.gs_build_accel(q)
+        Pr = sub.num_points
+        z0 = 8 * lo[2]
+        t = torch.from_numpy(np.ascontiguousarray(t3[z0:z0 + sub.batch_dims[2]].ravel())).cuda()
+        phi, I = torch.empty(Pr, device="cuda"), torch.empty(Pr, device="cuda")
+        loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ctx.gs_sample_fwd(q, phi, I, target=t, loss=loss)
+        grads = ctx.alloc_grads(g.n, flat=True)
+        ctx.gs_sample_bwd(q, None, None, None, grads)
+        torch.cuda.synchronize()
+        for k in total:
+            total[k] += grads[k]
+        loss_sum += float(loss.item())
+        phis.append(phi); Is.append(I)
+        ctx.close()
+    assert torch.equal(torch.cat(phis), one.phi[:P]) and torch.equal(torch.cat(Is), one.I[:P])
+    assert loss_sum == pytest.approx(float(one.loss.item()), rel=1e-9)
+    for k in total:
+        assert rel_l2(total[k].cpu().numpy(), one.grads[k].cpu().numpy()) <= 1e-5, k
+    # ... and against the oracle's one-batch gradients
+    xyz = oracle.grid_points(grid)
+    fwd = oracle.forward(g, xyz, TAU, mode=1)
+    _, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+    gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+    for k, v in gr.items():
+        assert rel_l2(total[k].cpu().numpy(), v) <= 1e-4, k
