@@ -21,6 +21,7 @@
 //       "per Gaussian, loop over the leaf's positions" shape.
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
+#include "f32x2.cuh"
 
 namespace gs {
 
@@ -264,7 +265,11 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// k_points_fwd: lane = point; the packet's list is consumed chunk by chunk (32 records staged in shared memory).
+// k_points_fwd: the packet's list is consumed chunk by chunk (32 records staged in shared memory).
+// Lane = (half h = lane >> 4, point pair q = lane & 15): the lane evaluates the packet's points 2q and 2q + 1, packed
+// in the two halves of f32x2 registers, against the entries j = h, h + 2, ... of the chunk (the record is a scalar
+// broadcast to both halves).  One warp-iteration therefore tests 2 Gaussians x 32 points in ~28 issue slots
+// (15 packed instructions for the canonical sequence) where the scalar form needed 27 slots per Gaussian.
 // ---------------------------------------------------------------------------------------------------------
 template <bool SETS>
 __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
@@ -275,11 +280,14 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
     const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
     if (packet * 32 >= P) return;
     float4 (*buf)[128] = buf_all[warp];
-    const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
-    const float px = pp.px, py = pp.py, pz = pp.pz;
-    float I = 0.f, Nacc = 0.f;
-    uint32_t cnt = 0, tested = 0;
-    unsigned long long hsum = 0, hxor = 0;
+    const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);   // lane's own point (epilogue); NaN when past the end
+    const int half = lane >> 4, q2 = 2 * (lane & 15);
+    const f2 px = pk(__shfl_sync(0xffffffffu, pp.px, q2), __shfl_sync(0xffffffffu, pp.px, q2 + 1));
+    const f2 py = pk(__shfl_sync(0xffffffffu, pp.py, q2), __shfl_sync(0xffffffffu, pp.py, q2 + 1));
+    const f2 pz = pk(__shfl_sync(0xffffffffu, pp.pz, q2), __shfl_sync(0xffffffffu, pp.pz, q2 + 1));
+    f2 I2 = pk(0.f, 0.f), N2 = pk(0.f, 0.f);
+    uint32_t cnt[2] = {0, 0}, tested = 0;
+    unsigned long long hsum[2] = {0, 0}, hxor[2] = {0, 0};
     // Software pipeline over the chain of chunks: while chunk k is evaluated, the records of chunk k+1 are being
     // copied into the other buffer and the ids of chunk k+2 are being loaded.
     const uint2 head = __ldg(L.head + packet);
@@ -299,20 +307,48 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
         if (c2 != NO_CHUNK) { pos2 = __ldg(L.ids + (size_t)c2 * 32 + lane); c3 = __ldg(L.link + c2); }
         const float4 *rb = buf[b];
 #pragma unroll 4
-        for (int j = 0; j < n0; j++) {
-            Rec q;
-            q.a = rb[4 * j]; q.b = rb[4 * j + 1]; q.c = rb[4 * j + 2]; q.d = rb[4 * j + 3];
-            float u0, u1, u2;
-            const float qd = mahalanobis(q, px, py, pz, u0, u1, u2);
-            const bool hit = qd <= r2;
-            const float G = hit ? gauss_weight(qd) : 0.f;
-            I = fmaf(q.a.w, G, I);
-            Nacc = fmaf(q.d.w, G, Nacc);  // d.w = v w
-            if (SETS && hit) { const unsigned long long h = mix64(__float_as_uint(q.c.w)); cnt++; hsum += h; hxor ^= h; }
+        for (int j = half; j < n0; j += 2) {
+            const float4 ga = rb[4 * j], gb = rb[4 * j + 1], gc = rb[4 * j + 2], gd = rb[4 * j + 3];
+            f2 u0, u1, u2;
+            const f2 qd = mahalanobis2(ga.x, ga.y, ga.z, gb.x, gb.y, gb.z, gc.x, gc.y, gc.z, gd.x, gd.y, gd.z, px, py, pz, u0, u1, u2);
+            bool h0, h1;
+            const f2 G = gauss_weight2(qd, r2, h0, h1);
+            I2 = fma2(bc(ga.w), G, I2);
+            N2 = fma2(bc(gd.w), G, N2);   // d.w = v w
+            if (SETS) {
+                const unsigned long long h = mix64(__float_as_uint(gc.w));
+                if (h0) { cnt[0]++; hsum[0] += h; hxor[0] ^= h; }
+                if (h1) { cnt[1]++; hsum[1] += h; hxor[1] ^= h; }
+            }
         }
         if (SETS) tested += (uint32_t)n0;
         __syncwarp();
         c0 = c1; n0 = 32; c1 = c2; pos1 = pos2; c2 = c3; b ^= 1;
+    }
+    // the two halves hold the sums over the even / odd entries: add them, then hand point `lane` its own result
+    float Il, Ih, Nl, Nh;
+    upk(I2, Il, Ih);
+    upk(N2, Nl, Nh);
+    Il += __shfl_xor_sync(0xffffffffu, Il, 16); Ih += __shfl_xor_sync(0xffffffffu, Ih, 16);
+    Nl += __shfl_xor_sync(0xffffffffu, Nl, 16); Nh += __shfl_xor_sync(0xffffffffu, Nh, 16);
+    const int src = lane >> 1;
+    const bool odd = lane & 1;
+    const float Ia = __shfl_sync(0xffffffffu, Il, src), Ib = __shfl_sync(0xffffffffu, Ih, src);
+    const float Na = __shfl_sync(0xffffffffu, Nl, src), Nb = __shfl_sync(0xffffffffu, Nh, src);
+    const float I = odd ? Ib : Ia, Nacc = odd ? Nb : Na;
+    uint32_t mycnt = 0;
+    unsigned long long mysum = 0, myxor = 0;
+    if (SETS) {
+#pragma unroll
+        for (int d = 0; d < 2; d++) {
+            cnt[d] += __shfl_xor_sync(0xffffffffu, cnt[d], 16);
+            hsum[d] += __shfl_xor_sync(0xffffffffu, hsum[d], 16);
+            hxor[d] ^= __shfl_xor_sync(0xffffffffu, hxor[d], 16);
+        }
+        const uint32_t ca = __shfl_sync(0xffffffffu, cnt[0], src), cb = __shfl_sync(0xffffffffu, cnt[1], src);
+        const unsigned long long sa = __shfl_sync(0xffffffffu, hsum[0], src), sb = __shfl_sync(0xffffffffu, hsum[1], src);
+        const unsigned long long xa = __shfl_sync(0xffffffffu, hxor[0], src), xb = __shfl_sync(0xffffffffu, hxor[1], src);
+        mycnt = odd ? cb : ca; mysum = odd ? sb : sa; myxor = odd ? xb : xa;
     }
     const bool active = pp.active;
     const uint64_t c = pp.c;
@@ -336,9 +372,9 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             }
         }
         if (SETS) {
-            if (o.set_count) o.set_count[c] = cnt;
-            if (o.set_sum) o.set_sum[c] = hsum;
-            if (o.set_xor) o.set_xor[c] = hxor;
+            if (o.set_count) o.set_count[c] = mycnt;
+            if (o.set_sum) o.set_sum[c] = mysum;
+            if (o.set_xor) o.set_xor[c] = myxor;
         }
     }
     if (o.gen.on) loss_flush(o.gen, lp, lane);
@@ -349,7 +385,7 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
         if (lane == 0 && s != 0.0) atomicAdd(o.loss, s * invP);
     }
     if (SETS && o.counters) {
-        unsigned long long t = active ? tested : 0, h = cnt;
+        unsigned long long t = active ? tested : 0, h = active ? mycnt : 0;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) { t += __shfl_xor_sync(0xffffffffu, t, d); h += __shfl_xor_sync(0xffffffffu, h, d); }
         if (lane == 0) { atomicAdd(o.counters, t); atomicAdd(o.counters + 1, h); }
@@ -366,12 +402,14 @@ __device__ __forceinline__ void red_add_v4(float *addr, float a, float b, float 
 __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, BwdIn in, float *__restrict__ gacc) {
-    __shared__ float4 pts_all[EVAL_WARPS][2][32];   // [0] x y z alpha   [1] beta eps - -
+    // the packet's points as PAIRS (2i, 2i + 1) for the packed arithmetic: [i][0] = x0 x1 y0 y1, [i][1] = z0 z1 alpha0 alpha1,
+    // [i][2] = beta0 beta1 eps0 eps1
+    __shared__ __align__(16) float pts_all[EVAL_WARPS][16][12];
     __shared__ float4 buf_all[EVAL_WARPS][2][128];  // two chunks of 32 records of 64 B, swizzled (see gather64)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
     if (packet * 32 >= P) return;
-    float4 (*pts)[32] = pts_all[warp];
+    float (*pts)[12] = pts_all[warp];
     float4 (*buf)[128] = buf_all[warp];
     {
         const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
@@ -390,8 +428,16 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
             beta = (in.dL_dI ? in.dL_dI[c] : 0.f) - alpha * ph;
             eps = (covered && in.target) ? fabsf(ph - in.target[c]) * inv : 0.f;
         }
-        pts[0][lane] = make_float4(pp.px, pp.py, pp.pz, alpha);   // inactive lanes hold NaN positions: never a hit
-        pts[1][lane] = make_float4(beta, eps, 0.f, 0.f);
+        // The sums below are accumulated without a branch (a miss has G = 0), so a NaN / infinite position would turn
+        // 0 * u into NaN for every Gaussian of the list.  Such a point (a lane past the end, or a non-finite query) lies
+        // in no support: it takes part with zero coefficients at a harmless finite position.
+        float x = pp.px, y = pp.py, z = pp.pz;
+        if (!(fabsf(x) <= 3.402823466e38f && fabsf(y) <= 3.402823466e38f && fabsf(z) <= 3.402823466e38f)) {
+            x = y = z = 0.f;
+            alpha = beta = eps = 0.f;
+        }
+        float *row = pts[lane >> 1] + (lane & 1);
+        row[0] = x; row[2] = y; row[4] = z; row[6] = alpha; row[8] = beta; row[10] = eps;
         __syncwarp();
     }
     // same software pipeline as the forward: records of chunk k+1 and ids of chunk k+2 are in flight during chunk k
@@ -415,25 +461,43 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
             const int f = (lane >> 1) & 3;
             Rec g;
             g.a = rb[f]; g.b = rb[1 ^ f]; g.c = rb[2 ^ f]; g.d = rb[3 ^ f];
-            float acc[12];
+            // lane = Gaussian (scalars, broadcast to both halves); two points per iteration ride in the halves.  A miss has
+            // G = 0 and adds nothing, so the 12 sums are accumulated unconditionally (no divergent branch).
+            f2 acc[12];
 #pragma unroll
-            for (int q = 0; q < 12; q++) acc[q] = 0.f;
+            for (int q = 0; q < 12; q++) acc[q] = pk(0.f, 0.f);
             bool any = false;
+            const f2 w2 = bc(g.a.w), v2 = bc(g.b.w);
 #pragma unroll 4
-            for (int p = 0; p < 32; p++) {
-                const float4 pa = pts[0][p], pb = pts[1][p];
-                float u0, u1, u2;
-                const float qd = mahalanobis(g, pa.x, pa.y, pa.z, u0, u1, u2);
-                if (qd <= r2) {
-                    any = true;
-                    bwd_accumulate(acc, pa.w, pb.x, pb.y, g.a.w, g.b.w, gauss_weight(qd), u0, u1, u2);
-                }
+            for (int i = 0; i < 16; i++) {
+                const ulonglong2 A = *reinterpret_cast<const ulonglong2 *>(pts[i]), B = *reinterpret_cast<const ulonglong2 *>(pts[i] + 4),
+                                 C = *reinterpret_cast<const ulonglong2 *>(pts[i] + 8);
+                f2 u0, u1, u2;
+                const f2 qd = mahalanobis2(g.a.x, g.a.y, g.a.z, g.b.x, g.b.y, g.b.z, g.c.x, g.c.y, g.c.z, g.d.x, g.d.y, g.d.z, A.x, A.y, B.x, u0, u1, u2);
+                bool h0, h1;
+                const f2 G = gauss_weight2(qd, r2, h0, h1);
+                any |= h0 | h1;
+                const f2 alpha = B.y, beta = C.x, eps = C.y;
+                // S7: gamma = alpha v + beta, t = gamma w G: dv += alpha w G, dw += gamma G, U += t u, W += t u u^T, E += eps w G
+                const f2 wG = mul2(w2, G);
+                const f2 gamma = fma2(alpha, v2, beta);
+                const f2 t = mul2(gamma, wG);
+                acc[0] = fma2(alpha, wG, acc[0]);
+                acc[1] = fma2(gamma, G, acc[1]);
+                const f2 t0 = mul2(t, u0), t1 = mul2(t, u1), t2 = mul2(t, u2);
+                acc[2] = add2(acc[2], t0); acc[3] = add2(acc[3], t1); acc[4] = add2(acc[4], t2);
+                acc[5] = fma2(t0, u0, acc[5]); acc[6] = fma2(t0, u1, acc[6]); acc[7] = fma2(t0, u2, acc[7]);
+                acc[8] = fma2(t1, u1, acc[8]); acc[9] = fma2(t1, u2, acc[9]); acc[10] = fma2(t2, u2, acc[10]);
+                acc[11] = fma2(eps, wG, acc[11]);
             }
             if (any) {
+                float s[12];
+#pragma unroll
+                for (int q = 0; q < 12; q++) s[q] = lo(acc[q]) + hi(acc[q]);
                 float *row = gacc + (size_t)__float_as_uint(g.c.w) * GACC;
-                red_add_v4(row, acc[0], acc[1], acc[2], acc[3]);
-                red_add_v4(row + 4, acc[4], acc[5], acc[6], acc[7]);
-                red_add_v4(row + 8, acc[8], acc[9], acc[10], acc[11]);
+                red_add_v4(row, s[0], s[1], s[2], s[3]);
+                red_add_v4(row + 4, s[4], s[5], s[6], s[7]);
+                red_add_v4(row + 8, s[8], s[9], s[10], s[11]);
             }
         }
         __syncwarp();
