@@ -64,6 +64,11 @@ __device__ __forceinline__ unsigned long long voxel_linear(int gx, int gy, int g
     return ((unsigned long long)gz * (unsigned long long)dimy + (unsigned long long)gy) * (unsigned long long)dimx + (unsigned long long)gx;
 }
 
+// Fused-MSE backward coefficients of a GRID batch (written by k_grid_fwd, read by k_grid_bwd): samples are stored in
+// aligned pairs, float4 per pair (c even) = (alpha_c, alpha_c+1, beta_c, beta_c+1), so that the two x-neighbours of a
+// row arrive as the two halves of packed registers.  Index of alpha_c in floats; beta_c sits 2 floats further.
+__device__ __forceinline__ size_t pack2_index(size_t c) { return ((c >> 1) << 2) | (c & 1); }
+
 // id hash for order-free set comparison (splitmix64 finaliser of id + golden gamma)
 __device__ __forceinline__ unsigned long long mix64(uint32_t id) {
     unsigned long long z = (unsigned long long)id + 0x9E3779B97F4A7C15ull;

@@ -24,6 +24,7 @@
 
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
+#include "f32x2.cuh"
 
 namespace gs {
 
@@ -134,14 +135,16 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
         const uint32_t base = ((uint32_t)(Z - first[2]) * bdy + (uint32_t)(Y - first[1])) * bdx + (uint32_t)(X - first[0]);
         // per-sample coefficients of the 8 voxels: issued up front (no data dependence on the predicate), so their
         // L1/L2 latency overlaps the arithmetic below
-        float al[8], be[8], ep[8];
+        // PACK2: al2[r] / be2[r] = (alpha, beta) of the row's two x-neighbours in packed halves (pair layout of pack2_index)
+        f2 al2[4], be2[4];
+        float ep[8];
         if (!EDGE && PACK2) {
-            const float2 *p2 = reinterpret_cast<const float2 *>(pack_);
+            const float4 *p4 = reinterpret_cast<const float4 *>(pack_);
 #pragma unroll
             for (int r = 0; r < 4; r++) {  // (y, z) rows of the cell: one 16-byte load per x-pair
                 const uint32_t c = base + ((uint32_t)(r >> 1) * bdy + (uint32_t)(r & 1)) * bdx;
-                const float4 s = on ? __ldg(reinterpret_cast<const float4 *>(p2 + c)) : make_float4(0.f, 0.f, 0.f, 0.f);
-                al[2 * r] = s.x; be[2 * r] = s.y; al[2 * r + 1] = s.z; be[2 * r + 1] = s.w;
+                const float4 s = on ? __ldg(p4 + (c >> 1)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                al2[r] = pk(s.x, s.y); be2[r] = pk(s.z, s.w);
             }
         } else {
             bool okx[2], oky[2], okz[2];
@@ -151,18 +154,21 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                 oky[d] = !EDGE || Y + d <= last[1];
                 okz[d] = !EDGE || Z + d <= last[2];
             }
+            float al[8], be[8];
 #pragma unroll
             for (int v = 0; v < 8; v++) {
                 const uint32_t c = base + ((uint32_t)(v >> 2) * bdy + (uint32_t)((v >> 1) & 1)) * bdx + (uint32_t)(v & 1);
                 const bool ok = on && okx[v & 1] && oky[(v >> 1) & 1] && okz[v >> 2];
                 if (PACK2) {
-                    const float2 s = ok ? __ldg(reinterpret_cast<const float2 *>(pack_) + c) : make_float2(0.f, 0.f);
-                    al[v] = s.x; be[v] = s.y;
+                    const float *pf = reinterpret_cast<const float *>(pack_) + pack2_index(c);
+                    al[v] = ok ? __ldg(pf) : 0.f; be[v] = ok ? __ldg(pf + 2) : 0.f;
                 } else {
                     const float4 s = ok ? __ldg(reinterpret_cast<const float4 *>(pack_) + c) : make_float4(0.f, 0.f, 0.f, 0.f);
                     al[v] = s.x; be[v] = s.y; ep[v] = s.z;
                 }
             }
+#pragma unroll
+            for (int r = 0; r < 4; r++) { al2[r] = pk(al[2 * r], al[2 * r + 1]); be2[r] = pk(be[2 * r], be[2 * r + 1]); }
         }
         if (JIT) {
             // jittered samples (D26): no two voxels of the cell share a coordinate and u is not affine in the
@@ -181,9 +187,10 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                 const float u2 = __fmaf_rn(gd4.z, dzv, __fmaf_rn(gd4.y, dyv, __fmul_rn(gd4.x, dxv)));
                 const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
                 const float G = qd <= r2 ? gauss_weight(qd) : 0.f;
-                const float gg = fmaf(al[v], gb.w, be[v]) * G;
-                acc[0] = fmaf(al[v], G, acc[0]);
-                acc[2] = fmaf(PACK2 ? fabsf(al[v]) : ep[v], G, acc[2]);
+                const float alv = (v & 1) ? hi(al2[v >> 1]) : lo(al2[v >> 1]), bev = (v & 1) ? hi(be2[v >> 1]) : lo(be2[v >> 1]);
+                const float gg = fmaf(alv, gb.w, bev) * G;
+                acc[0] = fmaf(alv, G, acc[0]);
+                acc[2] = fmaf(PACK2 ? fabsf(alv) : ep[v], G, acc[2]);
                 acc[1] += gg;
                 const float t0 = gg * u0, t1 = gg * u1, t2 = gg * u2;
                 acc[3] += t0; acc[4] += t1; acc[5] += t2;
@@ -192,45 +199,50 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
             }
             return;
         }
+        // canonical positions (D6) and sequence (D4), packed over the x-neighbours (f32x2.cuh) with the sub-expressions
+        // shared between voxels of equal x / equal (x, y): u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx))
         float dx[2], dy[2], dz[2];
-#pragma unroll
-        for (int d = 0; d < 2; d++) {  // canonical positions (D6)
-            dx[d] = __fsub_rn(voxel_centre(X + d, gd.spacing[0], gd.origin[0]), ga.x);
-            dy[d] = __fsub_rn(voxel_centre(Y + d, gd.spacing[1], gd.origin[1]), ga.y);
-            dz[d] = __fsub_rn(voxel_centre(Z + d, gd.spacing[2], gd.origin[2]), ga.z);
-        }
-        // canonical sequence (D4) with shared sub-expressions: u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx))
-        float ab[3][4];
+        const f2 dx2 = sub2(pk(voxel_centre(X, gd.spacing[0], gd.origin[0]), voxel_centre(X + 1, gd.spacing[0], gd.origin[0])), bc(ga.x));
+        upk(dx2, dx[0], dx[1]);
+        upk(sub2(pk(voxel_centre(Y, gd.spacing[1], gd.origin[1]), voxel_centre(Y + 1, gd.spacing[1], gd.origin[1])), bc(ga.y)), dy[0], dy[1]);
+        upk(sub2(pk(voxel_centre(Z, gd.spacing[2], gd.origin[2]), voxel_centre(Z + 1, gd.spacing[2], gd.origin[2])), bc(ga.z)), dz[0], dz[1]);
+        f2 qd[4];   // pair r = (y, z) row of the cell: voxels 2r, 2r + 1
+        float c0 = 0.f, c1 = 0.f, c2 = 0.f;  // c = u(voxel 0)
 #pragma unroll
         for (int row = 0; row < 3; row++) {
             const float4 mr = row == 0 ? gb : row == 1 ? gc : gd4;
-            const float a0 = __fmul_rn(mr.x, dx[0]), a1 = __fmul_rn(mr.x, dx[1]);
-            ab[row][0] = __fmaf_rn(mr.y, dy[0], a0); ab[row][1] = __fmaf_rn(mr.y, dy[0], a1);
-            ab[row][2] = __fmaf_rn(mr.y, dy[1], a0); ab[row][3] = __fmaf_rn(mr.y, dy[1], a1);
-        }
-        float g[8], c0 = 0.f, c1 = 0.f, c2 = 0.f;  // c = u(voxel 0)
+            const f2 a2 = mul2(bc(mr.x), dx2);
+            f2 ab[2];
 #pragma unroll
-        for (int v = 0; v < 8; v++) {  // v = x | y << 1 | z << 2
-            const float u0 = __fmaf_rn(gb.z, dz[v >> 2], ab[0][v & 3]);
-            const float u1 = __fmaf_rn(gc.z, dz[v >> 2], ab[1][v & 3]);
-            const float u2 = __fmaf_rn(gd4.z, dz[v >> 2], ab[2][v & 3]);
-            if (v == 0) { c0 = u0; c1 = u1; c2 = u2; }
-            const float qd = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
-            g[v] = qd <= r2 ? gauss_weight(qd) : 0.f;  // G; the canonical predicate decides membership
-        }
-        // the coefficients are first needed here, a whole cell's worth of arithmetic after their loads were issued
+            for (int iy = 0; iy < 2; iy++) ab[iy] = fma2(bc(mr.y), bc(dy[iy]), a2);
 #pragma unroll
-        for (int v = 0; v < 8; v++) {
-            const float G = g[v];
-            g[v] = fmaf(al[v], gb.w, be[v]) * G;
-            acc[0] = fmaf(al[v], G, acc[0]);
-            acc[2] = fmaf(PACK2 ? fabsf(al[v]) : ep[v], G, acc[2]);
+            for (int r = 0; r < 4; r++) {  // r = y | z << 1
+                const f2 u = fma2(bc(mr.z), bc(dz[r >> 1]), ab[r & 1]);
+                if (r == 0) { if (row == 0) c0 = lo(u); else if (row == 1) c1 = lo(u); else c2 = lo(u); }
+                qd[r] = row == 0 ? mul2(u, u) : fma2(u, u, qd[r]);
+            }
         }
+        // g = gamma G per voxel (G = 0 for a miss: the canonical predicate decides membership); the coefficients are first
+        // needed here, a whole cell's worth of arithmetic after their loads were issued
+        f2 g2[4], a0 = pk(0.f, 0.f);
+        float g[8];
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            bool h0, h1;
+            const f2 G = gauss_weight2(qd[r], r2, h0, h1);
+            g2[r] = mul2(fma2(al2[r], bc(gb.w), be2[r]), G);
+            a0 = fma2(al2[r], G, a0);
+            float G0, G1;
+            upk(G, G0, G1);
+            acc[2] = fmaf(PACK2 ? fabsf(lo(al2[r])) : ep[2 * r], G0, acc[2]);
+            acc[2] = fmaf(PACK2 ? fabsf(hi(al2[r])) : ep[2 * r + 1], G1, acc[2]);
+            upk(g2[r], g[2 * r], g[2 * r + 1]);
+        }
+        acc[0] += lo(a0) + hi(a0);
         // index moments of g over the cell
-        const float s01 = g[0] + g[1], s23 = g[2] + g[3], s45 = g[4] + g[5], s67 = g[6] + g[7];
-        const float x13 = g[1] + g[3], m101 = g[5] + g[7], m110 = g[3] + g[7];
-        const float m100 = x13 + m101, m010 = s23 + s67, m001 = s45 + s67, m011 = s67;
-        const float m000 = (s01 + s23) + m001;
+        const f2 sA = add2(g2[0], g2[1]), sB = add2(g2[2], g2[3]), sS = add2(sA, sB), sT = add2(g2[1], g2[3]);
+        const float m100 = hi(sS), m000 = lo(sS) + m100, m110 = hi(sT), m010 = lo(sT) + m110, m101 = hi(sB), m001 = lo(sB) + m101,
+                    m011 = g[6] + g[7];
         // exact position steps of this cell (the canonical positions are rounded, so they differ from the spacing by an ulp)
         const float ex = dx[1] - dx[0], ey = dy[1] - dy[0], ez = dz[1] - dz[0];
         const float a100 = m100 * ex, a010 = m010 * ey, a001 = m001 * ez;

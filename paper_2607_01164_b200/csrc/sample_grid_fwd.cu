@@ -13,6 +13,7 @@
 // Epilogue S6 is fused: coverage rule, normalisation, MSE partial sums, dL/dPhi, per-sample error.
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
+#include "f32x2.cuh"
 
 namespace gs {
 
@@ -51,17 +52,23 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
         py[d] = (ly + d < gd.bdim[1]) ? voxel_centre(ly + d + BRICK * gd.brick_lo[1], gd.spacing[1], gd.origin[1]) : nanv;
         pz[d] = (lz + d < gd.bdim[2]) ? voxel_centre(lz + d + BRICK * gd.brick_lo[2], gd.spacing[2], gd.origin[2]) : nanv;
     }
-    // JIT: every voxel has its own position inside its cell (D26); v = x | y << 1 | z << 2
-    float jp[JIT ? 8 : 1][3];
+    // the two x-neighbours of a row ride in the halves of one packed register (f32x2.cuh)
+    const f2 px2 = pk(px[0], px[1]), py2 = pk(py[0], py[1]), pz2 = pk(pz[0], pz[1]);
+    // JIT: every voxel has its own position inside its cell (D26); pair r = voxels (2r, 2r + 1), v = x | y << 1 | z << 2
+    f2 jp[JIT ? 4 : 1][3];
     if (JIT) {
 #pragma unroll
-        for (int v = 0; v < 8; v++) {
-            const int x = lx + (v & 1), y = ly + ((v >> 1) & 1), z = lz + (v >> 2);
-            const bool in = x < gd.bdim[0] && y < gd.bdim[1] && z < gd.bdim[2];
-            const int gx = x + BRICK * gd.brick_lo[0], gy = y + BRICK * gd.brick_lo[1], gz = z + BRICK * gd.brick_lo[2];
-            float4 sp = make_float4(nanv, nanv, nanv, 0.f);
-            if (in) sp = jit[((uint32_t)z * (uint32_t)gd.bdim[1] + (uint32_t)y) * (uint32_t)gd.bdim[0] + (uint32_t)x];
-            jp[v][0] = sp.x; jp[v][1] = sp.y; jp[v][2] = sp.z;
+        for (int r = 0; r < 4; r++) {
+            float c[2][3];
+#pragma unroll
+            for (int d = 0; d < 2; d++) {
+                const int x = lx + d, y = ly + (r & 1), z = lz + (r >> 1);
+                const bool in = x < gd.bdim[0] && y < gd.bdim[1] && z < gd.bdim[2];
+                float4 sp = make_float4(nanv, nanv, nanv, 0.f);
+                if (in) sp = jit[((uint32_t)z * (uint32_t)gd.bdim[1] + (uint32_t)y) * (uint32_t)gd.bdim[0] + (uint32_t)x];
+                c[d][0] = sp.x; c[d][1] = sp.y; c[d][2] = sp.z;
+            }
+            jp[r][0] = pk(c[0][0], c[1][0]); jp[r][1] = pk(c[0][1], c[1][1]); jp[r][2] = pk(c[0][2], c[1][2]);
         }
     }
     // cull geometry (not canonical): centre of the warp's cell (0,0,0), cell pitch = 2 voxels, half extent = half a voxel
@@ -73,11 +80,11 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
     const float hx = hh * gd.spacing[0], hy = hh * gd.spacing[1], hz = hh * gd.spacing[2];
     const float rcut = sqrtf(r2);
 
-    float I[8], Nacc[8];
+    f2 I2[4], N2[4];   // pair r = voxels (2r, 2r + 1) of the cell
     uint32_t cnt[SETS ? 8 : 1], ntest = 0;
     unsigned long long hsum[SETS ? 8 : 1], hxor[SETS ? 8 : 1];
 #pragma unroll
-    for (int v = 0; v < 8; v++) { I[v] = 0.f; Nacc[v] = 0.f; }
+    for (int r = 0; r < 4; r++) { I2[r] = pk(0.f, 0.f); N2[r] = pk(0.f, 0.f); }
     if (SETS) {
 #pragma unroll
         for (int v = 0; v < 8; v++) { cnt[v] = 0; hsum[v] = 0; hxor[v] = 0; }
@@ -144,63 +151,59 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
         }
         __syncwarp();
         // ---- evaluation: lane = cell, walking its own masks over the whole round; 8 voxels per listed Gaussian.
-        // The 128-bit mask is walked with 32-bit operations: `cur` is the word being consumed, w1..w3 the ones behind it.
+        // The 128-bit mask is walked as 32-bit words.  Empty words are squeezed out first (once per round), so that inside
+        // the loop ONE predicated refill is enough whenever the current word runs dry (left > 0 => the next word has a bit).
         const uint4 mk = smask[warp][lane];
-        uint32_t cur = mk.x, w1 = mk.y, w2 = mk.z, w3 = mk.w;
-        int jbase = 0;
-        for (int left = __popc(cur) + __popc(w1) + __popc(w2) + __popc(w3); left > 0; left--) {
-            while (cur == 0u) { cur = w1; w1 = w2; w2 = w3; w3 = 0u; jbase += 32; }
-            const int j = jbase + __ffs((int)cur) - 1;
-            cur &= cur - 1u;
+        uint32_t w0 = mk.x, w1 = mk.y, w2 = mk.z, w3 = mk.w;
+        int b0 = 0, b1 = 32, b2 = 64, b3 = 96;
+        if (w2 == 0u) { w2 = w3; b2 = b3; w3 = 0u; }
+        if (w1 == 0u) { w1 = w2; b1 = b2; w2 = w3; b2 = b3; w3 = 0u; }
+        if (w0 == 0u) { w0 = w1; b0 = b1; w1 = w2; b1 = b2; w2 = w3; b2 = b3; w3 = 0u; }
+        for (int left = __popc(w0) + __popc(w1) + __popc(w2) + __popc(w3); left > 0; left--) {
+            if (w0 == 0u) { w0 = w1; b0 = b1; w1 = w2; b1 = b2; w2 = w3; b2 = b3; }
+            const int j = b0 + __ffs((int)w0) - 1;
+            w0 &= w0 - 1u;
             const float4 ga = srec[0][j], gb = srec[1][j], gc = srec[2][j], gd4 = srec[3][j];
-            // canonical sequence (D4), shared between voxels: d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx));
-            // qd = fma(u2, u2, fma(u1, u1, u0 * u0))
-            float qd[8];
-            if (JIT) {  // no two voxels share a coordinate: the plain canonical sequence per voxel
+            // canonical sequence (D4): d = p - mu; u_j = fma(M_j2, dz, fma(M_j1, dy, M_j0 * dx)); qd = fma(u2, u2, fma(u1, u1, u0 * u0)),
+            // packed over the x-neighbours (every packed instruction is the scalar one on both halves) and shared between the
+            // voxels of equal x / equal (x, y): 36 packed instructions for the 8 voxels of the cell
+            f2 qd[4];
+            if (JIT) {  // no two voxels share a coordinate: the plain canonical sequence per pair
 #pragma unroll
-                for (int v = 0; v < 8; v++) {
-                    const float dx = __fsub_rn(jp[v][0], ga.x), dy = __fsub_rn(jp[v][1], ga.y), dz = __fsub_rn(jp[v][2], ga.z);
-                    const float u0 = __fmaf_rn(gb.z, dz, __fmaf_rn(gb.y, dy, __fmul_rn(gb.x, dx)));
-                    const float u1 = __fmaf_rn(gc.z, dz, __fmaf_rn(gc.y, dy, __fmul_rn(gc.x, dx)));
-                    const float u2 = __fmaf_rn(gd4.z, dz, __fmaf_rn(gd4.y, dy, __fmul_rn(gd4.x, dx)));
-                    qd[v] = __fmaf_rn(u2, u2, __fmaf_rn(u1, u1, __fmul_rn(u0, u0)));
+                for (int r = 0; r < 4; r++) {
+                    f2 u0, u1, u2;
+                    qd[r] = mahalanobis2(ga.x, ga.y, ga.z, gb.x, gb.y, gb.z, gc.x, gc.y, gc.z, gd4.x, gd4.y, gd4.z, jp[r][0], jp[r][1], jp[r][2], u0, u1, u2);
                 }
             } else {
-            float dx[2], dy[2], dz[2];
+                const f2 dx2 = sub2(px2, bc(ga.x));
+                float dy[2], dz[2];
+                upk(sub2(py2, bc(ga.y)), dy[0], dy[1]);
+                upk(sub2(pz2, bc(ga.z)), dz[0], dz[1]);
 #pragma unroll
-            for (int d = 0; d < 2; d++) {
-                dx[d] = __fsub_rn(px[d], ga.x);
-                dy[d] = __fsub_rn(py[d], ga.y);
-                dz[d] = __fsub_rn(pz[d], ga.z);
-            }
+                for (int row = 0; row < 3; row++) {
+                    const float4 mr = row == 0 ? gb : row == 1 ? gc : gd4;
+                    const f2 a2 = mul2(bc(mr.x), dx2);
+                    f2 ab[2];
 #pragma unroll
-            for (int row = 0; row < 3; row++) {
-                const float4 mr = row == 0 ? gb : row == 1 ? gc : gd4;
-                float a[2], ab[4];
+                    for (int iy = 0; iy < 2; iy++) ab[iy] = fma2(bc(mr.y), bc(dy[iy]), a2);
 #pragma unroll
-                for (int ix = 0; ix < 2; ix++) a[ix] = __fmul_rn(mr.x, dx[ix]);
-#pragma unroll
-                for (int iy = 0; iy < 2; iy++)
-#pragma unroll
-                    for (int ix = 0; ix < 2; ix++) ab[iy * 2 + ix] = __fmaf_rn(mr.y, dy[iy], a[ix]);
-#pragma unroll
-                for (int v = 0; v < 8; v++) {
-                    const float u = __fmaf_rn(mr.z, dz[v >> 2], ab[v & 3]);
-                    qd[v] = row == 0 ? __fmul_rn(u, u) : __fmaf_rn(u, u, qd[v]);
+                    for (int r = 0; r < 4; r++) {  // r = y | z << 1
+                        const f2 u = fma2(bc(mr.z), bc(dz[r >> 1]), ab[r & 1]);
+                        qd[r] = row == 0 ? mul2(u, u) : fma2(u, u, qd[r]);
+                    }
                 }
-            }
             }
             if (SETS) ntest += 8;
 #pragma unroll
-            for (int v = 0; v < 8; v++) {
-                if (qd[v] <= r2) {
-                    const float G = gauss_weight(qd[v]);
-                    I[v] = fmaf(ga.w, G, I[v]);
-                    Nacc[v] = fmaf(gd4.w, G, Nacc[v]);  // gd4.w = v w
-                    if (SETS) {
-                        const unsigned long long h = mix64(sid[j]);
-                        cnt[v]++; hsum[v] += h; hxor[v] ^= h;
-                    }
+            for (int r = 0; r < 4; r++) {
+                bool h0, h1;
+                const f2 G = gauss_weight2(qd[r], r2, h0, h1);   // G = 0 for a miss
+                I2[r] = fma2(bc(ga.w), G, I2[r]);
+                N2[r] = fma2(bc(gd4.w), G, N2[r]);  // gd4.w = v w
+                if (SETS) {
+                    const unsigned long long h = mix64(sid[j]);
+                    if (h0) { cnt[2 * r]++; hsum[2 * r] += h; hxor[2 * r] ^= h; }
+                    if (h1) { cnt[2 * r + 1]++; hsum[2 * r + 1] += h; hxor[2 * r + 1] ^= h; }
                 }
             }
         }
@@ -213,6 +216,9 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
     const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
     const bool vec2 = !SETS && !(bdx & 1u) && !o.gen.on && o.vec_ok;  // x-pairs are 8-byte aligned when the batch's x extent is even
     LossPartial lp;
+    float I[8], Nacc[8];
+#pragma unroll
+    for (int r = 0; r < 4; r++) { upk(I2[r], I[2 * r], I[2 * r + 1]); upk(N2[r], Nacc[2 * r], Nacc[2 * r + 1]); }
 #pragma unroll
     for (int r = 0; r < 4; r++) {  // the cell's four x-rows: (y, z) = (ly + (r & 1), lz + (r >> 1))
         const uint32_t y = (uint32_t)ly + (r & 1), z = (uint32_t)lz + (r >> 1);
@@ -238,7 +244,7 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
                 if (o.sample_err) *reinterpret_cast<float2 *>(o.sample_err + c) = make_float2(fabsf(r0), fabsf(r1));
                 if (o.pack2) {  // backward coefficients of the fused MSE: alpha = a / I, beta = -alpha Phi (eps = |alpha| P / 2)
                     const float a0 = cov[0] ? __fdividef(dscale * r0, Iv[0]) : 0.f, a1 = cov[1] ? __fdividef(dscale * r1, Iv[1]) : 0.f;
-                    *reinterpret_cast<float4 *>(o.pack2 + c) = make_float4(a0, -a0 * ph[0], a1, -a1 * ph[1]);
+                    *reinterpret_cast<float4 *>(o.pack2 + c) = make_float4(a0, a1, -a0 * ph[0], -a1 * ph[1]);   // pair layout, see pack2_index
                 }
             }
         } else {
@@ -257,7 +263,8 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
                     if (o.sample_err) o.sample_err[c + d] = fabsf(res);
                     if (o.pack2) {
                         const float al = cov[d] ? __fdividef(dscale * res, Iv[d]) : 0.f;
-                        o.pack2[c + d] = make_float2(al, -al * ph[d]);
+                        float *pk2 = reinterpret_cast<float *>(o.pack2) + pack2_index(c + d);
+                        pk2[0] = al; pk2[2] = -al * ph[d];
                     }
                 }
                 if (SETS) {
