@@ -160,6 +160,16 @@ def shard_workload(wl, rank: int, world: int):
     return [dict(xyz=np.ascontiguousarray(x[a:b]), target=np.ascontiguousarray(t[a:b])) for x, t in wl["batches"]], P_total
 
 
+# point queries: which acceleration mode each configuration runs in by default (the measured winner)
+POINTS_MODE_DEFAULT = {"c3": "gather", "c5": "gather"}
+
+
+def points_mode(wl, args):
+    if wl["kind"] != "points":
+        return None
+    return POINTS_MODE_DEFAULT.get(wl["name"], "gather") if args.points_accel == "default" else args.points_accel
+
+
 def config_of(wl) -> dict:
     """The `config` object: identical in the `ours` and the `reference` arm (no measured quantity in it)."""
     P = wl["grid"].num_points if wl["kind"] == "grid" else len(wl["batches"][0][0])
@@ -277,6 +287,9 @@ def measure(wl, args, sampler, world, rank, headline: bool):
 
     g = wl["g"]
     ctx = api.Context()
+    mode = points_mode(wl, args)
+    if mode is not None:
+        ctx.gs_set_option(api.OPT_POINTS_ACCEL, api.POINTS_SCATTER if mode == "scatter" else api.POINTS_GATHER)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     gd = [dev(a) for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
     # ---- this rank's share of the samples: same model everywhere, bricks / points are sharded
@@ -350,7 +363,7 @@ def measure(wl, args, sampler, world, rank, headline: bool):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / steps
-    out = {"config": config_of(wl), "steps": steps, "ms_per_step": ms_step, "value": P_total / (ms_step * 1e-3), "unit": "points/s",
+    out = {"config": config_of(wl), "points_accel": mode, "steps": steps, "ms_per_step": ms_step, "value": P_total / (ms_step * 1e-3), "unit": "points/s",
            "gpu_launches": launches, "clocks": sampler.window(w0, w1) if rank == 0 else None,
            "hit_pairs": hits, "tested_pairs": tested, "cull_efficiency": hits / tested if tested else None}
     per = {k: (stage_ms[k] / stage_calls[k] if stage_calls[k] else 0.0) for k in stage_ms}
@@ -551,6 +564,8 @@ def main():
     ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--points-accel", default="default", choices=["default", "gather", "scatter"],
+                    help="point queries: gather = LBVH over the Gaussians (north_star); scatter = the paper's tree over the samples")
     ap.add_argument("--record-traffic", nargs=3, metavar=("NCU_RAW_CSV", "WORKLOAD", "SOURCE"),
                     help="store dram bytes per launch of an `ncu --page raw --csv` export in profiles/traffic.json")
     args = ap.parse_args()

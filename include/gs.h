@@ -157,6 +157,21 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
 gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, float *phi, float *I, double *loss,
                         float *dL_dphi, float *sample_err);
 
+/* Context options.
+ * GS_OPT_POINTS_ACCEL selects how the NEXT gs_build_accel of a point query (and the forward / backward on it) works:
+ *   GS_POINTS_GATHER  (default; north_star (2)): LBVH over the Gaussians, per-packet traversal into cull lists, forward
+ *                     with lane = point, backward with lane = Gaussian.
+ *   GS_POINTS_SCATTER (the paper's own formulation, section 5.1, Fig. 7): a wide tree over the Morton-sorted
+ *                     SAMPLE POSITIONS, one warp per Gaussian walking it with the Gaussian's cutoff box; the forward adds
+ *                     (w G, v w G) to the samples with vector atomics and normalises in a second kernel; the backward
+ *                     keeps the 12 per-Gaussian sums in registers and writes one row per Gaussian (no atomics).
+ * Both modes decide membership with the same canonical predicate: ID sets are identical, values differ by summation
+ * order only.  The LBVH debug items (nodes, parents, boxes) exist in gather mode only.
+ * Errors: INVALID_ARG (unknown key / value). */
+typedef enum { GS_OPT_POINTS_ACCEL = 0 } gs_option;
+typedef enum { GS_POINTS_GATHER = 0, GS_POINTS_SCATTER = 1 } gs_points_accel;
+gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value);
+
 /* Sample-sharded (multi-GPU) use: the number of samples the fused MSE mean of gs_sample_fwd runs over (loss,
  * dL_dphi = 2 res / total, and the error statistic of the fused backward).  0 (the default) = the query's own P.
  * A rank that holds 1/R of the samples sets the global count, so that the per-rank losses and gradients ADD UP

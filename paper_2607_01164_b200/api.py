@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -79,6 +79,8 @@ class _AdamCfg(C.Structure):
 
 
 LOSS_MSE, LOSS_L1 = 0, 1
+OPT_POINTS_ACCEL = 0
+POINTS_GATHER, POINTS_SCATTER = 0, 1
 PAPER_LR = (0.00016, 0.001, 0.0001, 0.025, 0.0025)  # mean, scale, quat, opacity (weights), scalar (values): PAPER.md:231
 
 _lib = None
@@ -120,6 +122,7 @@ def load_library():
                                C.c_float, C.c_float, C.POINTER(C.c_uint32)]
     lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_set_sample_count.argtypes = [P, C.c_uint64]
+    lib.gs_set_option.argtypes = [P, C.c_int32, C.c_int64]
     lib.gs_status_query.argtypes = [P, C.POINTER(_StatusInfo)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
@@ -315,6 +318,9 @@ class Context:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b), C.byref(c)))
         return float(a.value), float(b.value), float(c.value)
+
+    def gs_set_option(self, key: int, value: int):
+        self._check(self.lib.gs_set_option(self.h, C.c_int32(int(key)), C.c_int64(int(value))))
 
     def gs_set_sample_count(self, total_samples: int):
         self._check(self.lib.gs_set_sample_count(self.h, C.c_uint64(int(total_samples))))

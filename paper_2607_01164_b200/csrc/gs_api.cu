@@ -150,7 +150,7 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
-                     &ctx->sel_val[0], &ctx->sel_val[1]};
+                     &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
@@ -278,10 +278,13 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         uint32_t *keys[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
         uint32_t *vals[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
         CK(radix_sort_pairs(keys, vals, N, 31, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "morton sort (gaussians)");
-        CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), ctx->rec.as<float4>(), N,
-                       ctx->node_left.as<int32_t>(), ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(),
-                       ctx->leaf_parent.as<int32_t>(), ctx->node_aabb.as<float>(),
-                       ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), ctx->sorted_rec.as<float4>(), s), "lbvh");
+        const bool scatter = ctx->opt_points_accel == GS_POINTS_SCATTER;
+        ctx->points_mode = ctx->opt_points_accel;
+        if (!scatter)   // the scatter mode only needs the Morton ORDER of the Gaussians (processing order), no tree over them
+            CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), ctx->rec.as<float4>(), N,
+                           ctx->node_left.as<int32_t>(), ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(),
+                           ctx->leaf_parent.as<int32_t>(), ctx->node_aabb.as<float>(),
+                           ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), ctx->sorted_rec.as<float4>(), s), "lbvh");
         // coherence sort of the queries
         ctx->have_pt_order = false;
         if (!q->presorted && P > 0) {
@@ -300,7 +303,16 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         // list chunks grows on demand: the kernel counts the chunks it needs, the host reads that count back (the one
         // device->host crossing of the unstructured path, like T of the structured path) and repeats the pass if it
         // did not fit.
-        if (P > 0) {
+        if (scatter) {
+            // the paper's structure: a wide tree over the SORTED SAMPLE POSITIONS, rebuilt per query
+            const uint64_t Ppad = scatter_padded_points(P ? P : 1);
+            const uint32_t nodes = scatter_tree_shape(P, &ctx->sc_tree);
+            CK(ctx->sc_spt.reserve(Ppad * 16), "alloc sorted points");
+            CK(ctx->sc_box.reserve((size_t)nodes * 24), "alloc point tree");
+            ctx->sc_tree.box = ctx->sc_box.as<float>();
+            CK(launch_scatter_build(q->xyz, ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->sc_tree,
+                                    ctx->sc_spt.as<float4>(), ctx->sc_box.as<float>(), s), "point tree");
+        } else if (P > 0) {
             Stage cull_stage(ctx, GS_PROF_CULL);
             const uint64_t packets = (P + 31) / 32;
             CK(ctx->cull_head.reserve(packets * 8), "alloc cull heads");
@@ -349,6 +361,13 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_gauss.as<uint32_t>(),
                            ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<float4>(), s), "grid forward");
+    } else if (ctx->points_mode == GS_POINTS_SCATTER) {
+        Stage stage(ctx, GS_PROF_FWD);
+        CK(ctx->sc_acc.reserve(scatter_padded_points(ctx->P ? ctx->P : 1) * 8), "alloc accumulators");
+        CK(launch_scatter_fwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), ctx->N, ctx->sc_tree,
+                              ctx->sc_spt.as<float4>(), ctx->sc_acc.as<float2>(),
+                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, o, s),
+           "points forward (scatter)");
     } else {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
@@ -459,6 +478,13 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused2, ctx->r2,
                            ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<float4>(), s), "grid backward");
+    } else if (ctx->points_mode == GS_POINTS_SCATTER) {
+        CK(ctx->sc_coef.reserve(scatter_padded_points(ctx->P ? ctx->P : 1) * 32), "alloc backward coefficients");
+        Stage stage(ctx, GS_PROF_BWD);
+        CK(launch_scatter_bwd(ctx->rec.as<float4>(), ctx->aabb.as<float>(), ctx->leaf_val[ctx->leaf_sel].as<uint32_t>(), N, ctx->sc_tree,
+                              ctx->sc_spt.as<float4>(), ctx->sc_coef.as<float4>(),
+                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, in,
+                              ctx->gacc.as<float>(), s), "points backward (scatter)");
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
@@ -479,6 +505,7 @@ gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *
     if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "nothing built yet");
     const size_t N = ctx->N;
     const bool grid = ctx->accel_kind == GS_QUERY_GRID, pts = ctx->accel_kind == GS_QUERY_POINTS;
+    const bool tree = pts && ctx->points_mode == GS_POINTS_GATHER;   // the scatter mode builds no tree over the Gaussians
     const size_t ni = N >= 1 ? N - 1 : 0;
     switch (what) {
         case GS_DBG_RECORDS: *dev_ptr = ctx->rec.p; *count = N; return GS_OK;
@@ -498,11 +525,11 @@ gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *
         case GS_DBG_BRICK_START: if (!grid) break; *dev_ptr = ctx->brick_start.p; *count = (size_t)ctx->nbricks + 1; return GS_OK;
         case GS_DBG_LEAF_MORTON: if (!pts) break; *dev_ptr = ctx->leaf_key[ctx->leaf_sel].p; *count = N; return GS_OK;
         case GS_DBG_LEAF_ORDER: if (!pts) break; *dev_ptr = ctx->leaf_val[ctx->leaf_sel].p; *count = N; return GS_OK;
-        case GS_DBG_NODE_LEFT: if (!pts) break; *dev_ptr = ctx->node_left.p; *count = ni; return GS_OK;
-        case GS_DBG_NODE_RIGHT: if (!pts) break; *dev_ptr = ctx->node_right.p; *count = ni; return GS_OK;
-        case GS_DBG_NODE_PARENT: if (!pts) break; *dev_ptr = ctx->node_parent.p; *count = ni; return GS_OK;
-        case GS_DBG_LEAF_PARENT: if (!pts) break; *dev_ptr = ctx->leaf_parent.p; *count = N; return GS_OK;
-        case GS_DBG_NODE_AABB: if (!pts) break; *dev_ptr = ctx->node_aabb.p; *count = ni; return GS_OK;
+        case GS_DBG_NODE_LEFT: if (!tree) break; *dev_ptr = ctx->node_left.p; *count = ni; return GS_OK;
+        case GS_DBG_NODE_RIGHT: if (!tree) break; *dev_ptr = ctx->node_right.p; *count = ni; return GS_OK;
+        case GS_DBG_NODE_PARENT: if (!tree) break; *dev_ptr = ctx->node_parent.p; *count = ni; return GS_OK;
+        case GS_DBG_LEAF_PARENT: if (!tree) break; *dev_ptr = ctx->leaf_parent.p; *count = N; return GS_OK;
+        case GS_DBG_NODE_AABB: if (!tree) break; *dev_ptr = ctx->node_aabb.p; *count = ni; return GS_OK;
         case GS_DBG_POINT_ORDER: if (!pts || !ctx->have_pt_order) break; *dev_ptr = ctx->pt_val[ctx->pt_sel].p; *count = ctx->P; return GS_OK;
         case GS_DBG_POINT_MORTON: if (!pts || !ctx->have_pt_order) break; *dev_ptr = ctx->pt_key[ctx->pt_sel].p; *count = ctx->P; return GS_OK;
         default: return fail(ctx, GS_ERR_INVALID_ARG, "unknown debug item");
@@ -652,6 +679,17 @@ gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2
     CK(ctx->dbg.reserve(64), "alloc scratch");
     CK(measure_alu_peaks(ctx->dbg.as<float>(), ctx->stream, ffma_per_s_host, ex2_per_s_host, ffma2_per_s_host), "alu peaks");
     return GS_OK;
+}
+
+gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value) {
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    switch (key) {
+        case GS_OPT_POINTS_ACCEL:
+            if (value != GS_POINTS_GATHER && value != GS_POINTS_SCATTER) return fail(ctx, GS_ERR_INVALID_ARG, "GS_OPT_POINTS_ACCEL: unknown mode");
+            ctx->opt_points_accel = (int)value;
+            return GS_OK;
+        default: return fail(ctx, GS_ERR_INVALID_ARG, "unknown option");
+    }
 }
 
 gs_status gs_set_sample_count(gs_ctx *ctx, uint64_t total_samples) {

@@ -46,6 +46,14 @@ struct GridDesc {          // one batch of a structured grid (gs_query, GS_QUERY
     unsigned long long jitter_seed;
 };
 
+// scatter mode of a point query (sample_scatter.cu): implicit 32-ary tree over the Morton-sorted query points
+struct PtTree {
+    const float *box;   // per level SoA boxes: box[off[l] + k * n[l] + i], k = lo.xyz hi.xyz
+    uint32_t off[8];    // in floats
+    uint32_t n[8];      // nodes per level (level 0 = leaves)
+    int levels;
+};
+
 // 30-bit Morton code of a position inside the domain box (D8): 10 bits per axis, x in the low bit,
 // q = (int) min(max((x - lo) * (1024 / (hi - lo)), 0), 1023) with the scale computed once on the host in fp32.
 struct MortonParams { float lo[3], scale[3]; };
@@ -128,6 +136,10 @@ struct gs_ctx {
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr;
+    int opt_points_accel = 0;   // gs_set_option(GS_OPT_POINTS_ACCEL): mode the NEXT point accel is built in
+    int points_mode = 0;        // mode of the current point accel (gs_points_accel)
+    gs::DevBuf sc_spt, sc_box, sc_acc, sc_coef;  // scatter mode: sorted positions, tree boxes, (I, Nacc) accumulators, backward coefficients
+    gs::PtTree sc_tree{};
     uint64_t sample_count = 0;  // gs_set_sample_count: samples the fused loss mean runs over (0 = the query's own P)
     // ---- measurement (gs_profile_*)
     unsigned long long launches = 0;  // kernels launched for this context since the last gs_profile_read
@@ -234,6 +246,15 @@ cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, cudaStream_t s);
 cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const FwdOut &o, cudaStream_t s);
+// scatter mode (the paper's formulation): see sample_scatter.cu
+uint64_t scatter_padded_points(uint64_t P);
+uint32_t scatter_tree_shape(uint64_t P, PtTree *T);
+cudaError_t launch_scatter_build(const float *xyz, const uint32_t *pt_order, uint64_t P, PtTree T, float4 *spt, float *box, cudaStream_t s);
+cudaError_t launch_scatter_fwd(const float4 *rec, const float *aabb, const uint32_t *gorder, uint32_t N, const PtTree &T, const float4 *spt,
+                               float2 *acc, const uint32_t *pt_order, uint64_t P, float tau, float r2, const FwdOut &o, cudaStream_t s);
+cudaError_t launch_scatter_bwd(const float4 *rec, const float *aabb, const uint32_t *gorder, uint32_t N, const PtTree &T, const float4 *spt,
+                               float4 *coef, const uint32_t *pt_order, uint64_t P, float tau, float r2, const BwdIn &in, float *gacc,
+                               cudaStream_t s);
 cudaError_t launch_points_bwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s);
 

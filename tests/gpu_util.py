@@ -15,7 +15,7 @@ class GpuRun:
     """One preprocess -> build -> fwd (fused MSE) -> bwd pass on the GPU; results as numpy arrays."""
 
     def __init__(self, g, query_kind, query_obj, target, domain=None, dL_dI=None, presorted=False, tau=TAU, fused=False,
-                 jitter_seed=None):
+                 jitter_seed=None, points_accel=None):
         """fused=True: gs_sample_bwd(dL_dphi=NULL), i.e. the backward of the forward's fused MSE loss."""
         import torch
         from paper_2607_01164_b200 import api
@@ -24,6 +24,8 @@ class GpuRun:
         self.ctx = api.Context()
         ctx = self.ctx
         self.dev = to_dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+        if points_accel is not None:   # gather (LBVH over the Gaussians) or scatter (the paper's tree over the samples)
+            ctx.gs_set_option(api.OPT_POINTS_ACCEL, points_accel)
         ctx.gs_preprocess(*self.dev, domain=domain, tau=tau)
         if query_kind == "grid":
             self.q = api.grid_query(query_obj, jitter_seed=jitter_seed)
