@@ -327,11 +327,12 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
                 CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
                 CK(launch_points_cull(ctx->sorted_rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), q->xyz,
                                       ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->dom, ctx->r,
-                                      cull_lists(ctx), ovf, s), "points cull");
+                                      cull_lists(ctx), ovf, ctx->cull_per_packet > 512.0 ? 2 : 4, s), "points cull");
                 uint32_t host[3] = {0, 0, 0};   // [0] stack overflow flag, [2] chunks requested
                 CK(cudaMemcpyAsync(host, ctx->counters.p, 12, cudaMemcpyDeviceToHost, s), "read cull counters");
                 CK(cudaStreamSynchronize(s), "sync");
                 if (host[0]) return fail(ctx, GS_ERR_OVERFLOW, "BVH traversal stack overflow");
+                ctx->cull_per_packet = 32.0 * (double)host[2] / (double)packets;
                 if (host[2] <= ctx->cull_cap) break;
                 if (attempt >= 2) return fail(ctx, GS_ERR_OVERFLOW, "cull list pool did not converge");
                 const uint64_t want = (uint64_t)host[2] + host[2] / 8 + 1024;

@@ -125,6 +125,7 @@ struct gs_ctx {
     gs::DevBuf sorted_rec; // float4 [N][4]: records in leaf order (id in plane c's .w)
     gs::DevBuf cull_ids, cull_link, cull_head;  // per-packet survivor lists (see CullLists)
     uint32_t cull_cap = 0;   // chunks the pool holds
+    double cull_per_packet = 0.0;   // list entries per packet of the last build (picks the cull kernel's group size)
     gs::DevBuf pt_key[2], pt_val[2];
     int pt_sel = 0;
     bool have_pt_order = false;
@@ -243,7 +244,8 @@ struct CullLists {
     uint32_t cap;
 };
 cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
-                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, cudaStream_t s);
+                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group /*2 or 4 packets per warp*/,
+                               cudaStream_t s);
 cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const FwdOut &o, cudaStream_t s);
 // scatter mode (the paper's formulation): see sample_scatter.cu

@@ -136,35 +136,97 @@ __device__ __forceinline__ void gather64(const float4 *__restrict__ base, uint32
 // ---------------------------------------------------------------------------------------------------------
 // k_points_cull: per-packet list of the Gaussians (sorted positions) whose cutoff ellipsoid can reach the packet.
 // List = chain of chunks: head[packet] = (first chunk, entries in it); every further chunk (link[chunk]) is full.
+// One warp serves a GROUP of CULL_GP consecutive packets (128 Morton-adjacent points): the tree is walked ONCE per group
+// with the group's two boxes -- the upper levels of the walk, a chain of dependent L2 round trips with a handful of busy
+// lanes, were half the kernel when every packet walked alone (configs[4]: 12 of 32 lanes busy per step) -- and the refine
+// stage tests every candidate against the boxes of each of the group's packets and feeds one survivor queue per packet.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *__restrict__ srt, uint32_t N, const float4 *__restrict__ nodes,
+#ifndef GS_CULL_MINB
+#define GS_CULL_MINB 6
+#endif
+// CULL_GP = packets per group (per warp): 4 when the lists are short (the walk dominates), 2 when they are long (the refine
+// stage, which tests every candidate against every packet of the group, dominates); chosen per build from the list sizes
+// of the previous step (launch_points_cull)
+template <int CULL_GP>
+__global__ void __launch_bounds__(CULL_WARPS * 32, GS_CULL_MINB) k_points_cull(const float4 *__restrict__ srt, uint32_t N, const float4 *__restrict__ nodes,
                                                                   const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
                                                                   uint64_t P, MortonParams mp, float rcut, CullLists o,
                                                                   uint32_t *__restrict__ overflow) {
     __shared__ int32_t stack_all[CULL_WARPS][STK_CAP];
     __shared__ uint32_t cand_all[CULL_WARPS][CQ_CAP];
-    __shared__ uint32_t surv_all[CULL_WARPS][64];
+    __shared__ uint32_t surv_all[CULL_WARPS][CULL_GP][64];
+    __shared__ CullBox cbox_all[CULL_WARPS][CULL_GP][2];                      // the two segment boxes of every packet of the group
     __shared__ float4 nbuf_all[CULL_WARPS][128], rbuf_all[CULL_WARPS][128];   // 32 nodes / 32 records of 64 B, swizzled
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint64_t packet = (uint64_t)blockIdx.x * CULL_WARPS + warp;
-    if (packet * 32 >= P) return;
+    const uint64_t npackets = (P + 31) / 32;
+    const uint64_t packet0 = ((uint64_t)blockIdx.x * CULL_WARPS + warp) * CULL_GP;   // first packet of this warp's group
+    if (packet0 >= npackets) return;
     int32_t *stack = stack_all[warp];
-    uint32_t *cand = cand_all[warp], *surv = surv_all[warp];
+    uint32_t *cand = cand_all[warp];
+    uint32_t (*surv)[64] = surv_all[warp];
+    CullBox (*cbox)[2] = cbox_all[warp];
     float4 *nbuf = nbuf_all[warp], *rbuf = rbuf_all[warp];
-    const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
-    PacketBox box0, box1;
-    CullBox cb0, cb1;
+    PacketBox box0, box1;   // the group's two boxes (the node tests of the walk)
     {
-        const uint32_t code = morton30(pp.px, pp.py, pp.pz, mp);
-        const uint32_t next = __shfl_down_sync(0xffffffffu, code, 1);
-        const uint32_t jump = (lane < 31 && (packet * 32 + lane + 1) < P) ? (code ^ next) : 0u;
-        const uint32_t top = __reduce_max_sync(0xffffffffu, jump);
-        const int cut = top ? __ffs(__ballot_sync(0xffffffffu, jump == top)) - 1 : 31;   // part 0 = lanes [0, cut], part 1 = the rest
-        segment_box(pp.px, pp.py, pp.pz, lane <= cut, box0, cb0);
-        segment_box(pp.px, pp.py, pp.pz, lane > cut, box1, cb1);
+        // Packets and the group are cut at their highest-level jump of the Z curve (largest code[i] ^ code[i + 1]): each part
+        // lies inside one Morton cell and gets its own box.
+        PacketPoint pp[CULL_GP];
+        uint32_t code[CULL_GP], gjump[CULL_GP];
+#pragma unroll
+        for (int g = 0; g < CULL_GP; g++) {
+            pp[g] = load_point(xyz, pt_order, P, packet0 + g, lane);
+            code[g] = morton30(pp[g].px, pp[g].py, pp[g].pz, mp);
+        }
+        uint32_t gtop = 0;
+#pragma unroll
+        for (int g = 0; g < CULL_GP; g++) {
+            const uint32_t next = __shfl_down_sync(0xffffffffu, code[g], 1);
+            const uint32_t jump = (lane < 31 && ((packet0 + g) * 32 + lane + 1) < P) ? (code[g] ^ next) : 0u;
+            const uint32_t top = __reduce_max_sync(0xffffffffu, jump);
+            const int cut = top ? __ffs(__ballot_sync(0xffffffffu, jump == top)) - 1 : 31;   // part 0 = lanes [0, cut], part 1 = the rest
+            PacketBox b;
+            CullBox c0, c1;
+            segment_box(pp[g].px, pp[g].py, pp[g].pz, lane <= cut, b, c0);
+            segment_box(pp[g].px, pp[g].py, pp[g].pz, lane > cut, b, c1);
+            if (lane == 0) { cbox[g][0] = c0; cbox[g][1] = c1; }
+            // jump to the first point of the next packet of the group (lane 31 only)
+            uint32_t across = 0u;
+            if (g + 1 < CULL_GP) {
+                const uint32_t first_next = __shfl_sync(0xffffffffu, code[g + 1 < CULL_GP ? g + 1 : g], 0);
+                if (lane == 31 && (packet0 + g + 1) * 32 < P) across = code[g] ^ first_next;
+            }
+            gjump[g] = lane == 31 ? across : jump;
+            gtop = max(gtop, __reduce_max_sync(0xffffffffu, gjump[g]));
+        }
+        // position (packet, lane) of the group's cut: the first occurrence of the largest jump
+        int cut_g = CULL_GP, cut_l = 31;
+#pragma unroll
+        for (int g = CULL_GP - 1; g >= 0; g--) {
+            const uint32_t hitm = __ballot_sync(0xffffffffu, gtop != 0u && gjump[g] == gtop);
+            if (hitm) { cut_g = g; cut_l = __ffs((int)hitm) - 1; }
+        }
+        const float nanv = __int_as_float(0x7fc00000);
+        float lo0[3] = {nanv, nanv, nanv}, hi0[3] = {nanv, nanv, nanv}, lo1[3] = {nanv, nanv, nanv}, hi1[3] = {nanv, nanv, nanv};
+#pragma unroll
+        for (int g = 0; g < CULL_GP; g++) {   // fminf / fmaxf drop NaN operands (inactive lanes, the other part)
+            const bool first = g < cut_g || (g == cut_g && lane <= cut_l);
+            const float p3[3] = {pp[g].px, pp[g].py, pp[g].pz};
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                lo0[k] = fminf(lo0[k], first ? p3[k] : nanv); hi0[k] = fmaxf(hi0[k], first ? p3[k] : nanv);
+                lo1[k] = fminf(lo1[k], first ? nanv : p3[k]); hi1[k] = fmaxf(hi1[k], first ? nanv : p3[k]);
+            }
+        }
+        box0.lx = warp_min(lo0[0]); box0.ly = warp_min(lo0[1]); box0.lz = warp_min(lo0[2]);
+        box0.hx = warp_max(hi0[0]); box0.hy = warp_max(hi0[1]); box0.hz = warp_max(hi0[2]);
+        box1.lx = warp_min(lo1[0]); box1.ly = warp_min(lo1[1]); box1.lz = warp_min(lo1[2]);
+        box1.hx = warp_max(hi1[0]); box1.hy = warp_max(hi1[1]); box1.hz = warp_max(hi1[2]);
     }
-    int sp = 0, cn = 0, sn = 0;   // stack entries, queued candidates, survivors not yet written (all warp-uniform)
-    uint32_t prev = NO_CHUNK;
+    int sp = 0, cn = 0;   // stack entries, queued candidates (warp-uniform)
+    int sn[CULL_GP];      // survivors of every packet not yet written
+    uint32_t prev[CULL_GP];
+#pragma unroll
+    for (int g = 0; g < CULL_GP; g++) { sn[g] = 0; prev[g] = NO_CHUNK; }
     if (N >= 2) { if (lane == 0) stack[0] = 0; sp = 1; }
     else if (N == 1) { if (lane == 0) cand[0] = 0u; cn = 1; }
     __syncwarp();
@@ -181,17 +243,20 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
         if (kB > 0) gather64(srt, pos, kB, rbuf, lane);
         cn -= kB;
         const bool drain = kA == 0 && kB == 0;   // => stack and queue are empty
-        // ---- write a full chunk of survivors while the loads are in flight
-        if (sn >= 32) {
-            uint32_t c = 0;
-            if (lane == 0) c = atomicAdd(o.top, 1u);
-            c = __shfl_sync(0xffffffffu, c, 0);
-            if (c < o.cap) {
-                o.ids[(size_t)c * 32 + lane] = surv[sn - 32 + lane];
-                if (lane == 0) o.link[c] = prev;
+        // ---- write full chunks of survivors while the loads are in flight
+#pragma unroll
+        for (int g = 0; g < CULL_GP; g++) {
+            if (sn[g] >= 32) {
+                uint32_t c = 0;
+                if (lane == 0) c = atomicAdd(o.top, 1u);
+                c = __shfl_sync(0xffffffffu, c, 0);
+                if (c < o.cap) {
+                    o.ids[(size_t)c * 32 + lane] = surv[g][sn[g] - 32 + lane];
+                    if (lane == 0) o.link[c] = prev[g];
+                }
+                prev[g] = c;
+                sn[g] -= 32;
             }
-            prev = c;
-            sn -= 32;
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
         __syncwarp();
@@ -223,45 +288,77 @@ __global__ void __launch_bounds__(CULL_WARPS * 32) k_points_cull(const float4 *_
             if (lr) cand[cn + nll + __popc(blr & lt)] = (uint32_t)~rc;
             cn += nll + __popc(blr);
         }
-        // ---- refine: consume the records
+        // ---- refine: consume the records; every packet of the group keeps the candidates that reach one of its two boxes
         if (kB > 0) {
-            bool keep = false;
+            Rec g;
             if (lane < kB) {
                 const int f = (lane >> 1) & 3;
-                Rec g;
                 g.a = rbuf[4 * lane + f]; g.b = rbuf[4 * lane + (1 ^ f)]; g.c = rbuf[4 * lane + (2 ^ f)]; g.d = rbuf[4 * lane + (3 ^ f)];
-                keep = ellipsoid_reaches(g, cb0, rcut) | ellipsoid_reaches(g, cb1, rcut);
+            } else {
+                const float nanv = __int_as_float(0x7fc00000);
+                g.a = g.b = g.c = g.d = make_float4(nanv, nanv, nanv, nanv);   // never reaches anything
             }
-            const uint32_t bk = __ballot_sync(0xffffffffu, keep);
-            if (keep) surv[sn + __popc(bk & lt)] = pos;
-            sn += __popc(bk);
+            // world half extents of the cutoff ellipsoid from the whitening matrix alone (rows m_j = R_j / s_j):
+            // e_k^2 = r^2 sum_j s_j^2 R_jk^2 = r^2 sum_j M_jk^2 / |m_j|^4, inflated (a cull only; the walk tested this box against
+            // the GROUP's boxes, here it is tested against each packet's own)
+            float ex, ey, ez;
+            {
+                const float n0 = fmaf(g.b.z, g.b.z, fmaf(g.b.y, g.b.y, g.b.x * g.b.x)), n1 = fmaf(g.c.z, g.c.z, fmaf(g.c.y, g.c.y, g.c.x * g.c.x)),
+                            n2 = fmaf(g.d.z, g.d.z, fmaf(g.d.y, g.d.y, g.d.x * g.d.x));
+                const float i0 = __frcp_rn(n0 * n0), i1 = __frcp_rn(n1 * n1), i2 = __frcp_rn(n2 * n2);
+                const float rr = rcut * 1.004f;
+                ex = rr * sqrtf(fmaf(g.d.x * g.d.x, i2, fmaf(g.c.x * g.c.x, i1, g.b.x * g.b.x * i0)));
+                ey = rr * sqrtf(fmaf(g.d.y * g.d.y, i2, fmaf(g.c.y * g.c.y, i1, g.b.y * g.b.y * i0)));
+                ez = rr * sqrtf(fmaf(g.d.z * g.d.z, i2, fmaf(g.c.z * g.c.z, i1, g.b.z * g.b.z * i0)));
+            }
+#pragma unroll
+            for (int q = 0; q < CULL_GP; q++) {
+                if (packet0 + q >= npackets) continue;   // warp-uniform
+                bool keep = false;
+#pragma unroll
+                for (int sgm = 0; sgm < 2; sgm++) {
+                    const CullBox cb = cbox[q][sgm];
+                    // !(x > y) keeps NaN (an infinite box / an overflowing extent culls nothing); a NaN box (empty part) fails the ellipsoid test
+                    const bool near = !(fabsf(cb.cx - g.a.x) > cb.hx + ex) & !(fabsf(cb.cy - g.a.y) > cb.hy + ey) & !(fabsf(cb.cz - g.a.z) > cb.hz + ez);
+                    keep |= near & ellipsoid_reaches(g, cb, rcut);
+                }
+                const uint32_t bk = __ballot_sync(0xffffffffu, keep);
+                if (keep) surv[q][sn[q] + __popc(bk & lt)] = pos;
+                sn[q] += __popc(bk);
+            }
         }
         __syncwarp();
         if (drain) break;
     }
-    // the remaining (< 32 ... or exactly 32 from the last round) survivors: at most two more chunks; the last one written is the head
-    uint32_t head_cnt = prev == NO_CHUNK ? 0u : 32u;
-    while (sn > 0) {
-        const int k = min(sn, 32);
-        uint32_t c = 0;
-        if (lane == 0) c = atomicAdd(o.top, 1u);
-        c = __shfl_sync(0xffffffffu, c, 0);
-        if (c < o.cap) {
-            // a partial chunk must be the head (every linked chunk is full): write the full one first
-            if (lane < k) o.ids[(size_t)c * 32 + lane] = surv[(sn > 32 ? 0 : sn - k) + lane];
-            if (lane == 0) o.link[c] = prev;
+    // the remaining (< 32 ... or exactly 32 from the last round) survivors: at most two more chunks per packet; the last one
+    // written is the head
+#pragma unroll
+    for (int g = 0; g < CULL_GP; g++) {
+        if (packet0 + g >= npackets) continue;
+        uint32_t head_cnt = prev[g] == NO_CHUNK ? 0u : 32u;
+        int n = sn[g];
+        while (n > 0) {
+            const int k = min(n, 32);
+            uint32_t c = 0;
+            if (lane == 0) c = atomicAdd(o.top, 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c < o.cap) {
+                // a partial chunk must be the head (every linked chunk is full): write the full one first
+                if (lane < k) o.ids[(size_t)c * 32 + lane] = surv[g][(n > 32 ? 0 : n - k) + lane];
+                if (lane == 0) o.link[c] = prev[g];
+            }
+            prev[g] = c;
+            head_cnt = (uint32_t)k;
+            if (n > 32) {   // 32 < n < 64: entries [0, 32) went out as a full chunk, move the tail down
+                const uint32_t t = lane < n - 32 ? surv[g][32 + lane] : 0u;
+                __syncwarp();
+                if (lane < n - 32) surv[g][lane] = t;
+                __syncwarp();
+            }
+            n -= k;
         }
-        prev = c;
-        head_cnt = (uint32_t)k;
-        if (sn > 32) {   // 32 < sn < 64: entries [0, 32) went out as a full chunk, move the tail down
-            const uint32_t t = lane < sn - 32 ? surv[32 + lane] : 0u;
-            __syncwarp();
-            if (lane < sn - 32) surv[lane] = t;
-            __syncwarp();
-        }
-        sn -= k;
+        if (lane == 0) o.head[packet0 + g] = make_uint2(prev[g], head_cnt);
     }
-    if (lane == 0) o.head[packet] = make_uint2(prev, head_cnt);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -506,13 +603,15 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
 }
 
 cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
-                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, cudaStream_t s) {
+                               uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group,
+                               cudaStream_t s) {
     if (P == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(lists.top, 0, sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
-    const uint64_t packets = (P + 31) / 32;
-    const unsigned blocks = (unsigned)((packets + CULL_WARPS - 1) / CULL_WARPS);
-    k_points_cull<<<blocks, CULL_WARPS * 32, 0, s>>>(sorted_rec, N, nodes, xyz, pt_order, P, morton_params(dom), rcut, lists, overflow);
+    const uint64_t packets = (P + 31) / 32, groups = (packets + group - 1) / group;
+    const unsigned blocks = (unsigned)((groups + CULL_WARPS - 1) / CULL_WARPS);
+    if (group == 2) k_points_cull<2><<<blocks, CULL_WARPS * 32, 0, s>>>(sorted_rec, N, nodes, xyz, pt_order, P, morton_params(dom), rcut, lists, overflow);
+    else k_points_cull<4><<<blocks, CULL_WARPS * 32, 0, s>>>(sorted_rec, N, nodes, xyz, pt_order, P, morton_params(dom), rcut, lists, overflow);
     count_launch();
     return cudaGetLastError();
 }
