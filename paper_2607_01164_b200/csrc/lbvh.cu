@@ -4,8 +4,8 @@
 //   k_morton      : 30-bit Morton code of a position inside the domain box (D8), x in the low bit
 //   (radix sort)  : stable sort of (code, id) => order by the unique 64-bit key (code << 32 | id)
 //   k_karras      : binary radix tree, one thread per internal node (Karras 2012)
-//   k_refit       : bottom-up exact min/max boxes with per-node arrival counters
-//   k_pack_nodes  : 64-byte traversal nodes holding both children's boxes and links
+//   k_refit       : bottom-up exact min/max boxes with per-node arrival counters; the thread that completes a node also
+//                   writes its 64-byte traversal record (both children's boxes and links)
 //   k_sort_records: the Gaussian records in leaf order, 64 contiguous bytes each (neighbouring leaves are
 //                   neighbouring in memory; a record is two full 32-byte sectors)
 #include "gs_internal.cuh"
@@ -72,15 +72,21 @@ __global__ void __launch_bounds__(256) k_karras(const uint32_t *__restrict__ cod
     if (i == 0) parent[0] = -1;
 }
 
+// a 24-byte box is 8-byte aligned: three 8-byte loads / stores (L2: written by other threads of this launch)
 __device__ __forceinline__ void load_box(const float *p, float (&b)[6]) {
-#pragma unroll
-    for (int k = 0; k < 6; k++) b[k] = __ldcg(p + k);  // L2: written by other threads of this launch
+    const float2 *q = reinterpret_cast<const float2 *>(p);
+    const float2 a0 = __ldcg(q), a1 = __ldcg(q + 1), a2 = __ldcg(q + 2);
+    b[0] = a0.x; b[1] = a0.y; b[2] = a1.x; b[3] = a1.y; b[4] = a2.x; b[5] = a2.y;
 }
 
+// Bottom-up refit: the thread that arrives second at a node has both children complete; it unites their boxes, writes the
+// node's box (read by the parent and by the debug view) AND the node's 64-byte traversal record:
+//   [0] l.lo.xyz l.hi.x | [1] l.hi.yz r.lo.xy | [2] r.lo.z r.hi.xyz | [3] left, right (bits), -, -
+// child link >= 0: internal node; < 0: ~(sorted position of the leaf), which indexes the sorted records directly
 __global__ void __launch_bounds__(256) k_refit(const uint32_t *__restrict__ ids, const float *__restrict__ aabb, int n,
                                                 const int32_t *__restrict__ left, const int32_t *__restrict__ right,
                                                 const int32_t *__restrict__ parent, const int32_t *__restrict__ leaf_parent,
-                                                float *__restrict__ node_aabb, uint32_t *__restrict__ flags) {
+                                                float *__restrict__ node_aabb, uint32_t *__restrict__ flags, float4 *__restrict__ packed) {
     const int leaf = blockIdx.x * blockDim.x + threadIdx.x;
     if (leaf >= n) return;
     int node = leaf_parent[leaf];
@@ -91,30 +97,17 @@ __global__ void __launch_bounds__(256) k_refit(const uint32_t *__restrict__ ids,
         const int l = left[node], r = right[node];
         load_box(l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l, a);
         load_box(r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r, b);
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
-            __stcg(node_aabb + 6 * (size_t)node + k, fminf(a[k], b[k]));
-            __stcg(node_aabb + 6 * (size_t)node + 3 + k, fmaxf(a[3 + k], b[3 + k]));
-        }
+        float2 *out = reinterpret_cast<float2 *>(node_aabb + 6 * (size_t)node);
+        __stcg(out, make_float2(fminf(a[0], b[0]), fminf(a[1], b[1])));
+        __stcg(out + 1, make_float2(fminf(a[2], b[2]), fmaxf(a[3], b[3])));
+        __stcg(out + 2, make_float2(fmaxf(a[4], b[4]), fmaxf(a[5], b[5])));
+        packed[4 * (size_t)node + 0] = make_float4(a[0], a[1], a[2], a[3]);
+        packed[4 * (size_t)node + 1] = make_float4(a[4], a[5], b[0], b[1]);
+        packed[4 * (size_t)node + 2] = make_float4(b[2], b[3], b[4], b[5]);
+        packed[4 * (size_t)node + 3] = make_float4(__int_as_float(l), __int_as_float(r), 0.f, 0.f);
         __threadfence();
         node = parent[node];
     }
-}
-
-// traversal node (64 B): [0] l.lo.xyz l.hi.x | [1] l.hi.yz r.lo.xy | [2] r.lo.z r.hi.xyz | [3] left, right (bits), -, -
-// child link >= 0: internal node; < 0: ~(sorted position of the leaf), which indexes the sorted records directly
-__global__ void __launch_bounds__(256) k_pack_nodes(const uint32_t *__restrict__ ids, const float *__restrict__ aabb, int n,
-                                                     const int32_t *__restrict__ left, const int32_t *__restrict__ right,
-                                                     const float *__restrict__ node_aabb, float4 *__restrict__ packed) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n - 1) return;
-    const int l = left[i], r = right[i];
-    const float *a = l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l;
-    const float *b = r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r;
-    packed[4 * (size_t)i + 0] = make_float4(a[0], a[1], a[2], a[3]);
-    packed[4 * (size_t)i + 1] = make_float4(a[4], a[5], b[0], b[1]);
-    packed[4 * (size_t)i + 2] = make_float4(b[2], b[3], b[4], b[5]);
-    packed[4 * (size_t)i + 3] = make_float4(__int_as_float(l), __int_as_float(r), 0.f, 0.f);
 }
 
 // records in leaf order: sorted[4 k .. 4 k + 3] = planes a, b, c, d of Gaussian ids[k], with the id in c.w
@@ -141,8 +134,7 @@ cudaError_t launch_lbvh(const uint32_t *codes, const uint32_t *ids, const float 
     cudaError_t e = cudaMemsetAsync(flags, 0, sizeof(uint32_t) * (N - 1), s);
     if (e != cudaSuccess) return e;
     k_karras<<<(n - 1 + 255) / 256, 256, 0, s>>>(codes, ids, n, left, right, parent, leaf_parent); count_launch();
-    k_refit<<<(n + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, parent, leaf_parent, node_aabb, flags); count_launch();
-    k_pack_nodes<<<(n - 1 + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, node_aabb, packed); count_launch();
+    k_refit<<<(n + 255) / 256, 256, 0, s>>>(ids, aabb, n, left, right, parent, leaf_parent, node_aabb, flags, packed); count_launch();
     return cudaGetLastError();
 }
 

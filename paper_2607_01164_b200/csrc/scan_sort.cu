@@ -107,6 +107,19 @@ constexpr int SORT_ROUNDS = 16;
 constexpr int SORT_SEG = 32 * SORT_ROUNDS;            // 512 items per warp
 constexpr int SORT_TILE = SORT_WARPS * SORT_SEG;      // 4096 items per block
 constexpr int RADIX = 256;
+static_assert(SORT_WARPS * 32 == RADIX, "k_sort_scatter: one thread per digit");
+
+// lanes holding the same 8-bit digit as this one (inactive lanes pass d = 0xffffffff and are excluded by `ok`): eight ballots,
+// one per digit bit -- a fixed 16 instructions where match.any.sync iterates over the distinct values of the warp
+__device__ __forceinline__ uint32_t digit_peers(uint32_t d, bool ok) {
+    uint32_t peers = __ballot_sync(0xffffffffu, ok);
+#pragma unroll
+    for (int b = 0; b < 8; b++) {
+        const uint32_t bal = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+        peers &= ((d >> b) & 1u) ? bal : ~bal;
+    }
+    return peers;
+}
 
 // per-warp digit histogram of its segment into smem wh[warp][256] (no atomics: one warp owns a row)
 __device__ __forceinline__ void warp_histogram(const uint32_t *__restrict__ keys, size_t n, size_t seg_base, int shift, uint32_t mask,
@@ -118,39 +131,57 @@ __device__ __forceinline__ void warp_histogram(const uint32_t *__restrict__ keys
         const size_t idx = seg_base + (size_t)r * 32 + lane;
         const bool ok = idx < n;
         const uint32_t d = ok ? ((keys[idx] >> shift) & mask) : 0xffffffffu;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t peers = digit_peers(d, ok);
         if (ok && (int)(__ffs(peers) - 1) == lane) wh[d] += __popc(peers);
         __syncwarp();
     }
 }
 
+// per-tile digit counts: shared-memory atomics (a count needs no order)
 __global__ void __launch_bounds__(SORT_WARPS * 32) k_sort_hist(const uint32_t *__restrict__ keys, size_t n, int shift, uint32_t mask,
                                                                 uint32_t *__restrict__ hist /*[256][ntiles]*/, uint32_t ntiles) {
-    __shared__ uint32_t wh[SORT_WARPS][RADIX];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const size_t seg_base = (size_t)blockIdx.x * SORT_TILE + (size_t)warp * SORT_SEG;
-    warp_histogram(keys, n, seg_base, shift, mask, wh[warp], lane);
+    __shared__ uint32_t sh[RADIX];
+    for (int d = threadIdx.x; d < RADIX; d += blockDim.x) sh[d] = 0;
     __syncthreads();
-    for (int d = threadIdx.x; d < RADIX; d += blockDim.x) {
-        uint32_t s = 0;
-#pragma unroll
-        for (int w = 0; w < SORT_WARPS; w++) s += wh[w][d];
-        hist[(size_t)d * ntiles + blockIdx.x] = s;
+    const size_t base = (size_t)blockIdx.x * SORT_TILE;
+#pragma unroll 4
+    for (int r = 0; r < SORT_TILE / (SORT_WARPS * 32); r++) {
+        const size_t idx = base + (size_t)r * (SORT_WARPS * 32) + threadIdx.x;
+        if (idx < n) atomicAdd(&sh[(keys[idx] >> shift) & mask], 1u);
     }
+    __syncthreads();
+    for (int d = threadIdx.x; d < RADIX; d += blockDim.x) hist[(size_t)d * ntiles + blockIdx.x] = sh[d];
 }
 
+// Stable scatter of one tile.  The rank of an item inside the tile is (items of smaller digits) + (items of its digit in
+// earlier warps) + (earlier items of its digit in its own warp: __match_any_sync ranking, order (round, lane)).  The tile is
+// first permuted into that order in shared memory and then written out slot by slot, so that consecutive threads write
+// consecutive addresses of a digit's run (a direct scatter wrote 4 bytes per 32-byte sector).
 __global__ void __launch_bounds__(SORT_WARPS * 32) k_sort_scatter(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ vals,
                                                                    uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
                                                                    size_t n, int shift, uint32_t mask,
                                                                    const uint32_t *__restrict__ hist_scanned, uint32_t ntiles) {
     __shared__ uint32_t wh[SORT_WARPS][RADIX];
+    __shared__ uint32_t tstart[RADIX];   // first slot of the digit's run inside the tile
+    __shared__ uint32_t gbase[RADIX];    // global position of that slot
+    __shared__ uint32_t skey[SORT_TILE], sval[SORT_TILE];
+    __shared__ uint32_t scan_sm[40];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const size_t seg_base = (size_t)blockIdx.x * SORT_TILE + (size_t)warp * SORT_SEG;
+    const size_t tile_base = (size_t)blockIdx.x * SORT_TILE;
+    const size_t seg_base = tile_base + (size_t)warp * SORT_SEG;
     warp_histogram(keys, n, seg_base, shift, mask, wh[warp], lane);
     __syncthreads();
-    // per digit: global base of this tile + exclusive prefix over the warps of the tile
-    for (int d = threadIdx.x; d < RADIX; d += blockDim.x) {
-        uint32_t run = hist_scanned[(size_t)d * ntiles + blockIdx.x];
+    // per digit (thread d, RADIX == blockDim): tile count -> exclusive scan over the digits = run starts; per-warp offsets
+    {
+        const int d = threadIdx.x;
+        uint32_t cnt = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; w++) cnt += wh[w][d];
+        uint32_t total;
+        const uint32_t start = block_excl_scan(cnt, &total, scan_sm);
+        tstart[d] = start;
+        gbase[d] = hist_scanned[(size_t)d * ntiles + blockIdx.x];
+        uint32_t run = start;
 #pragma unroll
         for (int w = 0; w < SORT_WARPS; w++) {
             const uint32_t c = wh[w][d];
@@ -166,16 +197,25 @@ __global__ void __launch_bounds__(SORT_WARPS * 32) k_sort_scatter(const uint32_t
         const bool ok = idx < n;
         const uint32_t k = ok ? keys[idx] : 0u;
         const uint32_t d = ok ? ((k >> shift) & mask) : 0xffffffffu;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        uint32_t pos = 0;
-        if (ok) pos = base[d] + __popc(peers & ((1u << lane) - 1u));
+        const uint32_t peers = digit_peers(d, ok);
+        uint32_t slot = 0;
+        if (ok) slot = base[d] + __popc(peers & ((1u << lane) - 1u));
         __syncwarp();
         if (ok && (int)(__ffs(peers) - 1) == lane) base[d] += __popc(peers);
         __syncwarp();
         if (ok) {
-            keys_out[pos] = k;
-            vals_out[pos] = vals[idx];
+            skey[slot] = k;
+            sval[slot] = vals[idx];
         }
+    }
+    __syncthreads();
+    const uint32_t count = (uint32_t)(n - tile_base < (size_t)SORT_TILE ? n - tile_base : (size_t)SORT_TILE);
+    for (uint32_t i = threadIdx.x; i < count; i += SORT_WARPS * 32) {
+        const uint32_t k = skey[i];
+        const uint32_t d = (k >> shift) & mask;
+        const uint32_t dst = gbase[d] + (i - tstart[d]);
+        keys_out[dst] = k;
+        vals_out[dst] = sval[i];
     }
 }
 
