@@ -323,3 +323,44 @@ def points_domain(xyz: np.ndarray):
     lo = xyz.min(axis=0).astype(F32)
     hi = np.nextafter(xyz.max(axis=0).astype(F32), F32(np.inf))
     return lo, hi
+
+
+# ----------------------------------------------------------------------------------------
+# Rays and transfer functions for the volume-rendering consumer of the sampler
+# ----------------------------------------------------------------------------------------
+def camera_rays(width: int, height: int, eye, look_at, up=(0.0, 0.0, 1.0), fov_y_deg: float = 40.0,
+                box=((0.0, 0.0, 0.0), (1.0, 1.0, 1.0))):
+    """Pinhole-camera rays through the pixel centres, clipped to an axis-aligned box (slab test).
+    Returns origins [n,3], unit directions [n,3], t_range [n,2] (t_near, t_far; t_far <= t_near for a ray that misses the
+    box), all float32, row-major over (y, x).  Input preparation only: the renderer and its oracle both take these arrays."""
+    eye = np.asarray(eye, np.float64)
+    f = np.asarray(look_at, np.float64) - eye
+    f /= np.linalg.norm(f)
+    r = np.cross(f, np.asarray(up, np.float64))
+    r /= np.linalg.norm(r)
+    u = np.cross(r, f)
+    ty = np.tan(np.radians(fov_y_deg) / 2.0)
+    tx = ty * width / height
+    xs = (2.0 * (np.arange(width) + 0.5) / width - 1.0) * tx
+    ys = (1.0 - 2.0 * (np.arange(height) + 0.5) / height) * ty
+    d = f[None, None, :] + xs[None, :, None] * r[None, None, :] + ys[:, None, None] * u[None, None, :]
+    d /= np.linalg.norm(d, axis=2, keepdims=True)
+    d = d.reshape(-1, 3)
+    o = np.broadcast_to(eye, d.shape)
+    lo, hi = np.asarray(box[0], np.float64), np.asarray(box[1], np.float64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t1 = (lo - o) / d
+        t2 = (hi - o) / d
+    tn = np.nanmax(np.minimum(t1, t2), axis=1)
+    tf = np.nanmin(np.maximum(t1, t2), axis=1)
+    tn = np.maximum(tn, 0.0)
+    return o.astype(F32), d.astype(F32), np.stack([tn, tf], axis=1).astype(F32)
+
+
+def diverging_transfer(k: int = 256, extinction: float = 40.0) -> np.ndarray:
+    """A transfer function table [k,4] float32: a blue-white-red diverging colour ramp (in the spirit of the "coolwarm" map
+    the paper renders with) and a LINEAR opacity map (extinction per unit length = extinction * value)."""
+    x = np.linspace(0.0, 1.0, k)
+    cold, mid, warm = np.array([0.23, 0.30, 0.75]), np.array([0.87, 0.87, 0.87]), np.array([0.71, 0.02, 0.15])
+    rgb = np.where(x[:, None] < 0.5, cold + (mid - cold) * (2 * x[:, None]), mid + (warm - mid) * (2 * x[:, None] - 1))
+    return np.concatenate([rgb, (extinction * x)[:, None]], axis=1).astype(F32)
