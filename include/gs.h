@@ -341,6 +341,22 @@ typedef struct gs_status_info {
 } gs_status_info;
 gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host);
 
+/* ---- volume rendering over the sampler (Fig. 1, Fig. 9) ---------------
+ * Emission-absorption ray marching of the current model (the one given to the last gs_preprocess, which must have had a
+ * domain): every ray r takes spp samples at t_k = t_near + (k + 1/2) dt, dt = (t_far - t_near) / spp, p = o + t_k d
+ * (float32: dt = (t1 - t0) / spp; t_k = fmaf((float)k + 0.5f, dt, t0); p = fmaf(t_k, d, o), DESIGN D27), evaluates the model
+ * there with the point-query forward of this library, and composites front to back
+ *     alpha_k = I_k > tau ? 1 - exp(-sigma(Phi_k) dt) : 0;   C += T alpha_k rgb(Phi_k);   T *= 1 - alpha_k
+ * A sample the model does not cover (I <= tau) is empty space: the model's own domain test, no
+ * surface mesh.  (rgb, sigma)(x) = linear interpolation of table[table_size][4] over x = clamp(Phi, 0, 1).
+ * All pointers are DEVICE memory: origins[n,3], dirs[n,3], t_range[n,2] (a ray with t_far <= t_near sees nothing),
+ * table (16-byte aligned), rgba[n,4] (16-byte aligned; OVERWRITTEN with (C, 1 - T)).  Rays are processed in chunks of
+ * <= 2^24 samples; each chunk rebuilds the point acceleration structure in the mode of GS_OPT_POINTS_ACCEL, so a
+ * caller's own accel is invalid afterwards (gs_build_accel again).  No window, swapchain or graphics API is involved:
+ * the image is the rgba buffer.  Errors: STATE (no preprocess / no domain), INVALID_ARG, OOM, OVERFLOW, CUDA. */
+gs_status gs_render(gs_ctx *ctx, uint32_t num_rays, const float *origins, const float *dirs, const float *t_range, uint32_t spp,
+                    const float *table, uint32_t table_size, float *rgba);
+
 /* ---- measurement: CUDA-event timing of the stages, on the context's stream --------------------
  * While enabled, every stage of the calls above is bracketed by a pair of CUDA events recorded on
  * the context's stream.  gs_profile_read synchronises the stream, adds up the elapsed time of all

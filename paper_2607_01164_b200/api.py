@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -123,6 +123,7 @@ def load_library():
     lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_set_sample_count.argtypes = [P, C.c_uint64]
     lib.gs_set_option.argtypes = [P, C.c_int32, C.c_int64]
+    lib.gs_render.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, C.c_uint32, P]
     lib.gs_status_query.argtypes = [P, C.POINTER(_StatusInfo)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
@@ -318,6 +319,11 @@ class Context:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b), C.byref(c)))
         return float(a.value), float(b.value), float(c.value)
+
+    def gs_render(self, origins, dirs, t_range, spp: int, table, rgba):
+        """Ray-march the current model (gs.h gs_render): device tensors origins/dirs [n,3], t_range [n,2], table [K,4], rgba [n,4]."""
+        self._check(self.lib.gs_render(self.h, C.c_uint32(int(origins.shape[0])), _ptr(origins), _ptr(dirs), _ptr(t_range),
+                                       C.c_uint32(int(spp)), _ptr(table), C.c_uint32(int(table.shape[0])), _ptr(rgba)))
 
     def gs_set_option(self, key: int, value: int):
         self._check(self.lib.gs_set_option(self.h, C.c_int32(int(key)), C.c_int64(int(value))))

@@ -150,7 +150,7 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
-                     &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef};
+                     &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef, &ctx->rn_xyz, &ctx->rn_phi, &ctx->rn_I};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
@@ -679,6 +679,42 @@ gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     CK(ctx->dbg.reserve(64), "alloc scratch");
     CK(measure_alu_peaks(ctx->dbg.as<float>(), ctx->stream, ffma_per_s_host, ex2_per_s_host, ffma2_per_s_host), "alu peaks");
+    return GS_OK;
+}
+
+gs_status gs_render(gs_ctx *ctx, uint32_t num_rays, const float *origins, const float *dirs, const float *t_range, uint32_t spp,
+                    const float *table, uint32_t table_size, float *rgba) {
+    LaunchScope launch_scope(ctx);
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "gs_render before gs_preprocess");
+    if (!ctx->have_dom) return fail(ctx, GS_ERR_STATE, "gs_render needs the domain given to gs_preprocess");
+    if (num_rays > 0 && (!origins || !dirs || !t_range || !rgba)) return fail(ctx, GS_ERR_INVALID_ARG, "gs_render: null pointer");
+    if (spp == 0 || spp > 65535u || !table || table_size < 2) return fail(ctx, GS_ERR_INVALID_ARG, "gs_render: spp in [1, 65535], table of >= 2 entries");
+    if (((uintptr_t)table | (uintptr_t)rgba) & 15) return fail(ctx, GS_ERR_INVALID_ARG, "gs_render: table and rgba must be 16-byte aligned");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    // chunks of rays whose samples fit one point query of <= 2^24 points
+    const uint32_t chunk_rays = (1u << 24) / spp ? (1u << 24) / spp : 1u;
+    for (uint32_t r0 = 0; r0 < num_rays; r0 += chunk_rays) {
+        const uint32_t nr = num_rays - r0 < chunk_rays ? num_rays - r0 : chunk_rays;
+        const size_t ns = (size_t)nr * spp;
+        CK(ctx->rn_xyz.reserve(ns * 12), "alloc ray samples");
+        CK(ctx->rn_phi.reserve(ns * 4), "alloc ray samples");
+        CK(ctx->rn_I.reserve(ns * 4), "alloc ray samples");
+        CK(launch_ray_samples(origins + 3 * (size_t)r0, dirs + 3 * (size_t)r0, t_range + 2 * (size_t)r0, nr, spp, ctx->rn_xyz.as<float>(), s),
+           "ray samples");
+        gs_query q{};
+        q.kind = GS_QUERY_POINTS;
+        q.num_points = ns;
+        q.xyz = ctx->rn_xyz.as<float>();
+        gs_status st = gs_build_accel(ctx, &q);
+        if (st != GS_OK) return st;
+        st = gs_sample_fwd(ctx, &q, nullptr, ctx->rn_phi.as<float>(), ctx->rn_I.as<float>(), nullptr, nullptr, nullptr);
+        if (st != GS_OK) return st;
+        CK(launch_composite(ctx->rn_phi.as<float>(), ctx->rn_I.as<float>(), t_range + 2 * (size_t)r0, nr, spp, ctx->tau,
+                            reinterpret_cast<const float4 *>(table), table_size, reinterpret_cast<float4 *>(rgba) + r0, s), "composite");
+    }
+    ctx->accel_kind = -1;   // the accel now belongs to the last chunk of ray samples, not to a query of the caller
     return GS_OK;
 }
 

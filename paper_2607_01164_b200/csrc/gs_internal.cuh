@@ -134,6 +134,7 @@ struct gs_ctx {
     gs::DevBuf dens_work, dens_scratch, sel_key[2], sel_val[2];  // gs_prune / gs_densify
     int fused_pack = 0;  // misc holds backward coefficients written by the last forward: 1 = float2 (alpha, beta) of gs_sample_fwd's
                          // fused MSE, 2 = float4 (alpha, beta, eps, -) of gs_sample_fwd_loss on a grid; 0 = none
+    gs::DevBuf rn_xyz, rn_phi, rn_I;   // gs_render: samples of a chunk of rays
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr;
@@ -225,6 +226,12 @@ cudaError_t launch_select_keys(const float *err, const float *I, const uint8_t *
 cudaError_t launch_new_gaussians(const gs_raw_params &p, float *m, float *v, uint32_t n_new, const uint32_t *sel, const GridDesc &gd,
                                  const float4 *jit, const float *xyz, const float *target, float raw_scale_init, float raw_opacity_init, float clamp,
                                  float *scratch, cudaStream_t s);
+
+// render.cu: samples of a chunk of rays (sample-major: sample k of ray r at k * nrays + r) and their compositing
+cudaError_t launch_ray_samples(const float *org, const float *dir, const float *trange, uint32_t nrays, uint32_t spp, float *xyz,
+                               cudaStream_t s);
+cudaError_t launch_composite(const float *phi, const float *I, const float *trange, uint32_t nrays, uint32_t spp, float tau,
+                             const float4 *table, uint32_t K, float4 *rgba, cudaStream_t s);
 
 // peaks.cu: FP32 FMA and MUFU.EX2 lane-instructions per second (register-only loops, CUDA events on `s`; synchronises)
 cudaError_t measure_alu_peaks(float *sink, cudaStream_t s, double *ffma_per_s, double *ex2_per_s, double *ffma2_per_s);

@@ -354,7 +354,7 @@ def camera_rays(width: int, height: int, eye, look_at, up=(0.0, 0.0, 1.0), fov_y
     tn = np.nanmax(np.minimum(t1, t2), axis=1)
     tf = np.nanmin(np.maximum(t1, t2), axis=1)
     tn = np.maximum(tn, 0.0)
-    return o.astype(F32), d.astype(F32), np.stack([tn, tf], axis=1).astype(F32)
+    return np.ascontiguousarray(o, F32), np.ascontiguousarray(d, F32), np.ascontiguousarray(np.stack([tn, tf], axis=1), F32)
 
 
 def diverging_transfer(k: int = 256, extinction: float = 40.0) -> np.ndarray:
