@@ -290,6 +290,8 @@ def measure(wl, args, sampler, world, rank, headline: bool):
     mode = points_mode(wl, args)
     if mode is not None:
         ctx.gs_set_option(api.OPT_POINTS_ACCEL, api.POINTS_SCATTER if mode == "scatter" else api.POINTS_GATHER)
+    if wl["kind"] == "grid" and not args.sync_build:
+        ctx.gs_set_option(api.OPT_ASYNC_BUILD, 1)   # steady-state builds without a host round trip (gs.h)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     gd = [dev(a) for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
     # ---- this rank's share of the samples: same model everywhere, bricks / points are sharded
@@ -363,7 +365,7 @@ def measure(wl, args, sampler, world, rank, headline: bool):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / steps
-    out = {"config": config_of(wl), "points_accel": mode, "steps": steps, "ms_per_step": ms_step, "value": P_total / (ms_step * 1e-3), "unit": "points/s",
+    out = {"config": config_of(wl), "points_accel": mode, "async_build": bool(wl["kind"] == "grid" and not args.sync_build), "steps": steps, "ms_per_step": ms_step, "value": P_total / (ms_step * 1e-3), "unit": "points/s",
            "gpu_launches": launches, "clocks": sampler.window(w0, w1) if rank == 0 else None,
            "hit_pairs": hits, "tested_pairs": tested, "cull_efficiency": hits / tested if tested else None}
     per = {k: (stage_ms[k] / stage_calls[k] if stage_calls[k] else 0.0) for k in stage_ms}
@@ -564,6 +566,7 @@ def main():
     ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sync-build", action="store_true", help="grid queries: keep the host round trip in gs_build_accel (GS_OPT_ASYNC_BUILD = 0)")
     ap.add_argument("--points-accel", default="default", choices=["default", "gather", "scatter"],
                     help="point queries: gather = LBVH over the Gaussians (north_star); scatter = the paper's tree over the samples")
     ap.add_argument("--record-traffic", nargs=3, metavar=("NCU_RAW_CSV", "WORKLOAD", "SOURCE"),

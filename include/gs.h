@@ -167,8 +167,15 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
  *                     keeps the 12 per-Gaussian sums in registers and writes one row per Gaussian (no atomics).
  * Both modes decide membership with the same canonical predicate: ID sets are identical, values differ by summation
  * order only.  The LBVH debug items (nodes, parents, boxes) exist in gather mode only.
+ * GS_OPT_ASYNC_BUILD (0 / 1, default 0) removes the host round trip from gs_build_accel of a GRID query in steady state.
+ *   The first build for a model size is synchronous and leaves 50 % headroom in the pair list; the following builds fill
+ *   the list speculatively and send the pair count T and the touched-Gaussian count M to pinned host memory WITHOUT
+ *   waiting; forward, backward and finalize read M on the device.  The price is CUDA's own error model: if a later batch
+ *   produces more than 1.5x the pairs of the sizing build, its kernels do nothing (they check T against the capacity on
+ *   the device) and the NEXT call on the context returns GS_ERR_OVERFLOW ("repeat the batch"; the following build is
+ *   synchronous again).  gs_debug_get / gs_status_query wait for the counts.  Point queries always synchronise once.
  * Errors: INVALID_ARG (unknown key / value). */
-typedef enum { GS_OPT_POINTS_ACCEL = 0 } gs_option;
+typedef enum { GS_OPT_POINTS_ACCEL = 0, GS_OPT_ASYNC_BUILD = 1 } gs_option;
 typedef enum { GS_POINTS_GATHER = 0, GS_POINTS_SCATTER = 1 } gs_points_accel;
 gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value);
 

@@ -116,6 +116,41 @@ CullLists cull_lists(gs_ctx *ctx) {
                      ctx->counters.as<uint32_t>() + 2, ctx->cull_cap};
 }
 
+// GS_OPT_ASYNC_BUILD: pick up the pair count T and the touched count M of the last grid build once they have arrived in
+// pinned host memory.  If T outgrew the speculative buffer the kernels of that batch did nothing: grow, and report it.
+gs_status resolve_grid_counts(gs_ctx *ctx) {
+    if (!ctx->grid_pending) return GS_OK;
+    ctx->grid_pending = false;
+    cudaError_t e = cudaEventSynchronize(ctx->grid_event);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "wait for the pair count");
+    const unsigned long long T = ctx->grid_host[0], M = ctx->grid_host[1];
+    const size_t cap = ctx->pair_gauss.cap / 4;
+    if (T >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
+    if (T > cap) {
+        ctx->accel_kind = -1;
+        ctx->grid_warm_N = 0xffffffffu;   // the next build is synchronous and sizes the buffer
+        return fail(ctx, GS_ERR_OVERFLOW, "asynchronous build: the pair list of the previous batch outgrew its speculative capacity; "
+                                          "that batch's outputs are invalid -- repeat it (the next gs_build_accel is synchronous)");
+    }
+    ctx->T = (uint32_t)T;
+    ctx->M = ctx->M_hint = (uint32_t)M;
+    return GS_OK;
+}
+
+DevCount dev_count(gs_ctx *ctx) {
+    if (ctx->accel_kind == GS_QUERY_GRID && ctx->grid_pending)
+        return DevCount{ctx->counters.as<unsigned long long>() + 4, (uint32_t)(ctx->pair_gauss.cap / 4 < 0xffffffffull ? ctx->pair_gauss.cap / 4 : 0xffffffffull)};
+    return DevCount{nullptr, 0};
+}
+
+// number of order-list entries the backward / finalize launches are sized for: M, or (M still on the device) a bound from
+// the last known M -- the kernels stride over the real one
+uint32_t grid_M_launch(gs_ctx *ctx) {
+    if (!ctx->grid_pending) return ctx->M;
+    const uint64_t b = (uint64_t)ctx->M_hint + ctx->M_hint / 4 + 4096;
+    return (uint32_t)(b < ctx->N ? b : ctx->N);
+}
+
 int bits_for(uint64_t n) {  // bits needed to represent values in [0, n)
     int b = 0;
     while (b < 32 && (1ull << b) < n) b++;
@@ -156,6 +191,7 @@ void gs_destroy(gs_ctx *ctx) {
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
         for (auto &pp : *v) { cudaEventDestroy(pp.a); cudaEventDestroy(pp.b); }
     if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_event); }
+    if (ctx->grid_host) { cudaFreeHost(ctx->grid_host); cudaEventDestroy(ctx->grid_event); }
     delete ctx;
 }
 
@@ -174,6 +210,7 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
             if (!(dom->hi[k] > dom->lo[k]) || !isfinite(dom->hi[k]) || !isfinite(dom->lo[k]))
                 return fail(ctx, GS_ERR_INVALID_ARG, "domain: need finite lo < hi");
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
     ctx->have_pre = false;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
@@ -206,6 +243,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     gs_status st = validate_query(ctx, q, &gd, &P);
     if (st != GS_OK) return st;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    if ((st = resolve_grid_counts(ctx)) != GS_OK) return st;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
     cudaStream_t s = ctx->stream;
@@ -234,7 +272,21 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         // The pair list is filled speculatively into the buffer the previous step left; T is read back once, at the
         // end, and the fill is repeated only when the buffer had to grow (it writes nothing when T exceeds `cap`).
         unsigned long long T64[2] = {0, 0};
-        for (int attempt = 0; attempt < 2; attempt++) {
+        // GS_OPT_ASYNC_BUILD, steady state (same model size as the last synchronous build, which left 50 % headroom): fill the
+        // pair list speculatively and send T / M to pinned host memory WITHOUT waiting for them -- no host round trip in the step
+        const bool async = ctx->opt_async_build && ctx->grid_warm_N == N && ctx->pair_gauss.cap >= 4;
+        if (async) {
+            const size_t cap = ctx->pair_gauss.cap / 4;
+            CK(launch_pair_fill(ctx->aabb.as<float>(), ctx->bcount.as<uint32_t>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
+                                ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
+                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), s), "pair fill");
+            CK(cudaMemcpyAsync(ctx->grid_host, total, 16, cudaMemcpyDeviceToHost, s), "read T (async)");
+            CK(cudaEventRecord(ctx->grid_event, s), "event");
+            ctx->grid_pending = true;
+            T64[0] = ctx->T;        // last known values until the real ones arrive (debug views resolve first)
+            T64[1] = ctx->M_hint;
+        }
+        for (int attempt = 0; attempt < 2 && !async; attempt++) {
             const size_t cap = ctx->pair_gauss.cap / 4;
             CK(launch_pair_fill(ctx->aabb.as<float>(), ctx->bcount.as<uint32_t>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
                                 ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
@@ -244,11 +296,23 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
                 CK(cudaStreamSynchronize(s), "sync (T)");
                 if (T64[0] >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
             }
-            if (T64[0] <= cap) break;
-            CK(ctx->pair_gauss.reserve((size_t)T64[0] * 4), "alloc pair list");
+            // with GS_OPT_ASYNC_BUILD the buffer keeps 50 % headroom for the speculative fills of the following steps
+            const size_t need = ctx->opt_async_build ? (size_t)T64[0] + (size_t)T64[0] / 2 + 1024 : (size_t)T64[0];
+            if (need <= cap) break;
+            CK(ctx->pair_gauss.reserve(need * 4), "alloc pair list");
         }
         const uint32_t T = (uint32_t)T64[0];
         ctx->M = (uint32_t)T64[1];
+        if (!async) {
+            ctx->M_hint = ctx->M;
+            if (ctx->opt_async_build) {
+                if (!ctx->grid_host) {
+                    CK(cudaMallocHost(reinterpret_cast<void **>(&ctx->grid_host), 16), "alloc pinned counters");
+                    CK(cudaEventCreateWithFlags(&ctx->grid_event, cudaEventDisableTiming), "event");
+                }
+                ctx->grid_warm_N = N;
+            }
+        }
         ctx->have_pair_brick = false;
         if (gd.jitter && P > 0) {
             CK(ctx->jit.reserve(P * sizeof(float4)), "alloc jitter table");
@@ -361,7 +425,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
     if (ctx->accel_kind == GS_QUERY_GRID) {
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_grid_fwd(ctx->rec.as<float4>(), ctx->N, ctx->grid, ctx->pair_gauss.as<uint32_t>(),
-                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<float4>(), s), "grid forward");
+                           ctx->brick_start.as<uint32_t>(), ctx->tau, ctx->r2, o, ctx->jit.as<float4>(), dev_count(ctx), s), "grid forward");
     } else if (ctx->points_mode == GS_POINTS_SCATTER) {
         Stage stage(ctx, GS_PROF_FWD);
         CK(ctx->sc_acc.reserve(scatter_padded_points(ctx->P ? ctx->P : 1) * 8), "alloc accumulators");
@@ -478,7 +542,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         }
         Stage stage(ctx, GS_PROF_BWD);
         CK(launch_grid_bwd(ctx->rec.as<float4>(), ctx->bwd_setup.as<float4>(), N, ctx->grid, ctx->misc.p, fused2, ctx->r2,
-                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), ctx->M, ctx->jit.as<float4>(), s), "grid backward");
+                           ctx->gacc.as<float>(), ctx->grid_order.as<uint32_t>(), grid_M_launch(ctx), ctx->jit.as<float4>(), dev_count(ctx), s), "grid backward");
     } else if (ctx->points_mode == GS_POINTS_SCATTER) {
         CK(ctx->sc_coef.reserve(scatter_padded_points(ctx->P ? ctx->P : 1) * 32), "alloc backward coefficients");
         Stage stage(ctx, GS_PROF_BWD);
@@ -496,12 +560,13 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     Stage stage(ctx, GS_PROF_FINALIZE);
     const bool grid = ctx->accel_kind == GS_QUERY_GRID;
     CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused2) ? in.eps_scale : 1.f,
-                       *out, grid ? ctx->grid_order.as<uint32_t>() : nullptr, grid ? ctx->M : 0, s), "finalize");
+                       *out, grid ? ctx->bcount.as<uint32_t>() : nullptr, grid ? dev_count(ctx) : DevCount{nullptr, 0}, s), "finalize");
     return GS_OK;
 }
 
 gs_status gs_debug_get(gs_ctx *ctx, int32_t what, const void **dev_ptr, size_t *count) {
     LaunchScope launch_scope(ctx);
+    if (ctx && ctx->grid_pending) { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
     if (!ctx || !dev_ptr || !count) return GS_ERR_INVALID_ARG;
     if (!ctx->have_pre) return fail(ctx, GS_ERR_STATE, "nothing built yet");
     const size_t N = ctx->N;
@@ -635,6 +700,7 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
                      const float *sample_err, const float *I, const uint8_t *defined, uint64_t num_defined, const float *target,
                      uint32_t k, float raw_scale_init, float raw_opacity_init, uint32_t *n_new_host) {
     LaunchScope launch_scope(ctx);
+    if (ctx && ctx->grid_pending) { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
     if (!ctx || !p || !n_new_host) return GS_ERR_INVALID_ARG;
     gs_status st = check_ready(ctx, q, "gs_densify before gs_preprocess/gs_build_accel");
     if (st != GS_OK) return st;
@@ -725,6 +791,12 @@ gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value) {
             if (value != GS_POINTS_GATHER && value != GS_POINTS_SCATTER) return fail(ctx, GS_ERR_INVALID_ARG, "GS_OPT_POINTS_ACCEL: unknown mode");
             ctx->opt_points_accel = (int)value;
             return GS_OK;
+        case GS_OPT_ASYNC_BUILD:
+            if (value != 0 && value != 1) return fail(ctx, GS_ERR_INVALID_ARG, "GS_OPT_ASYNC_BUILD: 0 or 1");
+            if (!value) { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
+            ctx->opt_async_build = (int)value;
+            ctx->grid_warm_N = 0xffffffffu;
+            return GS_OK;
         default: return fail(ctx, GS_ERR_INVALID_ARG, "unknown option");
     }
 }
@@ -737,6 +809,7 @@ gs_status gs_set_sample_count(gs_ctx *ctx, uint64_t total_samples) {
 }
 
 gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host) {
+    if (ctx && ctx->grid_pending) { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
     if (!ctx || !out_host) return GS_ERR_INVALID_ARG;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     CK(cudaStreamSynchronize(ctx->stream), "sync");

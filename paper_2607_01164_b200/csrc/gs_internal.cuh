@@ -138,6 +138,12 @@ struct gs_ctx {
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr;
+    int opt_async_build = 0;    // gs_set_option(GS_OPT_ASYNC_BUILD)
+    bool grid_pending = false;  // T / M of the current grid accel are still on their way to grid_host (grid_event)
+    unsigned long long *grid_host = nullptr;   // pinned [2]: T, M
+    cudaEvent_t grid_event = nullptr;
+    uint32_t grid_warm_N = 0xffffffffu;        // N of the last synchronously built grid accel (async needs a known capacity)
+    uint32_t M_hint = 0;                       // M of the last resolved build: sizes the backward's grid while M is pending
     int opt_points_accel = 0;   // gs_set_option(GS_OPT_POINTS_ACCEL): mode the NEXT point accel is built in
     int points_mode = 0;        // mode of the current point accel (gs_points_accel)
     gs::DevBuf sc_spt, sc_box, sc_acc, sc_coef;  // scatter mode: sorted positions, tree boxes, (I, Nacc) accumulators, backward coefficients
@@ -179,6 +185,14 @@ cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t 
                              uint32_t *order, cudaStream_t s);
 cudaError_t launch_expand_bricks(const uint32_t *start, uint32_t nbricks, uint32_t *key, cudaStream_t s);
 
+// GS_OPT_ASYNC_BUILD: the pair count T and the touched-Gaussian count M of a grid batch stay on the device (total[0],
+// total[1]); kernels read M there and return at once when T outgrew the speculative pair buffer (total == NULL: the
+// host knows both, the synchronous build)
+struct DevCount {
+    const unsigned long long *total;
+    uint32_t cap;
+};
+
 struct FwdOut {
     const float *target; float *phi; float *I; double *loss; float *dL_dphi; float *sample_err;
     uint32_t *set_count; unsigned long long *set_sum; unsigned long long *set_xor;   // debug sets (nullable)
@@ -195,20 +209,20 @@ struct BwdIn {
 };
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
-                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, cudaStream_t s);
+                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, DevCount dc, cudaStream_t s);
 // per-voxel sample positions of a jittered batch (gd.jitter; D26), batch-local sample order, written once per gs_build_accel
 cudaError_t launch_jitter_table(const GridDesc &gd, float4 *jit, cudaStream_t s);
 // second pass of gs_sample_fwd_loss: dL_dI[c] /= |D-| or |U+| (by sign), loss_terms = (L_rec, L_FN, L_FP)
 cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *loss_terms, cudaStream_t s);
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s);
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, cudaStream_t s);
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, DevCount dc, cudaStream_t s);
 
-// grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the
-// cell steps are folded in); eps_scale multiplies the error share (fused MSE: eps = |alpha| * eps_scale, else 1)
-// grid_moments: only the M Gaussians of `order` have a row; the gradients of the others are set to zero
+// grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the cell steps are
+// folded in), only for the Gaussians with touched[i] != 0 (the others get zero gradients); eps_scale multiplies the error share
+// (fused MSE: eps = |alpha| * eps_scale, else 1)
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
-                            float eps_scale, const gs_grads &out, const uint32_t *order, uint32_t M, cudaStream_t s);
+                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, cudaStream_t s);
 
 // optim.cu: activations of the raw parameters and one Adam step on them
 cudaError_t launch_activate(const gs_raw_params &p, float *scale, float *opacity, float *scalar, cudaStream_t s);

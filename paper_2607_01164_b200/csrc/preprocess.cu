@@ -105,11 +105,21 @@ cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float
 template <bool MOMENTS>
 __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
                                                    const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
-                                                   const uint32_t *__restrict__ order, uint32_t M) {
-    // order != NULL: only the M Gaussians of the list are finalised (the others keep the zeros the launcher wrote)
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (order ? M : N)) return;
-    const uint32_t i = order ? order[t] : t;
+                                                   const uint32_t *__restrict__ touched, DevCount dc) {
+    // touched != NULL (structured): touched[i] = bricks of the batch Gaussian i overlaps; only those with a non-zero count have
+    // an accumulator row, the others get zero gradients right here (no memset pass, no order list, coalesced either way)
+    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;   // asynchronous build whose pair list overflowed
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    if (touched && touched[i] == 0u) {
+#pragma unroll
+        for (int k = 0; k < 3; k++) { out.dmean[3 * (size_t)i + k] = 0.f; out.dscale[3 * (size_t)i + k] = 0.f; }
+        reinterpret_cast<float4 *>(out.dquat)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        out.dopacity[i] = 0.f;
+        out.dscalar[i] = 0.f;
+        if (out.err) out.err[i] = 0.f;
+        return;
+    }
     float dv, dw, E, U[3], W00, W01, W02, W11, W12, W22;
     if (MOMENTS) {
         const float4 *ga = reinterpret_cast<const float4 *>(gacc) + (GACC_GRID / 4) * (size_t)i;
@@ -227,27 +237,11 @@ cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *lo
 }
 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
-                            float eps_scale, const gs_grads &out, const uint32_t *order, uint32_t M, cudaStream_t s) {
+                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    if (grid_moments) {
-        // Only the M Gaussians that touch the batch have an accumulator row; the gradients of the others are zero.
-        // (A 128^3 batch of configs[3] touches 0.3 % of the 4.2 M Gaussians: reading 128-byte rows of all of them
-        // cost 0.21 ms per batch.)
-        if (M < N) {
-            const struct { float *p; size_t cnt; } z[] = {{out.dmean, 3 * (size_t)N}, {out.dscale, 3 * (size_t)N}, {out.dquat, 4 * (size_t)N},
-                                                          {out.dopacity, N}, {out.dscalar, N}, {out.err, N}};
-            for (const auto &a : z) {
-                if (!a.p) continue;
-                cudaError_t e = cudaMemsetAsync(a.p, 0, a.cnt * sizeof(float), s);
-                if (e != cudaSuccess) return e;
-            }
-        }
-        if (M == 0) return cudaSuccess;
-        if (M == N) order = nullptr;  // every Gaussian has a row: plain (coalesced) indexing
-        k_finalize<true><<<(M + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, order, M);
-    } else {
-        k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, 0);
-    }
+    // A 128^3 batch of configs[3] touches 0.3 % of the 4.2 M Gaussians: only those read their 128-byte row.
+    if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc);
+    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, DevCount{nullptr, 0});
     count_launch();
     return cudaGetLastError();
 }

@@ -77,18 +77,24 @@ __device__ __forceinline__ void warp_reduce32(float (&v)[32], int lane) {
     }
 }
 
-template <bool PACK2, bool JIT>
+template <bool PACK2, bool JIT, bool ASYNC>
 __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
                                                               GridDesc gd, const void *__restrict__ pack_, float r2,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
-                                                              uint32_t M, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/) {
+                                                              uint32_t M, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/, DevCount dc) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // a warp processes GPW consecutive Gaussians of the brick-ordered list of the M Gaussians that touch the batch
     // slot `rep` of this warp is entry w0 + rep * wstride of the order list
+    if (ASYNC) {   // asynchronous build: M lives on the device; nothing to do if the pair list overflowed its buffer
+        if (dc.total[0] > (unsigned long long)dc.cap) return;
+        M = (uint32_t)dc.total[1];
+    }
     const uint32_t wstride = INTERLEAVE ? BWD_WARPS : 1;
-    const uint32_t w0 = INTERLEAVE ? blockIdx.x * (BWD_WARPS * GPW) + warp : (blockIdx.x * BWD_WARPS + warp) * GPW;
-    if (w0 >= M) return;  // whole warps leave; no block-wide barrier is used below
+    // the launch covers every entry of the order list when the host knew M; with a device-side M the CTAs stride over it
+    for (uint32_t cta = blockIdx.x; ASYNC ? (uint64_t)cta * (BWD_WARPS * GPW) < M : cta == blockIdx.x; cta += gridDim.x) {
+    const uint32_t w0 = INTERLEAVE ? cta * (BWD_WARPS * GPW) + warp : (cta * BWD_WARPS + warp) * GPW;
+    if (w0 >= M) return;  // whole warps leave; no block-wide barrier is used below (later CTA slots start beyond this one)
     const uint32_t my_id = (lane < GPW && w0 + lane * wstride < M) ? order[w0 + lane * wstride] : 0u;
     const uint32_t bdx = (uint32_t)gd.bdim[0], bdy = (uint32_t)gd.bdim[1];
     int first[3], last[3];
@@ -324,6 +330,7 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     gacc[(size_t)i * GACC_GRID + lane] = acc[0];
     __syncwarp();
     }  // rep
+    }  // cta slot
 }
 
 cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pack, cudaStream_t s) {
@@ -334,17 +341,21 @@ cudaError_t launch_pack_samples(const BwdIn &in, size_t P, float tau, float4 *pa
 }
 
 cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, const GridDesc &gd, const void *pack, bool pack2,
-                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, cudaStream_t s) {
+                            float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, DevCount dc, cudaStream_t s) {
     // only the M Gaussians of the order list get (and need) an accumulator row: k_finalize reads those alone
     if (M == 0) return cudaSuccess;
     const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
+#define GS_BWD_LAUNCH(P2_, JIT_, ASYNC_) \
+    k_grid_bwd<P2_, JIT_, ASYNC_><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit, dc)
+    const bool as = dc.total != nullptr;
     if (gd.jitter) {
-        if (pack2) k_grid_bwd<true, true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit);
-        else k_grid_bwd<false, true><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit);
+        if (pack2) { if (as) GS_BWD_LAUNCH(true, true, true); else GS_BWD_LAUNCH(true, true, false); }
+        else { if (as) GS_BWD_LAUNCH(false, true, true); else GS_BWD_LAUNCH(false, true, false); }
     } else {
-        if (pack2) k_grid_bwd<true, false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit);
-        else k_grid_bwd<false, false><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit);
+        if (pack2) { if (as) GS_BWD_LAUNCH(true, false, true); else GS_BWD_LAUNCH(true, false, false); }
+        else { if (as) GS_BWD_LAUNCH(false, false, true); else GS_BWD_LAUNCH(false, false, false); }
     }
+#undef GS_BWD_LAUNCH
     count_launch();
     return cudaGetLastError();
 }

@@ -29,14 +29,15 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
 
-template <bool SETS, bool JIT>
+template <bool SETS, bool JIT, bool ASYNC>
 __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const float4 *__restrict__ rec, uint32_t N, GridDesc gd,
                                                            const uint32_t *__restrict__ pair_gauss,
                                                            const uint32_t *__restrict__ brick_start, float tau, float r2, FwdOut o,
-                                                           double invP, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/) {
+                                                           double invP, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/, DevCount dc) {
     __shared__ float4 srec[4][CAP];
     __shared__ uint32_t sid[CAP];
     __shared__ uint4 smask[FWD_THREADS / 32][32];  // [warp][cell] -> masks of the 4 sub-chunks
+    if (ASYNC && dc.total[0] > (unsigned long long)dc.cap) return;   // the speculative pair list did not fit: nothing valid to read
     const uint32_t b = blockIdx.x;
     const int bx = b % gd.brick_cnt[0], by = (b / gd.brick_cnt[0]) % gd.brick_cnt[1], bz = b / (gd.brick_cnt[0] * gd.brick_cnt[1]);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -295,18 +296,22 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
 }
 
 cudaError_t launch_grid_fwd(const float4 *rec, uint32_t N, const GridDesc &gd, const uint32_t *pair_gauss,
-                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, cudaStream_t s) {
+                            const uint32_t *brick_start, float tau, float r2, const FwdOut &o, const float4 *jit, DevCount dc, cudaStream_t s) {
     const uint32_t nbricks = (uint32_t)gd.brick_cnt[0] * gd.brick_cnt[1] * gd.brick_cnt[2];
     if (nbricks == 0) return cudaSuccess;
     const double P = o.inv_count > 0.0 ? 1.0 / o.inv_count : (double)gd.bdim[0] * gd.bdim[1] * gd.bdim[2];
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
+#define GS_FWD_LAUNCH(SETS_, JIT_, ASYNC_) \
+    k_grid_fwd<SETS_, JIT_, ASYNC_><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit, dc)
+    const bool as = dc.total != nullptr;
     if (gd.jitter) {
-        if (sets) k_grid_fwd<true, true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit);
-        else k_grid_fwd<false, true><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit);
+        if (sets) { if (as) GS_FWD_LAUNCH(true, true, true); else GS_FWD_LAUNCH(true, true, false); }
+        else { if (as) GS_FWD_LAUNCH(false, true, true); else GS_FWD_LAUNCH(false, true, false); }
     } else {
-        if (sets) k_grid_fwd<true, false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit);
-        else k_grid_fwd<false, false><<<nbricks, FWD_THREADS, 0, s>>>(rec, N, gd, pair_gauss, brick_start, tau, r2, o, 1.0 / P, jit);
+        if (sets) { if (as) GS_FWD_LAUNCH(true, false, true); else GS_FWD_LAUNCH(true, false, false); }
+        else { if (as) GS_FWD_LAUNCH(false, false, true); else GS_FWD_LAUNCH(false, false, false); }
     }
+#undef GS_FWD_LAUNCH
     count_launch();
     return cudaGetLastError();
 }

@@ -162,3 +162,58 @@ def test_two_sample_shards_add_up_on_one_gpu(oracle):
     gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
     for k, v in gr.items():
         assert rel_l2(total[k].cpu().numpy(), v) <= 1e-4, k
+
+
+def test_async_build_matches_synchronous_and_reports_overflow(oracle):
+    # GS_OPT_ASYNC_BUILD (gs.h): steady-state grid builds without a host round trip give bit-identical results; a batch whose
+    # pair list outgrows the speculative capacity does nothing and the NEXT call reports GS_ERR_OVERFLOW
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c4_gaussians(seed=3, n_grid=64, n=20000)
+    full = inputs.Grid((64, 64, 64), (0.0, 0.0, 0.0), (1 / 64, 1 / 64, 1 / 64))
+    P = full.num_points
+    target = np.random.default_rng(1).uniform(0, 1, P).astype(np.float32)
+    ref = GpuRun(g, "grid", full, target, fused=True)
+    ctx = api.Context()
+    ctx.gs_set_option(api.OPT_ASYNC_BUILD, 1)
+    dev = _dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+    t = torch.from_numpy(target).cuda()
+    q = api.grid_query(full)
+    phi, I = torch.empty(P, device="cuda"), torch.empty(P, device="cuda")
+    grads = ctx.alloc_grads(g.n)
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for step in range(4):   # step 0 is the synchronous sizing build, 1..3 run without a host round trip
+        loss.zero_()
+        for v in grads.values():
+            v.fill_(-7.0)
+        ctx.gs_preprocess(*dev)
+        ctx.gs_build_accel(q)
+        ctx.gs_sample_fwd(q, phi, I, target=t, loss=loss)
+        ctx.gs_sample_bwd(q, None, None, None, grads)
+        torch.cuda.synchronize()
+        assert torch.equal(phi, ref.phi[:P]) and torch.equal(I, ref.I[:P])
+        assert float(loss.item()) == float(ref.loss.item())
+        for k, v in grads.items():
+            assert torch.equal(v, ref.grads[k]), (step, k)
+    st = ctx.gs_status_query()
+    assert st["grid_pairs"] == ref.ctx.gs_status_query()["grid_pairs"] and st["grid_touched"] == ref.ctx.gs_status_query()["grid_touched"]
+    # overflow: size the buffer with a one-brick batch, then ask for the whole grid asynchronously
+    small = full.batch((3, 3, 3), (1, 1, 1))
+    ctx2 = api.Context()
+    ctx2.gs_set_option(api.OPT_ASYNC_BUILD, 1)
+    ctx2.gs_preprocess(*dev)
+    qs = api.grid_query(small)
+    ctx2.gs_build_accel(qs)                      # synchronous: capacity = 1.5 x a few hundred pairs
+    ctx2.gs_build_accel(q)                       # asynchronous: T is far beyond the capacity
+    phi.fill_(-7.0)
+    ctx2.gs_sample_fwd(q, phi, I)                # does nothing
+    torch.cuda.synchronize()
+    assert float(phi.min().item()) == -7.0 and float(phi.max().item()) == -7.0
+    with pytest.raises(api.GsError) as e:
+        ctx2.gs_build_accel(q)
+    assert e.value.status == api.GS_ERR_OVERFLOW
+    ctx2.gs_build_accel(q)                       # synchronous again: grows the buffer
+    ctx2.gs_sample_fwd(q, phi, I)
+    torch.cuda.synchronize()
+    assert torch.equal(phi, ref.phi[:P])
+    ctx.close(); ctx2.close()
