@@ -190,7 +190,7 @@ void gs_destroy(gs_ctx *ctx) {
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
         for (auto &pp : *v) { cudaEventDestroy(pp.a); cudaEventDestroy(pp.b); }
-    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_event); }
+    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_event); cudaEventDestroy(ctx->aux_event2); }
     if (ctx->grid_host) { cudaFreeHost(ctx->grid_host); cudaEventDestroy(ctx->grid_event); }
     delete ctx;
 }
@@ -351,6 +351,10 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
                            ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), ctx->sorted_rec.as<float4>(), s), "lbvh");
         // coherence sort of the queries
         ctx->have_pt_order = false;
+        if (ctx->points_ready) {   // gs_step_host: the points' H2D copy ran on the aux stream beside preprocess and the LBVH build
+            CK(cudaStreamWaitEvent(s, ctx->points_ready, 0), "wait for the points");
+            ctx->points_ready = nullptr;
+        }
         if (!q->presorted && P > 0) {
             for (int k = 0; k < 2; k++) {
                 CK(ctx->pt_key[k].reserve(P * 4), "alloc point keys");
@@ -872,21 +876,26 @@ gs_status gs_step_host(gs_ctx *ctx, const gs_gaussians *gh, const gs_domain *dom
     for (int k = 0; k < 5; k++)
         if (N) CK(cudaMemcpyAsync(ctx->h2d[k].p, src[k], N * (sizes[k] / n1), cudaMemcpyHostToDevice, s), "H2D model");
     gs_query q = *qh;
-    if (q.kind == GS_QUERY_POINTS) {
-        if (P) CK(cudaMemcpyAsync(ctx->h2d[5].p, qh->xyz, P * 12, cudaMemcpyHostToDevice, s), "H2D points");
-        q.xyz = ctx->h2d[5].as<float>();
-    }
-    // the target is first needed by the forward's epilogue: its copy runs on a second stream beside preprocess + build
+    // The model is needed first (preprocess, LBVH over the Gaussians): its copy leads on the context's stream.  The query
+    // points are first needed by the coherence sort inside gs_build_accel and the target by the forward's epilogue: their
+    // copies run on a second stream beside preprocess and the Gaussian side of the build.
     if (!ctx->aux_stream) {
         CK(cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking), "aux stream");
         CK(cudaEventCreateWithFlags(&ctx->aux_event, cudaEventDisableTiming), "aux event");
+        CK(cudaEventCreateWithFlags(&ctx->aux_event2, cudaEventDisableTiming), "aux event");
     }
     if (P) {
         CK(cudaEventRecord(ctx->aux_event, s), "event");                       // after everything enqueued so far
         CK(cudaStreamWaitEvent(ctx->aux_stream, ctx->aux_event, 0), "wait");
+        if (q.kind == GS_QUERY_POINTS) {
+            CK(cudaMemcpyAsync(ctx->h2d[5].p, qh->xyz, P * 12, cudaMemcpyHostToDevice, ctx->aux_stream), "H2D points");
+            CK(cudaEventRecord(ctx->aux_event2, ctx->aux_stream), "event");
+            ctx->points_ready = ctx->aux_event2;
+        }
         CK(cudaMemcpyAsync(ctx->h2d[6].p, target_host, P * 4, cudaMemcpyHostToDevice, ctx->aux_stream), "H2D target");
         CK(cudaEventRecord(ctx->aux_event, ctx->aux_stream), "event");
     }
+    if (q.kind == GS_QUERY_POINTS) q.xyz = ctx->h2d[5].as<float>();
     CK(cudaMemsetAsync(ctx->h2d[10].p, 0, 8, s), "zero loss");
     gs_gaussians gdv{gh->n, ctx->h2d[0].as<float>(), ctx->h2d[1].as<float>(), ctx->h2d[2].as<float>(), ctx->h2d[3].as<float>(),
                      ctx->h2d[4].as<float>()};

@@ -137,7 +137,8 @@ struct gs_ctx {
     gs::DevBuf rn_xyz, rn_phi, rn_I;   // gs_render: samples of a chunk of rays
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
-    cudaEvent_t aux_event = nullptr;
+    cudaEvent_t aux_event = nullptr, aux_event2 = nullptr;
+    cudaEvent_t points_ready = nullptr;   // set by gs_step_host: gs_build_accel waits for it before it touches the query points
     int opt_async_build = 0;    // gs_set_option(GS_OPT_ASYNC_BUILD)
     bool grid_pending = false;  // T / M of the current grid accel are still on their way to grid_host (grid_event)
     unsigned long long *grid_host = nullptr;   // pinned [2]: T, M
