@@ -454,6 +454,27 @@ def measure(wl, args, sampler, world, rank, headline: bool):
                          "build_ms_per_chunk": sm["build"] / max(sc["build"], 1), "fwd_ms_per_chunk": sm["fwd"] / max(sc["fwd"], 1)}
         del xs, qs, pp, ii
 
+    # ---- volume rendering through gs_render: 512 x 512 rays x 64 samples of the configs[2] model = one 2^24-sample chunk
+    if world == 1 and wl["name"] == "c3":
+        from paper_2607_01164_b200 import inputs
+        lo, hi = wl["domain"]
+        ctr = 0.5 * (np.asarray(lo, np.float64) + np.asarray(hi, np.float64))
+        o_, d_, tr_ = inputs.camera_rays(512, 512, eye=tuple(ctr + np.array([1.6, -1.3, 1.1])), look_at=tuple(ctr), fov_y_deg=35.0,
+                                         box=(tuple(float(x) for x in lo), tuple(float(x) for x in hi)))
+        od, dd, td, tab = dev(o_), dev(d_), dev(tr_), dev(inputs.diverging_transfer(256, 30.0))
+        rgba = torch.empty((len(o_), 4), device="cuda")
+        ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
+        ctx.gs_render(od, dd, td, 64, tab, rgba); barrier()
+        e0.record()
+        for _ in range(3):
+            ctx.gs_render(od, dd, td, 64, tab, rgba)
+        e1.record(); barrier()
+        ms_r = e0.elapsed_time(e1) / 3
+        out["render"] = {"what": "gs_render: 512 x 512 rays x 64 samples per ray (1.68e7 samples, one chunk) of this model, emission-absorption, "
+                                 "coverage as the domain test; includes the LBVH / query sort / cull of the sample positions",
+                         "ms_per_frame": ms_r, "samples_per_s": len(o_) * 64 / (ms_r * 1e-3), "covered_pixels": int((rgba[:, 3] > 0).sum().item())}
+        del od, dd, td, rgba
+
     # ---- e2e through the HOST-buffer entry point (pinned memory, copies inside the timed region)
     if world == 1:
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -548,7 +569,9 @@ def run_ours(args):
                 "config": r["config"], "clocks": r["clocks"], "gpu_launches": r["gpu_launches"], "e2e": r.get("e2e"),
                 "stage_ms": r["stage_ms"], "roofline": r["roofline"], "csrc_sha16": csrc_sha16(),
                 "extra": {"hit_pairs": r["hit_pairs"], "tested_pairs": r["tested_pairs"], "cull_efficiency": r["cull_efficiency"],
-                          "rates": r["rates"], "decode": r.get("decode"), "hbm_peak_gbs_measured": _peaks().get("hbm_gbs")}}
+                          "rates": r["rates"], "decode": r.get("decode"), "render": r.get("render"),
+                          "points_accel": r.get("points_accel"), "async_build": r.get("async_build"),
+                          "hbm_peak_gbs_measured": _peaks().get("hbm_gbs")}}
         if "cpu_baseline" in r:
             line["cpu_baseline"] = r["cpu_baseline"]
         if len(names) > 1:

@@ -371,15 +371,16 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         // list chunks grows on demand: the kernel counts the chunks it needs, the host reads that count back (the one
         // device->host crossing of the unstructured path, like T of the structured path) and repeats the pass if it
         // did not fit.
+        // sorted copy of the query points: every point kernel reads positions from it (one coalesced 16-byte load per lane)
+        CK(ctx->sc_spt.reserve(scatter_padded_points(P ? P : 1) * 16), "alloc sorted points");
+        CK(launch_sorted_points(q->xyz, ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->sc_spt.as<float4>(), s),
+           "sorted points");
         if (scatter) {
             // the paper's structure: a wide tree over the SORTED SAMPLE POSITIONS, rebuilt per query
-            const uint64_t Ppad = scatter_padded_points(P ? P : 1);
             const uint32_t nodes = scatter_tree_shape(P, &ctx->sc_tree);
-            CK(ctx->sc_spt.reserve(Ppad * 16), "alloc sorted points");
             CK(ctx->sc_box.reserve((size_t)nodes * 24), "alloc point tree");
             ctx->sc_tree.box = ctx->sc_box.as<float>();
-            CK(launch_scatter_build(q->xyz, ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->sc_tree,
-                                    ctx->sc_spt.as<float4>(), ctx->sc_box.as<float>(), s), "point tree");
+            CK(launch_scatter_build(P, ctx->sc_tree, ctx->sc_spt.as<float4>(), ctx->sc_box.as<float>(), s), "point tree");
         } else if (P > 0) {
             Stage cull_stage(ctx, GS_PROF_CULL);
             const uint64_t packets = (P + 31) / 32;
@@ -393,7 +394,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
             uint32_t *ovf = ctx->counters.as<uint32_t>();
             for (int attempt = 0;; attempt++) {
                 CK(cudaMemsetAsync(ovf, 0, 4, s), "memset");
-                CK(launch_points_cull(ctx->sorted_rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), q->xyz,
+                CK(launch_points_cull(ctx->sorted_rec.as<float4>(), N, ctx->bvh_nodes.as<float4>(), ctx->sc_spt.as<float4>(),
                                       ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, P, ctx->dom, ctx->r,
                                       cull_lists(ctx), ovf, ctx->cull_per_packet > 512.0 ? 2 : 4, s), "points cull");
                 uint32_t host[3] = {0, 0, 0};   // [0] stack overflow flag, [2] chunks requested
@@ -439,7 +440,7 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
            "points forward (scatter)");
     } else {
         Stage stage(ctx, GS_PROF_FWD);
-        CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
+        CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
                              ctx->r2, o, s), "points forward");
     }
@@ -557,7 +558,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
-        CK(launch_points_bwd(ctx->sorted_rec.as<float4>(), ctx->accel_q.xyz,
+        CK(launch_points_bwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
                              ctx->r2, in, ctx->gacc.as<float>(), s), "points backward");
     }

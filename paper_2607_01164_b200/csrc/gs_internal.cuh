@@ -265,21 +265,23 @@ struct CullLists {
     uint32_t *top;    // chunks requested so far (may exceed cap: the host then grows the pool and repeats)
     uint32_t cap;
 };
-cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
+cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order,
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group /*2 or 4 packets per warp*/,
                                cudaStream_t s);
-cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+cudaError_t launch_points_fwd(const float4 *sorted_rec, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const FwdOut &o, cudaStream_t s);
 // scatter mode (the paper's formulation): see sample_scatter.cu
 uint64_t scatter_padded_points(uint64_t P);
 uint32_t scatter_tree_shape(uint64_t P, PtTree *T);
-cudaError_t launch_scatter_build(const float *xyz, const uint32_t *pt_order, uint64_t P, PtTree T, float4 *spt, float *box, cudaStream_t s);
+// sorted copy of the query points (float4, padded with NaN to a multiple of 64): read by every point kernel of both modes
+cudaError_t launch_sorted_points(const float *xyz, const uint32_t *pt_order, uint64_t P, float4 *spt, cudaStream_t s);
+cudaError_t launch_scatter_build(uint64_t P, PtTree T, const float4 *spt, float *box, cudaStream_t s);
 cudaError_t launch_scatter_fwd(const float4 *rec, const float *aabb, const uint32_t *gorder, uint32_t N, const PtTree &T, const float4 *spt,
                                float2 *acc, const uint32_t *pt_order, uint64_t P, float tau, float r2, const FwdOut &o, cudaStream_t s);
 cudaError_t launch_scatter_bwd(const float4 *rec, const float *aabb, const uint32_t *gorder, uint32_t N, const PtTree &T, const float4 *spt,
                                float4 *coef, const uint32_t *pt_order, uint64_t P, float tau, float r2, const BwdIn &in, float *gacc,
                                cudaStream_t s);
-cudaError_t launch_points_bwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+cudaError_t launch_points_bwd(const float4 *sorted_rec, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s);
 
 }  // namespace gs

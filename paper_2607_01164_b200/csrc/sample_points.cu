@@ -103,14 +103,17 @@ __device__ __forceinline__ void segment_box(float px, float py, float pz, bool i
 
 // The point of lane `lane` of packet `packet` (NaN for lanes past the end: never inside anything).
 struct PacketPoint { uint64_t c; bool active; float px, py, pz; };
-__device__ __forceinline__ PacketPoint load_point(const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order, uint64_t P,
+// Positions come from the SORTED copy of the query points (float4 per point, written once per gs_build_accel; the slots past
+// the end hold NaN): one coalesced 16-byte load per lane instead of three scattered 4-byte gathers through the order array in
+// each of the cull, forward and backward kernels.
+__device__ __forceinline__ PacketPoint load_point(const float4 *__restrict__ spt, const uint32_t *__restrict__ pt_order, uint64_t P,
                                                   uint64_t packet, int lane) {
     PacketPoint pp;
     const uint64_t k = packet * 32 + lane;
     pp.active = k < P;
     pp.c = pp.active ? (pt_order ? (uint64_t)pt_order[k] : k) : 0;
-    const float nanv = __int_as_float(0x7fc00000);
-    pp.px = pp.active ? xyz[3 * pp.c] : nanv; pp.py = pp.active ? xyz[3 * pp.c + 1] : nanv; pp.pz = pp.active ? xyz[3 * pp.c + 2] : nanv;
+    const float4 v = __ldg(spt + k);   // the copy is padded to a whole number of packets
+    pp.px = v.x; pp.py = v.y; pp.pz = v.z;
     return pp;
 }
 
@@ -149,7 +152,7 @@ __device__ __forceinline__ void gather64(const float4 *__restrict__ base, uint32
 // of the previous step (launch_points_cull)
 template <int CULL_GP>
 __global__ void __launch_bounds__(CULL_WARPS * 32, GS_CULL_MINB) k_points_cull(const float4 *__restrict__ srt, uint32_t N, const float4 *__restrict__ nodes,
-                                                                  const float *__restrict__ xyz, const uint32_t *__restrict__ pt_order,
+                                                                  const float4 *__restrict__ xyz /*sorted copy*/, const uint32_t *__restrict__ pt_order,
                                                                   uint64_t P, MortonParams mp, float rcut, CullLists o,
                                                                   uint32_t *__restrict__ overflow) {
     __shared__ int32_t stack_all[CULL_WARPS][STK_CAP];
@@ -369,7 +372,7 @@ __global__ void __launch_bounds__(CULL_WARPS * 32, GS_CULL_MINB) k_points_cull(c
 // (15 packed instructions for the canonical sequence) where the scalar form needed 27 slots per Gaussian.
 // ---------------------------------------------------------------------------------------------------------
 template <bool SETS>
-__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
+__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, FwdOut o, double invP) {
     __shared__ float4 buf_all[EVAL_WARPS][2][128];   // two chunks of 32 records of 64 B (plane c's .w carries the Gaussian id)
@@ -463,9 +466,9 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             res2 = res * res;
             if (o.dL_dphi) o.dL_dphi[c] = covered ? (float)(2.0 * invP) * res : 0.f;
             if (o.sample_err) o.sample_err[c] = fabsf(res);
-            if (o.pack2) {
+            if (o.pack2) {   // kept in SORTED order (position packet * 32 + lane): the backward reads it back coalesced
                 const float al = covered ? __fdividef((float)(2.0 * invP) * res, I) : 0.f;
-                o.pack2[c] = make_float2(al, -al * phi);
+                o.pack2[packet * 32 + lane] = make_float2(al, -al * phi);
             }
         }
         if (SETS) {
@@ -496,7 +499,7 @@ __device__ __forceinline__ void red_add_v4(float *addr, float a, float b, float 
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
-__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__restrict__ srt, const float *__restrict__ xyz,
+__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, BwdIn in, float *__restrict__ gacc) {
     // the packet's points as PAIRS (2i, 2i + 1) for the packed arithmetic: [i][0] = x0 x1 y0 y1, [i][1] = z0 z1 alpha0 alpha1,
@@ -515,7 +518,7 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
         const uint64_t c = pp.c;
         float alpha = 0.f, beta = 0.f, eps = 0.f;
         if (active && in.pack2) {  // fused MSE: eps = |res| / I = |alpha| * P / 2
-            const float2 s = __ldg(in.pack2 + c);
+            const float2 s = __ldg(in.pack2 + packet * 32 + lane);   // sorted order, see k_points_fwd
             alpha = s.x; beta = s.y; eps = fabsf(s.x) * in.eps_scale;
         } else if (active) {
             const float Ic = in.I[c], ph = in.phi[c];
@@ -602,7 +605,7 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
     }
 }
 
-cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float *xyz, const uint32_t *pt_order,
+cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float4 *xyz, const uint32_t *pt_order,
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group,
                                cudaStream_t s) {
     if (P == 0) return cudaSuccess;
@@ -616,7 +619,7 @@ cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float
     return cudaGetLastError();
 }
 
-cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+cudaError_t launch_points_fwd(const float4 *sorted_rec, const float4 *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const FwdOut &o, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
     const uint64_t packets = (P + 31) / 32;
@@ -628,7 +631,7 @@ cudaError_t launch_points_fwd(const float4 *sorted_rec, const float *xyz, const 
     return cudaGetLastError();
 }
 
-cudaError_t launch_points_bwd(const float4 *sorted_rec, const float *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
+cudaError_t launch_points_bwd(const float4 *sorted_rec, const float4 *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
                               float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
     const uint64_t packets = (P + 31) / 32;

@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(256) k_sc_norm(const float2 *__restrict__ acc,
             if (o.sample_err) o.sample_err[c] = fabsf(res);
             if (o.pack2) {
                 const float al = covered ? __fdividef((float)(2.0 * invP) * res, I) : 0.f;
-                o.pack2[c] = make_float2(al, -al * phi);
+                o.pack2[k] = make_float2(al, -al * phi);   // sorted order, as in gather mode
             }
         }
         if (set_count_for_hits) hits = set_count_for_hits[c];
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(256) k_sc_coef(const float4 *__restrict__ spt,
     if (ok) {
         const uint64_t c = pt_order ? pt_order[k] : k;
         if (in.pack2) {  // fused MSE: eps = |res| / I = |alpha| * P / 2
-            const float2 s = __ldg(in.pack2 + c);
+            const float2 s = __ldg(in.pack2 + k);
             alpha = s.x; beta = s.y; eps = fabsf(s.x) * in.eps_scale;
         } else {
             const float Ic = in.I[c], ph = in.phi[c];
@@ -337,7 +337,8 @@ __global__ void __launch_bounds__(SC_WARPS * 32) k_sc_bwd(const float4 *__restri
 }
 
 // ---- launchers -----------------------------------------------------------------------------------------------------------
-uint64_t scatter_padded_points(uint64_t P) { return (P + 32 * SC_PPL - 1) / (32 * SC_PPL) * (32 * SC_PPL); }
+uint64_t scatter_padded_points(uint64_t P) { return (P + 63) / 64 * 64; }   // whole leaves (32 * SC_PPL <= 64) and whole packets
+static_assert(64 % (32 * SC_PPL) == 0, "leaf size");
 
 // number of tree levels and nodes per level for P points; returns the total node count
 uint32_t scatter_tree_shape(uint64_t P, PtTree *T) {
@@ -356,9 +357,13 @@ uint32_t scatter_tree_shape(uint64_t P, PtTree *T) {
     return off;
 }
 
-cudaError_t launch_scatter_build(const float *xyz, const uint32_t *pt_order, uint64_t P, PtTree T, float4 *spt, float *box, cudaStream_t s) {
+cudaError_t launch_sorted_points(const float *xyz, const uint32_t *pt_order, uint64_t P, float4 *spt, cudaStream_t s) {
     const uint64_t Ppad = scatter_padded_points(P ? P : 1);
     k_sc_sorted<<<(unsigned)((Ppad + 255) / 256), 256, 0, s>>>(xyz, pt_order, P, Ppad, spt); count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_build(uint64_t P, PtTree T, const float4 *spt, float *box, cudaStream_t s) {
     for (int l = 0; l < T.levels; l++) {
         const uint32_t n = T.n[l];
         k_sc_level<<<(unsigned)(((size_t)n * 32 + 255) / 256), 256, 0, s>>>(l == 0 ? spt : nullptr, l ? box + T.off[l - 1] : nullptr, l ? T.n[l - 1] : 0u,
