@@ -404,10 +404,12 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         Is = torch.empty(len(qs) * Pb, device="cuda")
         ctx.gs_preprocess(*gd, tau=TAU)
 
+        views = [(q, phis[k * Pb:(k + 1) * Pb], Is[k * Pb:(k + 1) * Pb]) for k, q in enumerate(qs)]
+
         def decode():
-            for k, q in enumerate(qs):
+            for q, p_, i_ in views:
                 ctx.gs_build_accel(q)
-                ctx.gs_sample_fwd(q, phis[k * Pb:(k + 1) * Pb], Is[k * Pb:(k + 1) * Pb])
+                ctx.gs_sample_fwd(q, p_, i_)
         decode(); barrier()
         reps = max(1, int(math.ceil(1e3 * MIN_TIMED_S / (0.2 * len(qs)))))
         ctx.profile_read(); ctx.profile_enable(True)

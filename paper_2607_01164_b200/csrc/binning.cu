@@ -14,6 +14,8 @@
 // Brick ranges are integer decisions: fixed fp32 sequence (D7).
 #include "gs_internal.cuh"
 #include "pair_math.cuh"
+#include <algorithm>
+using std::max;
 
 namespace gs {
 
@@ -111,6 +113,67 @@ __device__ __forceinline__ void for_each_pair(const BrickRange &br, uint32_t c, 
     }
 }
 
+// ---- coarse index (small batches of a large grid).  A batch looks only at the Gaussians listed in the coarse cells it
+// overlaps; a Gaussian listed in several of them is handled in the FIRST one (lowest coordinates) of the batch it overlaps.
+__device__ __forceinline__ void coarse_range(const float *__restrict__ bb, const GridDesc &gd, int (&lo)[3], int (&hi)[3], bool &empty) {
+    empty = false;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const float nb = (float)gd.nb_total[k];
+        float fl = floorf(__fmul_rn(__fsub_rn(bb[k], gd.origin[k]), gd.inv_brick[k]));
+        float fh = floorf(__fmul_rn(__fsub_rn(bb[3 + k], gd.origin[k]), gd.inv_brick[k]));
+        fl = fminf(fmaxf(fl, -1.0f), nb);
+        fh = fminf(fmaxf(fh, -1.0f), nb);
+        const int l = max((int)fl, 0), h = min((int)fh, gd.nb_total[k] - 1);
+        empty |= h < l;   // also the (+inf, -inf) box of an invalid Gaussian
+        lo[k] = l / COARSE_B;
+        hi[k] = h / COARSE_B;
+    }
+}
+
+// which Gaussian does thread t of a count / fill pass look at?  Returns false for a thread without one.
+__device__ __forceinline__ bool pick_gaussian(const CandSegs &cs, const float *__restrict__ aabb, const GridDesc &gd, uint32_t N, uint32_t t,
+                                              uint32_t &i) {
+    if (!cs.ids) { i = t; return t < N; }
+    // With an index the candidates are few (a batch touches a sliver of the model): ONE candidate per warp, held by lane 0, so
+    // that for_each_pair deals its bricks to the 32 lanes at once (32 candidates per warp made every warp walk a chain of
+    // dependent atomic round trips: 30 us for 12,600 candidates)
+    if (t & 31u) return false;
+    t >>= 5;
+    if (t >= cs.total) return false;
+    int sg = 0;
+    while (t >= cs.prefix[sg + 1]) sg++;
+    i = cs.ids[cs.start[sg] + (t - cs.prefix[sg])];
+    int lo[3], hi[3];
+    bool empty;
+    float b6[6];
+#pragma unroll
+    for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
+    coarse_range(b6, gd, lo, hi, empty);
+    // owner = the first coarse cell of (Gaussian's cells) intersected with (batch's cells)
+    return !empty && max(lo[0], cs.clo[0]) == cs.cell[sg][0] && max(lo[1], cs.clo[1]) == cs.cell[sg][1] && max(lo[2], cs.clo[2]) == cs.cell[sg][2];
+}
+
+__global__ void __launch_bounds__(256) k_coarse_index(const float *__restrict__ aabb, uint32_t N, GridDesc gd, int ncx, int ncy,
+                                                       uint32_t *__restrict__ hist, const uint32_t *__restrict__ start, uint32_t *__restrict__ ids) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float b6[6];
+#pragma unroll
+    for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
+    int lo[3], hi[3];
+    bool empty;
+    coarse_range(b6, gd, lo, hi, empty);
+    if (empty) return;
+    for (int z = lo[2]; z <= hi[2]; z++)
+        for (int y = lo[1]; y <= hi[1]; y++)
+            for (int x = lo[0]; x <= hi[0]; x++) {
+                const uint32_t c = ((uint32_t)z * ncy + y) * ncx + x;
+                if (ids) ids[start[c] + (atomicSub(hist + c, 1u) - 1u)] = i;   // second pass: take a slot (counts the cell down to zero)
+                else atomicAdd(hist + c, 1u);
+            }
+}
+
 // Morton code of the Gaussian's central brick, coarsened to at most ORDER_BITS bits per axis: the processing
 // order of the backward pass (performance only: neighbouring Gaussians are processed together so that their
 // voxel data stays in L1/L2).
@@ -130,12 +193,14 @@ __device__ __forceinline__ uint32_t order_key(const BrickRange &br, const GridDe
 __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ aabb, const float4 *__restrict__ rec, uint32_t N,
                                                       GridDesc gd, float rcut, uint32_t *__restrict__ count,
                                                       unsigned long long *__restrict__ total, uint32_t *__restrict__ hist,
-                                                      uint32_t nbricks, int order_shift, float4 *__restrict__ setup) {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+                                                      uint32_t nbricks, int order_shift, float4 *__restrict__ setup,
+                                                      const __grid_constant__ CandSegs cs) {
+    uint32_t i = 0;
+    const bool mine = pick_gaussian(cs, aabb, gd, N, blockIdx.x * blockDim.x + threadIdx.x, i);
     const int lane = threadIdx.x & 31;
     uint32_t c = 0;
     BrickRange br{};
-    if (i < N) {
+    if (mine) {
         const float *bb = aabb + 6 * (size_t)i;
         // an invalid Gaussian has the empty box (+inf, -inf): fmaxf/fminf clamp it to an empty range.
         // NaN cannot occur here (preprocess writes inf for invalid ones).
@@ -181,7 +246,7 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
                                                reach * reach * 1.001953125f, 1.0f / (e0 * e0 + e1 * e1 + e2 * e2), 0.f);
       }
     }
-    if (!__any_sync(0xffffffffu, c != 0u)) return;  // a warp whose 32 Gaussians all miss the batch (most warps of a small batch)
+    if (!cs.ids && !__any_sync(0xffffffffu, c != 0u)) return;  // a warp whose 32 Gaussians all miss the batch (most warps of a small batch)
     for_each_pair(br, c, i, gd, lane, [&](uint32_t b, uint32_t) { atomicAdd(hist + b, 1u); });
     // 64-bit totals: pairs (overflow check) in the low counter, touched Gaussians in the next one
     unsigned long long s = c, m = c ? 1ull : 0ull;
@@ -189,6 +254,15 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
     for (int d = 16; d > 0; d >>= 1) {
         s += __shfl_xor_sync(0xffffffffu, s, d);
         m += __shfl_xor_sync(0xffffffffu, m, d);
+    }
+    if (cs.ids) {   // a warp per candidate: thousands of warps would queue up on the two counters; add them per CTA
+        __shared__ unsigned long long red[2];
+        if (threadIdx.x == 0) { red[0] = 0ull; red[1] = 0ull; }
+        __syncthreads();
+        if (lane == 0 && s) { atomicAdd(&red[0], s); atomicAdd(&red[1], m); }
+        __syncthreads();
+        if (threadIdx.x == 0 && red[0]) { atomicAdd(total, red[0]); atomicAdd(total + 1, red[1]); }
+        return;
     }
     if (lane == 0 && s) { atomicAdd(total, s); atomicAdd(total + 1, m); }
 }
@@ -199,14 +273,19 @@ __global__ void __launch_bounds__(256) k_brick_count(const float *__restrict__ a
 __global__ void __launch_bounds__(256) k_pair_fill(const float *__restrict__ aabb, const uint32_t *__restrict__ count, uint32_t N, GridDesc gd,
                                                     const unsigned long long *__restrict__ total, uint32_t cap,
                                                     uint32_t *__restrict__ hist, const uint32_t *__restrict__ start, uint32_t nbricks,
-                                                    int order_shift, uint32_t *__restrict__ pair_gauss, uint32_t *__restrict__ order) {
-    if (total[0] > (unsigned long long)cap) return;
+                                                    int order_shift, uint32_t *__restrict__ pair_gauss, uint32_t *__restrict__ order,
+                                                    const __grid_constant__ CandSegs cs) {
+    if (total[0] > (unsigned long long)cap) {   // the list does not fit: write nothing; total[3] remembers it for the host (sticky)
+        if (blockIdx.x == 0 && threadIdx.x == 0) const_cast<unsigned long long *>(total)[3] = 1ull;
+        return;
+    }
     const uint32_t T = (uint32_t)total[0];
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t i = 0;
+    const bool mine = pick_gaussian(cs, aabb, gd, N, blockIdx.x * blockDim.x + threadIdx.x, i);
     const int lane = threadIdx.x & 31;
     uint32_t c = 0;
     BrickRange br{};
-    if (i < N && count[i]) {  // the count pass left n_i: untouched Gaussians cost 4 bytes here
+    if (mine && count[i]) {  // the count pass left n_i: untouched Gaussians cost 4 bytes here
         float b6[6];
 #pragma unroll
         for (int k = 0; k < 6; k++) b6[k] = aabb[6 * (size_t)i + k];
@@ -344,23 +423,60 @@ __global__ void __launch_bounds__(256) k_expand_bricks(const uint32_t *__restric
 
 cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
                                unsigned long long *total, uint32_t *hist, uint32_t nbricks, uint32_t norder, int order_shift,
-                               float4 *setup, cudaStream_t s) {
-    cudaError_t e = cudaMemsetAsync(total, 0, 2 * sizeof(unsigned long long), s);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(hist, 0, ((size_t)nbricks + norder) * sizeof(uint32_t), s);
-    if (e != cudaSuccess || N == 0) return e;
-    k_brick_count<<<(N + 255) / 256, 256, 0, s>>>(aabb, rec, N, gd, rcut, count, total, hist, nbricks, order_shift, setup); count_launch();
+                               float4 *setup, const CandSegs &cs, cudaStream_t s) {
+    // (total, hist and -- with an index -- the stale counts were reset by launch_build_reset)
+    if (N == 0) return cudaSuccess;
+    const uint64_t work64 = cs.ids ? (uint64_t)cs.total * 32 : N;   // with an index: a warp per candidate (pick_gaussian)
+    if (work64 == 0 || work64 > 0xffffff00ull) return work64 ? cudaErrorInvalidValue : cudaSuccess;
+    const uint32_t work = (uint32_t)work64;
+    k_brick_count<<<(work + 255) / 256, 256, 0, s>>>(aabb, rec, N, gd, rcut, count, total, hist, nbricks, order_shift, setup, cs); count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
                              uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
-                             uint32_t *order, cudaStream_t s) {
+                             uint32_t *order, const CandSegs &cs, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
-    k_pair_fill<<<(N + 255) / 256, 256, 0, s>>>(aabb, count, N, gd, total, cap, hist, start, nbricks, order_shift, pair_gauss, order); count_launch();
+    const uint32_t work = cs.ids ? cs.total * 32u : N;
+    if (work) { k_pair_fill<<<(work + 255) / 256, 256, 0, s>>>(aabb, count, N, gd, total, cap, hist, start, nbricks, order_shift, pair_gauss, order, cs); count_launch(); }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_bucket_sort<<<(nbricks + BS_WARPS - 1) / BS_WARPS, BS_WARPS * 32, 0, s>>>(total, cap, start, nbricks, pair_gauss); count_launch();
+    return cudaGetLastError();
+}
+
+// One launch instead of three memsets in front of every build (small batches are bound by the host's launch rate): zero the
+// pair / touched totals and the brick + order histogram, and -- when the previous batch came from the coarse index -- put the
+// counts of ITS candidates back to zero (the other Gaussians already read "touches nothing").
+__global__ void __launch_bounds__(256) k_build_reset(unsigned long long *__restrict__ total, uint32_t *__restrict__ hist, uint32_t nh,
+                                                      uint32_t *__restrict__ count, const __grid_constant__ CandSegs prev) {
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < 2) total[t] = 0ull;
+    if (t < nh) hist[t] = 0u;
+    if (prev.ids && t < prev.total) {
+        int sg = 0;
+        while (t >= prev.prefix[sg + 1]) sg++;
+        count[prev.ids[prev.start[sg] + (t - prev.prefix[sg])]] = 0u;
+    }
+}
+
+cudaError_t launch_build_reset(unsigned long long *total, uint32_t *hist, uint32_t nh, uint32_t *count, const CandSegs &prev, cudaStream_t s) {
+    const uint32_t work = max(max(nh, prev.ids ? prev.total : 0u), 2u);
+    k_build_reset<<<(work + 255) / 256, 256, 0, s>>>(total, hist, nh, count, prev); count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_coarse_count(const float *aabb, uint32_t N, const GridDesc &full, const int nc[3], uint32_t *hist, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(hist, 0, (size_t)nc[0] * nc[1] * nc[2] * sizeof(uint32_t), s);
+    if (e != cudaSuccess || N == 0) return e;
+    k_coarse_index<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, full, nc[0], nc[1], hist, nullptr, nullptr); count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_coarse_fill(const float *aabb, uint32_t N, const GridDesc &full, const int nc[3], uint32_t *hist, const uint32_t *start,
+                               uint32_t *ids, cudaStream_t s) {
+    if (N == 0) return cudaSuccess;
+    k_coarse_index<<<(N + 255) / 256, 256, 0, s>>>(aabb, N, full, nc[0], nc[1], hist, start, ids); count_launch();
     return cudaGetLastError();
 }
 

@@ -118,20 +118,26 @@ CullLists cull_lists(gs_ctx *ctx) {
 
 // GS_OPT_ASYNC_BUILD: pick up the pair count T and the touched count M of the last grid build once they have arrived in
 // pinned host memory.  If T outgrew the speculative buffer the kernels of that batch did nothing: grow, and report it.
-gs_status resolve_grid_counts(gs_ctx *ctx) {
+gs_status resolve_grid_counts(gs_ctx *ctx, bool wait = true) {
     if (!ctx->grid_pending) return GS_OK;
+    if (!wait) {   // between the batches of a stream of builds: take the counts if they have arrived, never stall the host
+        const cudaError_t q = cudaEventQuery(ctx->grid_event);
+        if (q == cudaErrorNotReady) return GS_OK;
+        if (q != cudaSuccess) return fail_cuda(ctx, q, "query the pair count");
+    } else {
+        cudaError_t e = cudaEventSynchronize(ctx->grid_event);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "wait for the pair count");
+    }
     ctx->grid_pending = false;
-    cudaError_t e = cudaEventSynchronize(ctx->grid_event);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "wait for the pair count");
-    const unsigned long long T = ctx->grid_host[0], M = ctx->grid_host[1];
-    const size_t cap = ctx->pair_gauss.cap / 4;
-    if (T >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
-    if (T > cap) {
+    const unsigned long long T = ctx->grid_host[0], M = ctx->grid_host[1], sticky = ctx->grid_host[3];
+    if (sticky) {   // some batch since the last look outgrew the speculative pair buffer: its kernels did nothing
+        cudaMemsetAsync(ctx->counters.as<unsigned long long>() + 7, 0, 8, ctx->stream);
         ctx->accel_kind = -1;
         ctx->grid_warm_N = 0xffffffffu;   // the next build is synchronous and sizes the buffer
-        return fail(ctx, GS_ERR_OVERFLOW, "asynchronous build: the pair list of the previous batch outgrew its speculative capacity; "
+        return fail(ctx, GS_ERR_OVERFLOW, "asynchronous build: the pair list of an earlier batch outgrew its speculative capacity; "
                                           "that batch's outputs are invalid -- repeat it (the next gs_build_accel is synchronous)");
     }
+    if (T >= (1ull << 32)) return fail(ctx, GS_ERR_OVERFLOW, "pair count T does not fit 32 bits");
     ctx->T = (uint32_t)T;
     ctx->M = ctx->M_hint = (uint32_t)M;
     return GS_OK;
@@ -149,6 +155,67 @@ uint32_t grid_M_launch(gs_ctx *ctx) {
     if (!ctx->grid_pending) return ctx->M;
     const uint64_t b = (uint64_t)ctx->M_hint + ctx->M_hint / 4 + 4096;
     return (uint32_t)(b < ctx->N ? b : ctx->N);
+}
+
+bool same_geometry(const GridDesc &a, const GridDesc &b) {
+    for (int k = 0; k < 3; k++)
+        if (a.dims[k] != b.dims[k] || a.origin[k] != b.origin[k] || a.spacing[k] != b.spacing[k]) return false;
+    return true;
+}
+
+// Candidate Gaussians of a grid batch.  A batch that covers a small part of a large grid (configs[3]: a 128^3 batch touches
+// 0.3 % of the model) should not look at every Gaussian: from the second such batch after a gs_preprocess on, a coarse index
+// (cells of COARSE_B^3 bricks) built once over the whole model hands every batch the Gaussians of the <= 8 cells it overlaps.
+gs_status batch_candidates(gs_ctx *ctx, const GridDesc &gd, uint32_t nbricks, CandSegs *cs) {
+    memset(cs, 0, sizeof *cs);
+    const uint32_t N = ctx->N;
+    int nc[3], clo[3], chi[3];
+    uint64_t total_bricks = 1, ncell = 1, nbatch = 1;
+    for (int k = 0; k < 3; k++) {
+        nc[k] = (gd.nb_total[k] + COARSE_B - 1) / COARSE_B;
+        clo[k] = gd.brick_lo[k] / COARSE_B;
+        chi[k] = (gd.brick_lo[k] + gd.brick_cnt[k] - 1) / COARSE_B;
+        total_bricks *= (uint64_t)gd.nb_total[k];
+        ncell *= (uint64_t)nc[k];
+        nbatch *= (uint64_t)(chi[k] - clo[k] + 1);
+    }
+    const bool small = N >= 65536 && (uint64_t)nbricks * 8 <= total_bricks && nbatch <= 8 && ncell <= (1u << 24);
+    if (!small || ctx->builds_since_pre < 1) return GS_OK;   // the first batch after a preprocess pays the full pass (a training step has only one)
+    cudaStream_t s = ctx->stream;
+    if (!ctx->cidx_valid || !same_geometry(ctx->cidx_geom, gd)) {
+        GridDesc full = gd;
+        for (int k = 0; k < 3; k++) { full.brick_lo[k] = 0; full.brick_cnt[k] = gd.nb_total[k]; full.bdim[k] = gd.dims[k]; }
+        CK(ctx->cidx_hist.reserve(ncell * 4), "alloc coarse index");
+        CK(ctx->cidx_start.reserve((ncell + 1) * 4), "alloc coarse index");
+        CK(launch_coarse_count(ctx->aabb.as<float>(), N, full, nc, ctx->cidx_hist.as<uint32_t>(), s), "coarse count");
+        CK(exclusive_scan_u32(ctx->cidx_hist.as<uint32_t>(), ctx->cidx_start.as<uint32_t>(), ncell, ctx->scan_tmp, s), "coarse scan");
+        ctx->cidx_start_host.resize(ncell + 1);
+        CK(cudaMemcpyAsync(ctx->cidx_start_host.data(), ctx->cidx_start.p, (ncell + 1) * 4, cudaMemcpyDeviceToHost, s), "read coarse index");
+        CK(cudaStreamSynchronize(s), "sync (coarse index)");   // once per index, i.e. once per decode
+        CK(ctx->cidx_ids.reserve(((size_t)ctx->cidx_start_host[ncell] + 1) * 4), "alloc coarse index");
+        CK(launch_coarse_fill(ctx->aabb.as<float>(), N, full, nc, ctx->cidx_hist.as<uint32_t>(), ctx->cidx_start.as<uint32_t>(),
+                              ctx->cidx_ids.as<uint32_t>(), s), "coarse fill");
+        ctx->cidx_valid = true;
+        ctx->cidx_geom = gd;
+        for (int k = 0; k < 3; k++) ctx->cidx_nc[k] = nc[k];
+    }
+    cs->ids = ctx->cidx_ids.as<uint32_t>();
+    uint32_t n = 0, run = 0;
+    for (int z = clo[2]; z <= chi[2]; z++)
+        for (int y = clo[1]; y <= chi[1]; y++)
+            for (int x = clo[0]; x <= chi[0]; x++) {
+                const size_t c = ((size_t)z * nc[1] + y) * nc[0] + x;
+                cs->start[n] = ctx->cidx_start_host[c];
+                cs->prefix[n] = run;
+                run += ctx->cidx_start_host[c + 1] - ctx->cidx_start_host[c];
+                cs->cell[n][0] = x; cs->cell[n][1] = y; cs->cell[n][2] = z;
+                n++;
+            }
+    for (uint32_t k = n; k <= 8; k++) cs->prefix[k] = run;
+    cs->n = n;
+    cs->total = run;
+    for (int k = 0; k < 3; k++) cs->clo[k] = clo[k];
+    return GS_OK;
 }
 
 int bits_for(uint64_t n) {  // bits needed to represent values in [0, n)
@@ -185,7 +252,7 @@ void gs_destroy(gs_ctx *ctx) {
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
                      &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
-                     &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef, &ctx->rn_xyz, &ctx->rn_phi, &ctx->rn_I};
+                     &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef, &ctx->rn_xyz, &ctx->rn_phi, &ctx->rn_I, &ctx->cidx_hist, &ctx->cidx_start, &ctx->cidx_ids};
     for (DevBuf *b : all) b->release();
     for (DevBuf &b : ctx->h2d) b.release();
     for (auto *v : {&ctx->prof_pending, &ctx->prof_free})
@@ -214,6 +281,10 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     ctx->have_pre = false;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
+    ctx->cidx_valid = false;
+    ctx->builds_since_pre = 0;
+    ctx->prev_cand.ids = nullptr;
+    ctx->bcount_exact = false;
     const size_t n = g->n ? g->n : 1;
     CK(ctx->rec.reserve(n * 64), "alloc records");
     CK(ctx->aabb.reserve(n * 24), "alloc aabb");
@@ -243,7 +314,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     gs_status st = validate_query(ctx, q, &gd, &P);
     if (st != GS_OK) return st;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
-    if ((st = resolve_grid_counts(ctx)) != GS_OK) return st;
+    if ((st = resolve_grid_counts(ctx, /*wait=*/false)) != GS_OK) return st;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
     cudaStream_t s = ctx->stream;
@@ -266,8 +337,22 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         CK(ctx->bwd_setup.reserve(n1 * 32), "alloc backward setup");
         CK(ctx->pair_gauss.reserve(4), "alloc pair list");
         unsigned long long *total = ctx->counters.as<unsigned long long>() + 4;
+        CandSegs cs;
+        if ((st = batch_candidates(ctx, gd, nbricks, &cs)) != GS_OK) return st;
+        ctx->builds_since_pre++;
+        {   // reset of the counters in front of the passes: one launch (plus a whole-array memset the first time the index is used)
+            CandSegs prev = ctx->prev_cand;
+            if (cs.ids && !ctx->bcount_exact) {
+                CK(cudaMemsetAsync(ctx->bcount.p, 0, (size_t)N * 4, s), "memset counts");
+                prev.ids = nullptr;
+            }
+            if (!cs.ids) prev.ids = nullptr;   // a full pass writes every count itself
+            CK(launch_build_reset(total, ctx->bhist.as<uint32_t>(), (uint32_t)nh, ctx->bcount.as<uint32_t>(), prev, s), "build reset");
+            ctx->prev_cand = cs;
+            ctx->bcount_exact = cs.ids != nullptr;
+        }
         CK(launch_brick_count(ctx->aabb.as<float>(), ctx->rec.as<float4>(), N, gd, ctx->r, ctx->bcount.as<uint32_t>(), total,
-                              ctx->bhist.as<uint32_t>(), nbricks, norder, order_shift, ctx->bwd_setup.as<float4>(), s), "brick count");
+                              ctx->bhist.as<uint32_t>(), nbricks, norder, order_shift, ctx->bwd_setup.as<float4>(), cs, s), "brick count");
         CK(exclusive_scan_u32(ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nh, ctx->scan_tmp, s), "scan");
         // The pair list is filled speculatively into the buffer the previous step left; T is read back once, at the
         // end, and the fill is repeated only when the buffer had to grow (it writes nothing when T exceeds `cap`).
@@ -279,8 +364,8 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
             const size_t cap = ctx->pair_gauss.cap / 4;
             CK(launch_pair_fill(ctx->aabb.as<float>(), ctx->bcount.as<uint32_t>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
                                 ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
-                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), s), "pair fill");
-            CK(cudaMemcpyAsync(ctx->grid_host, total, 16, cudaMemcpyDeviceToHost, s), "read T (async)");
+                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), cs, s), "pair fill");
+            CK(cudaMemcpyAsync(ctx->grid_host, total, 32, cudaMemcpyDeviceToHost, s), "read T (async)");   // T, M, (invalid count), sticky overflow
             CK(cudaEventRecord(ctx->grid_event, s), "event");
             ctx->grid_pending = true;
             T64[0] = ctx->T;        // last known values until the real ones arrive (debug views resolve first)
@@ -290,7 +375,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
             const size_t cap = ctx->pair_gauss.cap / 4;
             CK(launch_pair_fill(ctx->aabb.as<float>(), ctx->bcount.as<uint32_t>(), N, gd, total, (uint32_t)(cap < 0xffffffffull ? cap : 0xffffffffull),
                                 ctx->bhist.as<uint32_t>(), ctx->brick_start.as<uint32_t>(), nbricks, order_shift,
-                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), s), "pair fill");
+                                ctx->pair_gauss.as<uint32_t>(), ctx->grid_order.as<uint32_t>(), cs, s), "pair fill");
             if (attempt == 0) {
                 CK(cudaMemcpyAsync(T64, total, sizeof T64, cudaMemcpyDeviceToHost, s), "read T");
                 CK(cudaStreamSynchronize(s), "sync (T)");
@@ -304,10 +389,12 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         const uint32_t T = (uint32_t)T64[0];
         ctx->M = (uint32_t)T64[1];
         if (!async) {
+            // the synchronous path handles an overflowing fill itself (grow + repeat): forget the device's sticky note of it
+            if (ctx->opt_async_build) CK(cudaMemsetAsync(total + 3, 0, 8, s), "clear overflow note");
             ctx->M_hint = ctx->M;
             if (ctx->opt_async_build) {
                 if (!ctx->grid_host) {
-                    CK(cudaMallocHost(reinterpret_cast<void **>(&ctx->grid_host), 16), "alloc pinned counters");
+                    CK(cudaMallocHost(reinterpret_cast<void **>(&ctx->grid_host), 32), "alloc pinned counters");
                     CK(cudaEventCreateWithFlags(&ctx->grid_event, cudaEventDisableTiming), "event");
                 }
                 ctx->grid_warm_N = N;

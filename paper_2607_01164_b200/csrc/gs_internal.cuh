@@ -46,6 +46,17 @@ struct GridDesc {          // one batch of a structured grid (gs_query, GS_QUERY
     unsigned long long jitter_seed;
 };
 
+// Candidate Gaussians of a grid batch from the coarse index (binning.cu): up to 8 coarse cells, each a slice of the index's
+// id list.  ids == NULL: no index, every Gaussian of the model is looked at.
+constexpr int COARSE_B = 16;   // bricks per coarse cell and axis (128 voxels: the batch size of configs[3])
+struct CandSegs {
+    const uint32_t *ids;
+    uint32_t n, total;          // segments, candidates (with duplicates: a Gaussian is listed in every coarse cell it overlaps)
+    uint32_t start[8], prefix[9];
+    int cell[8][3];             // coarse coordinates of the segment's cell
+    int clo[3];                 // first coarse cell of the batch per axis
+};
+
 // scatter mode of a point query (sample_scatter.cu): implicit 32-ary tree over the Morton-sorted query points
 struct PtTree {
     const float *box;   // per level SoA boxes: box[off[l] + k * n[l] + i], k = lo.xyz hi.xyz
@@ -114,6 +125,15 @@ struct gs_ctx {
     gs::DevBuf pair_brick;   // uint32 [T]: debug view only (gs_debug_get)
     gs::DevBuf grid_order;   // uint32 [M]: processing order of the backward
     gs::DevBuf brick_start;  // uint32 [nbricks + norder + 1]: runs of the bricks, then of the order buckets (offset by T)
+    // coarse index over the Gaussians (built when small batches of a large grid follow one another without a gs_preprocess)
+    gs::DevBuf cidx_hist, cidx_start, cidx_ids;
+    std::vector<uint32_t> cidx_start_host;
+    bool cidx_valid = false;
+    int cidx_nc[3] = {0, 0, 0};
+    gs::GridDesc cidx_geom{};
+    uint32_t builds_since_pre = 0;   // grid builds since the last gs_preprocess
+    gs::CandSegs prev_cand{};        // candidates of the previous build (their counts are cleared by the next one); ids == NULL: none
+    bool bcount_exact = false;       // bcount holds 0 for every Gaussian outside prev_cand (false: unknown, clear everything)
     gs::DevBuf jit;          // float4 [P]: sample positions of a jittered grid batch (D26)
     gs::DevBuf bwd_setup;    // float4 [N][2]: per-Gaussian constants of the structured backward (k_brick_count)
     // ---- accel (points)
@@ -180,10 +200,15 @@ cudaError_t radix_sort_pairs(uint32_t *keys[2], uint32_t *vals[2], size_t n, int
 // start = exclusive scan of hist (nbricks + norder + 1 entries).  launch_pair_fill writes nothing when *total > cap.
 cudaError_t launch_brick_count(const float *aabb, const float4 *rec, uint32_t N, const GridDesc &gd, float rcut, uint32_t *count,
                                unsigned long long *total, uint32_t *hist, uint32_t nbricks, uint32_t norder, int order_shift,
-                               float4 *setup, cudaStream_t s);
+                               float4 *setup, const CandSegs &cs, cudaStream_t s);
 cudaError_t launch_pair_fill(const float *aabb, const uint32_t *count, uint32_t N, const GridDesc &gd, const unsigned long long *total, uint32_t cap,
                              uint32_t *hist, const uint32_t *start, uint32_t nbricks, int order_shift, uint32_t *pair_gauss,
-                             uint32_t *order, cudaStream_t s);
+                             uint32_t *order, const CandSegs &cs, cudaStream_t s);
+cudaError_t launch_build_reset(unsigned long long *total, uint32_t *hist, uint32_t nh, uint32_t *count, const CandSegs &prev, cudaStream_t s);
+// coarse index over the Gaussians for small batches of a large grid: cell = COARSE_B^3 bricks; CSR (start[ncells + 1], ids)
+cudaError_t launch_coarse_count(const float *aabb, uint32_t N, const GridDesc &full, const int nc[3], uint32_t *hist, cudaStream_t s);
+cudaError_t launch_coarse_fill(const float *aabb, uint32_t N, const GridDesc &full, const int nc[3], uint32_t *hist, const uint32_t *start,
+                               uint32_t *ids, cudaStream_t s);
 cudaError_t launch_expand_bricks(const uint32_t *start, uint32_t nbricks, uint32_t *key, cudaStream_t s);
 
 // GS_OPT_ASYNC_BUILD: the pair count T and the touched-Gaussian count M of a grid batch stay on the device (total[0],

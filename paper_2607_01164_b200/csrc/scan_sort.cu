@@ -75,6 +75,31 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_tile(const uint32_t *__re
     if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_THREADS - 1) out[n] = pre;
 }
 
+// small inputs (a grid batch's brick histogram): ONE launch, one CTA walking the tiles with a running carry
+constexpr int SCAN_SMALL_THREADS = 1024;
+__global__ void __launch_bounds__(SCAN_SMALL_THREADS) k_scan_small(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, size_t n) {
+    __shared__ uint32_t sm[40];
+    uint32_t carry = 0;
+    for (size_t tile = 0; tile < n; tile += (size_t)SCAN_SMALL_THREADS * SCAN_ITEMS) {
+        const size_t base = tile + (size_t)threadIdx.x * SCAN_ITEMS;
+        uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; k++) {
+            v[k] = (base + k < n) ? in[base + k] : 0u;
+            s += v[k];
+        }
+        uint32_t total;
+        uint32_t pre = block_excl_scan(s, &total, sm) + carry;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; k++) {
+            if (base + k < n) out[base + k] = pre;
+            pre += v[k];
+        }
+        carry += total;
+    }
+    if (threadIdx.x == 0) out[n] = carry;
+}
+
 static cudaError_t scan_rec(const uint32_t *in, uint32_t *out, size_t n, uint32_t *tmp, int write_total, cudaStream_t s) {
     const size_t tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (tiles <= 1) {
@@ -92,6 +117,10 @@ static cudaError_t scan_rec(const uint32_t *in, uint32_t *out, size_t n, uint32_
 
 cudaError_t exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, DevBuf &tmp, cudaStream_t s) {
     if (n == 0) return cudaMemsetAsync(out, 0, sizeof(uint32_t), s);
+    if (n <= 16 * SCAN_TILE) {
+        k_scan_small<<<1, SCAN_SMALL_THREADS, 0, s>>>(in, out, n); count_launch();
+        return cudaGetLastError();
+    }
     const size_t tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     cudaError_t e = tmp.reserve((tiles + 64 + tiles / 1024 + 128) * 2 * sizeof(uint32_t));
     if (e != cudaSuccess) return e;

@@ -265,3 +265,57 @@ def test_jittered_grid(oracle, fused):
         # another seed gives other samples
         run2 = GpuRun(g, "grid", grid, target, fused=True, jitter_seed=seed + 1)
         assert not np.array_equal(run2.np(run2.phi), run.np(run.phi))
+
+
+def test_small_batches_use_the_coarse_index(oracle):
+    # From the second small batch after a gs_preprocess on, the build looks only at the Gaussians of the coarse cells
+    # (16^3 bricks) the batch overlaps.  Batches that straddle 8 / 2 / 1 coarse cells must give the same sorted keys, counts,
+    # ID sets and gradients as the oracle (a Gaussian listed in several cells is handled exactly once).
+    import torch
+    from paper_2607_01164_b200 import api
+    n_grid = 512
+    g = inputs.c4_gaussians(seed=11, n_grid=n_grid, n=70000)
+    g.scale[:] = (g.scale * 6.0).astype(np.float32)      # many Gaussians overlap several coarse cells
+    g.scale[5, 2] = np.nan                                # an invalid one
+    full = inputs.c4_grid(n_grid)
+    ctx = api.Context()
+    dev = [torch.from_numpy(x).cuda() for x in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    ctx.gs_preprocess(*dev)
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    rng = np.random.default_rng(0)
+    for lo, cnt in (((3, 3, 3), (2, 2, 2)),          # first batch: full pass
+                    ((10, 26, 12), (12, 8, 10)),     # straddles 2 x 2 x 2 coarse cells
+                    ((16, 32, 5), (4, 3, 6)),        # one coarse cell, aligned at its corner
+                    ((30, 40, 50), (5, 2, 2)),       # 2 x 1 x 1
+                    ((60, 60, 60), (4, 4, 4))):      # upper corner of the grid
+        batch = full.batch(lo, cnt)
+        P = batch.num_points
+        q = api.grid_query(batch)
+        ctx.gs_build_accel(q)
+        blo, bhi, bc = oracle.brick_ranges(aabb, valid, batch)
+        keys, start = oracle.brick_keys(blo, bhi, bc, batch)
+        assert np.array_equal(ctx.debug_get(api.DBG_BRICK_COUNT, np.uint32), bc)
+        pb = ctx.debug_get(api.DBG_PAIR_BRICK, np.uint32)
+        pg = ctx.debug_get(api.DBG_PAIR_GAUSS, np.uint32)
+        assert np.array_equal((pb.astype(np.uint64) << np.uint64(32)) | pg.astype(np.uint64), keys)
+        assert np.array_equal(ctx.debug_get(api.DBG_BRICK_START, np.uint32).astype(np.int64), start)
+        target = rng.uniform(0, 1, P).astype(np.float32)
+        xyz = oracle.grid_points(batch)
+        fwd = oracle.forward(g, xyz, TAU, mode=1)
+        _, a, _ = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
+        gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
+        phi, I = torch.empty(P, device="cuda"), torch.empty(P, device="cuda")
+        loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ctx.gs_sample_fwd(q, phi, I, target=torch.from_numpy(target).cuda(), loss=loss)
+        grads = ctx.alloc_grads(g.n)
+        for v in grads.values():
+            v.fill_(-7.0)
+        ctx.gs_sample_bwd(q, None, None, None, grads)
+        cnt_, hs, hx, tested, hits = ctx.debug_point_sets(q)
+        assert np.array_equal(cnt_, fwd["count"]) and np.array_equal(hs, fwd["hsum"]) and np.array_equal(hx, fwd["hxor"])
+        assert hits > 0
+        for k, v in gr.items():
+            got = grads[k].cpu().numpy().astype(np.float64)
+            assert np.linalg.norm(got - v) <= 1e-4 * max(np.linalg.norm(v), 1e-30), k
+    assert ctx.gs_status_query()["num_gaussians"] == 70000
+    ctx.close()
