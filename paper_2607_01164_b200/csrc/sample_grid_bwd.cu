@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 #ifndef GS_BWD_WARPS
 #define GS_BWD_WARPS 4
 #define GS_BWD_MINB 4
-#define GS_BWD_GPW 4
+#define GS_BWD_GPW 8
 #define GS_BWD_INTERLEAVE 1
 #endif
 constexpr int BWD_WARPS = GS_BWD_WARPS;
