@@ -537,11 +537,17 @@ def run_ours(args):
         t_wait = time.time()
         while not os.path.exists(gs_build.LIB) and time.time() - t_wait < 600:
             time.sleep(0.5)
-    torch.cuda.set_device(local)
+    torch.cuda.set_device(local % max(torch.cuda.device_count(), 1))
     if world > 1:
         os.environ.setdefault("NCCL_DEBUG", "INFO")          # a scaling run prints its communicator / transport lines
         os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        # one rank per GPU over NCCL; GS_BENCH_BACKEND=gloo only exists to smoke-test this arm's code path where fewer GPUs than
+        # ranks are available (two processes sharing one GPU; never a measurement)
+        backend = os.environ.get("GS_BENCH_BACKEND", "nccl")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
     names = ["c2", "c3", "c4", HEADLINE] if args.workload == "all" else [args.workload]
     head = names[-1]
     sampler = ClockSampler(local)
