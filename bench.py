@@ -378,7 +378,10 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         ms = per[nm]
         ach = hits * instr / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
         tr = traffic.get(f"{wl['name']}/{kpre}{nm}")
-        kernels[nm] = {"kernel": kpre + nm, "launch_ms": ms, "achieved": ach, "frac": ach / ALU_PEAK_TINSTR,
+        # the same figure over the pairs the kernel actually EVALUATES (SURVEY 8d's "issue" fraction, counted for the point
+        # kernels, whose forward and backward walk the same lists): how busy the arithmetic pipes are; frac / issue_frac = cull efficiency
+        issue = tested * instr / (ms * 1e-3) / 1e12 / ALU_PEAK_TINSTR if (ms > 0 and wl["kind"] == "points") else None
+        kernels[nm] = {"kernel": kpre + nm, "launch_ms": ms, "achieved": ach, "frac": ach / ALU_PEAK_TINSTR, "issue_frac": issue,
                        "algorithmic_lane_instr": hits * instr, "traffic": tr["bytes"] if tr else None,
                        "traffic_source": tr["source"] if tr else tsrc}
     dom = "fwd" if per["fwd"] >= per["bwd"] else "bwd"

@@ -183,6 +183,8 @@ gs_status batch_candidates(gs_ctx *ctx, const GridDesc &gd, uint32_t nbricks, Ca
     if (!small || ctx->builds_since_pre < 1) return GS_OK;   // the first batch after a preprocess pays the full pass (a training step has only one)
     cudaStream_t s = ctx->stream;
     if (!ctx->cidx_valid || !same_geometry(ctx->cidx_geom, gd)) {
+        ctx->prev_cand.ids = nullptr;   // the id list is about to be rebuilt (and may move): the counts are cleared wholesale
+        ctx->bcount_exact = false;
         GridDesc full = gd;
         for (int k = 0; k < 3; k++) { full.brick_lo[k] = 0; full.brick_cnt[k] = gd.nb_total[k]; full.bdim[k] = gd.dims[k]; }
         CK(ctx->cidx_hist.reserve(ncell * 4), "alloc coarse index");

@@ -319,3 +319,30 @@ def test_small_batches_use_the_coarse_index(oracle):
             assert np.linalg.norm(got - v) <= 1e-4 * max(np.linalg.norm(v), 1e-30), k
     assert ctx.gs_status_query()["num_gaussians"] == 70000
     ctx.close()
+
+
+def test_coarse_index_follows_a_change_of_grid(oracle):
+    # two different grids queried in small batches against ONE preprocess: the coarse index is rebuilt for the new geometry
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c4_gaussians(seed=12, n_grid=256, n=66000)
+    g.scale[:] = (g.scale * 3.0).astype(np.float32)
+    ctx = api.Context()
+    ctx.gs_preprocess(*[torch.from_numpy(x).cuda() for x in (g.mean, g.scale, g.quat, g.opacity, g.scalar)])
+    M, aabb, valid = oracle.preprocess_f32(g, TAU)
+    for n_grid, batches in ((256, (((2, 2, 2), (3, 3, 3)), ((14, 15, 16), (4, 4, 4)))), (384, (((1, 1, 1), (2, 2, 2)), ((30, 31, 15), (5, 3, 4)), ((0, 0, 0), (3, 2, 2))))):
+        full = inputs.c4_grid(n_grid)
+        for lo, cnt in batches:
+            batch = full.batch(lo, cnt)
+            q = api.grid_query(batch)
+            ctx.gs_build_accel(q)
+            blo, bhi, bc = oracle.brick_ranges(aabb, valid, batch)
+            keys, start = oracle.brick_keys(blo, bhi, bc, batch)
+            assert np.array_equal(ctx.debug_get(api.DBG_BRICK_COUNT, np.uint32), bc)
+            pb = ctx.debug_get(api.DBG_PAIR_BRICK, np.uint32)
+            pg = ctx.debug_get(api.DBG_PAIR_GAUSS, np.uint32)
+            assert np.array_equal((pb.astype(np.uint64) << np.uint64(32)) | pg.astype(np.uint64), keys)
+            ref = oracle.forward(g, oracle.grid_points(batch), TAU, mode=1)
+            cnt_, hs, hx, tested, hits = ctx.debug_point_sets(q)
+            assert np.array_equal(cnt_, ref["count"]) and np.array_equal(hs, ref["hsum"]) and np.array_equal(hx, ref["hxor"])
+    ctx.close()
