@@ -83,6 +83,10 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
                                                               uint32_t M, const float4 *__restrict__ jit /*JIT: per-voxel sample positions*/, DevCount dc) {
     __shared__ uint32_t queue[BWD_WARPS][QCAP];
+    // records (4 planes) + setup rows (2) of the Gaussian being processed and of the next one: copied asynchronously one
+    // Gaussian ahead, so that a Gaussian starts from shared memory instead of six dependent L2 round trips
+    __shared__ float4 gstage[BWD_WARPS][2][8];
+    __shared__ __align__(16) float red[BWD_WARPS][32][32];   // the 32 x 32 transpose of the final reduction
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // a warp processes GPW consecutive Gaussians of the brick-ordered list of the M Gaussians that touch the batch
     // slot `rep` of this warp is entry w0 + rep * wstride of the order list
@@ -106,12 +110,25 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     const bool odd_x = (gd.bdim[0] & 1) != 0;  // x-pairs of coefficients are 16-byte aligned only for an even x extent
     uint32_t *q = queue[warp];
 
+    // lane l < 6 copies piece l of Gaussian `id` (planes a..d, setup rows 0..1) into stage buffer `buf`
+    auto fetch = [&](uint32_t id, int buf) {
+        if (lane < 6) {
+            const float4 *src = lane < 4 ? rec + (size_t)lane * N + id : setup + 2 * (size_t)id + (lane - 4);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&gstage[warp][buf][lane]);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    fetch(__shfl_sync(0xffffffffu, my_id, 0), 0);
     for (int rep = 0; rep < GPW && w0 + rep * wstride < M; rep++) {
     const uint32_t i = __shfl_sync(0xffffffffu, my_id, rep);
-    const float4 ga = __ldg(rec + i), gb = __ldg(rec + (size_t)N + i), gc = __ldg(rec + 2 * (size_t)N + i),
-                 gd4 = __ldg(rec + 3 * (size_t)N + i);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+    const float4 *gs_ = gstage[warp][rep & 1];
+    const float4 ga = gs_[0], gb = gs_[1], gc = gs_[2], gd4 = gs_[3];
     // cell box of the AABB inside the batch, cull threshold and 1 / |e|^2: precomputed per Gaussian (k_brick_count)
-    const float4 s0 = __ldg(setup + 2 * (size_t)i), s1 = __ldg(setup + 2 * (size_t)i + 1);
+    const float4 s0 = gs_[4], s1 = gs_[5];
+    if (rep + 1 < GPW && w0 + (rep + 1) * wstride < M) fetch(__shfl_sync(0xffffffffu, my_id, rep + 1), (rep + 1) & 1);
     const int clo[3] = {__float_as_int(s0.x), __float_as_int(s0.y), __float_as_int(s0.z)};
     const uint32_t flags = __float_as_uint(s0.w), ncp = __float_as_uint(s1.x);
     if (flags & 1u) {  // touches a brick of the batch but none of its voxels: a zero row (rows are not pre-zeroed)
@@ -121,11 +138,6 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     const bool edge = (flags & 2u) || odd_x;
     const int ncx = (int)(ncp & 1023u) + 1, ncy = (int)((ncp >> 10) & 1023u) + 1, ncz = (int)((ncp >> 20) & 1023u) + 1;
     const float thr = s1.y, invA = s1.z;
-    if (rep + 1 < GPW && w0 + (rep + 1) * wstride < M) {  // pull the next Gaussian's records towards L1 while this one is processed
-        const uint32_t nx = __shfl_sync(0xffffffffu, my_id, rep + 1);
-        const void *pf = lane < 4 ? (const void *)(rec + (size_t)lane * N + nx) : (const void *)(setup + 2 * (size_t)nx);
-        if (lane < 5) asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
-    }
 
     float acc[32];
 #pragma unroll
@@ -325,10 +337,23 @@ __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const flo
     }
     drain(0u);
 
-    warp_reduce32(acc, lane);
-    // lane c holds component c: one coalesced 128-byte row per Gaussian
-    gacc[(size_t)i * GACC_GRID + lane] = acc[0];
-    __syncwarp();
+    // Reduction over the lanes through a 32 x 32 transpose in shared memory: lane L stores its 32 partial sums as row L
+    // (16-byte chunks swizzled by L & 7: conflict-free per quarter warp), then sums column L (for a fixed row the 32 lanes read
+    // the 32 distinct words of one 128-byte row).  8 STS.128 + 32 LDS + 32 FADD instead of the 31-shuffle butterfly with its
+    // 62 selects; the summation order is fixed, so the result stays bit-deterministic.
+    {
+        float4 *row = reinterpret_cast<float4 *>(red[warp][lane]);
+#pragma unroll
+        for (int k = 0; k < 8; k++) row[k ^ (lane & 7)] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
+        __syncwarp();
+        const int kc = lane >> 2, e = lane & 3;
+        float s4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int r = 0; r < 32; r++) s4[r & 3] += red[warp][r][((kc ^ (r & 7)) << 2) | e];
+        // lane c holds component c: one coalesced 128-byte row per Gaussian
+        gacc[(size_t)i * GACC_GRID + lane] = (s4[0] + s4[1]) + (s4[2] + s4[3]);
+        __syncwarp();
+    }
     }  // rep
     }  // cta slot
 }
