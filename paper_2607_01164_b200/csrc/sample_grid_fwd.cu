@@ -18,7 +18,7 @@
 namespace gs {
 
 #ifndef GS_FWD_MINB
-#define GS_FWD_MINB 14  // resident CTAs per SM the register allocation must allow (swept 1, 12, 14, 16, 20, 24)
+#define GS_FWD_MINB 12  // resident CTAs per SM the register allocation must allow (swept 10, 12, 14, 16 with the packed list building)
 #endif
 constexpr int FWD_THREADS = 64;
 constexpr int CAP = 128;  // Gaussians staged per round (4 sub-chunks of 32)
@@ -132,20 +132,27 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
             const float ez0 = gb.z * sz2, ez1 = gc.z * sz2, ez2 = gd4.z * sz2;
             const float exx = ex0 * ex0 + ex1 * ex1 + ex2 * ex2;  // |ex|^2
             const int word = sub >> 5;
+            // two y-rows of cells per packed instruction (f32x2.cuh; a cull bound, not the canonical sequence):
+            // y = z + iy ey for iy = (0, 1) and (2, 3) in the halves; |y + ix ex|^2 = |y|^2 + ix (2 y.ex) + ix^2 |ex|^2
+            const f2 ex0d = bc(2.f * ex0), ex1d = bc(2.f * ex1), ex2d = bc(2.f * ex2);
 #pragma unroll
             for (int iz = 0; iz < 2; iz++) {
                 const float z0 = fmaf((float)iz, ez0, ub0), z1 = fmaf((float)iz, ez1, ub1), z2 = fmaf((float)iz, ez2, ub2);
 #pragma unroll
-                for (int iy = 0; iy < 4; iy++) {
-                    const float y0 = fmaf((float)iy, ey0, z0), y1 = fmaf((float)iy, ey1, z1), y2 = fmaf((float)iy, ey2, z2);
-                    // |y + ix ex|^2 = |y|^2 + ix (2 y.ex) + ix^2 |ex|^2
-                    const float yy = y0 * y0 + y1 * y1 + y2 * y2;
-                    const float ye = 2.f * (y0 * ex0 + y1 * ex1 + y2 * ex2);
+                for (int ip = 0; ip < 2; ip++) {   // row pair: iy = 2 ip, 2 ip + 1
+                    const f2 iy2 = pk((float)(2 * ip), (float)(2 * ip + 1));
+                    const f2 y0 = fma2(iy2, bc(ey0), bc(z0)), y1 = fma2(iy2, bc(ey1), bc(z1)), y2 = fma2(iy2, bc(ey2), bc(z2));
+                    const f2 yy = fma2(y2, y2, fma2(y1, y1, mul2(y0, y0)));
+                    const f2 ye = fma2(y2, ex2d, fma2(y1, ex1d, mul2(y0, ex0d)));
 #pragma unroll
                     for (int ix = 0; ix < 4; ix++) {
-                        const float qc = fmaf((float)(ix * ix), exx, fmaf((float)ix, ye, yy));
-                        const uint32_t bal = __ballot_sync(0xffffffffu, qc <= thr);
-                        if (lane == 0) mywords[4 * (iz * 16 + iy * 4 + ix) + word] = bal;
+                        float qa, qb;
+                        upk(ix == 0 ? yy : fma2(bc((float)(ix * ix)), bc(exx), fma2(bc((float)ix), ye, yy)), qa, qb);
+                        const uint32_t bala = __ballot_sync(0xffffffffu, qa <= thr), balb = __ballot_sync(0xffffffffu, qb <= thr);
+                        if (lane == 0) {
+                            mywords[4 * (iz * 16 + (2 * ip) * 4 + ix) + word] = bala;
+                            mywords[4 * (iz * 16 + (2 * ip + 1) * 4 + ix) + word] = balb;
+                        }
                     }
                 }
             }
