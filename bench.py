@@ -434,6 +434,30 @@ def measure(wl, args, sampler, world, rank, headline: bool):
                                       "frac": (Pb * 8 / (fwd_ms * 1e-3) / 1e9 / hbm) if (fwd_ms and hbm) else None,
                                       "algorithmic_bytes": "8 B written per sample (Phi, I); records and lists are L2-resident",
                                       "peak_source": "MEASURED_PEAKS.json hbm_gbs (burst copy)"}}
+        # the same 512^3 block as ONE batch (brick-aligned batches may span up to 2048 voxels per axis): the per-batch figure above is
+        # bound by the launch and tail latencies of ~6 small kernels per 128^3 batch, not by arithmetic or bandwidth
+        lo0 = blocks[0]
+        qb = api.grid_query(wl["full"].batch(lo0, (64, 64, 64)))
+        Pbig = api.query_num_points(qb)
+        if Pbig == len(qs) * Pb:
+            ctx.gs_set_option(api.OPT_ASYNC_BUILD, 0)   # 64x the pairs of the batches before: size the pair list synchronously
+            ctx.gs_build_accel(qb); ctx.gs_sample_fwd(qb, phis, Is); barrier()
+            if not args.sync_build:
+                ctx.gs_set_option(api.OPT_ASYNC_BUILD, 1)
+            repb = 5
+            ctx.profile_read(); ctx.profile_enable(True)
+            e0.record()
+            for _ in range(repb):
+                ctx.gs_build_accel(qb)
+                ctx.gs_sample_fwd(qb, phis, Is)
+            e1.record(); barrier()
+            smb, scb, _ = ctx.profile_read(); ctx.profile_enable(False)
+            ms_big = e0.elapsed_time(e1) / repb
+            fwd_big = smb["fwd"] / max(scb["fwd"], 1)
+            out["decode"]["one_batch_512"] = {
+                "what": "the same 512^3 block decoded as ONE brick-aligned batch (gs_build_accel + gs_sample_fwd)",
+                "ms": ms_big, "points_per_s": Pbig / (ms_big * 1e-3), "build_ms": smb["build"] / max(scb["build"], 1), "fwd_ms": fwd_big,
+                "fwd_hbm_frac": (Pbig * 8 / (fwd_big * 1e-3) / 1e9 / hbm) if (fwd_big and hbm) else None}
         del phis, Is
     if world == 1 and wl.get("decode_xyz") is not None:
         allx = wl["decode_xyz"]

@@ -386,6 +386,12 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
             // with GS_OPT_ASYNC_BUILD the buffer keeps 50 % headroom for the speculative fills of the following steps
             const size_t need = ctx->opt_async_build ? (size_t)T64[0] + (size_t)T64[0] / 2 + 1024 : (size_t)T64[0];
             if (need <= cap) break;
+            if ((size_t)T64[0] <= cap) {
+                // the list fitted and IS written (the fill consumed the histogram, so it cannot be repeated): only the headroom
+                // of the asynchronous builds to come is missing -- grow the buffer around its contents
+                CK(ctx->pair_gauss.reserve_keep(need * 4, (size_t)T64[0] * 4, s), "grow pair list");
+                break;
+            }
             CK(ctx->pair_gauss.reserve(need * 4), "alloc pair list");
         }
         const uint32_t T = (uint32_t)T64[0];

@@ -31,6 +31,21 @@ struct DevBuf {
         cap = want;
         return cudaSuccess;
     }
+    // grow to at least `bytes`, keeping the first `keep` bytes of the contents (waits for stream s)
+    cudaError_t reserve_keep(size_t bytes, size_t keep, cudaStream_t s) {
+        if (bytes <= cap) return cudaSuccess;
+        const size_t want = bytes + bytes / 8 + 256;
+        void *np = nullptr;
+        cudaError_t e = cudaMalloc(&np, want);
+        if (e != cudaSuccess) return e;
+        if (p && keep) e = cudaMemcpyAsync(np, p, keep < cap ? keep : cap, cudaMemcpyDeviceToDevice, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { cudaFree(np); return e; }
+        if (p) cudaFree(p);
+        p = np;
+        cap = want;
+        return cudaSuccess;
+    }
     void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
     template <class T> T *as() const { return reinterpret_cast<T *>(p); }
 };

@@ -217,3 +217,31 @@ def test_async_build_matches_synchronous_and_reports_overflow(oracle):
     torch.cuda.synchronize()
     assert torch.equal(phi, ref.phi[:P])
     ctx.close(); ctx2.close()
+
+
+def test_async_sizing_build_keeps_a_list_that_fitted(oracle):
+    # A sizing build under GS_OPT_ASYNC_BUILD whose pair list FITS the buffer it finds (T <= capacity < 1.5 T + headroom): the
+    # list is written by the first fill, which consumes the histogram, so the fill must not be repeated -- the buffer is grown
+    # around its contents instead.  (The situation arises when the option is switched on for a context that has built before,
+    # or when the model grows a little between two sizing builds; it used to write out of bounds.)
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c4_gaussians(seed=5, n_grid=64, n=30000)
+    full = inputs.Grid((64, 64, 64), (0.0, 0.0, 0.0), (1 / 64, 1 / 64, 1 / 64))
+    P = full.num_points
+    ref = GpuRun(g, "grid", full, None)
+    ctx = api.Context()
+    dev = _dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+    q = api.grid_query(full)
+    phi, I = torch.empty(P, device="cuda"), torch.empty(P, device="cuda")
+    ctx.gs_preprocess(*dev)
+    ctx.gs_build_accel(q)                         # synchronous, option off: the buffer holds exactly T pairs (+ 12 % slack)
+    ctx.gs_set_option(api.OPT_ASYNC_BUILD, 1)
+    for step in range(3):                         # step 0: sizing build that finds T <= capacity < 1.5 T; 1, 2: asynchronous
+        phi.fill_(-7.0)
+        ctx.gs_build_accel(q)
+        ctx.gs_sample_fwd(q, phi, I)
+        torch.cuda.synchronize()
+        assert torch.equal(phi, ref.phi[:P]) and torch.equal(I, ref.I[:P]), step
+    assert ctx.gs_status_query()["grid_pairs"] == ref.ctx.gs_status_query()["grid_pairs"]
+    ctx.close()
