@@ -520,6 +520,47 @@ def measure(wl, args, sampler, world, rank, headline: bool):
                          "build_ms_per_chunk": sm["build"] / max(sc["build"], 1), "fwd_ms_per_chunk": sm["fwd"] / max(sc["fwd"], 1)}
         del xs, qs, pp, ii
 
+    # ---- the paper's own training step at this scale: raw parameters, a new random
+    #      position in every cell per iteration, L1 + the false-negative term Eq. 4 fused into the forward, fused
+    #      backward, Adam -- five C-ABI calls, no host arithmetic
+    if world == 1 and wl["name"] == "c2":
+        logit = lambda x: np.log(x / (1 - x))
+        gdr = [dev(a) for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]   # the recipe updates its own copy of the model
+        raw = dict(mean=gdr[0], raw_scale=dev(np.log(g.scale)), quat=gdr[2],
+                   raw_opacity=dev(logit(np.clip(g.opacity.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)),
+                   raw_scalar=dev(logit(np.clip(g.scalar.astype(np.float64), 1e-3, 1 - 1e-3)).astype(np.float32)))
+        m_d, v_d = torch.zeros(12 * g.n, device="cuda"), torch.zeros(12 * g.n, device="cuda")
+        terms = torch.zeros(3, dtype=torch.float64, device="cuda")
+        gr2 = ctx.alloc_grads(g.n)
+        res = {}
+        for label, jit in (("voxel_centres", False), ("jittered", True)):
+            itr = [0]
+
+            def rstep():
+                itr[0] += 1
+                qj = api.grid_query(wl["grid"], jitter_seed=itr[0] if jit else None)
+                ctx.gs_preprocess(raw["mean"], gdr[1], raw["quat"], gdr[3], gdr[4], tau=TAU)
+                ctx.gs_build_accel(qj)
+                ctx.gs_sample_fwd_loss(qj, phi, I, tgt[0], kind=api.LOSS_L1, lambda_fn=0.5, eps_fn=0.5, loss_terms=terms)
+                ctx.gs_sample_bwd(qj, None, None, None, gr2)
+                ctx.gs_adam_step(raw, gr2, m_d, v_d, itr[0], scale_out=gdr[1], opacity_out=gdr[3], scalar_out=gdr[4])
+            for _ in range(3):
+                rstep()
+            barrier()
+            nrep = 100
+            ctx.profile_read(); ctx.profile_enable(True)
+            e0.record()
+            for _ in range(nrep):
+                rstep()
+            e1.record(); barrier()
+            smr, scr, _ = ctx.profile_read(); ctx.profile_enable(False)
+            ms_r = e0.elapsed_time(e1) / nrep
+            res[label] = {"ms_per_step": ms_r, "samples_per_s": P / (ms_r * 1e-3),
+                          "stage_ms": {k: (smr[k] / scr[k] if scr[k] else 0.0) for k in smr}}
+        out["paper_recipe"] = {"what": "preprocess + build_accel + gs_sample_fwd_loss (L1 + Eq. 4) + gs_sample_bwd (fused) + gs_adam_step on all "
+                                       "samples of the grid, 100 consecutive steps of a model that is being updated", **res}
+        del gdr, raw, m_d, v_d, gr2
+
     # ---- volume rendering through gs_render: 512 x 512 rays x 64 samples of the configs[2] model = one 2^24-sample chunk
     if world == 1 and wl["name"] == "c3":
         from paper_2607_01164_b200 import inputs
@@ -641,7 +682,7 @@ def run_ours(args):
                 "config": r["config"], "clocks": r["clocks"], "gpu_launches": r["gpu_launches"], "e2e": r.get("e2e"),
                 "stage_ms": r["stage_ms"], "roofline": r["roofline"], "csrc_sha16": csrc_sha16(),
                 "extra": {"hit_pairs": r["hit_pairs"], "tested_pairs": r["tested_pairs"], "cull_efficiency": r["cull_efficiency"],
-                          "rates": r["rates"], "decode": r.get("decode"), "render": r.get("render"),
+                          "rates": r["rates"], "decode": r.get("decode"), "render": r.get("render"), "paper_recipe": r.get("paper_recipe"),
                           "points_accel": r.get("points_accel"), "async_build": r.get("async_build"),
                           "hbm_peak_gbs_measured": _peaks().get("hbm_gbs")}}
         if "cpu_baseline" in r:

@@ -245,3 +245,44 @@ def test_async_sizing_build_keeps_a_list_that_fitted(oracle):
         assert torch.equal(phi, ref.phi[:P]) and torch.equal(I, ref.I[:P]), step
     assert ctx.gs_status_query()["grid_pairs"] == ref.ctx.gs_status_query()["grid_pairs"]
     ctx.close()
+
+
+def test_contexts_on_their_own_streams_run_side_by_side(oracle):
+    # Contexts are independent (gs.h: a context is bound to the stream given to gs_create; all scratch is context-owned): batches
+    # of one grid dealt round-robin to three contexts on three CUDA streams give exactly the output of one context doing them
+    # in turn.  This is how `bench.py` overlaps the builds and forwards of a configs[3] decode.
+    import torch
+    from paper_2607_01164_b200 import api
+    g = inputs.c4_gaussians(seed=7, n_grid=64, n=40000)
+    full = inputs.Grid((64, 64, 64), (0.0, 0.0, 0.0), (1 / 64, 1 / 64, 1 / 64))
+    dev = _dev(torch, g.mean, g.scale, g.quat, g.opacity, g.scalar)
+    batches = [full.batch((2 * x, 2 * y, 2 * z), (2, 2, 2)) for z in range(4) for y in range(4) for x in range(4)]
+    qs = [api.grid_query(b) for b in batches]
+    Pb = api.query_num_points(qs[0])
+    one = api.Context()
+    one.gs_preprocess(*dev)
+    phi1, I1 = torch.empty(len(qs) * Pb, device="cuda"), torch.empty(len(qs) * Pb, device="cuda")
+    for k, q in enumerate(qs):
+        one.gs_build_accel(q)
+        one.gs_sample_fwd(q, phi1[k * Pb:(k + 1) * Pb], I1[k * Pb:(k + 1) * Pb])
+    torch.cuda.synchronize()
+    ref = oracle.forward(g, oracle.grid_points(batches[5]), TAU, mode=1)    # one batch against the oracle, the rest against `one`
+    assert np.abs(phi1[5 * Pb:6 * Pb].cpu().numpy() - ref["phi"]).max() <= 1e-5
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    ctxs = [api.Context(stream=s_) for s_ in streams]
+    for c, s_ in zip(ctxs, streams):
+        s_.wait_stream(torch.cuda.current_stream())
+        c.gs_set_option(api.OPT_ASYNC_BUILD, 1)
+        c.gs_preprocess(*dev)
+    phi3, I3 = torch.full_like(phi1, -7.0), torch.full_like(I1, -7.0)
+    for s_ in streams:
+        s_.wait_stream(torch.cuda.current_stream())
+    for rep in range(2):
+        for k, q in enumerate(qs):
+            c = ctxs[k % 3]
+            c.gs_build_accel(q)
+            c.gs_sample_fwd(q, phi3[k * Pb:(k + 1) * Pb], I3[k * Pb:(k + 1) * Pb])
+    torch.cuda.synchronize()
+    assert torch.equal(phi3, phi1) and torch.equal(I3, I1)
+    for c in ctxs + [one]:
+        c.close()
