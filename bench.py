@@ -461,44 +461,33 @@ def measure(wl, args, sampler, world, rank, headline: bool):
                 "what": "the same 512^3 block decoded as ONE brick-aligned batch (gs_build_accel + gs_sample_fwd)",
                 "ms": ms_big, "points_per_s": Pbig / (ms_big * 1e-3), "build_ms": smb["build"] / max(scb["build"], 1), "fwd_ms": fwd_big,
                 "fwd_hbm_frac": (Pbig * 8 / (fwd_big * 1e-3) / 1e9 / hbm) if (fwd_big and hbm) else None}
-        # the 128^3 batches again, dealt to SEVERAL contexts on as many streams (each with its own gs_preprocess of the same model):
-        # the build of one batch runs beside the forward of another -- plain use of the public API, a context being bound to a stream
+        # gs_decode_grid: the library's own batch decode -- the same batches dealt to worker contexts on their own streams, so that
+        # the build of one batch runs beside the forward of another.  First the 512^3 block (output compared with the loop above),
+        # then the FULL 1024^3 grid of configs[3] (512 batches of 128^3, 1.07e9 samples, 8.6 GB of output).
         chk = float(phis.double().sum().item())
-        out["decode"]["multi_context"] = []
-        for nctx in (2, 4):
-            streams = [torch.cuda.Stream() for _ in range(nctx - 1)]
-            ctxs = [ctx] + [api.Context(stream=st_) for st_ in streams]
-            for c, st_ in zip(ctxs[1:], streams):
-                if not args.sync_build:
-                    c.gs_set_option(api.OPT_ASYNC_BUILD, 1)
-                st_.wait_stream(torch.cuda.current_stream())
-            for c in ctxs:
-                c.gs_preprocess(*gd, tau=TAU)
-
-            def decode_n():
-                for k, (q, p_, i_) in enumerate(views):
-                    c = ctxs[k % nctx]
-                    c.gs_build_accel(q)
-                    c.gs_sample_fwd(q, p_, i_)
-            phis.zero_()
-            decode_n(); torch.cuda.synchronize()
-            same = float(phis.double().sum().item()) == chk
-            for st_ in streams:
-                st_.wait_stream(torch.cuda.current_stream())
-            e0.record()
-            for _ in range(reps):
-                decode_n()
-            for st_ in streams:
-                torch.cuda.current_stream().wait_stream(st_)
-            e1.record(); torch.cuda.synchronize()
-            ms_bn = e0.elapsed_time(e1) / (reps * len(qs))
-            out["decode"]["multi_context"].append({"contexts": nctx, "ms_per_batch": ms_bn, "points_per_s": Pb / (ms_bn * 1e-3),
-                                                   "same_output_as_one_context": same})
-            for c in ctxs[1:]:
-                c.close()
-        out["decode"]["multi_context_what"] = ("the same 64 batches of 128^3 dealt round-robin to 2 / 4 contexts on their own CUDA streams "
-                                               "(one gs_preprocess of the same model per context): builds and forwards of different batches overlap")
+        region = wl["full"].batch(blocks[0], (64, 64, 64))
+        phis.zero_()
+        ctx.gs_decode_grid(*gd, api.grid_query(region), (16, 16, 16), phis, Is, streams=4, tau=TAU)
+        same = float(phis.double().sum().item()) == chk
         del phis, Is
+        full_q = api.grid_query(wl["full"])
+        Pfull = api.query_num_points(full_q)
+        phif, If = torch.empty(Pfull, device="cuda"), torch.empty(Pfull, device="cuda")
+        sweep = []
+        for nstr in (1, 2, 4, 8):
+            ctx.gs_decode_grid(*gd, full_q, (16, 16, 16), phif, If, streams=nstr, tau=TAU)   # warm: worker contexts, buffers
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ctx.gs_decode_grid(*gd, full_q, (16, 16, 16), phif, If, streams=nstr, tau=TAU)   # returns when the decode is complete
+            dt = time.perf_counter() - t0
+            sweep.append({"streams": nstr, "ms_total": 1e3 * dt, "ms_per_batch": 1e3 * dt / 512, "points_per_s": Pfull / dt,
+                          "hbm_write_frac": (Pfull * 8 / dt / 1e9 / hbm) if hbm else None})
+        best = max(sweep, key=lambda r: r["points_per_s"])
+        out["decode"]["full_grid"] = {"what": "gs_decode_grid over the whole 1024^3 grid of configs[3]: 512 batches of 128^3, forward only, host "
+                                              "wall clock around the (synchronous) call, including the workers' gs_preprocess of the model",
+                                      "points": Pfull, "best": best, "sweep": sweep, "block_512_same_output_as_one_context": same,
+                                      "covered_fraction": float((If > TAU).float().mean().item())}
+        del phif, If
     if world == 1 and wl.get("decode_xyz") is not None:
         allx = wl["decode_xyz"]
         chunk = 1 << 24

@@ -345,8 +345,24 @@ typedef struct gs_status_info {
     uint64_t grid_pairs;          /* grid accel: T = (brick, gaussian) pairs of the current batch          */
     uint64_t grid_touched;        /* grid accel: Gaussians that overlap a brick of the current batch       */
     uint64_t cull_chunk_capacity; /* point accel: 32-entry list chunks the pool holds                      */
+    uint64_t decode_repeats;      /* batches gs_decode_grid repeated so far (asynchronous build overflow)  */
 } gs_status_info;
 gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host);
+
+/* ---- forward-only decode of a region of a structured grid in brick-aligned batches (BASELINE.json configs[3]: "decoded in
+ * 128^3 brick-aligned batches, forward-only full decode"; the use the paper's models are made for) ----------
+ * `region` is a GS_QUERY_GRID descriptor (no jitter) whose brick_lo / brick_cnt give the sub-box to decode; it is cut into
+ * batches of batch_bricks[0..2] bricks (the last batch per axis may be smaller), enumerated x fastest.  Every batch is one
+ * gs_build_accel + gs_sample_fwd; the batches are dealt round-robin to num_streams (1..8, 0 = 4) worker contexts that the
+ * library keeps on CUDA streams of its own, each with its own gs_preprocess of the model, so that the build of one batch
+ * runs beside the forward of another (a 128^3 batch is a chain of small kernels: launch- and tail-bound on one stream).
+ * Output layout: BATCH-MAJOR.  phi / I (device, region's sample count) hold batch 0's samples first (in that batch's own
+ * x-fastest order, exactly what gs_sample_fwd writes for it), then batch 1's, ...  The values are those of gs_sample_fwd.
+ * g: device arrays, read on ctx's stream order (the workers wait for everything enqueued on it so far).  The call returns
+ * when the decode is COMPLETE (it synchronises the worker streams).  The context's own preprocess / accel state is not
+ * touched.  Errors: INVALID_ARG, OOM, OVERFLOW, CUDA. */
+gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs_query *region, const int32_t *batch_bricks,
+                         int32_t num_streams, float *phi, float *I);
 
 /* ---- volume rendering over the sampler (Fig. 1, Fig. 9) ---------------
  * Emission-absorption ray marching of the current model (the one given to the last gs_preprocess, which must have had a

@@ -25,7 +25,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render", "gs_decode_grid"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -71,7 +71,7 @@ class _RawParams(C.Structure):
 
 class _StatusInfo(C.Structure):
     _fields_ = [("num_gaussians", C.c_uint64), ("invalid_gaussians", C.c_uint64), ("grid_pairs", C.c_uint64),
-                ("grid_touched", C.c_uint64), ("cull_chunk_capacity", C.c_uint64)]
+                ("grid_touched", C.c_uint64), ("cull_chunk_capacity", C.c_uint64), ("decode_repeats", C.c_uint64)]
 
 
 class _AdamCfg(C.Structure):
@@ -124,6 +124,7 @@ def load_library():
     lib.gs_set_sample_count.argtypes = [P, C.c_uint64]
     lib.gs_set_option.argtypes = [P, C.c_int32, C.c_int64]
     lib.gs_render.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, C.c_uint32, P]
+    lib.gs_decode_grid.argtypes = [P, C.POINTER(_Gaussians), C.c_float, C.POINTER(_Query), C.POINTER(C.c_int32), C.c_int32, P, P]
     lib.gs_status_query.argtypes = [P, C.POINTER(_StatusInfo)]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
@@ -324,6 +325,13 @@ class Context:
         """Ray-march the current model (gs.h gs_render): device tensors origins/dirs [n,3], t_range [n,2], table [K,4], rgba [n,4]."""
         self._check(self.lib.gs_render(self.h, C.c_uint32(int(origins.shape[0])), _ptr(origins), _ptr(dirs), _ptr(t_range),
                                        C.c_uint32(int(spp)), _ptr(table), C.c_uint32(int(table.shape[0])), _ptr(rgba)))
+
+    def gs_decode_grid(self, mean, scale, quat, opacity, scalar, region: _Query, batch_bricks, phi, I, streams: int = 0, tau: float = 0.01):
+        """Forward-only decode of `region` (a grid query: its brick_lo / brick_cnt give the sub-box) in batches of batch_bricks
+        bricks, dealt to `streams` worker contexts (gs.h gs_decode_grid).  phi / I: device tensors, BATCH-MAJOR."""
+        g = _gaussians(mean, scale, quat, opacity, scalar)
+        bb = (C.c_int32 * 3)(*[int(x) for x in batch_bricks])
+        self._check(self.lib.gs_decode_grid(self.h, C.byref(g), C.c_float(tau), C.byref(region), bb, C.c_int32(int(streams)), _ptr(phi), _ptr(I)))
 
     def gs_set_option(self, key: int, value: int):
         self._check(self.lib.gs_set_option(self.h, C.c_int32(int(key)), C.c_int64(int(value))))

@@ -248,6 +248,9 @@ gs_status gs_create(int device, void *cuda_stream, gs_ctx **out) {
 void gs_destroy(gs_ctx *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    for (gs_ctx *w : ctx->decode_workers) gs_destroy(w);
+    for (cudaStream_t ws : ctx->decode_streams) cudaStreamDestroy(ws);
+    if (ctx->decode_event) cudaEventDestroy(ctx->decode_event);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->bhist, &ctx->pair_gauss, &ctx->pair_brick,
                      &ctx->grid_order, &ctx->brick_start, &ctx->jit, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
@@ -884,6 +887,99 @@ gs_status gs_render(gs_ctx *ctx, uint32_t num_rays, const float *origins, const 
     return GS_OK;
 }
 
+gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs_query *region, const int32_t *batch_bricks,
+                         int32_t num_streams, float *phi, float *I) {
+    LaunchScope launch_scope(ctx);
+    if (!ctx) return GS_ERR_INVALID_ARG;
+    if (!g || !region || !batch_bricks) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: NULL argument");
+    if (region->kind != GS_QUERY_GRID || region->jitter) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: region must be a grid query without jitter");
+    if (num_streams == 0) num_streams = 4;
+    if (num_streams < 1 || num_streams > 8) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: num_streams must lie in [1, 8] (0 = 4)");
+    uint64_t nbatch[3], total_batches = 1;
+    for (int k = 0; k < 3; k++) {
+        if (batch_bricks[k] < 1 || batch_bricks[k] > 256) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: batch_bricks must lie in [1, 256]");
+        if (region->dims[k] < 1 || region->brick_lo[k] < 0 || region->brick_cnt[k] < 1 || BRICK * (int64_t)region->brick_lo[k] >= region->dims[k])
+            return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: empty or misplaced region");
+        nbatch[k] = ((uint64_t)region->brick_cnt[k] + batch_bricks[k] - 1) / batch_bricks[k];
+        total_batches *= nbatch[k];
+    }
+    uint64_t Ptot = 1;
+    for (int k = 0; k < 3; k++) {
+        const int64_t ext = BRICK * (int64_t)region->brick_cnt[k], rest = (int64_t)region->dims[k] - BRICK * (int64_t)region->brick_lo[k];
+        Ptot *= (uint64_t)(ext < rest ? ext : rest);
+    }
+    if (Ptot > 0 && (!phi || !I)) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: phi and I must be given");
+    CK(cudaSetDevice(ctx->device), "cudaSetDevice");
+    // ---- workers: one context per stream, each with its own preprocess of the model (records, index, build buffers)
+    while ((int)ctx->decode_workers.size() < num_streams) {
+        cudaStream_t ws = nullptr;
+        CK(cudaStreamCreateWithFlags(&ws, cudaStreamNonBlocking), "decode stream");
+        gs_ctx *w = nullptr;
+        if (gs_create(ctx->device, ws, &w) != GS_OK) { cudaStreamDestroy(ws); return fail(ctx, GS_ERR_OOM, "gs_decode_grid: worker context"); }
+        gs_set_option(w, GS_OPT_ASYNC_BUILD, 1);
+        ctx->decode_streams.push_back(ws);
+        ctx->decode_workers.push_back(w);
+    }
+    if (!ctx->decode_event) CK(cudaEventCreateWithFlags(&ctx->decode_event, cudaEventDisableTiming), "event");
+    CK(cudaEventRecord(ctx->decode_event, ctx->stream), "event");   // the model arrays may be produced on the caller's stream
+    auto worker_fail = [&](gs_ctx *w, gs_status st) { return fail(ctx, st, gs_last_error(w)); };
+    for (int k = 0; k < num_streams; k++) {
+        gs_ctx *w = ctx->decode_workers[k];
+        CK(cudaStreamWaitEvent(ctx->decode_streams[k], ctx->decode_event, 0), "wait");
+        const gs_status st = gs_preprocess(w, g, nullptr, tau);
+        if (st != GS_OK) return worker_fail(w, st);
+    }
+    // ---- batches, round-robin over the workers.  Builds are asynchronous (gs.h GS_OPT_ASYNC_BUILD): a batch whose pair list
+    //      outgrows the worker's speculative buffer does nothing and is reported by the worker's next call; it is then repeated
+    struct Job { gs_query q; uint64_t off; bool valid; };
+    std::vector<Job> last((size_t)num_streams, Job{gs_query{}, 0, false});
+    auto run = [&](gs_ctx *w, const Job &j) -> gs_status {
+        gs_status st = gs_build_accel(w, &j.q);
+        if (st != GS_OK) return st;
+        return gs_sample_fwd(w, &j.q, nullptr, phi + j.off, I + j.off, nullptr, nullptr, nullptr);
+    };
+    uint64_t off = 0, b = 0;
+    for (uint64_t bz = 0; bz < nbatch[2]; bz++)
+        for (uint64_t by = 0; by < nbatch[1]; by++)
+            for (uint64_t bx = 0; bx < nbatch[0]; bx++, b++) {
+                Job j{*region, off, true};
+                const uint64_t bi[3] = {bx, by, bz};
+                uint64_t Pb = 1;
+                for (int k = 0; k < 3; k++) {
+                    const int lo = region->brick_lo[k] + (int)bi[k] * batch_bricks[k];
+                    const int left = region->brick_lo[k] + region->brick_cnt[k] - lo;
+                    j.q.brick_lo[k] = lo;
+                    j.q.brick_cnt[k] = left < batch_bricks[k] ? left : batch_bricks[k];
+                    const int64_t ext = BRICK * (int64_t)j.q.brick_cnt[k], rest = (int64_t)region->dims[k] - BRICK * (int64_t)lo;
+                    Pb *= (uint64_t)(rest <= 0 ? 0 : (ext < rest ? ext : rest));
+                }
+                if (Pb == 0) continue;   // the region's upper end lies beyond the grid
+                const int k = (int)(b % (uint64_t)num_streams);
+                gs_ctx *w = ctx->decode_workers[k];
+                gs_status st = run(w, j);
+                if (st == GS_ERR_OVERFLOW && last[k].valid) {   // the worker's PREVIOUS batch did nothing: repeat it (synchronous build), then this one
+                    ctx->decode_repeats++;
+                    if ((st = run(w, last[k])) != GS_OK) return worker_fail(w, st);
+                    st = run(w, j);
+                }
+                if (st != GS_OK) return worker_fail(w, st);
+                last[k] = j;
+                off += Pb;
+            }
+    // ---- join: pick up the last asynchronous counts of every worker (repeating its last batch if that one overflowed)
+    for (int k = 0; k < num_streams; k++) {
+        gs_ctx *w = ctx->decode_workers[k];
+        gs_status_info info;
+        gs_status st = gs_status_query(w, &info);
+        if (st == GS_ERR_OVERFLOW && last[k].valid) { ctx->decode_repeats++; st = run(w, last[k]); }
+        if (st != GS_OK) return worker_fail(w, st);
+        CK(cudaStreamSynchronize(ctx->decode_streams[k]), "sync (decode)");
+        ctx->launches += w->launches;
+        w->launches = 0;
+    }
+    return GS_OK;
+}
+
 gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value) {
     if (!ctx) return GS_ERR_INVALID_ARG;
     switch (key) {
@@ -920,6 +1016,7 @@ gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host) {
     out_host->invalid_gaussians = ctx->have_pre ? inv : 0;
     if (ctx->accel_kind == GS_QUERY_GRID) { out_host->grid_pairs = ctx->T; out_host->grid_touched = ctx->M; }
     if (ctx->accel_kind == GS_QUERY_POINTS) out_host->cull_chunk_capacity = ctx->cull_cap;
+    out_host->decode_repeats = ctx->decode_repeats;
     return GS_OK;
 }
 

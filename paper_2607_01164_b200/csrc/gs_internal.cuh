@@ -174,6 +174,11 @@ struct gs_ctx {
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr, aux_event2 = nullptr;
     cudaEvent_t points_ready = nullptr;   // set by gs_step_host: gs_build_accel waits for it before it touches the query points
+    // gs_decode_grid: worker contexts on streams of their own (created on first use, destroyed with this context)
+    std::vector<gs_ctx *> decode_workers;
+    std::vector<cudaStream_t> decode_streams;
+    cudaEvent_t decode_event = nullptr;
+    uint64_t decode_repeats = 0;   // batches gs_decode_grid had to repeat (asynchronous build overflow)
     int opt_async_build = 0;    // gs_set_option(GS_OPT_ASYNC_BUILD)
     bool grid_pending = false;  // T / M of the current grid accel are still on their way to grid_host (grid_event)
     unsigned long long *grid_host = nullptr;   // pinned [2]: T, M
