@@ -172,8 +172,10 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
  *   the list speculatively and send the pair count T and the touched-Gaussian count M to pinned host memory WITHOUT
  *   waiting; forward, backward and finalize read M on the device.  The price is CUDA's own error model: if a later batch
  *   produces more than 1.5x the pairs of the sizing build, its kernels do nothing (they check T against the capacity on
- *   the device) and the NEXT call on the context returns GS_ERR_OVERFLOW ("repeat the batch"; the following build is
- *   synchronous again).  gs_debug_get / gs_status_query wait for the counts.  Point queries always synchronise once.
+ *   the device) and a LATER call on the context returns GS_ERR_OVERFLOW (the following build is synchronous again and sizes
+ *   the buffer).  The counts are picked up without stalling the host, so the report can trail the batch by several builds:
+ *   every batch built since the last call that WAITED for the counts (gs_status_query, gs_debug_get, a synchronous build) is
+ *   suspect and should be repeated -- gs_decode_grid does exactly that.  Point queries always synchronise once.
  * Errors: INVALID_ARG (unknown key / value). */
 typedef enum { GS_OPT_POINTS_ACCEL = 0, GS_OPT_ASYNC_BUILD = 1 } gs_option;
 typedef enum { GS_POINTS_GATHER = 0, GS_POINTS_SCATTER = 1 } gs_points_accel;

@@ -4,6 +4,7 @@
 #include <stdio.h>
 #include <string.h>
 #include <new>
+#include <thread>
 
 #include "gs_internal.cuh"
 
@@ -929,53 +930,82 @@ gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs
         const gs_status st = gs_preprocess(w, g, nullptr, tau);
         if (st != GS_OK) return worker_fail(w, st);
     }
-    // ---- batches, round-robin over the workers.  Builds are asynchronous (gs.h GS_OPT_ASYNC_BUILD): a batch whose pair list
-    //      outgrows the worker's speculative buffer does nothing and is reported by the worker's next call; it is then repeated
-    struct Job { gs_query q; uint64_t off; bool valid; };
-    std::vector<Job> last((size_t)num_streams, Job{gs_query{}, 0, false});
-    auto run = [&](gs_ctx *w, const Job &j) -> gs_status {
-        gs_status st = gs_build_accel(w, &j.q);
-        if (st != GS_OK) return st;
-        return gs_sample_fwd(w, &j.q, nullptr, phi + j.off, I + j.off, nullptr, nullptr, nullptr);
-    };
-    uint64_t off = 0, b = 0;
-    for (uint64_t bz = 0; bz < nbatch[2]; bz++)
-        for (uint64_t by = 0; by < nbatch[1]; by++)
-            for (uint64_t bx = 0; bx < nbatch[0]; bx++, b++) {
-                Job j{*region, off, true};
-                const uint64_t bi[3] = {bx, by, bz};
-                uint64_t Pb = 1;
-                for (int k = 0; k < 3; k++) {
-                    const int lo = region->brick_lo[k] + (int)bi[k] * batch_bricks[k];
-                    const int left = region->brick_lo[k] + region->brick_cnt[k] - lo;
-                    j.q.brick_lo[k] = lo;
-                    j.q.brick_cnt[k] = left < batch_bricks[k] ? left : batch_bricks[k];
-                    const int64_t ext = BRICK * (int64_t)j.q.brick_cnt[k], rest = (int64_t)region->dims[k] - BRICK * (int64_t)lo;
-                    Pb *= (uint64_t)(rest <= 0 ? 0 : (ext < rest ? ext : rest));
+    // ---- batches, round-robin over the workers; every worker is driven by a host thread of its own (a 128^3 batch is ~7 CUDA
+    //      calls of a few microseconds each: one thread issuing for all streams would be the bottleneck).  Builds are asynchronous
+    //      (gs.h GS_OPT_ASYNC_BUILD): a batch whose pair list outgrows the worker's speculative buffer does nothing and is reported
+    //      by the worker's next call; it is then repeated.
+    struct Job { gs_query q; uint64_t off; };
+    std::vector<std::vector<Job>> jobs((size_t)num_streams);
+    {
+        uint64_t off = 0, b = 0;
+        for (uint64_t bz = 0; bz < nbatch[2]; bz++)
+            for (uint64_t by = 0; by < nbatch[1]; by++)
+                for (uint64_t bx = 0; bx < nbatch[0]; bx++, b++) {
+                    Job j{*region, off};
+                    const uint64_t bi[3] = {bx, by, bz};
+                    uint64_t Pb = 1;
+                    for (int k = 0; k < 3; k++) {
+                        const int lo = region->brick_lo[k] + (int)bi[k] * batch_bricks[k];
+                        const int left = region->brick_lo[k] + region->brick_cnt[k] - lo;
+                        j.q.brick_lo[k] = lo;
+                        j.q.brick_cnt[k] = left < batch_bricks[k] ? left : batch_bricks[k];
+                        const int64_t ext = BRICK * (int64_t)j.q.brick_cnt[k], rest = (int64_t)region->dims[k] - BRICK * (int64_t)lo;
+                        Pb *= (uint64_t)(rest <= 0 ? 0 : (ext < rest ? ext : rest));
+                    }
+                    if (Pb == 0) continue;   // the region's upper end lies beyond the grid
+                    jobs[(size_t)(b % (uint64_t)num_streams)].push_back(j);
+                    off += Pb;
                 }
-                if (Pb == 0) continue;   // the region's upper end lies beyond the grid
-                const int k = (int)(b % (uint64_t)num_streams);
-                gs_ctx *w = ctx->decode_workers[k];
-                gs_status st = run(w, j);
-                if (st == GS_ERR_OVERFLOW && last[k].valid) {   // the worker's PREVIOUS batch did nothing: repeat it (synchronous build), then this one
-                    ctx->decode_repeats++;
-                    if ((st = run(w, last[k])) != GS_OK) return worker_fail(w, st);
-                    st = run(w, j);
-                }
-                if (st != GS_OK) return worker_fail(w, st);
-                last[k] = j;
-                off += Pb;
+    }
+    std::vector<gs_status> wst((size_t)num_streams, GS_OK);
+    std::vector<uint64_t> wrep((size_t)num_streams, 0);
+    auto drive = [&](int k) {
+        gs_ctx *w = ctx->decode_workers[(size_t)k];
+        if (cudaSetDevice(ctx->device) != cudaSuccess) { wst[(size_t)k] = GS_ERR_CUDA; return; }
+        auto run = [&](const Job &j) -> gs_status {
+            const gs_status bs = gs_build_accel(w, &j.q);
+            if (bs != GS_OK) return bs;
+            return gs_sample_fwd(w, &j.q, nullptr, phi + j.off, I + j.off, nullptr, nullptr, nullptr);
+        };
+        const std::vector<Job> &mine = jobs[(size_t)k];
+        // An overflow is reported by a LATER call (the counts are picked up without stalling the host, so the report can trail the
+        // batch by several builds): every batch since the last checkpoint -- a call that waited for the counts and found them
+        // fine -- is then suspect and is done again with SYNCHRONOUS builds (each sizes the grow-only pair list for itself, so the
+        // batch that overflowed fits afterwards and the loop terminates).
+        constexpr size_t CHECK_EVERY = 32;
+        gs_status st = GS_OK;
+        size_t ckpt = 0, n = 0;
+        while (n < mine.size() && st == GS_OK) {
+            st = run(mine[n]);
+            if (st == GS_OK) {
+                n++;
+                if (n - ckpt < CHECK_EVERY && n < mine.size()) continue;
+                gs_status_info info;
+                st = gs_status_query(w, &info);   // waits for the counts of the builds so far
+                if (st == GS_OK) { ckpt = n; continue; }
             }
-    // ---- join: pick up the last asynchronous counts of every worker (repeating its last batch if that one overflowed)
+            if (st != GS_ERR_OVERFLOW) break;
+            wrep[(size_t)k] += n - ckpt;
+            st = gs_set_option(w, GS_OPT_ASYNC_BUILD, 0);
+            for (size_t m = ckpt; m < n && st == GS_OK; m++) st = run(mine[m]);
+            if (st == GS_OK) st = gs_set_option(w, GS_OPT_ASYNC_BUILD, 1);
+            ckpt = n;
+        }
+        if (st == GS_OK && cudaStreamSynchronize(ctx->decode_streams[(size_t)k]) != cudaSuccess) st = GS_ERR_CUDA;
+        wst[(size_t)k] = st;
+    };
+    {
+        std::vector<std::thread> threads;
+        for (int k = 1; k < num_streams; k++) threads.emplace_back(drive, k);
+        drive(0);
+        for (std::thread &t : threads) t.join();
+    }
     for (int k = 0; k < num_streams; k++) {
-        gs_ctx *w = ctx->decode_workers[k];
-        gs_status_info info;
-        gs_status st = gs_status_query(w, &info);
-        if (st == GS_ERR_OVERFLOW && last[k].valid) { ctx->decode_repeats++; st = run(w, last[k]); }
-        if (st != GS_OK) return worker_fail(w, st);
-        CK(cudaStreamSynchronize(ctx->decode_streams[k]), "sync (decode)");
+        gs_ctx *w = ctx->decode_workers[(size_t)k];
         ctx->launches += w->launches;
         w->launches = 0;
+        ctx->decode_repeats += wrep[(size_t)k];
+        if (wst[(size_t)k] != GS_OK) return worker_fail(w, wst[(size_t)k]);
     }
     return GS_OK;
 }
