@@ -495,9 +495,8 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         qs = [api.points_query(x) for x in xs]
         pp = [torch.empty(len(x), device="cuda") for x in xs]
         ii = [torch.empty(len(x), device="cuda") for x in xs]
-        ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
-
-        def decode():
+        def decode():   # from scratch: gs_preprocess, then per chunk gs_build_accel (the first one builds the LBVH, the others reuse it) + forward
+            ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
             for q, p_, i_ in zip(qs, pp, ii):
                 ctx.gs_build_accel(q)
                 ctx.gs_sample_fwd(q, p_, i_)
@@ -506,8 +505,9 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         e0.record(); decode(); decode(); e1.record(); barrier()
         sm, sc, _ = ctx.profile_read(); ctx.profile_enable(False)
         ms_all = e0.elapsed_time(e1) / 2
-        out["decode"] = {"what": f"forward-only decode of the {len(allx)}-point draw in {len(qs)} chunks of <= 2^24 points, one "
-                                 "gs_preprocess, gs_build_accel (LBVH + query sort + cull lists) + gs_sample_fwd per chunk",
+        out["decode"] = {"what": f"forward-only decode of the {len(allx)}-point draw in {len(qs)} chunks of <= 2^24 points: one gs_preprocess "
+                                 "(inside the timed region), then gs_build_accel (query sort + cull lists; the first chunk also builds the LBVH over "
+                                 "the Gaussians, the others reuse it) + gs_sample_fwd per chunk",
                          "chunks": len(qs), "ms_total": ms_all, "points_per_s": len(allx) / (ms_all * 1e-3),
                          "build_ms_per_chunk": sm["build"] / max(sc["build"], 1), "fwd_ms_per_chunk": sm["fwd"] / max(sc["fwd"], 1)}
         del xs, qs, pp, ii

@@ -143,6 +143,9 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
  *   memory) and its list of reachable Gaussians is stored for gs_sample_fwd AND gs_sample_bwd of this
  *   query; the pool of list chunks is context-owned, grow-only, and sized by count-and-repeat.
  *   The lists are conservative culls: membership is decided per pair by the canonical predicate (D4).
+ *   The Gaussian side (codes, sort, tree, refit, records in leaf order) depends on the model alone: the FIRST point query
+ *   after a gs_preprocess builds it, the following ones (the chunks of a decode, of gs_render) reuse it and only sort and
+ *   cull their own points.  A training step calls gs_preprocess and therefore rebuilds the LBVH every step.
  * Errors: STATE (no preprocess; no domain for a point query), INVALID_ARG, OVERFLOW, OOM, CUDA. */
 gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q);
 

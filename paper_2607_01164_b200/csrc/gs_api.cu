@@ -285,6 +285,7 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
     { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
     ctx->have_pre = false;
+    ctx->lbvh_state = 0;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
     ctx->cidx_valid = false;
@@ -435,19 +436,26 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
         CK(ctx->node_flag.reserve(n * 4), "alloc nodes");
         CK(ctx->bvh_nodes.reserve(n * 64), "alloc nodes");
         CK(ctx->sorted_rec.reserve(n * 64), "alloc sorted records");
-        // Morton codes of the means (record plane 0: mu.xyz, w; NaN marks an invalid Gaussian)
-        CK(launch_morton(ctx->rec.as<float>(), 4, ctx->rec.as<float>(), N, ctx->dom, ctx->leaf_key[0].as<uint32_t>(),
-                         ctx->leaf_val[0].as<uint32_t>(), s), "morton (gaussians)");
-        uint32_t *keys[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
-        uint32_t *vals[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
-        CK(radix_sort_pairs(keys, vals, N, 31, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "morton sort (gaussians)");
+        // The Gaussian side depends on the model alone: it is built by the first point query after a gs_preprocess and reused by
+        // the following ones (the chunks of a decode or of gs_render; a training step calls gs_preprocess, so it rebuilds)
         const bool scatter = ctx->opt_points_accel == GS_POINTS_SCATTER;
         ctx->points_mode = ctx->opt_points_accel;
-        if (!scatter)   // the scatter mode only needs the Morton ORDER of the Gaussians (processing order), no tree over them
+        uint32_t *keys[2] = {ctx->leaf_key[0].as<uint32_t>(), ctx->leaf_key[1].as<uint32_t>()};
+        uint32_t *vals[2] = {ctx->leaf_val[0].as<uint32_t>(), ctx->leaf_val[1].as<uint32_t>()};
+        if (ctx->lbvh_state < 1) {
+            // Morton codes of the means (record plane 0: mu.xyz, w; NaN marks an invalid Gaussian)
+            CK(launch_morton(ctx->rec.as<float>(), 4, ctx->rec.as<float>(), N, ctx->dom, ctx->leaf_key[0].as<uint32_t>(),
+                             ctx->leaf_val[0].as<uint32_t>(), s), "morton (gaussians)");
+            CK(radix_sort_pairs(keys, vals, N, 31, ctx->sort_hist, ctx->scan_tmp, s, &ctx->leaf_sel), "morton sort (gaussians)");
+            ctx->lbvh_state = 1;
+        }
+        if (!scatter && ctx->lbvh_state < 2) {   // the scatter mode only needs the Morton ORDER of the Gaussians (processing order), no tree over them
             CK(launch_lbvh(keys[ctx->leaf_sel], vals[ctx->leaf_sel], ctx->aabb.as<float>(), ctx->rec.as<float4>(), N,
                            ctx->node_left.as<int32_t>(), ctx->node_right.as<int32_t>(), ctx->node_parent.as<int32_t>(),
                            ctx->leaf_parent.as<int32_t>(), ctx->node_aabb.as<float>(),
                            ctx->node_flag.as<uint32_t>(), ctx->bvh_nodes.as<float4>(), ctx->sorted_rec.as<float4>(), s), "lbvh");
+            ctx->lbvh_state = 2;
+        }
         // coherence sort of the queries
         ctx->have_pt_order = false;
         if (ctx->points_ready) {   // gs_step_host: the points' H2D copy ran on the aux stream beside preprocess and the LBVH build

@@ -173,6 +173,7 @@ struct gs_ctx {
     gs::DevBuf h2d[16];  // staging for gs_step_host
     cudaStream_t aux_stream = nullptr;  // gs_step_host: the target's H2D copy overlaps preprocess + build
     cudaEvent_t aux_event = nullptr, aux_event2 = nullptr;
+    int lbvh_state = 0;   // Gaussian side of a point accel since the last gs_preprocess: 0 = not built, 1 = Morton order (scatter mode), 2 = + LBVH
     cudaEvent_t points_ready = nullptr;   // set by gs_step_host: gs_build_accel waits for it before it touches the query points
     // gs_decode_grid: worker contexts on streams of their own (created on first use, destroyed with this context)
     std::vector<gs_ctx *> decode_workers;

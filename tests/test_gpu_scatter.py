@@ -134,3 +134,44 @@ def test_scatter_c3_full_size(oracle):
     assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6)
     errs = check_grads(run, gr)
     print("C3 full size, scatter mode: hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs)
+
+
+def test_gaussian_side_is_reused_between_queries_of_one_preprocess(oracle):
+    # gs.h (gs_build_accel): the Gaussian side of a point accel (Morton order, LBVH, records in leaf order) is built by the first
+    # point query after a gs_preprocess and reused by the following ones.  Three different queries after ONE preprocess, with
+    # the mode switched in between (the scatter mode builds the Morton order only, the gather mode then adds the tree), must
+    # give what fresh contexts give; a new preprocess (a moved model) must not see the old tree.
+    import torch
+    from paper_2607_01164_b200 import api
+    xyz_all, t_all = inputs.c3_points(seed=3, p=30000)
+    g = inputs.c3_gaussians(xyz_all, t_all, seed=3, n=8000, sigma_lo=0.004, sigma_hi=0.04)
+    dom = inputs.points_domain(xyz_all)
+    chunks = [np.ascontiguousarray(xyz_all[a:b]) for a, b in ((0, 9001), (9001, 20000), (20000, 30000))]
+    refs = [oracle.forward(g, c, TAU, mode=1) for c in chunks]
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    ctx = api.Context()
+    ctx.gs_preprocess(*dev, domain=dom)
+    modes = [api.POINTS_SCATTER, api.POINTS_GATHER, api.POINTS_GATHER]
+    for c, ref, mode in zip(chunks, refs, modes):
+        ctx.gs_set_option(api.OPT_POINTS_ACCEL, mode)
+        xd = torch.from_numpy(c).cuda()
+        q = api.points_query(xd)
+        ctx.gs_build_accel(q)
+        phi, I = torch.empty(len(c), device="cuda"), torch.empty(len(c), device="cuda")
+        ctx.gs_sample_fwd(q, phi, I)
+        cnt, hs, hx, _, _ = ctx.debug_point_sets(q)
+        assert np.array_equal(cnt, ref["count"]) and np.array_equal(hs, ref["hsum"]) and np.array_equal(hx, ref["hxor"])
+        near = np.abs(ref["I"] - TAU) <= 2e-6 * TAU
+        assert np.abs(phi.cpu().numpy() - ref["phi"])[~near].max() <= 1e-5
+    # the model moves: the next query must rebuild
+    g2 = g.subset(np.arange(g.n))
+    g2.mean[:] = (g.mean + np.float32(0.01)).astype(np.float32)
+    dev2 = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (g2.mean, g2.scale, g2.quat, g2.opacity, g2.scalar)]
+    ctx.gs_preprocess(*dev2, domain=dom)
+    xd = torch.from_numpy(chunks[0]).cuda()
+    q = api.points_query(xd)
+    ctx.gs_build_accel(q)
+    ref2 = oracle.forward(g2, chunks[0], TAU, mode=1)
+    cnt, hs, hx, _, _ = ctx.debug_point_sets(q)
+    assert np.array_equal(cnt, ref2["count"]) and np.array_equal(hs, ref2["hsum"]) and np.array_equal(hx, ref2["hxor"])
+    ctx.close()
