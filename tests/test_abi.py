@@ -40,6 +40,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(api._RawParams) == 48 and api._RawParams.mean.offset == 8
     assert ctypes.sizeof(api._AdamCfg) == 36 and api._AdamCfg.step.offset == 32
     assert api._Loss.defined.offset == 16 and api._Loss.num_defined.offset == 24 and ctypes.sizeof(api._Loss) == 32
+    assert ctypes.sizeof(api._StatusInfo) == 48 and api._StatusInfo.decode_repeats.offset == 40   # gs_status_info: six uint64
 
 
 def test_fails_loudly_without_gpu(lib):
