@@ -53,7 +53,8 @@ __global__ void __launch_bounds__(256) k_pack_samples(const float *__restrict__ 
 #endif
 constexpr int BWD_WARPS = GS_BWD_WARPS;
 constexpr int BWD_MINB = GS_BWD_MINB;  // resident CTAs per SM the register allocation must allow
-constexpr int GPW = GS_BWD_GPW;        // Gaussians per warp
+constexpr int GPW_MANY = GS_BWD_GPW;   // Gaussians per warp when the batch touches many Gaussians (launch sized by Gaussians / (warps x GPW))
+constexpr int GPW_FEW = 1;             // ... when it touches few (configs[3] batches: ~10 k): one Gaussian per warp keeps every SM busy
 constexpr bool INTERLEAVE = GS_BWD_INTERLEAVE;  // the warps of a CTA take neighbouring Gaussians of the order list at the same time
 constexpr int QCAP = 512;  // per-warp ring of surviving cells (power of two, >= 31 + 32 * SLICE)
 constexpr int SLICE = 8;   // cells of its interval a lane pushes per pass
@@ -77,7 +78,7 @@ __device__ __forceinline__ void warp_reduce32(float (&v)[32], int lane) {
     }
 }
 
-template <bool PACK2, bool JIT, bool ASYNC>
+template <bool PACK2, bool JIT, bool ASYNC, int GPW>
 __global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB) k_grid_bwd(const float4 *__restrict__ rec, const float4 *__restrict__ setup, uint32_t N,
                                                               GridDesc gd, const void *__restrict__ pack_, float r2,
                                                               float *__restrict__ gacc, const uint32_t *__restrict__ order,
@@ -369,9 +370,13 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
                             float r2, float *gacc, const uint32_t *order, uint32_t M, const float4 *jit, DevCount dc, cudaStream_t s) {
     // only the M Gaussians of the order list get (and need) an accumulator row: k_finalize reads those alone
     if (M == 0) return cudaSuccess;
-    const unsigned blocks = (M + BWD_WARPS * GPW - 1) / (BWD_WARPS * GPW);
+    // few Gaussians (the launch bound M of a small batch): one per warp, so that the launch has enough CTAs for every SM
+    const bool few = M < 148u * BWD_MINB * BWD_WARPS * GPW_MANY;
+    const int gpw = few ? GPW_FEW : GPW_MANY;
+    const unsigned blocks = (M + BWD_WARPS * gpw - 1) / (BWD_WARPS * gpw);
 #define GS_BWD_LAUNCH(P2_, JIT_, ASYNC_) \
-    k_grid_bwd<P2_, JIT_, ASYNC_><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit, dc)
+    do { if (few) k_grid_bwd<P2_, JIT_, ASYNC_, GPW_FEW><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit, dc); \
+         else k_grid_bwd<P2_, JIT_, ASYNC_, GPW_MANY><<<blocks, BWD_WARPS * 32, 0, s>>>(rec, setup, N, gd, pack, r2, gacc, order, M, jit, dc); } while (0)
     const bool as = dc.total != nullptr;
     if (gd.jitter) {
         if (pack2) { if (as) GS_BWD_LAUNCH(true, true, true); else GS_BWD_LAUNCH(true, true, false); }
