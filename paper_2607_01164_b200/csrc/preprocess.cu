@@ -105,11 +105,33 @@ cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float
 template <bool MOMENTS>
 __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
                                                    const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
-                                                   const uint32_t *__restrict__ touched, DevCount dc) {
+                                                   const uint32_t *__restrict__ touched, DevCount dc, bool vec_zero) {
     // touched != NULL (structured): touched[i] = bricks of the batch Gaussian i overlaps; only those with a non-zero count have
     // an accumulator row, the others get zero gradients right here (no memset pass, no order list, coalesced either way)
     if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;   // asynchronous build whose pair list overflowed
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (touched) {
+        // A small batch of a large model (configs[3]: 0.3 % of 4.2 M Gaussians) leaves almost every warp without a touched
+        // Gaussian: such a warp zeroes its 32 rows of every tensor with 16-byte stores (dmean / dscale: 384 contiguous bytes =
+        // 24 float4, dquat 32, the scalars 8 each) instead of ten strided 4-byte stores per lane
+        const int lane = threadIdx.x & 31;
+        const bool mine = i < N && touched[i] != 0u;
+        const uint32_t i0 = i - (uint32_t)lane;
+        if (vec_zero && !__any_sync(0xffffffffu, mine) && i0 + 32u <= N) {
+            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (lane < 24) {
+                reinterpret_cast<float4 *>(out.dmean + 3 * (size_t)i0)[lane] = z;
+                reinterpret_cast<float4 *>(out.dscale + 3 * (size_t)i0)[lane] = z;
+            }
+            reinterpret_cast<float4 *>(out.dquat)[i] = z;
+            if (lane < 8) {
+                reinterpret_cast<float4 *>(out.dopacity + i0)[lane] = z;
+                reinterpret_cast<float4 *>(out.dscalar + i0)[lane] = z;
+                if (out.err) reinterpret_cast<float4 *>(out.err + i0)[lane] = z;
+            }
+            return;
+        }
+    }
     if (i >= N) return;
     if (touched && touched[i] == 0u) {
 #pragma unroll
@@ -240,8 +262,10 @@ cudaError_t launch_finalize(const float4 *rec, const float *params, const float 
                             float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
     // A 128^3 batch of configs[3] touches 0.3 % of the 4.2 M Gaussians: only those read their 128-byte row.
-    if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc);
-    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, DevCount{nullptr, 0});
+    // the warp-wide zero fill needs 16-byte aligned rows: 32 rows of every tensor start at a multiple of 128 / 384 bytes of its base
+    const bool vec_zero = !(((uintptr_t)out.dmean | (uintptr_t)out.dscale | (uintptr_t)out.dopacity | (uintptr_t)out.dscalar | (uintptr_t)out.err) & 15);
+    if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc, vec_zero);
+    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, DevCount{nullptr, 0}, false);
     count_launch();
     return cudaGetLastError();
 }
