@@ -672,7 +672,8 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     Stage stage(ctx, GS_PROF_FINALIZE);
     const bool grid = ctx->accel_kind == GS_QUERY_GRID;
     CK(launch_finalize(ctx->rec.as<float4>(), ctx->params.as<float>(), ctx->gacc.as<float>(), N, grid, (grid && fused2) ? in.eps_scale : 1.f,
-                       *out, grid ? ctx->bcount.as<uint32_t>() : nullptr, grid ? dev_count(ctx) : DevCount{nullptr, 0}, s), "finalize");
+                       *out, grid ? ctx->bcount.as<uint32_t>() : nullptr, grid ? dev_count(ctx) : DevCount{nullptr, 0},
+                       grid ? grid_M_launch(ctx) : N, s), "finalize");
     return GS_OK;
 }
 

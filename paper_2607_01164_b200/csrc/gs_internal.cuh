@@ -267,9 +267,9 @@ cudaError_t launch_grid_bwd(const float4 *rec, const float4 *setup, uint32_t N, 
 
 // grid_moments: gacc holds the structured backward's rows of moment sums (GACC_GRID floats, spacing-free: the cell steps are
 // folded in), only for the Gaussians with touched[i] != 0 (the others get zero gradients); eps_scale multiplies the error share
-// (fused MSE: eps = |alpha| * eps_scale, else 1)
+// (fused MSE: eps = |alpha| * eps_scale, else 1); touched_bound: an upper bound of the number of touched Gaussians (picks the kernel)
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
-                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, cudaStream_t s);
+                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, uint32_t touched_bound, cudaStream_t s);
 
 // optim.cu: activations of the raw parameters and one Adam step on them
 cudaError_t launch_activate(const gs_raw_params &p, float *scale, float *opacity, float *scalar, cudaStream_t s);

@@ -103,36 +103,9 @@ cudaError_t launch_preprocess(const gs_gaussians &g, float r, float4 *rec, float
 // weight w factored out.  With E_a = column a of M:
 //   U = A + sum_a s1_a E_a;   W = Q + sum_a (E_a B_a^T + B_a E_a^T) + sum_{a<=b} s2_ab (E_a E_b^T + E_b E_a^T) / (1 + [a = b])
 template <bool MOMENTS>
-__global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
-                                                   const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
-                                                   const uint32_t *__restrict__ touched, DevCount dc, bool vec_zero) {
-    // touched != NULL (structured): touched[i] = bricks of the batch Gaussian i overlaps; only those with a non-zero count have
-    // an accumulator row, the others get zero gradients right here (no memset pass, no order list, coalesced either way)
-    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;   // asynchronous build whose pair list overflowed
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (touched) {
-        // A small batch of a large model (configs[3]: 0.3 % of 4.2 M Gaussians) leaves almost every warp without a touched
-        // Gaussian: such a warp zeroes its 32 rows of every tensor with 16-byte stores (dmean / dscale: 384 contiguous bytes =
-        // 24 float4, dquat 32, the scalars 8 each) instead of ten strided 4-byte stores per lane
-        const int lane = threadIdx.x & 31;
-        const bool mine = i < N && touched[i] != 0u;
-        const uint32_t i0 = i - (uint32_t)lane;
-        if (vec_zero && !__any_sync(0xffffffffu, mine) && i0 + 32u <= N) {
-            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (lane < 24) {
-                reinterpret_cast<float4 *>(out.dmean + 3 * (size_t)i0)[lane] = z;
-                reinterpret_cast<float4 *>(out.dscale + 3 * (size_t)i0)[lane] = z;
-            }
-            reinterpret_cast<float4 *>(out.dquat)[i] = z;
-            if (lane < 8) {
-                reinterpret_cast<float4 *>(out.dopacity + i0)[lane] = z;
-                reinterpret_cast<float4 *>(out.dscalar + i0)[lane] = z;
-                if (out.err) reinterpret_cast<float4 *>(out.err + i0)[lane] = z;
-            }
-            return;
-        }
-    }
-    if (i >= N) return;
+__device__ __forceinline__ void finalize_one(uint32_t i, const float4 *__restrict__ rec, const float *__restrict__ params,
+                                             const float *__restrict__ gacc, uint32_t N, float eps_scale, const gs_grads &out,
+                                             const uint32_t *__restrict__ touched) {
     if (touched && touched[i] == 0u) {
 #pragma unroll
         for (int k = 0; k < 3; k++) { out.dmean[3 * (size_t)i + k] = 0.f; out.dscale[3 * (size_t)i + k] = 0.f; }
@@ -227,6 +200,59 @@ __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec
     if (out.err) out.err[i] = valid ? E : 0.f;
 }
 
+template <bool MOMENTS>
+__global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
+                                                   const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
+                                                   const uint32_t *__restrict__ touched, DevCount dc) {
+    // touched != NULL (structured): touched[i] = bricks of the batch Gaussian i overlaps; only those with a non-zero count have
+    // an accumulator row, the others get zero gradients right here (no memset pass, no order list)
+    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;   // asynchronous build whose pair list overflowed
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    finalize_one<MOMENTS>(i, rec, params, gacc, N, eps_scale, out, touched);
+}
+
+// Structured batches that touch a small part of a large model (configs[3]: 0.3 % of 4.2 M Gaussians): a warp owns 128
+// consecutive Gaussians; it reads their touch counts with one 16-byte load per lane and, when none is touched (nearly always),
+// zeroes its 128 rows of every gradient tensor with 16-byte stores (13 per lane) -- a write stream instead of ten strided
+// 4-byte stores per Gaussian; a warp with a touched Gaussian falls back to the per-Gaussian code.  Needs 16-byte aligned tensors.
+template <bool MOMENTS>
+__global__ void __launch_bounds__(256) k_finalize_sparse(const float4 *__restrict__ rec, const float *__restrict__ params,
+                                                          const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
+                                                          const uint32_t *__restrict__ touched, DevCount dc) {
+    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;
+    const int lane = threadIdx.x & 31;
+    const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
+    const uint32_t ngroups = (N + 127u) / 128u;
+    for (uint32_t grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); grp < ngroups; grp += nwarps) {
+        const uint32_t i0 = grp * 128u;
+        const bool full = i0 + 128u <= N;
+        bool any = true;
+        if (full) {
+            const uint4 t = __ldg(reinterpret_cast<const uint4 *>(touched + i0) + lane);
+            any = (t.x | t.y | t.z | t.w) != 0u;
+        }
+        if (!__any_sync(0xffffffffu, any)) {
+            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 *dm = reinterpret_cast<float4 *>(out.dmean + 3 * (size_t)i0), *ds = reinterpret_cast<float4 *>(out.dscale + 3 * (size_t)i0);
+            float4 *dq = reinterpret_cast<float4 *>(out.dquat) + i0;
+#pragma unroll
+            for (int k = 0; k < 3; k++) { dm[32 * k + lane] = z; ds[32 * k + lane] = z; }
+#pragma unroll
+            for (int k = 0; k < 4; k++) dq[32 * k + lane] = z;
+            reinterpret_cast<float4 *>(out.dopacity + i0)[lane] = z;
+            reinterpret_cast<float4 *>(out.dscalar + i0)[lane] = z;
+            if (out.err) reinterpret_cast<float4 *>(out.err + i0)[lane] = z;
+        } else {
+#pragma unroll 1
+            for (int k = 0; k < 4; k++) {
+                const uint32_t i = i0 + 32u * k + lane;
+                if (i < N) finalize_one<MOMENTS>(i, rec, params, gacc, N, eps_scale, out, touched);
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // second pass of gs_sample_fwd_loss (loss.cuh): the forward wrote dL/dI = -lambda_fn on D- and +lambda_fp on U+;
 // Eq. 4 / Eq. 5 divide by |D-| and |U+|, which are complete only now.
@@ -259,13 +285,18 @@ cudaError_t launch_loss_finish(const GenLoss &L, size_t P, double nd, double *lo
 }
 
 cudaError_t launch_finalize(const float4 *rec, const float *params, const float *gacc, uint32_t N, bool grid_moments,
-                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, cudaStream_t s) {
+                            float eps_scale, const gs_grads &out, const uint32_t *touched, DevCount dc, uint32_t touched_bound, cudaStream_t s) {
     if (N == 0) return cudaSuccess;
     // A 128^3 batch of configs[3] touches 0.3 % of the 4.2 M Gaussians: only those read their 128-byte row.
-    // the warp-wide zero fill needs 16-byte aligned rows: 32 rows of every tensor start at a multiple of 128 / 384 bytes of its base
-    const bool vec_zero = !(((uintptr_t)out.dmean | (uintptr_t)out.dscale | (uintptr_t)out.dopacity | (uintptr_t)out.dscalar | (uintptr_t)out.err) & 15);
-    if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc, vec_zero);
-    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, DevCount{nullptr, 0}, false);
+    // sparse variant: a structured batch with a touch-count array over a large model; it needs 16-byte aligned tensors (the rows
+    // of 128 Gaussians then start at multiples of 512 / 1536 bytes of the bases) and the counts 16-byte aligned
+    const bool aligned = !(((uintptr_t)out.dmean | (uintptr_t)out.dscale | (uintptr_t)out.dquat | (uintptr_t)out.dopacity | (uintptr_t)out.dscalar |
+                            (uintptr_t)out.err | (uintptr_t)touched) & 15);
+    if (grid_moments && touched && aligned && N >= (1u << 16) && (uint64_t)touched_bound * 16 <= N) {
+        const unsigned blocks = 148 * 8;   // 8 CTAs of 8 warps per SM, each warp striding over groups of 128 Gaussians
+        k_finalize_sparse<true><<<blocks, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc);
+    } else if (grid_moments) k_finalize<true><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, eps_scale, out, touched, dc);
+    else k_finalize<false><<<(N + 255) / 256, 256, 0, s>>>(rec, params, gacc, N, 1.f, out, nullptr, DevCount{nullptr, 0});
     count_launch();
     return cudaGetLastError();
 }
