@@ -21,8 +21,9 @@
  *     frees it in gs_destroy.
  *   - All work is enqueued on the stream given to gs_create.  Calls return after enqueueing,
  *     except that gs_build_accel synchronises once (grid: to read the pair count T; points: to read
- *     the size of the per-packet cull lists and grow their pool if needed), and gs_step_host / gs_debug_point_sets synchronise before returning.  Outputs are valid once the
- *     caller synchronises the stream.
+ *     the size of the per-packet cull lists and grow their pool if needed; GS_OPT_ASYNC_BUILD removes the grid's), and
+ *     gs_step_host, gs_decode_grid, gs_status_query and the gs_debug_* calls synchronise before returning.  Outputs are
+ *     valid once the caller synchronises the stream.
  *   - Every call returns a gs_status; no exception or abort crosses the ABI.  Arguments are
  *     validated before any launch.  gs_last_error gives a human-readable message for the last
  *     non-OK status of that context.
