@@ -76,7 +76,7 @@ def rel_l2(a, b):
     return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a))
 
 
-def check_forward(run, ref, scalar_range=1.0, tol=1e-5):
+def check_forward(run, ref, scalar_range=1.0, tol=1e-5, tol_I=2e-5):
     """fp32 forward: max abs error <= tol * scalar range (BASELINE.json north_star); I relative.
     Samples whose oracle I is within rounding of tau may legitimately flip coverage: excluded, counted."""
     phi = run.np(run.phi).astype(np.float64)
@@ -88,7 +88,8 @@ def check_forward(run, ref, scalar_range=1.0, tol=1e-5):
     assert err_phi <= tol * scalar_range, f"phi max abs err {err_phi}"
     # I has no north_star tolerance; fp32 bound: |dq| <~ 2 |u| |M||d| 2^-24 * few ~ 1e-5
     # for the anisotropies tested, G = exp(-q/2) => relative error of I up to ~1e-5
-    assert err_I <= 2e-5, f"I max rel err {err_I}"
+    # (the bound grows with the anisotropy: callers that draw more than 20:1 pass tol_I = 2e-5 * anisotropy / 20)
+    assert err_I <= tol_I, f"I max rel err {err_I}"
     return int(near.sum()), float(err_phi), float(err_I)
 
 

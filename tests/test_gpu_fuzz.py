@@ -32,10 +32,29 @@ def _oracle_all(oracle, g, xyz, target, dI):
     return fwd, loss, gr
 
 
-def _floors(gr):
-    # tensors whose exact value may vanish (no hit anywhere, one isolated Gaussian): compare against the size of dL/dv
+def _tol_I(g):
+    # I has no north_star tolerance; its fp32 error is |dq| / 2 with |dq| <~ 2 |u| |M||d| 2^-24, which grows
+    # with the ratio of the longest to the shortest axis: 2e-5 at the 20:1 of the configs, in proportion beyond
+    aniso = float((g.scale.max(axis=1) / g.scale.min(axis=1)).max())
+    return 2e-5 * max(1.0, aniso / 20.0)
+
+
+def _check_loss(run, loss):
+    # L = mean (Phi - t)^2 with Phi to 1e-5: |dL| <= 2 mean|res| 1e-5 <= 2 sqrt(L) 1e-5; the 1e-6 relative figure of the other
+    # tests holds once the rounding errors of thousands of samples average out, not for P = 1
+    got = float(run.loss.item())
+    assert abs(got - loss) <= 1e-6 * loss + (2e-5 * np.sqrt(loss) if run.P < 1000 else 0.0) + 1e-12, (got, loss, run.P)
+
+
+def _floors(gr, g):
+    # Tensors whose exact value vanishes by cancellation (no hit anywhere; an isolated Gaussian, where Phi = v wherever it is
+    # covered): the fp32 result is compared against the size of the terms that cancel -- |dL/dv| times what the chain rule
+    # multiplies it by (1 / sigma for the mean and the scales, the anisotropy for the rotation, 1 / w for the weight)
     ref = max(float(np.linalg.norm(gr["dscalar"])), 1e-30)
-    return {k: ref for k in ("dmean", "dscale", "dquat", "dopacity") if float(np.linalg.norm(gr[k])) < 1e-3 * ref}
+    inv_sigma = float(1.0 / g.scale.min())
+    mult = {"dmean": inv_sigma, "dscale": inv_sigma, "dquat": float((g.scale.max(axis=1) / g.scale.min(axis=1)).max()),
+            "dopacity": float(1.0 / g.opacity.min())}
+    return {k: ref * m for k, m in mult.items() if float(np.linalg.norm(gr[k])) < 1e-3 * ref * m}
 
 
 @pytest.mark.parametrize("seed", range(12))
@@ -69,9 +88,9 @@ def test_random_grid_case(oracle, seed):
         run.ctx.gs_sample_fwd(run.q, run.phi, run.I, target=run.target, loss=run.loss.zero_(), dL_dphi=run.dphi, sample_err=run.serr)
         torch.cuda.synchronize()
     check_sets(run, fwd)
-    check_forward(run, fwd)
-    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6, abs=1e-12)
-    check_grads(run, gr, zero_floor=_floors(gr))
+    check_forward(run, fwd, tol_I=_tol_I(g))
+    _check_loss(run, loss)
+    check_grads(run, gr, zero_floor=_floors(gr, g))
 
 
 @pytest.mark.parametrize("seed", range(12))
@@ -97,6 +116,6 @@ def test_random_points_case(oracle, seed):
     run = GpuRun(g, "points", xyz, target, domain=dom, dL_dI=dI, fused=(dI is None and seed % 2 == 1), presorted=False,
                  points_accel=api.POINTS_SCATTER if seed % 6 == 5 else None)
     check_sets(run, fwd)
-    check_forward(run, fwd)
-    assert float(run.loss.item()) == pytest.approx(loss, rel=1e-6, abs=1e-12)
-    check_grads(run, gr, zero_floor=_floors(gr))
+    check_forward(run, fwd, tol_I=_tol_I(g))
+    _check_loss(run, loss)
+    check_grads(run, gr, zero_floor=_floors(gr, g))
