@@ -415,6 +415,49 @@ gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uin
  * HOST outputs; synchronises.  Errors: INVALID_ARG, OOM, CUDA. */
 gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host);
 
+/* ---- sampling without device allocation ----------------------------------------------------------------------------
+ * Forward sampling (Eq. 2 / Eq. 3; cutoff PAPER.md:116; coverage rule PAPER.md:126) of a SMALL model at a
+ * list of points, for callers that cannot allocate device memory: a host application that handed the whole GPU to its own
+ * memory pool at start-up (cudaMalloc then fails or eats the pool's head-room), a real-time loop that cannot take the
+ * device-wide stall of cudaMalloc / cudaFree, a plug-in that may only touch buffers its host gives it.  Everything else in
+ * this header works through a gs_ctx whose scratch arenas are cudaMalloc'd (gs_create already allocates); this call takes
+ * no context and calls no cudaMalloc, cudaFree or other allocating routine, on any call.
+ *
+ * Its scratch (the per-Gaussian records of S1: means, weights, whitening matrices, cutoff boxes) is a fixed array inside
+ * the library's device image, sized for GS_PROBE_MAX_GAUSSIANS Gaussians: about 1.9 MiB that EVERY GPU which loads this
+ * library holds until the process exits, whether or not this call is ever made.  A model with more Gaussians is refused
+ * (GS_ERR_INVALID_ARG, nothing launched); so are more than GS_PROBE_MAX_POINTS points per call -- split the list.
+ *
+ * device / cuda_stream: the GPU and the cudaStream_t (NULL = default stream) the work is enqueued on; the call returns
+ * after enqueueing and leaves the thread's current device as it found it.  g, xyz[num_points,3], phi[num_points],
+ * I[num_points]: DEVICE memory on that GPU, owned by the caller, layouts and value conventions as for gs_preprocess /
+ * gs_sample_fwd (activated parameters, quaternion normalised inside, invalid Gaussians have empty support, a NaN point
+ * gets I = 0, Phi = 0).  Outputs, valid once the stream is synchronised:
+ *     I_c = sum_hits w_i G_i(p_c),   Phi_c = I_c > tau ? (sum_hits v_i w_i G_i(p_c)) / I_c : 0
+ * with the same per-pair membership decision as gs_sample_fwd (the sets of contributing Gaussians are identical; values
+ * differ from gs_sample_fwd's by fp32 summation order only).  Every Gaussian is tested against every point: the cost is
+ * n * num_points pair tests, which is why the model size is capped.
+ *
+ * First call on a device: it looks up the device address of the scratch array (cudaGetSymbolAddress, once per device,
+ * under a host mutex).  That lookup may make the CUDA runtime load the library's device code onto the GPU, so make the
+ * first call on each device during start-up -- before any stream capture begins and before the time-critical part.
+ * A call with num_points = 0 does the set-up and launches nothing.
+ *
+ * Sharing: all calls on a device use the ONE array, and it keeps the previous call's contents.  Each call overwrites the
+ * rows of its own n Gaussians and clears its one counter before use, and never reads rows beyond n, so calls that run one
+ * after the other (same stream, or ordered by events) are independent of each other.  Calls that may OVERLAP on the GPU
+ * -- different streams without ordering, or several host threads on their own streams -- race on the array and produce
+ * garbage: serialise them.  gs_ctx-based calls never touch the array and may overlap with it freely.
+ *
+ * err_host (nullable): a caller-owned HOST buffer of err_cap bytes that receives a NUL-terminated message for a non-OK
+ * status (there is no context for gs_last_error to consult).
+ * Errors: INVALID_ARG (null pointer, n > GS_PROBE_MAX_GAUSSIANS, num_points > GS_PROBE_MAX_POINTS, tau outside (0,1)),
+ * CUDA (no such device, set-up or launch failure). */
+#define GS_PROBE_MAX_GAUSSIANS 16384u
+#define GS_PROBE_MAX_POINTS (1ull << 31)
+gs_status gs_probe_points_static(int device, void *cuda_stream, const gs_gaussians *g, float tau, const float *xyz,
+                                 uint64_t num_points, float *phi, float *I, char *err_host, size_t err_cap);
+
 #ifdef __cplusplus
 }
 #endif

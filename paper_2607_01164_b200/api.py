@@ -25,7 +25,8 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
            "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
-           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render", "gs_decode_grid"]
+           "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render", "gs_decode_grid",
+           "gs_probe_points_static"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
 
 
@@ -126,6 +127,7 @@ def load_library():
     lib.gs_render.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, C.c_uint32, P]
     lib.gs_decode_grid.argtypes = [P, C.POINTER(_Gaussians), C.c_float, C.POINTER(_Query), C.POINTER(C.c_int32), C.c_int32, P, P]
     lib.gs_status_query.argtypes = [P, C.POINTER(_StatusInfo)]
+    lib.gs_probe_points_static.argtypes = [C.c_int, P, C.POINTER(_Gaussians), C.c_float, P, C.c_uint64, P, P, C.c_char_p, C.c_size_t]
     lib.gs_profile_enable.argtypes = [P, C.c_int32]
     lib.gs_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
     for name in EXPORTS:
@@ -198,6 +200,31 @@ def _domain(dom):
         d.lo[k] = float(dom[0][k])
         d.hi[k] = float(dom[1][k])
     return C.byref(d)
+
+
+PROBE_MAX_GAUSSIANS = 16384   # GS_PROBE_MAX_GAUSSIANS
+
+
+def gs_probe_points_static(mean, scale, quat, opacity, scalar, xyz, phi, I, tau: float = 0.01, device: int | None = None, stream=None):
+    """gs_probe_points_static (gs.h): Phi and I of a model of at most PROBE_MAX_GAUSSIANS Gaussians at xyz[P,3], written
+    into the caller's phi[P] / I[P], without a Context and without any device allocation by the library -- for code
+    that runs inside another application's memory pool or a real-time loop and so cannot call cudaMalloc.  All arrays
+    are device tensors the caller allocated beforehand.  The scratch is one fixed array shared by all calls on the
+    device: do not let two calls overlap on the GPU (use one stream, or order them).  The first call per device does
+    a one-time address lookup; make it at start-up."""
+    import torch
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise GsLibraryError("no CUDA device: the W-VEG sampler has no CPU fallback")
+    device = torch.cuda.current_device() if device is None else int(device)
+    stream = torch.cuda.current_stream(device) if stream is None else stream
+    g = _gaussians(mean, scale, quat, opacity, scalar)
+    n = int(xyz.shape[0])
+    msg = C.create_string_buffer(512)
+    st = lib.gs_probe_points_static(device, C.c_void_p(stream.cuda_stream), C.byref(g), C.c_float(tau), _ptr(xyz) if n else None,
+                                    C.c_uint64(n), _ptr(phi) if n else None, _ptr(I) if n else None, msg, C.c_size_t(len(msg)))
+    if st != GS_OK:
+        raise GsError(st, msg.value.decode())
 
 
 class Context:

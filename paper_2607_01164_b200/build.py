@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgs.so")
 SOURCES = ["gs_api.cu", "preprocess.cu", "scan_sort.cu", "binning.cu", "lbvh.cu", "sample_grid_fwd.cu", "sample_grid_bwd.cu",
-           "sample_points.cu", "sample_scatter.cu", "render.cu", "peaks.cu", "optim.cu", "densify.cu"]
+           "sample_points.cu", "sample_scatter.cu", "render.cu", "peaks.cu", "optim.cu", "densify.cu", "probe_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--expt-extended-lambda", "--expt-relaxed-constexpr"]
 
