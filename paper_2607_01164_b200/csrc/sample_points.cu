@@ -112,7 +112,10 @@ __device__ __forceinline__ PacketPoint load_point(const float4 *__restrict__ spt
     const uint64_t k = packet * 32 + lane;
     pp.active = k < P;
     pp.c = pp.active ? (pt_order ? (uint64_t)pt_order[k] : k) : 0;
-    const float4 v = __ldg(spt + k);   // the copy is padded to a whole number of packets
+    // the copy is NaN-padded to a multiple of 64 points (scatter_padded_points); a cull group of 4 packets can reach past
+    // that, where nothing was allocated: those lanes get NaN without a load
+    const float nan = __int_as_float(0x7fc00000);
+    const float4 v = k < ((P + 63) & ~(uint64_t)63) ? __ldg(spt + k) : make_float4(nan, nan, nan, nan);
     pp.px = v.x; pp.py = v.y; pp.pz = v.z;
     return pp;
 }
