@@ -200,15 +200,26 @@ __device__ __forceinline__ void finalize_one(uint32_t i, const float4 *__restric
     if (out.err) out.err[i] = valid ? E : 0.f;
 }
 
+// zero gradients for Gaussian i: an untouched Gaussian, or every Gaussian of a batch whose asynchronous build overflowed
+// (its backward did nothing; stale rows of an earlier step must not reach the optimiser)
+__device__ __forceinline__ void zero_row(uint32_t i, const gs_grads &out) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) { out.dmean[3 * (size_t)i + k] = 0.f; out.dscale[3 * (size_t)i + k] = 0.f; }
+    reinterpret_cast<float4 *>(out.dquat)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    out.dopacity[i] = 0.f;
+    out.dscalar[i] = 0.f;
+    if (out.err) out.err[i] = 0.f;
+}
+
 template <bool MOMENTS>
 __global__ void __launch_bounds__(256) k_finalize(const float4 *__restrict__ rec, const float *__restrict__ params,
                                                    const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
                                                    const uint32_t *__restrict__ touched, DevCount dc) {
     // touched != NULL (structured): touched[i] = bricks of the batch Gaussian i overlaps; only those with a non-zero count have
     // an accumulator row, the others get zero gradients right here (no memset pass, no order list)
-    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;   // asynchronous build whose pair list overflowed
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) { zero_row(i, out); return; }   // asynchronous build whose pair list overflowed
     finalize_one<MOMENTS>(i, rec, params, gacc, N, eps_scale, out, touched);
 }
 
@@ -220,7 +231,7 @@ template <bool MOMENTS>
 __global__ void __launch_bounds__(256) k_finalize_sparse(const float4 *__restrict__ rec, const float *__restrict__ params,
                                                           const float *__restrict__ gacc, uint32_t N, float eps_scale, gs_grads out,
                                                           const uint32_t *__restrict__ touched, DevCount dc) {
-    if (dc.total && dc.total[0] > (unsigned long long)dc.cap) return;
+    const bool overflowed = dc.total && dc.total[0] > (unsigned long long)dc.cap;   // asynchronous build whose pair list did not fit: all zero
     const int lane = threadIdx.x & 31;
     const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
     const uint32_t ngroups = (N + 127u) / 128u;
@@ -230,7 +241,7 @@ __global__ void __launch_bounds__(256) k_finalize_sparse(const float4 *__restric
         bool any = true;
         if (full) {
             const uint4 t = __ldg(reinterpret_cast<const uint4 *>(touched + i0) + lane);
-            any = (t.x | t.y | t.z | t.w) != 0u;
+            any = !overflowed && (t.x | t.y | t.z | t.w) != 0u;
         }
         if (!__any_sync(0xffffffffu, any)) {
             const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -247,7 +258,10 @@ __global__ void __launch_bounds__(256) k_finalize_sparse(const float4 *__restric
 #pragma unroll 1
             for (int k = 0; k < 4; k++) {
                 const uint32_t i = i0 + 32u * k + lane;
-                if (i < N) finalize_one<MOMENTS>(i, rec, params, gacc, N, eps_scale, out, touched);
+                if (i < N) {
+                    if (overflowed) zero_row(i, out);
+                    else finalize_one<MOMENTS>(i, rec, params, gacc, N, eps_scale, out, touched);
+                }
             }
         }
     }

@@ -37,7 +37,15 @@ __global__ void __launch_bounds__(FWD_THREADS, GS_FWD_MINB) k_grid_fwd(const flo
     __shared__ float4 srec[4][CAP];
     __shared__ uint32_t sid[CAP];
     __shared__ uint4 smask[FWD_THREADS / 32][32];  // [warp][cell] -> masks of the 4 sub-chunks
-    if (ASYNC && dc.total[0] > (unsigned long long)dc.cap) return;   // the speculative pair list did not fit: nothing valid to read
+    if (ASYNC && dc.total[0] > (unsigned long long)dc.cap) {   // the speculative pair list did not fit: nothing valid to read
+        // the status only reaches the host with a later call; a NaN loss tells the caller in band that this batch did not happen
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            const double nan = __longlong_as_double(0x7ff8000000000000ll);
+            if (o.gen.on) atomicAdd(o.gen.sums, nan);
+            else if (o.target && o.loss) atomicAdd(o.loss, nan);
+        }
+        return;
+    }
     const uint32_t b = blockIdx.x;
     const int bx = b % gd.brick_cnt[0], by = (b / gd.brick_cnt[0]) % gd.brick_cnt[1], bz = b / (gd.brick_cnt[0] * gd.brick_cnt[1]);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

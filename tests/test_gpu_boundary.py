@@ -209,6 +209,17 @@ def test_async_build_matches_synchronous_and_reports_overflow(oracle):
     ctx2.gs_sample_fwd(q, phi, I)                # does nothing
     torch.cuda.synchronize()
     assert float(phi.min().item()) == -7.0 and float(phi.max().item()) == -7.0
+    # with a loss and a backward, the batch that did not happen says so in band: NaN loss, zero gradients (never the
+    # -7 "previous step" values), long before the status reaches the host
+    loss.zero_()
+    for v in grads.values():
+        v.fill_(-7.0)
+    ctx2.gs_sample_fwd(q, phi, I, target=t, loss=loss)
+    ctx2.gs_sample_bwd(q, None, None, None, grads)
+    torch.cuda.synchronize()
+    assert np.isnan(float(loss.item()))
+    for k, v in grads.items():
+        assert float(v.abs().max().item()) == 0.0, k
     with pytest.raises(api.GsError) as e:
         ctx2.gs_build_accel(q)
     assert e.value.status == api.GS_ERR_OVERFLOW
