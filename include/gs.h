@@ -175,9 +175,13 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
  *   The first build for a model size is synchronous and leaves 50 % headroom in the pair list; the following builds fill
  *   the list speculatively and send the pair count T and the touched-Gaussian count M to pinned host memory WITHOUT
  *   waiting; forward, backward and finalize read M on the device.  The price is CUDA's own error model: if a later batch
- *   produces more than 1.5x the pairs of the sizing build, its kernels do nothing (they check T against the capacity on
+ *   produces more than 1.5x the pairs of the sizing build, its kernels sample nothing (they check T against the capacity on
  *   the device) and a LATER call on the context returns GS_ERR_OVERFLOW (the following build is synchronous again and sizes
- *   the buffer).  The counts are picked up without stalling the host, so the report can trail the batch by several builds:
+ *   the buffer).  What such a batch leaves behind: phi / I / dL_dphi / sample_err untouched; NaN added to *loss (loss_terms[0]
+ *   of gs_sample_fwd_loss is NaN) -- the in-band sign that the batch did not happen; gs_sample_bwd writes ZERO gradients and
+ *   err for every Gaussian (never the previous step's), so an optimiser step taken before the status arrives sees an empty
+ *   batch.  The call that returns GS_ERR_OVERFLOW has itself done nothing (a gs_preprocess that reports it preprocessed
+ *   nothing: call it again).  The counts are picked up without stalling the host, so the report can trail the batch by several builds:
  *   every batch built since the last call that WAITED for the counts (gs_status_query, gs_debug_get, a synchronous build) is
  *   suspect and should be repeated -- gs_decode_grid does exactly that.  Point queries always synchronise once.
  * Errors: INVALID_ARG (unknown key / value). */
@@ -357,7 +361,8 @@ gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host);
 
 /* ---- forward-only decode of a region of a structured grid in brick-aligned batches (BASELINE.json configs[3]: "decoded in
  * 128^3 brick-aligned batches, forward-only full decode"; the use the paper's models are made for) ----------
- * `region` is a GS_QUERY_GRID descriptor (no jitter) whose brick_lo / brick_cnt give the sub-box to decode; it is cut into
+ * `region` is a GS_QUERY_GRID descriptor (no jitter) whose brick_lo / brick_cnt give the sub-box to decode (inside the grid:
+ * brick_lo + brick_cnt <= ceil(dims / 8) per axis, checked before anything is enqueued); it is cut into
  * batches of batch_bricks[0..2] bricks (the last batch per axis may be smaller), enumerated x fastest.  Every batch is one
  * gs_build_accel + gs_sample_fwd; the batches are dealt round-robin to num_streams (1..8, 0 = 4) worker contexts that the
  * library keeps on CUDA streams of its own, each with its own gs_preprocess of the model, so that the build of one batch
@@ -365,7 +370,8 @@ gs_status gs_status_query(gs_ctx *ctx, gs_status_info *out_host);
  * Output layout: BATCH-MAJOR.  phi / I (device, region's sample count) hold batch 0's samples first (in that batch's own
  * x-fastest order, exactly what gs_sample_fwd writes for it), then batch 1's, ...  The values are those of gs_sample_fwd.
  * g: device arrays, read on ctx's stream order (the workers wait for everything enqueued on it so far).  The call returns
- * when the decode is COMPLETE (it synchronises the worker streams).  The context's own preprocess / accel state is not
+ * when the decode is COMPLETE (it synchronises the worker streams -- on failure too: no work of this call is in flight once
+ * it has returned, but phi / I may then hold the batches that did finish).  The context's own preprocess / accel state is not
  * touched.  Errors: INVALID_ARG, OOM, OVERFLOW, CUDA. */
 gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs_query *region, const int32_t *batch_bricks,
                          int32_t num_streams, float *phi, float *I);
@@ -413,7 +419,11 @@ gs_status gs_profile_read(gs_ctx *ctx, float *ms_host, uint32_t *calls_host, uin
  * current clocks, from register-only loops timed with CUDA events on the context's stream; ffma2 (nullable) =
  * FMA lane-OPERATIONS per second through the packed fma.rn.f32x2 form (two per lane-instruction).
  * HOST outputs; synchronises.  Errors: INVALID_ARG, OOM, CUDA. */
-gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host);
+gs_status gs_measure_alu_peaks2(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host);
+/* The same measurement under the name and prototype this header had before the packed-FMA figure was added (three
+ * arguments, all required).  Kept so that a caller compiled against that header keeps working: an exported C symbol
+ * carries no prototype, so its argument list must never change -- a new argument means a new name. */
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host);
 
 /* ---- sampling without device allocation ----------------------------------------------------------------------------
  * Forward sampling (Eq. 2 / Eq. 3; cutoff PAPER.md:116; coverage rule PAPER.md:126) of a SMALL model at a

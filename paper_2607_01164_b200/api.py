@@ -24,7 +24,7 @@ _STATUS = {0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_STATE", 3: "GS_ERR_OO
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_build_accel", "gs_sample_fwd", "gs_sample_bwd",
            "gs_step_host", "gs_debug_get", "gs_debug_read", "gs_debug_point_sets", "gs_debug_counters",
-           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_sample_fwd_loss",
+           "gs_profile_enable", "gs_profile_read", "gs_measure_alu_peaks", "gs_measure_alu_peaks2", "gs_sample_fwd_loss",
            "gs_params_activate", "gs_adam_step", "gs_prune", "gs_densify", "gs_set_sample_count", "gs_status_query", "gs_set_option", "gs_render", "gs_decode_grid",
            "gs_probe_points_static"]
 PROF_STAGES = ["preprocess", "build", "fwd", "bwd_pack", "bwd", "finalize", "cull"]
@@ -121,7 +121,8 @@ def load_library():
     lib.gs_prune.argtypes = [P, C.POINTER(_RawParams), P, P, P, C.c_float, C.POINTER(C.c_uint32)]
     lib.gs_densify.argtypes = [P, C.POINTER(_RawParams), P, P, C.c_uint32, C.POINTER(_Query), P, P, P, C.c_uint64, P, C.c_uint32,
                                C.c_float, C.c_float, C.POINTER(C.c_uint32)]
-    lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.gs_measure_alu_peaks.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.gs_measure_alu_peaks2.argtypes = [P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.gs_set_sample_count.argtypes = [P, C.c_uint64]
     lib.gs_set_option.argtypes = [P, C.c_int32, C.c_int64]
     lib.gs_render.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, C.c_uint32, P]
@@ -345,7 +346,7 @@ class Context:
         """(FP32 FMA lane-instructions per second, MUFU.EX2 per second, FMA lane-operations per second through the packed
         f32x2 form) of this device now; synchronises."""
         a, b, c = C.c_double(), C.c_double(), C.c_double()
-        self._check(self.lib.gs_measure_alu_peaks(self.h, C.byref(a), C.byref(b), C.byref(c)))
+        self._check(self.lib.gs_measure_alu_peaks2(self.h, C.byref(a), C.byref(b), C.byref(c)))
         return float(a.value), float(b.value), float(c.value)
 
     def gs_render(self, origins, dirs, t_range, spp: int, table, rgba):

@@ -852,7 +852,11 @@ gs_status gs_densify(gs_ctx *ctx, const gs_raw_params *p, float *m, float *v, ui
     return GS_OK;
 }
 
-gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host) {
+gs_status gs_measure_alu_peaks(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host) {
+    return gs_measure_alu_peaks2(ctx, ffma_per_s_host, ex2_per_s_host, nullptr);
+}
+
+gs_status gs_measure_alu_peaks2(gs_ctx *ctx, double *ffma_per_s_host, double *ex2_per_s_host, double *ffma2_per_s_host) {
     LaunchScope launch_scope(ctx);
     if (!ctx || !ffma_per_s_host || !ex2_per_s_host) return GS_ERR_INVALID_ARG;
     CK(cudaSetDevice(ctx->device), "cudaSetDevice");
@@ -910,6 +914,12 @@ gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs
         if (batch_bricks[k] < 1 || batch_bricks[k] > 256) return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: batch_bricks must lie in [1, 256]");
         if (region->dims[k] < 1 || region->brick_lo[k] < 0 || region->brick_cnt[k] < 1 || BRICK * (int64_t)region->brick_lo[k] >= region->dims[k])
             return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: empty or misplaced region");
+        // the same rules as gs_build_accel applies to every batch, checked ONCE here: a bad region fails before anything is enqueued
+        // instead of inside a worker thread after other batches have already written into phi / I
+        if (!(region->spacing[k] > 0.f) || !isfinite(region->spacing[k]) || !isfinite(region->origin[k]))
+            return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: spacing must be positive and finite, origin finite");
+        if ((int64_t)region->brick_lo[k] + region->brick_cnt[k] > ((int64_t)region->dims[k] + BRICK - 1) / BRICK)
+            return fail(ctx, GS_ERR_INVALID_ARG, "gs_decode_grid: brick_lo + brick_cnt reaches beyond the grid");
         nbatch[k] = ((uint64_t)region->brick_cnt[k] + batch_bricks[k] - 1) / batch_bricks[k];
         total_batches *= nbatch[k];
     }
@@ -932,10 +942,18 @@ gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs
     }
     if (!ctx->decode_event) CK(cudaEventCreateWithFlags(&ctx->decode_event, cudaEventDisableTiming), "event");
     CK(cudaEventRecord(ctx->decode_event, ctx->stream), "event");   // the model arrays may be produced on the caller's stream
-    auto worker_fail = [&](gs_ctx *w, gs_status st) { return fail(ctx, st, gs_last_error(w)); };
+    // every way out of this call, failures included, first waits for all worker streams: nothing of this call may still be reading
+    // the caller's model or writing the caller's phi / I once it has returned
+    auto worker_fail = [&](gs_ctx *w, gs_status st) {
+        const std::string msg = gs_last_error(w);
+        for (int k = 0; k < num_streams; k++) cudaStreamSynchronize(ctx->decode_streams[(size_t)k]);
+        cudaGetLastError();
+        return fail(ctx, st, msg.c_str());
+    };
     for (int k = 0; k < num_streams; k++) {
         gs_ctx *w = ctx->decode_workers[k];
-        CK(cudaStreamWaitEvent(ctx->decode_streams[k], ctx->decode_event, 0), "wait");
+        const cudaError_t we = cudaStreamWaitEvent(ctx->decode_streams[k], ctx->decode_event, 0);
+        if (we != cudaSuccess) { w->err = std::string("wait: ") + cudaGetErrorString(we); return worker_fail(w, GS_ERR_CUDA); }
         const gs_status st = gs_preprocess(w, g, nullptr, tau);
         if (st != GS_OK) return worker_fail(w, st);
     }
@@ -1000,7 +1018,8 @@ gs_status gs_decode_grid(gs_ctx *ctx, const gs_gaussians *g, float tau, const gs
             if (st == GS_OK) st = gs_set_option(w, GS_OPT_ASYNC_BUILD, 1);
             ckpt = n;
         }
-        if (st == GS_OK && cudaStreamSynchronize(ctx->decode_streams[(size_t)k]) != cudaSuccess) st = GS_ERR_CUDA;
+        const cudaError_t se = cudaStreamSynchronize(ctx->decode_streams[(size_t)k]);   // whatever the status: see worker_fail
+        if (st == GS_OK && se != cudaSuccess) { st = GS_ERR_CUDA; w->err = std::string("gs_decode_grid: ") + cudaGetErrorString(se); }
         wst[(size_t)k] = st;
     };
     {

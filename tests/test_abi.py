@@ -19,7 +19,7 @@ def lib():
 def _declared():
     text = open(os.path.join(ROOT, "include", "gs.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(gs_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(gs_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_exports_match_header(lib):
@@ -29,6 +29,42 @@ def test_exports_match_header(lib):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in gs.h but not exported"
     assert set(api.EXPORTS) == set(names)
+
+
+def _prototypes():
+    """{name: [C type of each parameter]} of every function include/gs.h declares."""
+    text = open(os.path.join(ROOT, "include", "gs.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    out = {}
+    for m in re.finditer(r"\b(gs_[a-z_0-9]+)\s*\(([^()]*)\)\s*;", text):
+        params = [p.strip() for p in m.group(2).split(",")]
+        out[m.group(1)] = [] if params == ["void"] else [re.sub(r"\s*\w+$", "", p).strip() if not p.endswith("*") else p for p in params]
+    return out
+
+
+def _kind(ctype):
+    """Coarse class of a C parameter type / a ctypes type: pointers are one class, scalars must match exactly."""
+    if isinstance(ctype, str):
+        if "*" in ctype:
+            return "ptr"
+        return {"int": "i32", "int32_t": "i32", "uint32_t": "u32", "int64_t": "i64", "uint64_t": "u64", "size_t": "u64", "float": "f32"}[ctype]   # LP64: size_t is 64 bits
+    if ctype in (ctypes.c_void_p, ctypes.c_char_p) or hasattr(ctype, "contents"):
+        return "ptr"
+    return {ctypes.c_int: "i32", ctypes.c_int32: "i32", ctypes.c_uint32: "u32", ctypes.c_int64: "i64", ctypes.c_uint64: "u64",
+            ctypes.c_size_t: "u64", ctypes.c_float: "f32"}[ctype]
+
+
+def test_binding_argtypes_match_header_prototypes(lib):
+    # an exported symbol carries no prototype: the binding (and any caller built against an older header) only stays in
+    # step with the library if every parameter list is checked against the header
+    protos = _prototypes()
+    assert set(protos) == set(_declared())
+    for name, params in protos.items():
+        argtypes = getattr(lib, name).argtypes
+        assert argtypes is not None, f"{name}: the binding declares no argtypes"
+        assert [_kind(a) for a in argtypes] == [_kind(p) for p in params], f"{name}: binding {argtypes} vs header {params}"
+    # the round-1 prototype of gs_measure_alu_peaks (three arguments) is frozen; the packed-FMA figure lives in ...peaks2
+    assert len(protos["gs_measure_alu_peaks"]) == 3 and len(protos["gs_measure_alu_peaks2"]) == 4
 
 
 def test_struct_layouts_match_header():

@@ -95,4 +95,13 @@ def test_decode_repeats_a_batch_that_outgrew_the_speculative_buffer(oracle):
     with pytest.raises(api.GsError) as e:
         ctx.gs_decode_grid(*dev, api.grid_query(full), (0, 4, 4), phi, I)
     assert e.value.status == api.GS_ERR_INVALID_ARG
+    # a region that reaches beyond the grid is refused before any batch runs (it used to fail inside a worker thread, after
+    # other batches had written their part of phi / I)
+    phi.fill_(-7.0)
+    over = inputs.Grid(full.dims, full.origin, full.spacing, (0, 0, 4), (8, 8, 5))
+    with pytest.raises(api.GsError) as e:
+        ctx.gs_decode_grid(*dev, api.grid_query(over), bb, phi, I, streams=2)
+    assert e.value.status == api.GS_ERR_INVALID_ARG and "beyond the grid" in str(e.value)
+    torch.cuda.synchronize()
+    assert float(phi.max().item()) == -7.0
     ctx.close()
