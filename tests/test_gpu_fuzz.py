@@ -46,18 +46,37 @@ def _check_loss(run, loss):
     assert abs(got - loss) <= 1e-6 * loss + (2e-5 * np.sqrt(loss) if run.P < 1000 else 0.0) + 1e-12, (got, loss, run.P)
 
 
-def _floors(gr, g):
-    # Tensors whose exact value vanishes by cancellation (no hit anywhere; an isolated Gaussian, where Phi = v wherever it is
-    # covered): the fp32 result is compared against the size of the terms that cancel -- |dL/dv| times what the chain rule
-    # multiplies it by (1 / sigma for the mean and the scales, the anisotropy for the rotation, 1 / w for the weight)
-    ref = max(float(np.linalg.norm(gr["dscalar"])), 1e-30)
-    inv_sigma = float(1.0 / g.scale.min())
-    mult = {"dmean": inv_sigma, "dscale": inv_sigma, "dquat": float((g.scale.max(axis=1) / g.scale.min(axis=1)).max()),
-            "dopacity": float(1.0 / g.opacity.min())}
-    return {k: ref * m for k, m in mult.items() if float(np.linalg.norm(gr[k])) < 1e-3 * ref * m}
+FLOORED = []   # (test, seed, tensor) of every comparison that used a cancellation floor instead of the plain 1e-4: printed below
 
 
-@pytest.mark.parametrize("seed", range(12))
+def _floors(gr, g, tag):
+    # A gradient tensor whose EXACT value vanishes by cancellation (an isolated Gaussian, where Phi = v wherever it is covered, so
+    # every term of dL/dmu, dL/ds, dL/dq, dL/dw cancels against its neighbour) cannot be held to a relative error: fp32 leaves the
+    # rounding of the terms that cancel.  Only then -- the oracle's tensor is below 1e-6 of the size of those terms, i.e. zero to
+    # fp32 -- is the result compared against that size instead of against the tensor's own norm; everything else is held to the
+    # plain 1e-4.  Size of the cancelling terms, per Gaussian that is hit at all: |dL/dv_i| times what the chain rule multiplies it
+    # by (1 / sigma_min,i for the mean and the scales, the Gaussian's own anisotropy for the rotation, 1 / w_i for the weight).
+    dv = np.abs(np.asarray(gr["dscalar"], np.float64).ravel())
+    hit = dv > 0
+    if not hit.any():
+        return {}
+    smin, smax = g.scale.min(axis=1).astype(np.float64), g.scale.max(axis=1).astype(np.float64)
+    mult = {"dmean": 1.0 / smin, "dscale": 1.0 / smin, "dquat": smax / smin, "dopacity": 1.0 / g.opacity.astype(np.float64)}
+    out = {}
+    for k, m in mult.items():
+        size = float(np.linalg.norm((dv * m)[hit]))
+        if float(np.linalg.norm(gr[k])) < 1e-6 * size:
+            out[k] = size
+            FLOORED.append((*tag, k))
+    return out
+
+
+# seeds beyond the first twelve: the ones that failed under the fixed 1e-5 / 2e-5 / 1e-6 / 1e-4 bounds when a wider range was
+# run by hand in round 2 (P = 1 losses, I at > 20:1 anisotropy, isolated Gaussians), kept as fixed cases
+SEEDS = list(range(12)) + [45, 53, 79, 111, 116, 132, 251]
+
+
+@pytest.mark.parametrize("seed", SEEDS)
 def test_random_grid_case(oracle, seed):
     import torch
     rng = np.random.default_rng(1000 + seed)
@@ -90,10 +109,10 @@ def test_random_grid_case(oracle, seed):
     check_sets(run, fwd)
     check_forward(run, fwd, tol_I=_tol_I(g))
     _check_loss(run, loss)
-    check_grads(run, gr, zero_floor=_floors(gr, g))
+    check_grads(run, gr, zero_floor=_floors(gr, g, ("grid", seed)))
 
 
-@pytest.mark.parametrize("seed", range(12))
+@pytest.mark.parametrize("seed", SEEDS)
 def test_random_points_case(oracle, seed):
     rng = np.random.default_rng(2000 + seed)
     P = int(rng.choice([1, 31, 32, 33, 1000, 20011, 70000]))
@@ -118,4 +137,10 @@ def test_random_points_case(oracle, seed):
     check_sets(run, fwd)
     check_forward(run, fwd, tol_I=_tol_I(g))
     _check_loss(run, loss)
-    check_grads(run, gr, zero_floor=_floors(gr, g))
+    check_grads(run, gr, zero_floor=_floors(gr, g, ("points", seed)))
+
+
+def test_zz_report_floored_comparisons():
+    # not a check of the kernels: says how many of the comparisons above used a cancellation floor (run with -s to see them)
+    print(f"\ncancellation floors used in {len(FLOORED)} tensor comparisons: {FLOORED}")
+    assert len(FLOORED) <= 2 * len(SEEDS), "floors are for the rare exact cancellation, not the rule"
