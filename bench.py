@@ -293,6 +293,8 @@ def measure(wl, args, sampler, world, rank, headline: bool):
     mode = points_mode(wl, args)
     if mode is not None:
         ctx.gs_set_option(api.OPT_POINTS_ACCEL, api.POINTS_SCATTER if mode == "scatter" else api.POINTS_GATHER)
+    if args.no_hit_masks:
+        ctx.gs_set_option(api.OPT_BWD_HIT_MASKS, 0)   # A/B: the point backward evaluates every cull-list entry (gs.h)
     if wl["kind"] == "grid" and not args.sync_build:
         ctx.gs_set_option(api.OPT_ASYNC_BUILD, 1)   # steady-state builds without a host round trip (gs.h)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -695,6 +697,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sync-build", action="store_true", help="grid queries: keep the host round trip in gs_build_accel (GS_OPT_ASYNC_BUILD = 0)")
+    ap.add_argument("--no-hit-masks", action="store_true", help="point queries: backward without the forward's hit masks (GS_OPT_BWD_HIT_MASKS = 0)")
     ap.add_argument("--points-accel", default="default", choices=["default", "gather", "scatter"],
                     help="point queries: gather = LBVH over the Gaussians (north_star); scatter = the paper's tree over the samples")
     ap.add_argument("--record-traffic", nargs=3, metavar=("NCU_RAW_CSV", "WORKLOAD", "SOURCE"),

@@ -184,8 +184,14 @@ gs_status gs_sample_fwd(gs_ctx *ctx, const gs_query *q, const float *target, flo
  *   nothing: call it again).  The counts are picked up without stalling the host, so the report can trail the batch by several builds:
  *   every batch built since the last call that WAITED for the counts (gs_status_query, gs_debug_get, a synchronous build) is
  *   suspect and should be repeated -- gs_decode_grid does exactly that.  Point queries always synchronise once.
+ * GS_OPT_BWD_HIT_MASKS (0 / 1, default 1; point queries in gather mode): gs_sample_fwd / gs_sample_fwd_loss leave one bit per
+ *   cull-list entry -- does the Gaussian hit any of the packet's 32 points -- and gs_sample_bwd on the same accel evaluates only
+ *   the entries whose bit is set, compacted across list chunks so that every lane holds a Gaussian that reaches the packet
+ *   (on configs[4] 44 % of the list entries hit nothing, on configs[2] 33 %).  Same per-entry arithmetic: the gradients differ
+ *   from the unmasked backward's by the order of the atomic additions only.  0 = evaluate every entry (the A/B baseline);
+ *   a gs_sample_bwd without a preceding forward on the accel falls back to that by itself.
  * Errors: INVALID_ARG (unknown key / value). */
-typedef enum { GS_OPT_POINTS_ACCEL = 0, GS_OPT_ASYNC_BUILD = 1 } gs_option;
+typedef enum { GS_OPT_POINTS_ACCEL = 0, GS_OPT_ASYNC_BUILD = 1, GS_OPT_BWD_HIT_MASKS = 2 } gs_option;
 typedef enum { GS_POINTS_GATHER = 0, GS_POINTS_SCATTER = 1 } gs_points_accel;
 gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value);
 

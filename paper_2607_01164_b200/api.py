@@ -80,7 +80,7 @@ class _AdamCfg(C.Structure):
 
 
 LOSS_MSE, LOSS_L1 = 0, 1
-OPT_POINTS_ACCEL, OPT_ASYNC_BUILD = 0, 1
+OPT_POINTS_ACCEL, OPT_ASYNC_BUILD, OPT_BWD_HIT_MASKS = 0, 1, 2
 POINTS_GATHER, POINTS_SCATTER = 0, 1
 PAPER_LR = (0.00016, 0.001, 0.0001, 0.025, 0.0025)  # mean, scale, quat, opacity (weights), scalar (values): PAPER.md:231
 

@@ -114,7 +114,7 @@ gs_status validate_query(gs_ctx *ctx, const gs_query *q, GridDesc *gd, uint64_t 
 
 CullLists cull_lists(gs_ctx *ctx) {
     return CullLists{ctx->cull_ids.as<uint32_t>(), ctx->cull_link.as<uint32_t>(), ctx->cull_head.as<uint2>(),
-                     ctx->counters.as<uint32_t>() + 2, ctx->cull_cap};
+                     ctx->counters.as<uint32_t>() + 2, ctx->cull_cap, nullptr};
 }
 
 // GS_OPT_ASYNC_BUILD: pick up the pair count T and the touched count M of the last grid build once they have arrived in
@@ -256,7 +256,7 @@ void gs_destroy(gs_ctx *ctx) {
     DevBuf *all[] = {&ctx->rec, &ctx->aabb, &ctx->params, &ctx->bcount, &ctx->bhist, &ctx->pair_gauss, &ctx->pair_brick,
                      &ctx->grid_order, &ctx->brick_start, &ctx->jit, &ctx->bwd_setup, &ctx->leaf_key[0], &ctx->leaf_key[1],
                      &ctx->leaf_val[0], &ctx->leaf_val[1], &ctx->node_left, &ctx->node_right, &ctx->node_parent,
-                     &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->pt_key[0], &ctx->pt_key[1],
+                     &ctx->leaf_parent, &ctx->node_aabb, &ctx->node_flag, &ctx->bvh_nodes, &ctx->sorted_rec, &ctx->cull_ids, &ctx->cull_link, &ctx->cull_head, &ctx->cull_mask, &ctx->pt_key[0], &ctx->pt_key[1],
                      &ctx->pt_val[0], &ctx->pt_val[1], &ctx->scan_tmp, &ctx->sort_hist, &ctx->gacc, &ctx->misc, &ctx->counters, &ctx->dbg, &ctx->dens_work, &ctx->dens_scratch, &ctx->sel_key[0], &ctx->sel_key[1],
                      &ctx->sel_val[0], &ctx->sel_val[1], &ctx->sc_spt, &ctx->sc_box, &ctx->sc_acc, &ctx->sc_coef, &ctx->rn_xyz, &ctx->rn_phi, &ctx->rn_I, &ctx->cidx_hist, &ctx->cidx_start, &ctx->cidx_ids};
     for (DevBuf *b : all) b->release();
@@ -287,6 +287,7 @@ gs_status gs_preprocess(gs_ctx *ctx, const gs_gaussians *g, const gs_domain *dom
     ctx->have_pre = false;
     ctx->lbvh_state = 0;
     ctx->accel_kind = -1;
+    ctx->have_hit_masks = false;
     ctx->fused_pack = 0;
     ctx->cidx_valid = false;
     ctx->builds_since_pre = 0;
@@ -324,6 +325,7 @@ gs_status gs_build_accel(gs_ctx *ctx, const gs_query *q) {
     if ((st = resolve_grid_counts(ctx, /*wait=*/false)) != GS_OK) return st;
     ctx->accel_kind = -1;
     ctx->fused_pack = 0;
+    ctx->have_hit_masks = false;
     cudaStream_t s = ctx->stream;
     const uint32_t N = ctx->N;
     Stage stage(ctx, GS_PROF_BUILD);
@@ -546,10 +548,18 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
                               ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, ctx->tau, ctx->r2, o, s),
            "points forward (scatter)");
     } else {
+        // the forward leaves one hit bit per list entry for gs_sample_bwd (k_points_bwd_masked); the debug-set variant does not
+        CullLists lists = cull_lists(ctx);
+        const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
+        if (ctx->opt_bwd_hit_masks && !sets && ctx->P > 0) {
+            CK(ctx->cull_mask.reserve(((size_t)ctx->cull_cap + 1) * 4), "alloc hit masks");
+            lists.mask = ctx->cull_mask.as<uint32_t>();
+        }
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, lists, ctx->tau,
                              ctx->r2, o, s), "points forward");
+        if (lists.mask) ctx->have_hit_masks = true;
     }
     return GS_OK;
 }
@@ -665,9 +675,12 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
     } else {
         CK(cudaMemsetAsync(ctx->gacc.p, 0, (size_t)N * GACC * 4, s), "memset gacc");
         Stage stage(ctx, GS_PROF_BWD);
+        CullLists lists = cull_lists(ctx);
+        const bool masked = ctx->have_hit_masks && ctx->opt_bwd_hit_masks;   // a forward on these lists left its hit bits
+        if (masked) lists.mask = ctx->cull_mask.as<uint32_t>();
         CK(launch_points_bwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
-                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, cull_lists(ctx), ctx->tau,
-                             ctx->r2, in, ctx->gacc.as<float>(), s), "points backward");
+                             ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, lists, ctx->tau,
+                             ctx->r2, in, ctx->gacc.as<float>(), masked, s), "points backward");
     }
     Stage stage(ctx, GS_PROF_FINALIZE);
     const bool grid = ctx->accel_kind == GS_QUERY_GRID;
@@ -1050,6 +1063,11 @@ gs_status gs_set_option(gs_ctx *ctx, int32_t key, int64_t value) {
             if (!value) { gs_status rs__ = resolve_grid_counts(ctx); if (rs__ != GS_OK) return rs__; }
             ctx->opt_async_build = (int)value;
             ctx->grid_warm_N = 0xffffffffu;
+            return GS_OK;
+        case GS_OPT_BWD_HIT_MASKS:
+            if (value != 0 && value != 1) return fail(ctx, GS_ERR_INVALID_ARG, "GS_OPT_BWD_HIT_MASKS: 0 or 1");
+            ctx->opt_bwd_hit_masks = (int)value;
+            ctx->have_hit_masks = false;
             return GS_OK;
         default: return fail(ctx, GS_ERR_INVALID_ARG, "unknown option");
     }

@@ -159,6 +159,9 @@ struct gs_ctx {
     gs::DevBuf bvh_nodes;  // packed traversal nodes
     gs::DevBuf sorted_rec; // float4 [N][4]: records in leaf order (id in plane c's .w)
     gs::DevBuf cull_ids, cull_link, cull_head;  // per-packet survivor lists (see CullLists)
+    gs::DevBuf cull_mask;      // uint32 [cull_cap]: per-chunk hit bits of the last forward on the current lists
+    bool have_hit_masks = false;   // cull_mask is valid for the current point accel (a gather-mode forward ran since its build)
+    int opt_bwd_hit_masks = 1;     // gs_set_option(GS_OPT_BWD_HIT_MASKS)
     uint32_t cull_cap = 0;   // chunks the pool holds
     double cull_per_packet = 0.0;   // list entries per packet of the last build (picks the cull kernel's group size)
     gs::DevBuf pt_key[2], pt_val[2];
@@ -310,6 +313,8 @@ struct CullLists {
     uint2 *head;      // [packets] (first chunk, entries in it)
     uint32_t *top;    // chunks requested so far (may exceed cap: the host then grows the pool and repeats)
     uint32_t cap;
+    uint32_t *mask;   // [cap] nullable: bit j of mask[c] = entry j of chunk c hits at least one point of its packet.  Written by
+                      // k_points_fwd (which evaluates every (entry, point) predicate anyway), read by k_points_bwd_masked
 };
 cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order,
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group /*2 or 4 packets per warp*/,
@@ -327,7 +332,9 @@ cudaError_t launch_scatter_fwd(const float4 *rec, const float *aabb, const uint3
 cudaError_t launch_scatter_bwd(const float4 *rec, const float *aabb, const uint32_t *gorder, uint32_t N, const PtTree &T, const float4 *spt,
                                float4 *coef, const uint32_t *pt_order, uint64_t P, float tau, float r2, const BwdIn &in, float *gacc,
                                cudaStream_t s);
+// use_masks: lists.mask holds the hit bits of a forward on these lists (k_points_bwd_masked: entries without a hit are dropped and
+// the surviving ones compacted across chunks before their records are gathered); false: every entry is evaluated (k_points_bwd)
 cudaError_t launch_points_bwd(const float4 *sorted_rec, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
-                              float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s);
+                              float tau, float r2, const BwdIn &in, float *gacc, bool use_masks, cudaStream_t s);
 
 }  // namespace gs

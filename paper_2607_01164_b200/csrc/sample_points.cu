@@ -374,7 +374,7 @@ __global__ void __launch_bounds__(CULL_WARPS * 32, GS_CULL_MINB) k_points_cull(c
 // broadcast to both halves).  One warp-iteration therefore tests 2 Gaussians x 32 points in ~28 issue slots
 // (15 packed instructions for the canonical sequence) where the scalar form needed 27 slots per Gaussian.
 // ---------------------------------------------------------------------------------------------------------
-template <bool SETS>
+template <bool SETS, bool MASKS>
 __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
                                                                  const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                  float r2, FwdOut o, double invP) {
@@ -409,6 +409,9 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
         if (c1 != NO_CHUNK) gather64<false>(srt, pos1, 32, buf[b ^ 1], lane);
         if (c2 != NO_CHUNK) { pos2 = __ldg(L.ids + (size_t)c2 * 32 + lane); c3 = __ldg(L.link + c2); }
         const float4 *rb = buf[b];
+        // bit j: entry j of this chunk hits one of THIS LANE's two points (the halves hold the even / odd entries); one OR-reduction
+        // over the warp per chunk then gives the chunk's mask (a vote per entry cost the forward 50 %: measured)
+        uint32_t emask = 0, ebit = 1u << half;
 #pragma unroll 4
         for (int j = half; j < n0; j += 2) {
             const float4 ga = rb[4 * j], gb = rb[4 * j + 1], gc = rb[4 * j + 2], gd = rb[4 * j + 3];
@@ -416,6 +419,10 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
             const f2 qd = mahalanobis2(ga.x, ga.y, ga.z, gb.x, gb.y, gb.z, gc.x, gc.y, gc.z, gd.x, gd.y, gd.z, px, py, pz, u0, u1, u2);
             bool h0, h1;
             const f2 G = gauss_weight2(qd, r2, h0, h1);
+            if (MASKS) {
+                if (h0 | h1) emask |= ebit;
+                ebit <<= 2;
+            }
             I2 = fma2(bc(ga.w), G, I2);
             N2 = fma2(bc(gd.w), G, N2);   // d.w = v w
             if (SETS) {
@@ -426,6 +433,10 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
         }
         if (SETS) tested += (uint32_t)n0;
         __syncwarp();
+        if (MASKS) {   // the backward drops the entries that hit nothing (44 % of configs[4]'s, 33 % of configs[2]'s) before it gathers their records
+            emask = __reduce_or_sync(0xffffffffu, emask);
+            if (lane == 0) L.mask[c0] = emask;
+        }
         c0 = c1; n0 = 32; c1 = c2; pos1 = pos2; c2 = c3; b ^= 1;
     }
     // the two halves hold the sums over the even / odd entries: add them, then hand point `lane` its own result
@@ -608,6 +619,127 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// k_points_bwd_masked: the same sums as k_points_bwd over the entries that HIT.  The forward left one bit per list entry
+// (CullLists::mask); here a warp walks its packet's chain, keeps the ids whose bit is set in a 64-slot ring, and as soon as 32
+// have come together gathers their records and evaluates them, lane = Gaussian -- so every lane holds a Gaussian that reaches
+// the packet, whatever chunk it came from, and the records of the others are never read.  One batch's gather is in flight
+// while the previous batch is evaluated.  Per entry the arithmetic and its order are those of k_points_bwd.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd_masked(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
+                                                                        const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
+                                                                        float r2, BwdIn in, float *__restrict__ gacc) {
+    __shared__ __align__(16) float pts_all[EVAL_WARPS][16][12];   // as in k_points_bwd
+    __shared__ float4 buf_all[EVAL_WARPS][2][128];
+    __shared__ uint32_t ring_all[EVAL_WARPS][64];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint64_t packet = (uint64_t)blockIdx.x * EVAL_WARPS + warp;
+    if (packet * 32 >= P) return;
+    float (*pts)[12] = pts_all[warp];
+    float4 (*buf)[128] = buf_all[warp];
+    uint32_t *ring = ring_all[warp];
+    {
+        const PacketPoint pp = load_point(xyz, pt_order, P, packet, lane);
+        const bool active = pp.active;
+        const uint64_t c = pp.c;
+        float alpha = 0.f, beta = 0.f, eps = 0.f;
+        if (active && in.pack2) {
+            const float2 s = __ldg(in.pack2 + packet * 32 + lane);
+            alpha = s.x; beta = s.y; eps = fabsf(s.x) * in.eps_scale;
+        } else if (active) {
+            const float Ic = in.I[c], ph = in.phi[c];
+            const bool covered = Ic > tau;
+            const float inv = covered ? 1.0f / Ic : 0.f;
+            alpha = covered ? in.dL_dphi[c] * inv : 0.f;
+            beta = (in.dL_dI ? in.dL_dI[c] : 0.f) - alpha * ph;
+            eps = (covered && in.target) ? fabsf(ph - in.target[c]) * inv : 0.f;
+        }
+        float x = pp.px, y = pp.py, z = pp.pz;
+        if (!(fabsf(x) <= 3.402823466e38f && fabsf(y) <= 3.402823466e38f && fabsf(z) <= 3.402823466e38f)) {   // see k_points_bwd
+            x = y = z = 0.f;
+            alpha = beta = eps = 0.f;
+        }
+        float *row = pts[lane >> 1] + (lane & 1);
+        row[0] = x; row[2] = y; row[4] = z; row[6] = alpha; row[8] = beta; row[10] = eps;
+        __syncwarp();
+    }
+    const uint2 head = __ldg(L.head + packet);
+    uint32_t c = head.x, id = 0u, m = 0u, nxt = NO_CHUNK;
+    if (c != NO_CHUNK) {   // the head chunk holds head.y entries, every linked chunk 32
+        const int n = (int)head.y;
+        id = lane < n ? __ldg(L.ids + (size_t)c * 32 + lane) : 0u;
+        m = __ldg(L.mask + c) & (n < 32 ? (1u << n) - 1u : 0xffffffffu);
+        nxt = __ldg(L.link + c);
+    }
+    uint32_t cnt = 0, done = 0;   // ids appended to the ring / ids handed to a gather so far
+    int pend = 0, slot = 0;        // entries of the batch whose records are on their way into buf[slot]
+    while (true) {
+        while (c != NO_CHUNK && cnt - done < 32u) {
+            uint32_t id2 = 0u, m2 = 0u, nxt2 = NO_CHUNK;
+            if (nxt != NO_CHUNK) { id2 = __ldg(L.ids + (size_t)nxt * 32 + lane); m2 = __ldg(L.mask + nxt); nxt2 = __ldg(L.link + nxt); }
+            if ((m >> lane) & 1u) ring[(cnt + __popc(m & ((1u << lane) - 1u))) & 63u] = id;
+            cnt += __popc(m);
+            c = nxt; id = id2; m = m2; nxt = nxt2;
+        }
+        __syncwarp();
+        const int nb = (int)(cnt - done < 32u ? cnt - done : 32u);
+        if (pend) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncwarp();
+        }
+        if (nb) {
+            const uint32_t pos = lane < nb ? ring[(done + lane) & 63u] : 0u;
+            gather64<true>(srt, pos, nb, buf[slot ^ 1], lane);
+            done += (uint32_t)nb;
+        }
+        if (lane < pend) {
+            const float4 *rb = buf[slot] + 4 * lane;
+            const int f = (lane >> 1) & 3;
+            Rec g;
+            g.a = rb[f]; g.b = rb[1 ^ f]; g.c = rb[2 ^ f]; g.d = rb[3 ^ f];
+            f2 acc[12];
+#pragma unroll
+            for (int q = 0; q < 12; q++) acc[q] = pk(0.f, 0.f);
+            bool any = false;
+            const f2 w2 = bc(g.a.w), v2 = bc(g.b.w);
+#pragma unroll 4
+            for (int i = 0; i < 16; i++) {
+                const ulonglong2 A = *reinterpret_cast<const ulonglong2 *>(pts[i]), B = *reinterpret_cast<const ulonglong2 *>(pts[i] + 4),
+                                 C = *reinterpret_cast<const ulonglong2 *>(pts[i] + 8);
+                f2 u0, u1, u2;
+                const f2 qd = mahalanobis2(g.a.x, g.a.y, g.a.z, g.b.x, g.b.y, g.b.z, g.c.x, g.c.y, g.c.z, g.d.x, g.d.y, g.d.z, A.x, A.y, B.x, u0, u1, u2);
+                bool h0, h1;
+                const f2 G = gauss_weight2(qd, r2, h0, h1);
+                any |= h0 | h1;
+                const f2 alpha = B.y, beta = C.x, eps = C.y;
+                const f2 wG = mul2(w2, G);
+                const f2 gamma = fma2(alpha, v2, beta);
+                const f2 t = mul2(gamma, wG);
+                acc[0] = fma2(alpha, wG, acc[0]);
+                acc[1] = fma2(gamma, G, acc[1]);
+                const f2 t0 = mul2(t, u0), t1 = mul2(t, u1), t2 = mul2(t, u2);
+                acc[2] = add2(acc[2], t0); acc[3] = add2(acc[3], t1); acc[4] = add2(acc[4], t2);
+                acc[5] = fma2(t0, u0, acc[5]); acc[6] = fma2(t0, u1, acc[6]); acc[7] = fma2(t0, u2, acc[7]);
+                acc[8] = fma2(t1, u1, acc[8]); acc[9] = fma2(t1, u2, acc[9]); acc[10] = fma2(t2, u2, acc[10]);
+                acc[11] = fma2(eps, wG, acc[11]);
+            }
+            if (any) {
+                float s[12];
+#pragma unroll
+                for (int q = 0; q < 12; q++) s[q] = lo(acc[q]) + hi(acc[q]);
+                float *row = gacc + (size_t)__float_as_uint(g.c.w) * GACC;
+                red_add_v4(row, s[0], s[1], s[2], s[3]);
+                red_add_v4(row + 4, s[4], s[5], s[6], s[7]);
+                red_add_v4(row + 8, s[8], s[9], s[10], s[11]);
+            }
+        }
+        __syncwarp();
+        if (!nb) break;
+        pend = nb;
+        slot ^= 1;
+    }
+}
+
 cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float4 *xyz, const uint32_t *pt_order,
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group,
                                cudaStream_t s) {
@@ -628,18 +760,21 @@ cudaError_t launch_points_fwd(const float4 *sorted_rec, const float4 *xyz, const
     const uint64_t packets = (P + 31) / 32;
     const unsigned blocks = (unsigned)((packets + EVAL_WARPS - 1) / EVAL_WARPS);
     const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
-    if (sets) k_points_fwd<true><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, o.inv_count > 0.0 ? o.inv_count : 1.0 / (double)P);
-    else k_points_fwd<false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, o.inv_count > 0.0 ? o.inv_count : 1.0 / (double)P);
+    const double invP = o.inv_count > 0.0 ? o.inv_count : 1.0 / (double)P;
+    if (sets) k_points_fwd<true, false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, invP);
+    else if (lists.mask) k_points_fwd<false, true><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, invP);
+    else k_points_fwd<false, false><<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, o, invP);
     count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_points_bwd(const float4 *sorted_rec, const float4 *xyz, const uint32_t *pt_order, uint64_t P, const CullLists &lists,
-                              float tau, float r2, const BwdIn &in, float *gacc, cudaStream_t s) {
+                              float tau, float r2, const BwdIn &in, float *gacc, bool use_masks, cudaStream_t s) {
     if (P == 0) return cudaSuccess;
     const uint64_t packets = (P + 31) / 32;
     const unsigned blocks = (unsigned)((packets + EVAL_WARPS - 1) / EVAL_WARPS);
-    k_points_bwd<<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, in, gacc);
+    if (use_masks && lists.mask) k_points_bwd_masked<<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, in, gacc);
+    else k_points_bwd<<<blocks, EVAL_WARPS * 32, 0, s>>>(sorted_rec, xyz, pt_order, P, lists, tau, r2, in, gacc);
     count_launch();
     return cudaGetLastError();
 }
