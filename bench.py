@@ -41,13 +41,22 @@ TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 MIN_TIMED_S = 0.3   # secondary workloads repeat their step until the timed region is at least this long
 
 
+def _code_only(text: str) -> str:
+    """C / CUDA source without comments and blank lines: what the compiler sees."""
+    import re
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    text = re.sub(r"//[^\n]*", "", text)
+    return "\n".join(ln.rstrip() for ln in text.splitlines() if ln.strip())
+
+
 def csrc_sha16() -> str:
-    """Identity of the kernels this run executes: sha256 over csrc/* and include/gs.h (the GPU box has no .git)."""
+    """Identity of the kernels this run executes: sha256 over the CODE (comments stripped) of csrc/* and include/gs.h, so
+    that a stale ncu capture in profiles/traffic.json reads null and a comment edit does not (the GPU box has no .git)."""
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2607_01164_b200", "csrc")
     for f in sorted(os.listdir(d)) + ["../../include/gs.h"]:
-        with open(os.path.join(d, f), "rb") as fh:
-            h.update(f.encode() + b"\0" + fh.read())
+        with open(os.path.join(d, f), "r", encoding="utf-8", errors="replace") as fh:
+            h.update(f.encode() + b"\0" + _code_only(fh.read()).encode())
     return h.hexdigest()[:16]
 
 
@@ -130,15 +139,15 @@ def make_workload(name: str):
                     desc="C4 structured 1024^3 turbulence field, 4194304 Gaussians (5% 20:1 needles), one 128^3 brick-aligned batch "
                          "per step (BASELINE.json configs[3])")
     if name == "c5":
-        xyz_all, t_all = inputs.c5_points(seed=5, p=40_000_000)
+        xyz_all, t_all = inputs.c5_points(seed=5)   # the whole 200,000,000-point set (2.4 GB of positions; drawn by a thread pool)
         g = inputs.c5_gaussians(xyz_all, t_all)
         batches = []
         for b in range(2):
             idx = inputs.batch_indices(5, b, len(xyz_all), 1 << 24)
             batches.append((np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])))
         return dict(name=name, kind="points", g=g, batches=batches, domain=inputs.points_domain(xyz_all), decode_xyz=xyz_all,
-                    desc="C5 unstructured shell-and-fragments, 2^24-point batches (2 distinct, alternating) of a 40M-point draw of the "
-                         "200M-point set, 8388608 Gaussians, LBVH rebuilt per step (BASELINE.json configs[4])")
+                    desc="C5 unstructured shell-and-fragments, 2^24-point batches (2 distinct, alternating) drawn without replacement from the "
+                         "200,000,000-point set, 8388608 Gaussians centred on points of that set, LBVH rebuilt per step (BASELINE.json configs[4])")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -375,29 +384,69 @@ def measure(wl, args, sampler, world, rank, headline: bool):
            "hit_pairs": hits, "tested_pairs": tested, "cull_efficiency": hits / tested if tested else None}
     per = {k: (stage_ms[k] / stage_calls[k] if stage_calls[k] else 0.0) for k in stage_ms}
     out["stage_ms"] = per
-    # ---- roofline of the sampling kernels (this rank's share of the hits; ALU-bound)
+    # ---- roofline of the sampling kernels (this rank's share of the work): per kernel (a) the algorithmic FP32-pipe
+    #      lane-instructions of its HIT pairs at the ALU issue peak and (b) its compulsory bytes at the measured HBM copy bandwidth;
+    #      the larger of the two times is the bound, frac = that time / the measured launch time
     traffic, tsrc = load_traffic()
-    kpre = "k_grid_" if wl["kind"] == "grid" else "k_points_"
+    pts = wl["kind"] == "points"
+    kpre = "k_points_" if pts else "k_grid_"
+    hbm_gbs = _peaks().get("hbm_gbs") or 6547.0
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs" if _peaks().get("hbm_gbs") else "fallback 6547 GB/s (B200_PROFILING.md)"
+    alu_peak = ALU_PEAK_TINSTR   # replaced by the FFMA rate measured in this run for the headline (see below)
+    # Gaussians whose record a launch must read: the whole model for a point batch, the Gaussians that overlap the batch for a grid one
+    Ng = g.n if pts else int(ctx.gs_status_query().get("grid_touched", g.n))
+    # compulsory bytes per launch, term by term
+    recipe = {
+        "fwd": {"per_point": (4 + 8) + ((12 + 4) if pts else 0), "per_gaussian": 64,
+                "terms": "per point: 4 B target + 8 B (Phi, I) written" + (" + 12 B xyz + 4 B order" if pts else "") + "; per Gaussian: 64 B record"
+                         + ("" if pts else "; + 4 B per (brick, Gaussian) list entry")},
+        "bwd": {"per_point": 16 + ((12 + 4) if pts else 0), "per_gaussian": 64 + 2 * 48,
+                "terms": "per point: 16 B (Phi, I, dL/dPhi, dL/dI or the packed coefficients)" + (" + 12 B xyz + 4 B order" if pts else "")
+                         + "; per Gaussian: 64 B record + 48 B accumulator row read and written"
+                         + ("" if pts else "; + 4 B per (brick, Gaussian) list entry")},
+        "cull": {"per_point": 16, "per_gaussian": 128,
+                 "terms": "per point: 16 B of the sorted copy; per Gaussian: 64 B traversal node + 64 B record (the lists themselves are scratch, not compulsory)"},
+    }
+    list_bytes = 0 if pts else 4 * int(ctx.gs_status_query().get("grid_pairs", 0))
     kernels = {}
-    for nm, instr in (("fwd", INSTR_FWD), ("bwd", INSTR_BWD)):
+    names = (("fwd", INSTR_FWD), ("bwd", INSTR_BWD)) + ((("cull", None),) if pts and per.get("cull", 0.0) > 0 else ())
+    for nm, instr in names:
         ms = per[nm]
-        ach = hits * instr / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
-        tr = traffic.get(f"{wl['name']}/{kpre}{nm}")
-        # the same figure over the pairs the kernel actually EVALUATES (SURVEY 8d's "issue" fraction, counted for the point
-        # kernels, whose forward and backward walk the same lists): how busy the arithmetic pipes are; frac / issue_frac = cull efficiency
-        issue = tested * instr / (ms * 1e-3) / 1e12 / ALU_PEAK_TINSTR if (ms > 0 and wl["kind"] == "points") else None
-        kernels[nm] = {"kernel": kpre + nm, "launch_ms": ms, "achieved": ach, "frac": ach / ALU_PEAK_TINSTR, "issue_frac": issue,
-                       "algorithmic_lane_instr": hits * instr, "traffic": tr["bytes"] if tr else None,
-                       "traffic_source": tr["source"] if tr else tsrc}
+        rb = recipe[nm]
+        nbytes = P * rb["per_point"] + Ng * rb["per_gaussian"] + (list_bytes if nm != "cull" else 0)
+        alu_ms = hits * instr / (alu_peak * 1e12) * 1e3 if instr else None
+        hbm_ms = nbytes / (hbm_gbs * 1e9) * 1e3
+        bound = "alu" if (alu_ms is not None and alu_ms >= hbm_ms) else "hbm"
+        bound_ms = alu_ms if bound == "alu" else hbm_ms
+        ach = hits * instr / (ms * 1e-3) / 1e12 if (ms > 0 and instr) else None
+        kname = kpre + nm + ("_masked" if (pts and nm == "bwd" and not args.no_hit_masks and mode != "scatter") else "")
+        tr = traffic.get(f"{wl['name']}/{kname}")
+        # the ALU figure over the pairs the kernel actually EVALUATES (how busy the pipes are; frac_alu / issue_frac = cull efficiency)
+        # (not for a backward that drops the entries without a hit, GS_OPT_BWD_HIT_MASKS: it evaluates fewer pairs than `tested`)
+        issue = tested * instr / (ms * 1e-3) / 1e12 / alu_peak if (ms > 0 and pts and instr and (nm == "fwd" or args.no_hit_masks)) else None
+        kernels[nm] = {"kernel": kname, "launch_ms": ms, "alu_ms": alu_ms, "hbm_ms": hbm_ms, "bound": bound,
+                       "frac": bound_ms / ms if ms > 0 else None, "frac_alu": (alu_ms / ms if (ms > 0 and alu_ms is not None) else None),
+                       "frac_hbm": hbm_ms / ms if ms > 0 else None, "achieved": ach, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9 if ms > 0 else None,
+                       "issue_frac": issue, "algorithmic_lane_instr": hits * instr if instr else None, "algorithmic_bytes": nbytes,
+                       "bytes_recipe": rb["terms"], "traffic": tr["bytes"] if tr else None, "traffic_source": tr["source"] if tr else tsrc}
     dom = "fwd" if per["fwd"] >= per["bwd"] else "bwd"
+    kd = kernels[dom]
     fb_ms = per["fwd"] + per["bwd_pack"] + per["bwd"]
+    samp_ms = fb_ms + (per.get("cull", 0.0) if pts else 0.0)
+    both_alu_ms = hits * (INSTR_FWD + INSTR_BWD) / (alu_peak * 1e12) * 1e3
+    both_hbm_ms = kernels["fwd"]["hbm_ms"] + kernels["bwd"]["hbm_ms"]
+    both_ms = max(both_alu_ms, both_hbm_ms)
     out["roofline"] = {
-        "bound": "alu", "kernel": kernels[dom]["kernel"], "achieved": kernels[dom]["achieved"], "peak": ALU_PEAK_TINSTR,
-        "unit": "T FP32 lane-instr/s (algorithmic: hit pairs x 19 fwd / x 40 bwd)", "frac": kernels[dom]["frac"],
-        "traffic": kernels[dom]["traffic"], "traffic_unit": "bytes per launch (dram read + write, ncu --set full)",
-        "traffic_source": kernels[dom]["traffic_source"], "launch_ms": kernels[dom]["launch_ms"], "kernels": kernels,
-        "fwd_bwd_frac": (hits * (INSTR_FWD + INSTR_BWD) / (fb_ms * 1e-3) / 1e12 / ALU_PEAK_TINSTR) if fb_ms > 0 else None,
-        "step_frac": hits * (INSTR_FWD + INSTR_BWD) / (ms_step * 1e-3) / 1e12 / ALU_PEAK_TINSTR,
+        "bound": kd["bound"], "kernel": kd["kernel"],
+        "achieved": kd["achieved"] if kd["bound"] == "alu" else kd["achieved_gbs"],
+        "peak": alu_peak if kd["bound"] == "alu" else hbm_gbs,
+        "unit": "T FP32 lane-instr/s (algorithmic: hit pairs x 19 fwd / x 40 bwd)" if kd["bound"] == "alu" else "GB/s",
+        "frac": kd["frac"], "traffic": kd["traffic"], "traffic_unit": "bytes per launch (dram read + write, ncu --set full)",
+        "traffic_source": kd["traffic_source"], "launch_ms": kd["launch_ms"], "kernels": kernels,
+        "fwd_bwd_frac": both_ms / fb_ms if fb_ms > 0 else None,
+        "sampling_frac": both_ms / samp_ms if samp_ms > 0 else None,   # cull + fwd + bwd: the traversal is half of S5
+        "step_frac": both_ms / ms_step,
+        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src, "alu_peak_nominal": ALU_PEAK_TINSTR,
         "peak_source": "148 SM x 128 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max SM clock)"}
     out["rates"] = {"fwd_points_per_s": P / (per["fwd"] * 1e-3) if per["fwd"] else None,
                     "fwd_gaussian_evals_per_s": hits / (per["fwd"] * 1e-3) if per["fwd"] else None,
@@ -493,6 +542,58 @@ def measure(wl, args, sampler, world, rank, headline: bool):
     if world == 1 and wl.get("decode_xyz") is not None:
         allx = wl["decode_xyz"]
         chunk = 1 << 24
+        # end to end first (it needs two chunk buffers only): the set stays in HOST memory, chunk k+1 is copied in on a copy
+        # stream while chunk k is built and sampled, Phi / I of every chunk go back to the host
+        e2e_decode = None
+        if len(allx) > chunk:
+            nck = (len(allx) + chunk - 1) // chunk
+            cs = torch.cuda.Stream()
+            xb = [torch.empty((chunk, 3), device="cuda") for _ in range(2)]
+            pb = [torch.empty(chunk, device="cuda") for _ in range(2)]
+            ib = [torch.empty(chunk, device="cuda") for _ in range(2)]
+            hx = torch.from_numpy(allx)   # pageable host memory is pinned chunk by chunk (cudaHostRegister on 2.4 GB takes seconds)
+            hx_pin = [torch.empty((chunk, 3), pin_memory=True) for _ in range(2)]
+            hphi = torch.empty(len(allx), pin_memory=True)
+            hI = torch.empty(len(allx), pin_memory=True)
+            ready = [torch.cuda.Event() for _ in range(2)]
+            freed = [torch.cuda.Event() for _ in range(2)]
+            main = torch.cuda.current_stream()
+
+            def stage(k):
+                a = k * chunk
+                n_ = min(chunk, len(allx) - a)
+                hx_pin[k % 2][:n_].copy_(hx[a:a + n_])          # host memcpy into the pinned staging buffer
+                with torch.cuda.stream(cs):
+                    cs.wait_event(freed[k % 2])
+                    xb[k % 2][:n_].copy_(hx_pin[k % 2][:n_], non_blocking=True)
+                    ready[k % 2].record(cs)
+                return n_
+
+            def decode_e2e():
+                ctx.gs_preprocess(*gd, domain=wl["domain"], tau=TAU)
+                for e in freed:
+                    e.record(main)
+                n_next = stage(0)
+                for k in range(nck):
+                    n_ = n_next
+                    main.wait_event(ready[k % 2])
+                    q_ = api.points_query(xb[k % 2][:n_])
+                    ctx.gs_build_accel(q_)
+                    ctx.gs_sample_fwd(q_, pb[k % 2][:n_], ib[k % 2][:n_])
+                    a = k * chunk
+                    hphi[a:a + n_].copy_(pb[k % 2][:n_], non_blocking=True)
+                    hI[a:a + n_].copy_(ib[k % 2][:n_], non_blocking=True)
+                    freed[k % 2].record(main)
+                    if k + 1 < nck:
+                        n_next = stage(k + 1)   # the pinned staging buffer of chunk k+1 was last read by the copy of chunk k-1: done (build synchronised)
+                torch.cuda.synchronize()
+
+            decode_e2e()
+            t0 = time.perf_counter(); decode_e2e(); dt_e2e = time.perf_counter() - t0
+            e2e_decode = {"ms_total": 1e3 * dt_e2e, "points_per_s": len(allx) / dt_e2e, "h2d_bytes": int(allx.nbytes), "d2h_bytes": int(8 * len(allx)),
+                          "what": "the same decode with the point set in host memory: per chunk a host copy into a pinned staging buffer, H2D on a copy "
+                                  "stream overlapped with the previous chunk's build + forward, D2H of Phi / I; host wall clock, one gs_preprocess inside"}
+            del xb, pb, ib, hx_pin, hphi, hI
         xs = [dev(allx[a:a + chunk]) for a in range(0, len(allx), chunk)]
         qs = [api.points_query(x) for x in xs]
         pp = [torch.empty(len(x), device="cuda") for x in xs]
@@ -507,7 +608,8 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         e0.record(); decode(); decode(); e1.record(); barrier()
         sm, sc, _ = ctx.profile_read(); ctx.profile_enable(False)
         ms_all = e0.elapsed_time(e1) / 2
-        out["decode"] = {"what": f"forward-only decode of the {len(allx)}-point draw in {len(qs)} chunks of <= 2^24 points: one gs_preprocess "
+        out["decode"] = {"end_to_end": e2e_decode,
+                         "what": f"forward-only decode of ALL {len(allx)} points of the set in {len(qs)} chunks of <= 2^24 points (device-resident): one gs_preprocess "
                                  "(inside the timed region), then gs_build_accel (query sort + cull lists; the first chunk also builds the LBVH over "
                                  "the Gaussians, the others reuse it) + gs_sample_fwd per chunk",
                          "chunks": len(qs), "ms_total": ms_all, "points_per_s": len(allx) / (ms_all * 1e-3),
@@ -608,7 +710,30 @@ def measure(wl, args, sampler, world, rank, headline: bool):
         out["roofline"]["peak_measured"] = {"ffma_tinstr_s": ffma_peak / 1e12, "ffma2_tlaneop_s": ffma2_peak / 1e12,
                                             "mufu_ex2_tinstr_s": ex2_peak / 1e12,
                                             "how": "gs_measure_alu_peaks: register-only FMA / packed FMA / EX2 loops, CUDA events, this run"}
-        out["roofline"]["frac_of_measured"] = out["roofline"]["achieved"] / (ffma_peak / 1e12) if ffma_peak else None
+        # re-state the ALU side of every kernel against the FFMA rate measured in this run (the nominal figure stays beside it)
+        if ffma_peak:
+            scale = ALU_PEAK_TINSTR / (ffma_peak / 1e12)
+            rf = out["roofline"]
+            for kk in rf["kernels"].values():
+                if kk["alu_ms"] is None:
+                    continue
+                kk["alu_ms"] *= scale
+                kk["frac_alu"] = kk["alu_ms"] / kk["launch_ms"] if kk["launch_ms"] else None
+                kk["issue_frac"] = kk["issue_frac"] * scale if kk["issue_frac"] is not None else None
+                kk["bound"] = "alu" if kk["alu_ms"] >= kk["hbm_ms"] else "hbm"
+                kk["frac"] = max(kk["alu_ms"], kk["hbm_ms"]) / kk["launch_ms"] if kk["launch_ms"] else None
+            kd_ = rf["kernels"]["fwd" if rf["kernel"].endswith("fwd") else "bwd"]   # the slower of the two sampling kernels
+            rf.update(bound=kd_["bound"], frac=kd_["frac"], peak=(ffma_peak / 1e12) if kd_["bound"] == "alu" else rf["hbm_peak_gbs"],
+                      achieved=kd_["achieved"] if kd_["bound"] == "alu" else kd_["achieved_gbs"],
+                      unit="T FP32 lane-instr/s (algorithmic: hit pairs x 19 fwd / x 40 bwd)" if kd_["bound"] == "alu" else "GB/s",
+                      peak_source="FFMA lane-instr/s measured in this run (gs_measure_alu_peaks2); nominal 37.2 T beside it")
+            f_, b_ = rf["kernels"]["fwd"], rf["kernels"]["bwd"]
+            both = max(f_["alu_ms"] + b_["alu_ms"], f_["hbm_ms"] + b_["hbm_ms"])
+            fbm = f_["launch_ms"] + b_["launch_ms"]
+            cm = rf["kernels"].get("cull", {}).get("launch_ms", 0.0) or 0.0
+            rf["fwd_bwd_frac"] = both / fbm if fbm else None
+            rf["sampling_frac"] = both / (fbm + cm) if fbm else None
+            rf["step_frac"] = both / out["ms_per_step"]
     ctx.close()
     del gd, phi, I, grads
     torch.cuda.empty_cache()
@@ -657,7 +782,7 @@ def run_ours(args):
     for nm in names:
         wl = make_workload(nm)
         results[nm] = measure(wl, args, sampler, world, rank, headline=(nm == head))
-        if nm == head and rank == 0 and not args.no_cpu and world == 1:
+        if rank == 0 and not args.no_cpu and world == 1:   # the oracle beside EVERY workload, on a bounded sample of each
             from oracle import wveg_oracle as oracle
             oracle.build()
             xyz, target, note = oracle_sample(wl)

@@ -552,8 +552,8 @@ static gs_status run_fwd(gs_ctx *ctx, const FwdOut &o) {
         CullLists lists = cull_lists(ctx);
         const bool sets = o.set_count || o.set_sum || o.set_xor || o.counters;
         if (ctx->opt_bwd_hit_masks && !sets && ctx->P > 0) {
-            CK(ctx->cull_mask.reserve(((size_t)ctx->cull_cap + 1) * 4), "alloc hit masks");
-            lists.mask = ctx->cull_mask.as<uint32_t>();
+            CK(ctx->cull_mask.reserve(((size_t)ctx->cull_cap + 1) * 8), "alloc hit masks");
+            lists.mask = ctx->cull_mask.as<uint2>();
         }
         Stage stage(ctx, GS_PROF_FWD);
         CK(launch_points_fwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
@@ -677,7 +677,7 @@ gs_status gs_sample_bwd(gs_ctx *ctx, const gs_query *q, const float *phi, const 
         Stage stage(ctx, GS_PROF_BWD);
         CullLists lists = cull_lists(ctx);
         const bool masked = ctx->have_hit_masks && ctx->opt_bwd_hit_masks;   // a forward on these lists left its hit bits
-        if (masked) lists.mask = ctx->cull_mask.as<uint32_t>();
+        if (masked) lists.mask = ctx->cull_mask.as<uint2>();
         CK(launch_points_bwd(ctx->sorted_rec.as<float4>(), ctx->sc_spt.as<float4>(),
                              ctx->have_pt_order ? ctx->pt_val[ctx->pt_sel].as<uint32_t>() : nullptr, ctx->P, lists, ctx->tau,
                              ctx->r2, in, ctx->gacc.as<float>(), masked, s), "points backward");

@@ -159,7 +159,7 @@ struct gs_ctx {
     gs::DevBuf bvh_nodes;  // packed traversal nodes
     gs::DevBuf sorted_rec; // float4 [N][4]: records in leaf order (id in plane c's .w)
     gs::DevBuf cull_ids, cull_link, cull_head;  // per-packet survivor lists (see CullLists)
-    gs::DevBuf cull_mask;      // uint32 [cull_cap]: per-chunk hit bits of the last forward on the current lists
+    gs::DevBuf cull_mask;      // uint2 [cull_cap]: per-chunk hit bits (+ skip link) of the last forward on the current lists
     bool have_hit_masks = false;   // cull_mask is valid for the current point accel (a gather-mode forward ran since its build)
     int opt_bwd_hit_masks = 1;     // gs_set_option(GS_OPT_BWD_HIT_MASKS)
     uint32_t cull_cap = 0;   // chunks the pool holds
@@ -313,8 +313,10 @@ struct CullLists {
     uint2 *head;      // [packets] (first chunk, entries in it)
     uint32_t *top;    // chunks requested so far (may exceed cap: the host then grows the pool and repeats)
     uint32_t cap;
-    uint32_t *mask;   // [cap] nullable: bit j of mask[c] = entry j of chunk c hits at least one point of its packet.  Written by
-                      // k_points_fwd (which evaluates every (entry, point) predicate anyway), read by k_points_bwd_masked
+    uint2 *mask;      // [cap] nullable: .x bit j = entry j of chunk c hits at least one point of its packet; .y = the chunk TWO links
+                      // further down the chain (what link[link[c]] would give, 0xffffffff = none), so that a reader can have the loads
+                      // of two chunks in flight instead of chasing one link at a time.  Written by k_points_fwd (which evaluates every
+                      // (entry, point) predicate and walks the chain anyway), read by k_points_bwd_masked
 };
 cudaError_t launch_points_cull(const float4 *sorted_rec, uint32_t N, const float4 *nodes, const float4 *xyz /*sorted copy*/, const uint32_t *pt_order,
                                uint64_t P, const gs_domain &dom, float rcut, const CullLists &lists, uint32_t *overflow, int group /*2 or 4 packets per warp*/,

@@ -90,22 +90,32 @@ __global__ void __launch_bounds__(256) k_refit(const uint32_t *__restrict__ ids,
     const int leaf = blockIdx.x * blockDim.x + threadIdx.x;
     if (leaf >= n) return;
     int node = leaf_parent[leaf];
+    // the thread carries the box of the subtree it has finished in registers: at a node only the SIBLING's box is loaded
+    float mine[6];
+    load_box(aabb + 6 * (size_t)ids[leaf], mine);
+    int from = ~leaf;   // the child link under which the parent knows this subtree
     while (node >= 0) {
         if (atomicAdd(&flags[node], 1u) == 0u) return;  // first arrival: the sibling subtree is not done yet
         __threadfence();
-        float a[6], b[6];
         const int l = left[node], r = right[node];
-        load_box(l < 0 ? aabb + 6 * (size_t)ids[~l] : node_aabb + 6 * (size_t)l, a);
-        load_box(r < 0 ? aabb + 6 * (size_t)ids[~r] : node_aabb + 6 * (size_t)r, b);
+        const bool am_left = l == from;
+        const int sib = am_left ? r : l;
+        float other[6], a[6], b[6];
+        load_box(sib < 0 ? aabb + 6 * (size_t)ids[~sib] : node_aabb + 6 * (size_t)sib, other);
+#pragma unroll
+        for (int k = 0; k < 6; k++) { a[k] = am_left ? mine[k] : other[k]; b[k] = am_left ? other[k] : mine[k]; }
+#pragma unroll
+        for (int k = 0; k < 3; k++) { mine[k] = fminf(a[k], b[k]); mine[3 + k] = fmaxf(a[3 + k], b[3 + k]); }
         float2 *out = reinterpret_cast<float2 *>(node_aabb + 6 * (size_t)node);
-        __stcg(out, make_float2(fminf(a[0], b[0]), fminf(a[1], b[1])));
-        __stcg(out + 1, make_float2(fminf(a[2], b[2]), fmaxf(a[3], b[3])));
-        __stcg(out + 2, make_float2(fmaxf(a[4], b[4]), fmaxf(a[5], b[5])));
+        __stcg(out, make_float2(mine[0], mine[1]));
+        __stcg(out + 1, make_float2(mine[2], mine[3]));
+        __stcg(out + 2, make_float2(mine[4], mine[5]));
         packed[4 * (size_t)node + 0] = make_float4(a[0], a[1], a[2], a[3]);
         packed[4 * (size_t)node + 1] = make_float4(a[4], a[5], b[0], b[1]);
         packed[4 * (size_t)node + 2] = make_float4(b[2], b[3], b[4], b[5]);
         packed[4 * (size_t)node + 3] = make_float4(__int_as_float(l), __int_as_float(r), 0.f, 0.f);
         __threadfence();
+        from = node;
         node = parent[node];
     }
 }

@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_fwd(const float4 *__
         __syncwarp();
         if (MASKS) {   // the backward drops the entries that hit nothing (44 % of configs[4]'s, 33 % of configs[2]'s) before it gathers their records
             emask = __reduce_or_sync(0xffffffffu, emask);
-            if (lane == 0) L.mask[c0] = emask;
+            if (lane == 0) L.mask[c0] = make_uint2(emask, c2);   // c2: the chunk two links on, already in a register here
         }
         c0 = c1; n0 = 32; c1 = c2; pos1 = pos2; c2 = c3; b ^= 1;
     }
@@ -626,7 +626,10 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd(const float4 *__
 // the packet, whatever chunk it came from, and the records of the others are never read.  One batch's gather is in flight
 // while the previous batch is evaluated.  Per entry the arithmetic and its order are those of k_points_bwd.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd_masked(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
+#ifndef GS_BWDM_MINB
+#define GS_BWDM_MINB 4   // measured: 5 resident CTAs (96 registers, a few spills) is slower (configs[4] 3.34 vs 3.18 ms)
+#endif
+__global__ void __launch_bounds__(EVAL_WARPS * 32, GS_BWDM_MINB) k_points_bwd_masked(const float4 *__restrict__ srt, const float4 *__restrict__ xyz /*sorted copy*/,
                                                                         const uint32_t *__restrict__ pt_order, uint64_t P, CullLists L, float tau,
                                                                         float r2, BwdIn in, float *__restrict__ gacc) {
     __shared__ __align__(16) float pts_all[EVAL_WARPS][16][12];   // as in k_points_bwd
@@ -663,23 +666,32 @@ __global__ void __launch_bounds__(EVAL_WARPS * 32) k_points_bwd_masked(const flo
         row[0] = x; row[2] = y; row[4] = z; row[6] = alpha; row[8] = beta; row[10] = eps;
         __syncwarp();
     }
+    // The chain is read two chunks ahead: A is the chunk being appended, B the next one (its loads in flight), and as soon as A's
+    // mask word is here its skip link names the chunk after B, whose loads are issued before A is used.
     const uint2 head = __ldg(L.head + packet);
-    uint32_t c = head.x, id = 0u, m = 0u, nxt = NO_CHUNK;
-    if (c != NO_CHUNK) {   // the head chunk holds head.y entries, every linked chunk 32
+    uint32_t cA = head.x, cB = NO_CHUNK, idA = 0u, idB = 0u;
+    uint2 wA = make_uint2(0u, NO_CHUNK), wB = make_uint2(0u, NO_CHUNK);
+    if (cA != NO_CHUNK) {   // the head chunk holds head.y entries, every linked chunk 32
         const int n = (int)head.y;
-        id = lane < n ? __ldg(L.ids + (size_t)c * 32 + lane) : 0u;
-        m = __ldg(L.mask + c) & (n < 32 ? (1u << n) - 1u : 0xffffffffu);
-        nxt = __ldg(L.link + c);
+        idA = lane < n ? __ldg(L.ids + (size_t)cA * 32 + lane) : 0u;
+        wA = __ldg(L.mask + cA);
+        if (n < 32) wA.x &= (1u << n) - 1u;
+        cB = __ldg(L.link + cA);
+        if (cB != NO_CHUNK) { idB = __ldg(L.ids + (size_t)cB * 32 + lane); wB = __ldg(L.mask + cB); }
     }
     uint32_t cnt = 0, done = 0;   // ids appended to the ring / ids handed to a gather so far
     int pend = 0, slot = 0;        // entries of the batch whose records are on their way into buf[slot]
     while (true) {
-        while (c != NO_CHUNK && cnt - done < 32u) {
-            uint32_t id2 = 0u, m2 = 0u, nxt2 = NO_CHUNK;
-            if (nxt != NO_CHUNK) { id2 = __ldg(L.ids + (size_t)nxt * 32 + lane); m2 = __ldg(L.mask + nxt); nxt2 = __ldg(L.link + nxt); }
-            if ((m >> lane) & 1u) ring[(cnt + __popc(m & ((1u << lane) - 1u))) & 63u] = id;
+        while (cA != NO_CHUNK && cnt - done < 32u) {
+            const uint32_t cC = cB != NO_CHUNK ? wA.y : NO_CHUNK;
+            uint32_t idC = 0u;
+            uint2 wC = make_uint2(0u, NO_CHUNK);
+            if (cC != NO_CHUNK) { idC = __ldg(L.ids + (size_t)cC * 32 + lane); wC = __ldg(L.mask + cC); }
+            const uint32_t m = wA.x;
+            if ((m >> lane) & 1u) ring[(cnt + __popc(m & ((1u << lane) - 1u))) & 63u] = idA;
             cnt += __popc(m);
-            c = nxt; id = id2; m = m2; nxt = nxt2;
+            cA = cB; idA = idB; wA = wB;
+            cB = cC; idB = idC; wB = wC;
         }
         __syncwarp();
         const int nb = (int)(cnt - done < 32u ? cnt - done : 32u);

@@ -286,30 +286,48 @@ def c4_target(grid: Grid, field: FourierField) -> np.ndarray:
 # C5: large unstructured, shell and fragments
 # ----------------------------------------------------------------------------------------
 def c5_points(seed: int = 5, p: int = 200_000_000, clusters: int = 4096, shell_frac: float = 0.7,
-              chunk: int = 1 << 22):
+              chunk: int = 1 << 21, workers: int | None = None):
     """configs[4]: 70 % of points in a spherical shell (radius 0.35, thickness 0.05, centre 0.5),
     30 % in ``clusters`` small fragments (sigma 0.004); scalar = radial profile + high-frequency
-    noise.  Generated in chunks; returns (xyz f32 [P,3], t f32 [P])."""
+    noise.  Returns (xyz f32 [P,3], t f32 [P]).
+
+    The full set is 200 M points (3.2 GB with the scalars): it is generated in chunks of 2^21 points, each from a random
+    stream of its own (seed, chunk index), so that the chunks can be drawn by a pool of threads and the first k points
+    are the same for every p >= k."""
+    import concurrent.futures
+    import os
     rng = np.random.Generator(np.random.PCG64(seed))
     centres = rng.uniform(0.05, 0.95, (clusters, 3))
     kf = rng.uniform(40.0, 120.0, (4, 3)) * np.sign(rng.standard_normal((4, 3)))
     xyz = np.empty((p, 3), F32)
     t = np.empty(p, F32)
-    for a in range(0, p, chunk):
-        m = min(chunk, p - a)
-        is_shell = rng.uniform(0.0, 1.0, m) < shell_frac
-        d = rng.standard_normal((m, 3))
+
+    def draw(a: int):
+        n_keep = min(chunk, p - a)
+        m = chunk   # a whole chunk is always drawn (and the tail dropped), so that a shorter set is a prefix of a longer one
+        r_ = np.random.Generator(np.random.PCG64([seed, 1 + a // chunk]))
+        is_shell = r_.uniform(0.0, 1.0, m) < shell_frac
+        d = r_.standard_normal((m, 3))
         d /= np.linalg.norm(d, axis=1, keepdims=True)
-        rad = 0.35 + 0.05 * (rng.uniform(0.0, 1.0, m) - 0.5)
+        rad = 0.35 + 0.05 * (r_.uniform(0.0, 1.0, m) - 0.5)
         pts_shell = 0.5 + d * rad[:, None]
-        k = rng.integers(0, clusters, m)
-        pts_frag = centres[k] + 0.004 * rng.standard_normal((m, 3))
+        k = r_.integers(0, clusters, m)
+        pts_frag = centres[k] + 0.004 * r_.standard_normal((m, 3))
         pts = np.where(is_shell[:, None], pts_shell, pts_frag)
         pts = np.clip(pts, 0.0, np.nextafter(1.0, 0.0))
         r = np.linalg.norm(pts - 0.5, axis=1)
         val = 0.5 + 0.35 * np.cos(9.0 * r) + 0.0375 * np.sum(np.sin(pts @ kf.T), axis=1)
-        xyz[a:a + m] = pts.astype(F32)
-        t[a:a + m] = np.clip(val, 0.0, 1.0).astype(F32)
+        xyz[a:a + n_keep] = pts[:n_keep].astype(F32)
+        t[a:a + n_keep] = np.clip(val[:n_keep], 0.0, 1.0).astype(F32)
+
+    starts = list(range(0, p, chunk))
+    nw = workers if workers else min(len(starts), os.cpu_count() or 1, 32)
+    if nw <= 1:
+        for a in starts:
+            draw(a)
+    else:
+        with concurrent.futures.ThreadPoolExecutor(max_workers=nw) as ex:
+            list(ex.map(draw, starts))
     return xyz, t
 
 

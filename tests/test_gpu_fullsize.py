@@ -190,17 +190,27 @@ def test_c4_full_batch(oracle):
     ctx.close()
 
 
+_C5 = {}
+
+
+def _c5_pool():
+    """configs[4] as BASELINE.json states it: the 200,000,000-point set (2.4 GB of positions, drawn once per test session by
+    a pool of threads) and the 8,388,608 Gaussians centred on points of THAT set."""
+    if not _C5:
+        xyz_all, t_all = inputs.c5_points(seed=5)
+        assert len(xyz_all) == 200_000_000
+        _C5.update(xyz=xyz_all, t=t_all, g=inputs.c5_gaussians(xyz_all, t_all), dom=inputs.points_domain(xyz_all))
+    return _C5["xyz"], _C5["t"], _C5["g"], _C5["dom"]
+
+
 def test_c5_full_batch(oracle):
     # BASELINE.json configs[4] at its stated size: 8,388,608 Gaussians (sigma 0.0005-0.002) centred on points of the
-    # shell-and-fragments distribution; one batch of 2^24 random points of a 40 M-point draw (the full 200 M-point set is
-    # only ever seen in such batches); LBVH, query sort and cull lists rebuilt by gs_build_accel
-    xyz_all, t_all = inputs.c5_points(seed=5, p=40_000_000)
-    g = inputs.c5_gaussians(xyz_all, t_all)
+    # shell-and-fragments distribution; one batch of 2^24 random points of the 200 M-point set, forward + backward; LBVH,
+    # query sort and cull lists rebuilt by gs_build_accel
+    xyz_all, t_all, g, dom = _c5_pool()
     assert g.n == 8_388_608
     idx = inputs.batch_indices(5, 0, len(xyz_all), 1 << 24)
     xyz, target = np.ascontiguousarray(xyz_all[idx]), np.ascontiguousarray(t_all[idx])
-    dom = inputs.points_domain(xyz_all)
-    del xyz_all, t_all
     fwd = oracle.forward(g, xyz, TAU, mode=1)
     loss, a, serr = oracle.mse(fwd["phi"], fwd["I"], target, TAU)
     gr = oracle.backward(g, xyz, fwd["phi"], fwd["I"], a, None, target, TAU, mode=1)
@@ -225,3 +235,37 @@ def test_c5_full_batch(oracle):
     assert got["dscalar"].sum() == pytest.approx(a[covered].sum(), rel=1e-4, abs=1e-7)
     assert got["err"].sum() == pytest.approx(serr[covered].sum(), rel=1e-4)
     print("C5 full batch: hits", hits, "tested", tested, "phi err", e_phi, "grad errs", errs)
+
+
+def test_c5_decode_first_and_last_chunk(oracle):
+    # configs[4]'s "full forward decode of all points": the 200 M points go through the sampler in 12 chunks of <= 2^24 in
+    # set order, after ONE gs_preprocess -- the first gs_build_accel builds the LBVH over the Gaussians, the later ones reuse it
+    # and only sort and cull their own points.  The first and the last chunk (ragged: 15,450,624 points) are compared with the
+    # oracle, every intersection set and every value; bench.py times all twelve.
+    import torch
+    from paper_2607_01164_b200 import api
+    xyz_all, t_all, g, dom = _c5_pool()
+    chunk = 1 << 24
+    starts = list(range(0, len(xyz_all), chunk))
+    assert len(starts) == 12 and len(xyz_all) - starts[-1] == 15_450_624
+    ctx = api.Context()
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (g.mean, g.scale, g.quat, g.opacity, g.scalar)]
+    ctx.gs_preprocess(*dev, domain=dom, tau=TAU)
+    for a in (starts[0], starts[-1]):
+        xyz = np.ascontiguousarray(xyz_all[a:a + chunk])
+        P = len(xyz)
+        fwd = oracle.forward(g, xyz, TAU, mode=1)
+        x = torch.from_numpy(xyz).cuda()
+        q = api.points_query(x)
+        ctx.gs_build_accel(q)
+        phi, I = torch.full((P,), -7.0, device="cuda"), torch.full((P,), -7.0, device="cuda")
+        ctx.gs_sample_fwd(q, phi, I)
+        torch.cuda.synchronize()
+        run = _Shim(ctx, q, P, phi, I, None)
+        tested, hits = check_sets(run, fwd)
+        assert hits > 10 * P
+        near, e_phi, e_I = check_forward(run, fwd)
+        assert near <= 64
+        print("C5 decode chunk at", a, "P", P, "hits", hits, "tested", tested, "phi err", e_phi, "I err", e_I)
+        del x, phi, I
+    ctx.close()
